@@ -1,0 +1,146 @@
+"""CPU ORACLE loader -- TEST INFRASTRUCTURE, NOT THE PRODUCT.
+
+Only ``tests/``, ``__graft_entry__.smoke()`` and ``bench.py``'s ``cpu_baseline`` /
+``--impl reference`` legs may import this package.  It builds (g++) and loads
+``oracle/cube_oracle.cpp`` through ctypes.  It shares nothing with, and never imports,
+``paper_1211_4896_b200`` (the CUDA path); the CUDA path never imports this.
+
+Every function is a thin marshalling wrapper over one ``extern "C"`` function of
+cube_oracle.cpp; the passages each follows are cited there.
+"""
+import ctypes
+import os
+import subprocess
+
+import numpy as np
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+_SRC = os.path.join(_HERE, "cube_oracle.cpp")
+_LIB = os.path.join(_HERE, "libcube_oracle.so")
+_FLAGS = ["-O2", "-std=c++17", "-ffp-contract=off", "-fno-fast-math", "-fPIC", "-shared"]
+
+
+def build(force=False):
+    """Compile cube_oracle.cpp -> libcube_oracle.so (no-op when up to date)."""
+    if (not force and os.path.exists(_LIB)
+            and os.path.getmtime(_LIB) >= os.path.getmtime(_SRC)):
+        return _LIB
+    tmp = _LIB + ".tmp.%d" % os.getpid()
+    subprocess.check_call(["g++"] + _FLAGS + ["-o", tmp, _SRC])
+    os.replace(tmp, _LIB)
+    return _LIB
+
+
+class Moments(ctypes.Structure):
+    _fields_ = [("count", ctypes.c_uint64), ("nan_count", ctypes.c_uint64),
+                ("min", ctypes.c_float), ("max", ctypes.c_float),
+                ("mean", ctypes.c_double), ("std", ctypes.c_double)]
+
+
+_lib = None
+
+
+def lib():
+    global _lib
+    if _lib is None:
+        L = ctypes.CDLL(build())
+        fp = ctypes.POINTER(ctypes.c_float)
+        u64p = ctypes.POINTER(ctypes.c_uint64)
+        L.oracle_moments.argtypes = [fp, ctypes.c_uint64, ctypes.c_int, ctypes.POINTER(Moments)]
+        L.oracle_bin_index.argtypes = [ctypes.c_float, ctypes.c_int, ctypes.c_float, ctypes.c_float]
+        L.oracle_bin_index.restype = ctypes.c_int
+        L.oracle_histogram.argtypes = [fp, ctypes.c_uint64, ctypes.c_int, ctypes.c_float,
+                                       ctypes.c_float, u64p, u64p]
+        L.oracle_kth.argtypes = [fp, ctypes.c_uint64, ctypes.c_uint64, fp]
+        L.oracle_median.argtypes = [fp, ctypes.c_uint64, fp]
+        L.oracle_rank_counts.argtypes = [fp, ctypes.c_uint64, ctypes.c_float, u64p, u64p]
+        L.oracle_torben_guess.argtypes = [ctypes.c_float, ctypes.c_float]
+        L.oracle_torben_guess.restype = ctypes.c_float
+        L.oracle_torben_stop.argtypes = [ctypes.c_uint64] * 3
+        L.oracle_torben_pick.argtypes = [ctypes.c_uint64] * 3 + [ctypes.c_float] * 3
+        L.oracle_torben_pick.restype = ctypes.c_float
+        L.oracle_torben_median.argtypes = [fp, ctypes.c_uint64, fp,
+                                           ctypes.POINTER(ctypes.c_double), ctypes.c_int]
+        _lib = L
+    return _lib
+
+
+def _arr(a):
+    a = np.ascontiguousarray(a, dtype=np.float32).reshape(-1)
+    return a, a.ctypes.data_as(ctypes.POINTER(ctypes.c_float))
+
+
+def moments(a, sample_std=False):
+    """-> dict(count, nan_count, min, max, mean, std).  PAPER.md:265, 273."""
+    a, p = _arr(a)
+    m = Moments()
+    lib().oracle_moments(p, a.size, int(bool(sample_std)), ctypes.byref(m))
+    return dict(count=m.count, nan_count=m.nan_count, min=np.float32(m.min),
+                max=np.float32(m.max), mean=m.mean, std=m.std)
+
+
+def bin_index(x, nbins, lo, hi):
+    return lib().oracle_bin_index(float(np.float32(x)), int(nbins),
+                                  float(np.float32(lo)), float(np.float32(hi)))
+
+
+def histogram(a, nbins, lo, hi):
+    """-> (bins[nbins] uint64, outside[2] uint64).  PAPER.md:259-261."""
+    a, p = _arr(a)
+    bins = np.zeros(nbins, dtype=np.uint64)
+    outside = np.zeros(2, dtype=np.uint64)
+    u64p = ctypes.POINTER(ctypes.c_uint64)
+    rc = lib().oracle_histogram(p, a.size, int(nbins), float(np.float32(lo)), float(np.float32(hi)),
+                                bins.ctypes.data_as(u64p), outside.ctypes.data_as(u64p))
+    if rc != 0:
+        raise ValueError("oracle_histogram: invalid arguments")
+    return bins, outside
+
+
+def kth(a, k):
+    """k-th (0-based) smallest non-NaN value in total order.  PAPER.md:281."""
+    a, p = _arr(a)
+    out = ctypes.c_float()
+    rc = lib().oracle_kth(p, a.size, int(k), ctypes.byref(out))
+    if rc != 0:
+        raise IndexError("k >= non-NaN count")
+    return np.float32(out.value)
+
+
+def median(a):
+    """Lower median, k=(n-1)/2; NaN if there is no non-NaN voxel."""
+    a, p = _arr(a)
+    out = ctypes.c_float()
+    lib().oracle_median(p, a.size, ctypes.byref(out))
+    return np.float32(out.value)
+
+
+def rank_counts(a, m):
+    """-> (#{x<m}, #{x==m}) in total order over the non-NaN voxels."""
+    a, p = _arr(a)
+    less, equal = ctypes.c_uint64(), ctypes.c_uint64()
+    lib().oracle_rank_counts(p, a.size, float(np.float32(m)), ctypes.byref(less), ctypes.byref(equal))
+    return less.value, equal.value
+
+
+def torben_guess(mn, mx):
+    return np.float32(lib().oracle_torben_guess(float(np.float32(mn)), float(np.float32(mx))))
+
+
+def torben_stop(less, greater, n):
+    return bool(lib().oracle_torben_stop(int(less), int(greater), int(n)))
+
+
+def torben_pick(less, equal, n, maxlt, guess, mingt):
+    return np.float32(lib().oracle_torben_pick(int(less), int(equal), int(n), float(np.float32(maxlt)),
+                                               float(np.float32(guess)), float(np.float32(mingt))))
+
+
+def torben_median(a, max_trace=64):
+    """Alg. 1.  -> (median, iterations, trace[iterations,6])."""
+    a, p = _arr(a)
+    out = ctypes.c_float()
+    trace = np.zeros((max_trace, 6), dtype=np.float64)
+    it = lib().oracle_torben_median(p, a.size, ctypes.byref(out),
+                                    trace.ctypes.data_as(ctypes.POINTER(ctypes.c_double)), max_trace)
+    return np.float32(out.value), it, trace[:max(0, min(it, max_trace))]

@@ -1,0 +1,262 @@
+// cube_oracle.cpp -- CPU ORACLE for the global-statistics path of arXiv:1211.4896.
+//
+// THIS IS TEST INFRASTRUCTURE, NOT THE PRODUCT.  Only tests/, __graft_entry__.smoke()
+// and bench.py's cpu_baseline / --impl reference legs may build, load or call it.
+// It shares no code, header, table or helper with the CUDA path under
+// paper_1211_4896_b200/ and neither side includes the other.
+//
+// Plain, single-threaded, obviously-correct C++.  Every result below has a plain
+// definition; the oracle is that definition written out:
+//
+//   count / nan_count   PAPER.md:252, 265  "count of the non-null data values"; NULL == IEEE NaN
+//   min / max           PAPER.md:261, 518  data minimum / maximum (total order: -0.0 < +0.0)
+//   mean / std          PAPER.md:265, 273  from "summation and summation of squares and count";
+//                       evaluated here as the exact-arithmetic value (long double, compensated,
+//                       two-pass corrected) rounded to double -- NOT the paper's float32-per-slice
+//                       partial sums, reading R17
+//   histogram           PAPER.md:259-261   b = floor((x-lo) * (nbins/(hi-lo))) in float32,
+//                       closed top bin, values outside [lo,hi] counted separately (R10-R13)
+//   k-th / median       PAPER.md:281       "sort and select the middle element" is the definition
+//                       the paper avoids for cost; here std::nth_element on a copy.  Lower
+//                       median k=(n-1)/2 (R5), which is what Alg. 1 returns.
+//   Torben (Alg. 1)     PAPER.md:570-610   restated step by step as a second, independent CPU
+//                       algorithm for the median, with the garbled lines restored (R1-R4);
+//                       Table 1 pins the restoration.
+//   rank certificate    necessary-and-sufficient check of a claimed k-th value in one pass:
+//                       #{x<m} <= k < #{x<m} + #{x==m}  (total order), independent of both
+//                       selection algorithms.
+//
+// Parity pins (tests/test_oracle_*.py): closed forms (constant cube, ramp 0..N-1, two-value
+// cube), exact rational sums computed with Python big integers, brute-force full sort on
+// tiny cubes, power-of-two ramp histograms, Table 1 of the paper.  The only unpinned
+// behaviour is +-Inf voxels in mean/std (R8): "parity unpinned" for that case.
+//
+// Build: g++ -O2 -std=c++17 -ffp-contract=off -fno-fast-math -fPIC -shared (oracle/build.py).
+
+#include <algorithm>
+#include <cmath>
+#include <cstdint>
+#include <cstring>
+#include <limits>
+#include <vector>
+
+namespace {
+
+inline bool is_nan(float x) { return x != x; }
+
+// IEEE totalOrder restricted to non-NaN values: -0.0 < +0.0 (reading R7).
+inline bool total_less(float a, float b) {
+    if (a < b) return true;
+    if (a == b) return std::signbit(a) && !std::signbit(b);
+    return false;
+}
+inline bool total_equal(float a, float b) {
+    return a == b && std::signbit(a) == std::signbit(b);
+}
+
+// Neumaier-compensated accumulator in long double.
+struct Comp {
+    long double s = 0.0L, c = 0.0L;
+    inline void add(long double v) {
+        long double t = s + v;
+        if (fabsl(s) >= fabsl(v)) c += (s - t) + v; else c += (v - t) + s;
+        s = t;
+    }
+    inline long double value() const { return s + c; }
+};
+
+}  // namespace
+
+extern "C" {
+
+struct oracle_moments_t {
+    uint64_t count;      // non-NaN voxels
+    uint64_t nan_count;  // NaN voxels
+    float min, max;      // NaN if count == 0
+    double mean, std;    // NaN if count == 0
+};
+
+// PAPER.md:265, 273.  sample_std != 0 -> divide M2 by (n-1) (n==1 -> NaN, reading R15).
+int oracle_moments(const float* d, uint64_t N, int sample_std, oracle_moments_t* out) {
+    uint64_t n = 0;
+    float mn = 0.f, mx = 0.f;
+    Comp sum;
+    for (uint64_t i = 0; i < N; ++i) {
+        float x = d[i];
+        if (is_nan(x)) continue;
+        if (n == 0) { mn = x; mx = x; }
+        else {
+            if (total_less(x, mn)) mn = x;
+            if (total_less(mx, x)) mx = x;
+        }
+        ++n;
+        sum.add((long double)x);
+    }
+    out->count = n;
+    out->nan_count = N - n;
+    if (n == 0) {
+        out->min = out->max = std::numeric_limits<float>::quiet_NaN();
+        out->mean = out->std = std::numeric_limits<double>::quiet_NaN();
+        return 0;
+    }
+    long double mean = sum.value() / (long double)n;
+    // second pass: corrected two-pass M2 = sum(delta^2) - (sum delta)^2 / n
+    Comp sd, sd2;
+    for (uint64_t i = 0; i < N; ++i) {
+        float x = d[i];
+        if (is_nan(x)) continue;
+        long double delta = (long double)x - mean;
+        sd.add(delta);
+        sd2.add(delta * delta);
+    }
+    long double m2 = sd2.value() - sd.value() * sd.value() / (long double)n;
+    if (m2 < 0.0L) m2 = 0.0L;
+    out->min = mn;
+    out->max = mx;
+    out->mean = (double)(mean + sd.value() / (long double)n);
+    long double denom = sample_std ? (long double)n - 1.0L : (long double)n;
+    out->std = (denom > 0.0L) ? (double)sqrtl(m2 / denom)
+                              : std::numeric_limits<double>::quiet_NaN();
+    return 0;
+}
+
+// Float32 bin index of one in-range value (readings R10, R11, R13).  `scale` is
+// (float)nbins / (hi - lo), both operations rounded to float32.  Exposed so tests can
+// pin the formula on single values.
+int oracle_bin_index(float x, int nbins, float lo, float hi) {
+    if (hi == lo) return 0;
+    float width = hi - lo;
+    float scale = (float)nbins / width;
+    float t = x - lo;
+    float v = t * scale;
+    if (!(v < (float)nbins)) return nbins - 1;  // closed top bin
+    int b = (int)floorf(v);
+    if (b > nbins - 1) b = nbins - 1;
+    if (b < 0) b = 0;
+    return b;
+}
+
+// PAPER.md:259-261.  bins[nbins], outside[2] = {#x<lo, #x>hi}; NaN counted nowhere.
+// Returns 1 on invalid arguments (nbins<1, !(lo<=hi), non-finite lo/hi or scale).
+int oracle_histogram(const float* d, uint64_t N, int nbins, float lo, float hi,
+                     uint64_t* bins, uint64_t* outside) {
+    if (nbins < 1 || !(lo <= hi) || !std::isfinite(lo) || !std::isfinite(hi)) return 1;
+    if (hi != lo && !std::isfinite((float)nbins / (hi - lo))) return 1;
+    for (int b = 0; b < nbins; ++b) bins[b] = 0;
+    outside[0] = outside[1] = 0;
+    for (uint64_t i = 0; i < N; ++i) {
+        float x = d[i];
+        if (is_nan(x)) continue;
+        if (x < lo) { ++outside[0]; continue; }
+        if (x > hi) { ++outside[1]; continue; }
+        ++bins[oracle_bin_index(x, nbins, lo, hi)];
+    }
+    return 0;
+}
+
+// sort-and-select, k 0-based among the non-NaN values in total order.
+// Returns 1 if k >= count (out = NaN).
+int oracle_kth(const float* d, uint64_t N, uint64_t k, float* out) {
+    std::vector<float> v;
+    v.reserve(N);
+    for (uint64_t i = 0; i < N; ++i) if (!is_nan(d[i])) v.push_back(d[i]);
+    if (k >= v.size()) { *out = std::numeric_limits<float>::quiet_NaN(); return 1; }
+    std::nth_element(v.begin(), v.begin() + (std::ptrdiff_t)k, v.end(), total_less);
+    *out = v[k];
+    return 0;
+}
+
+// Lower median: k = (n-1)/2 (reading R5).  Returns 1 if there is no non-NaN voxel.
+int oracle_median(const float* d, uint64_t N, float* out) {
+    std::vector<float> v;
+    v.reserve(N);
+    for (uint64_t i = 0; i < N; ++i) if (!is_nan(d[i])) v.push_back(d[i]);
+    if (v.empty()) { *out = std::numeric_limits<float>::quiet_NaN(); return 1; }
+    uint64_t k = (v.size() - 1) / 2;
+    std::nth_element(v.begin(), v.begin() + (std::ptrdiff_t)k, v.end(), total_less);
+    *out = v[k];
+    return 0;
+}
+
+// One streaming pass: less = #{x < m}, equal = #{x == m} in total order over non-NaN x.
+// m is the k-th value  <=>  equal >= 1 and less <= k < less + equal.
+int oracle_rank_counts(const float* d, uint64_t N, float m, uint64_t* less, uint64_t* equal) {
+    uint64_t l = 0, e = 0;
+    for (uint64_t i = 0; i < N; ++i) {
+        float x = d[i];
+        if (is_nan(x)) continue;
+        if (total_less(x, m)) ++l;
+        else if (total_equal(x, m)) ++e;
+    }
+    *less = l; *equal = e;
+    return 0;
+}
+
+// ---------------------------------------------------------------------------------
+// Alg. 1, Torben's median method, restated in the paper's order.
+// ---------------------------------------------------------------------------------
+
+// PAPER.md:575 "Guess = (Min+Max)/" -- denominator lost in extraction; restored as /2
+// evaluated in float32 (reading R1; every Guess printed in Table 1 equals this).
+float oracle_torben_guess(float mn, float mx) { return (mn + mx) / 2.0f; }
+
+// "if LessCount <= (data_length+1)/2 and GreaterCount <= (data_length+1)/2
+// then" -- empty body restored as `break` (R2); integer division (R4).
+int oracle_torben_stop(uint64_t less, uint64_t greater, uint64_t n) {
+    uint64_t half = (n + 1) / 2;
+    return (less <= half && greater <= half) ? 1 : 0;
+}
+
+// final selection.
+float oracle_torben_pick(uint64_t less, uint64_t equal, uint64_t n,
+                         float maxlt, float guess, float mingt) {
+    uint64_t half = (n + 1) / 2;
+    if (less >= half) return maxlt;
+    if (less + equal >= half) return guess;
+    return mingt;
+}
+
+// Full Alg. 1 over the non-NaN voxels.  trace (optional, may be NULL) receives up to
+// max_trace rows of 6 doubles: guess, min, max, less, greater, equal.
+// Returns the number of iterations, or -1 if there is no non-NaN voxel.
+int oracle_torben_median(const float* d, uint64_t N, float* out, double* trace, int max_trace) {
+    uint64_t n = 0;
+    float Min = 0.f, Max = 0.f;
+    for (uint64_t i = 0; i < N; ++i) {
+        float x = d[i];
+        if (is_nan(x)) continue;
+        if (n == 0) { Min = Max = x; }
+        else { if (x < Min) Min = x; if (x > Max) Max = x; }
+        ++n;
+    }
+    if (n == 0) { *out = std::numeric_limits<float>::quiet_NaN(); return -1; }
+    int iter = 0;
+    float Guess, MaxLt, MinGt;
+    uint64_t Less, Greater, Equal;
+    for (;;) {
+        Guess = oracle_torben_guess(Min, Max);
+        Less = Greater = Equal = 0;
+        MaxLt = Min;
+        MinGt = Max;
+        for (uint64_t i = 0; i < N; ++i) {          // i in [0, data_length)  (R3)
+            float x = d[i];
+            if (is_nan(x)) continue;                // NULL voxels excluded
+            if (x < Guess) { ++Less; if (x > MaxLt) MaxLt = x; }
+            else if (x > Guess) { ++Greater; if (x < MinGt) MinGt = x; }
+            else ++Equal;
+        }
+        if (trace && iter < max_trace) {
+            double* r = trace + 6 * iter;
+            r[0] = Guess; r[1] = Min; r[2] = Max;
+            r[3] = (double)Less; r[4] = (double)Greater; r[5] = (double)Equal;
+        }
+        ++iter;
+        if (oracle_torben_stop(Less, Greater, n)) break;
+        else if (Less > Greater) Max = MaxLt;
+        else Min = MinGt;
+    }
+    *out = oracle_torben_pick(Less, Equal, n, MaxLt, Guess, MinGt);
+    return iter;
+}
+
+}  // extern "C"
