@@ -1,0 +1,142 @@
+/* cube.h -- C ABI of libcube: global statistics of a float32 spectral cube on one B200.
+ *
+ * The operations are the "quantitative" tasks of arXiv:1211.4896 (cited as PAPER.md:<line> of
+ * /root/reference/PAPER.md):
+ *   - global mean / standard deviation (+ count of non-null voxels, min, max)   PAPER.md:263-275 (sec. 4.2),
+ *     min/max "calculated while the dataset is loading"
+ *   - global intensity histogram                                                PAPER.md:257-261 (sec. 4.1, Fig. 4)
+ *   - exact global median / k-th value                                          PAPER.md:277-296 (sec. 4.3),
+ *     Alg. 1; here reached by a 11/11/10-bit radix select on
+ *     order-preserving keys instead of ~31 bisection passes
+ *   - NULL (undefined) voxels are excluded from every statistic
+ *     (NULL == IEEE NaN of any sign/payload, reading R6)
+ *
+ * Conventions
+ *   - `d` is a DEVICE pointer to nx*ny*nz float32 voxels, x fastest, then y, then z. It is never
+ *     written (the paper keeps the cube read-only) and stays owned by the caller.
+ *     Any 4-byte alignment is accepted. All results are order independent, so only N = nx*ny*nz matters.
+ *   - Every output pointer (`out`, `bins`, `outside`) may be a device pointer, pinned host memory or
+ *     pageable host memory (detected by the driver through unified addressing). Results are produced
+ *     on the device and copied with cudaMemcpyAsync on `stream`: for device/pinned destinations the
+ *     call returns without synchronising the host; for pageable host memory the copy (and therefore
+ *     the call) completes before returning.
+ *   - All work is enqueued on `stream`; there is no hidden allocation after cube_create().
+ *     A cube_ctx must not be used from two streams/threads at the same time.
+ *   - Counts are 64-bit everywhere (N up to 2^37).
+ *   - Return value: 0 (CUBE_OK) or a CUBE_E* code; never throws, exits or prints.
+ *     Argument errors are detected before any work is enqueued.
+ *   - There is NO CPU fallback: without a CUDA device cube_create() fails with CUBE_ECUDA.
+ */
+#ifndef CUBE_H_
+#define CUBE_H_
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#ifndef __DRIVER_TYPES_H__
+typedef struct CUstream_st* cudaStream_t;
+#endif
+
+typedef struct cube_ctx cube_ctx; /* opaque; owns all device scratch (partials, bins, select state) */
+
+enum {
+    CUBE_OK = 0,
+    CUBE_EINVAL = 1, /* null pointer, dim <= 0, nbins out of range, !(lo <= hi), non-finite lo/hi/scale */
+    CUBE_EEMPTY = 2, /* reserved: not returned by the asynchronous calls (see cube_moments) */
+    CUBE_ECUDA = 3,  /* a CUDA call failed; cube_last_cuda_error() gives the cudaError_t */
+    CUBE_ERANGE = 4, /* reserved */
+    CUBE_ENOMEM = 5  /* host or device allocation failed in cube_create */
+};
+
+/* flags */
+enum {
+    CUBE_SAMPLE_STD = 1u,  /* std = sqrt(M2/(n-1)) instead of the population sqrt(M2/n); n==1 -> NaN */
+    CUBE_COARSE_HIST = 2u, /* cube_moments: also accumulate the first radix-select digit histogram
+                              (2048 bins of key>>21) in the same pass and keep it in the context */
+    CUBE_REUSE_COARSE = 4u /* cube_kth_ex/cube_median_ex: skip select pass 1 and use the digit
+                              histogram left by the last cube_moments(CUBE_COARSE_HIST) call on the
+                              SAME data (the caller vouches for that) */
+};
+
+#define CUBE_MAX_BINS 65536
+
+typedef struct {
+    uint64_t count;     /* voxels that are not NaN */
+    uint64_t nan_count; /* NaN (blanked) voxels; count + nan_count == nx*ny*nz */
+    float min, max;     /* extrema in IEEE total order (-0.0 < +0.0); NaN when count == 0 */
+    double mean, std;   /* NaN when count == 0 */
+} cube_moments_t;
+
+/* Create a context on the CURRENT device. `scratch_bytes_hint` sizes the optional candidate buffer of
+ * the select (0 = default, 64 MiB); everything else is fixed size (< 4 MiB). */
+int cube_create(cube_ctx** out, size_t scratch_bytes_hint);
+int cube_destroy(cube_ctx* ctx);
+
+/* PAPER.md:263-275, 261. One streaming pass: count, nan_count, min, max, mean, std.
+ * mean and std are accumulated in fp64 about per-thread pivots and merged with the pairwise
+ * (n, mean, M2) update in a fixed tree (deterministic run to run); |rel. error| << 1e-9.
+ * An all-NaN (or empty-of-values) cube gives count = 0 and NaN min/max/mean/std; the call still
+ * returns CUBE_OK because the result is only known on the device. */
+int cube_moments(cube_ctx* ctx, const float* d, int64_t nx, int64_t ny, int64_t nz, unsigned flags,
+                 cube_moments_t* out, cudaStream_t stream);
+
+/* PAPER.md:257-261. bins[b] = #{x : lo <= x <= hi, bin(x) == b}, 0 <= b < nbins, with
+ *   bin(x) = min( floor( (x - lo) * ((float)nbins / (hi - lo)) ), nbins-1 )
+ * every operation rounded to float32, no FMA contraction; hi == lo puts every in-range voxel in bin 0.
+ * outside[0] = #{x < lo}, outside[1] = #{x > hi}; NaN voxels are counted nowhere, so
+ * sum(bins) + outside[0] + outside[1] == count.  1 <= nbins <= CUBE_MAX_BINS. */
+int cube_histogram(cube_ctx* ctx, const float* d, int64_t nx, int64_t ny, int64_t nz, int nbins, float lo,
+                   float hi, uint64_t* bins /* [nbins] */, uint64_t* outside /* [2] */, cudaStream_t stream);
+
+/* PAPER.md:277-296. *out = the element of rank k (0-based) of the non-NaN voxels sorted ascending in
+ * IEEE total order. Exact. If k >= count (known only on the device) *out = NaN. */
+int cube_kth(cube_ctx* ctx, const float* d, int64_t nx, int64_t ny, int64_t nz, uint64_t k, float* out,
+             cudaStream_t stream);
+int cube_kth_ex(cube_ctx* ctx, const float* d, int64_t nx, int64_t ny, int64_t nz, uint64_t k, unsigned flags,
+                float* out, cudaStream_t stream);
+
+/* Lower median: k = (count-1)/2 with count = number of non-NaN voxels (what Alg. 1, PAPER.md:603-609,
+ * returns). count == 0 -> NaN. */
+int cube_median(cube_ctx* ctx, const float* d, int64_t nx, int64_t ny, int64_t nz, float* out,
+                cudaStream_t stream);
+int cube_median_ex(cube_ctx* ctx, const float* d, int64_t nx, int64_t ny, int64_t nz, unsigned flags,
+                   float* out, cudaStream_t stream);
+
+/* ---- Out-of-core / streamed cubes (north_star (4); the paper is in-core by design).
+ * The cube is presented brick by brick (any split into contiguous runs of voxels); each brick is a device
+ * buffer the caller has filled (e.g. by cudaMemcpyAsync from pinned host memory on a side stream).
+ * Sweep 1 accumulates moments + histogram + the first select digit; each further sweep (the caller
+ * re-presents all bricks) refines the median by one digit.  cube_ooc_next_sweep() tells whether another
+ * sweep is needed: *more = 1 until the median is exact (3 sweeps in all, 1 if want_median == 0). */
+int cube_ooc_begin(cube_ctx* ctx, int nbins, float lo, float hi, int want_median, cudaStream_t stream);
+int cube_ooc_brick(cube_ctx* ctx, const float* d_brick, uint64_t nvox, cudaStream_t stream);
+int cube_ooc_next_sweep(cube_ctx* ctx, int* more, cudaStream_t stream);
+int cube_ooc_result(cube_ctx* ctx, unsigned flags, cube_moments_t* moments, uint64_t* bins, uint64_t* outside,
+                    float* median, cudaStream_t stream);
+
+/* Whole-cube convenience over HOST memory (pinned for full speed): streams the cube H2D through
+ * double-buffered chunks overlapped with the kernels and returns moments, histogram and the exact lower
+ * median in HOST memory. If the cube fits in the device workspace given at cube_host_workspace() it is kept
+ * resident after the first sweep, so the host link is crossed once. Synchronises before returning. */
+int cube_host_workspace(cube_ctx* ctx, size_t resident_bytes /* 0 = never keep resident */, size_t chunk_bytes);
+int cube_stats_host(cube_ctx* ctx, const float* h_cube, int64_t nx, int64_t ny, int64_t nz, int nbins, float lo,
+                    float hi, unsigned flags, cube_moments_t* moments, uint64_t* bins, uint64_t* outside,
+                    float* median);
+
+const char* cube_strerror(int code);
+int cube_last_cuda_error(const cube_ctx* ctx);
+
+/* Launch-configuration knobs (0 keeps the default): threads per CTA, resident CTAs per SM. For tuning and
+ * for the tests that check tiling invariance. */
+int cube_set_launch(cube_ctx* ctx, int ctas_per_sm);
+/* Number of kernels launched through this context since creation (bench.py's gpu_launches). */
+uint64_t cube_launch_count(const cube_ctx* ctx);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* CUBE_H_ */

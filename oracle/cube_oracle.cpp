@@ -137,11 +137,11 @@ int oracle_bin_index(float x, int nbins, float lo, float hi) {
 }
 
 // PAPER.md:259-261.  bins[nbins], outside[2] = {#x<lo, #x>hi}; NaN counted nowhere.
-// Returns 1 on invalid arguments (nbins<1, !(lo<=hi), non-finite lo/hi or scale).
+// Returns 1 on invalid arguments (nbins<1, !(lo<=hi), non-finite lo/hi, width or scale; R19).
 int oracle_histogram(const float* d, uint64_t N, int nbins, float lo, float hi,
                      uint64_t* bins, uint64_t* outside) {
     if (nbins < 1 || !(lo <= hi) || !std::isfinite(lo) || !std::isfinite(hi)) return 1;
-    if (hi != lo && !std::isfinite((float)nbins / (hi - lo))) return 1;
+    if (hi != lo && (!std::isfinite(hi - lo) || !std::isfinite((float)nbins / (hi - lo)))) return 1;
     for (int b = 0; b < nbins; ++b) bins[b] = 0;
     outside[0] = outside[1] = 0;
     for (uint64_t i = 0; i < N; ++i) {

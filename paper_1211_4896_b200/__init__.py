@@ -1,0 +1,211 @@
+"""paper_1211_4896_b200 -- thin Python binding of libcube (include/cube.h).
+
+Argument marshalling only: every step of the statistics path runs in the CUDA
+kernels of ``csrc/``.  PyTorch is used by callers for device memory and streams; this module itself
+needs only ctypes.  There is NO CPU fallback: if ``libcube.so`` is missing or no CUDA device is
+present, ``Context()`` raises.  This package never imports ``oracle``.
+
+    ctx = Context()
+    m = ctx.moments(ptr, nx, ny, nz)            # ptr: device pointer (int), e.g. tensor.data_ptr()
+    bins, outside = ctx.histogram(ptr, nx, ny, nz, 4096, -0.02, 0.5)
+    med = ctx.median(ptr, nx, ny, nz)
+"""
+import ctypes
+import os
+
+import numpy as np
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+_LIBPATH = os.path.join(_HERE, "libcube.so")
+
+OK, EINVAL, EEMPTY, ECUDA, ERANGE, ENOMEM = 0, 1, 2, 3, 4, 5
+SAMPLE_STD, COARSE_HIST, REUSE_COARSE = 1, 2, 4
+MAX_BINS = 65536
+
+# every symbol include/cube.h declares (checked by tests/test_abi.py)
+SYMBOLS = ["cube_create", "cube_destroy", "cube_moments", "cube_histogram", "cube_kth", "cube_kth_ex",
+           "cube_median", "cube_median_ex", "cube_ooc_begin", "cube_ooc_brick", "cube_ooc_next_sweep",
+           "cube_ooc_result", "cube_host_workspace", "cube_stats_host", "cube_strerror",
+           "cube_last_cuda_error", "cube_set_launch", "cube_launch_count"]
+
+
+class CubeError(RuntimeError):
+    def __init__(self, code, msg):
+        super().__init__("libcube: %s (code %d)" % (msg, code))
+        self.code = code
+
+
+class MomentsT(ctypes.Structure):
+    _fields_ = [("count", ctypes.c_uint64), ("nan_count", ctypes.c_uint64),
+                ("min", ctypes.c_float), ("max", ctypes.c_float),
+                ("mean", ctypes.c_double), ("std", ctypes.c_double)]
+
+    def as_dict(self):
+        return dict(count=int(self.count), nan_count=int(self.nan_count), min=np.float32(self.min),
+                    max=np.float32(self.max), mean=float(self.mean), std=float(self.std))
+
+
+_lib = None
+
+
+def load():
+    """dlopen libcube.so (built by ``python -m paper_1211_4896_b200.build``).  Fails loudly."""
+    global _lib
+    if _lib is not None:
+        return _lib
+    if not os.path.exists(_LIBPATH):
+        raise ImportError("libcube.so not built: run `python -m paper_1211_4896_b200.build` "
+                          "(there is no CPU fallback)")
+    L = ctypes.CDLL(_LIBPATH)
+    vp, i64, u64, ci, cu, f32, sz = (ctypes.c_void_p, ctypes.c_int64, ctypes.c_uint64, ctypes.c_int,
+                                     ctypes.c_uint, ctypes.c_float, ctypes.c_size_t)
+    L.cube_create.argtypes = [ctypes.POINTER(vp), sz]
+    L.cube_destroy.argtypes = [vp]
+    L.cube_moments.argtypes = [vp, vp, i64, i64, i64, cu, vp, vp]
+    L.cube_histogram.argtypes = [vp, vp, i64, i64, i64, ci, f32, f32, vp, vp, vp]
+    L.cube_kth.argtypes = [vp, vp, i64, i64, i64, u64, vp, vp]
+    L.cube_kth_ex.argtypes = [vp, vp, i64, i64, i64, u64, cu, vp, vp]
+    L.cube_median.argtypes = [vp, vp, i64, i64, i64, vp, vp]
+    L.cube_median_ex.argtypes = [vp, vp, i64, i64, i64, cu, vp, vp]
+    L.cube_ooc_begin.argtypes = [vp, ci, f32, f32, ci, vp]
+    L.cube_ooc_brick.argtypes = [vp, vp, u64, vp]
+    L.cube_ooc_next_sweep.argtypes = [vp, ctypes.POINTER(ci), vp]
+    L.cube_ooc_result.argtypes = [vp, cu, vp, vp, vp, vp, vp]
+    L.cube_host_workspace.argtypes = [vp, sz, sz]
+    L.cube_stats_host.argtypes = [vp, vp, i64, i64, i64, ci, f32, f32, cu, vp, vp, vp, vp]
+    L.cube_strerror.argtypes = [ci]
+    L.cube_strerror.restype = ctypes.c_char_p
+    L.cube_last_cuda_error.argtypes = [vp]
+    L.cube_set_launch.argtypes = [vp, ci]
+    L.cube_launch_count.argtypes = [vp]
+    L.cube_launch_count.restype = u64
+    for name in SYMBOLS:
+        getattr(L, name)
+    _lib = L
+    return L
+
+
+def _ptr(p):
+    """Device/host address as c_void_p.  Accepts int, ctypes pointers, numpy arrays, or anything with
+    ``data_ptr()`` (torch tensors)."""
+    if p is None:
+        return ctypes.c_void_p(None)
+    if hasattr(p, "data_ptr"):
+        return ctypes.c_void_p(p.data_ptr())
+    if isinstance(p, np.ndarray):
+        return ctypes.c_void_p(p.ctypes.data)
+    if isinstance(p, int):
+        return ctypes.c_void_p(p)
+    return ctypes.cast(p, ctypes.c_void_p)
+
+
+class Context:
+    """Owns one ``cube_ctx`` on the current CUDA device.  Methods with ``out=None`` return host values
+    (and therefore synchronise, because results are copied to pageable host memory); pass device or
+    pinned buffers (``out=`` / ``bins=``) for fully asynchronous use."""
+
+    def __init__(self, scratch_bytes_hint=0):
+        self._L = load()
+        h = ctypes.c_void_p()
+        rc = self._L.cube_create(ctypes.byref(h), scratch_bytes_hint)
+        if rc != OK:
+            raise CubeError(rc, "cube_create failed (%s) -- a CUDA device is required, there is no CPU "
+                                "fallback" % self._L.cube_strerror(rc).decode())
+        self._h = h
+
+    def close(self):
+        if getattr(self, "_h", None):
+            self._L.cube_destroy(self._h)
+            self._h = None
+
+    __del__ = close
+
+    def _check(self, rc):
+        if rc != OK:
+            msg = self._L.cube_strerror(rc).decode()
+            if rc == ECUDA:
+                msg += " cudaError=%d" % self._L.cube_last_cuda_error(self._h)
+            raise CubeError(rc, msg)
+
+    # --- in-core operations (d: device pointer) ---------------------------------------------------
+    def moments(self, d, nx, ny, nz, flags=0, out=None, stream=0):
+        if out is not None:
+            self._check(self._L.cube_moments(self._h, _ptr(d), nx, ny, nz, flags, _ptr(out), stream))
+            return None
+        m = MomentsT()
+        self._check(self._L.cube_moments(self._h, _ptr(d), nx, ny, nz, flags,
+                                         ctypes.cast(ctypes.byref(m), ctypes.c_void_p), stream))
+        return m.as_dict()
+
+    def histogram(self, d, nx, ny, nz, nbins, lo, hi, bins=None, outside=None, stream=0):
+        if bins is not None:
+            self._check(self._L.cube_histogram(self._h, _ptr(d), nx, ny, nz, nbins, lo, hi,
+                                               _ptr(bins), _ptr(outside), stream))
+            return None
+        b = np.zeros(max(int(nbins), 1), dtype=np.uint64)
+        o = np.zeros(2, dtype=np.uint64)
+        self._check(self._L.cube_histogram(self._h, _ptr(d), nx, ny, nz, nbins, lo, hi, _ptr(b), _ptr(o), stream))
+        return b, o
+
+    def kth(self, d, nx, ny, nz, k, flags=0, out=None, stream=0):
+        if out is not None:
+            self._check(self._L.cube_kth_ex(self._h, _ptr(d), nx, ny, nz, k, flags, _ptr(out), stream))
+            return None
+        r = ctypes.c_float()
+        self._check(self._L.cube_kth_ex(self._h, _ptr(d), nx, ny, nz, k, flags,
+                                        ctypes.cast(ctypes.byref(r), ctypes.c_void_p), stream))
+        return np.float32(r.value)
+
+    def median(self, d, nx, ny, nz, flags=0, out=None, stream=0):
+        if out is not None:
+            self._check(self._L.cube_median_ex(self._h, _ptr(d), nx, ny, nz, flags, _ptr(out), stream))
+            return None
+        r = ctypes.c_float()
+        self._check(self._L.cube_median_ex(self._h, _ptr(d), nx, ny, nz, flags,
+                                           ctypes.cast(ctypes.byref(r), ctypes.c_void_p), stream))
+        return np.float32(r.value)
+
+    # --- brick-streamed (out-of-core) ------------------------------------------------------------------
+    def ooc_begin(self, nbins, lo, hi, want_median=True, stream=0):
+        self._check(self._L.cube_ooc_begin(self._h, nbins, lo, hi, int(bool(want_median)), stream))
+
+    def ooc_brick(self, d_brick, nvox, stream=0):
+        self._check(self._L.cube_ooc_brick(self._h, _ptr(d_brick), nvox, stream))
+
+    def ooc_next_sweep(self, stream=0):
+        more = ctypes.c_int()
+        self._check(self._L.cube_ooc_next_sweep(self._h, ctypes.byref(more), stream))
+        return bool(more.value)
+
+    def ooc_result(self, nbins, flags=0, want_median=True, stream=0):
+        m = MomentsT()
+        b = np.zeros(max(int(nbins), 1), dtype=np.uint64)
+        o = np.zeros(2, dtype=np.uint64)
+        r = ctypes.c_float(float("nan"))
+        self._check(self._L.cube_ooc_result(self._h, flags, ctypes.cast(ctypes.byref(m), ctypes.c_void_p),
+                                            _ptr(b) if nbins else None, _ptr(o) if nbins else None,
+                                            ctypes.cast(ctypes.byref(r), ctypes.c_void_p) if want_median else None,
+                                            stream))
+        return m.as_dict(), b, o, np.float32(r.value)
+
+    # --- whole cube in HOST memory ---------------------------------------------------------------------
+    def host_workspace(self, resident_bytes=0, chunk_bytes=0):
+        self._check(self._L.cube_host_workspace(self._h, resident_bytes, chunk_bytes))
+
+    def stats_host(self, h_cube, nx, ny, nz, nbins, lo, hi, flags=0, want_median=True):
+        m = MomentsT()
+        b = np.zeros(max(int(nbins), 1), dtype=np.uint64)
+        o = np.zeros(2, dtype=np.uint64)
+        r = ctypes.c_float(float("nan"))
+        self._check(self._L.cube_stats_host(self._h, _ptr(h_cube), nx, ny, nz, nbins, lo, hi, flags,
+                                            ctypes.cast(ctypes.byref(m), ctypes.c_void_p), _ptr(b), _ptr(o),
+                                            ctypes.cast(ctypes.byref(r), ctypes.c_void_p) if want_median else None))
+        return m.as_dict(), b, o, np.float32(r.value)
+
+    # --- knobs -----------------------------------------------------------------------------------------
+    def set_launch(self, ctas_per_sm):
+        self._check(self._L.cube_set_launch(self._h, ctas_per_sm))
+
+    @property
+    def launch_count(self):
+        return int(self._L.cube_launch_count(self._h))

@@ -1,0 +1,33 @@
+"""Build libcube.so (the C-ABI CUDA library) in-tree with nvcc for sm_100a.
+
+    python -m paper_1211_4896_b200.build [--force]
+"""
+import os
+import subprocess
+import sys
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+CSRC = os.path.join(_HERE, "csrc")
+LIB = os.path.join(_HERE, "libcube.so")
+SOURCES = ["cube.cu"]
+DEPS = ["cube.cu", "cube_ooc.inl", "cube_kernels.cuh", "cube_common.cuh", os.path.join("..", "..", "include", "cube.h")]
+NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17",
+              "--fmad=true",            # contraction is confined to fp64 fma() calls we write ourselves;
+                                        # the float32 bin formula uses __fsub_rn/__fmul_rn (never contracted)
+              "-Xcompiler", "-fPIC", "-shared"]
+
+
+def build(force=False, verbose=False):
+    newest = max(os.path.getmtime(os.path.join(CSRC, d)) for d in DEPS)
+    if not force and os.path.exists(LIB) and os.path.getmtime(LIB) >= newest:
+        return LIB
+    tmp = LIB + ".tmp.%d" % os.getpid()
+    cmd = ["nvcc"] + NVCC_FLAGS + (["-Xptxas", "-v"] if verbose else []) + ["-o", tmp] + \
+          [os.path.join(CSRC, s) for s in SOURCES]
+    subprocess.check_call(cmd)
+    os.replace(tmp, LIB)
+    return LIB
+
+
+if __name__ == "__main__":
+    print(build(force="--force" in sys.argv, verbose="-v" in sys.argv))

@@ -1,0 +1,137 @@
+// cube_common.cuh -- shared device helpers of libcube (CUDA path only; the CPU oracle under
+// oracle/ shares nothing with this file).
+//
+// Streaming model: every operation of the paper's statistics path visits each
+// voxel once per pass ("visiting each data value once"; "visiting each data
+// point and classifying it").  On B200 that is an HBM-read-bound scan, so all kernels share one
+// persistent, coalesced, 128-bit streaming loop and differ only in the per-voxel functor.
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+namespace cube {
+
+constexpr int kThreads = 256;  // threads per CTA (8 warps)
+constexpr int kUnroll = 8;     // independent 128-bit loads in flight per thread per tile
+constexpr int kTileVec = kThreads * kUnroll;  // float4 per tile (32 KiB)
+
+// 128-bit read-only load that does not allocate in L1 (each voxel is used once per pass).  L2 policy is
+// left at the default so that cubes smaller than the 126 MB L2 (config 1) are re-read from L2 by the
+// later select passes.
+__device__ __forceinline__ float4 ld_stream(const float4* p) {
+    float4 r;
+    asm volatile("ld.global.nc.L1::no_allocate.v4.f32 {%0,%1,%2,%3}, [%4];"
+                 : "=f"(r.x), "=f"(r.y), "=f"(r.z), "=f"(r.w)
+                 : "l"(p));
+    return r;
+}
+
+// Order-preserving map float32 bits -> uint32 (IEEE total order on non-NaN: -0.0 < +0.0; R7).
+// Negative values: flip all bits; non-negative: set the sign bit.
+__device__ __forceinline__ uint32_t key_of(float x) {
+    uint32_t u = __float_as_uint(x);
+    return u ^ ((uint32_t)((int32_t)u >> 31) | 0x80000000u);
+}
+__host__ __device__ __forceinline__ uint32_t bits_of_key(uint32_t k) {
+    return (k & 0x80000000u) ? (k ^ 0x80000000u) : ~k;
+}
+
+// Visit all n voxels of d exactly once across the grid.  F provides `void operator()(float)`.
+// Tiles of kTileVec float4 are dealt round-robin to the CTAs, so concurrently running CTAs read adjacent
+// 32 KiB tiles (DRAM page locality) and the assignment is static => per-CTA results are deterministic.
+// The <= 3 voxels before the first 16-byte boundary and the <= 3 after the last full float4 are visited
+// by CTA 0.
+template <class F>
+__device__ __forceinline__ void stream_cube(const float* __restrict__ d, uint64_t n, F& f) {
+    uint64_t head = ((16u - (uint32_t)((uintptr_t)d & 15u)) & 15u) >> 2;
+    if (head > n) head = n;
+    const float4* __restrict__ v = reinterpret_cast<const float4*>(d + head);
+    const uint64_t nvec = (n - head) >> 2;
+    const uint64_t tail0 = head + (nvec << 2);
+    if (blockIdx.x == 0) {
+        if (threadIdx.x < head) f(d[threadIdx.x]);
+        if (threadIdx.x >= 32 && threadIdx.x < 35) {
+            uint64_t t = tail0 + (threadIdx.x - 32);
+            if (t < n) f(d[t]);
+        }
+    }
+    const uint64_t ntiles = (nvec + kTileVec - 1) / kTileVec;
+    for (uint64_t t = blockIdx.x; t < ntiles; t += gridDim.x) {
+        const uint64_t base = t * kTileVec + threadIdx.x;
+        if (base + (uint64_t)(kUnroll - 1) * kThreads < nvec) {
+            float4 r[kUnroll];
+#pragma unroll
+            for (int j = 0; j < kUnroll; ++j) r[j] = ld_stream(v + base + (uint64_t)j * kThreads);
+#pragma unroll
+            for (int j = 0; j < kUnroll; ++j) {
+                f(r[j].x); f(r[j].y); f(r[j].z); f(r[j].w);
+            }
+        } else {
+#pragma unroll 1
+            for (int j = 0; j < kUnroll; ++j) {
+                uint64_t i = base + (uint64_t)j * kThreads;
+                if (i < nvec) {
+                    float4 r = ld_stream(v + i);
+                    f(r.x); f(r.y); f(r.z); f(r.w);
+                }
+            }
+        }
+    }
+}
+
+// ---------------------------------------------------------------- (n, mean, M2, min, max) partials
+// Pairwise update of Chan, Golub & LeVeque for merging two (n, mean, M2) summaries; what the paper's
+// server does with (count, sum, sum of squares) in O(1), in a cancellation-free form.
+struct Partial {
+    uint64_t n;
+    double mean, m2;
+    uint32_t kmin, kmax;  // order-preserving keys; kmin=0xFFFFFFFF / kmax=0 when n == 0
+};
+
+__device__ __forceinline__ Partial partial_empty() {
+    Partial p;
+    p.n = 0; p.mean = 0.0; p.m2 = 0.0; p.kmin = 0xFFFFFFFFu; p.kmax = 0u;
+    return p;
+}
+
+__device__ __forceinline__ Partial partial_merge(const Partial& a, const Partial& b) {
+    Partial r;
+    r.kmin = min(a.kmin, b.kmin);
+    r.kmax = max(a.kmax, b.kmax);
+    r.n = a.n + b.n;
+    if (b.n == 0) { r.mean = a.mean; r.m2 = a.m2; return r; }
+    if (a.n == 0) { r.mean = b.mean; r.m2 = b.m2; return r; }
+    const double na = (double)a.n, nb = (double)b.n, nn = (double)r.n;
+    const double delta = b.mean - a.mean;
+    r.mean = a.mean + delta * (nb / nn);
+    r.m2 = a.m2 + b.m2 + delta * delta * (na * (nb / nn));
+    return r;
+}
+
+__device__ __forceinline__ Partial partial_shfl_down(const Partial& p, int off) {
+    Partial q;
+    q.n = __shfl_down_sync(0xffffffffu, p.n, off);
+    q.mean = __shfl_down_sync(0xffffffffu, p.mean, off);
+    q.m2 = __shfl_down_sync(0xffffffffu, p.m2, off);
+    q.kmin = __shfl_down_sync(0xffffffffu, p.kmin, off);
+    q.kmax = __shfl_down_sync(0xffffffffu, p.kmax, off);
+    return q;
+}
+
+// Fixed-shape tree over the CTA: lanes (shuffle, offsets 16..1) then warps (first warp).  Result valid
+// in thread 0.  `scratch` holds kThreads/32 Partials of shared memory.
+__device__ __forceinline__ Partial partial_block_reduce(Partial p, Partial* scratch) {
+#pragma unroll
+    for (int off = 16; off > 0; off >>= 1) p = partial_merge(p, partial_shfl_down(p, off));
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    if (lane == 0) scratch[warp] = p;
+    __syncthreads();
+    if (warp == 0) {
+        p = (lane < kThreads / 32) ? scratch[lane] : partial_empty();
+#pragma unroll
+        for (int off = 16; off > 0; off >>= 1) p = partial_merge(p, partial_shfl_down(p, off));
+    }
+    return p;
+}
+
+}  // namespace cube

@@ -1,0 +1,146 @@
+// cube_ooc.inl -- brick-streamed (out-of-core) statistics and the host-cube driver.  Included by cube.cu.
+//
+// The paper's framework is in-core by design and rules out host memory; north_star (4)
+// adds cubes larger than HBM: bricks are staged through device buffers and every accumulator
+// (running (n, mean, M2, min, max), histogram bins, select digit bins) lives on the device across bricks.
+// The merges are the associative/commutative ones the paper relies on.
+
+extern "C" {
+
+int cube_ooc_begin(cube_ctx* c, int nbins, float lo, float hi, int want_median, cudaStream_t s) {
+    if (!c) return CUBE_EINVAL;
+    float scale = 0.f;
+    if (nbins != 0 && !hist_scale(nbins, lo, hi, &scale)) return CUBE_EINVAL;
+    c->ooc_active = 1; c->ooc_sweep = 0; c->ooc_bricks = 0;
+    c->ooc_nbins = nbins; c->ooc_lo = lo; c->ooc_hi = hi; c->ooc_scale = scale;
+    c->ooc_want_median = want_median ? 1 : 0;
+    CUBE_CUDA(c, cudaMemsetAsync(c->gbins, 0, (CUBE_MAX_BINS + 2) * sizeof(unsigned long long), s));
+    CUBE_CUDA(c, cudaMemsetAsync(c->gdigits, 0, kDigitBins * sizeof(unsigned long long), s));
+    return select_init(c, 0, 1, s);
+}
+
+int cube_ooc_brick(cube_ctx* c, const float* d, uint64_t nvox, cudaStream_t s) {
+    if (!c || !c->ooc_active || !d || nvox == 0 || nvox > (1ull << 37)) return CUBE_EINVAL;
+    int rc = CUBE_OK;
+    if (c->ooc_sweep == 0) {
+        if ((rc = launch_moments(c, d, nvox, 0u, c->ooc_bricks > 0, s))) return rc;
+        if (c->ooc_nbins > 0 &&
+            (rc = launch_hist(c, d, nvox, c->ooc_nbins, c->ooc_lo, c->ooc_hi, c->ooc_scale, s))) return rc;
+        if (c->ooc_want_median && (rc = launch_select_pass<0>(c, d, nvox, s))) return rc;
+    } else if (c->ooc_sweep == 1) {
+        rc = launch_select_pass<1>(c, d, nvox, s);
+    } else if (c->ooc_sweep == 2) {
+        rc = launch_select_pass<2>(c, d, nvox, s);
+    } else {
+        return CUBE_EINVAL;
+    }
+    c->ooc_bricks++;
+    return rc;
+}
+
+int cube_ooc_next_sweep(cube_ctx* c, int* more, cudaStream_t s) {
+    if (!c || !c->ooc_active || !more) return CUBE_EINVAL;
+    int rc = CUBE_OK;
+    *more = 0;
+    if (c->ooc_want_median) {
+        if (c->ooc_sweep == 0) { rc = launch_select_scan<0>(c, c->gdigits, s); *more = 1; }
+        else if (c->ooc_sweep == 1) { rc = launch_select_scan<1>(c, c->gdigits, s); *more = 1; }
+        else if (c->ooc_sweep == 2) { rc = launch_select_scan<2>(c, c->gdigits, s); }
+    }
+    c->ooc_sweep++;
+    return rc;
+}
+
+int cube_ooc_result(cube_ctx* c, unsigned flags, cube_moments_t* moments, uint64_t* bins, uint64_t* outside,
+                    float* median, cudaStream_t s) {
+    if (!c || !c->ooc_active) return CUBE_EINVAL;
+    if (moments) {
+        if (flags & CUBE_SAMPLE_STD) {
+            // re-finalise the running partial with the sample-std denominator
+            moments_refinalize_kernel<<<1, 1, 0, s>>>(c->acc, c->nvox_acc, flags, c->mom_out);
+            c->launches++;
+            CUBE_CUDA(c, cudaGetLastError());
+        }
+        CUBE_CUDA(c, cudaMemcpyAsync(moments, c->mom_out, sizeof(MomentsOut), cudaMemcpyDefault, s));
+    }
+    if (bins && c->ooc_nbins > 0)
+        CUBE_CUDA(c, cudaMemcpyAsync(bins, c->gbins, (size_t)c->ooc_nbins * sizeof(uint64_t), cudaMemcpyDefault, s));
+    if (outside && c->ooc_nbins > 0)
+        CUBE_CUDA(c, cudaMemcpyAsync(outside, c->gbins + CUBE_MAX_BINS, 2 * sizeof(uint64_t), cudaMemcpyDefault, s));
+    if (median) {
+        if (!c->ooc_want_median || c->ooc_sweep < 3) return CUBE_EINVAL;
+        CUBE_CUDA(c, cudaMemcpyAsync(median, &c->sel->result, sizeof(float), cudaMemcpyDefault, s));
+    }
+    return CUBE_OK;
+}
+
+int cube_host_workspace(cube_ctx* c, size_t resident_bytes, size_t chunk_bytes) {
+    if (!c) return CUBE_EINVAL;
+    if (chunk_bytes == 0) chunk_bytes = (size_t)256 << 20;
+    chunk_bytes = (chunk_bytes + 15) & ~(size_t)15;
+    cudaFree(c->resident); c->resident = nullptr; c->resident_bytes = 0;
+    cudaFree(c->chunk[0]); cudaFree(c->chunk[1]); c->chunk[0] = c->chunk[1] = nullptr;
+    c->chunk_bytes = chunk_bytes;
+    if (resident_bytes) {
+        if (cudaMalloc(&c->resident, resident_bytes) != cudaSuccess) { cudaGetLastError(); return CUBE_ENOMEM; }
+        c->resident_bytes = resident_bytes;
+    }
+    for (int i = 0; i < 2; ++i)
+        if (cudaMalloc(&c->chunk[i], chunk_bytes) != cudaSuccess) { cudaGetLastError(); return CUBE_ENOMEM; }
+    if (!c->copy_stream) {
+        CUBE_CUDA(c, cudaStreamCreateWithFlags(&c->copy_stream, cudaStreamNonBlocking));
+        CUBE_CUDA(c, cudaStreamCreateWithFlags(&c->work_stream, cudaStreamNonBlocking));
+        for (int i = 0; i < 2; ++i) {
+            CUBE_CUDA(c, cudaEventCreateWithFlags(&c->ev_copied[i], cudaEventDisableTiming));
+            CUBE_CUDA(c, cudaEventCreateWithFlags(&c->ev_consumed[i], cudaEventDisableTiming));
+        }
+    }
+    return CUBE_OK;
+}
+
+int cube_stats_host(cube_ctx* c, const float* h, int64_t nx, int64_t ny, int64_t nz, int nbins, float lo, float hi,
+                    unsigned flags, cube_moments_t* moments, uint64_t* bins, uint64_t* outside, float* median) {
+    uint64_t n;
+    if (!c || !h || !dims_ok(nx, ny, nz, &n)) return CUBE_EINVAL;
+    if (!c->chunk[0]) {
+        int rc0 = cube_host_workspace(c, 0, 0);
+        if (rc0) return rc0;
+    }
+    const int want_median = median != nullptr;
+    cudaStream_t ws = c->work_stream, cs = c->copy_stream;
+    int rc = cube_ooc_begin(c, (bins && outside) ? nbins : 0, lo, hi, want_median, ws);
+    if (rc) return rc;
+    const uint64_t chunk_vox = c->chunk_bytes / sizeof(float);
+    const uint64_t nchunks = (n + chunk_vox - 1) / chunk_vox;
+    const bool resident = c->resident && n * sizeof(float) <= c->resident_bytes;
+    int more = 1;
+    for (int sweep = 0; more; ++sweep) {
+        if (resident && sweep > 0) {
+            // the whole cube is in HBM now: finish the select in-core, one launch per pass
+            if ((rc = cube_ooc_brick(c, c->resident, n, ws))) return rc;
+        } else {
+            for (uint64_t i = 0; i < nchunks; ++i) {
+                const uint64_t off = i * chunk_vox;
+                const uint64_t cnt = (n - off < chunk_vox) ? n - off : chunk_vox;
+                const int b = (int)(i & 1);
+                float* dst = resident ? c->resident + off : c->chunk[b];
+                if (!resident) CUBE_CUDA(c, cudaStreamWaitEvent(cs, c->ev_consumed[b], 0));
+                CUBE_CUDA(c, cudaMemcpyAsync(dst, h + off, cnt * sizeof(float), cudaMemcpyHostToDevice, cs));
+                CUBE_CUDA(c, cudaEventRecord(c->ev_copied[b], cs));
+                CUBE_CUDA(c, cudaStreamWaitEvent(ws, c->ev_copied[b], 0));
+                if ((rc = cube_ooc_brick(c, dst, cnt, ws))) return rc;
+                CUBE_CUDA(c, cudaEventRecord(c->ev_consumed[b], ws));
+            }
+        }
+        if ((rc = cube_ooc_next_sweep(c, &more, ws))) return rc;
+    }
+    rc = cube_ooc_result(c, flags, moments, (bins && outside) ? bins : nullptr, (bins && outside) ? outside : nullptr,
+                         median, ws);
+    if (rc) return rc;
+    CUBE_CUDA(c, cudaStreamSynchronize(ws));
+    CUBE_CUDA(c, cudaStreamSynchronize(cs));
+    c->ooc_active = 0;
+    return CUBE_OK;
+}
+
+}  // extern "C"

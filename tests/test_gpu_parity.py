@@ -1,0 +1,354 @@
+"""GPU parity: the CUDA path (libcube through its C ABI) against the CPU oracle, element by element on
+the same seeded inputs.  Bar (BASELINE.json north_star): bit-exact count / nan_count / min / max /
+histogram / k-th / median; |rel. error| <= 1e-9 for mean and std (floor of DESIGN.md R16 on
+degenerate cubes).  Every test needs a CUDA device and FAILS without one (no CPU fallback)."""
+import math
+
+import numpy as np
+import pytest
+import torch
+
+import cubegen
+import oracle
+import paper_1211_4896_b200 as cube
+
+pytestmark = pytest.mark.gpu
+
+REL = 1e-9
+
+
+@pytest.fixture(scope="module")
+def ctx():
+    assert torch.cuda.is_available(), "gpu tests need a CUDA device (there is no CPU fallback)"
+    torch.cuda.init()
+    c = cube.Context()
+    yield c
+    c.close()
+
+
+def dev(a, misalign=0):
+    """numpy float32 -> device tensor; `misalign` floats of offset from a 16-byte boundary."""
+    a = np.ascontiguousarray(a, dtype=np.float32).reshape(-1)
+    buf = torch.empty(a.size + 4 + misalign, dtype=torch.float32, device="cuda")
+    view = buf[misalign:misalign + a.size]
+    view.copy_(torch.from_numpy(a))
+    assert view.data_ptr() % 16 == (4 * misalign) % 16
+    return view
+
+
+def bits(x):
+    return int(np.float32(x).view(np.uint32))
+
+
+def same_float(a, b):
+    a, b = np.float32(a), np.float32(b)
+    if math.isnan(float(a)) or math.isnan(float(b)):
+        return math.isnan(float(a)) and math.isnan(float(b))
+    return bits(a) == bits(b)
+
+
+def check_moments(got, ref, a):
+    assert got["count"] == ref["count"] and got["nan_count"] == ref["nan_count"]
+    assert same_float(got["min"], ref["min"]) and same_float(got["max"], ref["max"])
+    if ref["count"] == 0:
+        assert math.isnan(got["mean"]) and math.isnan(got["std"])
+        return
+    if math.isnan(ref["std"]):
+        assert math.isnan(got["std"])
+    fin = a[np.isfinite(a)] if a is not None else None
+    # R16: relative 1e-9, with a floor that only matters on degenerate cubes (std == 0, mean ~ 0)
+    mabs = float(np.mean(np.abs(fin.astype(np.float64)))) if fin is not None and fin.size else 0.0
+    mext = max(abs(float(ref["min"])), abs(float(ref["max"])))
+    assert abs(got["mean"] - ref["mean"]) <= REL * max(abs(ref["mean"]), 1e-6 * mabs), (got, ref)
+    if not math.isnan(ref["std"]):
+        assert abs(got["std"] - ref["std"]) <= REL * max(ref["std"], 1e-6 * mext), (got, ref)
+
+
+def full_check(ctx, a, hists=(), ks=(), misalign=0):
+    a = np.ascontiguousarray(a, dtype=np.float32).reshape(-1)
+    t = dev(a, misalign)
+    n = a.size
+    ref = oracle.moments(a)
+    check_moments(ctx.moments(t, n, 1, 1), ref, a)
+    check_moments(ctx.moments(t, n, 1, 1, flags=cube.SAMPLE_STD), oracle.moments(a, sample_std=True), a)
+    for nbins, lo, hi in hists:
+        try:
+            rb, ro = oracle.histogram(a, nbins, lo, hi)
+        except ValueError:                      # e.g. scale overflows float32 on a subnormal range (R19)
+            with pytest.raises(cube.CubeError):
+                ctx.histogram(t, n, 1, 1, nbins, lo, hi)
+            continue
+        b, o = ctx.histogram(t, n, 1, 1, nbins, lo, hi)
+        assert (b == rb).all() and (o == ro).all(), (nbins, lo, hi)
+        assert int(b.sum() + o.sum()) == ref["count"]
+    cnt = ref["count"]
+    med = ctx.median(t, n, 1, 1)
+    assert same_float(med, oracle.median(a))
+    for k in ks:
+        if k < cnt:
+            assert same_float(ctx.kth(t, n, 1, 1, k), oracle.kth(a, k)), k
+        else:
+            assert math.isnan(float(ctx.kth(t, n, 1, 1, k)))
+    return ref
+
+
+def std_ks(n):
+    return sorted(set(k for k in (0, 1, n // 100, (n - 1) // 2, n // 2, 99 * n // 100, n - 2, n - 1, n, n + 5)
+                      if k >= 0))
+
+
+# ------------------------------------------------------------------------------------------------ small
+@pytest.mark.parametrize("n", [1, 2, 3, 4, 5, 7, 31, 257, 1023, 4099, 8192 * 4 + 3, 37 * 41 * 43, 300001])
+@pytest.mark.parametrize("misalign", [0, 1, 3])
+def test_small_noise_with_nans(ctx, n, misalign):
+    r = np.random.default_rng(n * 7 + misalign)
+    a = (r.standard_normal(n) * 0.002).astype(np.float32)
+    if n > 4:
+        a[r.integers(0, n, max(1, n // 50))] = np.nan
+    cnt = int((~np.isnan(a)).sum())
+    full_check(ctx, a, hists=[(256, -0.005, 0.005), (4096, -0.02, 0.5), (1, -1.0, 1.0), (7, 0.0, 0.001)],
+               ks=std_ks(cnt), misalign=misalign)
+
+
+def test_degenerate_cubes(ctx):
+    qn = np.float32("nan")
+    neg_nan = np.frombuffer(np.uint32(0xFFC00000).tobytes(), dtype=np.float32)[0]
+    cases = [
+        np.full(100000, 0.1, np.float32),                                  # constant: std == 0 exactly
+        np.full(70001, -1234.567, np.float32),
+        np.full(5000, qn, np.float32),                                     # all blanked
+        np.array([qn, 2.5, neg_nan], np.float32),                          # single value
+        np.array([0.0, -0.0, 0.0, -0.0, -0.0], np.float32),                # signed zeros (R7)
+        np.array([1e-40, -1e-40, 0.0, -0.0, 1e-45, 3e-39], np.float32),    # subnormals (R9)
+        np.array([np.inf, -np.inf, 1.0, qn, 2.0], np.float32),             # infinities (R8)
+        np.concatenate([np.full(40000, 0.1, np.float32), np.full(30000, qn, np.float32),
+                        np.full(40000, 0.1, np.float32)]),                 # constant with a blanked slab
+        np.arange(1 << 20, dtype=np.float32),                              # ramp: closed forms
+        np.arange(1 << 20, dtype=np.float32)[::-1].copy() - np.float32(2 ** 19),
+    ]
+    for a in cases:
+        cnt = int((~np.isnan(a)).sum())
+        fin = a[np.isfinite(a)]
+        hists = [(16, -1.0, 1.0), (1024, 0.0, float(1 << 20))]
+        if fin.size:
+            hists.append((64, float(fin.min()), float(fin.max())))         # hi == lo on constant cubes (R13)
+        got = None
+        if np.isinf(a).any():
+            t = dev(a)
+            got, ref = ctx.moments(t, a.size, 1, 1), oracle.moments(a)
+            assert got["count"] == ref["count"] and same_float(got["min"], ref["min"]) and same_float(got["max"], ref["max"])
+            assert same_float(ctx.median(t, a.size, 1, 1), oracle.median(a))
+            for k in range(cnt):
+                assert same_float(ctx.kth(t, a.size, 1, 1, k), oracle.kth(a, k))
+            continue
+        ref = full_check(ctx, a, hists=hists, ks=std_ks(cnt))
+        if cnt and float(fin.min()) == float(fin.max()):
+            t = dev(a)
+            m = ctx.moments(t, a.size, 1, 1)
+            assert m["std"] == 0.0 and m["mean"] == float(fin[0])           # exactly
+
+
+def test_ramp_closed_forms_direct(ctx):
+    # independent of the oracle: north_star's closed forms
+    N = 1 << 24
+    t = torch.arange(N, dtype=torch.float32, device="cuda")
+    m = ctx.moments(t, 256, 256, 256)
+    assert m["count"] == N and m["min"] == 0.0 and m["max"] == np.float32(N - 1)
+    assert abs(m["mean"] - (N - 1) / 2.0) <= REL * (N - 1) / 2.0
+    assert abs(m["std"] - math.sqrt((N * N - 1) / 12.0)) <= REL * math.sqrt((N * N - 1) / 12.0)
+    b, o = ctx.histogram(t, 256, 256, 256, 65536, 0.0, float(N))
+    assert (b == N // 65536).all() and o.tolist() == [0, 0]
+    b, o = ctx.histogram(t, 256, 256, 256, 4096, 0.0, float(N))
+    assert (b == N // 4096).all()
+    for k in (0, 12345, (N - 1) // 2, N - 1):
+        assert ctx.kth(t, 256, 256, 256, k) == np.float32(k)
+    assert ctx.median(t, 256, 256, 256) == np.float32((N - 1) // 2)
+
+
+def test_heavy_ties_and_hot_bins(ctx):
+    r = np.random.default_rng(4)
+    n = 1 << 21
+    a = cubegen.generate_numpy(cubegen.scaled("c4", (256, 256, 32))).reshape(-1)
+    ref = full_check(ctx, a, hists=[(256, 0.0, float(a.max())), (65536, 0.0, float(a.max())), (4096, 0.0, 1.0)],
+                     ks=std_ks(n))
+    assert ref["min"] == 0.0
+    b = r.integers(0, 3, n).astype(np.float32)                             # three values only
+    full_check(ctx, b, hists=[(3, 0.0, 2.0), (65536, 0.0, 2.0)], ks=std_ks(n))
+
+
+@pytest.mark.parametrize("nbins", [1, 2, 255, 1024, 4096, 16384, 16385, 40000, 65536])
+def test_histogram_bin_counts_all_sizes(ctx, nbins):
+    r = np.random.default_rng(nbins)
+    a = np.concatenate([(r.standard_normal(200000) * 0.3).astype(np.float32),
+                        r.uniform(-2, 2, 100001).astype(np.float32)])
+    a[::97] = np.nan
+    t = dev(a)
+    for lo, hi in ((-1.0, 1.0), (float(np.nanmin(a)), float(np.nanmax(a))), (0.25, 0.25000003)):
+        b, o = ctx.histogram(t, a.size, 1, 1, nbins, lo, hi)
+        rb, ro = oracle.histogram(a, nbins, lo, hi)
+        assert (b == rb).all() and (o == ro).all()
+
+
+def test_invalid_arguments(ctx):
+    t = dev(np.zeros(16, np.float32))
+    for bad in ((0, 0.0, 1.0), (65537, 0.0, 1.0), (4, 1.0, 0.0), (4, float("nan"), 1.0), (4, 0.0, float("inf")),
+                (4, -3e38, 3e38)):
+        with pytest.raises(cube.CubeError) as e:
+            ctx.histogram(t, 16, 1, 1, *bad)
+        assert e.value.code == cube.EINVAL
+    for dims in ((0, 1, 1), (-4, 1, 1), (1 << 20, 1 << 20, 1 << 20)):
+        with pytest.raises(cube.CubeError):
+            ctx.moments(t, *dims)
+    with pytest.raises(cube.CubeError):
+        ctx.median(None, 16, 1, 1)
+
+
+def test_tiling_invariance(ctx):
+    # any tiling of the cube over CTAs gives identical integers (order-free merges)
+    a = cubegen.generate_numpy(cubegen.scaled("c3", (128, 128, 64))).reshape(-1)
+    t = dev(a, 2)
+    base = None
+    try:
+        for per_sm in (1, 2, 3, 5, 8):
+            ctx.set_launch(per_sm)
+            m = ctx.moments(t, a.size, 1, 1)
+            b, o = ctx.histogram(t, a.size, 1, 1, 1000, -0.01, 0.02)
+            med = ctx.median(t, a.size, 1, 1)
+            cur = (m["count"], m["nan_count"], bits(m["min"]), bits(m["max"]), b.tobytes(), o.tobytes(), bits(med))
+            if base is None:
+                base, m0 = cur, m
+            assert cur == base
+            assert abs(m["mean"] - m0["mean"]) <= 1e-13 * abs(m0["mean"]) + 1e-300
+            assert abs(m["std"] - m0["std"]) <= 1e-13 * m0["std"]
+    finally:
+        ctx.set_launch(0)
+    m1 = ctx.moments(t, a.size, 1, 1)
+    m2 = ctx.moments(t, a.size, 1, 1)
+    assert m1 == m2 or (m1["mean"] == m2["mean"] and m1["std"] == m2["std"])   # run-to-run deterministic
+
+
+def test_device_and_pinned_outputs_on_a_stream(ctx):
+    a = cubegen.generate_numpy(cubegen.scaled("c1", (64, 64, 64), nsrc=3)).reshape(-1)
+    t = dev(a)
+    s = torch.cuda.Stream()
+    out_m = torch.zeros(40, dtype=torch.uint8, device="cuda")
+    out_b = torch.zeros(1024, dtype=torch.int64, device="cuda")
+    out_o = torch.zeros(2, dtype=torch.int64, device="cuda")
+    out_med = torch.zeros(1, dtype=torch.float32).pin_memory()
+    with torch.cuda.stream(s):
+        ctx.moments(t, 64, 64, 64, out=out_m, stream=s.cuda_stream)
+        ctx.histogram(t, 64, 64, 64, 1024, -5.0, 5.0, bins=out_b, outside=out_o, stream=s.cuda_stream)
+        ctx.median(t, 64, 64, 64, out=out_med, stream=s.cuda_stream)
+    s.synchronize()
+    m = cube.MomentsT.from_buffer_copy(out_m.cpu().numpy().tobytes()).as_dict()
+    check_moments(m, oracle.moments(a), a)
+    rb, ro = oracle.histogram(a, 1024, -5.0, 5.0)
+    assert (out_b.cpu().numpy().astype(np.uint64) == rb).all() and (out_o.cpu().numpy().astype(np.uint64) == ro).all()
+    assert same_float(out_med.numpy()[0], oracle.median(a))
+
+
+def test_coarse_histogram_reuse(ctx):
+    a = cubegen.generate_numpy(cubegen.scaled("c2", (64, 64, 256), nsrc=4)).reshape(-1)
+    t = dev(a)
+    m = ctx.moments(t, a.size, 1, 1, flags=cube.COARSE_HIST)
+    check_moments(m, oracle.moments(a), a)
+    assert same_float(ctx.median(t, a.size, 1, 1, flags=cube.REUSE_COARSE), oracle.median(a))
+    m = ctx.moments(t, a.size, 1, 1, flags=cube.COARSE_HIST)
+    k = m["count"] // 100
+    assert same_float(ctx.kth(t, a.size, 1, 1, k, flags=cube.REUSE_COARSE), oracle.kth(a, k))
+
+
+# ------------------------------------------------------------------------------------------------ configs
+def _config_case(ctx, cfg, hists, extra_ks=()):
+    nx, ny, nz = cfg["dims"]
+    n = nx * ny * nz
+    t = torch.empty(n, dtype=torch.float32, device="cuda")
+    cubegen.generate_device(cfg, t.data_ptr())
+    torch.cuda.synchronize()
+    a = t.cpu().numpy()
+    ref = oracle.moments(a)
+    check_moments(ctx.moments(t, nx, ny, nz), ref, a)
+    for nbins, lo, hi in hists:
+        if lo is None:
+            lo, hi = float(ref["min"]), float(ref["max"])
+        b, o = ctx.histogram(t, nx, ny, nz, nbins, lo, hi)
+        rb, ro = oracle.histogram(a, nbins, lo, hi)
+        assert (b == rb).all() and (o == ro).all()
+    med = ctx.median(t, nx, ny, nz)
+    assert same_float(med, oracle.median(a))
+    less, equal = oracle.rank_counts(a, med)
+    kmed = (ref["count"] - 1) // 2
+    assert equal >= 1 and less <= kmed < less + equal
+    for k in extra_ks:
+        k = int(k(ref["count"]))
+        assert same_float(ctx.kth(t, nx, ny, nz, k), oracle.kth(a, k))
+    return a, ref
+
+
+def test_config1_full(ctx):
+    # BASELINE.json configs[0]: 256^3, seed 1; 1024 bins over [min,max]; exact lower median
+    a, ref = _config_case(ctx, cubegen.CONFIGS["c1"], [(1024, None, None)])
+    assert ref["nan_count"] == 0 and (ref["count"] - 1) // 2 == 8388607
+
+
+def test_config2_scaled(ctx):
+    _config_case(ctx, cubegen.scaled("c2", (256, 256, 1024)), [(4096, -0.02, 0.5)])
+
+
+def test_config3_scaled(ctx):
+    _config_case(ctx, cubegen.scaled("c3", (256, 256, 512)), [(65536, None, None)],
+                 extra_ks=(lambda n: n // 100, lambda n: 99 * n // 100))
+
+
+def test_config4_scaled(ctx):
+    a, ref = _config_case(ctx, cubegen.scaled("c4", (512, 512, 64)), [(256, None, None), (65536, None, None)])
+    assert ref["min"] == 0.0
+
+
+def test_config5_scaled_out_of_core(ctx):
+    # 8 bricks of 64^3 out of a 128^3 cube, streamed in brick order, vs the whole cube in-core and the oracle
+    cfg = cubegen.scaled("c5", (128, 128, 128), nsrc=40)
+    bricks = []
+    for oz in (0, 64):
+        for oy in (0, 64):
+            for ox in (0, 64):
+                t = torch.empty(64 ** 3, dtype=torch.float32, device="cuda")
+                cubegen.generate_device(cfg, t.data_ptr(), origin=(ox, oy, oz), brick=(64, 64, 64))
+                bricks.append(t)
+    torch.cuda.synchronize()
+    whole = torch.cat(bricks)
+    a = whole.cpu().numpy()
+    ctx.ooc_begin(4096, -0.02, 0.5, want_median=True)
+    more = True
+    sweeps = 0
+    while more:
+        for t in bricks:
+            ctx.ooc_brick(t, t.numel())
+        more = ctx.ooc_next_sweep()
+        sweeps += 1
+    assert sweeps == 3
+    m, b, o, med = ctx.ooc_result(4096)
+    check_moments(m, oracle.moments(a), a)
+    rb, ro = oracle.histogram(a, 4096, -0.02, 0.5)
+    assert (b == rb).all() and (o == ro).all()
+    assert same_float(med, oracle.median(a))
+    # identical integers to the in-core path on the same voxels
+    mi = ctx.moments(whole, a.size, 1, 1)
+    assert (mi["count"], bits(mi["min"]), bits(mi["max"])) == (m["count"], bits(m["min"]), bits(m["max"]))
+    assert abs(mi["mean"] - m["mean"]) <= REL * abs(m["mean"]) and abs(mi["std"] - m["std"]) <= REL * m["std"]
+    assert same_float(ctx.median(whole, a.size, 1, 1), med)
+    ms = ctx.ooc_result(4096, flags=cube.SAMPLE_STD)[0]
+    check_moments(ms, oracle.moments(a, sample_std=True), a)
+
+
+@pytest.mark.parametrize("resident", [False, True])
+def test_stats_host_matches_oracle(ctx, resident):
+    a = cubegen.generate_numpy(cubegen.scaled("c2", (96, 96, 200), nsrc=5)).reshape(-1)
+    h = torch.from_numpy(a).pin_memory()
+    ctx.host_workspace(resident_bytes=(a.nbytes + 4096) if resident else 0, chunk_bytes=1 << 20)
+    m, b, o, med = ctx.stats_host(h, 96, 96, 200, 4096, -0.02, 0.5)
+    check_moments(m, oracle.moments(a), a)
+    rb, ro = oracle.histogram(a, 4096, -0.02, 0.5)
+    assert (b == rb).all() and (o == ro).all()
+    assert same_float(med, oracle.median(a))
+    ctx.host_workspace(0, 1 << 20)
