@@ -72,7 +72,8 @@ typedef struct {
 } cube_moments_t;
 
 /* Create a context on the CURRENT device. `scratch_bytes_hint` sizes the optional candidate buffer of
- * the select (0 = default, 64 MiB); everything else is fixed size (< 4 MiB). */
+ * the select in bytes (0 = default, 256 MiB = 64 Mi keys); everything else is fixed size (< 4 MiB).
+ * The buffer only saves a pass: when the median's first-digit bucket does not fit, the cube is read a third time. */
 int cube_create(cube_ctx** out, size_t scratch_bytes_hint);
 int cube_destroy(cube_ctx* ctx);
 
@@ -111,7 +112,9 @@ int cube_median_ex(cube_ctx* ctx, const float* d, int64_t nx, int64_t ny, int64_
  * buffer the caller has filled (e.g. by cudaMemcpyAsync from pinned host memory on a side stream).
  * Sweep 1 accumulates moments + histogram + the first select digit; each further sweep (the caller
  * re-presents all bricks) refines the median by one digit.  cube_ooc_next_sweep() tells whether another
- * sweep is needed: *more = 1 until the median is exact (3 sweeps in all, 1 if want_median == 0). */
+ * sweep is needed: *more = 1 until the median is exact: 2 sweeps when the median's first-digit bucket fits the
+ * candidate buffer (the second sweep compacts it), else 3; 1 if want_median == 0.  The call after sweep 2
+ * synchronises `stream` once to read that decision. */
 int cube_ooc_begin(cube_ctx* ctx, int nbins, float lo, float hi, int want_median, cudaStream_t stream);
 int cube_ooc_brick(cube_ctx* ctx, const float* d_brick, uint64_t nvox, cudaStream_t stream);
 int cube_ooc_next_sweep(cube_ctx* ctx, int* more, cudaStream_t stream);
@@ -133,8 +136,31 @@ int cube_last_cuda_error(const cube_ctx* ctx);
 /* Launch-configuration knobs (0 keeps the default): threads per CTA, resident CTAs per SM. For tuning and
  * for the tests that check tiling invariance. */
 int cube_set_launch(cube_ctx* ctx, int ctas_per_sm);
+enum {
+    CUBE_KNOB_CTAS_PER_SM = 0, /* same as cube_set_launch */
+    CUBE_KNOB_BIGHIST = 1      /* histograms with more than 16384 bins: 0 = one CTA per SM with 16-bit packed
+                                  shared-memory counters (default), 1 = clusters of two CTAs holding 32-bit
+                                  counters in distributed shared memory */
+};
+int cube_set_knob(cube_ctx* ctx, int knob, int value);
 /* Number of kernels launched through this context since creation (bench.py's gpu_launches). */
 uint64_t cube_launch_count(const cube_ctx* ctx);
+
+/* ---- Per-kernel timing (what bench.py's roofline reads).  When enabled, every kernel launched through the
+ * context is bracketed by a cudaEvent pair on its own stream (about 2 us of stream time per launch, so keep
+ * it off when timing whole steps).  cube_profile_read() synchronises the device, then returns the summed
+ * duration and the number of launches of one kernel kind since the last cube_profile_reset(). */
+enum {
+    CUBE_K_MOMENTS = 0,     /* moments_kernel (with or without the fused coarse digit histogram) */
+    CUBE_K_HIST = 1,        /* histogram kernels */
+    CUBE_K_SELECT_PASS = 2, /* radix-select digit passes over the cube (or the candidate buffer) */
+    CUBE_K_SELECT_SCAN = 3, /* 1-CTA bucket location kernels */
+    CUBE_K_OTHER = 4,
+    CUBE_K_KINDS = 5
+};
+int cube_profile_enable(cube_ctx* ctx, int on);
+int cube_profile_reset(cube_ctx* ctx);
+int cube_profile_read(cube_ctx* ctx, int kind, double* total_ms, uint64_t* launches);
 
 #ifdef __cplusplus
 }

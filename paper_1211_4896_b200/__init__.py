@@ -26,7 +26,11 @@ MAX_BINS = 65536
 SYMBOLS = ["cube_create", "cube_destroy", "cube_moments", "cube_histogram", "cube_kth", "cube_kth_ex",
            "cube_median", "cube_median_ex", "cube_ooc_begin", "cube_ooc_brick", "cube_ooc_next_sweep",
            "cube_ooc_result", "cube_host_workspace", "cube_stats_host", "cube_strerror",
-           "cube_last_cuda_error", "cube_set_launch", "cube_launch_count"]
+           "cube_last_cuda_error", "cube_set_launch", "cube_set_knob", "cube_launch_count",
+           "cube_profile_enable", "cube_profile_reset", "cube_profile_read"]
+KNOB_CTAS_PER_SM, KNOB_BIGHIST = 0, 1
+K_MOMENTS, K_HIST, K_SELECT_PASS, K_SELECT_SCAN, K_OTHER = 0, 1, 2, 3, 4
+KIND_NAMES = ["moments", "histogram", "select_pass", "select_scan", "other"]
 
 
 class CubeError(RuntimeError):
@@ -77,8 +81,12 @@ def load():
     L.cube_strerror.restype = ctypes.c_char_p
     L.cube_last_cuda_error.argtypes = [vp]
     L.cube_set_launch.argtypes = [vp, ci]
+    L.cube_set_knob.argtypes = [vp, ci, ci]
     L.cube_launch_count.argtypes = [vp]
     L.cube_launch_count.restype = u64
+    L.cube_profile_enable.argtypes = [vp, ci]
+    L.cube_profile_reset.argtypes = [vp]
+    L.cube_profile_read.argtypes = [vp, ci, ctypes.POINTER(ctypes.c_double), ctypes.POINTER(u64)]
     for name in SYMBOLS:
         getattr(L, name)
     _lib = L
@@ -205,6 +213,24 @@ class Context:
     # --- knobs -----------------------------------------------------------------------------------------
     def set_launch(self, ctas_per_sm):
         self._check(self._L.cube_set_launch(self._h, ctas_per_sm))
+
+    def set_knob(self, knob, value):
+        self._check(self._L.cube_set_knob(self._h, knob, value))
+
+    def profile(self, on):
+        self._check(self._L.cube_profile_enable(self._h, int(bool(on))))
+
+    def profile_reset(self):
+        self._check(self._L.cube_profile_reset(self._h))
+
+    def profile_read(self):
+        """-> {kind name: (total_ms, launches)} since the last reset (synchronises the device)."""
+        out = {}
+        for k, name in enumerate(KIND_NAMES):
+            ms, n = ctypes.c_double(), ctypes.c_uint64()
+            self._check(self._L.cube_profile_read(self._h, k, ctypes.byref(ms), ctypes.byref(n)))
+            out[name] = (ms.value, int(n.value))
+        return out
 
     @property
     def launch_count(self):

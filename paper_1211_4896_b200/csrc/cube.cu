@@ -6,6 +6,7 @@
 #include <math.h>
 #include <new>
 #include <string.h>
+#include <vector>
 
 #include "cube_kernels.cuh"
 
@@ -15,6 +16,7 @@ struct cube_ctx {
     int device = 0;
     int num_sms = 0;
     int ctas_per_sm = 0;  // 0 = per-kernel default
+    int bighist = 0;      // CUBE_KNOB_BIGHIST: 0 = 16-bit packed counters, 1 = cluster DSM
     int last_cuda = 0;
     uint64_t launches = 0;
     // device scratch
@@ -27,6 +29,8 @@ struct cube_ctx {
     unsigned long long* gdigits = nullptr; // kDigitBins
     unsigned long long* coarse = nullptr;  // kDigitBins: digit histogram kept by CUBE_COARSE_HIST
     SelectState* sel = nullptr;
+    uint32_t* cand = nullptr;              // candidate keys of the select (step 8)
+    unsigned long long cand_cap = 0;       // in keys
     // out-of-core state (host side)
     int ooc_active = 0, ooc_sweep = 0, ooc_nbins = 0, ooc_want_median = 0, ooc_bricks = 0;
     float ooc_lo = 0.f, ooc_hi = 0.f, ooc_scale = 0.f;
@@ -39,6 +43,13 @@ struct cube_ctx {
     cudaEvent_t ev_copied[2] = {nullptr, nullptr}, ev_consumed[2] = {nullptr, nullptr};
     void* pinned_results = nullptr;  // staging for cube_stats_host results
     int max_ctas = 0;
+    // per-kernel timing (cube_profile_*)
+    int prof_on = 0;
+    std::vector<cudaEvent_t> prof_ev;   // pairs
+    std::vector<int> prof_kind;         // kind of pair i
+    size_t prof_used = 0;               // pairs in use
+    double prof_ms[CUBE_K_KINDS] = {0, 0, 0, 0, 0};
+    uint64_t prof_n[CUBE_K_KINDS] = {0, 0, 0, 0, 0};
 };
 
 namespace {
@@ -54,6 +65,39 @@ constexpr int kSmemHistMaxBins = 16384;  // 64 KiB of 32-bit counters per CTA
             return CUBE_ECUDA;                            \
         }                                                 \
     } while (0)
+
+// Brackets one kernel launch with an event pair when profiling is on.
+struct ProfScope {
+    cube_ctx* c; cudaStream_t s; cudaEvent_t stop = nullptr;
+    ProfScope(cube_ctx* c_, int kind, cudaStream_t s_) : c(c_), s(s_) {
+        c->launches++;
+        if (!c->prof_on) return;
+        if (c->prof_used * 2 + 2 > c->prof_ev.size()) {
+            cudaEvent_t a, b;
+            if (cudaEventCreate(&a) != cudaSuccess || cudaEventCreate(&b) != cudaSuccess) return;
+            c->prof_ev.push_back(a); c->prof_ev.push_back(b); c->prof_kind.push_back(kind);
+        }
+        c->prof_kind[c->prof_used] = kind;
+        cudaEventRecord(c->prof_ev[c->prof_used * 2], s);
+        stop = c->prof_ev[c->prof_used * 2 + 1];
+        c->prof_used++;
+    }
+    ~ProfScope() { if (stop) cudaEventRecord(stop, s); }
+};
+
+int prof_collect(cube_ctx* c) {
+    if (c->prof_used == 0) return CUBE_OK;
+    CUBE_CUDA(c, cudaDeviceSynchronize());
+    for (size_t i = 0; i < c->prof_used; ++i) {
+        float ms = 0.f;
+        if (cudaEventElapsedTime(&ms, c->prof_ev[2 * i], c->prof_ev[2 * i + 1]) == cudaSuccess) {
+            c->prof_ms[c->prof_kind[i]] += ms;
+            c->prof_n[c->prof_kind[i]]++;
+        }
+    }
+    c->prof_used = 0;
+    return CUBE_OK;
+}
 
 inline bool dims_ok(int64_t nx, int64_t ny, int64_t nz, uint64_t* n) {
     if (nx <= 0 || ny <= 0 || nz <= 0) return false;
@@ -84,16 +128,21 @@ inline bool hist_scale(int nbins, float lo, float hi, float* scale) {
 
 int launch_moments(cube_ctx* c, const float* d, uint64_t n, unsigned flags, int accumulate, cudaStream_t s) {
     const bool coarse = (flags & CUBE_COARSE_HIST) != 0;
-    const int grid = grid_for(c, coarse ? 3 : 4, kMaxCtasPerSm);
+    int occ_m = 0;
+    if ((coarse ? cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ_m, moments_kernel<true>, kThreads, 0)
+                : cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ_m, moments_kernel<false>, kThreads, 0)) != cudaSuccess) occ_m = 1;
+    const int grid = grid_for(c, 4, occ_m < kMaxCtasPerSm ? occ_m : kMaxCtasPerSm);
+    if (coarse && !accumulate) CUBE_CUDA(c, cudaMemsetAsync(c->coarse, 0, kDigitBins * sizeof(unsigned long long), s));
+    {
+    ProfScope prof(c, CUBE_K_MOMENTS, s);
     if (coarse) {
-        if (!accumulate) CUBE_CUDA(c, cudaMemsetAsync(c->coarse, 0, kDigitBins * sizeof(unsigned long long), s));
         moments_kernel<true><<<grid, kThreads, 0, s>>>(d, n, c->partials, c->ticket, c->acc, c->nvox_acc,
                                                        accumulate, flags, c->mom_out, c->coarse);
     } else {
         moments_kernel<false><<<grid, kThreads, 0, s>>>(d, n, c->partials, c->ticket, c->acc, c->nvox_acc,
                                                         accumulate, flags, c->mom_out, c->coarse);
     }
-    c->launches++;
+    }
     CUBE_CUDA(c, cudaGetLastError());
     return CUBE_OK;
 }
@@ -101,25 +150,39 @@ int launch_moments(cube_ctx* c, const float* d, uint64_t n, unsigned flags, int 
 int launch_hist(cube_ctx* c, const float* d, uint64_t n, int nbins, float lo, float hi, float scale,
                 cudaStream_t s) {
     unsigned long long* outside = c->gbins + CUBE_MAX_BINS;
+    {
+    ProfScope prof(c, CUBE_K_HIST, s);
     if (nbins <= kSmemHistMaxBins) {
-        const size_t smem = (size_t)nbins * sizeof(uint32_t);
-        int occ = (int)((200 * 1024) / (smem + 1024));
-        const int grid = grid_for(c, 4, occ < kMaxCtasPerSm ? occ : kMaxCtasPerSm);
+        const size_t smem = (size_t)(nbins + 1) * sizeof(uint32_t);  // + trash counter
+        int occ = 0;
+        if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, hist_smem_kernel, kThreads, smem) != cudaSuccess)
+            occ = 1;
+        const int grid = grid_for(c, 4, occ);
         hist_smem_kernel<<<grid, kThreads, smem, s>>>(d, n, nbins, lo, hi, scale, c->gbins, outside);
     } else {
-        const int grid = grid_for(c, 4, kMaxCtasPerSm);
-        hist_global_kernel<<<grid, kThreads, 0, s>>>(d, n, nbins, lo, hi, scale, c->gbins, outside);
+        // one CTA of 1024 threads per SM, 16-bit packed counters (128 KiB for 65536 bins)
+        const size_t smem = (size_t)((nbins + 1) / 2) * sizeof(uint32_t);
+        if (c->bighist == 1) {
+            hist_dsm_kernel<<<c->num_sms & ~1, kBigThreads, (32768 + 1) * sizeof(uint32_t), s>>>(
+                d, n, nbins, lo, hi, scale, c->gbins, outside);
+        } else {
+            hist_packed_kernel<<<c->num_sms, kBigThreads, smem, s>>>(d, n, nbins, lo, hi, scale, c->gbins, outside);
+        }
     }
-    c->launches++;
+    }
     CUBE_CUDA(c, cudaGetLastError());
     return CUBE_OK;
 }
 
 template <int PASS>
 int launch_select_pass(cube_ctx* c, const float* d, uint64_t n, cudaStream_t s) {
-    const int grid = grid_for(c, 4, kMaxCtasPerSm);
-    select_pass_kernel<PASS><<<grid, kThreads, 0, s>>>(d, n, c->sel, c->gdigits);
-    c->launches++;
+    int occ = 0;  // every CTA of the persistent grid must be resident (static tile dealing)
+    if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, select_pass_kernel<PASS>, kThreads, 0) != cudaSuccess) occ = 1;
+    const int grid = grid_for(c, 4, occ < kMaxCtasPerSm ? occ : kMaxCtasPerSm);
+    {
+        ProfScope prof(c, CUBE_K_SELECT_PASS, s);
+        select_pass_kernel<PASS><<<grid, kThreads, 0, s>>>(d, n, c->sel, c->gdigits, c->cand);
+    }
     CUBE_CUDA(c, cudaGetLastError());
     return CUBE_OK;
 }
@@ -127,8 +190,10 @@ int launch_select_pass(cube_ctx* c, const float* d, uint64_t n, cudaStream_t s) 
 template <int PASS>
 int launch_select_scan(cube_ctx* c, unsigned long long* digits, cudaStream_t s) {
     // the coarse histogram kept by CUBE_COARSE_HIST is left intact so that several k can reuse it
-    select_scan_kernel<PASS><<<1, 1024, 0, s>>>(c->sel, digits, digits == c->gdigits ? 1 : 0);
-    c->launches++;
+    {
+        ProfScope prof(c, CUBE_K_SELECT_SCAN, s);
+        select_scan_kernel<PASS><<<1, 1024, 0, s>>>(c->sel, digits, digits == c->gdigits ? 1 : 0);
+    }
     CUBE_CUDA(c, cudaGetLastError());
     return CUBE_OK;
 }
@@ -139,6 +204,8 @@ int select_init(cube_ctx* c, uint64_t k, int use_median, cudaStream_t s) {
     h.k = k;
     h.use_median = use_median ? 1u : 0u;
     h.result = nanf("");
+    h.cand_n = 0;
+    h.cand_cap = c->cand ? c->cand_cap : 0;
     // small H2D of a stack struct: cudaMemcpyAsync from pageable memory stages the bytes before returning
     CUBE_CUDA(c, cudaMemcpyAsync(c->sel, &h, sizeof(h), cudaMemcpyHostToDevice, s));
     return CUBE_OK;
@@ -168,7 +235,6 @@ int kth_impl(cube_ctx* c, const float* d, uint64_t n, uint64_t k, int use_median
 extern "C" {
 
 int cube_create(cube_ctx** out, size_t scratch_bytes_hint) {
-    (void)scratch_bytes_hint;
     if (!out) return CUBE_EINVAL;
     *out = nullptr;
     cube_ctx* c = new (std::nothrow) cube_ctx();
@@ -194,8 +260,16 @@ int cube_create(cube_ctx** out, size_t scratch_bytes_hint) {
     ok = ok && cudaMemset(c->gdigits, 0, kDigitBins * sizeof(unsigned long long)) == cudaSuccess;
     ok = ok && cudaMemset(c->coarse, 0, kDigitBins * sizeof(unsigned long long)) == cudaSuccess;
     ok = ok && cudaFuncSetAttribute(hist_smem_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                                    kSmemHistMaxBins * (int)sizeof(uint32_t)) == cudaSuccess;
+                                    (kSmemHistMaxBins + 1) * (int)sizeof(uint32_t)) == cudaSuccess;
+    ok = ok && cudaFuncSetAttribute(hist_packed_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                    (CUBE_MAX_BINS / 2) * (int)sizeof(uint32_t)) == cudaSuccess;
+    ok = ok && cudaFuncSetAttribute(hist_dsm_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                    (32768 + 1) * (int)sizeof(uint32_t)) == cudaSuccess;
     if (!ok) { cube_destroy(c); return CUBE_ENOMEM; }
+    // candidate buffer of the select: optional (without it pass 2 streams the cube a third time)
+    const size_t cand_bytes = scratch_bytes_hint ? scratch_bytes_hint : ((size_t)256 << 20);
+    if (cudaMalloc(&c->cand, cand_bytes) == cudaSuccess) c->cand_cap = cand_bytes / sizeof(uint32_t);
+    else { cudaGetLastError(); c->cand = nullptr; c->cand_cap = 0; }
     *out = c;
     return CUBE_OK;
 }
@@ -204,12 +278,14 @@ int cube_destroy(cube_ctx* c) {
     if (!c) return CUBE_EINVAL;
     cudaFree(c->partials); cudaFree(c->ticket); cudaFree(c->acc); cudaFree(c->nvox_acc);
     cudaFree(c->mom_out); cudaFree(c->gbins); cudaFree(c->gdigits); cudaFree(c->coarse); cudaFree(c->sel);
+    cudaFree(c->cand);
     cudaFree(c->resident); cudaFree(c->chunk[0]); cudaFree(c->chunk[1]);
     if (c->pinned_results) cudaFreeHost(c->pinned_results);
     for (int i = 0; i < 2; ++i) {
         if (c->ev_copied[i]) cudaEventDestroy(c->ev_copied[i]);
         if (c->ev_consumed[i]) cudaEventDestroy(c->ev_consumed[i]);
     }
+    for (cudaEvent_t e : c->prof_ev) cudaEventDestroy(e);
     if (c->copy_stream) cudaStreamDestroy(c->copy_stream);
     if (c->work_stream) cudaStreamDestroy(c->work_stream);
     delete c;
@@ -285,7 +361,41 @@ int cube_set_launch(cube_ctx* c, int ctas_per_sm) {
     return CUBE_OK;
 }
 
+int cube_set_knob(cube_ctx* c, int knob, int value) {
+    if (!c) return CUBE_EINVAL;
+    switch (knob) {
+        case CUBE_KNOB_CTAS_PER_SM: return cube_set_launch(c, value);
+        case CUBE_KNOB_BIGHIST:
+            if (value != 0 && value != 1) return CUBE_EINVAL;
+            c->bighist = value;
+            return CUBE_OK;
+        default: return CUBE_EINVAL;
+    }
+}
+
 uint64_t cube_launch_count(const cube_ctx* c) { return c ? c->launches : 0; }
+
+int cube_profile_enable(cube_ctx* c, int on) {
+    if (!c) return CUBE_EINVAL;
+    if (!on) { int rc = prof_collect(c); if (rc) return rc; }
+    c->prof_on = on ? 1 : 0;
+    return CUBE_OK;
+}
+
+int cube_profile_reset(cube_ctx* c) {
+    if (!c) return CUBE_EINVAL;
+    int rc = prof_collect(c);
+    for (int k = 0; k < CUBE_K_KINDS; ++k) { c->prof_ms[k] = 0.0; c->prof_n[k] = 0; }
+    return rc;
+}
+
+int cube_profile_read(cube_ctx* c, int kind, double* total_ms, uint64_t* launches) {
+    if (!c || kind < 0 || kind >= CUBE_K_KINDS || !total_ms || !launches) return CUBE_EINVAL;
+    int rc = prof_collect(c);
+    *total_ms = c->prof_ms[kind];
+    *launches = c->prof_n[kind];
+    return rc;
+}
 
 }  // extern "C"
 

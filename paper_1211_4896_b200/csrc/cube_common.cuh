@@ -13,7 +13,6 @@ namespace cube {
 
 constexpr int kThreads = 256;  // threads per CTA (8 warps)
 constexpr int kUnroll = 8;     // independent 128-bit loads in flight per thread per tile
-constexpr int kTileVec = kThreads * kUnroll;  // float4 per tile (32 KiB)
 
 // 128-bit read-only load that does not allocate in L1 (each voxel is used once per pass).  L2 policy is
 // left at the default so that cubes smaller than the 126 MB L2 (config 1) are re-read from L2 by the
@@ -36,13 +35,15 @@ __host__ __device__ __forceinline__ uint32_t bits_of_key(uint32_t k) {
     return (k & 0x80000000u) ? (k ^ 0x80000000u) : ~k;
 }
 
-// Visit all n voxels of d exactly once across the grid.  F provides `void operator()(float)`.
-// Tiles of kTileVec float4 are dealt round-robin to the CTAs, so concurrently running CTAs read adjacent
-// 32 KiB tiles (DRAM page locality) and the assignment is static => per-CTA results are deterministic.
+// Visit all n voxels of d exactly once across the grid.  F provides `void operator()(float)` for single
+// voxels and `void batch(const float4 (&)[kUnroll])` for a thread's share of a full tile.
+// Tiles of THREADS*kUnroll float4 are dealt round-robin to the CTAs, so concurrently running CTAs read
+// adjacent tiles (DRAM page locality) and the assignment is static => per-CTA results are deterministic.
 // The <= 3 voxels before the first 16-byte boundary and the <= 3 after the last full float4 are visited
 // by CTA 0.
-template <class F>
+template <int THREADS, class F>
 __device__ __forceinline__ void stream_cube(const float* __restrict__ d, uint64_t n, F& f) {
+    constexpr int TILE = THREADS * kUnroll;
     uint64_t head = ((16u - (uint32_t)((uintptr_t)d & 15u)) & 15u) >> 2;
     if (head > n) head = n;
     const float4* __restrict__ v = reinterpret_cast<const float4*>(d + head);
@@ -55,21 +56,19 @@ __device__ __forceinline__ void stream_cube(const float* __restrict__ d, uint64_
             if (t < n) f(d[t]);
         }
     }
-    const uint64_t ntiles = (nvec + kTileVec - 1) / kTileVec;
+    const uint64_t ntiles = (nvec + TILE - 1) / TILE;
     for (uint64_t t = blockIdx.x; t < ntiles; t += gridDim.x) {
-        const uint64_t base = t * kTileVec + threadIdx.x;
-        if (base + (uint64_t)(kUnroll - 1) * kThreads < nvec) {
+        const uint64_t base = t * TILE + threadIdx.x;
+        if ((t + 1) * TILE <= nvec) {  // whole tile in range: CTA-uniform, so batch() may use warp collectives
             float4 r[kUnroll];
 #pragma unroll
-            for (int j = 0; j < kUnroll; ++j) r[j] = ld_stream(v + base + (uint64_t)j * kThreads);
-#pragma unroll
-            for (int j = 0; j < kUnroll; ++j) {
-                f(r[j].x); f(r[j].y); f(r[j].z); f(r[j].w);
-            }
+            for (int j = 0; j < kUnroll; ++j) r[j] = ld_stream(v + base + (uint64_t)j * THREADS);
+            asm volatile("" ::: "memory");  // all kUnroll loads are issued before the first counter update
+            f.batch(r);
         } else {
 #pragma unroll 1
             for (int j = 0; j < kUnroll; ++j) {
-                uint64_t i = base + (uint64_t)j * kThreads;
+                uint64_t i = base + (uint64_t)j * THREADS;
                 if (i < nvec) {
                     float4 r = ld_stream(v + i);
                     f(r.x); f(r.y); f(r.z); f(r.w);
@@ -77,6 +76,33 @@ __device__ __forceinline__ void stream_cube(const float* __restrict__ d, uint64_
             }
         }
     }
+}
+
+// Default batch: the single-voxel functor applied to the 4*kUnroll values.
+#define CUBE_DEFAULT_BATCH()                                                        \
+    __device__ __forceinline__ void batch(const float4 (&r)[kUnroll]) {             \
+        _Pragma("unroll") for (int j = 0; j < kUnroll; ++j) {                       \
+            (*this)(r[j].x); (*this)(r[j].y); (*this)(r[j].z); (*this)(r[j].w);     \
+        }                                                                           \
+    }
+
+// 32-bit shared-window address of a shared-memory pointer (what ATOMS/RED take), computed once per kernel
+// instead of once per voxel.
+__device__ __forceinline__ uint32_t smem_addr(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
+
+// Predicated shared-memory increment: counter at byte address `saddr` += 1 when `p`.  Written in PTX so
+// that the compiler keeps it a predicated RED (SASS ATOMS.POPC.INC, which the hardware aggregates over
+// lanes hitting the same address) instead of a divergent branch around it.
+__device__ __forceinline__ void smem_inc_if(uint32_t saddr, bool p) {
+    asm volatile("{\n\t.reg .pred q;\n\tsetp.ne.u32 q, %1, 0;\n\t@q red.shared.add.u32 [%0], 1;\n\t}"
+                 :: "r"(saddr), "r"((uint32_t)p) : "memory");
+}
+
+// Same static tiling over an array of 32-bit keys (the select's candidate buffer, 16-byte aligned).
+template <int THREADS, class F>
+__device__ __forceinline__ void stream_keys(const uint32_t* __restrict__ k, uint64_t n, F& f) {
+    for (uint64_t i = (uint64_t)blockIdx.x * THREADS + threadIdx.x; i < n; i += (uint64_t)gridDim.x * THREADS)
+        f.key(__ldg(k + i));
 }
 
 // ---------------------------------------------------------------- (n, mean, M2, min, max) partials

@@ -1,5 +1,12 @@
 // cube_kernels.cuh -- the sm_100a kernels of libcube.  See DESIGN.md sec. 4 for the roofline of each.
+//
+// All of them are HBM-read-bound scans (4 B per voxel per pass, no dense contraction => no tensor cores).
+// At the measured ~7.3 TB/s read ceiling an SM must retire ~6 voxels per clock, i.e. the per-voxel budget
+// is ~21 issue slots, ~10 of them on the half-rate ALU pipe -- so the functors below are written to be
+// branch-free and light on integer/compare instructions (ncu: profiles/r1_*.md).
 #pragma once
+#include <math.h>
+
 #include "cube_common.cuh"
 
 namespace cube {
@@ -21,9 +28,8 @@ struct SelectState {
     uint32_t invalid;           // 1 when k >= count (result NaN)
     uint32_t use_median;        // 1: k = (count-1)/2 is set by the pass-0 scan
     float result;
-    unsigned long long cand_n;  // candidates written by the compacting pass
-    uint32_t cand_ok;           // 1 when all candidates fitted into the buffer
-    uint32_t pad;
+    unsigned long long cand_n;  // keys of the pass-0 bucket seen by the compacting pass 1
+    unsigned long long cand_cap;  // capacity of the candidate buffer, in keys
 };
 
 constexpr int kDigitBins = 2048;  // 11-bit digits (passes 0, 1); pass 2 uses the low 10 bits
@@ -32,32 +38,48 @@ constexpr int kDigitBins = 2048;  // 11-bit digits (passes 0, 1); pass 2 uses th
 // Moments: steps 1-3 of SURVEY.md sec. 8(a) (+ 3b when COARSE): count, min, max, pivoted fp64 sums.
 // PAPER.md:265 "local summation and summation of squares and count of the non-null data values".
 // The paper's float32-per-slice partial sums are replaced by per-thread fp64
-// accumulators about a per-thread pivot (R17).
+// accumulators about a per-thread pivot (R17): d = x - pivot is exact in fp64, so a constant
+// cube gives std == 0 exactly and sum(d^2) - sum(d)^2/n does not cancel catastrophically.
+// Per voxel: FSETP, FSEL, 2 FMNMX (alu pipe), F2F (xu), 2 DADD + DFMA (fp64), 1 predicated IADD.
+// min/max use FMNMX, which ignores NaN operands and orders -0.0 < +0.0.
 // ------------------------------------------------------------------------------------------------
 template <bool COARSE>
 struct MomentsF {
-    uint32_t n = 0, kmin = 0xFFFFFFFFu, kmax = 0u;
+    float mn = INFINITY, mx = -INFINITY;
+    float pivf = 0.0f;
     bool have = false;
+    uint32_t n = 0;
     double pivot = 0.0, s = 0.0, q = 0.0;
     uint32_t* sbins;  // COARSE: kDigitBins shared counters
-    __device__ __forceinline__ void operator()(float x) {
+    __device__ __forceinline__ void core(float x) {
         const bool ok = (x == x);  // NaN == blanked voxel
-        const uint32_t key = key_of(x);
-        kmin = min(kmin, ok ? key : 0xFFFFFFFFu);
-        kmax = max(kmax, ok ? key : 0u);
-        if (!have) { have = ok; pivot = ok ? (double)x : 0.0; }
-        const double dlt = ok ? (double)x - pivot : 0.0;
+        mn = fminf(mn, x);
+        mx = fmaxf(mx, x);
+        const float xs = ok ? x : pivf;  // a blanked voxel contributes d == 0
+        const double dlt = (double)xs - pivot;
         s += dlt;
         q = fma(dlt, dlt, q);
         n += ok ? 1u : 0u;
-        if (COARSE) { if (ok) atomicAdd(&sbins[key >> 21], 1u); }
+        if (COARSE) atomicAdd(&sbins[ok ? (key_of(x) >> 21) : kDigitBins], 1u);  // NaN -> trash counter
+    }
+    __device__ __forceinline__ void take_pivot(float x) {
+        if (!have && x == x) { have = true; pivf = x; pivot = (double)x; }
+    }
+    __device__ __forceinline__ void operator()(float x) { take_pivot(x); core(x); }
+    __device__ __forceinline__ void batch(const float4 (&r)[kUnroll]) {
+        if (!have) {  // only until this thread has met its first non-NaN voxel
+#pragma unroll
+            for (int j = 0; j < kUnroll; ++j) { take_pivot(r[j].x); take_pivot(r[j].y); take_pivot(r[j].z); take_pivot(r[j].w); }
+        }
+#pragma unroll
+        for (int j = 0; j < kUnroll; ++j) { core(r[j].x); core(r[j].y); core(r[j].z); core(r[j].w); }
     }
     __device__ __forceinline__ Partial partial() const {
         Partial p = partial_empty();
         if (n) {
             const double nn = (double)n, ms = s / nn;
             p.n = n; p.mean = pivot + ms; p.m2 = fmax(q - s * ms, 0.0);
-            p.kmin = kmin; p.kmax = kmax;
+            p.kmin = key_of(mn); p.kmax = key_of(mx);
         }
         return p;
     }
@@ -91,15 +113,15 @@ moments_kernel(const float* __restrict__ d, uint64_t n, Partial* __restrict__ pa
                unsigned long long* __restrict__ nvox_acc, int accumulate, unsigned flags,
                MomentsOut* __restrict__ out, unsigned long long* __restrict__ gdigits) {
     __shared__ Partial scratch[kThreads / 32];
-    __shared__ uint32_t sbins[COARSE ? kDigitBins : 1];
+    __shared__ uint32_t sbins[COARSE ? kDigitBins + 1 : 1];
     __shared__ bool is_last;
     MomentsF<COARSE> f;
     f.sbins = sbins;
     if (COARSE) {
-        for (int i = threadIdx.x; i < kDigitBins; i += kThreads) sbins[i] = 0;
+        for (int i = threadIdx.x; i <= kDigitBins; i += kThreads) sbins[i] = 0;
         __syncthreads();
     }
-    stream_cube(d, n, f);
+    stream_cube<kThreads>(d, n, f);
     Partial p = partial_block_reduce(f.partial(), scratch);
     if (COARSE) {
         __syncthreads();
@@ -145,192 +167,219 @@ __global__ void moments_refinalize_kernel(const Partial* __restrict__ acc, const
 
 // ------------------------------------------------------------------------------------------------
 // Histogram: steps 4-5.  PAPER.md:259-261; bin formula DESIGN.md R10-R13 (float32, no contraction).
-// Shared-memory privatised 32-bit counters per CTA, merged into the 64-bit global bins by atomics
+// Shared-memory privatised counters per CTA, merged into the 64-bit global bins by atomics
 // ("summation ... associative and commutative, any arbitrary data composition order is valid").
+// The shared-memory increment compiles to ATOMS.POPC.INC, which the hardware aggregates over lanes that
+// hit the same address -- hot bins (config 4: 30 % of the voxels in one bin) cost no serialisation.
 // ------------------------------------------------------------------------------------------------
-struct HistF {
+struct HistBase {
     float lo, hi, scale;
     int top;  // nbins-1
-    uint32_t* sbins;
     uint32_t below = 0, above = 0;
+    // bin of an in-range voxel; garbage (never used) otherwise
+    __device__ __forceinline__ int bin_of(float x) const {
+        const float v = __fmul_rn(__fsub_rn(x, lo), scale);
+        return min(__float2int_rd(v), top);  // floor (v >= 0), closed top bin (R11)
+    }
+    __device__ __forceinline__ void outside(float x) {  // rare path: NaN, x < lo, x > hi
+        below += (x < lo) ? 1u : 0u;
+        above += (x > hi) ? 1u : 0u;
+    }
+};
+
+// Per voxel, 9 instructions and no branch: 2 FSETP (range test on x itself, false for NaN), FADD, FMUL
+// (__fsub_rn / __fmul_rn: never contracted), F2I.FLOOR, VIMNMX (closed top bin), SEL, LEA,
+// ATOMS.POPC.INC.  The increment is unconditional: voxels that are NaN or outside [lo,hi] go to a trash
+// counter at index nbins (ptxas turns a predicated RED into a branch around the whole bin computation,
+// which costs more than the SEL).  Voxels outside [lo,hi] are rare on every config, so below/above are
+// found per batch from the batch min/max (FMNMX3, NaN-blind: NaN voxels are counted nowhere) and
+// counted in a cold path.
+struct HistF : HistBase {
+    uint32_t* sbins;  // nbins + 1 counters, the last one is the trash counter
+    __device__ __forceinline__ void inc(float x) const {
+        const bool in = (x >= lo) && (x <= hi);
+        const int b = in ? bin_of(x) : top + 1;
+        atomicAdd(&sbins[b], 1u);
+    }
     __device__ __forceinline__ void operator()(float x) {
-        if (x >= lo && x <= hi) {  // false for NaN
-            const float v = __fmul_rn(__fsub_rn(x, lo), scale);
-            int b = __float2int_rd(v);  // floor; v >= 0
-            b = min(b, top);            // closed top bin (R11)
-            atomicAdd(&sbins[b], 1u);
-        } else {
-            below += (x < lo) ? 1u : 0u;
-            above += (x > hi) ? 1u : 0u;
+        inc(x);
+        outside(x);
+    }
+    __device__ __forceinline__ void batch(const float4 (&r)[kUnroll]) {
+        float bmin = INFINITY, bmax = -INFINITY;
+#pragma unroll
+        for (int j = 0; j < kUnroll; ++j) {
+            inc(r[j].x); inc(r[j].y); inc(r[j].z); inc(r[j].w);
+            bmin = fminf(fminf(bmin, r[j].x), fminf(r[j].y, fminf(r[j].z, r[j].w)));
+            bmax = fmaxf(fmaxf(bmax, r[j].x), fmaxf(r[j].y, fmaxf(r[j].z, r[j].w)));
+        }
+        if (bmin < lo || bmax > hi) {
+#pragma unroll
+            for (int j = 0; j < kUnroll; ++j) { outside(r[j].x); outside(r[j].y); outside(r[j].z); outside(r[j].w); }
         }
     }
 };
 
+template <class F>
+__device__ __forceinline__ void hist_flush_outside(F& f, uint32_t* s_out, unsigned long long* goutside) {
+    if (f.below) atomicAdd(&s_out[0], f.below);
+    if (f.above) atomicAdd(&s_out[1], f.above);
+    __syncthreads();
+    if (threadIdx.x < 2 && s_out[threadIdx.x]) atomicAdd(&goutside[threadIdx.x], (unsigned long long)s_out[threadIdx.x]);
+}
+
+// nbins <= 16384: 32-bit counters, several CTAs per SM.
 __global__ void __launch_bounds__(kThreads)
 hist_smem_kernel(const float* __restrict__ d, uint64_t n, int nbins, float lo, float hi, float scale,
                  unsigned long long* __restrict__ gbins, unsigned long long* __restrict__ goutside) {
     extern __shared__ uint32_t dyn_bins[];
     __shared__ uint32_t s_out[2];
-    for (int i = threadIdx.x; i < nbins; i += kThreads) dyn_bins[i] = 0;
+    for (int i = threadIdx.x; i <= nbins; i += kThreads) dyn_bins[i] = 0;  // + trash counter
     if (threadIdx.x < 2) s_out[threadIdx.x] = 0;
     __syncthreads();
     HistF f;
     f.lo = lo; f.hi = hi; f.scale = scale; f.top = nbins - 1; f.sbins = dyn_bins;
-    stream_cube(d, n, f);
-    if (f.below) atomicAdd(&s_out[0], f.below);
-    if (f.above) atomicAdd(&s_out[1], f.above);
+    stream_cube<kThreads>(d, n, f);
     __syncthreads();
     for (int i = threadIdx.x; i < nbins; i += kThreads) {
         uint32_t c = dyn_bins[i];
         if (c) atomicAdd(&gbins[i], (unsigned long long)c);
     }
-    if (threadIdx.x < 2 && s_out[threadIdx.x]) atomicAdd(&goutside[threadIdx.x], (unsigned long long)s_out[threadIdx.x]);
+    hist_flush_outside(f, s_out, goutside);
 }
 
-// Large-nbins variant: counters do not fit one CTA's shared memory as 32-bit words; v1 counts straight
-// into the global 64-bit bins (L2 atomics).
-struct HistGlobalF {
-    float lo, hi, scale;
-    int top;
+// 16384 < nbins <= 65536: the counters of one CTA no longer fit shared memory as 32-bit words
+// (65536 * 4 B = 256 KiB > 227 KiB), so two 16-bit counters are packed per word (128 KiB, one CTA of
+// 1024 threads per SM) and every wrap of a 16-bit half is moved to the 64-bit global bin at once:
+//   even bin b (low half):  old = atomicAdd(w, 1);  low half wrapped iff (old & 0xFFFF) == 0xFFFF. The
+//       wrap carried +1 into the high half, so credit bins[b] += 65536, take the carry back with
+//       atomicSub(w, 0x10000), and treat both +-1 on the high half like any other change of it;
+//   odd bin b (high half):  old = atomicAdd(w, 0x10000);  wrapped iff (old >> 16) == 0xFFFF.
+// The high half is a mod-65536 counter whose every wrap up (credit +65536) and wrap down (debit -65536)
+// is observed by the atomic that caused it, so count = half + 65536 * (credits - debits) exactly,
+// whatever the interleaving; the global add is 64-bit two's complement.
+constexpr int kBigThreads = 1024;
+struct HistPackedF : HistBase {
+    uint32_t* sw;
     unsigned long long* gbins;
-    uint32_t below = 0, above = 0;
+    // rare: the increment just applied to bin b wrapped its 16-bit half (old = word before the add)
+    __device__ __noinline__ void wrapped(int b, uint32_t old, uint32_t* w) {
+        atomicAdd(&gbins[b], 65536ull);
+        if (!(b & 1)) {
+            if (old == 0xFFFFFFFFu) atomicAdd(&gbins[b + 1], 65536ull);   // the carry wrapped the high half too
+            const uint32_t old2 = atomicSub(w, 0x10000u);                 // take the carry back
+            if (old2 < 0x10000u) atomicAdd(&gbins[b + 1], (unsigned long long)(-65536ll));  // ...wrapping it down
+        }
+    }
+    __device__ __forceinline__ void inc(float x) {
+        const bool in = (x >= lo) && (x <= hi);
+        const int b = bin_of(x);
+        const uint32_t sh = ((uint32_t)b & 1u) << 4;
+        uint32_t* w = &sw[in ? (b >> 1) : 0];
+        const uint32_t old = atomicAdd(w, in ? (1u << sh) : 0u);   // voxels out of range add 0 to word 0
+        if (in && ((old >> sh) & 0xFFFFu) == 0xFFFFu) wrapped(b, old, w);
+    }
     __device__ __forceinline__ void operator()(float x) {
-        if (x >= lo && x <= hi) {
-            const float v = __fmul_rn(__fsub_rn(x, lo), scale);
-            int b = min(__float2int_rd(v), top);
-            atomicAdd(&gbins[b], 1ull);
-        } else {
-            below += (x < lo) ? 1u : 0u;
-            above += (x > hi) ? 1u : 0u;
+        inc(x);
+        outside(x);
+    }
+    __device__ __forceinline__ void batch(const float4 (&r)[kUnroll]) {
+        float bmin = INFINITY, bmax = -INFINITY;
+#pragma unroll
+        for (int j = 0; j < kUnroll; ++j) {
+            inc(r[j].x); inc(r[j].y); inc(r[j].z); inc(r[j].w);
+            bmin = fminf(fminf(bmin, r[j].x), fminf(r[j].y, fminf(r[j].z, r[j].w)));
+            bmax = fmaxf(fmaxf(bmax, r[j].x), fmaxf(r[j].y, fmaxf(r[j].z, r[j].w)));
+        }
+        if (bmin < lo || bmax > hi) {
+#pragma unroll
+            for (int j = 0; j < kUnroll; ++j) { outside(r[j].x); outside(r[j].y); outside(r[j].z); outside(r[j].w); }
         }
     }
 };
 
-__global__ void __launch_bounds__(kThreads)
-hist_global_kernel(const float* __restrict__ d, uint64_t n, int nbins, float lo, float hi, float scale,
+__global__ void __launch_bounds__(kBigThreads)
+hist_packed_kernel(const float* __restrict__ d, uint64_t n, int nbins, float lo, float hi, float scale,
                    unsigned long long* __restrict__ gbins, unsigned long long* __restrict__ goutside) {
+    extern __shared__ uint32_t dyn_bins[];  // (nbins+1)/2 words
     __shared__ uint32_t s_out[2];
+    const int nwords = (nbins + 1) >> 1;
+    for (int i = threadIdx.x; i < nwords; i += kBigThreads) dyn_bins[i] = 0;
     if (threadIdx.x < 2) s_out[threadIdx.x] = 0;
     __syncthreads();
-    HistGlobalF f;
-    f.lo = lo; f.hi = hi; f.scale = scale; f.top = nbins - 1; f.gbins = gbins;
-    stream_cube(d, n, f);
-    if (f.below) atomicAdd(&s_out[0], f.below);
-    if (f.above) atomicAdd(&s_out[1], f.above);
+    HistPackedF f;
+    f.lo = lo; f.hi = hi; f.scale = scale; f.top = nbins - 1; f.sw = dyn_bins; f.gbins = gbins;
+    stream_cube<kBigThreads>(d, n, f);
     __syncthreads();
-    if (threadIdx.x < 2 && s_out[threadIdx.x]) atomicAdd(&goutside[threadIdx.x], (unsigned long long)s_out[threadIdx.x]);
+    for (int i = threadIdx.x; i < nwords; i += kBigThreads) {
+        const uint32_t w = dyn_bins[i];
+        if (w & 0xFFFFu) atomicAdd(&gbins[2 * i], (unsigned long long)(w & 0xFFFFu));
+        if (w >> 16) atomicAdd(&gbins[2 * i + 1], (unsigned long long)(w >> 16));
+    }
+    hist_flush_outside(f, s_out, goutside);
 }
 
-// ------------------------------------------------------------------------------------------------
-// Exact k-th value: steps 6-8.  The paper's Torben bisection (Alg. 1) counts voxels
-// below/above/equal to a guess, ~31 passes; here each pass counts 2048 (1024) sub-ranges at once on the
-// order-preserving key, so three passes fix all 32 bits.  PASS 0: digit = key>>21 (all voxels);
-// PASS 1: voxels with key>>21 == prefix, digit = (key>>10)&2047; PASS 2: key>>10 == prefix,
-// digit = key&1023.
-// ------------------------------------------------------------------------------------------------
-template <int PASS>
-struct SelectF {
-    uint32_t prefix;
-    uint32_t* sbins;
+// Alternative for 16384 < nbins <= 65536 (north_star (2)): a thread-block cluster of two CTAs on two SMs
+// holds the whole histogram as 32-bit counters in DISTRIBUTED shared memory -- bin b lives in CTA (b & 1)
+// of the pair at index b >> 1 (interleaved, so a narrow hot range loads both SMs equally) -- and every
+// voxel does one red.shared::cluster.add to the owner.  Half of the increments cross the SM-to-SM
+// network.  Selected with cube_set_knob(CUBE_KNOB_BIGHIST, 1); DESIGN.md sec. 4 records which variant
+// is faster on B200 and why.
+struct HistDsmF : HistBase {
+    uint32_t base_local;  // shared::cta address of this CTA's counters
+    __device__ __forceinline__ void inc(float x) const {
+        const bool in = (x >= lo) && (x <= hi);
+        const int b = in ? bin_of(x) : 2 * 32768;            // trash: index 32768 of CTA 0
+        const uint32_t local = base_local + (((uint32_t)b >> 1) << 2);
+        uint32_t remote;
+        asm volatile("mapa.shared::cluster.u32 %0, %1, %2;" : "=r"(remote) : "r"(local), "r"((uint32_t)b & 1u));
+        asm volatile("red.relaxed.cluster.shared::cluster.add.u32 [%0], 1;" :: "r"(remote) : "memory");
+    }
     __device__ __forceinline__ void operator()(float x) {
-        const uint32_t key = key_of(x);
-        if (PASS == 0) {
-            if (x == x) atomicAdd(&sbins[key >> 21], 1u);
-        } else if (PASS == 1) {
-            if (x == x && (key >> 21) == prefix) atomicAdd(&sbins[(key >> 10) & 2047u], 1u);
-        } else {
-            if (x == x && (key >> 10) == prefix) atomicAdd(&sbins[key & 1023u], 1u);
+        inc(x);
+        outside(x);
+    }
+    __device__ __forceinline__ void batch(const float4 (&r)[kUnroll]) {
+        float bmin = INFINITY, bmax = -INFINITY;
+#pragma unroll
+        for (int j = 0; j < kUnroll; ++j) {
+            inc(r[j].x); inc(r[j].y); inc(r[j].z); inc(r[j].w);
+            bmin = fminf(fminf(bmin, r[j].x), fminf(r[j].y, fminf(r[j].z, r[j].w)));
+            bmax = fmaxf(fmaxf(bmax, r[j].x), fmaxf(r[j].y, fmaxf(r[j].z, r[j].w)));
+        }
+        if (bmin < lo || bmax > hi) {
+#pragma unroll
+            for (int j = 0; j < kUnroll; ++j) { outside(r[j].x); outside(r[j].y); outside(r[j].z); outside(r[j].w); }
         }
     }
 };
 
-template <int PASS>
-__global__ void __launch_bounds__(kThreads)
-select_pass_kernel(const float* __restrict__ d, uint64_t n, const SelectState* __restrict__ st,
-                   unsigned long long* __restrict__ gdigits) {
-    __shared__ uint32_t sbins[kDigitBins];
-    for (int i = threadIdx.x; i < kDigitBins; i += kThreads) sbins[i] = 0;
-    __syncthreads();
-    SelectF<PASS> f;
-    f.prefix = (PASS == 0) ? 0u : st->prefix;
-    f.sbins = sbins;
-    if (PASS == 0 || !st->invalid) stream_cube(d, n, f);
-    __syncthreads();
-    for (int i = threadIdx.x; i < kDigitBins; i += kThreads) {
-        uint32_t c = sbins[i];
-        if (c) atomicAdd(&gdigits[i], (unsigned long long)c);
-    }
+__device__ __forceinline__ void cluster_sync_all() {
+    asm volatile("barrier.cluster.arrive.release.aligned;\n\tbarrier.cluster.wait.acquire.aligned;" ::: "memory");
 }
 
-// One CTA of 1024 threads: exclusive scan of the digit histogram, pick the bucket holding rank k,
-// update (prefix, k), clear the histogram for the next pass.  After PASS 2 the 32-bit key is complete
-// and is mapped back to the float.
-template <int PASS>
-__global__ void __launch_bounds__(1024)
-select_scan_kernel(SelectState* __restrict__ st, unsigned long long* __restrict__ gdigits, int clear) {
-    constexpr int NB = (PASS == 2) ? 1024 : kDigitBins;
-    constexpr int BITS = (PASS == 2) ? 10 : 11;
-    __shared__ unsigned long long warp_tot[32];
-    __shared__ unsigned long long s_k;
-    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
-    // thread t owns bins [t*PER, t*PER+PER)
-    constexpr int PER = NB / 1024;
-    unsigned long long c[PER > 0 ? PER : 1];
-    unsigned long long mine = 0;
-#pragma unroll
-    for (int j = 0; j < PER; ++j) { c[j] = gdigits[tid * PER + j]; mine += c[j]; }
-    unsigned long long incl = mine;
-#pragma unroll
-    for (int off = 1; off < 32; off <<= 1) {
-        unsigned long long v = __shfl_up_sync(0xffffffffu, incl, off);
-        if (lane >= off) incl += v;
+__global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(kBigThreads)
+hist_dsm_kernel(const float* __restrict__ d, uint64_t n, int nbins, float lo, float hi, float scale,
+                unsigned long long* __restrict__ gbins, unsigned long long* __restrict__ goutside) {
+    extern __shared__ uint32_t dyn_bins[];  // 32768 + 1 counters per CTA
+    __shared__ uint32_t s_out[2];
+    uint32_t rank;
+    asm volatile("mov.u32 %0, %%cluster_ctarank;" : "=r"(rank));
+    for (int i = threadIdx.x; i <= 32768; i += kBigThreads) dyn_bins[i] = 0;
+    if (threadIdx.x < 2) s_out[threadIdx.x] = 0;
+    cluster_sync_all();  // both CTAs zeroed before any remote increment
+    HistDsmF f;
+    f.lo = lo; f.hi = hi; f.scale = scale; f.top = nbins - 1; f.base_local = smem_addr(dyn_bins);
+    stream_cube<kBigThreads>(d, n, f);
+    cluster_sync_all();  // all remote increments have landed
+    for (int i = threadIdx.x; i < 32768; i += kBigThreads) {
+        const uint32_t c = dyn_bins[i];
+        const int b = 2 * i + (int)rank;
+        if (c && b < nbins) atomicAdd(&gbins[b], (unsigned long long)c);
     }
-    if (lane == 31) warp_tot[warp] = incl;
-    __syncthreads();
-    if (warp == 0) {
-        unsigned long long w = warp_tot[lane], wi = w;
-#pragma unroll
-        for (int off = 1; off < 32; off <<= 1) {
-            unsigned long long v = __shfl_up_sync(0xffffffffu, wi, off);
-            if (lane >= off) wi += v;
-        }
-        warp_tot[lane] = wi - w;  // exclusive prefix of warp totals
-        if (lane == 31 && tid == 31) {
-            // total over all bins
-            unsigned long long total = wi;
-            if (PASS == 0) {
-                st->count = total;
-                if (st->use_median) st->k = total ? (total - 1) / 2 : 0;
-                st->invalid = (st->k >= total) ? 1u : 0u;
-            }
-            s_k = st->k;
-        }
-    }
-    __syncthreads();
-    const unsigned long long k = s_k;
-    unsigned long long excl = warp_tot[warp] + (incl - mine);
-    const bool invalid = st->invalid != 0;
-    __syncthreads();
-    if (!invalid) {
-#pragma unroll
-        for (int j = 0; j < PER; ++j) {
-            if (c[j] && excl <= k && k < excl + c[j]) {  // exactly one (thread, j) satisfies this
-                const uint32_t b = (uint32_t)(tid * PER + j);
-                const uint32_t pre = (PASS == 0) ? b : ((st->prefix << BITS) | b);
-                st->prefix = pre;
-                st->k = k - excl;
-                if (PASS == 2) st->result = __uint_as_float(bits_of_key(pre));
-            }
-            excl += c[j];
-        }
-    } else if (tid == 0) {
-        st->result = __int_as_float(0x7fc00000);
-    }
-    if (clear) {  // leave the digit bins zeroed for the next pass
-#pragma unroll
-        for (int j = 0; j < PER; ++j) gdigits[tid * PER + j] = 0ull;
-        if (PASS == 2) gdigits[1024 + tid] = 0ull;
-    }
+    hist_flush_outside(f, s_out, goutside);
 }
 
 }  // namespace cube
+
+#include "cube_select.cuh"

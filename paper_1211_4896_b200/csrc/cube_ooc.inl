@@ -44,7 +44,25 @@ int cube_ooc_next_sweep(cube_ctx* c, int* more, cudaStream_t s) {
     *more = 0;
     if (c->ooc_want_median) {
         if (c->ooc_sweep == 0) { rc = launch_select_scan<0>(c, c->gdigits, s); *more = 1; }
-        else if (c->ooc_sweep == 1) { rc = launch_select_scan<1>(c, c->gdigits, s); *more = 1; }
+        else if (c->ooc_sweep == 1) {
+            if ((rc = launch_select_scan<1>(c, c->gdigits, s))) return rc;
+            *more = 1;
+            // Did the median's bucket fit the candidate buffer?  One 16-byte read per cube: if so the last
+            // digit is counted on the candidates right now and no third sweep over the bricks is needed.
+            unsigned long long cn[2] = {0, 0};
+            CUBE_CUDA(c, cudaMemcpyAsync(cn, &c->sel->cand_n, sizeof(cn), cudaMemcpyDeviceToHost, s));
+            CUBE_CUDA(c, cudaStreamSynchronize(s));
+            if (c->cand && cn[0] <= cn[1]) {
+                {
+                    ProfScope prof(c, CUBE_K_SELECT_PASS, s);
+                    select_cand_kernel<<<c->num_sms, kThreads, 0, s>>>(c->sel, c->gdigits, c->cand);
+                }
+                CUBE_CUDA(c, cudaGetLastError());
+                if ((rc = launch_select_scan<2>(c, c->gdigits, s))) return rc;
+                c->ooc_sweep = 2;  // becomes 3 below: result ready
+                *more = 0;
+            }
+        }
         else if (c->ooc_sweep == 2) { rc = launch_select_scan<2>(c, c->gdigits, s); }
     }
     c->ooc_sweep++;
@@ -57,8 +75,10 @@ int cube_ooc_result(cube_ctx* c, unsigned flags, cube_moments_t* moments, uint64
     if (moments) {
         if (flags & CUBE_SAMPLE_STD) {
             // re-finalise the running partial with the sample-std denominator
-            moments_refinalize_kernel<<<1, 1, 0, s>>>(c->acc, c->nvox_acc, flags, c->mom_out);
-            c->launches++;
+            {
+                ProfScope prof(c, CUBE_K_OTHER, s);
+                moments_refinalize_kernel<<<1, 1, 0, s>>>(c->acc, c->nvox_acc, flags, c->mom_out);
+            }
             CUBE_CUDA(c, cudaGetLastError());
         }
         CUBE_CUDA(c, cudaMemcpyAsync(moments, c->mom_out, sizeof(MomentsOut), cudaMemcpyDefault, s));

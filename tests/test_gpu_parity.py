@@ -123,6 +123,9 @@ def test_degenerate_cubes(ctx):
         np.array([np.inf, -np.inf, 1.0, qn, 2.0], np.float32),             # infinities (R8)
         np.concatenate([np.full(40000, 0.1, np.float32), np.full(30000, qn, np.float32),
                         np.full(40000, 0.1, np.float32)]),                 # constant with a blanked slab
+        np.tile(np.array([0.0, -0.0], np.float32), 60000),                 # -0.0 < +0.0 inside one thread's batch
+        np.tile(np.array([-0.0, 0.0, 0.0], np.float32), 40001),
+        np.concatenate([np.full(50000, 0.0, np.float32), np.full(50000, -0.0, np.float32)]),
         np.arange(1 << 20, dtype=np.float32),                              # ramp: closed forms
         np.arange(1 << 20, dtype=np.float32)[::-1].copy() - np.float32(2 ** 19),
     ]
@@ -326,7 +329,7 @@ def test_config5_scaled_out_of_core(ctx):
             ctx.ooc_brick(t, t.numel())
         more = ctx.ooc_next_sweep()
         sweeps += 1
-    assert sweeps == 3
+    assert sweeps == 2                      # the median's bucket fitted the candidate buffer: no third sweep
     m, b, o, med = ctx.ooc_result(4096)
     check_moments(m, oracle.moments(a), a)
     rb, ro = oracle.histogram(a, 4096, -0.02, 0.5)
@@ -339,6 +342,51 @@ def test_config5_scaled_out_of_core(ctx):
     assert same_float(ctx.median(whole, a.size, 1, 1), med)
     ms = ctx.ooc_result(4096, flags=cube.SAMPLE_STD)[0]
     check_moments(ms, oracle.moments(a, sample_std=True), a)
+
+
+def test_candidate_buffer_overflow_falls_back_to_a_third_pass():
+    # a 4 KiB candidate buffer cannot hold the median's bucket: pass 2 must stream the cube again (in-core)
+    # and the brick-streamed path must ask for a third sweep -- same exact results either way
+    small = cube.Context(scratch_bytes_hint=4096)
+    try:
+        cases = [cubegen.generate_numpy(cubegen.scaled("c2", (64, 64, 128), nsrc=3)).reshape(-1),
+                 np.full(300000, 0.25, np.float32),                       # every key in one bucket
+                 cubegen.generate_numpy(cubegen.scaled("c4", (128, 128, 16))).reshape(-1)]
+        for a in cases:
+            t = dev(a, 1)
+            assert same_float(small.median(t, a.size, 1, 1), oracle.median(a))
+            cnt = int((~np.isnan(a)).sum())
+            for k in (0, cnt // 3, cnt - 1):
+                assert same_float(small.kth(t, a.size, 1, 1, k), oracle.kth(a, k))
+            small.ooc_begin(0, 0.0, 0.0, want_median=True)
+            sweeps, more = 0, True
+            half = (a.size // 2) & ~3
+            while more:
+                small.ooc_brick(t[:half], half)
+                small.ooc_brick(t[half:], a.size - half)
+                more = small.ooc_next_sweep()
+                sweeps += 1
+            assert sweeps == 3
+            assert same_float(small.ooc_result(0)[3], oracle.median(a))
+    finally:
+        small.close()
+
+
+def test_packed_histogram_counter_wraps(ctx):
+    # > 65535 voxels in even bins, odd bins and adjacent (even, odd) pairs of the 16-bit packed layout
+    r = np.random.default_rng(11)
+    n = 1 << 21
+    nb = 65536
+    centres = np.array([0, 1, 2, 100, 101, 32767, 32768, 65534, 65535], dtype=np.int64)
+    b = centres[r.integers(0, len(centres), n)]
+    b[r.integers(0, n, n // 16)] = r.integers(0, nb, n // 16)               # plus a uniform floor
+    a = ((b.astype(np.float64) + 0.5) / nb).astype(np.float32)             # lo=0, hi=1: exact bin centres
+    t = dev(a)
+    for nbins in (nb, nb - 1, 40001, 16385):
+        got, go = ctx.histogram(t, n, 1, 1, nbins, 0.0, 1.0)
+        rb, ro = oracle.histogram(a, nbins, 0.0, 1.0)
+        assert (got == rb).all() and (go == ro).all()
+    assert rb.max() > 3 * 65536
 
 
 @pytest.mark.parametrize("resident", [False, True])
