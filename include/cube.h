@@ -57,9 +57,11 @@ enum {
     CUBE_SAMPLE_STD = 1u,  /* std = sqrt(M2/(n-1)) instead of the population sqrt(M2/n); n==1 -> NaN */
     CUBE_COARSE_HIST = 2u, /* cube_moments: also accumulate the first radix-select digit histogram
                               (2048 bins of key>>21) in the same pass and keep it in the context */
-    CUBE_REUSE_COARSE = 4u /* cube_kth_ex/cube_median_ex: skip select pass 1 and use the digit
-                              histogram left by the last cube_moments(CUBE_COARSE_HIST) call on the
-                              SAME data (the caller vouches for that) */
+    CUBE_REUSE_COARSE = 4u,/* cube_kth_ex/cube_median_ex: skip the first select pass and use the digit
+                              histogram left by the last cube_moments(CUBE_COARSE_HIST) or cube_stats(median)
+                              call on the SAME data (the caller vouches for that) */
+    CUBE_RANGE_MINMAX = 8u /* cube_stats: histogram over [data min, data max] (found by its first pass, never
+                              leaves the device) instead of the lo/hi arguments */
 };
 
 #define CUBE_MAX_BINS 65536
@@ -107,6 +109,21 @@ int cube_median(cube_ctx* ctx, const float* d, int64_t nx, int64_t ny, int64_t n
 int cube_median_ex(cube_ctx* ctx, const float* d, int64_t nx, int64_t ny, int64_t nz, unsigned flags,
                    float* out, cudaStream_t stream);
 
+/* Everything at once, in TWO reads of the cube (SURVEY.md sec. 8(a) steps 1-8 fused):
+ *   pass A  count/min/max/mean/std + first select digit;   pass B  histogram + second digit + compaction of
+ *   the median's bucket;   then the last digit on the compacted candidates.
+ * Results are those of cube_moments, cube_histogram and cube_median, bit for bit.  Any of `moments`,
+ * (`bins`,`outside`) and `median` may be NULL to skip that output (bins and outside go together).
+ * flags: CUBE_SAMPLE_STD; CUBE_RANGE_MINMAX = histogram over [min,max] (lo/hi ignored).  With
+ * CUBE_RANGE_MINMAX, when there is no non-NaN voxel, an extremum is infinite, or max-min or nbins/(max-min)
+ * overflows float32 (the cases cube_histogram rejects with CUBE_EINVAL), all bins are 0 and
+ * outside[0] = outside[1] = UINT64_MAX.  More than 16384 bins together with the median take a third read
+ * (histogram and select run as separate kernels).  The first-digit histogram stays in the context for
+ * cube_kth_ex(..., CUBE_REUSE_COARSE). */
+int cube_stats(cube_ctx* ctx, const float* d, int64_t nx, int64_t ny, int64_t nz, int nbins, float lo, float hi,
+               unsigned flags, cube_moments_t* moments, uint64_t* bins /* [nbins] */, uint64_t* outside /* [2] */,
+               float* median, cudaStream_t stream);
+
 /* ---- Out-of-core / streamed cubes (north_star (4); the paper is in-core by design).
  * The cube is presented brick by brick (any split into contiguous runs of voxels); each brick is a device
  * buffer the caller has filled (e.g. by cudaMemcpyAsync from pinned host memory on a side stream).
@@ -151,14 +168,23 @@ uint64_t cube_launch_count(const cube_ctx* ctx);
  * it off when timing whole steps).  cube_profile_read() synchronises the device, then returns the summed
  * duration and the number of launches of one kernel kind since the last cube_profile_reset(). */
 enum {
-    CUBE_K_MOMENTS = 0,     /* moments_kernel (with or without the fused coarse digit histogram) */
-    CUBE_K_HIST = 1,        /* histogram kernels */
-    CUBE_K_SELECT_PASS = 2, /* radix-select digit passes over the cube (or the candidate buffer) */
-    CUBE_K_SELECT_SCAN = 3, /* 1-CTA bucket location kernels */
-    CUBE_K_OTHER = 4,
-    CUBE_K_KINDS = 5
+    CUBE_K_MOMENTS = 0,        /* moments_kernel<false> */
+    CUBE_K_MOMENTS_COARSE = 1, /* moments_kernel<true>: moments + first select digit (pass A of cube_stats) */
+    CUBE_K_HIST = 2,           /* histogram kernels */
+    CUBE_K_SELECT_PASS0 = 3,   /* first digit over the cube */
+    CUBE_K_SELECT_PASS1 = 4,   /* second digit + candidate compaction over the cube */
+    CUBE_K_SELECT_PASS2 = 5,   /* last digit: on the candidate buffer (normal) or over the cube (fallback) */
+    CUBE_K_SELECT_CAND = 6,    /* last digit on the candidates, brick-streamed path */
+    CUBE_K_SELECT_SCAN = 7,    /* 1-CTA bucket location kernels */
+    CUBE_K_HIST_SELECT = 8,    /* hist_select_kernel (pass B of cube_stats) */
+    CUBE_K_PROBE = 9,          /* cube_probe_read */
+    CUBE_K_OTHER = 10,
+    CUBE_K_KINDS = 11
 };
 int cube_profile_enable(cube_ctx* ctx, int on);
+/* Read-only STREAM probe: streams nvox float32 voxels through the same loop as the statistics kernels with one
+ * FADD per voxel and discards the result.  Time it (CUBE_K_PROBE) to get the read ceiling of this GPU. */
+int cube_probe_read(cube_ctx* ctx, const float* d, uint64_t nvox, cudaStream_t stream);
 int cube_profile_reset(cube_ctx* ctx);
 int cube_profile_read(cube_ctx* ctx, int kind, double* total_ms, uint64_t* launches);
 

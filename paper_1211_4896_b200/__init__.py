@@ -19,18 +19,18 @@ _HERE = os.path.dirname(os.path.abspath(__file__))
 _LIBPATH = os.path.join(_HERE, "libcube.so")
 
 OK, EINVAL, EEMPTY, ECUDA, ERANGE, ENOMEM = 0, 1, 2, 3, 4, 5
-SAMPLE_STD, COARSE_HIST, REUSE_COARSE = 1, 2, 4
+SAMPLE_STD, COARSE_HIST, REUSE_COARSE, RANGE_MINMAX = 1, 2, 4, 8
 MAX_BINS = 65536
 
 # every symbol include/cube.h declares (checked by tests/test_abi.py)
 SYMBOLS = ["cube_create", "cube_destroy", "cube_moments", "cube_histogram", "cube_kth", "cube_kth_ex",
-           "cube_median", "cube_median_ex", "cube_ooc_begin", "cube_ooc_brick", "cube_ooc_next_sweep",
+           "cube_median", "cube_median_ex", "cube_stats", "cube_probe_read", "cube_ooc_begin", "cube_ooc_brick", "cube_ooc_next_sweep",
            "cube_ooc_result", "cube_host_workspace", "cube_stats_host", "cube_strerror",
            "cube_last_cuda_error", "cube_set_launch", "cube_set_knob", "cube_launch_count",
            "cube_profile_enable", "cube_profile_reset", "cube_profile_read"]
 KNOB_CTAS_PER_SM, KNOB_BIGHIST = 0, 1
-K_MOMENTS, K_HIST, K_SELECT_PASS, K_SELECT_SCAN, K_OTHER = 0, 1, 2, 3, 4
-KIND_NAMES = ["moments", "histogram", "select_pass", "select_scan", "other"]
+KIND_NAMES = ["moments", "moments_coarse", "histogram", "select_pass0", "select_pass1", "select_pass2",
+              "select_cand", "select_scan", "hist_select", "probe_read", "other"]
 
 
 class CubeError(RuntimeError):
@@ -71,6 +71,8 @@ def load():
     L.cube_kth_ex.argtypes = [vp, vp, i64, i64, i64, u64, cu, vp, vp]
     L.cube_median.argtypes = [vp, vp, i64, i64, i64, vp, vp]
     L.cube_median_ex.argtypes = [vp, vp, i64, i64, i64, cu, vp, vp]
+    L.cube_stats.argtypes = [vp, vp, i64, i64, i64, ci, f32, f32, cu, vp, vp, vp, vp, vp]
+    L.cube_probe_read.argtypes = [vp, vp, u64, vp]
     L.cube_ooc_begin.argtypes = [vp, ci, f32, f32, ci, vp]
     L.cube_ooc_brick.argtypes = [vp, vp, u64, vp]
     L.cube_ooc_next_sweep.argtypes = [vp, ctypes.POINTER(ci), vp]
@@ -172,6 +174,32 @@ class Context:
         self._check(self._L.cube_median_ex(self._h, _ptr(d), nx, ny, nz, flags,
                                            ctypes.cast(ctypes.byref(r), ctypes.c_void_p), stream))
         return np.float32(r.value)
+
+    def stats(self, d, nx, ny, nz, nbins=0, lo=None, hi=None, flags=0, want_median=True,
+              out=None, bins=None, outside=None, median=None, stream=0):
+        """cube_stats: moments + histogram + exact lower median in two reads of the cube.
+        lo=None -> histogram over [min,max] (CUBE_RANGE_MINMAX); nbins=0 -> no histogram.
+        With no output buffers given returns (moments dict, bins, outside, median) on the host."""
+        if nbins and lo is None:
+            flags |= RANGE_MINMAX
+            lo = hi = 0.0
+        if out is not None or bins is not None or median is not None:
+            self._check(self._L.cube_stats(self._h, _ptr(d), nx, ny, nz, nbins, lo or 0.0, hi or 0.0, flags,
+                                           _ptr(out), _ptr(bins), _ptr(outside), _ptr(median), stream))
+            return None
+        m = MomentsT()
+        b = np.zeros(max(int(nbins), 1), dtype=np.uint64)
+        o = np.zeros(2, dtype=np.uint64)
+        r = ctypes.c_float(float("nan"))
+        self._check(self._L.cube_stats(self._h, _ptr(d), nx, ny, nz, nbins, lo or 0.0, hi or 0.0, flags,
+                                       ctypes.cast(ctypes.byref(m), ctypes.c_void_p),
+                                       _ptr(b) if nbins else None, _ptr(o) if nbins else None,
+                                       ctypes.cast(ctypes.byref(r), ctypes.c_void_p) if want_median else None,
+                                       stream))
+        return m.as_dict(), (b if nbins else None), (o if nbins else None), (np.float32(r.value) if want_median else None)
+
+    def probe_read(self, d, nvox, stream=0):
+        self._check(self._L.cube_probe_read(self._h, _ptr(d), nvox, stream))
 
     # --- brick-streamed (out-of-core) ------------------------------------------------------------------
     def ooc_begin(self, nbins, lo, hi, want_median=True, stream=0):

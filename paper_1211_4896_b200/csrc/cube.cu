@@ -29,6 +29,8 @@ struct cube_ctx {
     unsigned long long* gdigits = nullptr; // kDigitBins
     unsigned long long* coarse = nullptr;  // kDigitBins: digit histogram kept by CUBE_COARSE_HIST
     SelectState* sel = nullptr;
+    float* range3 = nullptr;               // (lo, hi, scale) resolved on the device by cube_stats
+    float* probe_out = nullptr;            // cube_probe_read sink
     uint32_t* cand = nullptr;              // candidate keys of the select (step 8)
     unsigned long long cand_cap = 0;       // in keys
     // out-of-core state (host side)
@@ -48,14 +50,18 @@ struct cube_ctx {
     std::vector<cudaEvent_t> prof_ev;   // pairs
     std::vector<int> prof_kind;         // kind of pair i
     size_t prof_used = 0;               // pairs in use
-    double prof_ms[CUBE_K_KINDS] = {0, 0, 0, 0, 0};
-    uint64_t prof_n[CUBE_K_KINDS] = {0, 0, 0, 0, 0};
+    double prof_ms[CUBE_K_KINDS] = {};
+    uint64_t prof_n[CUBE_K_KINDS] = {};
 };
 
 namespace {
 
 constexpr int kMaxCtasPerSm = 8;
 constexpr int kSmemHistMaxBins = 16384;  // 64 KiB of 32-bit counters per CTA
+// dynamic shared memory of hist_select_kernel: histogram + trash, digit bins + trash, stage slices + counters
+constexpr int hist_select_smem(int nbins) {
+    return (nbins + 1 + kDigitBins + 1 + (kThreads / 32) * ((int)kStageCap + 1)) * (int)sizeof(uint32_t);
+}
 
 #define CUBE_CUDA(ctx, call)                              \
     do {                                                  \
@@ -134,7 +140,7 @@ int launch_moments(cube_ctx* c, const float* d, uint64_t n, unsigned flags, int 
     const int grid = grid_for(c, 4, occ_m < kMaxCtasPerSm ? occ_m : kMaxCtasPerSm);
     if (coarse && !accumulate) CUBE_CUDA(c, cudaMemsetAsync(c->coarse, 0, kDigitBins * sizeof(unsigned long long), s));
     {
-    ProfScope prof(c, CUBE_K_MOMENTS, s);
+    ProfScope prof(c, coarse ? CUBE_K_MOMENTS_COARSE : CUBE_K_MOMENTS, s);
     if (coarse) {
         moments_kernel<true><<<grid, kThreads, 0, s>>>(d, n, c->partials, c->ticket, c->acc, c->nvox_acc,
                                                        accumulate, flags, c->mom_out, c->coarse);
@@ -148,7 +154,7 @@ int launch_moments(cube_ctx* c, const float* d, uint64_t n, unsigned flags, int 
 }
 
 int launch_hist(cube_ctx* c, const float* d, uint64_t n, int nbins, float lo, float hi, float scale,
-                cudaStream_t s) {
+                cudaStream_t s, const float* range3 = nullptr) {
     unsigned long long* outside = c->gbins + CUBE_MAX_BINS;
     {
     ProfScope prof(c, CUBE_K_HIST, s);
@@ -158,15 +164,16 @@ int launch_hist(cube_ctx* c, const float* d, uint64_t n, int nbins, float lo, fl
         if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, hist_smem_kernel, kThreads, smem) != cudaSuccess)
             occ = 1;
         const int grid = grid_for(c, 4, occ);
-        hist_smem_kernel<<<grid, kThreads, smem, s>>>(d, n, nbins, lo, hi, scale, c->gbins, outside);
+        hist_smem_kernel<<<grid, kThreads, smem, s>>>(d, n, nbins, lo, hi, scale, range3, c->gbins, outside);
     } else {
         // one CTA of 1024 threads per SM, 16-bit packed counters (128 KiB for 65536 bins)
         const size_t smem = (size_t)((nbins + 1) / 2) * sizeof(uint32_t);
         if (c->bighist == 1) {
             hist_dsm_kernel<<<c->num_sms & ~1, kBigThreads, (32768 + 1) * sizeof(uint32_t), s>>>(
-                d, n, nbins, lo, hi, scale, c->gbins, outside);
+                d, n, nbins, lo, hi, scale, range3, c->gbins, outside);
         } else {
-            hist_packed_kernel<<<c->num_sms, kBigThreads, smem, s>>>(d, n, nbins, lo, hi, scale, c->gbins, outside);
+            hist_packed_kernel<<<c->num_sms, kBigThreads, smem, s>>>(d, n, nbins, lo, hi, scale, range3, c->gbins,
+                                                                     outside);
         }
     }
     }
@@ -180,7 +187,7 @@ int launch_select_pass(cube_ctx* c, const float* d, uint64_t n, cudaStream_t s) 
     if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, select_pass_kernel<PASS>, kThreads, 0) != cudaSuccess) occ = 1;
     const int grid = grid_for(c, 4, occ < kMaxCtasPerSm ? occ : kMaxCtasPerSm);
     {
-        ProfScope prof(c, CUBE_K_SELECT_PASS, s);
+        ProfScope prof(c, PASS == 0 ? CUBE_K_SELECT_PASS0 : PASS == 1 ? CUBE_K_SELECT_PASS1 : CUBE_K_SELECT_PASS2, s);
         select_pass_kernel<PASS><<<grid, kThreads, 0, s>>>(d, n, c->sel, c->gdigits, c->cand);
     }
     CUBE_CUDA(c, cudaGetLastError());
@@ -256,11 +263,15 @@ int cube_create(cube_ctx** out, size_t scratch_bytes_hint) {
     ok = ok && cudaMalloc(&c->gdigits, kDigitBins * sizeof(unsigned long long)) == cudaSuccess;
     ok = ok && cudaMalloc(&c->coarse, kDigitBins * sizeof(unsigned long long)) == cudaSuccess;
     ok = ok && cudaMalloc(&c->sel, sizeof(SelectState)) == cudaSuccess;
+    ok = ok && cudaMalloc(&c->range3, 4 * sizeof(float)) == cudaSuccess;
+    ok = ok && cudaMalloc(&c->probe_out, sizeof(float)) == cudaSuccess;
     ok = ok && cudaMemset(c->ticket, 0, sizeof(unsigned int)) == cudaSuccess;
     ok = ok && cudaMemset(c->gdigits, 0, kDigitBins * sizeof(unsigned long long)) == cudaSuccess;
     ok = ok && cudaMemset(c->coarse, 0, kDigitBins * sizeof(unsigned long long)) == cudaSuccess;
     ok = ok && cudaFuncSetAttribute(hist_smem_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize,
                                     (kSmemHistMaxBins + 1) * (int)sizeof(uint32_t)) == cudaSuccess;
+    ok = ok && cudaFuncSetAttribute(hist_select_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                    hist_select_smem(kSmemHistMaxBins)) == cudaSuccess;
     ok = ok && cudaFuncSetAttribute(hist_packed_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize,
                                     (CUBE_MAX_BINS / 2) * (int)sizeof(uint32_t)) == cudaSuccess;
     ok = ok && cudaFuncSetAttribute(hist_dsm_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize,
@@ -278,6 +289,7 @@ int cube_destroy(cube_ctx* c) {
     if (!c) return CUBE_EINVAL;
     cudaFree(c->partials); cudaFree(c->ticket); cudaFree(c->acc); cudaFree(c->nvox_acc);
     cudaFree(c->mom_out); cudaFree(c->gbins); cudaFree(c->gdigits); cudaFree(c->coarse); cudaFree(c->sel);
+    cudaFree(c->range3); cudaFree(c->probe_out);
     cudaFree(c->cand);
     cudaFree(c->resident); cudaFree(c->chunk[0]); cudaFree(c->chunk[1]);
     if (c->pinned_results) cudaFreeHost(c->pinned_results);
@@ -339,6 +351,81 @@ int cube_median_ex(cube_ctx* c, const float* d, int64_t nx, int64_t ny, int64_t 
 
 int cube_median(cube_ctx* c, const float* d, int64_t nx, int64_t ny, int64_t nz, float* out, cudaStream_t s) {
     return cube_median_ex(c, d, nx, ny, nz, 0u, out, s);
+}
+
+int cube_stats(cube_ctx* c, const float* d, int64_t nx, int64_t ny, int64_t nz, int nbins, float lo, float hi,
+               unsigned flags, cube_moments_t* moments, uint64_t* bins, uint64_t* outside, float* median,
+               cudaStream_t s) {
+    uint64_t n;
+    if (!c || !d || !dims_ok(nx, ny, nz, &n)) return CUBE_EINVAL;
+    const bool want_hist = bins != nullptr || outside != nullptr;
+    const bool minmax = (flags & CUBE_RANGE_MINMAX) != 0;
+    const bool want_median = median != nullptr;
+    float scale = 0.f;
+    if (want_hist) {
+        if (!bins || !outside) return CUBE_EINVAL;
+        if (minmax) { if (nbins < 1 || nbins > CUBE_MAX_BINS) return CUBE_EINVAL; lo = hi = 0.f; }
+        else if (!hist_scale(nbins, lo, hi, &scale)) return CUBE_EINVAL;
+    }
+    int rc;
+    // pass A: moments (+ first select digit)
+    if (want_median && (rc = select_init(c, 0, 1, s))) return rc;
+    const unsigned mflags = (flags & CUBE_SAMPLE_STD) | (want_median ? (unsigned)CUBE_COARSE_HIST : 0u);
+    if ((rc = launch_moments(c, d, n, mflags, 0, s))) return rc;
+    if (want_median && (rc = launch_select_scan<0>(c, c->coarse, s))) return rc;
+    if (want_hist) {
+        CUBE_CUDA(c, cudaMemsetAsync(c->gbins, 0, (size_t)nbins * sizeof(unsigned long long), s));
+        CUBE_CUDA(c, cudaMemsetAsync(c->gbins + CUBE_MAX_BINS, 0, 2 * sizeof(unsigned long long), s));
+    }
+    // pass B: histogram + second digit + compaction
+    unsigned long long* goutside = c->gbins + CUBE_MAX_BINS;
+    if (want_median) CUBE_CUDA(c, cudaMemsetAsync(c->gdigits, 0, kDigitBins * sizeof(unsigned long long), s));
+    if (want_median && want_hist && nbins <= kSmemHistMaxBins) {
+        const size_t smem = (size_t)hist_select_smem(nbins);
+        int occ = 0;
+        if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, hist_select_kernel, kThreads, smem) != cudaSuccess) occ = 1;
+        const int grid = grid_for(c, 4, occ < kMaxCtasPerSm ? occ : kMaxCtasPerSm);
+        {
+            ProfScope prof(c, CUBE_K_HIST_SELECT, s);
+            hist_select_kernel<<<grid, kThreads, smem, s>>>(d, n, nbins, lo, hi, scale, minmax ? c->mom_out : nullptr,
+                                                            c->gbins, goutside, c->sel, c->gdigits, c->cand);
+        }
+        CUBE_CUDA(c, cudaGetLastError());
+    } else {
+        if (want_hist) {
+            if (minmax) {
+                {
+                    ProfScope prof(c, CUBE_K_OTHER, s);
+                    hist_range_kernel<<<1, 1, 0, s>>>(c->mom_out, nbins, c->range3, goutside);
+                }
+                CUBE_CUDA(c, cudaGetLastError());
+            }
+            if ((rc = launch_hist(c, d, n, nbins, lo, hi, scale, s, minmax ? c->range3 : nullptr))) return rc;
+        }
+        if (want_median && (rc = launch_select_pass<1>(c, d, n, s))) return rc;
+    }
+    if (want_median) {
+        if ((rc = launch_select_scan<1>(c, c->gdigits, s))) return rc;
+        if ((rc = launch_select_pass<2>(c, d, n, s))) return rc;   // on the candidates unless they did not fit
+        if ((rc = launch_select_scan<2>(c, c->gdigits, s))) return rc;
+        CUBE_CUDA(c, cudaMemcpyAsync(median, &c->sel->result, sizeof(float), cudaMemcpyDefault, s));
+    }
+    if (moments) CUBE_CUDA(c, cudaMemcpyAsync(moments, c->mom_out, sizeof(MomentsOut), cudaMemcpyDefault, s));
+    if (want_hist) {
+        CUBE_CUDA(c, cudaMemcpyAsync(bins, c->gbins, (size_t)nbins * sizeof(uint64_t), cudaMemcpyDefault, s));
+        CUBE_CUDA(c, cudaMemcpyAsync(outside, goutside, 2 * sizeof(uint64_t), cudaMemcpyDefault, s));
+    }
+    return CUBE_OK;
+}
+
+int cube_probe_read(cube_ctx* c, const float* d, uint64_t nvox, cudaStream_t s) {
+    if (!c || !d || nvox == 0) return CUBE_EINVAL;
+    {
+        ProfScope prof(c, CUBE_K_PROBE, s);
+        probe_read_kernel<<<grid_for(c, 4, kMaxCtasPerSm), kThreads, 0, s>>>(d, nvox, c->probe_out);
+    }
+    CUBE_CUDA(c, cudaGetLastError());
+    return CUBE_OK;
 }
 
 const char* cube_strerror(int code) {

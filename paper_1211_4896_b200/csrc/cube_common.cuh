@@ -31,12 +31,20 @@ __device__ __forceinline__ uint32_t key_of(float x) {
     uint32_t u = __float_as_uint(x);
     return u ^ ((uint32_t)((int32_t)u >> 31) | 0x80000000u);
 }
+// First radix digit (key >> 21, 11 bits) <-> raw top 11 bits of the float (bits >> 21): a
+// bijection (raw_of_digit maps digit -> raw), so a histogram indexed by the raw bits holds the same counts in
+// permuted order.
+__device__ __forceinline__ uint32_t raw_digit(float x) { return __float_as_uint(x) >> 21; }
+__host__ __device__ __forceinline__ uint32_t raw_of_digit(uint32_t digit) {
+    return (digit & 0x400u) ? (digit ^ 0x400u) : (~digit & 0x7FFu);
+}
 __host__ __device__ __forceinline__ uint32_t bits_of_key(uint32_t k) {
     return (k & 0x80000000u) ? (k ^ 0x80000000u) : ~k;
 }
 
 // Visit all n voxels of d exactly once across the grid.  F provides `void operator()(float)` for single
-// voxels and `void batch(const float4 (&)[kUnroll])` for a thread's share of a full tile.
+// voxels and `void batch(const float4 (&r)[kUnroll], const float4* p)` for a thread's share of a full tile
+// (r[j] was loaded from p[j * THREADS]).
 // Tiles of THREADS*kUnroll float4 are dealt round-robin to the CTAs, so concurrently running CTAs read
 // adjacent tiles (DRAM page locality) and the assignment is static => per-CTA results are deterministic.
 // The <= 3 voxels before the first 16-byte boundary and the <= 3 after the last full float4 are visited
@@ -64,7 +72,7 @@ __device__ __forceinline__ void stream_cube(const float* __restrict__ d, uint64_
 #pragma unroll
             for (int j = 0; j < kUnroll; ++j) r[j] = ld_stream(v + base + (uint64_t)j * THREADS);
             asm volatile("" ::: "memory");  // all kUnroll loads are issued before the first counter update
-            f.batch(r);
+            f.batch(r, v + base);
         } else {
 #pragma unroll 1
             for (int j = 0; j < kUnroll; ++j) {
@@ -80,7 +88,7 @@ __device__ __forceinline__ void stream_cube(const float* __restrict__ d, uint64_
 
 // Default batch: the single-voxel functor applied to the 4*kUnroll values.
 #define CUBE_DEFAULT_BATCH()                                                        \
-    __device__ __forceinline__ void batch(const float4 (&r)[kUnroll]) {             \
+    __device__ __forceinline__ void batch(const float4 (&r)[kUnroll], const float4*) { \
         _Pragma("unroll") for (int j = 0; j < kUnroll; ++j) {                       \
             (*this)(r[j].x); (*this)(r[j].y); (*this)(r[j].z); (*this)(r[j].w);     \
         }                                                                           \

@@ -60,13 +60,13 @@ struct MomentsF {
         s += dlt;
         q = fma(dlt, dlt, q);
         n += ok ? 1u : 0u;
-        if (COARSE) atomicAdd(&sbins[ok ? (key_of(x) >> 21) : kDigitBins], 1u);  // NaN -> trash counter
+        if (COARSE) atomicAdd(&sbins[ok ? raw_digit(x) : kDigitBins], 1u);  // raw top bits; NaN -> trash counter
     }
     __device__ __forceinline__ void take_pivot(float x) {
         if (!have && x == x) { have = true; pivf = x; pivot = (double)x; }
     }
     __device__ __forceinline__ void operator()(float x) { take_pivot(x); core(x); }
-    __device__ __forceinline__ void batch(const float4 (&r)[kUnroll]) {
+    __device__ __forceinline__ void batch(const float4 (&r)[kUnroll], const float4*) {
         if (!have) {  // only until this thread has met its first non-NaN voxel
 #pragma unroll
             for (int j = 0; j < kUnroll; ++j) { take_pivot(r[j].x); take_pivot(r[j].y); take_pivot(r[j].z); take_pivot(r[j].w); }
@@ -205,7 +205,7 @@ struct HistF : HistBase {
         inc(x);
         outside(x);
     }
-    __device__ __forceinline__ void batch(const float4 (&r)[kUnroll]) {
+    __device__ __forceinline__ void batch(const float4 (&r)[kUnroll], const float4*) {
         float bmin = INFINITY, bmax = -INFINITY;
 #pragma unroll
         for (int j = 0; j < kUnroll; ++j) {
@@ -220,8 +220,77 @@ struct HistF : HistBase {
     }
 };
 
+// Fast variant (the default): the range test and the top-bin clamp leave the per-voxel path.
+// With v = (x - lo) * scale as above and vb its bit pattern, ONE unsigned compare vb < bits((float)(nbins-1))
+// is true exactly for +0 <= v < nbins-1 -- false for negative v (sign bit; also -0.0), for NaN (0x7FFFFFFF) and
+// for everything from the top bin upwards.  For such a voxel lo <= x <= hi is guaranteed (t = x - lo has the
+// sign of the exact difference, and x > hi implies v >= fl(fl(hi-lo) * scale) > nbins - 1 whenever hi > lo and
+// scale is a normal number, nbins <= 65536) and its bin is floor(v), no clamp.  Everything else goes to the
+// trash counter, and the 4-voxel rows that contain such a voxel are flagged (VIMNMX3 on vb) and revisited by
+// a cold path that applies the exact definition (x < lo, x > hi, NaN, closed top bin).  On the ALU pipe --
+// the one that limits these kernels, 16 lanes/clk/SMSP -- that is ISETP + SEL + ~1 per voxel instead of
+// 2 FSETP + SEL + VIMNMX + FMNMX.  Not valid for hi == lo (scale 0): hist_use_fast().
+__host__ __device__ __forceinline__ bool hist_use_fast(int nbins, float lo, float hi, float scale) {
+    return hi > lo && nbins >= 8 && scale >= 1.17549435e-38f;
+}
+struct HistFastF {
+    float lo, hi, scale;
+    int top;
+    uint32_t topbits;  // bits of (float)top
+    uint32_t* sbins;   // nbins + 1 counters (last = trash)
+    uint32_t* s_out;   // shared {below, above}
+    uint32_t below = 0, above = 0;  // unused (kept for hist_flush_outside); the cold path counts in s_out
+    __device__ __forceinline__ void setup(float lo_, float hi_, float scale_, int nbins, uint32_t* sbins_,
+                                          uint32_t* s_out_) {
+        lo = lo_; hi = hi_; scale = scale_; top = nbins - 1; topbits = __float_as_uint((float)(nbins - 1));
+        sbins = sbins_; s_out = s_out_;
+    }
+    __device__ __forceinline__ uint32_t inc(float x) const {
+        const float v = __fmul_rn(__fsub_rn(x, lo), scale);
+        const uint32_t vb = __float_as_uint(v);
+        atomicAdd(&sbins[vb < topbits ? __float2int_rd(v) : top + 1], 1u);
+        return vb;
+    }
+    // exact definition for a voxel the hot path sent to the trash counter
+    static __device__ __forceinline__ void exact(float x, float lo, float hi, float scale, int top,
+                                                 uint32_t topbits, uint32_t* sbins, uint32_t* s_out) {
+        if (x < lo) atomicAdd(&s_out[0], 1u);
+        else if (x > hi) atomicAdd(&s_out[1], 1u);
+        else if (x == x) {  // in range: v >= nbins - 1 (closed top bin, R11) or v == -0.0 (x = -0.0, lo = +0.0)
+            const float v = __fmul_rn(__fsub_rn(x, lo), scale);
+            if (!(__float_as_uint(v) < topbits)) atomicAdd(&sbins[min(max(__float2int_rd(v), 0), top)], 1u);
+        }
+    }
+    static __device__ __noinline__ void cold(uint32_t rows, const float4* __restrict__ p, float lo, float hi,
+                                             float scale, int top, uint32_t topbits, uint32_t* sbins,
+                                             uint32_t* s_out) {
+        do {
+            const int j = __ffs(rows) - 1;
+            rows &= rows - 1;
+            const float4 q = __ldcg(p + j * kThreads);  // L2 hit: the line has just been streamed
+            exact(q.x, lo, hi, scale, top, topbits, sbins, s_out);
+            exact(q.y, lo, hi, scale, top, topbits, sbins, s_out);
+            exact(q.z, lo, hi, scale, top, topbits, sbins, s_out);
+            exact(q.w, lo, hi, scale, top, topbits, sbins, s_out);
+        } while (rows);
+    }
+    __device__ __forceinline__ void operator()(float x) {
+        if (!(inc(x) < topbits)) exact(x, lo, hi, scale, top, topbits, sbins, s_out);
+    }
+    __device__ __forceinline__ void batch(const float4 (&r)[kUnroll], const float4* __restrict__ p) {
+        uint32_t rows = 0;
+#pragma unroll
+        for (int j = 0; j < kUnroll; ++j) {
+            const uint32_t m = max(max(inc(r[j].x), inc(r[j].y)), max(inc(r[j].z), inc(r[j].w)));
+            rows |= (m >= topbits ? 1u : 0u) << j;
+        }
+        if (rows) cold(rows, p, lo, hi, scale, top, topbits, sbins, s_out);
+    }
+};
+
 template <class F>
 __device__ __forceinline__ void hist_flush_outside(F& f, uint32_t* s_out, unsigned long long* goutside) {
+    if (f.lo > f.hi) return;  // unusable device-side [min,max] range: hist_range_kernel has left the marker
     if (f.below) atomicAdd(&s_out[0], f.below);
     if (f.above) atomicAdd(&s_out[1], f.above);
     __syncthreads();
@@ -231,21 +300,35 @@ __device__ __forceinline__ void hist_flush_outside(F& f, uint32_t* s_out, unsign
 // nbins <= 16384: 32-bit counters, several CTAs per SM.
 __global__ void __launch_bounds__(kThreads)
 hist_smem_kernel(const float* __restrict__ d, uint64_t n, int nbins, float lo, float hi, float scale,
+                 const float* __restrict__ range3,
                  unsigned long long* __restrict__ gbins, unsigned long long* __restrict__ goutside) {
     extern __shared__ uint32_t dyn_bins[];
     __shared__ uint32_t s_out[2];
     for (int i = threadIdx.x; i <= nbins; i += kThreads) dyn_bins[i] = 0;  // + trash counter
     if (threadIdx.x < 2) s_out[threadIdx.x] = 0;
     __syncthreads();
-    HistF f;
-    f.lo = lo; f.hi = hi; f.scale = scale; f.top = nbins - 1; f.sbins = dyn_bins;
-    stream_cube<kThreads>(d, n, f);
+    if (range3) { lo = range3[0]; hi = range3[1]; scale = range3[2]; }  // resolved on the device (cube_stats)
+    uint32_t below = 0, above = 0;
+    if (hist_use_fast(nbins, lo, hi, scale)) {
+        HistFastF f;
+        f.setup(lo, hi, scale, nbins, dyn_bins, s_out);
+        stream_cube<kThreads>(d, n, f);
+    } else {
+        HistF f;
+        f.lo = lo; f.hi = hi; f.scale = scale; f.top = nbins - 1; f.sbins = dyn_bins;
+        stream_cube<kThreads>(d, n, f);
+        below = f.below; above = f.above;
+    }
     __syncthreads();
     for (int i = threadIdx.x; i < nbins; i += kThreads) {
         uint32_t c = dyn_bins[i];
         if (c) atomicAdd(&gbins[i], (unsigned long long)c);
     }
-    hist_flush_outside(f, s_out, goutside);
+    if (lo > hi) return;  // unusable device-side [min,max] range: hist_range_kernel has left the marker
+    if (below) atomicAdd(&s_out[0], below);
+    if (above) atomicAdd(&s_out[1], above);
+    __syncthreads();
+    if (threadIdx.x < 2 && s_out[threadIdx.x]) atomicAdd(&goutside[threadIdx.x], (unsigned long long)s_out[threadIdx.x]);
 }
 
 // 16384 < nbins <= 65536: the counters of one CTA no longer fit shared memory as 32-bit words
@@ -283,7 +366,7 @@ struct HistPackedF : HistBase {
         inc(x);
         outside(x);
     }
-    __device__ __forceinline__ void batch(const float4 (&r)[kUnroll]) {
+    __device__ __forceinline__ void batch(const float4 (&r)[kUnroll], const float4*) {
         float bmin = INFINITY, bmax = -INFINITY;
 #pragma unroll
         for (int j = 0; j < kUnroll; ++j) {
@@ -300,6 +383,7 @@ struct HistPackedF : HistBase {
 
 __global__ void __launch_bounds__(kBigThreads)
 hist_packed_kernel(const float* __restrict__ d, uint64_t n, int nbins, float lo, float hi, float scale,
+                   const float* __restrict__ range3,
                    unsigned long long* __restrict__ gbins, unsigned long long* __restrict__ goutside) {
     extern __shared__ uint32_t dyn_bins[];  // (nbins+1)/2 words
     __shared__ uint32_t s_out[2];
@@ -307,6 +391,7 @@ hist_packed_kernel(const float* __restrict__ d, uint64_t n, int nbins, float lo,
     for (int i = threadIdx.x; i < nwords; i += kBigThreads) dyn_bins[i] = 0;
     if (threadIdx.x < 2) s_out[threadIdx.x] = 0;
     __syncthreads();
+    if (range3) { lo = range3[0]; hi = range3[1]; scale = range3[2]; }
     HistPackedF f;
     f.lo = lo; f.hi = hi; f.scale = scale; f.top = nbins - 1; f.sw = dyn_bins; f.gbins = gbins;
     stream_cube<kBigThreads>(d, n, f);
@@ -339,7 +424,7 @@ struct HistDsmF : HistBase {
         inc(x);
         outside(x);
     }
-    __device__ __forceinline__ void batch(const float4 (&r)[kUnroll]) {
+    __device__ __forceinline__ void batch(const float4 (&r)[kUnroll], const float4*) {
         float bmin = INFINITY, bmax = -INFINITY;
 #pragma unroll
         for (int j = 0; j < kUnroll; ++j) {
@@ -360,6 +445,7 @@ __device__ __forceinline__ void cluster_sync_all() {
 
 __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(kBigThreads)
 hist_dsm_kernel(const float* __restrict__ d, uint64_t n, int nbins, float lo, float hi, float scale,
+                const float* __restrict__ range3,
                 unsigned long long* __restrict__ gbins, unsigned long long* __restrict__ goutside) {
     extern __shared__ uint32_t dyn_bins[];  // 32768 + 1 counters per CTA
     __shared__ uint32_t s_out[2];
@@ -368,6 +454,7 @@ hist_dsm_kernel(const float* __restrict__ d, uint64_t n, int nbins, float lo, fl
     for (int i = threadIdx.x; i <= 32768; i += kBigThreads) dyn_bins[i] = 0;
     if (threadIdx.x < 2) s_out[threadIdx.x] = 0;
     cluster_sync_all();  // both CTAs zeroed before any remote increment
+    if (range3) { lo = range3[0]; hi = range3[1]; scale = range3[2]; }
     HistDsmF f;
     f.lo = lo; f.hi = hi; f.scale = scale; f.top = nbins - 1; f.base_local = smem_addr(dyn_bins);
     stream_cube<kBigThreads>(d, n, f);
@@ -380,6 +467,22 @@ hist_dsm_kernel(const float* __restrict__ d, uint64_t n, int nbins, float lo, fl
     hist_flush_outside(f, s_out, goutside);
 }
 
+// Read-only STREAM probe: the same streaming loop with the lightest possible functor (one FADD per voxel).
+// Its rate is the measured read ceiling the statistics kernels are compared with (north_star: "a measured
+// STREAM-style read peak").
+struct ProbeF {
+    float acc = 0.f;
+    __device__ __forceinline__ void operator()(float x) { acc += x; }
+    CUBE_DEFAULT_BATCH()
+};
+__global__ void __launch_bounds__(kThreads)
+probe_read_kernel(const float* __restrict__ d, uint64_t n, float* __restrict__ out) {
+    ProbeF f;
+    stream_cube<kThreads>(d, n, f);
+    if (f.acc == 123.456f) *out = f.acc;  // keeps the loads alive; practically never true
+}
+
 }  // namespace cube
 
 #include "cube_select.cuh"
+#include "cube_fused.cuh"

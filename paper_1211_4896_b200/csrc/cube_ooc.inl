@@ -54,7 +54,7 @@ int cube_ooc_next_sweep(cube_ctx* c, int* more, cudaStream_t s) {
             CUBE_CUDA(c, cudaStreamSynchronize(s));
             if (c->cand && cn[0] <= cn[1]) {
                 {
-                    ProfScope prof(c, CUBE_K_SELECT_PASS, s);
+                    ProfScope prof(c, CUBE_K_SELECT_CAND, s);
                     select_cand_kernel<<<c->num_sms, kThreads, 0, s>>>(c->sel, c->gdigits, c->cand);
                 }
                 CUBE_CUDA(c, cudaGetLastError());

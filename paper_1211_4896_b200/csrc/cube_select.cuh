@@ -14,129 +14,150 @@
 
 namespace cube {
 
-constexpr uint32_t kCandChunk = 256;  // keys reserved per global atomic by one warp
+// PASS 1 compaction ("step 8"): every warp stages the keys of the prefix bucket in its own slice of shared
+// memory and moves them to the candidate buffer in coalesced runs, reserving the space with ONE global atomic
+// per flush.  A warp checks its fill level once per tile (1024 voxels per warp), so a slice holds the flush
+// threshold plus one whole tile and can never overflow -- also on a constant cube, where every voxel is a
+// candidate.  (v2 reserved space by ballot + warp scan per tile: at the 0.3 % bucket density of config 2
+// ~95 % of the warp tiles took that path to place ~3 keys, 564 M instructions, 5.1 TB/s;
+// profiles/r1_v2_baseline.md.)
+constexpr uint32_t kStageThresh = 128;                                 // flush when more keys than this wait
+constexpr uint32_t kStageCap = kStageThresh + 32u * 4u * kUnroll;      // + one tile of a warp: 1152 keys
+constexpr int kStageBytes = (kThreads / 32) * (int)kStageCap * 4;      // 36 KiB per CTA
 
-// Per-voxel work, written to stay at ~8 instructions with no branch:
-//   PASS 0:  idx = NaN ? trash : key >> 21
-//   PASS 1/2: kk = key - (prefix << S) (S = 21 / 10); the voxel is in the prefix bucket iff kk < 2^S
-//            (unsigned), and then its digit is kk >> 10 (PASS 1) or kk (PASS 2); so
-//            idx = min(kk >> 10, 2048) resp. min(kk, 1024) sends every other voxel to the trash counter
-//            without a compare.  NaN keys can only fall into the buckets next to +-inf (top digit 0-3 or
-//            2044-2047); only then (NANCHK) is the x == x test compiled in.
-// The counter increment is an unconditional ATOMS.POPC.INC (hardware-aggregated over equal addresses).
+// Per-voxel work, branch-free:
+//   PASS 0:  idx = NaN ? trash : bits >> 21 (the RAW top 11 bits; the scan kernel reads the bins in key order
+//            through raw_of_digit(), so the key transform is not paid per voxel); ATOMS.POPC.INC
+//            (hardware-aggregated over equal addresses).  SHF, FSETP, SEL, LEA, ATOMS.
+//   PASS 1:  the voxel is in the prefix bucket iff (bits ^ rawbase) < 2^21: LOP3 per voxel, VIMNMX3 per pair,
+//            one flag per 4-voxel row (~2 ALU instructions per voxel, NO shared-memory traffic).  Only the rows
+//            that hold a voxel of the bucket (the bucket is 0.05-3 % of the cube on the configs) are visited
+//            again by a cold path that re-loads the row (an L2 hit: its line has just been streamed), counts
+//            the digit (kk >> 10) and stages the key.  So pass 1 costs less issue bandwidth than pass 0.
+//   PASS 2 over the cube (only when the candidates did not fit): idx = min(key - (prefix << 10), 1024) sends every
+//            voxel outside the bucket to the trash counter without a compare.
+//   NaN keys can only fall into the buckets next to +-inf (top digit 0-3 or 2044-2047); only then (NANCHK)
+//   is the x == x test compiled in.
 template <int PASS, bool NANCHK>
 struct SelectF {
-    static constexpr uint32_t kSpan = (PASS == 1) ? (1u << 21) : (1u << 10);
-    static constexpr int kDShift = (PASS == 1) ? 10 : 0;
+    static constexpr uint32_t kSpan = 1u << 21;
     static constexpr uint32_t kTrash = (PASS == 2) ? 1024u : (uint32_t)kDigitBins;
     uint32_t base;     // prefix << 21 (PASS 1) or prefix << 10 (PASS 2)
     uint32_t* sbins;   // kDigitBins + 1 counters
-    // PASS 1 compaction: each warp appends into a private reservation [w_pos, w_end) of the candidate
-    // buffer and takes a new one of kCandChunk keys with ONE global atomic when it runs out (an atomic per
-    // warp per tile on the single counter serialises in L2: 1 M atomics cost ~1 ms on config 2).  What is
-    // left of the last reservation is filled with a key that cannot match, so the buffer has no stale slot.
-    uint32_t* cand;
-    unsigned long long* cand_n;
-    unsigned long long cand_cap;
-    unsigned long long w_pos = 0, w_end = 0;  // warp-uniform
+    // PASS 1 compaction state
+    bool compacting = false;    // false once the candidate buffer is known to be too small (or absent)
+    uint32_t* s_cnt = nullptr;  // this warp's fill counter (shared memory)
+    uint32_t* s_buf = nullptr;  // this warp's kStageCap slots (shared memory)
+    uint32_t* cand = nullptr;
+    unsigned long long* cand_n = nullptr;
+    unsigned long long cand_cap = 0;
 
+    // PASS 1 hot path: key >> 21 == prefix  <=>  bits >> 21 == raw_of_digit(prefix)  <=>  (bits ^ rawbase) < 2^21
+    // (LOP3), reduced over each 4-voxel row with VIMNMX3; NaN voxels may flag a row, the cold path drops them.
+    uint32_t rawbase = 0;  // raw_of_digit(prefix) << 21
     __device__ __forceinline__ uint32_t kk_of(float x) const {
         uint32_t kk = key_of(x) - base;
         if (NANCHK) kk = (x == x) ? kk : 0xFFFFFFFFu;
         return kk;
     }
-    __device__ __forceinline__ void count(float x, uint32_t kk) {
-        if (PASS == 0) atomicAdd(&sbins[(x == x) ? (key_of(x) >> 21) : kTrash], 1u);
-        else atomicAdd(&sbins[min(kk >> kDShift, kTrash)], 1u);
+    __device__ __forceinline__ void count(float x) {  // PASS 0 / PASS 2: every voxel increments a counter
+        if (PASS == 0) atomicAdd(&sbins[(x == x) ? raw_digit(x) : kTrash], 1u);
+        else atomicAdd(&sbins[min(kk_of(x), kTrash)], 1u);
     }
     __device__ __forceinline__ void key(uint32_t k) {  // PASS 2 over the candidate buffer (no NaN in it)
         atomicAdd(&sbins[min(k - base, kTrash)], 1u);
     }
     __device__ __forceinline__ void operator()(float x) {  // single voxels: head / tail / ragged last tile
-        const uint32_t kk = (PASS == 0) ? 0u : kk_of(x);
-        count(x, kk);
-        if (PASS == 1 && kk < kSpan) {
-            const unsigned long long pos = atomicAdd(cand_n, 1ull);
-            if (pos < cand_cap) cand[pos] = kk + base;
+        if (PASS != 1) { count(x); return; }
+        take1(x, base, sbins, compacting ? s_cnt : nullptr, s_buf);
+    }
+    // Cold path of PASS 1 (static, arguments by value: the functor itself stays in registers): revisit the
+    // flagged 4-voxel rows, count the second digit of the voxels of the bucket and stage their keys.
+    static __device__ __forceinline__ void take1(float x, uint32_t base_, uint32_t* sbins_, uint32_t* s_cnt_,
+                                                 uint32_t* s_buf_) {
+        const uint32_t kk = key_of(x) - base_;
+        if (kk < kSpan && x == x) {
+            atomicAdd(&sbins_[kk >> 10], 1u);
+            if (s_cnt_) s_buf_[atomicAdd(s_cnt_, 1u)] = kk + base_;
         }
     }
-    __device__ __forceinline__ void batch(const float4 (&r)[kUnroll]) {
+    static __device__ __noinline__ void cold(uint32_t rows, const float4* __restrict__ p, uint32_t base_,
+                                             uint32_t* sbins_, uint32_t* s_cnt_, uint32_t* s_buf_) {
+        do {
+            const int j = __ffs(rows) - 1;
+            rows &= rows - 1;
+            const float4 q = __ldcg(p + j * kThreads);  // L2 hit: the line has just been streamed
+            take1(q.x, base_, sbins_, s_cnt_, s_buf_);
+            take1(q.y, base_, sbins_, s_cnt_, s_buf_);
+            take1(q.z, base_, sbins_, s_cnt_, s_buf_);
+            take1(q.w, base_, sbins_, s_cnt_, s_buf_);
+        } while (rows);
+    }
+    // all lanes of the warp: move the c staged keys to the candidate buffer
+    __device__ __forceinline__ void flush(uint32_t c) {
+        const uint32_t lane = threadIdx.x & 31;
+        unsigned long long pos = 0;
+        if (lane == 0) pos = atomicAdd(cand_n, (unsigned long long)c);
+        pos = __shfl_sync(0xffffffffu, pos, 0);
+        if (pos + c <= cand_cap) {
+            for (uint32_t i = lane; i < c; i += 32) cand[pos + i] = s_buf[i];
+        } else {
+            compacting = false;  // the bucket does not fit: PASS 2 will stream the cube, stop staging
+        }
+        __syncwarp();
+        if (lane == 0) *s_cnt = 0;
+        __syncwarp();
+    }
+    __device__ __forceinline__ uint32_t staged() const {
+        __syncwarp();
+        return *reinterpret_cast<volatile uint32_t*>(s_cnt);
+    }
+    __device__ __forceinline__ void batch(const float4 (&r)[kUnroll], const float4* __restrict__ p) {
         if (PASS != 1) {
 #pragma unroll
-            for (int j = 0; j < kUnroll; ++j) {
-                const float v[4] = {r[j].x, r[j].y, r[j].z, r[j].w};
-#pragma unroll
-                for (int c = 0; c < 4; ++c) count(v[c], (PASS == 0) ? 0u : kk_of(v[c]));
-            }
+            for (int j = 0; j < kUnroll; ++j) { count(r[j].x); count(r[j].y); count(r[j].z); count(r[j].w); }
             return;
         }
-        uint32_t mask = 0;
+        uint32_t rows = 0;  // rows (float4) holding at least one voxel whose raw bits are in the bucket
 #pragma unroll
         for (int j = 0; j < kUnroll; ++j) {
-            const float v[4] = {r[j].x, r[j].y, r[j].z, r[j].w};
-#pragma unroll
-            for (int c = 0; c < 4; ++c) {
-                const uint32_t kk = kk_of(v[c]);
-                count(v[c], kk);
-                mask |= (kk < kSpan ? 1u : 0u) << (j * 4 + c);
-            }
+            const uint32_t m = min(min(__float_as_uint(r[j].x) ^ rawbase, __float_as_uint(r[j].y) ^ rawbase),
+                                   min(__float_as_uint(r[j].z) ^ rawbase, __float_as_uint(r[j].w) ^ rawbase));
+            rows |= (m < kSpan ? 1u : 0u) << j;
         }
-        if (__any_sync(0xffffffffu, mask != 0)) {  // the bucket is ~0.1-3 % of the cube on the configs
-            const uint32_t lane = threadIdx.x & 31;
-            const uint32_t cnt = __popc(mask);
-            uint32_t incl = cnt;
-#pragma unroll
-            for (int off = 1; off < 32; off <<= 1) {
-                const uint32_t t = __shfl_up_sync(0xffffffffu, incl, off);
-                if (lane >= off) incl += t;
-            }
-            const uint32_t total = __shfl_sync(0xffffffffu, incl, 31);
-            const unsigned long long rem = w_end - w_pos;
-            unsigned long long nb = 0;
-            uint32_t size = 0;
-            if (total > rem) {  // warp-uniform
-                const uint32_t need = total - (uint32_t)rem;
-                size = need > kCandChunk ? need : kCandChunk;
-                if (lane == 0) nb = atomicAdd(cand_n, (unsigned long long)size);
-                nb = __shfl_sync(0xffffffffu, nb, 0);
-            }
-            if (mask) {
-                uint32_t slot = incl - cnt;
-#pragma unroll
-                for (int j = 0; j < kUnroll; ++j) {
-                    const float v[4] = {r[j].x, r[j].y, r[j].z, r[j].w};
-#pragma unroll
-                    for (int c = 0; c < 4; ++c) {
-                        if (mask & (1u << (j * 4 + c))) {
-                            const unsigned long long idx = (slot < rem) ? w_pos + slot : nb + (slot - rem);
-                            if (idx < cand_cap) cand[idx] = key_of(v[c]);
-                            ++slot;
-                        }
-                    }
-                }
-            }
-            if (total > rem) { w_pos = nb + (total - rem); w_end = nb + size; }
-            else w_pos += total;
+        if (rows) cold(rows, p, base, sbins, compacting ? s_cnt : nullptr, s_buf);
+        if (compacting) {               // warp-uniform
+            const uint32_t c = staged();
+            if (c > kStageThresh) flush(c);
         }
     }
     // all lanes of every warp, after the streaming loop
     __device__ __forceinline__ void finish() {
-        if (PASS != 1) return;
-        const uint32_t sentinel = base ^ (1u << 21);  // top digit != prefix: never matches in PASS 2
-        for (unsigned long long i = w_pos + (threadIdx.x & 31); i < w_end; i += 32)
-            if (i < cand_cap) cand[i] = sentinel;
+        if (PASS != 1 || s_cnt == nullptr) return;
+        const uint32_t c = staged();
+        if (c) flush(c);
+    }
+    // PASS 1 set-up: `stage` = kThreads/32 slices of kStageCap keys + kThreads/32 counters (shared memory)
+    __device__ __forceinline__ void init_stage(uint32_t* stage, uint32_t* cand_, unsigned long long* cand_n_,
+                                               unsigned long long cap) {
+        const uint32_t warp = threadIdx.x >> 5;
+        s_buf = stage + warp * kStageCap;
+        s_cnt = stage + (kThreads / 32) * kStageCap + warp;
+        if ((threadIdx.x & 31) == 0) *s_cnt = 0;
+        __syncwarp();
+        cand = cand_; cand_n = cand_n_; cand_cap = cap;
+        compacting = (cand_ != nullptr) && cap != 0;
     }
 };
 
 template <int PASS, bool NANCHK>
 __device__ __forceinline__ void select_run(const float* __restrict__ d, uint64_t n, SelectState* __restrict__ st,
-                                           uint32_t* sbins, uint32_t* __restrict__ cand) {
+                                           uint32_t* sbins, uint32_t* stage, uint32_t* __restrict__ cand) {
     SelectF<PASS, NANCHK> f;
     f.base = (PASS == 0) ? 0u : (PASS == 1) ? (st->prefix << 21) : (st->prefix << 10);
+    f.rawbase = (PASS == 1) ? (raw_of_digit(st->prefix) << 21) : 0u;
     f.sbins = sbins;
-    f.cand = cand;
-    f.cand_n = &st->cand_n;
-    f.cand_cap = (PASS == 1 && cand) ? st->cand_cap : 0ull;
+    if (PASS == 1) f.init_stage(stage, cand, &st->cand_n, st->cand_cap);
     // cand_n is final when PASS 2 runs: it follows PASS 1 on the same stream
     if (PASS == 2 && cand && st->cand_n <= st->cand_cap) stream_keys<kThreads>(cand, st->cand_n, f);
     else stream_cube<kThreads>(d, n, f);
@@ -144,18 +165,19 @@ __device__ __forceinline__ void select_run(const float* __restrict__ d, uint64_t
 }
 
 template <int PASS>
-__global__ void __launch_bounds__(kThreads)
+__global__ void __launch_bounds__(kThreads, 4)
 select_pass_kernel(const float* __restrict__ d, uint64_t n, SelectState* __restrict__ st,
                    unsigned long long* __restrict__ gdigits, uint32_t* __restrict__ cand) {
     __shared__ uint32_t sbins[kDigitBins + 1];  // + trash counter
+    __shared__ uint32_t stage[(PASS == 1) ? (kThreads / 32) * (kStageCap + 1) : 1];
     for (int i = threadIdx.x; i <= kDigitBins; i += kThreads) sbins[i] = 0;
     __syncthreads();
     if (PASS == 0) {
-        select_run<0, true>(d, n, st, sbins, cand);
+        select_run<0, true>(d, n, st, sbins, stage, cand);
     } else if (!st->invalid) {
         const uint32_t top = (PASS == 1) ? st->prefix : (st->prefix >> 11);  // first digit of the bucket
-        if (top <= 3u || top >= 2044u) select_run<PASS, true>(d, n, st, sbins, cand);
-        else select_run<PASS, false>(d, n, st, sbins, cand);
+        if (top <= 3u || top >= 2044u) select_run<PASS, true>(d, n, st, sbins, stage, cand);
+        else select_run<PASS, false>(d, n, st, sbins, stage, cand);
     }
     __syncthreads();
     constexpr int NB = (PASS == 2) ? 1024 : kDigitBins;
@@ -200,7 +222,11 @@ select_scan_kernel(SelectState* __restrict__ st, unsigned long long* __restrict_
     unsigned long long c[PER > 0 ? PER : 1];
     unsigned long long mine = 0;
 #pragma unroll
-    for (int j = 0; j < PER; ++j) { c[j] = gdigits[tid * PER + j]; mine += c[j]; }
+    for (int j = 0; j < PER; ++j) {  // PASS 0 bins are indexed by the raw top bits of the float
+        const uint32_t b = (uint32_t)(tid * PER + j);
+        c[j] = gdigits[PASS == 0 ? raw_of_digit(b) : b];
+        mine += c[j];
+    }
     unsigned long long incl = mine;
 #pragma unroll
     for (int off = 1; off < 32; off <<= 1) {

@@ -84,12 +84,49 @@ def full_check(ctx, a, hists=(), ks=(), misalign=0):
     cnt = ref["count"]
     med = ctx.median(t, n, 1, 1)
     assert same_float(med, oracle.median(a))
+    check_stats(ctx, t, a, ref, hists)
     for k in ks:
         if k < cnt:
             assert same_float(ctx.kth(t, n, 1, 1, k), oracle.kth(a, k)), k
         else:
             assert math.isnan(float(ctx.kth(t, n, 1, 1, k)))
     return ref
+
+
+def check_stats(ctx, t, a, ref, hists, dims=None):
+    """cube_stats (everything in two reads) against the oracle: fixed ranges, [min,max], no histogram."""
+    nx, ny, nz = dims if dims else (a.size, 1, 1)
+    omed = oracle.median(a)
+    m, b, o, med = ctx.stats(t, nx, ny, nz)                                   # moments + median only
+    check_moments(m, ref, a)
+    assert b is None and same_float(med, omed)
+    for nbins, lo, hi in hists:
+        try:
+            rb, ro = oracle.histogram(a, nbins, lo, hi)
+        except ValueError:
+            with pytest.raises(cube.CubeError):
+                ctx.stats(t, nx, ny, nz, nbins, lo, hi)
+            continue
+        m, b, o, med = ctx.stats(t, nx, ny, nz, nbins, lo, hi)
+        check_moments(m, ref, a)
+        assert (b == rb).all() and (o == ro).all(), (nbins, lo, hi)
+        assert same_float(med, omed)
+        m, b, o, med = ctx.stats(t, nx, ny, nz, nbins, lo, hi, want_median=False)
+        assert med is None and (b == rb).all() and (o == ro).all()
+    for nbins in (64, 4096, 16385):                                           # histogram over [min,max]
+        m, b, o, med = ctx.stats(t, nx, ny, nz, nbins, flags=cube.SAMPLE_STD)
+        check_moments(m, oracle.moments(a, sample_std=True), a)
+        assert same_float(med, omed)
+        usable = ref["count"] > 0 and np.isfinite(ref["min"]) and np.isfinite(ref["max"])
+        if usable:
+            try:
+                rb, ro = oracle.histogram(a, nbins, float(ref["min"]), float(ref["max"]))
+            except ValueError:
+                usable = False
+        if usable:
+            assert (b == rb).all() and (o == ro).all() and int(b.sum()) == ref["count"], nbins
+        else:
+            assert not b.any() and (o == np.uint64(2 ** 64 - 1)).all()
 
 
 def std_ks(n):
@@ -143,6 +180,8 @@ def test_degenerate_cubes(ctx):
             assert same_float(ctx.median(t, a.size, 1, 1), oracle.median(a))
             for k in range(cnt):
                 assert same_float(ctx.kth(t, a.size, 1, 1, k), oracle.kth(a, k))
+            m, b, o, med = ctx.stats(t, a.size, 1, 1, 128)                    # [min,max] = [-inf,inf]: unusable
+            assert same_float(med, oracle.median(a)) and not b.any() and (o == np.uint64(2 ** 64 - 1)).all()
             continue
         ref = full_check(ctx, a, hists=hists, ks=std_ks(cnt))
         if cnt and float(fin.min()) == float(fin.max()):
@@ -279,6 +318,11 @@ def _config_case(ctx, cfg, hists, extra_ks=()):
         assert (b == rb).all() and (o == ro).all()
     med = ctx.median(t, nx, ny, nz)
     assert same_float(med, oracle.median(a))
+    for nbins, lo, hi in hists:                                               # the fused two-read path
+        m, b, o, smed = ctx.stats(t, nx, ny, nz, nbins, lo, hi)
+        check_moments(m, ref, a)
+        rb, ro = oracle.histogram(a, nbins, *((float(ref["min"]), float(ref["max"])) if lo is None else (lo, hi)))
+        assert (b == rb).all() and (o == ro).all() and same_float(smed, med)
     less, equal = oracle.rank_counts(a, med)
     kmed = (ref["count"] - 1) // 2
     assert equal >= 1 and less <= kmed < less + equal
@@ -350,6 +394,7 @@ def test_candidate_buffer_overflow_falls_back_to_a_third_pass():
     small = cube.Context(scratch_bytes_hint=4096)
     try:
         cases = [cubegen.generate_numpy(cubegen.scaled("c2", (64, 64, 128), nsrc=3)).reshape(-1),
+                 cubegen.generate_numpy(cubegen.scaled("c2", (128, 128, 128), nsrc=3)).reshape(-1),
                  np.full(300000, 0.25, np.float32),                       # every key in one bucket
                  cubegen.generate_numpy(cubegen.scaled("c4", (128, 128, 16))).reshape(-1)]
         for a in cases:
@@ -366,7 +411,14 @@ def test_candidate_buffer_overflow_falls_back_to_a_third_pass():
                 small.ooc_brick(t[half:], a.size - half)
                 more = small.ooc_next_sweep()
                 sweeps += 1
-            assert sweeps == 3
+            # the bucket = voxels sharing the top 11 bits of the median's order-preserving key; 3 sweeps iff it
+            # does not fit the 1024-key buffer
+            u = a[~np.isnan(a)].view(np.uint32)
+            key = np.where(u >> 31 == 1, ~u, u | np.uint32(0x80000000))
+            mu = np.array([oracle.median(a)], np.float32).view(np.uint32)
+            mkey = np.where(mu >> 31 == 1, ~mu, mu | np.uint32(0x80000000))[0]
+            bucket = int((key >> 21 == mkey >> 21).sum())
+            assert sweeps == (3 if bucket > 1024 else 2), (sweeps, bucket)
             assert same_float(small.ooc_result(0)[3], oracle.median(a))
     finally:
         small.close()
