@@ -6,7 +6,7 @@
  *     min/max "calculated while the dataset is loading"
  *   - global intensity histogram                                                PAPER.md:257-261 (sec. 4.1, Fig. 4)
  *   - exact global median / k-th value                                          PAPER.md:277-296 (sec. 4.3),
- *     Alg. 1; here reached by a 11/11/10-bit radix select on
+ *     Alg. 1; here reached by a 13/10/9-bit radix select on
  *     order-preserving keys instead of ~31 bisection passes
  *   - NULL (undefined) voxels are excluded from every statistic
  *     (NULL == IEEE NaN of any sign/payload, reading R6)
@@ -56,7 +56,7 @@ enum {
 enum {
     CUBE_SAMPLE_STD = 1u,  /* std = sqrt(M2/(n-1)) instead of the population sqrt(M2/n); n==1 -> NaN */
     CUBE_COARSE_HIST = 2u, /* cube_moments: also accumulate the first radix-select digit histogram
-                              (2048 bins of key>>21) in the same pass and keep it in the context */
+                              (8192 bins of key>>19) in the same pass and keep it in the context */
     CUBE_REUSE_COARSE = 4u,/* cube_kth_ex/cube_median_ex: skip the first select pass and use the digit
                               histogram left by the last cube_moments(CUBE_COARSE_HIST) or cube_stats(median)
                               call on the SAME data (the caller vouches for that) */

@@ -60,7 +60,7 @@ constexpr int kMaxCtasPerSm = 8;
 constexpr int kSmemHistMaxBins = 16384;  // 64 KiB of 32-bit counters per CTA
 // dynamic shared memory of hist_select_kernel: histogram + trash, digit bins + trash, stage slices + counters
 constexpr int hist_select_smem(int nbins) {
-    return (nbins + 1 + kDigitBins + 1 + (kThreads / 32) * ((int)kStageCap + 1)) * (int)sizeof(uint32_t);
+    return (nbins + 1 + kBins1 + 1 + (kThreads / 32) * ((int)kStageCap + 1)) * (int)sizeof(uint32_t);
 }
 
 #define CUBE_CUDA(ctx, call)                              \

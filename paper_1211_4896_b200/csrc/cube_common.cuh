@@ -31,12 +31,24 @@ __device__ __forceinline__ uint32_t key_of(float x) {
     uint32_t u = __float_as_uint(x);
     return u ^ ((uint32_t)((int32_t)u >> 31) | 0x80000000u);
 }
-// First radix digit (key >> 21, 11 bits) <-> raw top 11 bits of the float (bits >> 21): a
-// bijection (raw_of_digit maps digit -> raw), so a histogram indexed by the raw bits holds the same counts in
-// permuted order.
-__device__ __forceinline__ uint32_t raw_digit(float x) { return __float_as_uint(x) >> 21; }
+// Radix digits of the exact select: 13 + 10 + 9 bits of the order-preserving key.  A wide first
+// digit makes the median's bucket small (sign + exponent + 4 mantissa bits: ~0.08 % of config 2), which is what
+// the second pass has to revisit and compact.
+constexpr int kBits0 = 13, kBits1 = 10, kBits2 = 9;
+constexpr int kShift0 = 32 - kBits0;          // 19: key >> kShift0 is the first digit
+constexpr int kBins0 = 1 << kBits0, kBins1 = 1 << kBits1, kBins2 = 1 << kBits2;
+constexpr int kDigitBins = kBins0;            // size of the global digit arrays
+static_assert(kBits0 + kBits1 + kBits2 == 32, "digits must cover the key");
+// First digit (key >> 19) <-> raw top 13 bits of the float (bits >> 19): a bijection (raw_of_digit maps
+// digit -> raw), so a histogram indexed by the raw bits holds the same counts in permuted order.
+__device__ __forceinline__ uint32_t raw_digit(float x) { return __float_as_uint(x) >> kShift0; }
 __host__ __device__ __forceinline__ uint32_t raw_of_digit(uint32_t digit) {
-    return (digit & 0x400u) ? (digit ^ 0x400u) : (~digit & 0x7FFu);
+    constexpr uint32_t sign = 1u << (kBits0 - 1), all = (1u << kBits0) - 1u;
+    return (digit & sign) ? (digit ^ sign) : (~digit & all);
+}
+// NaN keys lie beyond +-inf, i.e. only in first-digit buckets whose raw exponent field is all ones.
+__host__ __device__ __forceinline__ bool digit_may_hold_nan(uint32_t digit) {
+    return ((raw_of_digit(digit) >> (kBits0 - 9)) & 0xFFu) == 0xFFu;
 }
 __host__ __device__ __forceinline__ uint32_t bits_of_key(uint32_t k) {
     return (k & 0x80000000u) ? (k ^ 0x80000000u) : ~k;
@@ -98,12 +110,15 @@ __device__ __forceinline__ void stream_cube(const float* __restrict__ d, uint64_
 // instead of once per voxel.
 __device__ __forceinline__ uint32_t smem_addr(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
 
-// Predicated shared-memory increment: counter at byte address `saddr` += 1 when `p`.  Written in PTX so
-// that the compiler keeps it a predicated RED (SASS ATOMS.POPC.INC, which the hardware aggregates over
-// lanes hitting the same address) instead of a divergent branch around it.
-__device__ __forceinline__ void smem_inc_if(uint32_t saddr, bool p) {
-    asm volatile("{\n\t.reg .pred q;\n\tsetp.ne.u32 q, %1, 0;\n\t@q red.shared.add.u32 [%0], 1;\n\t}"
-                 :: "r"(saddr), "r"((uint32_t)p) : "memory");
+// Shared-memory counter increment, counter[idx] += 1 with `saddr` the shared-window address of counter[0].
+// The byte offset is formed as idx * c_four + saddr with the 4 read from constant memory, so that ptxas emits one
+// IMAD (FMA pipe) instead of a LEA: the kernels are limited by the half-rate ALU pipe (ncu:
+// sm__inst_executed_pipe_alu 60-70 %, profiles/), and the FMA pipe is idle.  The RED compiles to
+// ATOMS.POPC.INC, which the hardware aggregates over lanes that hit the same address.
+__constant__ uint32_t c_four = 4u;
+__device__ __forceinline__ void smem_inc(uint32_t saddr, uint32_t idx) {
+    asm volatile("{\n\t.reg .u32 a;\n\tmad.lo.u32 a, %0, %1, %2;\n\tred.shared.add.u32 [a], 1;\n\t}"
+                 :: "r"(idx), "r"(c_four), "r"(saddr) : "memory");
 }
 
 // Same static tiling over an array of 32-bit keys (the select's candidate buffer, 16-byte aligned).

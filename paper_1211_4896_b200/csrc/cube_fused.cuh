@@ -3,7 +3,7 @@
 //
 // cube_stats() needs every statistic of the paper's path at once, so it reads the cube
 // exactly twice -- the minimum for an exact selection with O(bins) memory:
-//   pass A  moments_kernel<COARSE>: count, min, max, pivoted fp64 sums + first radix digit (2048 bins);
+//   pass A  moments_kernel<COARSE>: count, min, max, pivoted fp64 sums + first radix digit (8192 bins);
 //           1-CTA scan picks the median's bucket;
 //   pass B  this kernel: intensity histogram (range given, or [min,max] read from pass A's result on the
 //           device) + second digit of the voxels in the bucket + their keys staged into the candidate buffer;
@@ -39,7 +39,7 @@ __device__ __forceinline__ void hist_select_run(const float* __restrict__ d, uin
     HistSelectF<H> f;
     f.h = h;
     const uint32_t top = st->prefix;
-    f.s.base = top << 21; f.s.rawbase = raw_of_digit(top) << 21; f.s.sbins = sbins;
+    f.s.base = top << kShift0; f.s.rawbase = raw_of_digit(top) << kShift0; f.s.sbins = sbins;
     f.s.init_stage(stage, cand, &st->cand_n, st->cand_cap);
     stream_cube<kThreads>(d, n, f);
     f.s.finish();
@@ -62,7 +62,7 @@ __device__ __forceinline__ bool hist_range(const MomentsOut* __restrict__ range_
     return !(isinf(width) || isinf(scale));
 }
 
-// Dynamic shared memory: [nbins + 1 histogram counters][kDigitBins + 1 digit counters][stage slices + counters].
+// Dynamic shared memory: [nbins + 1 histogram counters][kBins1 + 1 digit counters][stage slices + counters].
 __global__ void __launch_bounds__(kThreads, 3)
 hist_select_kernel(const float* __restrict__ d, uint64_t n, int nbins, float lo, float hi, float scale,
                    const MomentsOut* __restrict__ range_from, unsigned long long* __restrict__ gbins,
@@ -72,8 +72,8 @@ hist_select_kernel(const float* __restrict__ d, uint64_t n, int nbins, float lo,
     __shared__ uint32_t s_out[2];
     uint32_t* hbins = dyn_bins;
     uint32_t* sbins = dyn_bins + (nbins + 1);
-    uint32_t* stage = sbins + (kDigitBins + 1);
-    for (int i = threadIdx.x; i < nbins + 1 + kDigitBins + 1; i += kThreads) dyn_bins[i] = 0;
+    uint32_t* stage = sbins + (kBins1 + 1);
+    for (int i = threadIdx.x; i < nbins + 1 + kBins1 + 1; i += kThreads) dyn_bins[i] = 0;
     if (threadIdx.x < 2) s_out[threadIdx.x] = 0;
     __syncthreads();
     const bool range_ok = hist_range(range_from, nbins, lo, hi, scale);
@@ -93,7 +93,7 @@ hist_select_kernel(const float* __restrict__ d, uint64_t n, int nbins, float lo,
         const uint32_t c = hbins[i];
         if (c) atomicAdd(&gbins[i], (unsigned long long)c);
     }
-    for (int i = threadIdx.x; i < kDigitBins; i += kThreads) {
+    for (int i = threadIdx.x; i < kBins1; i += kThreads) {
         const uint32_t c = sbins[i];
         if (c) atomicAdd(&gdigits[i], (unsigned long long)c);
     }

@@ -32,7 +32,6 @@ struct SelectState {
     unsigned long long cand_cap;  // capacity of the candidate buffer, in keys
 };
 
-constexpr int kDigitBins = 2048;  // 11-bit digits (passes 0, 1); pass 2 uses the low 10 bits
 
 // ------------------------------------------------------------------------------------------------
 // Moments: steps 1-3 of SURVEY.md sec. 8(a) (+ 3b when COARSE): count, min, max, pivoted fp64 sums.
@@ -50,7 +49,7 @@ struct MomentsF {
     bool have = false;
     uint32_t n = 0;
     double pivot = 0.0, s = 0.0, q = 0.0;
-    uint32_t* sbins;  // COARSE: kDigitBins shared counters
+    uint32_t sbins;   // COARSE: shared-window address of kDigitBins + 1 counters
     __device__ __forceinline__ void core(float x) {
         const bool ok = (x == x);  // NaN == blanked voxel
         mn = fminf(mn, x);
@@ -60,7 +59,7 @@ struct MomentsF {
         s += dlt;
         q = fma(dlt, dlt, q);
         n += ok ? 1u : 0u;
-        if (COARSE) atomicAdd(&sbins[ok ? raw_digit(x) : kDigitBins], 1u);  // raw top bits; NaN -> trash counter
+        if (COARSE) smem_inc(sbins, ok ? raw_digit(x) : (uint32_t)kDigitBins);  // raw top bits; NaN -> trash
     }
     __device__ __forceinline__ void take_pivot(float x) {
         if (!have && x == x) { have = true; pivf = x; pivot = (double)x; }
@@ -116,7 +115,7 @@ moments_kernel(const float* __restrict__ d, uint64_t n, Partial* __restrict__ pa
     __shared__ uint32_t sbins[COARSE ? kDigitBins + 1 : 1];
     __shared__ bool is_last;
     MomentsF<COARSE> f;
-    f.sbins = sbins;
+    f.sbins = smem_addr(sbins);
     if (COARSE) {
         for (int i = threadIdx.x; i <= kDigitBins; i += kThreads) sbins[i] = 0;
         __syncthreads();
@@ -238,17 +237,18 @@ struct HistFastF {
     int top;
     uint32_t topbits;  // bits of (float)top
     uint32_t* sbins;   // nbins + 1 counters (last = trash)
+    uint32_t sbase;    // shared-window address of sbins
     uint32_t* s_out;   // shared {below, above}
     uint32_t below = 0, above = 0;  // unused (kept for hist_flush_outside); the cold path counts in s_out
     __device__ __forceinline__ void setup(float lo_, float hi_, float scale_, int nbins, uint32_t* sbins_,
                                           uint32_t* s_out_) {
         lo = lo_; hi = hi_; scale = scale_; top = nbins - 1; topbits = __float_as_uint((float)(nbins - 1));
-        sbins = sbins_; s_out = s_out_;
+        sbins = sbins_; sbase = smem_addr(sbins_); s_out = s_out_;
     }
     __device__ __forceinline__ uint32_t inc(float x) const {
         const float v = __fmul_rn(__fsub_rn(x, lo), scale);
         const uint32_t vb = __float_as_uint(v);
-        atomicAdd(&sbins[vb < topbits ? __float2int_rd(v) : top + 1], 1u);
+        smem_inc(sbase, vb < topbits ? (uint32_t)__float2int_rd(v) : (uint32_t)(top + 1));
         return vb;
     }
     // exact definition for a voxel the hot path sent to the trash counter

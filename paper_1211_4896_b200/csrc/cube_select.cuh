@@ -1,12 +1,12 @@
 // cube_select.cuh -- exact k-th value / median by radix select (steps 6-8 of SURVEY.md sec. 8(a)).
 //
 // The paper's Torben bisection (Alg. 1) counts the voxels below / above /
-// equal to one guess per pass, ~31 passes over the cube.  Here each pass counts 2048 (1024) sub-ranges of
-// the order-preserving uint32 key at once, so three digits (11/11/10 bits) fix all 32 bits exactly:
-//   PASS 0: digit = key>>21 over all non-NaN voxels;
-//   PASS 1: voxels with key>>21 == prefix: digit = (key>>10)&2047, and their keys are appended to the
+// equal to one guess per pass, ~31 passes over the cube.  Here each pass counts 8192 (1024, 512) sub-ranges of
+// the order-preserving uint32 key at once, so three digits (13/10/9 bits) fix all 32 bits exactly:
+//   PASS 0: digit = key>>19 over all non-NaN voxels;
+//   PASS 1: voxels with key>>19 == prefix: digit = (key>>9)&1023, and their keys are appended to the
 //           candidate buffer (step 8, "compaction");
-//   PASS 2: key>>10 == prefix: digit = key&1023, read from the candidate buffer -- so the cube is read
+//   PASS 2: key>>9 == prefix: digit = key&511, read from the candidate buffer -- so the cube is read
 //           twice, not three times.  If the bucket did not fit the buffer, PASS 2 streams the cube again.
 // Like the paper's choice the cube itself is never written.
 #pragma once
@@ -26,24 +26,24 @@ constexpr uint32_t kStageCap = kStageThresh + 32u * 4u * kUnroll;      // + one 
 constexpr int kStageBytes = (kThreads / 32) * (int)kStageCap * 4;      // 36 KiB per CTA
 
 // Per-voxel work, branch-free:
-//   PASS 0:  idx = NaN ? trash : bits >> 21 (the RAW top 11 bits; the scan kernel reads the bins in key order
+//   PASS 0:  idx = NaN ? trash : bits >> 19 (the RAW top 13 bits; the scan kernel reads the bins in key order
 //            through raw_of_digit(), so the key transform is not paid per voxel); ATOMS.POPC.INC
 //            (hardware-aggregated over equal addresses).  SHF, FSETP, SEL, LEA, ATOMS.
-//   PASS 1:  the voxel is in the prefix bucket iff (bits ^ rawbase) < 2^21: LOP3 per voxel, VIMNMX3 per pair,
+//   PASS 1:  the voxel is in the prefix bucket iff (bits ^ rawbase) < 2^19: LOP3 per voxel, VIMNMX3 per pair,
 //            one flag per 4-voxel row (~2 ALU instructions per voxel, NO shared-memory traffic).  Only the rows
 //            that hold a voxel of the bucket (the bucket is 0.05-3 % of the cube on the configs) are visited
 //            again by a cold path that re-loads the row (an L2 hit: its line has just been streamed), counts
-//            the digit (kk >> 10) and stages the key.  So pass 1 costs less issue bandwidth than pass 0.
-//   PASS 2 over the cube (only when the candidates did not fit): idx = min(key - (prefix << 10), 1024) sends every
+//            the digit (kk >> 9) and stages the key.  So pass 1 costs less issue bandwidth than pass 0.
+//   PASS 2 over the cube (only when the candidates did not fit): idx = min(key - (prefix << 9), 512) sends every
 //            voxel outside the bucket to the trash counter without a compare.
-//   NaN keys can only fall into the buckets next to +-inf (top digit 0-3 or 2044-2047); only then (NANCHK)
+//   NaN keys can only fall into the buckets beyond +-inf (digit_may_hold_nan); only then (NANCHK)
 //   is the x == x test compiled in.
 template <int PASS, bool NANCHK>
 struct SelectF {
-    static constexpr uint32_t kSpan = 1u << 21;
-    static constexpr uint32_t kTrash = (PASS == 2) ? 1024u : (uint32_t)kDigitBins;
-    uint32_t base;     // prefix << 21 (PASS 1) or prefix << 10 (PASS 2)
-    uint32_t* sbins;   // kDigitBins + 1 counters
+    static constexpr uint32_t kSpan = 1u << kShift0;
+    static constexpr uint32_t kTrash = (PASS == 2) ? (uint32_t)kBins2 : (uint32_t)kBins0;
+    uint32_t base;     // prefix << 19 (PASS 1) or prefix << 9 (PASS 2)
+    uint32_t* sbins;   // bins of this pass + 1 trash counter
     // PASS 1 compaction state
     bool compacting = false;    // false once the candidate buffer is known to be too small (or absent)
     uint32_t* s_cnt = nullptr;  // this warp's fill counter (shared memory)
@@ -52,16 +52,16 @@ struct SelectF {
     unsigned long long* cand_n = nullptr;
     unsigned long long cand_cap = 0;
 
-    // PASS 1 hot path: key >> 21 == prefix  <=>  bits >> 21 == raw_of_digit(prefix)  <=>  (bits ^ rawbase) < 2^21
+    // PASS 1 hot path: key >> 19 == prefix  <=>  bits >> 19 == raw_of_digit(prefix)  <=>  (bits ^ rawbase) < 2^19
     // (LOP3), reduced over each 4-voxel row with VIMNMX3; NaN voxels may flag a row, the cold path drops them.
-    uint32_t rawbase = 0;  // raw_of_digit(prefix) << 21
+    uint32_t rawbase = 0;  // raw_of_digit(prefix) << 19
     __device__ __forceinline__ uint32_t kk_of(float x) const {
         uint32_t kk = key_of(x) - base;
         if (NANCHK) kk = (x == x) ? kk : 0xFFFFFFFFu;
         return kk;
     }
     __device__ __forceinline__ void count(float x) {  // PASS 0 / PASS 2: every voxel increments a counter
-        if (PASS == 0) atomicAdd(&sbins[(x == x) ? raw_digit(x) : kTrash], 1u);
+        if (PASS == 0) smem_inc(smem_addr(sbins), (x == x) ? raw_digit(x) : kTrash);
         else atomicAdd(&sbins[min(kk_of(x), kTrash)], 1u);
     }
     __device__ __forceinline__ void key(uint32_t k) {  // PASS 2 over the candidate buffer (no NaN in it)
@@ -77,7 +77,7 @@ struct SelectF {
                                                  uint32_t* s_buf_) {
         const uint32_t kk = key_of(x) - base_;
         if (kk < kSpan && x == x) {
-            atomicAdd(&sbins_[kk >> 10], 1u);
+            atomicAdd(&sbins_[kk >> kBits2], 1u);
             if (s_cnt_) s_buf_[atomicAdd(s_cnt_, 1u)] = kk + base_;
         }
     }
@@ -154,8 +154,8 @@ template <int PASS, bool NANCHK>
 __device__ __forceinline__ void select_run(const float* __restrict__ d, uint64_t n, SelectState* __restrict__ st,
                                            uint32_t* sbins, uint32_t* stage, uint32_t* __restrict__ cand) {
     SelectF<PASS, NANCHK> f;
-    f.base = (PASS == 0) ? 0u : (PASS == 1) ? (st->prefix << 21) : (st->prefix << 10);
-    f.rawbase = (PASS == 1) ? (raw_of_digit(st->prefix) << 21) : 0u;
+    f.base = (PASS == 0) ? 0u : (PASS == 1) ? (st->prefix << kShift0) : (st->prefix << kBits2);
+    f.rawbase = (PASS == 1) ? (raw_of_digit(st->prefix) << kShift0) : 0u;
     f.sbins = sbins;
     if (PASS == 1) f.init_stage(stage, cand, &st->cand_n, st->cand_cap);
     // cand_n is final when PASS 2 runs: it follows PASS 1 on the same stream
@@ -168,19 +168,19 @@ template <int PASS>
 __global__ void __launch_bounds__(kThreads, 4)
 select_pass_kernel(const float* __restrict__ d, uint64_t n, SelectState* __restrict__ st,
                    unsigned long long* __restrict__ gdigits, uint32_t* __restrict__ cand) {
-    __shared__ uint32_t sbins[kDigitBins + 1];  // + trash counter
+    constexpr int NB = (PASS == 0) ? kBins0 : (PASS == 1) ? kBins1 : kBins2;
+    __shared__ uint32_t sbins[NB + 1];  // + trash counter
     __shared__ uint32_t stage[(PASS == 1) ? (kThreads / 32) * (kStageCap + 1) : 1];
-    for (int i = threadIdx.x; i <= kDigitBins; i += kThreads) sbins[i] = 0;
+    for (int i = threadIdx.x; i <= NB; i += kThreads) sbins[i] = 0;
     __syncthreads();
     if (PASS == 0) {
         select_run<0, true>(d, n, st, sbins, stage, cand);
     } else if (!st->invalid) {
-        const uint32_t top = (PASS == 1) ? st->prefix : (st->prefix >> 11);  // first digit of the bucket
-        if (top <= 3u || top >= 2044u) select_run<PASS, true>(d, n, st, sbins, stage, cand);
+        const uint32_t top = (PASS == 1) ? st->prefix : (st->prefix >> kBits1);  // first digit of the bucket
+        if (digit_may_hold_nan(top)) select_run<PASS, true>(d, n, st, sbins, stage, cand);
         else select_run<PASS, false>(d, n, st, sbins, stage, cand);
     }
     __syncthreads();
-    constexpr int NB = (PASS == 2) ? 1024 : kDigitBins;
     for (int i = threadIdx.x; i < NB; i += kThreads) {
         uint32_t c = sbins[i];
         if (c) atomicAdd(&gdigits[i], (unsigned long long)c);
@@ -192,15 +192,15 @@ select_pass_kernel(const float* __restrict__ d, uint64_t n, SelectState* __restr
 __global__ void __launch_bounds__(kThreads)
 select_cand_kernel(SelectState* __restrict__ st, unsigned long long* __restrict__ gdigits,
                    const uint32_t* __restrict__ cand) {
-    __shared__ uint32_t sbins[kDigitBins + 1];
-    for (int i = threadIdx.x; i <= kDigitBins; i += kThreads) sbins[i] = 0;
+    __shared__ uint32_t sbins[kBins2 + 1];
+    for (int i = threadIdx.x; i <= kBins2; i += kThreads) sbins[i] = 0;
     __syncthreads();
     SelectF<2, false> f;
-    f.base = st->prefix << 10;
+    f.base = st->prefix << kBits2;
     f.sbins = sbins;
     if (!st->invalid) stream_keys<kThreads>(cand, st->cand_n, f);
     __syncthreads();
-    for (int i = threadIdx.x; i < 1024; i += kThreads) {
+    for (int i = threadIdx.x; i < kBins2; i += kThreads) {
         uint32_t c = sbins[i];
         if (c) atomicAdd(&gdigits[i], (unsigned long long)c);
     }
@@ -212,19 +212,18 @@ select_cand_kernel(SelectState* __restrict__ st, unsigned long long* __restrict_
 template <int PASS>
 __global__ void __launch_bounds__(1024)
 select_scan_kernel(SelectState* __restrict__ st, unsigned long long* __restrict__ gdigits, int clear) {
-    constexpr int NB = (PASS == 2) ? 1024 : kDigitBins;
-    constexpr int BITS = (PASS == 2) ? 10 : 11;
+    constexpr int NB = (PASS == 0) ? kBins0 : (PASS == 1) ? kBins1 : kBins2;
+    constexpr int BITS = (PASS == 0) ? kBits0 : (PASS == 1) ? kBits1 : kBits2;
+    constexpr int PER = (NB >= 1024) ? NB / 1024 : 1;   // thread t owns bins [t*PER, t*PER+PER) (those below NB)
     __shared__ unsigned long long warp_tot[32];
     __shared__ unsigned long long s_k;
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
-    // thread t owns bins [t*PER, t*PER+PER)
-    constexpr int PER = NB / 1024;
-    unsigned long long c[PER > 0 ? PER : 1];
+    unsigned long long c[PER];
     unsigned long long mine = 0;
 #pragma unroll
     for (int j = 0; j < PER; ++j) {  // PASS 0 bins are indexed by the raw top bits of the float
         const uint32_t b = (uint32_t)(tid * PER + j);
-        c[j] = gdigits[PASS == 0 ? raw_of_digit(b) : b];
+        c[j] = (b < (uint32_t)NB) ? gdigits[PASS == 0 ? raw_of_digit(b) : b] : 0ull;
         mine += c[j];
     }
     unsigned long long incl = mine;
@@ -257,13 +256,14 @@ select_scan_kernel(SelectState* __restrict__ st, unsigned long long* __restrict_
     const unsigned long long k = s_k;
     unsigned long long excl = warp_tot[warp] + (incl - mine);
     const bool invalid = st->invalid != 0;
+    const uint32_t prefix = st->prefix;
     __syncthreads();
     if (!invalid) {
 #pragma unroll
         for (int j = 0; j < PER; ++j) {
             if (c[j] && excl <= k && k < excl + c[j]) {  // exactly one (thread, j) satisfies this
                 const uint32_t b = (uint32_t)(tid * PER + j);
-                const uint32_t pre = (PASS == 0) ? b : ((st->prefix << BITS) | b);
+                const uint32_t pre = (PASS == 0) ? b : ((prefix << BITS) | b);
                 st->prefix = pre;
                 st->k = k - excl;
                 if (PASS == 2) st->result = __uint_as_float(bits_of_key(pre));
@@ -274,9 +274,7 @@ select_scan_kernel(SelectState* __restrict__ st, unsigned long long* __restrict_
         st->result = __int_as_float(0x7fc00000);
     }
     if (clear) {  // leave the digit bins zeroed for the next pass
-#pragma unroll
-        for (int j = 0; j < PER; ++j) gdigits[tid * PER + j] = 0ull;
-        if (PASS == 2) gdigits[1024 + tid] = 0ull;
+        for (int i = tid; i < kDigitBins; i += 1024) gdigits[i] = 0ull;
     }
 }
 

@@ -411,13 +411,13 @@ def test_candidate_buffer_overflow_falls_back_to_a_third_pass():
                 small.ooc_brick(t[half:], a.size - half)
                 more = small.ooc_next_sweep()
                 sweeps += 1
-            # the bucket = voxels sharing the top 11 bits of the median's order-preserving key; 3 sweeps iff it
+            # the bucket = voxels sharing the top 13 bits of the median's order-preserving key; 3 sweeps iff it
             # does not fit the 1024-key buffer
             u = a[~np.isnan(a)].view(np.uint32)
             key = np.where(u >> 31 == 1, ~u, u | np.uint32(0x80000000))
             mu = np.array([oracle.median(a)], np.float32).view(np.uint32)
             mkey = np.where(mu >> 31 == 1, ~mu, mu | np.uint32(0x80000000))[0]
-            bucket = int((key >> 21 == mkey >> 21).sum())
+            bucket = int((key >> 19 == mkey >> 19).sum())
             assert sweeps == (3 if bucket > 1024 else 2), (sweeps, bucket)
             assert same_float(small.ooc_result(0)[3], oracle.median(a))
     finally:
