@@ -64,7 +64,7 @@ class ClockSampler:
         self.f = tempfile.NamedTemporaryFile("w+", suffix=".csv", delete=False)
         try:
             self.p = subprocess.Popen(["nvidia-smi", "-i", str(index), "--query-gpu=" + self.Q,
-                                       "--format=csv,noheader,nounits", "-lms", "100"],
+                                       "--format=csv,noheader,nounits", "-lms", "20"],
                                       stdout=self.f, stderr=subprocess.DEVNULL)
         except OSError:
             self.p = None
@@ -107,13 +107,28 @@ def replica_seed(seed, rank):
     return seed + 1000 * rank if rank else seed
 
 
-def oracle_sample(name, cfg, sample_voxels=1 << 24):
+_SAMPLE_CACHE = {}
+
+
+def sample_planes(cfg, sample_voxels):
+    nx, ny, nz = cfg["dims"]
+    return max(1, min(nz, sample_voxels // (nx * ny)))
+
+
+def oracle_sample(name, cfg, sample_voxels=1 << 24, a=None):
     """Time the CPU oracle (as it stands, single thread) on a bounded sample of the workload: the first
-    `planes` z-planes of the cube, generated by the numpy generator.  Returns (voxels/s, description)."""
+    `planes` z-planes of the cube -- `a` when the caller already holds those voxels (bench copies them from the
+    device cube it times), else generated here (CUDA generator when a device is present, numpy otherwise).
+    Returns (voxels/s, description, seconds)."""
     import oracle
     nx, ny, nz = cfg["dims"]
-    planes = max(1, min(nz, sample_voxels // (nx * ny)))    # default ~16 Mi voxels: ~10-20 s of oracle work
-    a = cubegen.generate_numpy(cfg, origin=(0, 0, 0), brick=(nx, ny, planes)).reshape(-1)
+    planes = sample_planes(cfg, sample_voxels)
+    if a is None:
+        key = (name, cfg["seed"], planes)
+        if key not in _SAMPLE_CACHE:
+            _SAMPLE_CACHE.clear()
+            _SAMPLE_CACHE[key] = generate_sample(cfg, planes)
+        a = _SAMPLE_CACHE[key]
     nb, lo, hi = HIST[name]
     t0 = time.perf_counter()
     m = oracle.moments(a)
@@ -127,6 +142,31 @@ def oracle_sample(name, cfg, sample_voxels=1 << 24):
     return a.size / dt, desc, dt
 
 
+def generate_sample(cfg, planes):
+    """First `planes` z-planes of the workload as a host float32 array (inputs only: cubegen)."""
+    nx, ny, nz = cfg["dims"]
+    try:
+        import torch
+        if torch.cuda.is_available():
+            t = torch.empty(nx * ny * planes, dtype=torch.float32, device="cuda")
+            cubegen.generate_device(cfg, t.data_ptr(), origin=(0, 0, 0), brick=(nx, ny, planes))
+            torch.cuda.synchronize()
+            return t.cpu().numpy()
+    except ImportError:
+        pass
+    planes = min(planes, max(1, (1 << 25) // (nx * ny)))     # numpy generator: keep it to ~32 Mi voxels
+    return cubegen.generate_numpy(cfg, origin=(0, 0, 0), brick=(nx, ny, planes)).reshape(-1)
+
+
+def reference_sample_voxels(args):
+    """Per-step sample of the oracle arm: ~120 s of single-thread oracle work (~40 Mvoxel/s for the three
+    operations) over the whole --steps/--warmup run, between 2^20 and 2^29 voxels per step."""
+    if args.ref_voxels:
+        return args.ref_voxels
+    per = int(5e9 / max(1, args.steps + (1 if args.warmup > 0 else 0)))
+    return max(1 << 20, min(1 << 29, per))
+
+
 def run_reference(args):
     """--impl reference: the oracle on the host cores, same metric/config, bounded sample per step."""
     rank = int(os.environ.get("RANK", "0"))
@@ -134,10 +174,11 @@ def run_reference(args):
         return 0
     name = args.config
     cfg = cubegen.CONFIGS[name]
-    oracle_sample(name, cfg, args.ref_voxels) if args.warmup > 0 else None     # one warm-up (page-in, build)
+    sv = reference_sample_voxels(args)
+    oracle_sample(name, cfg, sv) if args.warmup > 0 else None     # one warm-up (page-in, build)
     vals, secs, desc = [], [], ""
     for _ in range(max(1, args.steps)):
-        v, desc, dt = oracle_sample(name, cfg, args.ref_voxels)
+        v, desc, dt = oracle_sample(name, cfg, sv)
         vals.append(v)
         secs.append(dt)
     value = float(np.mean(vals))
@@ -164,20 +205,133 @@ def aggregate_over_ranks(dist, local_ms, local_units, device=None):
     return float(t.item()), float(u.item())
 
 
+def run_out_of_core(args):
+    """--config c5: 4096^3 (256 GiB) produced per 512^3 brick into pinned host staging buffers (generated on the
+    device from the seed, copied D2H on the fill stream) and streamed H2D through cube_stats_stream.  One step =
+    the whole job: moments + 4096-bin histogram + exact lower median over all 512 bricks."""
+    import torch
+    import paper_1211_4896_b200 as cube
+
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py needs a CUDA device: libcube has no CPU fallback")
+    if int(os.environ.get("WORLD_SIZE", "1")) > 1:
+        raise SystemExit("--config c5 is a single-GPU job")
+    torch.cuda.set_device(0)
+    name = "c5"
+    cfg = cubegen.CONFIGS[name]
+    nx, ny, nz = cfg["dims"]
+    n = nx * ny * nz
+    brick = (512, 512, 512)
+    bvox = brick[0] * brick[1] * brick[2]
+    origins = cubegen.brick_grid(cfg, brick)
+    nb, lo, hi = HIST[name]
+    scratch = torch.empty(bvox, dtype=torch.float32, device="cuda")
+    scr = [scratch, torch.empty(bvox, dtype=torch.float32, device="cuda")]
+    for org in origins:                        # per-brick source lists, cached outside the timed region
+        cubegen.sources_in_brick(cfg, org, brick)
+    ctx = cube.Context(scratch_bytes_hint=1 << 30)
+    nres = int(args.resident_gib * 2 ** 30) // (bvox * 4)
+    ctx.stream_workspace(bvox * 4, host_slots=4, resident_bytes=nres * bvox * 4)
+
+    # measured pinned H2D peak of this box: 512 MiB copies, two in flight
+    hp = torch.empty(bvox, dtype=torch.float32, pin_memory=True)
+    s1, s2 = torch.cuda.Stream(), torch.cuda.Stream()
+    d2 = torch.empty(bvox, dtype=torch.float32, device="cuda")
+    torch.cuda.synchronize()
+    t0 = time.perf_counter()
+    reps = 16
+    for i in range(reps):
+        with torch.cuda.stream(s1 if i & 1 else s2):
+            (scratch if i & 1 else d2).copy_(hp, non_blocking=True)
+    torch.cuda.synchronize()
+    h2d_peak = reps * bvox * 4 / (time.perf_counter() - t0) / 1e9
+    del hp, d2
+
+    # producer: brick generated on the device (gen stream, two scratch buffers) and copied D2H on the driver's
+    # fill stream, so that generating brick i+1 overlaps the D2H of brick i and the H2D of brick i-1
+    gen = torch.cuda.Stream()
+    ev_gen = [torch.cuda.Event(), torch.cuda.Event()]
+    ev_d2h = [torch.cuda.Event(), torch.cuda.Event()]
+    produced = [0]
+
+    def fill(b, sweep, h_dst, nvox, fs):
+        k = produced[0] & 1
+        produced[0] += 1
+        fst = torch.cuda.ExternalStream(fs)
+        gen.wait_event(ev_d2h[k])
+        cubegen.generate_device(cfg, scr[k].data_ptr(), origin=origins[b], brick=brick, stream=gen.cuda_stream)
+        ev_gen[k].record(gen)
+        fst.wait_event(ev_gen[k])
+        cubegen.to_host(h_dst, scr[k].data_ptr(), nvox, fs)
+        ev_d2h[k].record(fst)
+
+    results = []
+    secs = []
+    sampler = None
+    for it in range(args.warmup + args.steps):
+        if it == args.warmup:
+            sampler = ClockSampler(0)
+        l0 = ctx.launch_count
+        torch.cuda.synchronize()
+        t0 = time.perf_counter()
+        m, b, o, med, info = ctx.stats_stream(len(origins), bvox, n, fill, nb, lo, hi)
+        dt = time.perf_counter() - t0
+        if it >= args.warmup:
+            secs.append(dt)
+            results.append((m, med, info, ctx.launch_count - l0))
+    clocks = sampler.stop() if sampler else None
+    dt = float(np.mean(secs))
+    m, med, info, launches = results[-1]
+    h2d_gbs = info["h2d_bytes"] / dt / 1e9
+    cpu = None
+    if not args.no_cpu_baseline:
+        v, desc, cdt = oracle_sample(name, cfg, min(args.cpu_voxels, 1 << 28))
+        cpu = {"value": v, "unit": "voxels/s", "cores": 1, "kind": "oracle", "sample": desc, "seconds": cdt}
+    line = {"metric": METRIC, "value": n / dt, "unit": "voxels/s", "n_gpus": 1, "steps": args.steps,
+            "warmup": args.warmup, "ms_per_step": dt * 1e3, "higher_is_better": True, "scaling": "weak",
+            "vs_baseline": None, "dtype": "f32", "data": "synthetic",
+            "config": {"workload": workload_desc(name, cfg) + "; out of core: 512 bricks of 512^3, %d kept in HBM after "
+                                   "sweep 1, the rest produced and streamed again in sweep 2" % min(nres, len(origins)),
+                       "l2": "bricks (512 MiB) are larger than the 126 MB L2",
+                       "timer": "host perf_counter around the synchronous cube_stats_stream call"},
+            "e2e": {"value": n / dt, "unit": "voxels/s", "h2d_bytes_per_step": info["h2d_bytes"],
+                    "d2h_bytes_per_step": 40 + nb * 8 + 16 + 4, "note": "the job IS end to end: every brick crosses the "
+                    "host link inside the timed region"},
+            "gpu_launches": launches, "clocks": clocks,
+            "roofline": {"bound": "h2d", "kernel": "cudaMemcpyAsync H2D of the bricks (the kernels have ~100x slack)",
+                         "achieved": h2d_gbs, "peak": h2d_peak, "unit": "GB/s", "frac": h2d_gbs / h2d_peak,
+                         "traffic": None, "peak_source": "pinned H2D copy, 512 MiB x 16, two streams, measured in this run",
+                         "sweeps": info["sweeps"]},
+            "cpu_baseline": cpu,
+            "result_check": {"median": float(med), "count": m["count"], "mean": m["mean"], "std": m["std"],
+                             "min": float(m["min"]), "max": float(m["max"])}}
+    print(json.dumps(line))
+    return 0
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
-    ap.add_argument("--steps", type=int, default=20)
-    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--steps", type=int, default=None, help="timed steps (default 200; 1 for c5)")
+    ap.add_argument("--warmup", type=int, default=None, help="untimed warm-up steps (default 3; 1 for c5)")
     ap.add_argument("--config", default="c2", choices=sorted(cubegen.CONFIGS))
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
-    ap.add_argument("--ref-voxels", type=int, default=1 << 24,
-                    help="voxels of the bounded oracle sample (--impl reference / cpu_baseline)")
+    ap.add_argument("--ref-voxels", type=int, default=0,
+                    help="voxels of the bounded oracle sample per step of --impl reference (0 = sized from --steps)")
+    ap.add_argument("--cpu-voxels", type=int, default=1 << 29,
+                    help="voxels of the cpu_baseline sample (first z-planes of the timed device cube)")
+    ap.add_argument("--resident-gib", type=float, default=128.0, help="c5: GiB of bricks kept in HBM after sweep 1")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     args = ap.parse_args()
+    if args.steps is None:
+        args.steps = 1 if args.config == "c5" else 200
+    if args.warmup is None:
+        args.warmup = 1 if args.config == "c5" else 3
     if args.impl == "reference":
         return run_reference(args)
+    if args.config == "c5":
+        return run_out_of_core(args)
     args.warmup = max(args.warmup, 3)
 
     import torch
@@ -226,6 +380,9 @@ def main():
     def op_histogram():
         ctx.histogram(cube_t, nx, ny, nz, nb, lo, hi, bins=out_b, outside=out_o, stream=stream)
 
+    def op_histogram_256():                 # config 4 also asks for a 256-bin histogram (hot-bin contention)
+        ctx.histogram(cube_t, nx, ny, nz, 256, lo, hi, bins=out_b, outside=out_o, stream=stream)
+
     def op_median():
         ctx.median(cube_t, nx, ny, nz, out=out_f, stream=stream)
 
@@ -262,7 +419,10 @@ def main():
     # the three operations of the metric through their own entry points (each its own timed region)
     peak, peak_src = measured_peak()
     ops = {}
-    for nm, fn, bpv in (("moments", op_moments, 4.0), ("histogram", op_histogram, 4.0), ("median", op_median, 8.0)):
+    op_list = [("moments", op_moments, 4.0), ("histogram", op_histogram, 4.0), ("median", op_median, 8.0)]
+    if name == "c4":
+        op_list.append(("histogram_256", op_histogram_256, 4.0))
+    for nm, fn, bpv in op_list:
         for _ in range(3):
             fn()
         ms = timed(fn, args.steps)
@@ -336,7 +496,9 @@ def main():
 
     cpu = None
     if rank == 0 and world == 1 and not args.no_cpu_baseline:
-        v, desc, dt = oracle_sample(name, cubegen.CONFIGS[name])
+        planes = sample_planes(cfg, args.cpu_voxels)
+        a_host = cube_t[:nx * ny * planes].cpu().numpy()          # the very bytes the GPU path was timed on
+        v, desc, dt = oracle_sample(name, cfg, args.cpu_voxels, a=a_host)
         cpu = {"value": v, "unit": "voxels/s", "cores": 1, "kind": "oracle", "sample": desc, "seconds": dt}
 
     if rank == 0:

@@ -128,6 +128,12 @@ int cubegen_nan_plane(float* d, int64_t bx, int64_t by, int64_t z, cudaStream_t 
     return (int)cudaGetLastError();
 }
 
+// Copy a generated brick from its device buffer into (pinned) host memory on the stream -- used when the
+// consumer wants the cube in host memory (out-of-core configuration).
+int cubegen_to_host(float* h_dst, const float* d_src, uint64_t nvox, cudaStream_t stream) {
+    return (int)cudaMemcpyAsync(h_dst, d_src, nvox * sizeof(float), cudaMemcpyDeviceToHost, stream);
+}
+
 // Host evaluation of the same Philox source, to pin the integers against the numpy restatement.
 int cubegen_philox(uint32_t c0, uint32_t c1, uint32_t c2, uint32_t c3, uint32_t k0, uint32_t k1,
                    uint32_t* out4) {

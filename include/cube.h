@@ -49,7 +49,8 @@ enum {
     CUBE_EEMPTY = 2, /* reserved: not returned by the asynchronous calls (see cube_moments) */
     CUBE_ECUDA = 3,  /* a CUDA call failed; cube_last_cuda_error() gives the cudaError_t */
     CUBE_ERANGE = 4, /* reserved */
-    CUBE_ENOMEM = 5  /* host or device allocation failed in cube_create */
+    CUBE_ENOMEM = 5, /* host or device allocation failed */
+    CUBE_ECALLBACK = 6 /* the brick callback of cube_stats_stream returned non-zero */
 };
 
 /* flags */
@@ -146,6 +147,31 @@ int cube_host_workspace(cube_ctx* ctx, size_t resident_bytes /* 0 = never keep r
 int cube_stats_host(cube_ctx* ctx, const float* h_cube, int64_t nx, int64_t ny, int64_t nz, int nbins, float lo,
                     float hi, unsigned flags, cube_moments_t* moments, uint64_t* bins, uint64_t* outside,
                     float* median);
+
+/* Cube PRODUCED brick by brick (BASELINE.json config 5: 256 GiB, larger than HBM and than host memory; north_star
+ * (4)).  The cube is `nbricks` contiguous runs of voxels, `brick_vox` each (the last one total_vox - (nbricks-1) *
+ * brick_vox).  For every brick that has to cross the host link the driver calls
+ *     fill(user, brick, sweep, h_dst, nvox, fill_stream)
+ * on the calling thread; it must put the brick's nvox float32 voxels into the PINNED HOST buffer h_dst, either
+ * before returning or by work enqueued on fill_stream (e.g. a generator kernel plus a device-to-host copy); it
+ * returns 0, or non-zero to abort (CUBE_ECALLBACK).  The same brick must get the same bytes in every sweep.
+ * h_dst is one of `host_slots` staging buffers owned by the context; the driver blocks the calling thread
+ * until the slot's previous host-to-device copy has completed, so at most host_slots bricks are in flight.
+ * Pipeline per brick: fill (fill_stream) -> H2D (copy stream) into one of two device brick buffers -> kernels
+ * (work stream), all three overlapped.  Sweep 1: moments + histogram + first select digit; sweep 2: second
+ * digit + compaction; last digit on the candidates (3 sweeps only if the median's bucket does not fit the
+ * candidate buffer).  The first resident_bytes / brick bytes bricks are kept in HBM after sweep 1 and are not
+ * asked for again.  Results are those of cube_stats, bit for bit (mean/std to rounding: the merge order is
+ * brick order).  Outputs are HOST pointers; synchronises before returning.
+ * cube_stream_workspace() allocates (pinned host: host_slots * brick_bytes, 2 <= host_slots <= 8; device:
+ * 2 * brick_bytes + resident_bytes); cube_stats_stream() calls it with (brick size, 3, 0) when it has not been. */
+typedef int (*cube_fill_fn)(void* user, uint64_t brick, int sweep, float* h_dst, uint64_t nvox, cudaStream_t fill_stream);
+int cube_stream_workspace(cube_ctx* ctx, size_t brick_bytes, int host_slots, size_t resident_bytes);
+int cube_stats_stream(cube_ctx* ctx, uint64_t nbricks, uint64_t brick_vox, uint64_t total_vox, cube_fill_fn fill,
+                      void* user, int nbins, float lo, float hi, unsigned flags, cube_moments_t* moments,
+                      uint64_t* bins, uint64_t* outside, float* median);
+/* After cube_stats_stream: bytes copied host-to-device and number of sweeps over the bricks. */
+int cube_stream_info(const cube_ctx* ctx, uint64_t* h2d_bytes, int* sweeps);
 
 const char* cube_strerror(int code);
 int cube_last_cuda_error(const cube_ctx* ctx);

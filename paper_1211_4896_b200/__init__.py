@@ -18,14 +18,18 @@ import numpy as np
 _HERE = os.path.dirname(os.path.abspath(__file__))
 _LIBPATH = os.path.join(_HERE, "libcube.so")
 
-OK, EINVAL, EEMPTY, ECUDA, ERANGE, ENOMEM = 0, 1, 2, 3, 4, 5
+OK, EINVAL, EEMPTY, ECUDA, ERANGE, ENOMEM, ECALLBACK = 0, 1, 2, 3, 4, 5, 6
+# int fill(void* user, uint64_t brick, int sweep, float* h_dst, uint64_t nvox, cudaStream_t fill_stream)
+FILL_FN = ctypes.CFUNCTYPE(ctypes.c_int, ctypes.c_void_p, ctypes.c_uint64, ctypes.c_int, ctypes.c_void_p,
+                           ctypes.c_uint64, ctypes.c_void_p)
 SAMPLE_STD, COARSE_HIST, REUSE_COARSE, RANGE_MINMAX = 1, 2, 4, 8
 MAX_BINS = 65536
 
 # every symbol include/cube.h declares (checked by tests/test_abi.py)
 SYMBOLS = ["cube_create", "cube_destroy", "cube_moments", "cube_histogram", "cube_kth", "cube_kth_ex",
            "cube_median", "cube_median_ex", "cube_stats", "cube_probe_read", "cube_ooc_begin", "cube_ooc_brick", "cube_ooc_next_sweep",
-           "cube_ooc_result", "cube_host_workspace", "cube_stats_host", "cube_strerror",
+           "cube_ooc_result", "cube_host_workspace", "cube_stats_host", "cube_stream_workspace", "cube_stats_stream",
+           "cube_stream_info", "cube_strerror",
            "cube_last_cuda_error", "cube_set_launch", "cube_set_knob", "cube_launch_count",
            "cube_profile_enable", "cube_profile_reset", "cube_profile_read"]
 KNOB_CTAS_PER_SM, KNOB_BIGHIST = 0, 1
@@ -79,6 +83,9 @@ def load():
     L.cube_ooc_result.argtypes = [vp, cu, vp, vp, vp, vp, vp]
     L.cube_host_workspace.argtypes = [vp, sz, sz]
     L.cube_stats_host.argtypes = [vp, vp, i64, i64, i64, ci, f32, f32, cu, vp, vp, vp, vp]
+    L.cube_stream_workspace.argtypes = [vp, sz, ci, sz]
+    L.cube_stats_stream.argtypes = [vp, u64, u64, u64, FILL_FN, vp, ci, f32, f32, cu, vp, vp, vp, vp]
+    L.cube_stream_info.argtypes = [vp, ctypes.POINTER(u64), ctypes.POINTER(ci)]
     L.cube_strerror.argtypes = [ci]
     L.cube_strerror.restype = ctypes.c_char_p
     L.cube_last_cuda_error.argtypes = [vp]
@@ -237,6 +244,38 @@ class Context:
                                             ctypes.cast(ctypes.byref(m), ctypes.c_void_p), _ptr(b), _ptr(o),
                                             ctypes.cast(ctypes.byref(r), ctypes.c_void_p) if want_median else None))
         return m.as_dict(), b, o, np.float32(r.value)
+
+    # --- cube produced brick by brick by a callback (config 5) -------------------------------------------
+    def stream_workspace(self, brick_bytes, host_slots=3, resident_bytes=0):
+        self._check(self._L.cube_stream_workspace(self._h, brick_bytes, host_slots, resident_bytes))
+
+    def stats_stream(self, nbricks, brick_vox, total_vox, fill, nbins, lo, hi, flags=0, want_median=True):
+        """``fill(brick, sweep, h_dst, nvox, fill_stream)``: put the brick's voxels into the pinned host buffer at
+        address ``h_dst`` (now, or by work enqueued on the raw stream ``fill_stream``); return None/0, non-zero aborts.
+        -> (moments dict, bins, outside, median, info dict(h2d_bytes, sweeps))."""
+        err = []
+
+        def _cb(user, brick, sweep, h_dst, nvox, fs):
+            try:
+                return int(fill(int(brick), int(sweep), int(h_dst), int(nvox), int(fs or 0)) or 0)
+            except BaseException as e:      # never unwind through the C frames
+                err.append(e)
+                return 1
+        cb = FILL_FN(_cb)
+        m = MomentsT()
+        b = np.zeros(max(int(nbins), 1), dtype=np.uint64)
+        o = np.zeros(2, dtype=np.uint64)
+        r = ctypes.c_float(float("nan"))
+        rc = self._L.cube_stats_stream(self._h, nbricks, brick_vox, total_vox, cb, None, nbins, lo, hi, flags,
+                                       ctypes.cast(ctypes.byref(m), ctypes.c_void_p),
+                                       _ptr(b) if nbins else None, _ptr(o) if nbins else None,
+                                       ctypes.cast(ctypes.byref(r), ctypes.c_void_p) if want_median else None)
+        if err:
+            raise err[0]
+        self._check(rc)
+        hb, sw = ctypes.c_uint64(), ctypes.c_int()
+        self._check(self._L.cube_stream_info(self._h, ctypes.byref(hb), ctypes.byref(sw)))
+        return m.as_dict(), b, o, np.float32(r.value), dict(h2d_bytes=int(hb.value), sweeps=int(sw.value))
 
     # --- knobs -----------------------------------------------------------------------------------------
     def set_launch(self, ctas_per_sm):

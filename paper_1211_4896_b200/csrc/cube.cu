@@ -31,6 +31,7 @@ struct cube_ctx {
     SelectState* sel = nullptr;
     float* range3 = nullptr;               // (lo, hi, scale) resolved on the device by cube_stats
     float* probe_out = nullptr;            // cube_probe_read sink
+    uint32_t* flip = nullptr;              // hist_flip_kernel's hint for hist_packed_kernel
     uint32_t* cand = nullptr;              // candidate keys of the select (step 8)
     unsigned long long cand_cap = 0;       // in keys
     // out-of-core state (host side)
@@ -44,6 +45,15 @@ struct cube_ctx {
     cudaStream_t copy_stream = nullptr, work_stream = nullptr;
     cudaEvent_t ev_copied[2] = {nullptr, nullptr}, ev_consumed[2] = {nullptr, nullptr};
     void* pinned_results = nullptr;  // staging for cube_stats_host results
+    // brick-callback driver (cube_stats_stream): pinned staging ring the callback fills
+    static constexpr int kMaxStage = 8;
+    float* h_stage[kMaxStage] = {};
+    cudaEvent_t ev_filled[kMaxStage] = {}, ev_h2d_done[kMaxStage] = {};
+    int stage_slots = 0;
+    size_t stage_bytes = 0;
+    cudaStream_t fill_stream = nullptr;
+    uint64_t stream_h2d_bytes = 0;   // bytes that crossed the host link in the last cube_stats_stream call
+    int stream_sweeps = 0;
     int max_ctas = 0;
     // per-kernel timing (cube_profile_*)
     int prof_on = 0;
@@ -167,13 +177,15 @@ int launch_hist(cube_ctx* c, const float* d, uint64_t n, int nbins, float lo, fl
         hist_smem_kernel<<<grid, kThreads, smem, s>>>(d, n, nbins, lo, hi, scale, range3, c->gbins, outside);
     } else {
         // one CTA of 1024 threads per SM, 16-bit packed counters (128 KiB for 65536 bins)
-        const size_t smem = (size_t)((nbins + 1) / 2) * sizeof(uint32_t);
+        const size_t smem = (size_t)(kBigWords + 4) * sizeof(uint32_t);
         if (c->bighist == 1) {
             hist_dsm_kernel<<<c->num_sms & ~1, kBigThreads, (32768 + 1) * sizeof(uint32_t), s>>>(
                 d, n, nbins, lo, hi, scale, range3, c->gbins, outside);
         } else {
-            hist_packed_kernel<<<c->num_sms, kBigThreads, smem, s>>>(d, n, nbins, lo, hi, scale, range3, c->gbins,
-                                                                     outside);
+            if (nbins > kBigWords)   // performance hint: which half of the bin range gets the +1 increments
+                hist_flip_kernel<<<1, kBigThreads, 0, s>>>(d, n, nbins, lo, hi, scale, range3, c->flip);
+            hist_packed_kernel<<<c->num_sms, kBigThreads, smem, s>>>(d, n, nbins, lo, hi, scale, range3, c->flip,
+                                                                     c->gbins, outside);
         }
     }
     }
@@ -265,6 +277,8 @@ int cube_create(cube_ctx** out, size_t scratch_bytes_hint) {
     ok = ok && cudaMalloc(&c->sel, sizeof(SelectState)) == cudaSuccess;
     ok = ok && cudaMalloc(&c->range3, 4 * sizeof(float)) == cudaSuccess;
     ok = ok && cudaMalloc(&c->probe_out, sizeof(float)) == cudaSuccess;
+    ok = ok && cudaMalloc(&c->flip, sizeof(uint32_t)) == cudaSuccess;
+    ok = ok && cudaMemset(c->flip, 0, sizeof(uint32_t)) == cudaSuccess;
     ok = ok && cudaMemset(c->ticket, 0, sizeof(unsigned int)) == cudaSuccess;
     ok = ok && cudaMemset(c->gdigits, 0, kDigitBins * sizeof(unsigned long long)) == cudaSuccess;
     ok = ok && cudaMemset(c->coarse, 0, kDigitBins * sizeof(unsigned long long)) == cudaSuccess;
@@ -273,7 +287,7 @@ int cube_create(cube_ctx** out, size_t scratch_bytes_hint) {
     ok = ok && cudaFuncSetAttribute(hist_select_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize,
                                     hist_select_smem(kSmemHistMaxBins)) == cudaSuccess;
     ok = ok && cudaFuncSetAttribute(hist_packed_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                                    (CUBE_MAX_BINS / 2) * (int)sizeof(uint32_t)) == cudaSuccess;
+                                    (kBigWords + 4) * (int)sizeof(uint32_t)) == cudaSuccess;
     ok = ok && cudaFuncSetAttribute(hist_dsm_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize,
                                     (32768 + 1) * (int)sizeof(uint32_t)) == cudaSuccess;
     if (!ok) { cube_destroy(c); return CUBE_ENOMEM; }
@@ -289,10 +303,16 @@ int cube_destroy(cube_ctx* c) {
     if (!c) return CUBE_EINVAL;
     cudaFree(c->partials); cudaFree(c->ticket); cudaFree(c->acc); cudaFree(c->nvox_acc);
     cudaFree(c->mom_out); cudaFree(c->gbins); cudaFree(c->gdigits); cudaFree(c->coarse); cudaFree(c->sel);
-    cudaFree(c->range3); cudaFree(c->probe_out);
+    cudaFree(c->range3); cudaFree(c->probe_out); cudaFree(c->flip);
     cudaFree(c->cand);
     cudaFree(c->resident); cudaFree(c->chunk[0]); cudaFree(c->chunk[1]);
     if (c->pinned_results) cudaFreeHost(c->pinned_results);
+    for (int i = 0; i < cube_ctx::kMaxStage; ++i) {
+        if (c->h_stage[i]) cudaFreeHost(c->h_stage[i]);
+        if (c->ev_filled[i]) cudaEventDestroy(c->ev_filled[i]);
+        if (c->ev_h2d_done[i]) cudaEventDestroy(c->ev_h2d_done[i]);
+    }
+    if (c->fill_stream) cudaStreamDestroy(c->fill_stream);
     for (int i = 0; i < 2; ++i) {
         if (c->ev_copied[i]) cudaEventDestroy(c->ev_copied[i]);
         if (c->ev_consumed[i]) cudaEventDestroy(c->ev_consumed[i]);
@@ -436,6 +456,7 @@ const char* cube_strerror(int code) {
         case CUBE_ECUDA: return "CUDA error (see cube_last_cuda_error)";
         case CUBE_ERANGE: return "out of range";
         case CUBE_ENOMEM: return "allocation failed";
+        case CUBE_ECALLBACK: return "brick callback failed";
         default: return "unknown error";
     }
 }

@@ -225,7 +225,7 @@ struct HistF : HistBase {
 // for everything from the top bin upwards.  For such a voxel lo <= x <= hi is guaranteed (t = x - lo has the
 // sign of the exact difference, and x > hi implies v >= fl(fl(hi-lo) * scale) > nbins - 1 whenever hi > lo and
 // scale is a normal number, nbins <= 65536) and its bin is floor(v), no clamp.  Everything else goes to the
-// trash counter, and the 4-voxel rows that contain such a voxel are flagged (VIMNMX3 on vb) and revisited by
+// trash counter, and the 4-voxel rows that contain such a non-NaN voxel are flagged (FMNMX3 on v) and revisited by
 // a cold path that applies the exact definition (x < lo, x > hi, NaN, closed top bin).  On the ALU pipe --
 // the one that limits these kernels, 16 lanes/clk/SMSP -- that is ISETP + SEL + ~1 per voxel instead of
 // 2 FSETP + SEL + VIMNMX + FMNMX.  Not valid for hi == lo (scale 0): hist_use_fast().
@@ -245,11 +245,10 @@ struct HistFastF {
         lo = lo_; hi = hi_; scale = scale_; top = nbins - 1; topbits = __float_as_uint((float)(nbins - 1));
         sbins = sbins_; sbase = smem_addr(sbins_); s_out = s_out_;
     }
-    __device__ __forceinline__ uint32_t inc(float x) const {
+    __device__ __forceinline__ float inc(float x) const {
         const float v = __fmul_rn(__fsub_rn(x, lo), scale);
-        const uint32_t vb = __float_as_uint(v);
-        smem_inc(sbase, vb < topbits ? (uint32_t)__float2int_rd(v) : (uint32_t)(top + 1));
-        return vb;
+        smem_inc(sbase, __float_as_uint(v) < topbits ? (uint32_t)__float2int_rd(v) : (uint32_t)(top + 1));
+        return v;
     }
     // exact definition for a voxel the hot path sent to the trash counter
     static __device__ __forceinline__ void exact(float x, float lo, float hi, float scale, int top,
@@ -275,14 +274,19 @@ struct HistFastF {
         } while (rows);
     }
     __device__ __forceinline__ void operator()(float x) {
-        if (!(inc(x) < topbits)) exact(x, lo, hi, scale, top, topbits, sbins, s_out);
+        if (!(__float_as_uint(inc(x)) < topbits)) exact(x, lo, hi, scale, top, topbits, sbins, s_out);
     }
     __device__ __forceinline__ void batch(const float4 (&r)[kUnroll], const float4* __restrict__ p) {
+        // A row is revisited iff it holds a voxel with v >= nbins - 1 or v < 0 (sign bit: also -0.0).  The row
+        // maximum / minimum are taken with FMNMX, which ignores NaN operands: blanked voxels count nowhere, so NaN
+        // alone never sends a row to the cold path (config 3 scatters a NaN into 2 % of the rows).
+        const float topf = __uint_as_float(topbits);
         uint32_t rows = 0;
 #pragma unroll
         for (int j = 0; j < kUnroll; ++j) {
-            const uint32_t m = max(max(inc(r[j].x), inc(r[j].y)), max(inc(r[j].z), inc(r[j].w)));
-            rows |= (m >= topbits ? 1u : 0u) << j;
+            const float a = inc(r[j].x), b = inc(r[j].y), c = inc(r[j].z), e = inc(r[j].w);
+            const float mx = fmaxf(fmaxf(a, b), fmaxf(c, e)), mn = fminf(fminf(a, b), fminf(c, e));
+            rows |= ((mx >= topf || __float_as_int(mn) < 0) ? 1u : 0u) << j;
         }
         if (rows) cold(rows, p, lo, hi, scale, top, topbits, sbins, s_out);
     }
@@ -331,78 +335,7 @@ hist_smem_kernel(const float* __restrict__ d, uint64_t n, int nbins, float lo, f
     if (threadIdx.x < 2 && s_out[threadIdx.x]) atomicAdd(&goutside[threadIdx.x], (unsigned long long)s_out[threadIdx.x]);
 }
 
-// 16384 < nbins <= 65536: the counters of one CTA no longer fit shared memory as 32-bit words
-// (65536 * 4 B = 256 KiB > 227 KiB), so two 16-bit counters are packed per word (128 KiB, one CTA of
-// 1024 threads per SM) and every wrap of a 16-bit half is moved to the 64-bit global bin at once:
-//   even bin b (low half):  old = atomicAdd(w, 1);  low half wrapped iff (old & 0xFFFF) == 0xFFFF. The
-//       wrap carried +1 into the high half, so credit bins[b] += 65536, take the carry back with
-//       atomicSub(w, 0x10000), and treat both +-1 on the high half like any other change of it;
-//   odd bin b (high half):  old = atomicAdd(w, 0x10000);  wrapped iff (old >> 16) == 0xFFFF.
-// The high half is a mod-65536 counter whose every wrap up (credit +65536) and wrap down (debit -65536)
-// is observed by the atomic that caused it, so count = half + 65536 * (credits - debits) exactly,
-// whatever the interleaving; the global add is 64-bit two's complement.
 constexpr int kBigThreads = 1024;
-struct HistPackedF : HistBase {
-    uint32_t* sw;
-    unsigned long long* gbins;
-    // rare: the increment just applied to bin b wrapped its 16-bit half (old = word before the add)
-    __device__ __noinline__ void wrapped(int b, uint32_t old, uint32_t* w) {
-        atomicAdd(&gbins[b], 65536ull);
-        if (!(b & 1)) {
-            if (old == 0xFFFFFFFFu) atomicAdd(&gbins[b + 1], 65536ull);   // the carry wrapped the high half too
-            const uint32_t old2 = atomicSub(w, 0x10000u);                 // take the carry back
-            if (old2 < 0x10000u) atomicAdd(&gbins[b + 1], (unsigned long long)(-65536ll));  // ...wrapping it down
-        }
-    }
-    __device__ __forceinline__ void inc(float x) {
-        const bool in = (x >= lo) && (x <= hi);
-        const int b = bin_of(x);
-        const uint32_t sh = ((uint32_t)b & 1u) << 4;
-        uint32_t* w = &sw[in ? (b >> 1) : 0];
-        const uint32_t old = atomicAdd(w, in ? (1u << sh) : 0u);   // voxels out of range add 0 to word 0
-        if (in && ((old >> sh) & 0xFFFFu) == 0xFFFFu) wrapped(b, old, w);
-    }
-    __device__ __forceinline__ void operator()(float x) {
-        inc(x);
-        outside(x);
-    }
-    __device__ __forceinline__ void batch(const float4 (&r)[kUnroll], const float4*) {
-        float bmin = INFINITY, bmax = -INFINITY;
-#pragma unroll
-        for (int j = 0; j < kUnroll; ++j) {
-            inc(r[j].x); inc(r[j].y); inc(r[j].z); inc(r[j].w);
-            bmin = fminf(fminf(bmin, r[j].x), fminf(r[j].y, fminf(r[j].z, r[j].w)));
-            bmax = fmaxf(fmaxf(bmax, r[j].x), fmaxf(r[j].y, fmaxf(r[j].z, r[j].w)));
-        }
-        if (bmin < lo || bmax > hi) {
-#pragma unroll
-            for (int j = 0; j < kUnroll; ++j) { outside(r[j].x); outside(r[j].y); outside(r[j].z); outside(r[j].w); }
-        }
-    }
-};
-
-__global__ void __launch_bounds__(kBigThreads)
-hist_packed_kernel(const float* __restrict__ d, uint64_t n, int nbins, float lo, float hi, float scale,
-                   const float* __restrict__ range3,
-                   unsigned long long* __restrict__ gbins, unsigned long long* __restrict__ goutside) {
-    extern __shared__ uint32_t dyn_bins[];  // (nbins+1)/2 words
-    __shared__ uint32_t s_out[2];
-    const int nwords = (nbins + 1) >> 1;
-    for (int i = threadIdx.x; i < nwords; i += kBigThreads) dyn_bins[i] = 0;
-    if (threadIdx.x < 2) s_out[threadIdx.x] = 0;
-    __syncthreads();
-    if (range3) { lo = range3[0]; hi = range3[1]; scale = range3[2]; }
-    HistPackedF f;
-    f.lo = lo; f.hi = hi; f.scale = scale; f.top = nbins - 1; f.sw = dyn_bins; f.gbins = gbins;
-    stream_cube<kBigThreads>(d, n, f);
-    __syncthreads();
-    for (int i = threadIdx.x; i < nwords; i += kBigThreads) {
-        const uint32_t w = dyn_bins[i];
-        if (w & 0xFFFFu) atomicAdd(&gbins[2 * i], (unsigned long long)(w & 0xFFFFu));
-        if (w >> 16) atomicAdd(&gbins[2 * i + 1], (unsigned long long)(w >> 16));
-    }
-    hist_flush_outside(f, s_out, goutside);
-}
 
 // Alternative for 16384 < nbins <= 65536 (north_star (2)): a thread-block cluster of two CTAs on two SMs
 // holds the whole histogram as 32-bit counters in DISTRIBUTED shared memory -- bin b lives in CTA (b & 1)
@@ -484,5 +417,6 @@ probe_read_kernel(const float* __restrict__ d, uint64_t n, float* __restrict__ o
 
 }  // namespace cube
 
+#include "cube_hist_big.cuh"
 #include "cube_select.cuh"
 #include "cube_fused.cuh"

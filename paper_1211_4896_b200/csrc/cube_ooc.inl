@@ -164,3 +164,94 @@ int cube_stats_host(cube_ctx* c, const float* h, int64_t nx, int64_t ny, int64_t
 }
 
 }  // extern "C"
+
+// ------------------------------------------------------------------------------------------------
+// Brick-callback driver: the cube never exists as a whole, neither in HBM nor in host memory (config 5).
+// ------------------------------------------------------------------------------------------------
+extern "C" {
+
+int cube_stream_workspace(cube_ctx* c, size_t brick_bytes, int host_slots, size_t resident_bytes) {
+    if (!c || brick_bytes == 0 || host_slots < 2 || host_slots > cube_ctx::kMaxStage) return CUBE_EINVAL;
+    brick_bytes = (brick_bytes + 15) & ~(size_t)15;
+    int rc = cube_host_workspace(c, resident_bytes, brick_bytes);   // device side: 2 brick buffers (+ resident)
+    if (rc) return rc;
+    for (int i = 0; i < cube_ctx::kMaxStage; ++i) {
+        if (c->h_stage[i]) { cudaFreeHost(c->h_stage[i]); c->h_stage[i] = nullptr; }
+    }
+    c->stage_slots = 0; c->stage_bytes = 0;
+    for (int i = 0; i < host_slots; ++i) {
+        if (cudaMallocHost(&c->h_stage[i], brick_bytes) != cudaSuccess) { cudaGetLastError(); return CUBE_ENOMEM; }
+        if (!c->ev_filled[i]) CUBE_CUDA(c, cudaEventCreateWithFlags(&c->ev_filled[i], cudaEventDisableTiming));
+        if (!c->ev_h2d_done[i]) CUBE_CUDA(c, cudaEventCreateWithFlags(&c->ev_h2d_done[i], cudaEventDisableTiming));
+    }
+    if (!c->fill_stream) CUBE_CUDA(c, cudaStreamCreateWithFlags(&c->fill_stream, cudaStreamNonBlocking));
+    c->stage_slots = host_slots; c->stage_bytes = brick_bytes;
+    return CUBE_OK;
+}
+
+int cube_stats_stream(cube_ctx* c, uint64_t nbricks, uint64_t brick_vox, uint64_t total_vox, cube_fill_fn fill,
+                      void* user, int nbins, float lo, float hi, unsigned flags, cube_moments_t* moments,
+                      uint64_t* bins, uint64_t* outside, float* median) {
+    if (!c || !fill || nbricks == 0 || brick_vox == 0 || total_vox == 0 || total_vox > (1ull << 37)) return CUBE_EINVAL;
+    if ((nbricks - 1) * brick_vox >= total_vox || nbricks * brick_vox < total_vox) return CUBE_EINVAL;
+    const bool want_hist = bins != nullptr || outside != nullptr;
+    if (want_hist && (!bins || !outside)) return CUBE_EINVAL;
+    int rc;
+    if (c->stage_slots == 0 || c->stage_bytes < brick_vox * sizeof(float) || !c->chunk[0] ||
+        c->chunk_bytes < brick_vox * sizeof(float)) {
+        if ((rc = cube_stream_workspace(c, brick_vox * sizeof(float), 3, 0))) return rc;
+    }
+    const int want_median = median != nullptr;
+    cudaStream_t ws = c->work_stream, cs = c->copy_stream, fs = c->fill_stream;
+    if ((rc = cube_ooc_begin(c, want_hist ? nbins : 0, lo, hi, want_median, ws))) return rc;
+    const uint64_t nres = c->resident ? (c->resident_bytes / (brick_vox * sizeof(float))) : 0;  // bricks kept in HBM
+    c->stream_h2d_bytes = 0; c->stream_sweeps = 0;
+    int more = 1;
+    uint64_t moved = 0;   // bricks that went through the staging ring so far (slot = moved % slots, buffer = moved & 1)
+    for (int sweep = 0; more; ++sweep) {
+        for (uint64_t i = 0; i < nbricks; ++i) {
+            const uint64_t cnt = (i + 1 == nbricks) ? total_vox - i * brick_vox : brick_vox;
+            if (i < nres && sweep > 0) {                       // still in HBM from sweep 1
+                if ((rc = cube_ooc_brick(c, c->resident + i * brick_vox, cnt, ws))) return rc;
+                continue;
+            }
+            const int slot = (int)(moved % (uint64_t)c->stage_slots), b = (int)(moved & 1);
+            // back-pressure: the slot's previous H2D copy must have left the staging buffer
+            if (moved >= (uint64_t)c->stage_slots) CUBE_CUDA(c, cudaEventSynchronize(c->ev_h2d_done[slot]));
+            if (fill(user, i, sweep, c->h_stage[slot], cnt, fs) != 0) {
+                cudaDeviceSynchronize(); c->ooc_active = 0;
+                return CUBE_ECALLBACK;
+            }
+            CUBE_CUDA(c, cudaEventRecord(c->ev_filled[slot], fs));
+            float* dst = (i < nres) ? c->resident + i * brick_vox : c->chunk[b];
+            CUBE_CUDA(c, cudaStreamWaitEvent(cs, c->ev_filled[slot], 0));
+            if (i >= nres && moved >= 2) CUBE_CUDA(c, cudaStreamWaitEvent(cs, c->ev_consumed[b], 0));
+            CUBE_CUDA(c, cudaMemcpyAsync(dst, c->h_stage[slot], cnt * sizeof(float), cudaMemcpyHostToDevice, cs));
+            CUBE_CUDA(c, cudaEventRecord(c->ev_h2d_done[slot], cs));
+            CUBE_CUDA(c, cudaEventRecord(c->ev_copied[b], cs));
+            CUBE_CUDA(c, cudaStreamWaitEvent(ws, c->ev_copied[b], 0));
+            if ((rc = cube_ooc_brick(c, dst, cnt, ws))) return rc;
+            CUBE_CUDA(c, cudaEventRecord(c->ev_consumed[b], ws));
+            c->stream_h2d_bytes += cnt * sizeof(float);
+            ++moved;
+        }
+        if ((rc = cube_ooc_next_sweep(c, &more, ws))) return rc;
+        c->stream_sweeps = sweep + 1;
+    }
+    rc = cube_ooc_result(c, flags, moments, want_hist ? bins : nullptr, want_hist ? outside : nullptr, median, ws);
+    if (rc) return rc;
+    CUBE_CUDA(c, cudaStreamSynchronize(ws));
+    CUBE_CUDA(c, cudaStreamSynchronize(cs));
+    CUBE_CUDA(c, cudaStreamSynchronize(fs));
+    c->ooc_active = 0;
+    return CUBE_OK;
+}
+
+int cube_stream_info(const cube_ctx* c, uint64_t* h2d_bytes, int* sweeps) {
+    if (!c) return CUBE_EINVAL;
+    if (h2d_bytes) *h2d_bytes = c->stream_h2d_bytes;
+    if (sweeps) *sweeps = c->stream_sweeps;
+    return CUBE_OK;
+}
+
+}  // extern "C"

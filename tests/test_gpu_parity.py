@@ -452,3 +452,57 @@ def test_stats_host_matches_oracle(ctx, resident):
     assert (b == rb).all() and (o == ro).all()
     assert same_float(med, oracle.median(a))
     ctx.host_workspace(0, 1 << 20)
+
+
+@pytest.mark.parametrize("mode", ["gpu_fill", "cpu_fill", "resident_half", "ragged_last_brick"])
+def test_stats_stream_brick_callback(ctx, mode):
+    # config 5 scaled: 128^3 produced brick by brick (8 x 64^3) by a callback into pinned staging buffers;
+    # same integers as the oracle on the concatenated bricks, exact median in two sweeps
+    import ctypes
+    cfg = cubegen.scaled("c5", (128, 128, 128), nsrc=40)
+    brick = (64, 64, 64)
+    bvox = 64 ** 3
+    origins = cubegen.brick_grid(cfg, brick)
+    scratch = torch.empty(bvox, dtype=torch.float32, device="cuda")
+    host_bricks = []
+    for org in origins:
+        cubegen.generate_device(cfg, scratch.data_ptr(), origin=org, brick=brick)
+        torch.cuda.synchronize()
+        host_bricks.append(scratch.cpu().numpy().copy())
+    a = np.concatenate(host_bricks)
+    total = a.size
+    nbricks = len(origins)
+    if mode == "ragged_last_brick":                 # bricks of 100000 voxels over the same bytes, last one short
+        bvox = 100000
+        nbricks = (total + bvox - 1) // bvox
+    calls = []
+
+    def fill(b, sweep, h_dst, nvox, fs):
+        calls.append((b, sweep, nvox))
+        if mode == "gpu_fill":
+            cubegen.generate_to_host(cfg, h_dst, scratch.data_ptr(), origin=origins[b], brick=brick, stream=fs)
+        else:
+            src = a[b * bvox: b * bvox + nvox]
+            assert src.size == nvox
+            ctypes.memmove(h_dst, src.ctypes.data, nvox * 4)
+        return 0
+
+    ctx.stream_workspace(bvox * 4, host_slots=3, resident_bytes=(4 * bvox * 4 if mode == "resident_half" else 0))
+    m, b, o, med, info = ctx.stats_stream(nbricks, bvox, total, fill, 4096, -0.02, 0.5)
+    check_moments(m, oracle.moments(a), a)
+    rb, ro = oracle.histogram(a, 4096, -0.02, 0.5)
+    assert (b == rb).all() and (o == ro).all()
+    assert same_float(med, oracle.median(a))
+    assert info["sweeps"] == 2
+    moved = nbricks * 2 - (4 if mode == "resident_half" else 0)
+    assert len(calls) == moved and info["h2d_bytes"] == (2 * total - (4 * bvox if mode == "resident_half" else 0)) * 4
+    assert [c[0] for c in calls if c[1] == 0] == list(range(nbricks))
+    # a failing callback aborts with CUBE_ECALLBACK and the context stays usable
+    with pytest.raises(cube.CubeError) as e:
+        ctx.stats_stream(nbricks, bvox, total, lambda *args: 7, 4096, -0.02, 0.5)
+    assert e.value.code == cube.ECALLBACK
+    with pytest.raises(ZeroDivisionError):
+        ctx.stats_stream(nbricks, bvox, total, lambda *args: 1 // 0, 4096, -0.02, 0.5)
+    m2, b2, o2, med2, _ = ctx.stats_stream(nbricks, bvox, total, fill, 4096, -0.02, 0.5, want_median=False)
+    assert (b2 == rb).all() and m2["count"] == m["count"]
+    ctx.host_workspace(0, 1 << 20)
