@@ -61,6 +61,11 @@ def lib():
         L.oracle_torben_pick.restype = ctypes.c_float
         L.oracle_torben_median.argtypes = [fp, ctypes.c_uint64, fp,
                                            ctypes.POINTER(ctypes.c_double), ctypes.c_int]
+        mp = ctypes.POINTER(Moments)
+        L.oracle_clipped_moments.argtypes = [fp, ctypes.c_uint64, ctypes.c_float, ctypes.c_float, ctypes.c_int, mp]
+        L.oracle_sigma_clip.argtypes = [fp, ctypes.c_uint64, ctypes.c_double, ctypes.c_int, ctypes.c_int, mp, fp]
+        L.oracle_mad.argtypes = [fp, ctypes.c_uint64, fp, fp]
+        L.oracle_minimap.argtypes = [fp] + [ctypes.c_int64] * 6 + [ctypes.c_int, mp]
         _lib = L
     return _lib
 
@@ -144,3 +149,52 @@ def torben_median(a, max_trace=64):
     it = lib().oracle_torben_median(p, a.size, ctypes.byref(out),
                                     trace.ctypes.data_as(ctypes.POINTER(ctypes.c_double)), max_trace)
     return np.float32(out.value), it, trace[:max(0, min(it, max_trace))]
+
+
+def _mdict(m):
+    return dict(count=m.count, nan_count=m.nan_count, min=np.float32(m.min), max=np.float32(m.max),
+                mean=m.mean, std=m.std)
+
+
+def clipped_moments(a, lo, hi, sample_std=False):
+    """Moments of the voxels with lo <= x <= hi (float32 window); nan_count = everything left out."""
+    a, p = _arr(a)
+    m = Moments()
+    lib().oracle_clipped_moments(p, a.size, float(np.float32(lo)), float(np.float32(hi)), int(bool(sample_std)),
+                                 ctypes.byref(m))
+    return _mdict(m)
+
+
+def sigma_clip(a, kappa, max_iter, sample_std=False):
+    """Iterated kappa-sigma clipping about the mean.
+    -> (moments dict of the last pass, clipped passes made, (lo, hi) of the last window)."""
+    a, p = _arr(a)
+    m = Moments()
+    w = (ctypes.c_float * 2)()
+    it = lib().oracle_sigma_clip(p, a.size, float(kappa), int(max_iter), int(bool(sample_std)), ctypes.byref(m), w)
+    return _mdict(m), it, (np.float32(w[0]), np.float32(w[1]))
+
+
+def mad(a):
+    """-> (lower median, median absolute deviation |fl32(x - med)|).  PAPER.md:292."""
+    a, p = _arr(a)
+    med, out = ctypes.c_float(), ctypes.c_float()
+    lib().oracle_mad(p, a.size, ctypes.byref(med), ctypes.byref(out))
+    return np.float32(med.value), np.float32(out.value)
+
+
+def minimap(a, dims, part, sample_std=False):
+    """Statistical mini-map.  dims = (nx, ny, nz) with x fastest, part = (px, py, pz).
+    -> structured array [mz, my, mx] with fields count, nan_count, min, max, mean, std."""
+    a, p = _arr(a)
+    nx, ny, nz = dims
+    px, py, pz = part
+    assert a.size == nx * ny * nz
+    mx, my, mz = -(-nx // px), -(-ny // py), -(-nz // pz)
+    cells = (Moments * (mx * my * mz))()
+    rc = lib().oracle_minimap(p, nx, ny, nz, px, py, pz, int(bool(sample_std)), cells)
+    if rc != 0:
+        raise ValueError("oracle_minimap: invalid arguments")
+    dt = np.dtype([("count", "<u8"), ("nan_count", "<u8"), ("min", "<f4"), ("max", "<f4"), ("mean", "<f8"),
+                   ("std", "<f8")])
+    return np.frombuffer(bytes(cells), dtype=dt).reshape(mz, my, mx).copy()

@@ -26,6 +26,9 @@
 //                       #{x<m} <= k < #{x<m} + #{x==m}  (total order), independent of both
 //                       selection algorithms.
 //
+//   MAD / clipped moments / sigma clip / mini-map   (PAPER.md:292, 336,
+//                       344, 352-356): definitions stated at the functions near the end of this file.
+//
 // Parity pins (tests/test_oracle_*.py): closed forms (constant cube, ramp 0..N-1, two-value
 // cube), exact rational sums computed with Python big integers, brute-force full sort on
 // tiny cubes, power-of-two ramp histograms, Table 1 of the paper.  The only unpinned
@@ -257,6 +260,108 @@ int oracle_torben_median(const float* d, uint64_t N, float* out, double* trace, 
     }
     *out = oracle_torben_pick(Less, Equal, n, MaxLt, Guess, MinGt);
     return iter;
+}
+
+// ---------------------------------------------------------------------------------
+// NEXT-1: median absolute deviation and sigma-clipped moments.
+// The paper only names them: Torben's method "can be easily modified to address the median absolute
+// deviation (MAD)"; "Thresholding (Sigma-Clipping) techniques where a data threshold is
+// defined based on the estimated noise properties", the threshold being chosen from "the
+// previously discussed statistical data computation ... (e.g mean and standard deviation)".
+// Definitions taken (readings R21-R24):
+//   MAD      med = lower median of the non-NaN voxels; y_i = |fl32(x_i - med)| (one float32 subtraction,
+//            then the sign bit cleared); MAD = lower median of the non-NaN y_i (y is NaN only for
+//            x = med = +-Inf, which is dropped like a NULL voxel).
+//   clipped  moments (count, min, max, mean, std) of the voxels with lo <= x <= hi (closed window, the test
+//            made on x itself; NaN fails it); nan_count = N - count = everything left out.
+//   sigma clip (kappa, max_iter): m_0 = moments of all voxels; for i = 1..max_iter:
+//            lo_i = fl32(mean - kappa*std), hi_i = fl32(mean + kappa*std) with mean, std of m_{i-1}
+//            (product and sum rounded to double separately, then one rounding to float32);
+//            m_i = clipped moments over [lo_i, hi_i]; stop after the first i with count_i == count_{i-1}
+//            (that m_i is returned; it equals m_{i-1}), or when count_{i-1} == 0 or std_{i-1} is not finite.
+//            Windows are always formed from the PREVIOUS iteration's statistics and applied to the
+//            whole cube, so counts never increase.
+// ---------------------------------------------------------------------------------
+
+int oracle_clipped_moments(const float* d, uint64_t N, float lo, float hi, int sample_std,
+                           oracle_moments_t* out) {
+    std::vector<float> v;
+    for (uint64_t i = 0; i < N; ++i) {
+        float x = d[i];
+        if (x >= lo && x <= hi) v.push_back(x);   // NaN fails both comparisons
+    }
+    oracle_moments(v.data(), v.size(), sample_std, out);
+    out->nan_count = N - out->count;
+    return 0;
+}
+
+// Returns the number of clipped passes made (0 .. max_iter).
+int oracle_sigma_clip(const float* d, uint64_t N, double kappa, int max_iter, int sample_std,
+                      oracle_moments_t* out, float* window /* [2]: last window used, NaN if none */) {
+    oracle_moments_t m;
+    oracle_moments(d, N, sample_std, &m);
+    window[0] = window[1] = std::numeric_limits<float>::quiet_NaN();
+    int iters = 0;
+    while (iters < max_iter) {
+        if (m.count == 0 || !std::isfinite(m.std) || !std::isfinite(m.mean)) break;
+        volatile double w = kappa * m.std;             // rounded to double before the sum (no contraction)
+        volatile double dl = m.mean - w, dh = m.mean + w;
+        float lo = (float)dl, hi = (float)dh;
+        oracle_moments_t m2;
+        oracle_clipped_moments(d, N, lo, hi, sample_std, &m2);
+        window[0] = lo; window[1] = hi;
+        ++iters;
+        bool same = (m2.count == m.count);
+        m = m2;
+        if (same) break;
+    }
+    *out = m;
+    return iters;
+}
+
+// MAD.  Returns 1 when there is no non-NaN voxel (both outputs NaN).
+int oracle_mad(const float* d, uint64_t N, float* median_out, float* mad_out) {
+    float med;
+    if (oracle_median(d, N, &med)) {
+        *median_out = *mad_out = std::numeric_limits<float>::quiet_NaN();
+        return 1;
+    }
+    std::vector<float> y;
+    y.reserve(N);
+    for (uint64_t i = 0; i < N; ++i) {
+        float x = d[i];
+        if (is_nan(x)) continue;
+        volatile float t = x - med;                    // float32 subtraction
+        y.push_back(fabsf(t));                         // NaN (Inf - Inf) is dropped by oracle_median below
+    }
+    *median_out = med;
+    oracle_median(y.data(), y.size(), mad_out);
+    return 0;
+}
+
+// ---------------------------------------------------------------------------------
+// NEXT-2: the statistical mini-map (Fig. 7): "a scaled-down version
+// of the data cube ... each data point represents the data statistics of a bigger region in the real
+// dataset", partitions of px x py x pz voxels ("30x30x30 pixel").  Cell (cx,cy,cz) covers
+// x in [cx*px, min((cx+1)*px, nx)) and likewise in y and z (ragged last cells are simply smaller; reading
+// R25); its record is the moments of those voxels.  Map dims: mx = ceil(nx/px) etc., x fastest.
+// ---------------------------------------------------------------------------------
+int oracle_minimap(const float* d, int64_t nx, int64_t ny, int64_t nz, int64_t px, int64_t py, int64_t pz,
+                   int sample_std, oracle_moments_t* cells) {
+    if (nx <= 0 || ny <= 0 || nz <= 0 || px <= 0 || py <= 0 || pz <= 0) return 1;
+    const int64_t mx = (nx + px - 1) / px, my = (ny + py - 1) / py, mz = (nz + pz - 1) / pz;
+    std::vector<float> v;
+    for (int64_t cz = 0; cz < mz; ++cz)
+        for (int64_t cy = 0; cy < my; ++cy)
+            for (int64_t cx = 0; cx < mx; ++cx) {
+                v.clear();
+                for (int64_t z = cz * pz; z < std::min((cz + 1) * pz, nz); ++z)
+                    for (int64_t y = cy * py; y < std::min((cy + 1) * py, ny); ++y)
+                        for (int64_t x = cx * px; x < std::min((cx + 1) * px, nx); ++x)
+                            v.push_back(d[(z * ny + y) * nx + x]);
+                oracle_moments(v.data(), v.size(), sample_std, &cells[(cz * my + cy) * mx + cx]);
+            }
+    return 0;
 }
 
 }  // extern "C"
