@@ -173,6 +173,46 @@ int cube_stats_stream(cube_ctx* ctx, uint64_t nbricks, uint64_t brick_vox, uint6
 /* After cube_stats_stream: bytes copied host-to-device and number of sweeps over the bricks. */
 int cube_stream_info(const cube_ctx* ctx, uint64_t* h2d_bytes, int* sweeps);
 
+/* ---- NEXT-1: robust noise estimates for source finding.
+ *
+ * cube_mad: *median = lower median m of the non-NaN voxels (may be NULL), *mad = lower median of
+ *   y = |fl32(x - m)| over the non-NaN voxels (one float32 subtraction, sign cleared; R21) -- "easily
+ *   modified to address the median absolute deviation".  Two exact selections with the same
+ *   radix-select kernels, the second ranking y instead of x: four reads of the cube (three with
+ *   CUBE_REUSE_COARSE after cube_moments(CUBE_COARSE_HIST) / cube_stats on the same data).  No non-NaN voxel -> NaN. */
+int cube_mad(cube_ctx* ctx, const float* d, int64_t nx, int64_t ny, int64_t nz, unsigned flags, float* median,
+             float* mad, cudaStream_t stream);
+
+/* cube_clipped_moments: cube_moments over the voxels with lo <= x <= hi only (closed window, tested on x itself;
+ *   NaN fails it).  out->count = voxels in the window, out->nan_count = nx*ny*nz - count = everything left out.
+ *   lo > hi selects nothing (count 0, NaN statistics); NaN lo/hi -> CUBE_EINVAL. */
+int cube_clipped_moments(cube_ctx* ctx, const float* d, int64_t nx, int64_t ny, int64_t nz, float lo, float hi,
+                         unsigned flags, cube_moments_t* out, cudaStream_t stream);
+
+/* cube_sigma_clip: iterated kappa-sigma clipping about the mean (the "Sigma-Clipping" threshold of PAPER.md:336
+ *   chosen from mean and standard deviation; R22-R23).  m_0 = cube_moments; for i = 1..max_iter:
+ *     lo = fl32(mean - kappa*std), hi = fl32(mean + kappa*std) from m_{i-1} (double product, double sum, one
+ *     rounding to float32);  m_i = cube_clipped_moments over [lo, hi];
+ *   stops after the first pass whose count equals the previous count, or when count == 0 or std is not finite.
+ *   The whole loop stays on the device (no host synchronisation): max_iter + 1 launches over the cube are
+ *   enqueued, and those after convergence return at once.  *out = the last statistics, *iters = clipped passes
+ *   made (may be NULL), window[2] = the last window used, NaN if none (may be NULL).  All three may be device,
+ *   pinned or pageable host memory.  CUBE_SAMPLE_STD applies to every std, including those that form the windows.
+ *   0 <= kappa < inf, 0 <= max_iter <= 1000. */
+int cube_sigma_clip(cube_ctx* ctx, const float* d, int64_t nx, int64_t ny, int64_t nz, double kappa, int max_iter,
+                    unsigned flags, cube_moments_t* out, int* iters, float* window /* [2] */, cudaStream_t stream);
+
+/* ---- NEXT-2: the statistical mini-map (Fig. 7): one cube_moments_t per partition of
+ * px x py x pz voxels ("30x30x30 pixel"), cell (cx,cy,cz) covering x in [cx*px, min((cx+1)*px, nx)) and likewise
+ * in y and z (ragged last cells are smaller; R25).  cells[(cz*my + cy)*mx + cx] with mx = ceil(nx/px),
+ * my, mz from cube_minimap_dims().  `cells` must be memory the DEVICE can write (device or pinned host memory):
+ * the map is consumed on the device (the second trilinear lookup of PAPER.md:354), so records are written in
+ * place by the kernel.  One read of the cube.  flags: CUBE_SAMPLE_STD. */
+int cube_minimap_dims(int64_t nx, int64_t ny, int64_t nz, int64_t px, int64_t py, int64_t pz, int64_t* mx,
+                      int64_t* my, int64_t* mz);
+int cube_minimap(cube_ctx* ctx, const float* d, int64_t nx, int64_t ny, int64_t nz, int64_t px, int64_t py,
+                 int64_t pz, unsigned flags, cube_moments_t* cells, cudaStream_t stream);
+
 const char* cube_strerror(int code);
 int cube_last_cuda_error(const cube_ctx* ctx);
 
@@ -194,8 +234,8 @@ uint64_t cube_launch_count(const cube_ctx* ctx);
  * it off when timing whole steps).  cube_profile_read() synchronises the device, then returns the summed
  * duration and the number of launches of one kernel kind since the last cube_profile_reset(). */
 enum {
-    CUBE_K_MOMENTS = 0,        /* moments_kernel<false> */
-    CUBE_K_MOMENTS_COARSE = 1, /* moments_kernel<true>: moments + first select digit (pass A of cube_stats) */
+    CUBE_K_MOMENTS = 0,        /* moments_kernel<plain> */
+    CUBE_K_MOMENTS_COARSE = 1, /* moments_kernel<coarse>: moments + first select digit (pass A of cube_stats) */
     CUBE_K_HIST = 2,           /* histogram kernels */
     CUBE_K_SELECT_PASS0 = 3,   /* first digit over the cube */
     CUBE_K_SELECT_PASS1 = 4,   /* second digit + candidate compaction over the cube */
@@ -205,7 +245,9 @@ enum {
     CUBE_K_HIST_SELECT = 8,    /* hist_select_kernel (pass B of cube_stats) */
     CUBE_K_PROBE = 9,          /* cube_probe_read */
     CUBE_K_OTHER = 10,
-    CUBE_K_KINDS = 11
+    CUBE_K_MOMENTS_WINDOW = 11, /* moments_kernel<window>: cube_clipped_moments, cube_sigma_clip passes */
+    CUBE_K_MINIMAP = 12,        /* minimap_kernel */
+    CUBE_K_KINDS = 13
 };
 int cube_profile_enable(cube_ctx* ctx, int on);
 /* Read-only STREAM probe: streams nvox float32 voxels through the same loop as the statistics kernels with one

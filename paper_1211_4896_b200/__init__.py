@@ -31,10 +31,11 @@ SYMBOLS = ["cube_create", "cube_destroy", "cube_moments", "cube_histogram", "cub
            "cube_ooc_result", "cube_host_workspace", "cube_stats_host", "cube_stream_workspace", "cube_stats_stream",
            "cube_stream_info", "cube_strerror",
            "cube_last_cuda_error", "cube_set_launch", "cube_set_knob", "cube_launch_count",
-           "cube_profile_enable", "cube_profile_reset", "cube_profile_read"]
+           "cube_profile_enable", "cube_profile_reset", "cube_profile_read",
+           "cube_mad", "cube_clipped_moments", "cube_sigma_clip", "cube_minimap_dims", "cube_minimap"]
 KNOB_CTAS_PER_SM, KNOB_BIGHIST = 0, 1
 KIND_NAMES = ["moments", "moments_coarse", "histogram", "select_pass0", "select_pass1", "select_pass2",
-              "select_cand", "select_scan", "hist_select", "probe_read", "other"]
+              "select_cand", "select_scan", "hist_select", "probe_read", "other", "moments_window", "minimap"]
 
 
 class CubeError(RuntimeError):
@@ -52,6 +53,10 @@ class MomentsT(ctypes.Structure):
         return dict(count=int(self.count), nan_count=int(self.nan_count), min=np.float32(self.min),
                     max=np.float32(self.max), mean=float(self.mean), std=float(self.std))
 
+
+# record layout of cube_moments_t as a numpy dtype (mini-map cells)
+MINIMAP_DTYPE = np.dtype([("count", "<u8"), ("nan_count", "<u8"), ("min", "<f4"), ("max", "<f4"), ("mean", "<f8"),
+                          ("std", "<f8")])
 
 _lib = None
 
@@ -96,6 +101,12 @@ def load():
     L.cube_profile_enable.argtypes = [vp, ci]
     L.cube_profile_reset.argtypes = [vp]
     L.cube_profile_read.argtypes = [vp, ci, ctypes.POINTER(ctypes.c_double), ctypes.POINTER(u64)]
+    f64 = ctypes.c_double
+    L.cube_mad.argtypes = [vp, vp, i64, i64, i64, cu, vp, vp, vp]
+    L.cube_clipped_moments.argtypes = [vp, vp, i64, i64, i64, f32, f32, cu, vp, vp]
+    L.cube_sigma_clip.argtypes = [vp, vp, i64, i64, i64, f64, ci, cu, vp, vp, vp, vp]
+    L.cube_minimap_dims.argtypes = [i64] * 6 + [ctypes.POINTER(i64)] * 3
+    L.cube_minimap.argtypes = [vp, vp, i64, i64, i64, i64, i64, i64, cu, vp, vp]
     for name in SYMBOLS:
         getattr(L, name)
     _lib = L
@@ -204,6 +215,50 @@ class Context:
                                        ctypes.cast(ctypes.byref(r), ctypes.c_void_p) if want_median else None,
                                        stream))
         return m.as_dict(), (b if nbins else None), (o if nbins else None), (np.float32(r.value) if want_median else None)
+
+    # --- NEXT-1 / NEXT-2 ------------------------------------------------------------
+    def mad(self, d, nx, ny, nz, flags=0, median_out=None, mad_out=None, stream=0):
+        """cube_mad -> (median, MAD) on the host, or None when device/pinned outputs are given."""
+        if mad_out is not None:
+            self._check(self._L.cube_mad(self._h, _ptr(d), nx, ny, nz, flags, _ptr(median_out), _ptr(mad_out), stream))
+            return None
+        m, r = ctypes.c_float(), ctypes.c_float()
+        self._check(self._L.cube_mad(self._h, _ptr(d), nx, ny, nz, flags, ctypes.cast(ctypes.byref(m), ctypes.c_void_p),
+                                     ctypes.cast(ctypes.byref(r), ctypes.c_void_p), stream))
+        return np.float32(m.value), np.float32(r.value)
+
+    def clipped_moments(self, d, nx, ny, nz, lo, hi, flags=0, out=None, stream=0):
+        if out is not None:
+            self._check(self._L.cube_clipped_moments(self._h, _ptr(d), nx, ny, nz, lo, hi, flags, _ptr(out), stream))
+            return None
+        m = MomentsT()
+        self._check(self._L.cube_clipped_moments(self._h, _ptr(d), nx, ny, nz, lo, hi, flags,
+                                                 ctypes.cast(ctypes.byref(m), ctypes.c_void_p), stream))
+        return m.as_dict()
+
+    def sigma_clip(self, d, nx, ny, nz, kappa, max_iter, flags=0, out=None, iters=None, window=None, stream=0):
+        """cube_sigma_clip -> (moments dict, clipped passes made, (lo, hi) of the last window) on the host, or
+        None when device/pinned outputs are given."""
+        if out is not None:
+            self._check(self._L.cube_sigma_clip(self._h, _ptr(d), nx, ny, nz, kappa, max_iter, flags, _ptr(out),
+                                                _ptr(iters), _ptr(window), stream))
+            return None
+        m, it, w = MomentsT(), ctypes.c_int(), (ctypes.c_float * 2)()
+        self._check(self._L.cube_sigma_clip(self._h, _ptr(d), nx, ny, nz, kappa, max_iter, flags,
+                                            ctypes.cast(ctypes.byref(m), ctypes.c_void_p),
+                                            ctypes.cast(ctypes.byref(it), ctypes.c_void_p),
+                                            ctypes.cast(w, ctypes.c_void_p), stream))
+        return m.as_dict(), int(it.value), (np.float32(w[0]), np.float32(w[1]))
+
+    def minimap_dims(self, nx, ny, nz, px, py, pz):
+        mx, my, mz = ctypes.c_int64(), ctypes.c_int64(), ctypes.c_int64()
+        self._check(self._L.cube_minimap_dims(nx, ny, nz, px, py, pz, ctypes.byref(mx), ctypes.byref(my),
+                                              ctypes.byref(mz)))
+        return int(mx.value), int(my.value), int(mz.value)
+
+    def minimap(self, d, nx, ny, nz, px, py, pz, cells, flags=0, stream=0):
+        """cube_minimap: ``cells`` = device (or pinned) buffer of mx*my*mz records of 40 bytes (MINIMAP_DTYPE)."""
+        self._check(self._L.cube_minimap(self._h, _ptr(d), nx, ny, nz, px, py, pz, flags, _ptr(cells), stream))
 
     def probe_read(self, d, nvox, stream=0):
         self._check(self._L.cube_probe_read(self._h, _ptr(d), nvox, stream))

@@ -32,6 +32,8 @@ struct cube_ctx {
     float* range3 = nullptr;               // (lo, hi, scale) resolved on the device by cube_stats
     float* probe_out = nullptr;            // cube_probe_read sink
     uint32_t* flip = nullptr;              // hist_flip_kernel's hint for hist_packed_kernel
+    ClipState* clip = nullptr;             // sigma-clip loop state (NEXT-1)
+    float* center = nullptr;               // cube_mad: the median the deviations are taken from
     uint32_t* cand = nullptr;              // candidate keys of the select (step 8)
     unsigned long long cand_cap = 0;       // in keys
     // out-of-core state (host side)
@@ -142,21 +144,30 @@ inline bool hist_scale(int nbins, float lo, float hi, float* scale) {
     return true;
 }
 
-int launch_moments(cube_ctx* c, const float* d, uint64_t n, unsigned flags, int accumulate, cudaStream_t s) {
-    const bool coarse = (flags & CUBE_COARSE_HIST) != 0;
+// mode: kMomPlain / kMomCoarse / kMomWindow (window = (wlo, whi), or the context's ClipState when use_clip)
+int launch_moments(cube_ctx* c, const float* d, uint64_t n, unsigned flags, int accumulate, cudaStream_t s,
+                   int mode = -1, float wlo = 0.f, float whi = 0.f, bool use_clip = false) {
+    if (mode < 0) mode = (flags & CUBE_COARSE_HIST) ? kMomCoarse : kMomPlain;
+    const bool coarse = mode == kMomCoarse;
     int occ_m = 0;
-    if ((coarse ? cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ_m, moments_kernel<true>, kThreads, 0)
-                : cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ_m, moments_kernel<false>, kThreads, 0)) != cudaSuccess) occ_m = 1;
+    cudaError_t e = mode == kMomCoarse ? cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ_m, moments_kernel<kMomCoarse>, kThreads, 0)
+                  : mode == kMomWindow ? cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ_m, moments_kernel<kMomWindow>, kThreads, 0)
+                                       : cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ_m, moments_kernel<kMomPlain>, kThreads, 0);
+    if (e != cudaSuccess) occ_m = 1;
     const int grid = grid_for(c, 4, occ_m < kMaxCtasPerSm ? occ_m : kMaxCtasPerSm);
     if (coarse && !accumulate) CUBE_CUDA(c, cudaMemsetAsync(c->coarse, 0, kDigitBins * sizeof(unsigned long long), s));
     {
-    ProfScope prof(c, coarse ? CUBE_K_MOMENTS_COARSE : CUBE_K_MOMENTS, s);
+    ProfScope prof(c, coarse ? CUBE_K_MOMENTS_COARSE : mode == kMomWindow ? CUBE_K_MOMENTS_WINDOW : CUBE_K_MOMENTS, s);
+    const ClipState* clip = use_clip ? c->clip : nullptr;
     if (coarse) {
-        moments_kernel<true><<<grid, kThreads, 0, s>>>(d, n, c->partials, c->ticket, c->acc, c->nvox_acc,
-                                                       accumulate, flags, c->mom_out, c->coarse);
+        moments_kernel<kMomCoarse><<<grid, kThreads, 0, s>>>(d, n, c->partials, c->ticket, c->acc, c->nvox_acc,
+                                                             accumulate, flags, c->mom_out, c->coarse, 0.f, 0.f, nullptr);
+    } else if (mode == kMomWindow) {
+        moments_kernel<kMomWindow><<<grid, kThreads, 0, s>>>(d, n, c->partials, c->ticket, c->acc, c->nvox_acc,
+                                                             accumulate, flags, c->mom_out, c->coarse, wlo, whi, clip);
     } else {
-        moments_kernel<false><<<grid, kThreads, 0, s>>>(d, n, c->partials, c->ticket, c->acc, c->nvox_acc,
-                                                        accumulate, flags, c->mom_out, c->coarse);
+        moments_kernel<kMomPlain><<<grid, kThreads, 0, s>>>(d, n, c->partials, c->ticket, c->acc, c->nvox_acc,
+                                                            accumulate, flags, c->mom_out, c->coarse, 0.f, 0.f, nullptr);
     }
     }
     CUBE_CUDA(c, cudaGetLastError());
@@ -193,14 +204,14 @@ int launch_hist(cube_ctx* c, const float* d, uint64_t n, int nbins, float lo, fl
     return CUBE_OK;
 }
 
-template <int PASS>
+template <int PASS, bool DEV = false>
 int launch_select_pass(cube_ctx* c, const float* d, uint64_t n, cudaStream_t s) {
     int occ = 0;  // every CTA of the persistent grid must be resident (static tile dealing)
-    if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, select_pass_kernel<PASS>, kThreads, 0) != cudaSuccess) occ = 1;
+    if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, select_pass_kernel<PASS, DEV>, kThreads, 0) != cudaSuccess) occ = 1;
     const int grid = grid_for(c, 4, occ < kMaxCtasPerSm ? occ : kMaxCtasPerSm);
     {
         ProfScope prof(c, PASS == 0 ? CUBE_K_SELECT_PASS0 : PASS == 1 ? CUBE_K_SELECT_PASS1 : CUBE_K_SELECT_PASS2, s);
-        select_pass_kernel<PASS><<<grid, kThreads, 0, s>>>(d, n, c->sel, c->gdigits, c->cand);
+        select_pass_kernel<PASS, DEV><<<grid, kThreads, 0, s>>>(d, n, c->sel, c->gdigits, c->cand, c->center);
     }
     CUBE_CUDA(c, cudaGetLastError());
     return CUBE_OK;
@@ -230,22 +241,24 @@ int select_init(cube_ctx* c, uint64_t k, int use_median, cudaStream_t s) {
     return CUBE_OK;
 }
 
+// DEV: rank |fl32(x - *c->center)| instead of x (cube_mad)
+template <bool DEV = false>
 int kth_impl(cube_ctx* c, const float* d, uint64_t n, uint64_t k, int use_median, unsigned flags, float* out,
              cudaStream_t s) {
     int rc;
     if ((rc = select_init(c, k, use_median, s))) return rc;
-    if (flags & CUBE_REUSE_COARSE) {
+    if (!DEV && (flags & CUBE_REUSE_COARSE)) {
         if ((rc = launch_select_scan<0>(c, c->coarse, s))) return rc;
     } else {
         CUBE_CUDA(c, cudaMemsetAsync(c->gdigits, 0, kDigitBins * sizeof(unsigned long long), s));
-        if ((rc = launch_select_pass<0>(c, d, n, s))) return rc;
+        if ((rc = launch_select_pass<0, DEV>(c, d, n, s))) return rc;
         if ((rc = launch_select_scan<0>(c, c->gdigits, s))) return rc;
     }
-    if ((rc = launch_select_pass<1>(c, d, n, s))) return rc;
+    if ((rc = launch_select_pass<1, DEV>(c, d, n, s))) return rc;
     if ((rc = launch_select_scan<1>(c, c->gdigits, s))) return rc;
-    if ((rc = launch_select_pass<2>(c, d, n, s))) return rc;
+    if ((rc = launch_select_pass<2, DEV>(c, d, n, s))) return rc;
     if ((rc = launch_select_scan<2>(c, c->gdigits, s))) return rc;
-    CUBE_CUDA(c, cudaMemcpyAsync(out, &c->sel->result, sizeof(float), cudaMemcpyDefault, s));
+    if (out) CUBE_CUDA(c, cudaMemcpyAsync(out, &c->sel->result, sizeof(float), cudaMemcpyDefault, s));
     return CUBE_OK;
 }
 
@@ -278,6 +291,8 @@ int cube_create(cube_ctx** out, size_t scratch_bytes_hint) {
     ok = ok && cudaMalloc(&c->range3, 4 * sizeof(float)) == cudaSuccess;
     ok = ok && cudaMalloc(&c->probe_out, sizeof(float)) == cudaSuccess;
     ok = ok && cudaMalloc(&c->flip, sizeof(uint32_t)) == cudaSuccess;
+    ok = ok && cudaMalloc(&c->clip, sizeof(ClipState)) == cudaSuccess;
+    ok = ok && cudaMalloc(&c->center, sizeof(float)) == cudaSuccess;
     ok = ok && cudaMemset(c->flip, 0, sizeof(uint32_t)) == cudaSuccess;
     ok = ok && cudaMemset(c->ticket, 0, sizeof(unsigned int)) == cudaSuccess;
     ok = ok && cudaMemset(c->gdigits, 0, kDigitBins * sizeof(unsigned long long)) == cudaSuccess;
@@ -303,7 +318,7 @@ int cube_destroy(cube_ctx* c) {
     if (!c) return CUBE_EINVAL;
     cudaFree(c->partials); cudaFree(c->ticket); cudaFree(c->acc); cudaFree(c->nvox_acc);
     cudaFree(c->mom_out); cudaFree(c->gbins); cudaFree(c->gdigits); cudaFree(c->coarse); cudaFree(c->sel);
-    cudaFree(c->range3); cudaFree(c->probe_out); cudaFree(c->flip);
+    cudaFree(c->range3); cudaFree(c->probe_out); cudaFree(c->flip); cudaFree(c->clip); cudaFree(c->center);
     cudaFree(c->cand);
     cudaFree(c->resident); cudaFree(c->chunk[0]); cudaFree(c->chunk[1]);
     if (c->pinned_results) cudaFreeHost(c->pinned_results);
@@ -354,7 +369,7 @@ int cube_kth_ex(cube_ctx* c, const float* d, int64_t nx, int64_t ny, int64_t nz,
                 float* out, cudaStream_t s) {
     uint64_t n;
     if (!c || !d || !out || !dims_ok(nx, ny, nz, &n)) return CUBE_EINVAL;
-    return kth_impl(c, d, n, k, 0, flags, out, s);
+    return kth_impl<false>(c, d, n, k, 0, flags, out, s);
 }
 
 int cube_kth(cube_ctx* c, const float* d, int64_t nx, int64_t ny, int64_t nz, uint64_t k, float* out,
@@ -366,7 +381,7 @@ int cube_median_ex(cube_ctx* c, const float* d, int64_t nx, int64_t ny, int64_t 
                    cudaStream_t s) {
     uint64_t n;
     if (!c || !d || !out || !dims_ok(nx, ny, nz, &n)) return CUBE_EINVAL;
-    return kth_impl(c, d, n, 0, 1, flags, out, s);
+    return kth_impl<false>(c, d, n, 0, 1, flags, out, s);
 }
 
 int cube_median(cube_ctx* c, const float* d, int64_t nx, int64_t ny, int64_t nz, float* out, cudaStream_t s) {
@@ -435,6 +450,84 @@ int cube_stats(cube_ctx* c, const float* d, int64_t nx, int64_t ny, int64_t nz, 
         CUBE_CUDA(c, cudaMemcpyAsync(bins, c->gbins, (size_t)nbins * sizeof(uint64_t), cudaMemcpyDefault, s));
         CUBE_CUDA(c, cudaMemcpyAsync(outside, goutside, 2 * sizeof(uint64_t), cudaMemcpyDefault, s));
     }
+    return CUBE_OK;
+}
+
+int cube_mad(cube_ctx* c, const float* d, int64_t nx, int64_t ny, int64_t nz, unsigned flags, float* median,
+             float* mad, cudaStream_t s) {
+    uint64_t n;
+    if (!c || !d || !mad || !dims_ok(nx, ny, nz, &n)) return CUBE_EINVAL;
+    int rc;
+    if ((rc = kth_impl<false>(c, d, n, 0, 1, flags & CUBE_REUSE_COARSE, median, s))) return rc;
+    CUBE_CUDA(c, cudaMemcpyAsync(c->center, &c->sel->result, sizeof(float), cudaMemcpyDeviceToDevice, s));
+    return kth_impl<true>(c, d, n, 0, 1, 0u, mad, s);
+}
+
+int cube_clipped_moments(cube_ctx* c, const float* d, int64_t nx, int64_t ny, int64_t nz, float lo, float hi,
+                         unsigned flags, cube_moments_t* out, cudaStream_t s) {
+    uint64_t n;
+    if (!c || !d || !out || !dims_ok(nx, ny, nz, &n) || lo != lo || hi != hi) return CUBE_EINVAL;
+    int rc = launch_moments(c, d, n, flags & CUBE_SAMPLE_STD, 0, s, kMomWindow, lo, hi, false);
+    if (rc) return rc;
+    CUBE_CUDA(c, cudaMemcpyAsync(out, c->mom_out, sizeof(MomentsOut), cudaMemcpyDefault, s));
+    return CUBE_OK;
+}
+
+int cube_sigma_clip(cube_ctx* c, const float* d, int64_t nx, int64_t ny, int64_t nz, double kappa, int max_iter,
+                    unsigned flags, cube_moments_t* out, int* iters, float* window, cudaStream_t s) {
+    uint64_t n;
+    if (!c || !d || !out || !dims_ok(nx, ny, nz, &n)) return CUBE_EINVAL;
+    if (!(kappa >= 0.0) || !isfinite(kappa) || max_iter < 0 || max_iter > 1000) return CUBE_EINVAL;
+    ClipState h;
+    memset(&h, 0, sizeof(h));
+    h.lo = h.hi = nanf("");
+    CUBE_CUDA(c, cudaMemcpyAsync(c->clip, &h, sizeof(h), cudaMemcpyHostToDevice, s));
+    const unsigned mflags = flags & CUBE_SAMPLE_STD;
+    int rc = launch_moments(c, d, n, mflags, 0, s, kMomPlain);
+    if (rc) return rc;
+    for (int i = 0; i < max_iter; ++i) {
+        {
+            ProfScope prof(c, CUBE_K_OTHER, s);
+            clip_step_kernel<<<1, 1, 0, s>>>(c->mom_out, c->clip, kappa);
+        }
+        CUBE_CUDA(c, cudaGetLastError());
+        if ((rc = launch_moments(c, d, n, mflags, 0, s, kMomWindow, 0.f, 0.f, true))) return rc;
+    }
+    CUBE_CUDA(c, cudaMemcpyAsync(out, c->mom_out, sizeof(MomentsOut), cudaMemcpyDefault, s));
+    if (iters) CUBE_CUDA(c, cudaMemcpyAsync(iters, &c->clip->iters, sizeof(int), cudaMemcpyDefault, s));
+    if (window) CUBE_CUDA(c, cudaMemcpyAsync(window, &c->clip->lo, 2 * sizeof(float), cudaMemcpyDefault, s));
+    return CUBE_OK;
+}
+
+int cube_minimap_dims(int64_t nx, int64_t ny, int64_t nz, int64_t px, int64_t py, int64_t pz, int64_t* mx,
+                      int64_t* my, int64_t* mz) {
+    uint64_t n;
+    if (!dims_ok(nx, ny, nz, &n) || px <= 0 || py <= 0 || pz <= 0 || !mx || !my || !mz) return CUBE_EINVAL;
+    *mx = (nx + px - 1) / px; *my = (ny + py - 1) / py; *mz = (nz + pz - 1) / pz;
+    return CUBE_OK;
+}
+
+int cube_minimap(cube_ctx* c, const float* d, int64_t nx, int64_t ny, int64_t nz, int64_t px, int64_t py,
+                 int64_t pz, unsigned flags, cube_moments_t* cells, cudaStream_t s) {
+    MapGeom g;
+    if (!c || !d || !cells) return CUBE_EINVAL;
+    if (cube_minimap_dims(nx, ny, nz, px, py, pz, (int64_t*)&g.mx, (int64_t*)&g.my, (int64_t*)&g.mz)) return CUBE_EINVAL;
+    g.nx = nx; g.ny = ny; g.nz = nz; g.px = px; g.py = py; g.pz = pz;
+    g.cells_per_seg = px > kMapThreads ? 1 : kMapThreads / px;
+    g.nseg = (g.mx + g.cells_per_seg - 1) / g.cells_per_seg;
+    const long double ctas = (long double)g.nseg * (long double)g.my * (long double)g.mz;
+    if (ctas > 2147483647.0L) return CUBE_EINVAL;   // 1-D grid limit (cells of a few voxels on a huge cube)
+    cudaPointerAttributes at;   // the map is consumed on the device: records are written in place
+    if (cudaPointerGetAttributes(&at, cells) != cudaSuccess || at.type == cudaMemoryTypeUnregistered) {
+        cudaGetLastError();
+        return CUBE_EINVAL;
+    }
+    {
+        ProfScope prof(c, CUBE_K_MINIMAP, s);
+        minimap_kernel<<<(unsigned)(g.nseg * g.my * g.mz), kMapThreads, 0, s>>>(d, g, flags & CUBE_SAMPLE_STD,
+                                                                               reinterpret_cast<MomentsOut*>(cells));
+    }
+    CUBE_CUDA(c, cudaGetLastError());
     return CUBE_OK;
 }
 

@@ -168,19 +168,23 @@ __device__ __forceinline__ Partial partial_shfl_down(const Partial& p, int off) 
 }
 
 // Fixed-shape tree over the CTA: lanes (shuffle, offsets 16..1) then warps (first warp).  Result valid
-// in thread 0.  `scratch` holds kThreads/32 Partials of shared memory.
-__device__ __forceinline__ Partial partial_block_reduce(Partial p, Partial* scratch) {
+// in thread 0.  `scratch` holds THREADS/32 Partials of shared memory.
+template <int THREADS>
+__device__ __forceinline__ Partial partial_block_reduce_n(Partial p, Partial* scratch) {
 #pragma unroll
     for (int off = 16; off > 0; off >>= 1) p = partial_merge(p, partial_shfl_down(p, off));
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
     if (lane == 0) scratch[warp] = p;
     __syncthreads();
     if (warp == 0) {
-        p = (lane < kThreads / 32) ? scratch[lane] : partial_empty();
+        p = (lane < THREADS / 32) ? scratch[lane] : partial_empty();
 #pragma unroll
         for (int off = 16; off > 0; off >>= 1) p = partial_merge(p, partial_shfl_down(p, off));
     }
     return p;
+}
+__device__ __forceinline__ Partial partial_block_reduce(Partial p, Partial* scratch) {
+    return partial_block_reduce_n<kThreads>(p, scratch);
 }
 
 }  // namespace cube

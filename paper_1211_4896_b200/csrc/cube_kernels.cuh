@@ -42,19 +42,33 @@ struct SelectState {
 // Per voxel: FSETP, FSEL, 2 FMNMX (alu pipe), F2F (xu), 2 DADD + DFMA (fp64), 1 predicated IADD.
 // min/max use FMNMX, which ignores NaN operands and orders -0.0 < +0.0.
 // ------------------------------------------------------------------------------------------------
-template <bool COARSE>
+// MODE: kMomPlain, kMomCoarse (+ first select digit, step 3b) or kMomWindow (NEXT-1, clipped moments: only
+// voxels with wlo <= x <= whi take part -- the test is made on x itself and fails for NaN; one more FSETP + FSEL).
+constexpr int kMomPlain = 0, kMomCoarse = 1, kMomWindow = 2;
+template <int MODE>
 struct MomentsF {
+    static constexpr bool COARSE = (MODE == kMomCoarse);
     float mn = INFINITY, mx = -INFINITY;
     float pivf = 0.0f;
     bool have = false;
     uint32_t n = 0;
     double pivot = 0.0, s = 0.0, q = 0.0;
     uint32_t sbins;   // COARSE: shared-window address of kDigitBins + 1 counters
+    float wlo = -INFINITY, whi = INFINITY;  // kMomWindow
+    __device__ __forceinline__ bool taken(float x) const {
+        return (MODE == kMomWindow) ? (x >= wlo && x <= whi) : (x == x);  // NaN == blanked voxel
+    }
     __device__ __forceinline__ void core(float x) {
-        const bool ok = (x == x);  // NaN == blanked voxel
-        mn = fminf(mn, x);
-        mx = fmaxf(mx, x);
-        const float xs = ok ? x : pivf;  // a blanked voxel contributes d == 0
+        const bool ok = taken(x);
+        if (MODE == kMomWindow) {  // FMNMX ignores NaN operands: a voxel outside the window is fed as NaN
+            const float xw = ok ? x : __int_as_float(0x7fc00000);
+            mn = fminf(mn, xw);
+            mx = fmaxf(mx, xw);
+        } else {
+            mn = fminf(mn, x);
+            mx = fmaxf(mx, x);
+        }
+        const float xs = ok ? x : pivf;  // a voxel that is left out contributes d == 0
         const double dlt = (double)xs - pivot;
         s += dlt;
         q = fma(dlt, dlt, q);
@@ -62,11 +76,11 @@ struct MomentsF {
         if (COARSE) smem_inc(sbins, ok ? raw_digit(x) : (uint32_t)kDigitBins);  // raw top bits; NaN -> trash
     }
     __device__ __forceinline__ void take_pivot(float x) {
-        if (!have && x == x) { have = true; pivf = x; pivot = (double)x; }
+        if (!have && taken(x)) { have = true; pivf = x; pivot = (double)x; }
     }
     __device__ __forceinline__ void operator()(float x) { take_pivot(x); core(x); }
     __device__ __forceinline__ void batch(const float4 (&r)[kUnroll], const float4*) {
-        if (!have) {  // only until this thread has met its first non-NaN voxel
+        if (!have) {  // only until this thread has met its first voxel that takes part
 #pragma unroll
             for (int j = 0; j < kUnroll; ++j) { take_pivot(r[j].x); take_pivot(r[j].y); take_pivot(r[j].z); take_pivot(r[j].w); }
         }
@@ -103,19 +117,38 @@ __device__ __forceinline__ void moments_finalize(const Partial& t, uint64_t nvox
     *out = o;
 }
 
+// State of an iterated sigma clip (NEXT-1), kept on the device so that the loop
+// "statistics -> window -> clipped statistics" never crosses to the host.
+struct ClipState {
+    float lo, hi;                   // window of the pass about to run / last run (NaN before the first)
+    uint32_t done;                  // 1: converged or degenerate -- the remaining passes return at once
+    int iters;                      // clipped passes made
+    unsigned long long prev_count;  // count of the statistics the window was formed from
+};
+
 // acc : running Partial across calls (out-of-core bricks); merged in call order => deterministic.
 // nvox_acc : running voxel total.  When `accumulate` is 0 both are overwritten.
-template <bool COARSE>
+// kMomWindow: the window is (wlo, whi), or *clip when clip != nullptr (then a finished clip makes the kernel a no-op).
+template <int MODE>
 __global__ void __launch_bounds__(kThreads)
 moments_kernel(const float* __restrict__ d, uint64_t n, Partial* __restrict__ partials,
                unsigned int* __restrict__ ticket, Partial* __restrict__ acc,
                unsigned long long* __restrict__ nvox_acc, int accumulate, unsigned flags,
-               MomentsOut* __restrict__ out, unsigned long long* __restrict__ gdigits) {
+               MomentsOut* __restrict__ out, unsigned long long* __restrict__ gdigits,
+               float wlo, float whi, const ClipState* __restrict__ clip) {
+    constexpr bool COARSE = (MODE == kMomCoarse);
     __shared__ Partial scratch[kThreads / 32];
     __shared__ uint32_t sbins[COARSE ? kDigitBins + 1 : 1];
     __shared__ bool is_last;
-    MomentsF<COARSE> f;
+    MomentsF<MODE> f;
     f.sbins = smem_addr(sbins);
+    if (MODE == kMomWindow) {
+        if (clip) {
+            if (clip->done) return;  // uniform over the grid
+            wlo = clip->lo; whi = clip->hi;
+        }
+        f.wlo = wlo; f.whi = whi;
+    }
     if (COARSE) {
         for (int i = threadIdx.x; i <= kDigitBins; i += kThreads) sbins[i] = 0;
         __syncthreads();
@@ -156,6 +189,24 @@ moments_kernel(const float* __restrict__ d, uint64_t n, Partial* __restrict__ pa
         moments_finalize(m, tot, flags, out);
         *ticket = 0u;
     }
+}
+
+// One step of the sigma-clip loop, between two passes over the cube (1 thread): has the last pass
+// reproduced the count its window was formed from (converged)?  Otherwise form the next window
+//   lo = fl32(mean - kappa * std), hi = fl32(mean + kappa * std)
+// from the statistics of the last pass -- product and sum rounded to double separately (no FMA), one rounding
+// to float32 (R23).
+__global__ void clip_step_kernel(const MomentsOut* __restrict__ m, ClipState* __restrict__ st, double kappa) {
+    if (st->done) return;
+    const unsigned long long cnt = m->count;
+    if (st->iters > 0 && cnt == st->prev_count) { st->done = 1u; return; }
+    const double mean = m->mean, sd = m->std;
+    if (cnt == 0 || !isfinite(sd) || !isfinite(mean)) { st->done = 1u; return; }
+    const double w = __dmul_rn(kappa, sd);
+    st->lo = __double2float_rn(__dsub_rn(mean, w));
+    st->hi = __double2float_rn(__dadd_rn(mean, w));
+    st->prev_count = cnt;
+    st->iters += 1;
 }
 
 // Re-evaluate mean/std of the running partial with other flags (sample std) -- O(1).
@@ -420,3 +471,4 @@ probe_read_kernel(const float* __restrict__ d, uint64_t n, float* __restrict__ o
 #include "cube_hist_big.cuh"
 #include "cube_select.cuh"
 #include "cube_fused.cuh"
+#include "cube_minimap.cuh"

@@ -38,7 +38,10 @@ constexpr int kStageBytes = (kThreads / 32) * (int)kStageCap * 4;      // 36 KiB
 //            voxel outside the bucket to the trash counter without a compare.
 //   NaN keys can only fall into the buckets beyond +-inf (digit_may_hold_nan); only then (NANCHK)
 //   is the x == x test compiled in.
-template <int PASS, bool NANCHK>
+//   DEV (NEXT-1, median absolute deviation): the value that is ranked is y = |fl32(x - center)|
+//   instead of x (one FADD; the absolute value folds into the consumer as an operand modifier or a LOP).
+//   y is NaN exactly when x is (or for Inf - Inf), so the NaN handling carries over unchanged.
+template <int PASS, bool NANCHK, bool DEV = false>
 struct SelectF {
     static constexpr uint32_t kSpan = 1u << kShift0;
     static constexpr uint32_t kTrash = (PASS == 2) ? (uint32_t)kBins2 : (uint32_t)kBins0;
@@ -55,12 +58,17 @@ struct SelectF {
     // PASS 1 hot path: key >> 19 == prefix  <=>  bits >> 19 == raw_of_digit(prefix)  <=>  (bits ^ rawbase) < 2^19
     // (LOP3), reduced over each 4-voxel row with VIMNMX3; NaN voxels may flag a row, the cold path drops them.
     uint32_t rawbase = 0;  // raw_of_digit(prefix) << 19
+    float center = 0.0f;   // DEV
+    static __device__ __forceinline__ float xf(float x, float center_) {
+        return DEV ? fabsf(__fsub_rn(x, center_)) : x;
+    }
     __device__ __forceinline__ uint32_t kk_of(float x) const {
         uint32_t kk = key_of(x) - base;
         if (NANCHK) kk = (x == x) ? kk : 0xFFFFFFFFu;
         return kk;
     }
     __device__ __forceinline__ void count(float x) {  // PASS 0 / PASS 2: every voxel increments a counter
+        x = xf(x, center);
         if (PASS == 0) smem_inc(smem_addr(sbins), (x == x) ? raw_digit(x) : kTrash);
         else atomicAdd(&sbins[min(kk_of(x), kTrash)], 1u);
     }
@@ -69,7 +77,7 @@ struct SelectF {
     }
     __device__ __forceinline__ void operator()(float x) {  // single voxels: head / tail / ragged last tile
         if (PASS != 1) { count(x); return; }
-        take1(x, base, sbins, compacting ? s_cnt : nullptr, s_buf);
+        take1(xf(x, center), base, sbins, compacting ? s_cnt : nullptr, s_buf);
     }
     // Cold path of PASS 1 (static, arguments by value: the functor itself stays in registers): revisit the
     // flagged 4-voxel rows, count the second digit of the voxels of the bucket and stage their keys.
@@ -82,15 +90,15 @@ struct SelectF {
         }
     }
     static __device__ __noinline__ void cold(uint32_t rows, const float4* __restrict__ p, uint32_t base_,
-                                             uint32_t* sbins_, uint32_t* s_cnt_, uint32_t* s_buf_) {
+                                             uint32_t* sbins_, uint32_t* s_cnt_, uint32_t* s_buf_, float center_) {
         do {
             const int j = __ffs(rows) - 1;
             rows &= rows - 1;
             const float4 q = __ldcg(p + j * kThreads);  // L2 hit: the line has just been streamed
-            take1(q.x, base_, sbins_, s_cnt_, s_buf_);
-            take1(q.y, base_, sbins_, s_cnt_, s_buf_);
-            take1(q.z, base_, sbins_, s_cnt_, s_buf_);
-            take1(q.w, base_, sbins_, s_cnt_, s_buf_);
+            take1(xf(q.x, center_), base_, sbins_, s_cnt_, s_buf_);
+            take1(xf(q.y, center_), base_, sbins_, s_cnt_, s_buf_);
+            take1(xf(q.z, center_), base_, sbins_, s_cnt_, s_buf_);
+            take1(xf(q.w, center_), base_, sbins_, s_cnt_, s_buf_);
         } while (rows);
     }
     // all lanes of the warp: move the c staged keys to the candidate buffer
@@ -121,11 +129,11 @@ struct SelectF {
         uint32_t rows = 0;  // rows (float4) holding at least one voxel whose raw bits are in the bucket
 #pragma unroll
         for (int j = 0; j < kUnroll; ++j) {
-            const uint32_t m = min(min(__float_as_uint(r[j].x) ^ rawbase, __float_as_uint(r[j].y) ^ rawbase),
-                                   min(__float_as_uint(r[j].z) ^ rawbase, __float_as_uint(r[j].w) ^ rawbase));
+            const uint32_t m = min(min(__float_as_uint(xf(r[j].x, center)) ^ rawbase, __float_as_uint(xf(r[j].y, center)) ^ rawbase),
+                                   min(__float_as_uint(xf(r[j].z, center)) ^ rawbase, __float_as_uint(xf(r[j].w, center)) ^ rawbase));
             rows |= (m < kSpan ? 1u : 0u) << j;
         }
-        if (rows) cold(rows, p, base, sbins, compacting ? s_cnt : nullptr, s_buf);
+        if (rows) cold(rows, p, base, sbins, compacting ? s_cnt : nullptr, s_buf, center);
         if (compacting) {               // warp-uniform
             const uint32_t c = staged();
             if (c > kStageThresh) flush(c);
@@ -150,13 +158,15 @@ struct SelectF {
     }
 };
 
-template <int PASS, bool NANCHK>
+template <int PASS, bool NANCHK, bool DEV>
 __device__ __forceinline__ void select_run(const float* __restrict__ d, uint64_t n, SelectState* __restrict__ st,
-                                           uint32_t* sbins, uint32_t* stage, uint32_t* __restrict__ cand) {
-    SelectF<PASS, NANCHK> f;
+                                           uint32_t* sbins, uint32_t* stage, uint32_t* __restrict__ cand,
+                                           float center) {
+    SelectF<PASS, NANCHK, DEV> f;
     f.base = (PASS == 0) ? 0u : (PASS == 1) ? (st->prefix << kShift0) : (st->prefix << kBits2);
     f.rawbase = (PASS == 1) ? (raw_of_digit(st->prefix) << kShift0) : 0u;
     f.sbins = sbins;
+    f.center = center;
     if (PASS == 1) f.init_stage(stage, cand, &st->cand_n, st->cand_cap);
     // cand_n is final when PASS 2 runs: it follows PASS 1 on the same stream
     if (PASS == 2 && cand && st->cand_n <= st->cand_cap) stream_keys<kThreads>(cand, st->cand_n, f);
@@ -164,21 +174,24 @@ __device__ __forceinline__ void select_run(const float* __restrict__ d, uint64_t
     f.finish();
 }
 
-template <int PASS>
+// DEV: rank y = |fl32(x - *center)| (cube_mad); center is a device pointer (the median found just before).
+template <int PASS, bool DEV>
 __global__ void __launch_bounds__(kThreads, 4)
 select_pass_kernel(const float* __restrict__ d, uint64_t n, SelectState* __restrict__ st,
-                   unsigned long long* __restrict__ gdigits, uint32_t* __restrict__ cand) {
+                   unsigned long long* __restrict__ gdigits, uint32_t* __restrict__ cand,
+                   const float* __restrict__ center) {
     constexpr int NB = (PASS == 0) ? kBins0 : (PASS == 1) ? kBins1 : kBins2;
     __shared__ uint32_t sbins[NB + 1];  // + trash counter
     __shared__ uint32_t stage[(PASS == 1) ? (kThreads / 32) * (kStageCap + 1) : 1];
     for (int i = threadIdx.x; i <= NB; i += kThreads) sbins[i] = 0;
     __syncthreads();
+    const float ctr = DEV ? *center : 0.0f;
     if (PASS == 0) {
-        select_run<0, true>(d, n, st, sbins, stage, cand);
+        select_run<0, true, DEV>(d, n, st, sbins, stage, cand, ctr);
     } else if (!st->invalid) {
         const uint32_t top = (PASS == 1) ? st->prefix : (st->prefix >> kBits1);  // first digit of the bucket
-        if (digit_may_hold_nan(top)) select_run<PASS, true>(d, n, st, sbins, stage, cand);
-        else select_run<PASS, false>(d, n, st, sbins, stage, cand);
+        if (digit_may_hold_nan(top)) select_run<PASS, true, DEV>(d, n, st, sbins, stage, cand, ctr);
+        else select_run<PASS, false, DEV>(d, n, st, sbins, stage, cand, ctr);
     }
     __syncthreads();
     for (int i = threadIdx.x; i < NB; i += kThreads) {
