@@ -323,6 +323,7 @@ def main():
     ap.add_argument("--resident-gib", type=float, default=128.0, help="c5: GiB of bricks kept in HBM after sweep 1")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-next", action="store_true", help="skip the timings of the NEXT rows (MAD, clipping, mini-map)")
     args = ap.parse_args()
     if args.steps is None:
         args.steps = 1 if args.config == "c5" else 200
@@ -386,6 +387,25 @@ def main():
     def op_median():
         ctx.median(cube_t, nx, ny, nz, out=out_f, stream=stream)
 
+    # NEXT rows: MAD, clipped moments, sigma clipping, 30^3 statistical mini-map
+    out_w = torch.zeros(2, dtype=torch.float32, device=dev)
+    out_i = torch.zeros(1, dtype=torch.int32, device=dev)
+    part = (30, 30, 30)
+    mmx, mmy, mmz = ctx.minimap_dims(nx, ny, nz, *part)
+    out_cells = torch.zeros(mmx * mmy * mmz * 40, dtype=torch.uint8, device=dev)
+
+    def op_mad():
+        ctx.mad(cube_t, nx, ny, nz, median_out=out_f, mad_out=out_w[0:1], stream=stream)
+
+    def op_clipped():
+        ctx.clipped_moments(cube_t, nx, ny, nz, lo, hi, out=out_m, stream=stream)
+
+    def op_sigma_clip():
+        ctx.sigma_clip(cube_t, nx, ny, nz, 3.0, 5, out=out_m, iters=out_i, window=out_w, stream=stream)
+
+    def op_minimap():
+        ctx.minimap(cube_t, nx, ny, nz, part[0], part[1], part[2], out_cells, stream=stream)
+
     def barrier():
         if world > 1:
             dist.barrier()
@@ -428,6 +448,19 @@ def main():
         ms = timed(fn, args.steps)
         ops[nm] = {"ms": ms, "voxels_per_s": n / (ms * 1e-3), "algorithmic_bytes_per_voxel": bpv,
                    "algorithmic_gbs": bpv * n / (ms * 1e-3) / 1e9, "frac_of_peak": bpv * n / (ms * 1e-3) / 1e9 / peak}
+    if not args.no_next:
+        reps_n = max(3, args.steps // 4)
+        op_sigma_clip()
+        torch.cuda.synchronize()
+        clip_passes = int(out_i.item()) + 1          # the plain pass + the clipped passes actually made
+        for nm, fn, bpv in [("next_mad", op_mad, 16.0), ("next_clipped_moments", op_clipped, 4.0),
+                            ("next_sigma_clip_3sigma_max5", op_sigma_clip, 4.0 * clip_passes),
+                            ("next_minimap_30x30x30", op_minimap, 4.0)]:
+            for _ in range(2):
+                fn()
+            ms = timed(fn, reps_n)
+            ops[nm] = {"ms": ms, "voxels_per_s": n / (ms * 1e-3), "algorithmic_bytes_per_voxel": bpv,
+                       "algorithmic_gbs": bpv * n / (ms * 1e-3) / 1e9, "frac_of_peak": bpv * n / (ms * 1e-3) / 1e9 / peak}
     ops["stats_fused"] = {"ms": total_ms / args.steps, "voxels_per_s": total_units / (total_ms * 1e-3) / world,
                           "algorithmic_bytes_per_voxel": 8.0,
                           "algorithmic_gbs": 8.0 * n / (local_ms / args.steps * 1e-3) / 1e9,

@@ -31,7 +31,7 @@ struct cube_ctx {
     SelectState* sel = nullptr;
     float* range3 = nullptr;               // (lo, hi, scale) resolved on the device by cube_stats
     float* probe_out = nullptr;            // cube_probe_read sink
-    uint32_t* flip = nullptr;              // hist_flip_kernel's hint for hist_packed_kernel
+    BigHistPlan* plan = nullptr;           // hist_window_kernel's plan for the > 16384-bin histogram kernels
     ClipState* clip = nullptr;             // sigma-clip loop state (NEXT-1)
     float* center = nullptr;               // cube_mad: the median the deviations are taken from
     uint32_t* cand = nullptr;              // candidate keys of the select (step 8)
@@ -187,15 +187,22 @@ int launch_hist(cube_ctx* c, const float* d, uint64_t n, int nbins, float lo, fl
         const int grid = grid_for(c, 4, occ);
         hist_smem_kernel<<<grid, kThreads, smem, s>>>(d, n, nbins, lo, hi, scale, range3, c->gbins, outside);
     } else {
-        // one CTA of 1024 threads per SM, 16-bit packed counters (128 KiB for 65536 bins)
+        // one CTA of 1024 threads per SM: 32-bit counters for a 32768-bin window (default when the sampled plan
+        // allows it) or 16-bit packed counters for all bins; both are enqueued, the one not chosen returns at once
         const size_t smem = (size_t)(kBigWords + 4) * sizeof(uint32_t);
         if (c->bighist == 1) {
             hist_dsm_kernel<<<c->num_sms & ~1, kBigThreads, (32768 + 1) * sizeof(uint32_t), s>>>(
                 d, n, nbins, lo, hi, scale, range3, c->gbins, outside);
         } else {
-            if (nbins > kBigWords)   // performance hint: which half of the bin range gets the +1 increments
-                hist_flip_kernel<<<1, kBigThreads, 0, s>>>(d, n, nbins, lo, hi, scale, range3, c->flip);
-            hist_packed_kernel<<<c->num_sms, kBigThreads, smem, s>>>(d, n, nbins, lo, hi, scale, range3, c->flip,
+            hist_window_kernel<<<1, kBigThreads, 0, s>>>(d, n, nbins, lo, hi, scale, range3, c->plan);
+            const bool window_allowed = c->bighist != 2;
+            if (window_allowed) {
+                c->launches++;
+                hist_win_kernel<<<c->num_sms, kBigThreads, smem, s>>>(d, n, nbins, lo, hi, scale, range3, c->plan,
+                                                                      c->gbins, outside);
+            }
+            hist_packed_kernel<<<c->num_sms, kBigThreads, smem, s>>>(d, n, nbins, lo, hi, scale, range3, &c->plan->flip,
+                                                                     window_allowed ? &c->plan->use_window : nullptr,
                                                                      c->gbins, outside);
         }
     }
@@ -290,10 +297,10 @@ int cube_create(cube_ctx** out, size_t scratch_bytes_hint) {
     ok = ok && cudaMalloc(&c->sel, sizeof(SelectState)) == cudaSuccess;
     ok = ok && cudaMalloc(&c->range3, 4 * sizeof(float)) == cudaSuccess;
     ok = ok && cudaMalloc(&c->probe_out, sizeof(float)) == cudaSuccess;
-    ok = ok && cudaMalloc(&c->flip, sizeof(uint32_t)) == cudaSuccess;
+    ok = ok && cudaMalloc(&c->plan, sizeof(BigHistPlan)) == cudaSuccess;
     ok = ok && cudaMalloc(&c->clip, sizeof(ClipState)) == cudaSuccess;
     ok = ok && cudaMalloc(&c->center, sizeof(float)) == cudaSuccess;
-    ok = ok && cudaMemset(c->flip, 0, sizeof(uint32_t)) == cudaSuccess;
+    ok = ok && cudaMemset(c->plan, 0, sizeof(BigHistPlan)) == cudaSuccess;
     ok = ok && cudaMemset(c->ticket, 0, sizeof(unsigned int)) == cudaSuccess;
     ok = ok && cudaMemset(c->gdigits, 0, kDigitBins * sizeof(unsigned long long)) == cudaSuccess;
     ok = ok && cudaMemset(c->coarse, 0, kDigitBins * sizeof(unsigned long long)) == cudaSuccess;
@@ -302,6 +309,8 @@ int cube_create(cube_ctx** out, size_t scratch_bytes_hint) {
     ok = ok && cudaFuncSetAttribute(hist_select_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize,
                                     hist_select_smem(kSmemHistMaxBins)) == cudaSuccess;
     ok = ok && cudaFuncSetAttribute(hist_packed_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                    (kBigWords + 4) * (int)sizeof(uint32_t)) == cudaSuccess;
+    ok = ok && cudaFuncSetAttribute(hist_win_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize,
                                     (kBigWords + 4) * (int)sizeof(uint32_t)) == cudaSuccess;
     ok = ok && cudaFuncSetAttribute(hist_dsm_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize,
                                     (32768 + 1) * (int)sizeof(uint32_t)) == cudaSuccess;
@@ -318,7 +327,7 @@ int cube_destroy(cube_ctx* c) {
     if (!c) return CUBE_EINVAL;
     cudaFree(c->partials); cudaFree(c->ticket); cudaFree(c->acc); cudaFree(c->nvox_acc);
     cudaFree(c->mom_out); cudaFree(c->gbins); cudaFree(c->gdigits); cudaFree(c->coarse); cudaFree(c->sel);
-    cudaFree(c->range3); cudaFree(c->probe_out); cudaFree(c->flip); cudaFree(c->clip); cudaFree(c->center);
+    cudaFree(c->range3); cudaFree(c->probe_out); cudaFree(c->plan); cudaFree(c->clip); cudaFree(c->center);
     cudaFree(c->cand);
     cudaFree(c->resident); cudaFree(c->chunk[0]); cudaFree(c->chunk[1]);
     if (c->pinned_results) cudaFreeHost(c->pinned_results);
@@ -567,7 +576,7 @@ int cube_set_knob(cube_ctx* c, int knob, int value) {
     switch (knob) {
         case CUBE_KNOB_CTAS_PER_SM: return cube_set_launch(c, value);
         case CUBE_KNOB_BIGHIST:
-            if (value != 0 && value != 1) return CUBE_EINVAL;
+            if (value < 0 || value > 2) return CUBE_EINVAL;
             c->bighist = value;
             return CUBE_OK;
         default: return CUBE_EINVAL;

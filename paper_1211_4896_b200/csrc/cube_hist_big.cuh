@@ -9,7 +9,7 @@
 // old value -- DESIGN.md sec. 4).  ptxas turns a predicated shared atomic into a branch, so the hot path issues ONE
 // unconditional +1 per voxel: voxels of the "hot" half of the bin range go to their word, all others to a trash
 // word, and the rows that hold such a voxel are revisited by a cold path (+65536 on the high half, closed top bin,
-// outside counts).  Which half is hot is sampled before the launch (hist_flip_kernel): `flip` swaps the halves.
+// outside counts).  Which half is hot is sampled before the launch (hist_window_kernel): `flip` swaps the halves.
 //
 // No increment returns a value, so a 16-bit field must never be allowed to wrap.  That is guaranteed without
 // looking at the data: every kScanEvery tiles (a tile = 16384 voxels of the CTA) all threads meet at a barrier, each
@@ -143,39 +143,14 @@ __device__ __forceinline__ void big_scan(uint32_t* sw, uint32_t flip, int nbins,
     if (threadIdx.x == 0) sw[kBigWords] = 0;   // trash word
 }
 
-// Which half of the bin range holds most of the voxels?  One CTA samples 16384 voxels spread over the cube and
-// writes 0x8000 when the upper half wins (then the upper half gets the +1 increments).  A performance hint only:
-// the histogram is exact for either value.
-__global__ void __launch_bounds__(kBigThreads)
-hist_flip_kernel(const float* __restrict__ d, uint64_t n, int nbins, float lo, float hi, float scale,
-                 const float* __restrict__ range3, uint32_t* __restrict__ flip_out) {
-    __shared__ int s_lower, s_upper;
-    if (threadIdx.x == 0) { s_lower = 0; s_upper = 0; }
-    __syncthreads();
-    if (range3) { lo = range3[0]; hi = range3[1]; scale = range3[2]; }
-    const uint64_t stride = n / (16 * kBigThreads) + 1;
-    int lower = 0, upper = 0;
-    for (int j = 0; j < 16; ++j) {
-        const uint64_t i = ((uint64_t)j * kBigThreads + threadIdx.x) * stride;
-        if (i < n) {
-            const float x = d[i];
-            if (x >= lo && x <= hi) {
-                const int b = min(max(__float2int_rd(__fmul_rn(__fsub_rn(x, lo), scale)), 0), nbins - 1);
-                if (b < kBigWords) ++lower; else ++upper;
-            }
-        }
-    }
-    atomicAdd(&s_lower, lower); atomicAdd(&s_upper, upper);
-    __syncthreads();
-    if (threadIdx.x == 0) *flip_out = (s_upper > s_lower) ? 0x8000u : 0u;
-}
-
 __global__ void __launch_bounds__(kBigThreads, 1)
 hist_packed_kernel(const float* __restrict__ d, uint64_t n, int nbins, float lo, float hi, float scale,
                    const float* __restrict__ range3, const uint32_t* __restrict__ flip_in,
+                   const uint32_t* __restrict__ skip_if_set,
                    unsigned long long* __restrict__ gbins, unsigned long long* __restrict__ goutside) {
     extern __shared__ uint32_t dyn_bins[];  // kBigWords words + trash word
     __shared__ uint32_t s_out[2];
+    if (skip_if_set && *skip_if_set) return;   // hist_win_kernel has done this histogram (BigHistPlan::use_window)
     for (int i = threadIdx.x; i <= kBigWords; i += kBigThreads) dyn_bins[i] = 0;
     if (threadIdx.x < 2) s_out[threadIdx.x] = 0;
     __syncthreads();
@@ -238,6 +213,149 @@ hist_packed_kernel(const float* __restrict__ d, uint64_t n, int nbins, float lo,
         const uint32_t bl = (uint32_t)i ^ flip, bh = (uint32_t)(i + kBigWords) ^ flip;
         if ((w & 0xFFFFu) && bl < (uint32_t)nbins) atomicAdd(&gbins[bl], (unsigned long long)(w & 0xFFFFu));
         if ((w >> 16) && bh < (uint32_t)nbins) atomicAdd(&gbins[bh], (unsigned long long)(w >> 16));
+    }
+    if (lo > hi) return;  // unusable device-side [min,max] range: hist_range_kernel has left the marker
+    if (threadIdx.x < 2 && s_out[threadIdx.x]) atomicAdd(&goutside[threadIdx.x], (unsigned long long)s_out[threadIdx.x]);
+}
+
+// ------------------------------------------------------------------------------------------------
+// Windowed variant (the default when it applies): 32-bit counters for a WINDOW of 32768 consecutive bins
+// [w0, w0 + 32768) in shared memory (128 KiB, one CTA of 1024 threads per SM), everything else straight to the
+// 64-bit global bins with a RED.  Real cubes put almost all voxels into a narrow part of a 65536-bin range (noise
+// around zero, sparse sources above -- PAPER.md:294: median +0.0036 in a range -1.04 ... 0.82), so the global REDs
+// are rare; a 32-bit counter cannot wrap (a CTA sees < 2^32 voxels), so there is no scan, no barrier and no
+// second increment flavour: the hot path is HistFastF's (FADD, FMUL, FADD, ISETP, F2I, SEL, IMAD, ATOMS.POPC.INC).
+// hist_window_kernel (1 CTA) samples 16384 voxels, picks w0 (a multiple of 4096) and decides: when more than
+// 1/32 of the sampled in-range voxels fall outside the best window (e.g. uniformly distributed data) the packed
+// kernel above runs instead -- both kernels are always enqueued and the one not chosen returns at once, so the
+// choice never leaves the device.  For nbins <= 32768 the window holds every bin and no sampling is needed.
+// ------------------------------------------------------------------------------------------------
+struct BigHistPlan {
+    uint32_t flip;       // packed kernel: which half gets the +1 increments
+    uint32_t w0;         // window kernel: first bin of the shared-memory window
+    uint32_t use_window; // 1: hist_win_kernel does the work, 0: hist_packed_kernel
+    uint32_t pad;
+};
+
+struct HistWinF {
+    float lo, hi, scale, off;
+    int top;
+    uint32_t w0, limitbits, sbase;
+    uint32_t* sbins;                 // kBigWords counters + trash
+    uint32_t* s_out;                 // shared {below, above}
+    unsigned long long* gbins;
+    __device__ __forceinline__ void setup(float lo_, float hi_, float scale_, int nbins, uint32_t w0_, uint32_t* sbins_,
+                                          uint32_t* s_out_, unsigned long long* gbins_) {
+        lo = lo_; hi = hi_; scale = scale_; top = nbins - 1; w0 = w0_; off = -(float)w0_;
+        sbins = sbins_; sbase = smem_addr(sbins_); s_out = s_out_; gbins = gbins_;
+        // hot path: window bins below the closed top bin (R11), i.e. 0 <= v - w0 < min(32768, top - w0)
+        const int lim = min(kBigWords, top - (int)w0_);
+        limitbits = __float_as_uint((float)max(lim, 0));
+    }
+    // v - w0 is exact for w0 <= v < 65536 (a multiple of ulp(v), smaller than v), negative below the window
+    __device__ __forceinline__ float inc(float x) const {
+        const float vh = __fadd_rn(__fmul_rn(__fsub_rn(x, lo), scale), off);
+        smem_inc(sbase, __float_as_uint(vh) < limitbits ? (uint32_t)__float2int_rd(vh) : (uint32_t)kBigWords);
+        return vh;
+    }
+    __device__ __forceinline__ bool counted(float x) const {
+        return __float_as_uint(__fadd_rn(__fmul_rn(__fsub_rn(x, lo), scale), off)) < limitbits;
+    }
+    __device__ __forceinline__ void exact(float x) const {   // a voxel the hot path did not count
+        if (x < lo) atomicAdd(&s_out[0], 1u);
+        else if (x > hi) atomicAdd(&s_out[1], 1u);
+        else if (x == x) {
+            const uint32_t b = (uint32_t)min(max(__float2int_rd(__fmul_rn(__fsub_rn(x, lo), scale)), 0), top);
+            const uint32_t pb = b - w0;
+            if (pb < (uint32_t)kBigWords) atomicAdd(&sbins[pb], 1u);
+            else atomicAdd(&gbins[b], 1ull);
+        }
+    }
+    __device__ __forceinline__ void operator()(float x) const {   // head / tail / ragged tile
+        if (counted(x)) inc(x); else exact(x);
+    }
+    __device__ __noinline__ void cold(uint32_t rows, const float4* __restrict__ p) const {
+        do {
+            const int j = __ffs(rows) - 1;
+            rows &= rows - 1;
+            const float4 q = __ldcg(p + j * kBigThreads);   // L2 hit: the line has just been streamed
+            if (!counted(q.x)) exact(q.x);
+            if (!counted(q.y)) exact(q.y);
+            if (!counted(q.z)) exact(q.z);
+            if (!counted(q.w)) exact(q.w);
+        } while (rows);
+    }
+    __device__ __forceinline__ void batch(const float4 (&r)[kUnroll], const float4* __restrict__ p) const {
+        const float limf = __uint_as_float(limitbits);
+        uint32_t rows = 0;
+#pragma unroll
+        for (int j = 0; j < kUnroll; ++j) {
+            const float a = inc(r[j].x), b = inc(r[j].y), c = inc(r[j].z), e = inc(r[j].w);
+            const float mx = fmaxf(fmaxf(a, b), fmaxf(c, e)), mn = fminf(fminf(a, b), fminf(c, e));
+            rows |= ((mx >= limf || __float_as_int(mn) < 0) ? 1u : 0u) << j;   // FMNMX: NaN voxels flag nothing
+        }
+        if (rows) cold(rows, p);
+    }
+};
+
+// 1 CTA: sample 16384 voxels spread over the cube; block histogram (16 blocks of 4096 bins); best window of 8
+// consecutive blocks; also the packed kernel's flip hint.  A performance plan only: every choice is exact.
+__global__ void __launch_bounds__(kBigThreads)
+hist_window_kernel(const float* __restrict__ d, uint64_t n, int nbins, float lo, float hi, float scale,
+                   const float* __restrict__ range3, BigHistPlan* __restrict__ plan) {
+    __shared__ int blk[16];
+    if (threadIdx.x < 16) blk[threadIdx.x] = 0;
+    __syncthreads();
+    if (range3) { lo = range3[0]; hi = range3[1]; scale = range3[2]; }
+    const uint64_t stride = n / (16 * kBigThreads) + 1;
+    for (int j = 0; j < 16; ++j) {
+        const uint64_t i = ((uint64_t)j * kBigThreads + threadIdx.x) * stride;
+        if (i < n) {
+            const float x = d[i];
+            if (x >= lo && x <= hi) {
+                const int b = min(max(__float2int_rd(__fmul_rn(__fsub_rn(x, lo), scale)), 0), nbins - 1);
+                atomicAdd(&blk[b >> 12], 1);
+            }
+        }
+    }
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        int total = 0, best = -1, bestj = 0, lower = 0;
+        for (int j = 0; j < 16; ++j) { total += blk[j]; if (j < 8) lower += blk[j]; }
+        for (int j = 0; j <= 8; ++j) {
+            int sum = 0;
+            for (int q = 0; q < 8; ++q) sum += blk[j + q];
+            if (sum > best) { best = sum; bestj = j; }
+        }
+        BigHistPlan pl;
+        pl.flip = (total - lower > lower) ? 0x8000u : 0u;
+        pl.w0 = (uint32_t)bestj << 12;
+        pl.use_window = (hist_use_fast(nbins, lo, hi, scale) && (total - best) * 32 <= total) ? 1u : 0u;
+        pl.pad = 0;
+        if (nbins <= kBigWords) { pl.w0 = 0; pl.flip = 0; }
+        *plan = pl;
+    }
+}
+
+__global__ void __launch_bounds__(kBigThreads, 1)
+hist_win_kernel(const float* __restrict__ d, uint64_t n, int nbins, float lo, float hi, float scale,
+                const float* __restrict__ range3, const BigHistPlan* __restrict__ plan,
+                unsigned long long* __restrict__ gbins, unsigned long long* __restrict__ goutside) {
+    extern __shared__ uint32_t dyn_bins[];  // kBigWords counters + trash
+    __shared__ uint32_t s_out[2];
+    if (!plan->use_window) return;          // the packed kernel does this histogram
+    for (int i = threadIdx.x; i <= kBigWords; i += kBigThreads) dyn_bins[i] = 0;
+    if (threadIdx.x < 2) s_out[threadIdx.x] = 0;
+    __syncthreads();
+    if (range3) { lo = range3[0]; hi = range3[1]; scale = range3[2]; }
+    const uint32_t w0 = plan->w0;
+    HistWinF f;
+    f.setup(lo, hi, scale, nbins, w0, dyn_bins, s_out, gbins);
+    stream_cube<kBigThreads>(d, n, f);
+    __syncthreads();
+    for (int i = threadIdx.x; i < kBigWords; i += kBigThreads) {
+        const uint32_t c = dyn_bins[i];
+        if (c && w0 + i < (uint32_t)nbins) atomicAdd(&gbins[w0 + i], (unsigned long long)c);
     }
     if (lo > hi) return;  // unusable device-side [min,max] range: hist_range_kernel has left the marker
     if (threadIdx.x < 2 && s_out[threadIdx.x]) atomicAdd(&goutside[threadIdx.x], (unsigned long long)s_out[threadIdx.x]);

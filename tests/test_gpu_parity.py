@@ -441,6 +441,37 @@ def test_packed_histogram_counter_wraps(ctx):
     assert rb.max() > 3 * 65536
 
 
+@pytest.mark.parametrize("knob", [0, 1, 2])
+def test_big_histogram_variants(ctx, knob):
+    # > 16384 bins: 0 = automatic (32-bit window of 32768 bins + global REDs, or 16-bit packed when the sampled
+    # voxels do not fit a window), 1 = cluster DSM, 2 = always packed.  Same integers from all of them.
+    r = np.random.default_rng(77)
+    n = 700001
+    noise_low = (r.standard_normal(n) * 0.002).astype(np.float32)
+    noise_low[r.integers(0, n, n // 200)] = r.uniform(0.0, 0.9, n // 200).astype(np.float32)   # sparse sources
+    noise_high = (0.8 + r.standard_normal(n) * 0.004).astype(np.float32)                       # window with w0 > 0
+    noise_high[r.integers(0, n, n // 100)] = r.uniform(-0.1, 0.2, n // 100).astype(np.float32)
+    uniform = r.uniform(-1.0, 1.0, n).astype(np.float32)                                        # no window fits
+    mid = (r.standard_normal(n) * 0.05 + 0.47).astype(np.float32)                               # straddles bin 32768
+    ctx.set_knob(cube.KNOB_BIGHIST, knob)
+    try:
+        for a in (noise_low, noise_high, uniform, mid):
+            a = a.copy()
+            a[::131] = np.nan
+            t = dev(a, 1)
+            lo, hi = float(np.nanmin(a)), float(np.nanmax(a))
+            for nbins, (l, h) in ((65536, (lo, hi)), (65536, (-0.05, 0.95)), (40000, (lo, hi)), (16385, (0.0, 1.0)),
+                                  (32768, (lo, hi)), (32769, (lo, hi))):
+                b, o = ctx.histogram(t, a.size, 1, 1, nbins, l, h)
+                rb, ro = oracle.histogram(a, nbins, l, h)
+                assert (b == rb).all() and (o == ro).all(), (knob, nbins, l, h)
+            m, b, o, med = ctx.stats(t, a.size, 1, 1, 65536)                # [min,max] resolved on the device
+            rb, ro = oracle.histogram(a, 65536, lo, hi)
+            assert (b == rb).all() and (o == ro).all() and same_float(med, oracle.median(a))
+    finally:
+        ctx.set_knob(cube.KNOB_BIGHIST, 0)
+
+
 @pytest.mark.parametrize("resident", [False, True])
 def test_stats_host_matches_oracle(ctx, resident):
     a = cubegen.generate_numpy(cubegen.scaled("c2", (96, 96, 200), nsrc=5)).reshape(-1)
