@@ -79,13 +79,67 @@ struct MomentsF {
         if (!have && taken(x)) { have = true; pivf = x; pivot = (double)x; }
     }
     __device__ __forceinline__ void operator()(float x) { take_pivot(x); core(x); }
-    __device__ __forceinline__ void batch(const float4 (&r)[kUnroll], const float4*) {
-        if (!have) {  // only until this thread has met its first voxel that takes part
+
+    // A tile share (kUnroll rows of 4 voxels) whose sum of deviations came out NaN holds a NaN voxel (or +Inf and
+    // -Inf): the hot path has left it out of s, q and n, and has counted every one of its voxels in the digit bins.
+    // Revisit it (the lines are L2 hits): add the non-NaN voxels one by one and take the NaN voxels back out of
+    // the bins.
+    struct TileFix { double s, q; uint32_t n; };
+    static __device__ __noinline__ TileFix cold_tile(const float4* __restrict__ p, double pivot_, uint32_t sbins_) {
+        TileFix f;
+        f.s = 0.0; f.q = 0.0; f.n = 0;
+#pragma unroll 1
+        for (int j = 0; j < kUnroll; ++j) {
+            const float4 v = __ldcg(p + j * kThreads);
+            const float x[4] = {v.x, v.y, v.z, v.w};
 #pragma unroll
-            for (int j = 0; j < kUnroll; ++j) { take_pivot(r[j].x); take_pivot(r[j].y); take_pivot(r[j].z); take_pivot(r[j].w); }
+            for (int i = 0; i < 4; ++i) {
+                if (x[i] == x[i]) {
+                    const double dlt = (double)x[i] - pivot_;
+                    f.s += dlt; f.q = fma(dlt, dlt, f.q); f.n += 1;
+                } else if (COARSE) {
+                    asm volatile("red.shared.add.u32 [%0], -1;" :: "r"(sbins_ + 4u * raw_digit(x[i])) : "memory");
+                }
+            }
         }
+        return f;
+    }
+    // Full tile.  Hot path (kMomPlain / kMomCoarse), per row of 4 voxels: d_i = (double)x_i - pivot (exact);
+    // ts += (d0+d1)+(d2+d3); tq += d0^2+d1^2+d2^2+d3^2 (DFMA chain); the tile share joins s, q, n when ts is not
+    // NaN -- no per-voxel NaN test, select or count (FMNMX ignores NaN operands; the digit increment is
+    // unconditional).  ~8 issue slots per voxel instead of 14 (profiles/: the fused passes are issue/power bound
+    // once the SM clock drops under a sustained load).
+    __device__ __forceinline__ void batch(const float4 (&r)[kUnroll], const float4* __restrict__ p) {
+        if (MODE == kMomWindow || !have) {
+            if (!have) {  // only until this thread has met its first voxel that takes part
 #pragma unroll
-        for (int j = 0; j < kUnroll; ++j) { core(r[j].x); core(r[j].y); core(r[j].z); core(r[j].w); }
+                for (int j = 0; j < kUnroll; ++j) { take_pivot(r[j].x); take_pivot(r[j].y); take_pivot(r[j].z); take_pivot(r[j].w); }
+            }
+#pragma unroll
+            for (int j = 0; j < kUnroll; ++j) { core(r[j].x); core(r[j].y); core(r[j].z); core(r[j].w); }
+            return;
+        }
+        double ts[2] = {0.0, 0.0}, tq[2] = {0.0, 0.0};  // two chains for instruction-level parallelism
+#pragma unroll
+        for (int j = 0; j < kUnroll; ++j) {
+            const double d0 = (double)r[j].x - pivot, d1 = (double)r[j].y - pivot;
+            const double d2 = (double)r[j].z - pivot, d3 = (double)r[j].w - pivot;
+            ts[j & 1] += (d0 + d1) + (d2 + d3);
+            tq[j & 1] = fma(d3, d3, fma(d2, d2, fma(d1, d1, fma(d0, d0, tq[j & 1]))));
+            mn = fminf(fminf(mn, r[j].x), fminf(r[j].y, fminf(r[j].z, r[j].w)));
+            mx = fmaxf(fmaxf(mx, r[j].x), fmaxf(r[j].y, fmaxf(r[j].z, r[j].w)));
+            if (COARSE) {
+                smem_inc(sbins, raw_digit(r[j].x)); smem_inc(sbins, raw_digit(r[j].y));
+                smem_inc(sbins, raw_digit(r[j].z)); smem_inc(sbins, raw_digit(r[j].w));
+            }
+        }
+        const double tsum = ts[0] + ts[1];
+        if (tsum == tsum) {
+            s += tsum; q += tq[0] + tq[1]; n += 4u * kUnroll;
+        } else {
+            const TileFix f = cold_tile(p, pivot, sbins);
+            s += f.s; q += f.q; n += f.n;
+        }
     }
     __device__ __forceinline__ Partial partial() const {
         Partial p = partial_empty();
@@ -130,7 +184,7 @@ struct ClipState {
 // nvox_acc : running voxel total.  When `accumulate` is 0 both are overwritten.
 // kMomWindow: the window is (wlo, whi), or *clip when clip != nullptr (then a finished clip makes the kernel a no-op).
 template <int MODE>
-__global__ void __launch_bounds__(kThreads)
+__global__ void __launch_bounds__(kThreads, 4)
 moments_kernel(const float* __restrict__ d, uint64_t n, Partial* __restrict__ partials,
                unsigned int* __restrict__ ticket, Partial* __restrict__ acc,
                unsigned long long* __restrict__ nvox_acc, int accumulate, unsigned flags,
