@@ -72,7 +72,7 @@ constexpr int kMaxCtasPerSm = 8;
 constexpr int kSmemHistMaxBins = 16384;  // 64 KiB of 32-bit counters per CTA
 // dynamic shared memory of hist_select_kernel: histogram + trash, digit bins + trash, stage slices + counters
 constexpr int hist_select_smem(int nbins) {
-    return (nbins + 1 + kBins1 + 1 + (kThreads / 32) * ((int)kStageCap + 1)) * (int)sizeof(uint32_t);
+    return (nbins + 2 + kBins1 + 1 + (kThreads / 32) * ((int)kStageCap + 1)) * (int)sizeof(uint32_t);
 }
 
 #define CUBE_CUDA(ctx, call)                              \
@@ -180,7 +180,7 @@ int launch_hist(cube_ctx* c, const float* d, uint64_t n, int nbins, float lo, fl
     {
     ProfScope prof(c, CUBE_K_HIST, s);
     if (nbins <= kSmemHistMaxBins) {
-        const size_t smem = (size_t)(nbins + 1) * sizeof(uint32_t);  // + trash counter
+        const size_t smem = (size_t)(nbins + 2) * sizeof(uint32_t);  // + trash slot
         int occ = 0;
         if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, hist_smem_kernel, kThreads, smem) != cudaSuccess)
             occ = 1;
@@ -305,7 +305,7 @@ int cube_create(cube_ctx** out, size_t scratch_bytes_hint) {
     ok = ok && cudaMemset(c->gdigits, 0, kDigitBins * sizeof(unsigned long long)) == cudaSuccess;
     ok = ok && cudaMemset(c->coarse, 0, kDigitBins * sizeof(unsigned long long)) == cudaSuccess;
     ok = ok && cudaFuncSetAttribute(hist_smem_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                                    (kSmemHistMaxBins + 1) * (int)sizeof(uint32_t)) == cudaSuccess;
+                                    (kSmemHistMaxBins + 2) * (int)sizeof(uint32_t)) == cudaSuccess;
     ok = ok && cudaFuncSetAttribute(hist_select_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize,
                                     hist_select_smem(kSmemHistMaxBins)) == cudaSuccess;
     ok = ok && cudaFuncSetAttribute(hist_packed_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize,

@@ -116,6 +116,7 @@ __device__ __forceinline__ uint32_t smem_addr(const void* p) { return (uint32_t)
 // sm__inst_executed_pipe_alu 60-70 %, profiles/), and the FMA pipe is idle.  The RED compiles to
 // ATOMS.POPC.INC, which the hardware aggregates over lanes that hit the same address.
 __constant__ uint32_t c_four = 4u;
+__constant__ uint32_t c_one = 1u;
 __device__ __forceinline__ void smem_inc(uint32_t saddr, uint32_t idx) {
     asm volatile("{\n\t.reg .u32 a;\n\tmad.lo.u32 a, %0, %1, %2;\n\tred.shared.add.u32 [a], 1;\n\t}"
                  :: "r"(idx), "r"(c_four), "r"(saddr) : "memory");

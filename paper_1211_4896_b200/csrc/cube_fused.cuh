@@ -62,7 +62,7 @@ __device__ __forceinline__ bool hist_range(const MomentsOut* __restrict__ range_
     return !(isinf(width) || isinf(scale));
 }
 
-// Dynamic shared memory: [nbins + 1 histogram counters][kBins1 + 1 digit counters][stage slices + counters].
+// Dynamic shared memory: [nbins + 2 histogram slots][kBins1 + 1 digit counters][stage slices + counters].
 __global__ void __launch_bounds__(kThreads, 3)
 hist_select_kernel(const float* __restrict__ d, uint64_t n, int nbins, float lo, float hi, float scale,
                    const MomentsOut* __restrict__ range_from, unsigned long long* __restrict__ gbins,
@@ -71,9 +71,9 @@ hist_select_kernel(const float* __restrict__ d, uint64_t n, int nbins, float lo,
     extern __shared__ uint32_t dyn_bins[];
     __shared__ uint32_t s_out[2];
     uint32_t* hbins = dyn_bins;
-    uint32_t* sbins = dyn_bins + (nbins + 1);
+    uint32_t* sbins = dyn_bins + (nbins + 2);
     uint32_t* stage = sbins + (kBins1 + 1);
-    for (int i = threadIdx.x; i < nbins + 1 + kBins1 + 1; i += kThreads) dyn_bins[i] = 0;
+    for (int i = threadIdx.x; i < nbins + 2 + kBins1 + 1; i += kThreads) dyn_bins[i] = 0;
     if (threadIdx.x < 2) s_out[threadIdx.x] = 0;
     __syncthreads();
     const bool range_ok = hist_range(range_from, nbins, lo, hi, scale);
@@ -89,10 +89,7 @@ hist_select_kernel(const float* __restrict__ d, uint64_t n, int nbins, float lo,
         hist_select_run(d, n, h, st, sbins, stage, cand, below, above);
     }
     __syncthreads();
-    for (int i = threadIdx.x; i < nbins; i += kThreads) {
-        const uint32_t c = hbins[i];
-        if (c) atomicAdd(&gbins[i], (unsigned long long)c);
-    }
+    hist_flush_bins(hbins, nbins, gbins);
     for (int i = threadIdx.x; i < kBins1; i += kThreads) {
         const uint32_t c = sbins[i];
         if (c) atomicAdd(&gdigits[i], (unsigned long long)c);

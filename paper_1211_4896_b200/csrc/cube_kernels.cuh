@@ -104,19 +104,28 @@ struct MomentsF {
         }
         return f;
     }
-    // Full tile.  Hot path (kMomPlain / kMomCoarse), per row of 4 voxels: d_i = (double)x_i - pivot (exact);
-    // ts += (d0+d1)+(d2+d3); tq += d0^2+d1^2+d2^2+d3^2 (DFMA chain); the tile share joins s, q, n when ts is not
-    // NaN -- no per-voxel NaN test, select or count (FMNMX ignores NaN operands; the digit increment is
-    // unconditional).  ~8 issue slots per voxel instead of 14 (profiles/: the fused passes are issue/power bound
-    // once the SM clock drops under a sustained load).
+    // Full tile (all 32 lanes of the warp are here: stream_cube calls batch() CTA-uniformly).  Two ways through:
+    //  HOT (kMomPlain / kMomCoarse), per row of 4 voxels: d_i = (double)x_i - pivot (exact); ts += (d0+d1)+(d2+d3);
+    //   tq += d0^2+d1^2+d2^2+d3^2 (DFMA chain); the tile share joins s, q, n when ts is not NaN -- no per-voxel NaN
+    //   test, select or count (FMNMX ignores NaN operands; the digit increment is unconditional): ~8.5 issue slots
+    //   per voxel.  A lane whose ts is NaN (a NaN voxel, or +Inf and -Inf) repairs its share in cold_tile().
+    //  SAFE: the branch-free per-voxel form (core(): FSETP, FSEL, count; ~14 slots per voxel), which costs the same
+    //   whatever the NaN density.
+    // The warp runs HOT until a tile with a NaN shows up and SAFE until a tile without one has gone by (one vote
+    // per tile), so cubes with scattered NULL voxels (config 3: 0.5 %, i.e. some lane of every warp tile) never
+    // pay the divergent repair, and NaN-free stretches never pay the per-voxel tests (profiles/: the fused passes
+    // are issue/power bound once the SM clock drops under a sustained load).
+    bool safe = true;   // warp-uniform
     __device__ __forceinline__ void batch(const float4 (&r)[kUnroll], const float4* __restrict__ p) {
-        if (MODE == kMomWindow || !have) {
+        if (MODE == kMomWindow || safe) {
             if (!have) {  // only until this thread has met its first voxel that takes part
 #pragma unroll
                 for (int j = 0; j < kUnroll; ++j) { take_pivot(r[j].x); take_pivot(r[j].y); take_pivot(r[j].z); take_pivot(r[j].w); }
             }
+            const uint32_t n0 = n;
 #pragma unroll
             for (int j = 0; j < kUnroll; ++j) { core(r[j].x); core(r[j].y); core(r[j].z); core(r[j].w); }
+            if (MODE != kMomWindow) safe = __any_sync(0xffffffffu, n - n0 != 4u * kUnroll);  // every lane has a pivot then
             return;
         }
         double ts[2] = {0.0, 0.0}, tq[2] = {0.0, 0.0};  // two chains for instruction-level parallelism
@@ -134,12 +143,14 @@ struct MomentsF {
             }
         }
         const double tsum = ts[0] + ts[1];
-        if (tsum == tsum) {
+        const bool bad = !(tsum == tsum);
+        if (!bad) {
             s += tsum; q += tq[0] + tq[1]; n += 4u * kUnroll;
         } else {
             const TileFix f = cold_tile(p, pivot, sbins);
             s += f.s; q += f.q; n += f.n;
         }
+        safe = __any_sync(0xffffffffu, bad);
     }
     __device__ __forceinline__ Partial partial() const {
         Partial p = partial_empty();
@@ -291,19 +302,22 @@ struct HistBase {
     }
 };
 
-// Per voxel, 9 instructions and no branch: 2 FSETP (range test on x itself, false for NaN), FADD, FMUL
-// (__fsub_rn / __fmul_rn: never contracted), F2I.FLOOR, VIMNMX (closed top bin), SEL, LEA,
-// ATOMS.POPC.INC.  The increment is unconditional: voxels that are NaN or outside [lo,hi] go to a trash
-// counter at index nbins (ptxas turns a predicated RED into a branch around the whole bin computation,
-// which costs more than the SEL).  Voxels outside [lo,hi] are rare on every config, so below/above are
-// found per batch from the batch min/max (FMNMX3, NaN-blind: NaN voxels are counted nowhere) and
-// counted in a cold path.
+// Shared-memory layout of the <= 16384-bin kernels: slots 0 .. top-1 hold bins 0 .. top-1 (top = nbins-1), slot
+// `top` is a TRASH counter (never read) and slot top+1 holds the closed top bin.  So the hot path of the fast
+// functor can clamp with one unsigned minimum: everything at or beyond `top` -- the top bin, voxels above the
+// range, and negative positions (huge as unsigned) -- lands on the trash slot and is put right by a cold path.
+__device__ __forceinline__ uint32_t hist_slot(int b, int top) { return (uint32_t)(b + (b >= top ? 1 : 0)); }
+
+// General functor (hi == lo, fewer than 8 bins, subnormal scale): per voxel 2 FSETP (range test on x itself, false
+// for NaN), FADD, FMUL (__fsub_rn / __fmul_rn: never contracted), F2I.FLOOR, VIMNMX (closed top bin), SEL,
+// ATOMS.POPC.INC.  The increment is unconditional: voxels that are NaN or outside [lo,hi] go to the trash slot.
+// Voxels outside [lo,hi] are found per batch from the batch min/max (FMNMX3, NaN-blind) and counted in a cold path.
 struct HistF : HistBase {
-    uint32_t* sbins;  // nbins + 1 counters, the last one is the trash counter
+    uint32_t* sbins;  // nbins + 2 slots (layout above)
     __device__ __forceinline__ void inc(float x) const {
         const bool in = (x >= lo) && (x <= hi);
-        const int b = in ? bin_of(x) : top + 1;
-        atomicAdd(&sbins[b], 1u);
+        const uint32_t slot = in ? hist_slot(bin_of(x), top) : (uint32_t)top;
+        atomicAdd(&sbins[slot], 1u);
     }
     __device__ __forceinline__ void operator()(float x) {
         inc(x);
@@ -324,76 +338,81 @@ struct HistF : HistBase {
     }
 };
 
-// Fast variant (the default): the range test and the top-bin clamp leave the per-voxel path.
-// With v = (x - lo) * scale as above and vb its bit pattern, ONE unsigned compare vb < bits((float)(nbins-1))
-// is true exactly for +0 <= v < nbins-1 -- false for negative v (sign bit; also -0.0), for NaN (0x7FFFFFFF) and
-// for everything from the top bin upwards.  For such a voxel lo <= x <= hi is guaranteed (t = x - lo has the
-// sign of the exact difference, and x > hi implies v >= fl(fl(hi-lo) * scale) > nbins - 1 whenever hi > lo and
-// scale is a normal number, nbins <= 65536) and its bin is floor(v), no clamp.  Everything else goes to the
-// trash counter, and the 4-voxel rows that contain such a non-NaN voxel are flagged (FMNMX3 on v) and revisited by
-// a cold path that applies the exact definition (x < lo, x > hi, NaN, closed top bin).  On the ALU pipe --
-// the one that limits these kernels, 16 lanes/clk/SMSP -- that is ISETP + SEL + ~1 per voxel instead of
-// 2 FSETP + SEL + VIMNMX + FMNMX.  Not valid for hi == lo (scale 0): hist_use_fast().
+// Fast functor (the default).  With v = fl(fl(x - lo) * scale) (R10) the hot path does
+//     i = floor(max(v, -1));  counter[min((unsigned)i, top)] += 1;  tmax = max(tmax, i);  xmin = min(xmin, x)
+// i.e. per voxel FADD, FMUL, FMNMX, F2I.FLOOR, VIMNMX.U32, IMAD, ATOMS.POPC.INC and half a VIMNMX3 + half an FMNMX3
+// -- no compare, no select, no branch (8 issue slots; v3 had ISETP + SEL + FMNMX row flags: 8.7 and one more on the
+// half-rate ALU pipe).  FMNMX returns the other operand for a NaN, so a NULL voxel becomes i = -1 like any voxel
+// below the range, and min((unsigned)-1, top) sends both to the trash slot: NaN voxels need no further attention.
+// 0 <= i < top is exactly the case "+0 <= v < nbins-1", for which lo <= x <= hi is guaranteed (t = x - lo has
+// the sign of the exact difference, and x > hi implies v >= fl(fl(hi-lo) * scale) > nbins - 1 whenever hi > lo and
+// scale is a normal number, nbins <= 65536) and the bin is floor(v), no clamp.  What is left -- the closed top bin
+// (R11), x > hi (both: i >= top, signed) and x < lo (xmin < lo; FMNMX3 ignores NaN) -- is rare and detected per
+// tile share (32 voxels); a cold path reloads the 8 rows (L2 hits), finds the rows concerned and applies the exact
+// definition to their voxels.  Not valid for hi == lo (scale 0), fewer than 8 bins or a subnormal scale.
 __host__ __device__ __forceinline__ bool hist_use_fast(int nbins, float lo, float hi, float scale) {
     return hi > lo && nbins >= 8 && scale >= 1.17549435e-38f;
 }
 struct HistFastF {
     float lo, hi, scale;
     int top;
-    uint32_t topbits;  // bits of (float)top
-    uint32_t* sbins;   // nbins + 1 counters (last = trash)
+    uint32_t* sbins;   // nbins + 2 slots (layout above)
     uint32_t sbase;    // shared-window address of sbins
     uint32_t* s_out;   // shared {below, above}
     uint32_t below = 0, above = 0;  // unused (kept for hist_flush_outside); the cold path counts in s_out
     __device__ __forceinline__ void setup(float lo_, float hi_, float scale_, int nbins, uint32_t* sbins_,
                                           uint32_t* s_out_) {
-        lo = lo_; hi = hi_; scale = scale_; top = nbins - 1; topbits = __float_as_uint((float)(nbins - 1));
+        lo = lo_; hi = hi_; scale = scale_; top = nbins - 1;
         sbins = sbins_; sbase = smem_addr(sbins_); s_out = s_out_;
     }
-    __device__ __forceinline__ float inc(float x) const {
-        const float v = __fmul_rn(__fsub_rn(x, lo), scale);
-        smem_inc(sbase, __float_as_uint(v) < topbits ? (uint32_t)__float2int_rd(v) : (uint32_t)(top + 1));
-        return v;
+    static __device__ __forceinline__ int pos(float x, float lo, float scale) {   // i of the hot path
+        return __float2int_rd(fmaxf(__fmul_rn(__fsub_rn(x, lo), scale), -1.0f));
     }
-    // exact definition for a voxel the hot path sent to the trash counter
-    static __device__ __forceinline__ void exact(float x, float lo, float hi, float scale, int top,
-                                                 uint32_t topbits, uint32_t* sbins, uint32_t* s_out) {
+    // exact definition for a voxel the hot path sent to the trash slot (NaN: nothing to do)
+    static __device__ __forceinline__ void fix(float x, float lo, float hi, float scale, int top, uint32_t* sbins,
+                                               uint32_t* s_out) {
         if (x < lo) atomicAdd(&s_out[0], 1u);
         else if (x > hi) atomicAdd(&s_out[1], 1u);
-        else if (x == x) {  // in range: v >= nbins - 1 (closed top bin, R11) or v == -0.0 (x = -0.0, lo = +0.0)
-            const float v = __fmul_rn(__fsub_rn(x, lo), scale);
-            if (!(__float_as_uint(v) < topbits)) atomicAdd(&sbins[min(max(__float2int_rd(v), 0), top)], 1u);
+        else if (x == x) {
+            const int i = pos(x, lo, scale);
+            if ((uint32_t)i >= (uint32_t)top) atomicAdd(&sbins[hist_slot(min(max(i, 0), top), top)], 1u);
         }
     }
-    static __device__ __noinline__ void cold(uint32_t rows, const float4* __restrict__ p, float lo, float hi,
-                                             float scale, int top, uint32_t topbits, uint32_t* sbins,
-                                             uint32_t* s_out) {
-        do {
-            const int j = __ffs(rows) - 1;
-            rows &= rows - 1;
+    static __device__ __noinline__ void cold(const float4* __restrict__ p, float lo, float hi, float scale, int top,
+                                             uint32_t* sbins, uint32_t* s_out) {
+#pragma unroll 1
+        for (int j = 0; j < kUnroll; ++j) {
             const float4 q = __ldcg(p + j * kThreads);  // L2 hit: the line has just been streamed
-            exact(q.x, lo, hi, scale, top, topbits, sbins, s_out);
-            exact(q.y, lo, hi, scale, top, topbits, sbins, s_out);
-            exact(q.z, lo, hi, scale, top, topbits, sbins, s_out);
-            exact(q.w, lo, hi, scale, top, topbits, sbins, s_out);
-        } while (rows);
+            const int im = max(max(pos(q.x, lo, scale), pos(q.y, lo, scale)), max(pos(q.z, lo, scale), pos(q.w, lo, scale)));
+            const float xm = fminf(fminf(q.x, q.y), fminf(q.z, q.w));
+            if (im >= top || xm < lo) {
+                fix(q.x, lo, hi, scale, top, sbins, s_out);
+                fix(q.y, lo, hi, scale, top, sbins, s_out);
+                fix(q.z, lo, hi, scale, top, sbins, s_out);
+                fix(q.w, lo, hi, scale, top, sbins, s_out);
+            }
+        }
     }
-    __device__ __forceinline__ void operator()(float x) {
-        if (!(__float_as_uint(inc(x)) < topbits)) exact(x, lo, hi, scale, top, topbits, sbins, s_out);
+    __device__ __forceinline__ void operator()(float x) {   // head / tail / ragged last tile
+        const int i = pos(x, lo, scale);
+        if ((uint32_t)i < (uint32_t)top) atomicAdd(&sbins[i], 1u);
+        else fix(x, lo, hi, scale, top, sbins, s_out);
     }
     __device__ __forceinline__ void batch(const float4 (&r)[kUnroll], const float4* __restrict__ p) {
-        // A row is revisited iff it holds a voxel with v >= nbins - 1 or v < 0 (sign bit: also -0.0).  The row
-        // maximum / minimum are taken with FMNMX, which ignores NaN operands: blanked voxels count nowhere, so NaN
-        // alone never sends a row to the cold path (config 3 scatters a NaN into 2 % of the rows).
-        const float topf = __uint_as_float(topbits);
-        uint32_t rows = 0;
+        int tmax = -1;
+        float xmin = INFINITY;
 #pragma unroll
         for (int j = 0; j < kUnroll; ++j) {
-            const float a = inc(r[j].x), b = inc(r[j].y), c = inc(r[j].z), e = inc(r[j].w);
-            const float mx = fmaxf(fmaxf(a, b), fmaxf(c, e)), mn = fminf(fminf(a, b), fminf(c, e));
-            rows |= ((mx >= topf || __float_as_int(mn) < 0) ? 1u : 0u) << j;
+            const int i0 = pos(r[j].x, lo, scale), i1 = pos(r[j].y, lo, scale);
+            const int i2 = pos(r[j].z, lo, scale), i3 = pos(r[j].w, lo, scale);
+            smem_inc(sbase, min((uint32_t)i0, (uint32_t)top));
+            smem_inc(sbase, min((uint32_t)i1, (uint32_t)top));
+            smem_inc(sbase, min((uint32_t)i2, (uint32_t)top));
+            smem_inc(sbase, min((uint32_t)i3, (uint32_t)top));
+            tmax = max(max(tmax, max(i0, i1)), max(i2, i3));
+            xmin = fminf(fminf(xmin, fminf(r[j].x, r[j].y)), fminf(r[j].z, r[j].w));
         }
-        if (rows) cold(rows, p, lo, hi, scale, top, topbits, sbins, s_out);
+        if (tmax >= top || xmin < lo) cold(p, lo, hi, scale, top, sbins, s_out);
     }
 };
 
@@ -406,6 +425,15 @@ __device__ __forceinline__ void hist_flush_outside(F& f, uint32_t* s_out, unsign
     if (threadIdx.x < 2 && s_out[threadIdx.x]) atomicAdd(&goutside[threadIdx.x], (unsigned long long)s_out[threadIdx.x]);
 }
 
+// Flush of the per-CTA counters (layout above) into the 64-bit global bins.
+__device__ __forceinline__ void hist_flush_bins(const uint32_t* sbins, int nbins, unsigned long long* __restrict__ gbins) {
+    const int top = nbins - 1;
+    for (int i = threadIdx.x; i < nbins; i += kThreads) {
+        const uint32_t c = sbins[i < top ? i : top + 1];
+        if (c) atomicAdd(&gbins[i], (unsigned long long)c);
+    }
+}
+
 // nbins <= 16384: 32-bit counters, several CTAs per SM.
 __global__ void __launch_bounds__(kThreads)
 hist_smem_kernel(const float* __restrict__ d, uint64_t n, int nbins, float lo, float hi, float scale,
@@ -413,7 +441,7 @@ hist_smem_kernel(const float* __restrict__ d, uint64_t n, int nbins, float lo, f
                  unsigned long long* __restrict__ gbins, unsigned long long* __restrict__ goutside) {
     extern __shared__ uint32_t dyn_bins[];
     __shared__ uint32_t s_out[2];
-    for (int i = threadIdx.x; i <= nbins; i += kThreads) dyn_bins[i] = 0;  // + trash counter
+    for (int i = threadIdx.x; i < nbins + 2; i += kThreads) dyn_bins[i] = 0;  // + trash slot
     if (threadIdx.x < 2) s_out[threadIdx.x] = 0;
     __syncthreads();
     if (range3) { lo = range3[0]; hi = range3[1]; scale = range3[2]; }  // resolved on the device (cube_stats)
@@ -429,10 +457,7 @@ hist_smem_kernel(const float* __restrict__ d, uint64_t n, int nbins, float lo, f
         below = f.below; above = f.above;
     }
     __syncthreads();
-    for (int i = threadIdx.x; i < nbins; i += kThreads) {
-        uint32_t c = dyn_bins[i];
-        if (c) atomicAdd(&gbins[i], (unsigned long long)c);
-    }
+    hist_flush_bins(dyn_bins, nbins, gbins);
     if (lo > hi) return;  // unusable device-side [min,max] range: hist_range_kernel has left the marker
     if (below) atomicAdd(&s_out[0], below);
     if (above) atomicAdd(&s_out[1], above);

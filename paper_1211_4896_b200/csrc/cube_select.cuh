@@ -29,11 +29,12 @@ constexpr int kStageBytes = (kThreads / 32) * (int)kStageCap * 4;      // 36 KiB
 //   PASS 0:  idx = NaN ? trash : bits >> 19 (the RAW top 13 bits; the scan kernel reads the bins in key order
 //            through raw_of_digit(), so the key transform is not paid per voxel); ATOMS.POPC.INC
 //            (hardware-aggregated over equal addresses).  SHF, FSETP, SEL, LEA, ATOMS.
-//   PASS 1:  the voxel is in the prefix bucket iff (bits ^ rawbase) < 2^19: LOP3 per voxel, VIMNMX3 per pair,
-//            one flag per 4-voxel row (~2 ALU instructions per voxel, NO shared-memory traffic).  Only the rows
-//            that hold a voxel of the bucket (the bucket is 0.05-3 % of the cube on the configs) are visited
-//            again by a cold path that re-loads the row (an L2 hit: its line has just been streamed), counts
-//            the digit (kk >> 9) and stages the key.  So pass 1 costs less issue bandwidth than pass 0.
+//   PASS 1:  the voxel is in the prefix bucket iff bits - rawbase < 2^19 (mod 2^32): IMAD per voxel, row minima,
+//            one test per tile share of 32 voxels (1.7 issue slots per voxel, NO shared-memory traffic).
+//            Only the rows that hold a voxel of the bucket (the bucket is 0.05-3 % of the cube on the
+//            configs) are visited again by a cold path that re-loads the row (an L2 hit: its line has just been
+//            streamed), counts the digit (kk >> 9) and stages the key.  So pass 1 costs less issue bandwidth
+//            than pass 0.
 //   PASS 2 over the cube (only when the candidates did not fit): idx = min(key - (prefix << 9), 512) sends every
 //            voxel outside the bucket to the trash counter without a compare.
 //   NaN keys can only fall into the buckets beyond +-inf (digit_may_hold_nan); only then (NANCHK)
@@ -61,6 +62,11 @@ struct SelectF {
     float center = 0.0f;   // DEV
     static __device__ __forceinline__ float xf(float x, float center_) {
         return DEV ? fabsf(__fsub_rn(x, center_)) : x;
+    }
+    static __device__ __forceinline__ uint32_t sub_fma(float y, uint32_t negbase) {   // bits(y) - rawbase on the FMA pipe
+        uint32_t t;
+        asm("mad.lo.u32 %0, %1, %2, %3;" : "=r"(t) : "r"(__float_as_uint(y)), "r"(c_one), "r"(negbase));
+        return t;
     }
     __device__ __forceinline__ uint32_t kk_of(float x) const {
         uint32_t kk = key_of(x) - base;
@@ -126,14 +132,27 @@ struct SelectF {
             for (int j = 0; j < kUnroll; ++j) { count(r[j].x); count(r[j].y); count(r[j].z); count(r[j].w); }
             return;
         }
-        uint32_t rows = 0;  // rows (float4) holding at least one voxel whose raw bits are in the bucket
+        // Does this thread's share of the tile (8 rows of 4 voxels) hold a voxel of the bucket?  bits - rawbase <
+        // 2^19 (mod 2^32) <=> the top 13 raw bits match; the subtraction is issued as IMAD on the FMA pipe
+        // (multiplier 1 from constant memory), each row's minimum takes a VIMNMX3 + VIMNMX, the tile minimum four
+        // more VIMNMX3, then ONE test per tile share: 1.7 issue slots per voxel, 0.7 of them on the ALU pipe (v3:
+        // LOP3 per voxel and a test per row, 2.7 / 2.7).  The row flags are only formed behind the branch.
+        // NaN voxels may flag a row, the cold path drops them.
+        uint32_t rm[kUnroll];
+        const uint32_t negbase = 0u - rawbase;
 #pragma unroll
-        for (int j = 0; j < kUnroll; ++j) {
-            const uint32_t m = min(min(__float_as_uint(xf(r[j].x, center)) ^ rawbase, __float_as_uint(xf(r[j].y, center)) ^ rawbase),
-                                   min(__float_as_uint(xf(r[j].z, center)) ^ rawbase, __float_as_uint(xf(r[j].w, center)) ^ rawbase));
-            rows |= (m < kSpan ? 1u : 0u) << j;
+        for (int j = 0; j < kUnroll; ++j)
+            rm[j] = min(min(sub_fma(xf(r[j].x, center), negbase), sub_fma(xf(r[j].y, center), negbase)),
+                        min(sub_fma(xf(r[j].z, center), negbase), sub_fma(xf(r[j].w, center), negbase)));
+        uint32_t tmin = rm[0];
+#pragma unroll
+        for (int j = 1; j < kUnroll; ++j) tmin = min(tmin, rm[j]);
+        if (tmin < kSpan) {
+            uint32_t rows = 0;
+#pragma unroll
+            for (int j = 0; j < kUnroll; ++j) rows |= (rm[j] < kSpan ? 1u : 0u) << j;
+            cold(rows, p, base, sbins, compacting ? s_cnt : nullptr, s_buf, center);
         }
-        if (rows) cold(rows, p, base, sbins, compacting ? s_cnt : nullptr, s_buf, center);
         if (compacting) {               // warp-uniform
             const uint32_t c = staged();
             if (c > kStageThresh) flush(c);
