@@ -139,6 +139,35 @@ int cube_ooc_next_sweep(cube_ctx* ctx, int* more, cudaStream_t stream);
 int cube_ooc_result(cube_ctx* ctx, unsigned flags, cube_moments_t* moments, uint64_t* bins, uint64_t* outside,
                     float* median, cudaStream_t stream);
 
+/* ---- NEXT-3: one cube sharded over several GPUs as contiguous z-slabs, one process
+ * and one cube_ctx per GPU -- the paper's client/server decomposition whose merges are
+ * "associative and commutative".  libcube itself does no communication: each rank
+ * accumulates its slab with cube_ooc_begin() / cube_ooc_brick(), the caller combines the buffers below across ranks
+ * with its own collectives on the same stream (paper_1211_4896_b200/shard.py: NCCL through torch.distributed), and
+ * cube_shard_advance() then locates the bucket on the combined counts.  Per stage (three for an exact median, one
+ * without):
+ *     cube_ooc_brick(slab)                                   every rank, its own voxels (several bricks allowed)
+ *     stage 0 only:  all-gather `record` (CUBE_SHARD_RECORD_BYTES per rank) -> cube_shard_merge_records();
+ *                    all-reduce SUM `bins` (nbins x u64) and `outside` (2 x u64)
+ *     every stage:   all-reduce SUM `digits` (CUBE_SHARD_DIGITS x u64)
+ *     cube_shard_advance(&more)
+ * then cube_ooc_result() on any rank: every rank holds the same integers and, because the records are merged in
+ * rank order on every rank, the same mean / std bits.  Three rounds of 64 KiB instead of the paper's ~31 rounds of
+ * five scalars.  In stage 2 each rank counts the last digit on its own compacted candidates
+ * (or re-reads its slab when they did not fit): decided on the device, no host synchronisation anywhere. */
+#define CUBE_SHARD_RECORD_BYTES 40
+#define CUBE_SHARD_DIGITS 8192
+typedef struct {
+    void* record;      /* device: this rank's running {count, mean, M2, min key, max key, voxel total} */
+    uint64_t* bins;    /* device: histogram bins (the first nbins of CUBE_MAX_BINS) */
+    uint64_t* outside; /* device: [2] */
+    uint64_t* digits;  /* device: [CUBE_SHARD_DIGITS] digit counts of the current select pass */
+} cube_shard_buffers_t;
+int cube_shard_buffers(cube_ctx* ctx, cube_shard_buffers_t* out);
+/* `gathered`: device pointer to world x CUBE_SHARD_RECORD_BYTES (rank order).  flags: CUBE_SAMPLE_STD. */
+int cube_shard_merge_records(cube_ctx* ctx, const void* gathered, int world, unsigned flags, cudaStream_t stream);
+int cube_shard_advance(cube_ctx* ctx, int* more, cudaStream_t stream);
+
 /* Whole-cube convenience over HOST memory (pinned for full speed): streams the cube H2D through
  * double-buffered chunks overlapped with the kernels and returns moments, histogram and the exact lower
  * median in HOST memory. If the cube fits in the device workspace given at cube_host_workspace() it is kept

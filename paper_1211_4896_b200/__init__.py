@@ -32,7 +32,9 @@ SYMBOLS = ["cube_create", "cube_destroy", "cube_moments", "cube_histogram", "cub
            "cube_stream_info", "cube_strerror",
            "cube_last_cuda_error", "cube_set_launch", "cube_set_knob", "cube_launch_count",
            "cube_profile_enable", "cube_profile_reset", "cube_profile_read",
-           "cube_mad", "cube_clipped_moments", "cube_sigma_clip", "cube_minimap_dims", "cube_minimap"]
+           "cube_mad", "cube_clipped_moments", "cube_sigma_clip", "cube_minimap_dims", "cube_minimap",
+           "cube_shard_buffers", "cube_shard_merge_records", "cube_shard_advance"]
+SHARD_RECORD_BYTES, SHARD_DIGITS = 40, 8192
 KNOB_CTAS_PER_SM, KNOB_BIGHIST = 0, 1
 KIND_NAMES = ["moments", "moments_coarse", "histogram", "select_pass0", "select_pass1", "select_pass2",
               "select_cand", "select_scan", "hist_select", "probe_read", "other", "moments_window", "minimap"]
@@ -52,6 +54,11 @@ class MomentsT(ctypes.Structure):
     def as_dict(self):
         return dict(count=int(self.count), nan_count=int(self.nan_count), min=np.float32(self.min),
                     max=np.float32(self.max), mean=float(self.mean), std=float(self.std))
+
+
+class ShardBuffersT(ctypes.Structure):
+    _fields_ = [("record", ctypes.c_void_p), ("bins", ctypes.c_void_p), ("outside", ctypes.c_void_p),
+                ("digits", ctypes.c_void_p)]
 
 
 # record layout of cube_moments_t as a numpy dtype (mini-map cells)
@@ -107,6 +114,9 @@ def load():
     L.cube_sigma_clip.argtypes = [vp, vp, i64, i64, i64, f64, ci, cu, vp, vp, vp, vp]
     L.cube_minimap_dims.argtypes = [i64] * 6 + [ctypes.POINTER(i64)] * 3
     L.cube_minimap.argtypes = [vp, vp, i64, i64, i64, i64, i64, i64, cu, vp, vp]
+    L.cube_shard_buffers.argtypes = [vp, ctypes.POINTER(ShardBuffersT)]
+    L.cube_shard_merge_records.argtypes = [vp, vp, ci, cu, vp]
+    L.cube_shard_advance.argtypes = [vp, ctypes.POINTER(ci), vp]
     for name in SYMBOLS:
         getattr(L, name)
     _lib = L
@@ -285,6 +295,21 @@ class Context:
                                             ctypes.cast(ctypes.byref(r), ctypes.c_void_p) if want_median else None,
                                             stream))
         return m.as_dict(), b, o, np.float32(r.value)
+
+    # --- z-slab sharding over GPUs (NEXT-3; the collectives live in shard.py) ----------------------------
+    def shard_buffers(self):
+        """-> dict(record, bins, outside, digits) of device addresses (int)."""
+        b = ShardBuffersT()
+        self._check(self._L.cube_shard_buffers(self._h, ctypes.byref(b)))
+        return dict(record=int(b.record), bins=int(b.bins), outside=int(b.outside), digits=int(b.digits))
+
+    def shard_merge_records(self, gathered, world, flags=0, stream=0):
+        self._check(self._L.cube_shard_merge_records(self._h, _ptr(gathered), world, flags, stream))
+
+    def shard_advance(self, stream=0):
+        more = ctypes.c_int()
+        self._check(self._L.cube_shard_advance(self._h, ctypes.byref(more), stream))
+        return bool(more.value)
 
     # --- whole cube in HOST memory ---------------------------------------------------------------------
     def host_workspace(self, resident_bytes=0, chunk_bytes=0):

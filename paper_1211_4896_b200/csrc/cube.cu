@@ -288,8 +288,13 @@ int cube_create(cube_ctx** out, size_t scratch_bytes_hint) {
     bool ok = true;
     ok = ok && cudaMalloc(&c->partials, c->max_ctas * sizeof(Partial)) == cudaSuccess;
     ok = ok && cudaMalloc(&c->ticket, sizeof(unsigned int)) == cudaSuccess;
-    ok = ok && cudaMalloc(&c->acc, sizeof(Partial)) == cudaSuccess;
-    ok = ok && cudaMalloc(&c->nvox_acc, sizeof(unsigned long long)) == cudaSuccess;
+    // running (n, mean, M2, kmin, kmax) record followed by the voxel total: ONE 40-byte block, so that a sharded
+    // run can all-gather it as it is (cube_shard_buffers)
+    static_assert(sizeof(Partial) == 32, "shard record layout");
+    void* rec = nullptr;
+    ok = ok && cudaMalloc(&rec, CUBE_SHARD_RECORD_BYTES) == cudaSuccess;
+    c->acc = reinterpret_cast<Partial*>(rec);
+    c->nvox_acc = rec ? reinterpret_cast<unsigned long long*>(static_cast<char*>(rec) + sizeof(Partial)) : nullptr;
     ok = ok && cudaMalloc(&c->mom_out, sizeof(MomentsOut)) == cudaSuccess;
     ok = ok && cudaMalloc(&c->gbins, bytes_bins) == cudaSuccess;
     ok = ok && cudaMalloc(&c->gdigits, kDigitBins * sizeof(unsigned long long)) == cudaSuccess;
@@ -325,7 +330,7 @@ int cube_create(cube_ctx** out, size_t scratch_bytes_hint) {
 
 int cube_destroy(cube_ctx* c) {
     if (!c) return CUBE_EINVAL;
-    cudaFree(c->partials); cudaFree(c->ticket); cudaFree(c->acc); cudaFree(c->nvox_acc);
+    cudaFree(c->partials); cudaFree(c->ticket); cudaFree(c->acc);
     cudaFree(c->mom_out); cudaFree(c->gbins); cudaFree(c->gdigits); cudaFree(c->coarse); cudaFree(c->sel);
     cudaFree(c->range3); cudaFree(c->probe_out); cudaFree(c->plan); cudaFree(c->clip); cudaFree(c->center);
     cudaFree(c->cand);

@@ -274,6 +274,25 @@ __global__ void clip_step_kernel(const MomentsOut* __restrict__ m, ClipState* __
     st->iters += 1;
 }
 
+// NEXT-3 (z-slab sharding over GPUs): merge the all-gathered per-rank records {Partial, voxel total} in rank
+// order -- the paper's server-side O(1) combination of (count, sum, sum of squares) ("any
+// arbitrary data composition order is valid"), in Chan's cancellation-free form -- into the running record of this
+// rank and re-finalise.  Every rank does the same merge in the same order, so all ranks hold identical bits.
+__global__ void shard_merge_kernel(const unsigned char* __restrict__ gathered, int world, int rec_bytes, unsigned flags,
+                                   Partial* __restrict__ acc, unsigned long long* __restrict__ nvox,
+                                   MomentsOut* __restrict__ out) {
+    Partial m = partial_empty();
+    unsigned long long tot = 0;
+    for (int r = 0; r < world; ++r) {
+        const Partial* p = reinterpret_cast<const Partial*>(gathered + (size_t)r * rec_bytes);
+        tot += *reinterpret_cast<const unsigned long long*>(gathered + (size_t)r * rec_bytes + sizeof(Partial));
+        m = partial_merge(m, *p);
+    }
+    *acc = m;
+    *nvox = tot;
+    moments_finalize(m, tot, flags, out);
+}
+
 // Re-evaluate mean/std of the running partial with other flags (sample std) -- O(1).
 __global__ void moments_refinalize_kernel(const Partial* __restrict__ acc, const unsigned long long* __restrict__ nvox,
                                           unsigned flags, MomentsOut* __restrict__ out) {

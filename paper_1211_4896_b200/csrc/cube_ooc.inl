@@ -94,6 +94,45 @@ int cube_ooc_result(cube_ctx* c, unsigned flags, cube_moments_t* moments, uint64
     return CUBE_OK;
 }
 
+// ---- NEXT-3: z-slab sharding over several GPUs.  The library stays free of any
+// communication dependency: every rank accumulates its slab with cube_ooc_begin / cube_ooc_brick, the CALLER
+// combines the exported device buffers with its collectives (NCCL through torch.distributed in
+// paper_1211_4896_b200/shard.py), and cube_shard_advance runs the bucket-location kernel on the combined digit
+// counts -- identical on every rank, so all ranks pick the same bucket.  No host synchronisation anywhere.
+int cube_shard_buffers(cube_ctx* c, cube_shard_buffers_t* out) {
+    if (!c || !out) return CUBE_EINVAL;
+    out->record = c->acc;
+    out->bins = reinterpret_cast<uint64_t*>(c->gbins);
+    out->outside = reinterpret_cast<uint64_t*>(c->gbins + CUBE_MAX_BINS);
+    out->digits = reinterpret_cast<uint64_t*>(c->gdigits);
+    return CUBE_OK;
+}
+
+int cube_shard_merge_records(cube_ctx* c, const void* gathered, int world, unsigned flags, cudaStream_t s) {
+    if (!c || !c->ooc_active || !gathered || world < 1 || world > 65536) return CUBE_EINVAL;
+    {
+        ProfScope prof(c, CUBE_K_OTHER, s);
+        shard_merge_kernel<<<1, 1, 0, s>>>(static_cast<const unsigned char*>(gathered), world, CUBE_SHARD_RECORD_BYTES,
+                                           flags & CUBE_SAMPLE_STD, c->acc, c->nvox_acc, c->mom_out);
+    }
+    CUBE_CUDA(c, cudaGetLastError());
+    return CUBE_OK;
+}
+
+int cube_shard_advance(cube_ctx* c, int* more, cudaStream_t s) {
+    if (!c || !c->ooc_active || !more) return CUBE_EINVAL;
+    int rc = CUBE_OK;
+    *more = 0;
+    if (c->ooc_want_median) {
+        if (c->ooc_sweep == 0) { rc = launch_select_scan<0>(c, c->gdigits, s); *more = 1; }
+        else if (c->ooc_sweep == 1) { rc = launch_select_scan<1>(c, c->gdigits, s); *more = 1; }
+        else if (c->ooc_sweep == 2) { rc = launch_select_scan<2>(c, c->gdigits, s); }
+        else return CUBE_EINVAL;
+    }
+    c->ooc_sweep = c->ooc_want_median ? c->ooc_sweep + 1 : 3;
+    return rc;
+}
+
 int cube_host_workspace(cube_ctx* c, size_t resident_bytes, size_t chunk_bytes) {
     if (!c) return CUBE_EINVAL;
     if (chunk_bytes == 0) chunk_bytes = (size_t)256 << 20;
