@@ -527,19 +527,33 @@ int cube_minimap(cube_ctx* c, const float* d, int64_t nx, int64_t ny, int64_t nz
     if (!c || !d || !cells) return CUBE_EINVAL;
     if (cube_minimap_dims(nx, ny, nz, px, py, pz, (int64_t*)&g.mx, (int64_t*)&g.my, (int64_t*)&g.mz)) return CUBE_EINVAL;
     g.nx = nx; g.ny = ny; g.nz = nz; g.px = px; g.py = py; g.pz = pz;
-    g.cells_per_seg = px > kMapThreads ? 1 : kMapThreads / px;
-    g.nseg = (g.mx + g.cells_per_seg - 1) / g.cells_per_seg;
-    const long double ctas = (long double)g.nseg * (long double)g.my * (long double)g.mz;
-    if (ctas > 2147483647.0L) return CUBE_EINVAL;   // 1-D grid limit (cells of a few voxels on a huge cube)
     cudaPointerAttributes at;   // the map is consumed on the device: records are written in place
     if (cudaPointerGetAttributes(&at, cells) != cudaSuccess || at.type == cudaMemoryTypeUnregistered) {
         cudaGetLastError();
         return CUBE_EINVAL;
     }
+    // 128-bit kernel: rows 16-byte aligned, segments of whole cells that start on a multiple of 4 voxels
+    const long long unit = (px % 4 == 0) ? 1 : (px % 2 == 0) ? 2 : 4;     // cells per segment must be a multiple of it
+    const long long cps4 = (kMap4Cols / px) / unit * unit;
+    const bool v4 = (nx % 4 == 0) && (((uintptr_t)d & 15u) == 0) && cps4 >= 1 && px >= 4;
+    g.cells_per_seg = v4 ? cps4 : (px > kMapThreads ? 1 : kMapThreads / px);
+    g.nseg = (g.mx + g.cells_per_seg - 1) / g.cells_per_seg;
+    {   // balance the segments of a row (35 cells: 18 + 17 instead of 34 + 1)
+        const long long u = v4 ? unit : 1;
+        const long long even = ((g.mx + g.nseg - 1) / g.nseg + u - 1) / u * u;
+        if (even < g.cells_per_seg) { g.cells_per_seg = even; g.nseg = (g.mx + even - 1) / even; }
+    }
+    const long double ctas = (long double)g.nseg * (long double)g.my * (long double)g.mz;
+    if (ctas > 2147483647.0L) return CUBE_EINVAL;   // 1-D grid limit (cells of a few voxels on a huge cube)
     {
         ProfScope prof(c, CUBE_K_MINIMAP, s);
-        minimap_kernel<<<(unsigned)(g.nseg * g.my * g.mz), kMapThreads, 0, s>>>(d, g, flags & CUBE_SAMPLE_STD,
-                                                                               reinterpret_cast<MomentsOut*>(cells));
+        const unsigned grid = (unsigned)(g.nseg * g.my * g.mz);
+        g.main_threads = ((g.cells_per_seg * px / 4) + 31) / 32 * 32;
+        const unsigned block4 = (unsigned)g.main_threads + (unsigned)((g.cells_per_seg - 1 + 31) / 32 * 32);  // + boundary threads
+        if (v4) minimap_v4_kernel<<<grid, block4, 0, s>>>(d, g, flags & CUBE_SAMPLE_STD,
+                                                          reinterpret_cast<MomentsOut*>(cells));
+        else minimap_kernel<<<grid, kMapThreads, 0, s>>>(d, g, flags & CUBE_SAMPLE_STD,
+                                                         reinterpret_cast<MomentsOut*>(cells));
     }
     CUBE_CUDA(c, cudaGetLastError());
     return CUBE_OK;
