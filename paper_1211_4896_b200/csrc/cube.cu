@@ -22,6 +22,7 @@ struct cube_ctx {
     // device scratch
     Partial* partials = nullptr;           // one per CTA
     unsigned int* ticket = nullptr;
+    unsigned int* ticket2 = nullptr;       // arrival counter of the fused bucket-location step
     Partial* acc = nullptr;                // running moments (out-of-core)
     unsigned long long* nvox_acc = nullptr;
     MomentsOut* mom_out = nullptr;
@@ -57,6 +58,10 @@ struct cube_ctx {
     uint64_t stream_h2d_bytes = 0;   // bytes that crossed the host link in the last cube_stats_stream call
     int stream_sweeps = 0;
     int max_ctas = 0;
+    // occupancy of each kernel, asked once per (kernel, dynamic shared memory) instead of once per call
+    struct OccEntry { const void* fn; size_t smem; int occ; };
+    OccEntry occ_cache[24] = {};
+    int occ_used = 0;
     // per-kernel timing (cube_profile_*)
     int prof_on = 0;
     std::vector<cudaEvent_t> prof_ev;   // pairs
@@ -125,6 +130,17 @@ inline bool dims_ok(int64_t nx, int64_t ny, int64_t nz, uint64_t* n) {
     return true;
 }
 
+template <class K>
+int occupancy_of(cube_ctx* c, K kernel, int threads, size_t smem) {
+    const void* fn = reinterpret_cast<const void*>(kernel);
+    for (int i = 0; i < c->occ_used; ++i)
+        if (c->occ_cache[i].fn == fn && c->occ_cache[i].smem == smem) return c->occ_cache[i].occ;
+    int occ = 0;
+    if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, kernel, threads, smem) != cudaSuccess) { cudaGetLastError(); occ = 1; }
+    if (c->occ_used < 24) c->occ_cache[c->occ_used++] = {fn, smem, occ};
+    return occ;
+}
+
 inline int grid_for(const cube_ctx* c, int default_per_sm, int occ_limit) {
     int per = c->ctas_per_sm > 0 ? c->ctas_per_sm : default_per_sm;
     if (per > occ_limit) per = occ_limit;
@@ -146,28 +162,33 @@ inline bool hist_scale(int nbins, float lo, float hi, float* scale) {
 
 // mode: kMomPlain / kMomCoarse / kMomWindow (window = (wlo, whi), or the context's ClipState when use_clip)
 int launch_moments(cube_ctx* c, const float* d, uint64_t n, unsigned flags, int accumulate, cudaStream_t s,
-                   int mode = -1, float wlo = 0.f, float whi = 0.f, bool use_clip = false) {
+                   int mode = -1, float wlo = 0.f, float whi = 0.f, bool use_clip = false,
+                   const SelectInit* fuse_scan = nullptr) {
     if (mode < 0) mode = (flags & CUBE_COARSE_HIST) ? kMomCoarse : kMomPlain;
     const bool coarse = mode == kMomCoarse;
-    int occ_m = 0;
-    cudaError_t e = mode == kMomCoarse ? cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ_m, moments_kernel<kMomCoarse>, kThreads, 0)
-                  : mode == kMomWindow ? cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ_m, moments_kernel<kMomWindow>, kThreads, 0)
-                                       : cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ_m, moments_kernel<kMomPlain>, kThreads, 0);
-    if (e != cudaSuccess) occ_m = 1;
+    const int occ_m = mode == kMomCoarse ? occupancy_of(c, moments_kernel<kMomCoarse>, kThreads, 0)
+                    : mode == kMomWindow ? occupancy_of(c, moments_kernel<kMomWindow>, kThreads, 0)
+                                         : occupancy_of(c, moments_kernel<kMomPlain>, kThreads, 0);
     const int grid = grid_for(c, 4, occ_m < kMaxCtasPerSm ? occ_m : kMaxCtasPerSm);
     if (coarse && !accumulate) CUBE_CUDA(c, cudaMemsetAsync(c->coarse, 0, kDigitBins * sizeof(unsigned long long), s));
     {
     ProfScope prof(c, coarse ? CUBE_K_MOMENTS_COARSE : mode == kMomWindow ? CUBE_K_MOMENTS_WINDOW : CUBE_K_MOMENTS, s);
     const ClipState* clip = use_clip ? c->clip : nullptr;
-    if (coarse) {
+    SelectInit none;
+    none.k = 0; none.cand_cap = 0; none.use_median = 0; none.enabled = 0;
+    if (coarse) {   // fuse_scan: the kernel's last CTA also locates the first-digit bucket (cube_stats)
         moments_kernel<kMomCoarse><<<grid, kThreads, 0, s>>>(d, n, c->partials, c->ticket, c->acc, c->nvox_acc,
-                                                             accumulate, flags, c->mom_out, c->coarse, 0.f, 0.f, nullptr);
+                                                             accumulate, flags, c->mom_out, c->coarse, 0.f, 0.f, nullptr,
+                                                             c->sel, fuse_scan ? c->ticket2 : nullptr,
+                                                             fuse_scan ? *fuse_scan : none);
     } else if (mode == kMomWindow) {
         moments_kernel<kMomWindow><<<grid, kThreads, 0, s>>>(d, n, c->partials, c->ticket, c->acc, c->nvox_acc,
-                                                             accumulate, flags, c->mom_out, c->coarse, wlo, whi, clip);
+                                                             accumulate, flags, c->mom_out, c->coarse, wlo, whi, clip,
+                                                             nullptr, nullptr, none);
     } else {
         moments_kernel<kMomPlain><<<grid, kThreads, 0, s>>>(d, n, c->partials, c->ticket, c->acc, c->nvox_acc,
-                                                            accumulate, flags, c->mom_out, c->coarse, 0.f, 0.f, nullptr);
+                                                            accumulate, flags, c->mom_out, c->coarse, 0.f, 0.f, nullptr,
+                                                            nullptr, nullptr, none);
     }
     }
     CUBE_CUDA(c, cudaGetLastError());
@@ -181,10 +202,7 @@ int launch_hist(cube_ctx* c, const float* d, uint64_t n, int nbins, float lo, fl
     ProfScope prof(c, CUBE_K_HIST, s);
     if (nbins <= kSmemHistMaxBins) {
         const size_t smem = (size_t)(nbins + 2) * sizeof(uint32_t);  // + trash slot
-        int occ = 0;
-        if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, hist_smem_kernel, kThreads, smem) != cudaSuccess)
-            occ = 1;
-        const int grid = grid_for(c, 4, occ);
+        const int grid = grid_for(c, 4, occupancy_of(c, hist_smem_kernel, kThreads, smem));
         hist_smem_kernel<<<grid, kThreads, smem, s>>>(d, n, nbins, lo, hi, scale, range3, c->gbins, outside);
     } else {
         // one CTA of 1024 threads per SM: 32-bit counters for a 32768-bin window (default when the sampled plan
@@ -211,25 +229,34 @@ int launch_hist(cube_ctx* c, const float* d, uint64_t n, int nbins, float lo, fl
     return CUBE_OK;
 }
 
+inline SelectInit select_init_args(const cube_ctx* c, uint64_t k, int use_median, bool enabled) {
+    SelectInit i;
+    i.k = k; i.cand_cap = c->cand ? c->cand_cap : 0; i.use_median = use_median ? 1u : 0u; i.enabled = enabled ? 1u : 0u;
+    return i;
+}
+
+// fuse != nullptr: the last CTA of the pass also locates the bucket (select_scan_if_last) -- in-core selections
 template <int PASS, bool DEV = false>
-int launch_select_pass(cube_ctx* c, const float* d, uint64_t n, cudaStream_t s) {
-    int occ = 0;  // every CTA of the persistent grid must be resident (static tile dealing)
-    if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, select_pass_kernel<PASS, DEV>, kThreads, 0) != cudaSuccess) occ = 1;
+int launch_select_pass(cube_ctx* c, const float* d, uint64_t n, cudaStream_t s, const SelectInit* fuse = nullptr) {
+    const int occ = occupancy_of(c, select_pass_kernel<PASS, DEV>, kThreads, 0);  // every CTA must be resident (static tile dealing)
     const int grid = grid_for(c, 4, occ < kMaxCtasPerSm ? occ : kMaxCtasPerSm);
     {
         ProfScope prof(c, PASS == 0 ? CUBE_K_SELECT_PASS0 : PASS == 1 ? CUBE_K_SELECT_PASS1 : CUBE_K_SELECT_PASS2, s);
-        select_pass_kernel<PASS, DEV><<<grid, kThreads, 0, s>>>(d, n, c->sel, c->gdigits, c->cand, c->center);
+        select_pass_kernel<PASS, DEV><<<grid, kThreads, 0, s>>>(d, n, c->sel, c->gdigits, c->cand, c->center,
+                                                                fuse ? c->ticket2 : nullptr,
+                                                                fuse ? *fuse : select_init_args(c, 0, 0, false));
     }
     CUBE_CUDA(c, cudaGetLastError());
     return CUBE_OK;
 }
 
 template <int PASS>
-int launch_select_scan(cube_ctx* c, unsigned long long* digits, cudaStream_t s) {
+int launch_select_scan(cube_ctx* c, unsigned long long* digits, cudaStream_t s, const SelectInit* init = nullptr) {
     // the coarse histogram kept by CUBE_COARSE_HIST is left intact so that several k can reuse it
     {
         ProfScope prof(c, CUBE_K_SELECT_SCAN, s);
-        select_scan_kernel<PASS><<<1, 1024, 0, s>>>(c->sel, digits, digits == c->gdigits ? 1 : 0);
+        select_scan_kernel<PASS><<<1, 1024, 0, s>>>(c->sel, digits, digits == c->gdigits ? 1 : 0,
+                                                    init ? *init : select_init_args(c, 0, 0, false));
     }
     CUBE_CUDA(c, cudaGetLastError());
     return CUBE_OK;
@@ -253,18 +280,17 @@ template <bool DEV = false>
 int kth_impl(cube_ctx* c, const float* d, uint64_t n, uint64_t k, int use_median, unsigned flags, float* out,
              cudaStream_t s) {
     int rc;
-    if ((rc = select_init(c, k, use_median, s))) return rc;
+    // three launches: every pass kernel ends with the bucket location in its last CTA; the select state is
+    // initialised by the first of them from kernel arguments (no host-to-device copy)
+    const SelectInit init = select_init_args(c, k, use_median, true), cont = select_init_args(c, 0, 0, false);
     if (!DEV && (flags & CUBE_REUSE_COARSE)) {
-        if ((rc = launch_select_scan<0>(c, c->coarse, s))) return rc;
+        if ((rc = launch_select_scan<0>(c, c->coarse, s, &init))) return rc;
     } else {
         CUBE_CUDA(c, cudaMemsetAsync(c->gdigits, 0, kDigitBins * sizeof(unsigned long long), s));
-        if ((rc = launch_select_pass<0, DEV>(c, d, n, s))) return rc;
-        if ((rc = launch_select_scan<0>(c, c->gdigits, s))) return rc;
+        if ((rc = launch_select_pass<0, DEV>(c, d, n, s, &init))) return rc;
     }
-    if ((rc = launch_select_pass<1, DEV>(c, d, n, s))) return rc;
-    if ((rc = launch_select_scan<1>(c, c->gdigits, s))) return rc;
-    if ((rc = launch_select_pass<2, DEV>(c, d, n, s))) return rc;
-    if ((rc = launch_select_scan<2>(c, c->gdigits, s))) return rc;
+    if ((rc = launch_select_pass<1, DEV>(c, d, n, s, &cont))) return rc;
+    if ((rc = launch_select_pass<2, DEV>(c, d, n, s, &cont))) return rc;
     if (out) CUBE_CUDA(c, cudaMemcpyAsync(out, &c->sel->result, sizeof(float), cudaMemcpyDefault, s));
     return CUBE_OK;
 }
@@ -288,6 +314,8 @@ int cube_create(cube_ctx** out, size_t scratch_bytes_hint) {
     bool ok = true;
     ok = ok && cudaMalloc(&c->partials, c->max_ctas * sizeof(Partial)) == cudaSuccess;
     ok = ok && cudaMalloc(&c->ticket, sizeof(unsigned int)) == cudaSuccess;
+    ok = ok && cudaMalloc(&c->ticket2, sizeof(unsigned int)) == cudaSuccess;
+    ok = ok && cudaMemset(c->ticket2, 0, sizeof(unsigned int)) == cudaSuccess;
     // running (n, mean, M2, kmin, kmax) record followed by the voxel total: ONE 40-byte block, so that a sharded
     // run can all-gather it as it is (cube_shard_buffers)
     static_assert(sizeof(Partial) == 32, "shard record layout");
@@ -330,7 +358,7 @@ int cube_create(cube_ctx** out, size_t scratch_bytes_hint) {
 
 int cube_destroy(cube_ctx* c) {
     if (!c) return CUBE_EINVAL;
-    cudaFree(c->partials); cudaFree(c->ticket); cudaFree(c->acc);
+    cudaFree(c->partials); cudaFree(c->ticket); cudaFree(c->ticket2); cudaFree(c->acc);
     cudaFree(c->mom_out); cudaFree(c->gbins); cudaFree(c->gdigits); cudaFree(c->coarse); cudaFree(c->sel);
     cudaFree(c->range3); cudaFree(c->probe_out); cudaFree(c->plan); cudaFree(c->clip); cudaFree(c->center);
     cudaFree(c->cand);
@@ -418,10 +446,9 @@ int cube_stats(cube_ctx* c, const float* d, int64_t nx, int64_t ny, int64_t nz, 
     }
     int rc;
     // pass A: moments (+ first select digit)
-    if (want_median && (rc = select_init(c, 0, 1, s))) return rc;
+    const SelectInit init = select_init_args(c, 0, 1, true), cont = select_init_args(c, 0, 0, false);
     const unsigned mflags = (flags & CUBE_SAMPLE_STD) | (want_median ? (unsigned)CUBE_COARSE_HIST : 0u);
-    if ((rc = launch_moments(c, d, n, mflags, 0, s))) return rc;
-    if (want_median && (rc = launch_select_scan<0>(c, c->coarse, s))) return rc;
+    if ((rc = launch_moments(c, d, n, mflags, 0, s, -1, 0.f, 0.f, false, want_median ? &init : nullptr))) return rc;
     if (want_hist) {
         CUBE_CUDA(c, cudaMemsetAsync(c->gbins, 0, (size_t)nbins * sizeof(unsigned long long), s));
         CUBE_CUDA(c, cudaMemsetAsync(c->gbins + CUBE_MAX_BINS, 0, 2 * sizeof(unsigned long long), s));
@@ -431,13 +458,12 @@ int cube_stats(cube_ctx* c, const float* d, int64_t nx, int64_t ny, int64_t nz, 
     if (want_median) CUBE_CUDA(c, cudaMemsetAsync(c->gdigits, 0, kDigitBins * sizeof(unsigned long long), s));
     if (want_median && want_hist && nbins <= kSmemHistMaxBins) {
         const size_t smem = (size_t)hist_select_smem(nbins);
-        int occ = 0;
-        if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, hist_select_kernel, kThreads, smem) != cudaSuccess) occ = 1;
+        const int occ = occupancy_of(c, hist_select_kernel, kThreads, smem);
         const int grid = grid_for(c, 4, occ < kMaxCtasPerSm ? occ : kMaxCtasPerSm);
         {
             ProfScope prof(c, CUBE_K_HIST_SELECT, s);
             hist_select_kernel<<<grid, kThreads, smem, s>>>(d, n, nbins, lo, hi, scale, minmax ? c->mom_out : nullptr,
-                                                            c->gbins, goutside, c->sel, c->gdigits, c->cand);
+                                                            c->gbins, goutside, c->sel, c->gdigits, c->cand, c->ticket2);
         }
         CUBE_CUDA(c, cudaGetLastError());
     } else {
@@ -451,12 +477,10 @@ int cube_stats(cube_ctx* c, const float* d, int64_t nx, int64_t ny, int64_t nz, 
             }
             if ((rc = launch_hist(c, d, n, nbins, lo, hi, scale, s, minmax ? c->range3 : nullptr))) return rc;
         }
-        if (want_median && (rc = launch_select_pass<1>(c, d, n, s))) return rc;
+        if (want_median && (rc = launch_select_pass<1>(c, d, n, s, &cont))) return rc;
     }
     if (want_median) {
-        if ((rc = launch_select_scan<1>(c, c->gdigits, s))) return rc;
-        if ((rc = launch_select_pass<2>(c, d, n, s))) return rc;   // on the candidates unless they did not fit
-        if ((rc = launch_select_scan<2>(c, c->gdigits, s))) return rc;
+        if ((rc = launch_select_pass<2>(c, d, n, s, &cont))) return rc;   // on the candidates unless they did not fit
         CUBE_CUDA(c, cudaMemcpyAsync(median, &c->sel->result, sizeof(float), cudaMemcpyDefault, s));
     }
     if (moments) CUBE_CUDA(c, cudaMemcpyAsync(moments, c->mom_out, sizeof(MomentsOut), cudaMemcpyDefault, s));

@@ -67,7 +67,8 @@ __global__ void __launch_bounds__(kThreads, 3)
 hist_select_kernel(const float* __restrict__ d, uint64_t n, int nbins, float lo, float hi, float scale,
                    const MomentsOut* __restrict__ range_from, unsigned long long* __restrict__ gbins,
                    unsigned long long* __restrict__ goutside, SelectState* __restrict__ st,
-                   unsigned long long* __restrict__ gdigits, uint32_t* __restrict__ cand) {
+                   unsigned long long* __restrict__ gdigits, uint32_t* __restrict__ cand,
+                   unsigned int* __restrict__ scan_ticket) {
     extern __shared__ uint32_t dyn_bins[];
     __shared__ uint32_t s_out[2];
     uint32_t* hbins = dyn_bins;
@@ -101,6 +102,12 @@ hist_select_kernel(const float* __restrict__ d, uint64_t n, int nbins, float lo,
         if (threadIdx.x < 2 && s_out[threadIdx.x]) atomicAdd(&goutside[threadIdx.x], (unsigned long long)s_out[threadIdx.x]);
     } else if (blockIdx.x == 0 && threadIdx.x < 2) {
         goutside[threadIdx.x] = ~0ull;  // marker: the [min,max] range was unusable
+    }
+    if (scan_ticket) {   // the last CTA locates the second-digit bucket (no separate scan launch)
+        __shared__ unsigned long long scan_sm[kScanSmem];
+        SelectInit none;
+        none.k = 0; none.cand_cap = 0; none.use_median = 0; none.enabled = 0;
+        select_scan_if_last<1>(st, gdigits, 1, none, scan_ticket, scan_sm);
     }
 }
 

@@ -8,6 +8,7 @@
 #include <math.h>
 
 #include "cube_common.cuh"
+#include "cube_select.cuh"
 
 namespace cube {
 
@@ -17,21 +18,6 @@ struct MomentsOut {
     float min, max;
     double mean, std;
 };
-
-// State of one exact selection (radix select).  Lives in device memory so that the
-// bucket choice after each digit pass never crosses to the host (the paper's server round trip per
-// iteration, becomes a 1-CTA kernel).
-struct SelectState {
-    unsigned long long k;       // residual rank inside the current prefix bucket
-    unsigned long long count;   // non-NaN voxels (sum of the pass-0 digit histogram)
-    uint32_t prefix;            // key bits fixed so far (right aligned)
-    uint32_t invalid;           // 1 when k >= count (result NaN)
-    uint32_t use_median;        // 1: k = (count-1)/2 is set by the pass-0 scan
-    float result;
-    unsigned long long cand_n;  // keys of the pass-0 bucket seen by the compacting pass 1
-    unsigned long long cand_cap;  // capacity of the candidate buffer, in keys
-};
-
 
 // ------------------------------------------------------------------------------------------------
 // Moments: steps 1-3 of SURVEY.md sec. 8(a) (+ 3b when COARSE): count, min, max, pivoted fp64 sums.
@@ -200,7 +186,8 @@ moments_kernel(const float* __restrict__ d, uint64_t n, Partial* __restrict__ pa
                unsigned int* __restrict__ ticket, Partial* __restrict__ acc,
                unsigned long long* __restrict__ nvox_acc, int accumulate, unsigned flags,
                MomentsOut* __restrict__ out, unsigned long long* __restrict__ gdigits,
-               float wlo, float whi, const ClipState* __restrict__ clip) {
+               float wlo, float whi, const ClipState* __restrict__ clip,
+               SelectState* __restrict__ sel, unsigned int* __restrict__ scan_ticket, SelectInit init) {
     constexpr bool COARSE = (MODE == kMomCoarse);
     __shared__ Partial scratch[kThreads / 32];
     __shared__ uint32_t sbins[COARSE ? kDigitBins + 1 : 1];
@@ -225,6 +212,10 @@ moments_kernel(const float* __restrict__ d, uint64_t n, Partial* __restrict__ pa
         for (int i = threadIdx.x; i < kDigitBins; i += kThreads) {
             uint32_t c = sbins[i];
             if (c) atomicAdd(&gdigits[i], (unsigned long long)c);
+        }
+        if (scan_ticket) {   // cube_stats: the last CTA locates the median's first-digit bucket (no scan launch)
+            __shared__ unsigned long long scan_sm[kScanSmem];
+            select_scan_if_last<0>(sel, gdigits, 0, init, scan_ticket, scan_sm);
         }
     }
     if (threadIdx.x == 0) {
@@ -567,6 +558,5 @@ probe_read_kernel(const float* __restrict__ d, uint64_t n, float* __restrict__ o
 }  // namespace cube
 
 #include "cube_hist_big.cuh"
-#include "cube_select.cuh"
 #include "cube_fused.cuh"
 #include "cube_minimap.cuh"

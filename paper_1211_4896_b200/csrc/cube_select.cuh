@@ -14,6 +14,20 @@
 
 namespace cube {
 
+// State of one exact selection (radix select).  Lives in device memory so that the
+// bucket choice after each digit pass never crosses to the host (the paper's server round trip per
+// iteration, becomes a 1-CTA kernel).
+struct SelectState {
+    unsigned long long k;       // residual rank inside the current prefix bucket
+    unsigned long long count;   // non-NaN voxels (sum of the pass-0 digit histogram)
+    uint32_t prefix;            // key bits fixed so far (right aligned)
+    uint32_t invalid;           // 1 when k >= count (result NaN)
+    uint32_t use_median;        // 1: k = (count-1)/2 is set by the pass-0 scan
+    float result;
+    unsigned long long cand_n;  // keys of the pass-0 bucket seen by the compacting pass 1
+    unsigned long long cand_cap;  // capacity of the candidate buffer, in keys
+};
+
 // PASS 1 compaction ("step 8"): every warp stages the keys of the prefix bucket in its own slice of shared
 // memory and moves them to the candidate buffer in coalesced runs, reserving the space with ONE global atomic
 // per flush.  A warp checks its fill level once per tile (1024 voxels per warp), so a slice holds the flush
@@ -193,12 +207,160 @@ __device__ __forceinline__ void select_run(const float* __restrict__ d, uint64_t
     f.finish();
 }
 
+// Bucket location (step 7: the paper's server-side "determine the next guess"): exclusive scan of
+// the digit histogram, pick the bucket holding rank k, update (prefix, k), clear the histogram for the next pass.
+// After PASS 2 the 32-bit key is complete and is mapped back to the float.  Run by ONE CTA of THREADS threads:
+// either the stand-alone select_scan_kernel (brick-streamed and sharded runs, CUBE_REUSE_COARSE) or -- fused -- the
+// last CTA to finish the pass kernel that produced the counts (in-core calls: three launches fewer per selection).
+// With init.enabled (PASS 0) the whole SelectState is initialised here from kernel arguments, so no host-to-device
+// copy precedes a selection.  `sm` = kScanSmem words of shared memory.
+struct SelectInit {
+    unsigned long long k, cand_cap;
+    uint32_t use_median, enabled;
+};
+
+constexpr int kScanSmem = 256 + 4;   // words (u64) of shared memory select_scan_body needs
+
+__device__ __forceinline__ unsigned long long warp_sum_u64(unsigned long long v) {
+#pragma unroll
+    for (int off = 16; off > 0; off >>= 1) v += __shfl_xor_sync(0xffffffffu, v, off);
+    return v;
+}
+
+// Two levels, every global load coalesced and independent of the others: (1) each warp sums chunks of 32 consecutive
+// bins (one load per lane per chunk, several chunks in flight) into shared memory; (2) warp 0 scans the <= 256 chunk
+// totals, finds the chunk holding rank k, loads that chunk once more and finds the bin.  ~2-3 us for 8192 bins
+// (the one-thread-per-32-bins form spent 5-10 us in dependent L2 round trips).
+template <int PASS, int THREADS>
+__device__ __forceinline__ void select_scan_body(SelectState* __restrict__ st, unsigned long long* __restrict__ gdigits,
+                                                 int clear, const SelectInit& init, unsigned long long* sm) {
+    constexpr int NB = (PASS == 0) ? kBins0 : (PASS == 1) ? kBins1 : kBins2;
+    constexpr int BITS = (PASS == 0) ? kBits0 : (PASS == 1) ? kBits1 : kBits2;
+    constexpr int CHUNKS = NB / 32, NW = THREADS / 32;
+    constexpr int CPL = (CHUNKS + 31) / 32;     // chunk totals per lane of warp 0
+    static_assert(CHUNKS <= 256, "chunk totals must fit the shared array");
+    unsigned long long* ctot = sm;              // [256]
+    unsigned long long& s_excl = sm[256];       // rank of the first element of the chosen chunk
+    unsigned long long& s_k = sm[257];
+    unsigned long long& s_flags = sm[258];      // invalid | chunk << 1 | prefix << 32
+    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    auto bin = [&](uint32_t b) -> unsigned long long {   // PASS 0 bins are indexed by the raw top bits of the float
+        return __ldcg(&gdigits[PASS == 0 ? raw_of_digit(b) : b]);
+    };
+#pragma unroll 4
+    for (int ch = warp; ch < CHUNKS; ch += NW) {
+        const unsigned long long v = warp_sum_u64(bin((uint32_t)(ch * 32 + lane)));
+        if (lane == 0) ctot[ch] = v;
+    }
+    __syncthreads();
+    if (warp == 0) {
+        unsigned long long c[CPL], mine = 0;
+#pragma unroll
+        for (int j = 0; j < CPL; ++j) { c[j] = (lane * CPL + j < CHUNKS) ? ctot[lane * CPL + j] : 0ull; mine += c[j]; }
+        unsigned long long incl = mine;
+#pragma unroll
+        for (int off = 1; off < 32; off <<= 1) {
+            unsigned long long v = __shfl_up_sync(0xffffffffu, incl, off);
+            if (lane >= off) incl += v;
+        }
+        const unsigned long long total = __shfl_sync(0xffffffffu, incl, 31);
+        // rank, validity and prefix: the same values in every lane
+        unsigned long long k;
+        uint32_t invalid, prefix;
+        if (PASS == 0) {
+            const bool med = init.enabled ? init.use_median != 0 : st->use_median != 0;
+            k = init.enabled ? init.k : st->k;
+            if (med) k = total ? (total - 1) / 2 : 0;
+            invalid = (k >= total) ? 1u : 0u;
+            prefix = 0;
+        } else {
+            k = st->k; invalid = st->invalid; prefix = st->prefix;
+        }
+        __syncwarp();
+        if (lane == 0) {
+            if (PASS == 0) {
+                st->count = total; st->invalid = invalid;
+                if (init.enabled) {
+                    st->use_median = init.use_median; st->cand_n = 0; st->cand_cap = init.cand_cap;
+                }
+            }
+            if (PASS == 0 || invalid) { st->k = k; st->prefix = prefix; st->result = __int_as_float(0x7fc00000); }
+            s_k = k;
+            s_flags = (unsigned long long)invalid | ((unsigned long long)prefix << 32);
+        }
+        __syncwarp();
+        if (!invalid) {
+            unsigned long long excl = incl - mine;
+#pragma unroll
+            for (int j = 0; j < CPL; ++j) {
+                if (c[j] && excl <= k && k < excl + c[j]) {   // exactly one (lane, j)
+                    s_excl = excl;
+                    s_flags |= (unsigned long long)(lane * CPL + j) << 1;
+                }
+                excl += c[j];
+            }
+        }
+        __syncwarp();
+        if (!invalid) {
+            const uint32_t ch = (uint32_t)((s_flags >> 1) & 0x7FFFFFFFu);
+            const unsigned long long kk = s_k - s_excl;           // rank inside the chunk
+            const unsigned long long v = bin(ch * 32 + lane);
+            unsigned long long inc2 = v;
+#pragma unroll
+            for (int off = 1; off < 32; off <<= 1) {
+                unsigned long long u = __shfl_up_sync(0xffffffffu, inc2, off);
+                if (lane >= off) inc2 += u;
+            }
+            const unsigned long long ex2 = inc2 - v;
+            if (v && ex2 <= kk && kk < inc2) {                    // exactly one lane
+                const uint32_t b = ch * 32 + lane;
+                const uint32_t pre = (PASS == 0) ? b : ((prefix << BITS) | b);
+                st->prefix = pre;
+                st->k = kk - ex2;
+                if (PASS == 2) st->result = __uint_as_float(bits_of_key(pre));
+            }
+        }
+    }
+    if (clear) {  // leave the digit bins zeroed for the next pass
+        __syncthreads();   // warp 0 has re-read its chunk
+        for (int i = tid; i < kDigitBins; i += THREADS) gdigits[i] = 0ull;
+    }
+}
+
+template <int PASS>
+__global__ void __launch_bounds__(1024)
+select_scan_kernel(SelectState* __restrict__ st, unsigned long long* __restrict__ gdigits, int clear, SelectInit init) {
+    __shared__ unsigned long long sm[kScanSmem];
+    select_scan_body<PASS, 1024>(st, gdigits, clear, init, sm);
+}
+
+// Fused form: called by every thread of every CTA at the end of a pass kernel, after the CTA's counters have gone
+// to gdigits.  The last CTA to arrive (ticket) runs the scan; returns true in that CTA.
+template <int PASS>
+__device__ __forceinline__ bool select_scan_if_last(SelectState* __restrict__ st, unsigned long long* __restrict__ gdigits,
+                                                    int clear, const SelectInit& init, unsigned int* __restrict__ ticket,
+                                                    unsigned long long* sm) {
+    __shared__ bool last;
+    __threadfence();      // this thread's REDs to gdigits
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        const unsigned int t = atomicAdd(ticket, 1u);
+        last = (t == gridDim.x - 1);
+    }
+    __syncthreads();
+    if (!last) return false;
+    __threadfence();
+    select_scan_body<PASS, kThreads>(st, gdigits, clear, init, sm);
+    if (threadIdx.x == 0) *ticket = 0u;
+    return true;
+}
+
 // DEV: rank y = |fl32(x - *center)| (cube_mad); center is a device pointer (the median found just before).
 template <int PASS, bool DEV>
 __global__ void __launch_bounds__(kThreads, 4)
 select_pass_kernel(const float* __restrict__ d, uint64_t n, SelectState* __restrict__ st,
                    unsigned long long* __restrict__ gdigits, uint32_t* __restrict__ cand,
-                   const float* __restrict__ center) {
+                   const float* __restrict__ center, unsigned int* __restrict__ scan_ticket, SelectInit init) {
     constexpr int NB = (PASS == 0) ? kBins0 : (PASS == 1) ? kBins1 : kBins2;
     __shared__ uint32_t sbins[NB + 1];  // + trash counter
     __shared__ uint32_t stage[(PASS == 1) ? (kThreads / 32) * (kStageCap + 1) : 1];
@@ -216,6 +378,10 @@ select_pass_kernel(const float* __restrict__ d, uint64_t n, SelectState* __restr
     for (int i = threadIdx.x; i < NB; i += kThreads) {
         uint32_t c = sbins[i];
         if (c) atomicAdd(&gdigits[i], (unsigned long long)c);
+    }
+    if (scan_ticket) {   // in-core selection: the last CTA locates the bucket (no separate scan launch)
+        __shared__ unsigned long long scan_sm[kScanSmem];
+        select_scan_if_last<PASS>(st, gdigits, 1, init, scan_ticket, scan_sm);
     }
 }
 
@@ -235,78 +401,6 @@ select_cand_kernel(SelectState* __restrict__ st, unsigned long long* __restrict_
     for (int i = threadIdx.x; i < kBins2; i += kThreads) {
         uint32_t c = sbins[i];
         if (c) atomicAdd(&gdigits[i], (unsigned long long)c);
-    }
-}
-
-// One CTA of 1024 threads: exclusive scan of the digit histogram, pick the bucket holding rank k,
-// update (prefix, k), clear the histogram for the next pass (step 7: the paper's server-side "determine
-// the next guess").  After PASS 2 the 32-bit key is complete and is mapped back to the float.
-template <int PASS>
-__global__ void __launch_bounds__(1024)
-select_scan_kernel(SelectState* __restrict__ st, unsigned long long* __restrict__ gdigits, int clear) {
-    constexpr int NB = (PASS == 0) ? kBins0 : (PASS == 1) ? kBins1 : kBins2;
-    constexpr int BITS = (PASS == 0) ? kBits0 : (PASS == 1) ? kBits1 : kBits2;
-    constexpr int PER = (NB >= 1024) ? NB / 1024 : 1;   // thread t owns bins [t*PER, t*PER+PER) (those below NB)
-    __shared__ unsigned long long warp_tot[32];
-    __shared__ unsigned long long s_k;
-    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
-    unsigned long long c[PER];
-    unsigned long long mine = 0;
-#pragma unroll
-    for (int j = 0; j < PER; ++j) {  // PASS 0 bins are indexed by the raw top bits of the float
-        const uint32_t b = (uint32_t)(tid * PER + j);
-        c[j] = (b < (uint32_t)NB) ? gdigits[PASS == 0 ? raw_of_digit(b) : b] : 0ull;
-        mine += c[j];
-    }
-    unsigned long long incl = mine;
-#pragma unroll
-    for (int off = 1; off < 32; off <<= 1) {
-        unsigned long long v = __shfl_up_sync(0xffffffffu, incl, off);
-        if (lane >= off) incl += v;
-    }
-    if (lane == 31) warp_tot[warp] = incl;
-    __syncthreads();
-    if (warp == 0) {
-        unsigned long long w = warp_tot[lane], wi = w;
-#pragma unroll
-        for (int off = 1; off < 32; off <<= 1) {
-            unsigned long long v = __shfl_up_sync(0xffffffffu, wi, off);
-            if (lane >= off) wi += v;
-        }
-        warp_tot[lane] = wi - w;  // exclusive prefix of warp totals
-        if (lane == 31) {
-            const unsigned long long total = wi;  // over all bins
-            if (PASS == 0) {
-                st->count = total;
-                if (st->use_median) st->k = total ? (total - 1) / 2 : 0;
-                st->invalid = (st->k >= total) ? 1u : 0u;
-            }
-            s_k = st->k;
-        }
-    }
-    __syncthreads();
-    const unsigned long long k = s_k;
-    unsigned long long excl = warp_tot[warp] + (incl - mine);
-    const bool invalid = st->invalid != 0;
-    const uint32_t prefix = st->prefix;
-    __syncthreads();
-    if (!invalid) {
-#pragma unroll
-        for (int j = 0; j < PER; ++j) {
-            if (c[j] && excl <= k && k < excl + c[j]) {  // exactly one (thread, j) satisfies this
-                const uint32_t b = (uint32_t)(tid * PER + j);
-                const uint32_t pre = (PASS == 0) ? b : ((prefix << BITS) | b);
-                st->prefix = pre;
-                st->k = k - excl;
-                if (PASS == 2) st->result = __uint_as_float(bits_of_key(pre));
-            }
-            excl += c[j];
-        }
-    } else if (tid == 0) {
-        st->result = __int_as_float(0x7fc00000);
-    }
-    if (clear) {  // leave the digit bins zeroed for the next pass
-        for (int i = tid; i < kDigitBins; i += 1024) gdigits[i] = 0ull;
     }
 }
 
