@@ -196,7 +196,7 @@ int launch_moments(cube_ctx* c, const float* d, uint64_t n, unsigned flags, int 
 }
 
 int launch_hist(cube_ctx* c, const float* d, uint64_t n, int nbins, float lo, float hi, float scale,
-                cudaStream_t s, const float* range3 = nullptr) {
+                cudaStream_t s, const float* range3 = nullptr, bool fused_select = false) {
     unsigned long long* outside = c->gbins + CUBE_MAX_BINS;
     {
     ProfScope prof(c, CUBE_K_HIST, s);
@@ -214,7 +214,11 @@ int launch_hist(cube_ctx* c, const float* d, uint64_t n, int nbins, float lo, fl
         } else {
             hist_window_kernel<<<1, kBigThreads, 0, s>>>(d, n, nbins, lo, hi, scale, range3, c->plan);
             const bool window_allowed = c->bighist != 2;
-            if (window_allowed) {
+            if (fused_select) {   // cube_stats: window histogram + second select digit in one kernel
+                c->launches++;
+                hist_win_select_kernel<<<c->num_sms, kBigThreads, kBigFusedSmem, s>>>(
+                    d, n, nbins, lo, hi, scale, range3, c->plan, c->gbins, outside, c->sel, c->gdigits, c->cand, c->ticket2);
+            } else if (window_allowed) {
                 c->launches++;
                 hist_win_kernel<<<c->num_sms, kBigThreads, smem, s>>>(d, n, nbins, lo, hi, scale, range3, c->plan,
                                                                       c->gbins, outside);
@@ -237,14 +241,15 @@ inline SelectInit select_init_args(const cube_ctx* c, uint64_t k, int use_median
 
 // fuse != nullptr: the last CTA of the pass also locates the bucket (select_scan_if_last) -- in-core selections
 template <int PASS, bool DEV = false>
-int launch_select_pass(cube_ctx* c, const float* d, uint64_t n, cudaStream_t s, const SelectInit* fuse = nullptr) {
+int launch_select_pass(cube_ctx* c, const float* d, uint64_t n, cudaStream_t s, const SelectInit* fuse = nullptr,
+                       const uint32_t* skip_if_set = nullptr) {
     const int occ = occupancy_of(c, select_pass_kernel<PASS, DEV>, kThreads, 0);  // every CTA must be resident (static tile dealing)
     const int grid = grid_for(c, 4, occ < kMaxCtasPerSm ? occ : kMaxCtasPerSm);
     {
         ProfScope prof(c, PASS == 0 ? CUBE_K_SELECT_PASS0 : PASS == 1 ? CUBE_K_SELECT_PASS1 : CUBE_K_SELECT_PASS2, s);
         select_pass_kernel<PASS, DEV><<<grid, kThreads, 0, s>>>(d, n, c->sel, c->gdigits, c->cand, c->center,
                                                                 fuse ? c->ticket2 : nullptr,
-                                                                fuse ? *fuse : select_init_args(c, 0, 0, false));
+                                                                fuse ? *fuse : select_init_args(c, 0, 0, false), skip_if_set);
     }
     CUBE_CUDA(c, cudaGetLastError());
     return CUBE_OK;
@@ -345,6 +350,8 @@ int cube_create(cube_ctx** out, size_t scratch_bytes_hint) {
                                     (kBigWords + 4) * (int)sizeof(uint32_t)) == cudaSuccess;
     ok = ok && cudaFuncSetAttribute(hist_win_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize,
                                     (kBigWords + 4) * (int)sizeof(uint32_t)) == cudaSuccess;
+    ok = ok && cudaFuncSetAttribute(hist_win_select_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                    kBigFusedSmem) == cudaSuccess;
     ok = ok && cudaFuncSetAttribute(hist_dsm_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize,
                                     (32768 + 1) * (int)sizeof(uint32_t)) == cudaSuccess;
     if (!ok) { cube_destroy(c); return CUBE_ENOMEM; }
@@ -475,9 +482,15 @@ int cube_stats(cube_ctx* c, const float* d, int64_t nx, int64_t ny, int64_t nz, 
                 }
                 CUBE_CUDA(c, cudaGetLastError());
             }
-            if ((rc = launch_hist(c, d, n, nbins, lo, hi, scale, s, minmax ? c->range3 : nullptr))) return rc;
-        }
-        if (want_median && (rc = launch_select_pass<1>(c, d, n, s, &cont))) return rc;
+            // more than 16384 bins together with the median: the window histogram and the second select digit
+            // share one read (hist_win_select_kernel) when the sampled plan allows the window; the packed
+            // histogram and select_pass_kernel<1> are enqueued behind it and return at once in that case
+            const bool fused_big = want_median && nbins > kSmemHistMaxBins && c->bighist == 0;
+            if ((rc = launch_hist(c, d, n, nbins, lo, hi, scale, s, minmax ? c->range3 : nullptr, fused_big))) return rc;
+            if (fused_big) {
+                if ((rc = launch_select_pass<1>(c, d, n, s, &cont, &c->plan->use_window))) return rc;
+            } else if (want_median && (rc = launch_select_pass<1>(c, d, n, s, &cont))) return rc;
+        } else if (want_median && (rc = launch_select_pass<1>(c, d, n, s, &cont))) return rc;
     }
     if (want_median) {
         if ((rc = launch_select_pass<2>(c, d, n, s, &cont))) return rc;   // on the candidates unless they did not fit

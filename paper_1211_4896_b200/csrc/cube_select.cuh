@@ -336,10 +336,10 @@ select_scan_kernel(SelectState* __restrict__ st, unsigned long long* __restrict_
 
 // Fused form: called by every thread of every CTA at the end of a pass kernel, after the CTA's counters have gone
 // to gdigits.  The last CTA to arrive (ticket) runs the scan; returns true in that CTA.
-template <int PASS>
-__device__ __forceinline__ bool select_scan_if_last(SelectState* __restrict__ st, unsigned long long* __restrict__ gdigits,
-                                                    int clear, const SelectInit& init, unsigned int* __restrict__ ticket,
-                                                    unsigned long long* sm) {
+template <int PASS, int THREADS>
+__device__ __forceinline__ bool select_scan_if_last_n(SelectState* __restrict__ st, unsigned long long* __restrict__ gdigits,
+                                                      int clear, const SelectInit& init, unsigned int* __restrict__ ticket,
+                                                      unsigned long long* sm) {
     __shared__ bool last;
     __threadfence();      // this thread's REDs to gdigits
     __syncthreads();
@@ -350,9 +350,15 @@ __device__ __forceinline__ bool select_scan_if_last(SelectState* __restrict__ st
     __syncthreads();
     if (!last) return false;
     __threadfence();
-    select_scan_body<PASS, kThreads>(st, gdigits, clear, init, sm);
+    select_scan_body<PASS, THREADS>(st, gdigits, clear, init, sm);
     if (threadIdx.x == 0) *ticket = 0u;
     return true;
+}
+template <int PASS>
+__device__ __forceinline__ bool select_scan_if_last(SelectState* __restrict__ st, unsigned long long* __restrict__ gdigits,
+                                                    int clear, const SelectInit& init, unsigned int* __restrict__ ticket,
+                                                    unsigned long long* sm) {
+    return select_scan_if_last_n<PASS, kThreads>(st, gdigits, clear, init, ticket, sm);
 }
 
 // DEV: rank y = |fl32(x - *center)| (cube_mad); center is a device pointer (the median found just before).
@@ -360,8 +366,10 @@ template <int PASS, bool DEV>
 __global__ void __launch_bounds__(kThreads, 4)
 select_pass_kernel(const float* __restrict__ d, uint64_t n, SelectState* __restrict__ st,
                    unsigned long long* __restrict__ gdigits, uint32_t* __restrict__ cand,
-                   const float* __restrict__ center, unsigned int* __restrict__ scan_ticket, SelectInit init) {
+                   const float* __restrict__ center, unsigned int* __restrict__ scan_ticket, SelectInit init,
+                   const uint32_t* __restrict__ skip_if_set) {
     constexpr int NB = (PASS == 0) ? kBins0 : (PASS == 1) ? kBins1 : kBins2;
+    if (skip_if_set && *skip_if_set) return;   // hist_win_select_kernel has done this pass (BigHistPlan::use_window)
     __shared__ uint32_t sbins[NB + 1];  // + trash counter
     __shared__ uint32_t stage[(PASS == 1) ? (kThreads / 32) * (kStageCap + 1) : 1];
     for (int i = threadIdx.x; i <= NB; i += kThreads) sbins[i] = 0;
