@@ -118,9 +118,10 @@ int cube_median_ex(cube_ctx* ctx, const float* d, int64_t nx, int64_t ny, int64_
  * flags: CUBE_SAMPLE_STD; CUBE_RANGE_MINMAX = histogram over [min,max] (lo/hi ignored).  With
  * CUBE_RANGE_MINMAX, when there is no non-NaN voxel, an extremum is infinite, or max-min or nbins/(max-min)
  * overflows float32 (the cases cube_histogram rejects with CUBE_EINVAL), all bins are 0 and
- * outside[0] = outside[1] = UINT64_MAX.  More than 16384 bins together with the median take a third read
- * (histogram and select run as separate kernels).  The first-digit histogram stays in the context for
- * cube_kth_ex(..., CUBE_REUSE_COARSE). */
+ * outside[0] = outside[1] = UINT64_MAX.  More than 16384 bins: still two reads when the voxels concentrate in a
+ * window of 32768 consecutive bins (decided on the device from a sample; the usual case for a noise-dominated cube),
+ * else a third read (packed histogram and select as separate kernels).  The first-digit histogram stays in the
+ * context for cube_kth_ex(..., CUBE_REUSE_COARSE). */
 int cube_stats(cube_ctx* ctx, const float* d, int64_t nx, int64_t ny, int64_t nz, int nbins, float lo, float hi,
                unsigned flags, cube_moments_t* moments, uint64_t* bins /* [nbins] */, uint64_t* outside /* [2] */,
                float* median, cudaStream_t stream);
@@ -275,7 +276,7 @@ enum {
     CUBE_K_SELECT_PASS2 = 5,   /* last digit: on the candidate buffer (normal) or over the cube (fallback) */
     CUBE_K_SELECT_CAND = 6,    /* last digit on the candidates, brick-streamed path */
     CUBE_K_SELECT_SCAN = 7,    /* 1-CTA bucket location kernels */
-    CUBE_K_HIST_SELECT = 8,    /* hist_select_kernel (pass B of cube_stats) */
+    CUBE_K_HIST_SELECT = 8,    /* hist_select_kernel / hist_win_select_kernel (pass B of cube_stats) */
     CUBE_K_PROBE = 9,          /* cube_probe_read */
     CUBE_K_OTHER = 10,
     CUBE_K_MOMENTS_WINDOW = 11, /* moments_kernel<window>: cube_clipped_moments, cube_sigma_clip passes */

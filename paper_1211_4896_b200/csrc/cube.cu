@@ -199,7 +199,7 @@ int launch_hist(cube_ctx* c, const float* d, uint64_t n, int nbins, float lo, fl
                 cudaStream_t s, const float* range3 = nullptr, bool fused_select = false) {
     unsigned long long* outside = c->gbins + CUBE_MAX_BINS;
     {
-    ProfScope prof(c, CUBE_K_HIST, s);
+    ProfScope prof(c, fused_select ? CUBE_K_HIST_SELECT : CUBE_K_HIST, s);
     if (nbins <= kSmemHistMaxBins) {
         const size_t smem = (size_t)(nbins + 2) * sizeof(uint32_t);  // + trash slot
         const int grid = grid_for(c, 4, occupancy_of(c, hist_smem_kernel, kThreads, smem));

@@ -357,7 +357,8 @@ struct HistF : HistBase {
 // 0 <= i < top is exactly the case "+0 <= v < nbins-1", for which lo <= x <= hi is guaranteed (t = x - lo has
 // the sign of the exact difference, and x > hi implies v >= fl(fl(hi-lo) * scale) > nbins - 1 whenever hi > lo and
 // scale is a normal number, nbins <= 65536) and the bin is floor(v), no clamp.  What is left -- the closed top bin
-// (R11), x > hi (both: i >= top, signed) and x < lo (xmin < lo; FMNMX3 ignores NaN) -- is rare and detected per
+// (R11), x > hi (both: i >= top, signed) and x < lo (xmin < lo; FMNMX3 ignores NaN; such a voxel is i = -1, or i = 0
+// when the product underflows to -0.0, which the cold path takes back out of bin 0) -- is rare and detected per
 // tile share (32 voxels); a cold path reloads the 8 rows (L2 hits), finds the rows concerned and applies the exact
 // definition to their voxels.  Not valid for hi == lo (scale 0), fewer than 8 bins or a subnormal scale.
 __host__ __device__ __forceinline__ bool hist_use_fast(int nbins, float lo, float hi, float scale) {
@@ -381,10 +382,13 @@ struct HistFastF {
     // exact definition for a voxel the hot path sent to the trash slot (NaN: nothing to do)
     static __device__ __forceinline__ void fix(float x, float lo, float hi, float scale, int top, uint32_t* sbins,
                                                uint32_t* s_out) {
-        if (x < lo) atomicAdd(&s_out[0], 1u);
-        else if (x > hi) atomicAdd(&s_out[1], 1u);
-        else if (x == x) {
-            const int i = pos(x, lo, scale);
+        const int i = pos(x, lo, scale);
+        if (x < lo || x > hi) {
+            atomicAdd(&s_out[x < lo ? 0 : 1], 1u);
+            // (x - lo) * scale can underflow to -0.0 for x just below lo (scale < 1): the hot path has then
+            // counted the voxel in bin 0 -- take it back out
+            if ((uint32_t)i < (uint32_t)top) atomicSub(&sbins[i], 1u);
+        } else if (x == x) {
             if ((uint32_t)i >= (uint32_t)top) atomicAdd(&sbins[hist_slot(min(max(i, 0), top), top)], 1u);
         }
     }
@@ -405,7 +409,8 @@ struct HistFastF {
     }
     __device__ __forceinline__ void operator()(float x) {   // head / tail / ragged last tile
         const int i = pos(x, lo, scale);
-        if ((uint32_t)i < (uint32_t)top) atomicAdd(&sbins[i], 1u);
+        if ((uint32_t)i < (uint32_t)top && x >= lo) atomicAdd(&sbins[i], 1u);
+        else if ((uint32_t)i < (uint32_t)top) atomicAdd(&s_out[0], 1u);   // x < lo with a product that underflowed to -0.0
         else fix(x, lo, hi, scale, top, sbins, s_out);
     }
     __device__ __forceinline__ void batch(const float4 (&r)[kUnroll], const float4* __restrict__ p) {

@@ -441,6 +441,27 @@ def test_packed_histogram_counter_wraps(ctx):
     assert rb.max() > 3 * 65536
 
 
+@pytest.mark.parametrize("nbins", [16, 256, 4096, 65536])
+def test_histogram_underflow_below_lo(ctx, nbins):
+    # (x - lo) * scale underflows to -0.0 for subnormal x just below lo = 0 when scale < 1: such voxels are
+    # outside[0], not bin 0 (the fast functors place voxels by floor(v) without a range test)
+    r = np.random.default_rng(nbins)
+    n = 70001
+    a = r.uniform(0.0, 1000.0, n).astype(np.float32)
+    tiny = np.array([-1e-45, -3e-45, -1e-40, 1e-45, -0.0, 0.0], dtype=np.float32)
+    a[r.integers(0, n, 600)] = tiny[r.integers(0, tiny.size, 600)]
+    a[::501] = np.nan
+    for misalign in (0, 1):
+        t = dev(a, misalign)
+        for lo, hi in ((0.0, 1000.0), (0.0, 1e6), (-1e-42, 4000.0)):
+            b, o = ctx.histogram(t, n, 1, 1, nbins, lo, hi)
+            rb, ro = oracle.histogram(a, nbins, lo, hi)
+            assert (b == rb).all() and (o == ro).all(), (nbins, lo, hi, o, ro, b[:2], rb[:2])
+            if nbins <= 16384:
+                m, b2, o2, med = ctx.stats(t, n, 1, 1, nbins, lo, hi)
+                assert (b2 == rb).all() and (o2 == ro).all()
+
+
 @pytest.mark.parametrize("knob", [0, 1, 2])
 def test_big_histogram_variants(ctx, knob):
     # > 16384 bins: 0 = automatic (32-bit window of 32768 bins + global REDs, or 16-bit packed when the sampled
