@@ -462,6 +462,81 @@ def test_histogram_underflow_below_lo(ctx, nbins):
                 assert (b2 == rb).all() and (o2 == ro).all()
 
 
+@pytest.mark.parametrize("seed", range(16))
+def test_selection_randomised_values_and_ranks(ctx, seed):
+    # differential test of the radix select (three fused pass kernels, candidate compaction, bucket location in the
+    # last CTA) on mixtures with heavy ties, both zeros, subnormals, +-Inf, NaN of both signs, at random ranks
+    r = np.random.default_rng(7000 + seed)
+    n = int(r.integers(1, 400000))
+    kind = seed % 4
+    if kind == 0:
+        a = (r.standard_normal(n) * 10.0 ** r.uniform(-30, 30)).astype(np.float32)
+    elif kind == 1:
+        a = r.integers(-3, 4, n).astype(np.float32)                              # seven values
+    elif kind == 2:
+        a = np.exp(np.round(r.standard_normal(n) * 2, 1)).astype(np.float32) * np.float32(r.choice([1.0, -1.0]))
+    else:
+        a = (r.standard_normal(n) * 1e-41).astype(np.float32)                    # subnormals
+    specials = np.array([0.0, -0.0, np.inf, -np.inf, np.nan, 1e-45, -1e-45, 3.4e38, -3.4e38], dtype=np.float32)
+    idx = r.integers(0, n, n // 8 + 1)
+    a[idx] = specials[r.integers(0, specials.size, idx.size)]
+    a[r.integers(0, n, 3)] = np.frombuffer(np.uint32(0xFFC00001).tobytes(), dtype=np.float32)[0]
+    t = dev(a, seed % 4)
+    cnt = int((~np.isnan(a)).sum())
+    assert same_float(ctx.median(t, n, 1, 1), oracle.median(a))
+    ks = {0, max(cnt - 1, 0), cnt // 2, cnt // 100, int(r.integers(0, max(cnt, 1)))}
+    for k in sorted(ks):
+        if k < cnt:
+            assert same_float(ctx.kth(t, n, 1, 1, k), oracle.kth(a, k)), (seed, k, cnt)
+    assert math.isnan(float(ctx.kth(t, n, 1, 1, cnt)))                          # k >= count -> NaN
+    m = ctx.moments(t, n, 1, 1, flags=cube.COARSE_HIST)
+    assert m["count"] == cnt
+    if cnt:
+        k = int(r.integers(0, cnt))
+        assert same_float(ctx.kth(t, n, 1, 1, k, flags=cube.REUSE_COARSE), oracle.kth(a, k))
+    s_m, _, _, s_med = ctx.stats(t, n, 1, 1, 0)
+    assert same_float(s_med, oracle.median(a)) and s_m["count"] == cnt
+
+
+@pytest.mark.parametrize("seed", range(24))
+def test_histogram_randomised_ranges_and_specials(ctx, seed):
+    # differential test of every histogram path (general / fast / window / packed functors, cube_histogram and the
+    # fused cube_stats pass B) on random ranges of every magnitude with the awkward values planted: the range ends
+    # and their float neighbours, +-0, subnormals, +-Inf, NaN of both signs, values far outside
+    r = np.random.default_rng(9000 + seed)
+    nbins = int(r.choice([1, 2, 7, 8, 9, 255, 1000, 4096, 16384, 16385, 32768, 32769, 50000, 65536]))
+    mag = 10.0 ** r.uniform(-42, 30) if seed % 3 else 10.0 ** r.uniform(-3, 3)
+    lo = np.float32(r.uniform(-1, 1) * mag)
+    width = np.float32(abs(r.standard_normal()) * mag * 10.0 ** r.uniform(-6, 2))
+    hi = np.float32(lo + width) if seed % 7 else lo                      # hi == lo now and then (R13)
+    if not np.isfinite(hi) or hi < lo:
+        hi = lo
+    n = int(r.integers(1000, 200000))
+    centre, spread = (float(lo) + float(hi)) / 2, max(float(hi) - float(lo), abs(float(lo)) * 1e-6 + 1e-45)
+    a = (centre + r.standard_normal(n) * spread * 10.0 ** r.uniform(-1.5, 0.5)).astype(np.float32)
+    specials = np.array([lo, hi, np.nextafter(lo, np.float32(-np.inf)), np.nextafter(lo, np.float32(np.inf)),
+                         np.nextafter(hi, np.float32(-np.inf)), np.nextafter(hi, np.float32(np.inf)),
+                         0.0, -0.0, 1e-45, -1e-45, 1e-39, -1e-39, np.inf, -np.inf, np.nan, 3e38, -3e38],
+                        dtype=np.float32)
+    idx = r.integers(0, n, n // 10)
+    a[idx] = specials[r.integers(0, specials.size, idx.size)]
+    a[r.integers(0, n, 5)] = np.frombuffer(np.uint32(0xFFC00001).tobytes(), dtype=np.float32)[0]   # negative NaN
+    t = dev(a, seed % 4)
+    try:
+        rb, ro = oracle.histogram(a, nbins, lo, hi)
+    except ValueError:
+        with pytest.raises(cube.CubeError):
+            ctx.histogram(t, n, 1, 1, nbins, float(lo), float(hi))
+        return
+    b, o = ctx.histogram(t, n, 1, 1, nbins, float(lo), float(hi))
+    assert (o == ro).all() and (b == rb).all(), (nbins, lo, hi, o, ro, np.nonzero(b != rb)[0][:5])
+    m, b2, o2, med = ctx.stats(t, n, 1, 1, nbins, float(lo), float(hi))
+    assert (o2 == ro).all() and (b2 == rb).all(), (nbins, lo, hi, o2, ro)
+    fin = a[~np.isnan(a)]
+    assert same_float(med, oracle.median(a)) and m["count"] == fin.size
+    assert int(b.sum() + o.sum()) == fin.size
+
+
 @pytest.mark.parametrize("knob", [0, 1, 2])
 def test_big_histogram_variants(ctx, knob):
     # > 16384 bins: 0 = automatic (32-bit window of 32768 bins + global REDs, or 16-bit packed when the sampled
