@@ -462,6 +462,59 @@ def test_histogram_underflow_below_lo(ctx, nbins):
                 assert (b2 == rb).all() and (o2 == ro).all()
 
 
+@pytest.mark.parametrize("seed", range(10))
+def test_moments_nan_patterns_switch_hot_and_safe_paths(ctx, seed):
+    # the moments kernels run a NaN-blind hot path and a per-voxel safe path and switch per warp and tile (8192
+    # voxels per CTA tile, 1024 per warp): NULL runs of every length and alignment, single NULL voxels at tile
+    # edges, all-NULL stretches followed by data (late pivots), +-0 and constant stretches
+    r = np.random.default_rng(5000 + seed)
+    n = int(r.integers(200000, 1200000))
+    a = (r.standard_normal(n) * 0.002 + 0.0007).astype(np.float32)
+    for _ in range(int(r.integers(1, 40))):
+        start = int(r.integers(0, n))
+        length = int(r.choice([1, 2, 3, 4, 31, 32, 33, 1023, 1024, 1025, 8191, 8192, 8193, 50000]))
+        if r.random() < 0.5:
+            start = (start // 1024) * 1024 + int(r.choice([0, -1, 1, 4]))          # hug the warp-tile edges
+        a[max(start, 0):start + length] = np.nan
+    if seed % 3 == 0:
+        a[:int(r.integers(1, n // 2))] = np.nan                                    # every thread starts without a pivot
+    if seed % 4 == 1:
+        a[r.integers(0, n, n // 200)] = np.nan                                     # scattered: warps stay on the safe path
+    if seed % 5 == 2:
+        a[n // 3:n // 3 + 70000] = np.float32(0.125)                               # constant stretch
+    t = dev(a, seed % 4)
+    ref = oracle.moments(a)
+    check_moments(ctx.moments(t, n, 1, 1), ref, a)
+    check_moments(ctx.moments(t, n, 1, 1, flags=cube.COARSE_HIST), ref, a)
+    m, b, o, med = ctx.stats(t, n, 1, 1, 4096, -0.02, 0.5)
+    check_moments(m, ref, a)
+    rb, ro = oracle.histogram(a, 4096, -0.02, 0.5)
+    assert (b == rb).all() and (o == ro).all() and same_float(med, oracle.median(a))
+    k = ref["count"] // 3
+    assert same_float(ctx.kth(t, n, 1, 1, k, flags=cube.REUSE_COARSE), oracle.kth(a, k))   # digit bins after the NaN repairs
+    lo, hi = np.float32(ref["mean"] - ref["std"]), np.float32(ref["mean"] + 2 * ref["std"])
+    got, want = ctx.clipped_moments(t, n, 1, 1, float(lo), float(hi)), oracle.clipped_moments(a, lo, hi)
+    assert got["count"] == want["count"] and abs(got["mean"] - want["mean"]) <= REL * abs(want["mean"])
+    # mini-map rows over the same voxels (hot / safe groups of 8 lines)
+    nx, ny = 256, 64
+    nz = n // (nx * ny)
+    if nz >= 2:
+        sub = a[:nx * ny * nz]
+        mx, my, mz = ctx.minimap_dims(nx, ny, nz, 30, 30, 30)
+        cells = torch.zeros(mx * my * mz * 40, dtype=torch.uint8, device="cuda")
+        ts = dev(sub, 0)
+        ctx.minimap(ts, nx, ny, nz, 30, 30, 30, cells)
+        torch.cuda.synchronize()
+        gotm = np.frombuffer(cells.cpu().numpy().tobytes(), dtype=cube.MINIMAP_DTYPE).reshape(mz, my, mx)
+        refm = oracle.minimap(sub, (nx, ny, nz), (30, 30, 30))
+        assert (gotm["count"] == refm["count"]).all() and (gotm["nan_count"] == refm["nan_count"]).all()
+        okc = refm["count"] > 0
+        assert (gotm["min"][okc] == refm["min"][okc]).all() and (gotm["max"][okc] == refm["max"][okc]).all()
+        assert np.allclose(gotm["mean"][okc], refm["mean"][okc], rtol=1e-9, atol=1e-12)
+        okv = okc & (refm["std"] > 0)
+        assert np.allclose(gotm["std"][okv], refm["std"][okv], rtol=1e-9, atol=0)
+
+
 @pytest.mark.parametrize("seed", range(16))
 def test_selection_randomised_values_and_ranks(ctx, seed):
     # differential test of the radix select (three fused pass kernels, candidate compaction, bucket location in the
