@@ -162,8 +162,13 @@ struct MapV4F : MomentsF<kMomPlain> {
 #pragma unroll
         for (int c = 0; c < 4; ++c) { const float xm = own[c] ? x[c] : qnan; take_pivot(xm); core(xm); }
     }
-    // repair of a HOT group whose sum came out NaN: reload the lines (L2 hits), add the owned non-NaN voxels
-    __device__ __noinline__ void redo_group(MapLines at) {
+    // repair of a HOT group whose sum came out NaN: reload the lines (L2 hits), add the owned non-NaN voxels.
+    // Static, arguments and result by value: the functor itself stays in registers (a member function taking
+    // `this` put it on the stack -- 116 M local-memory sectors per pass, profiles/r1_v8_c2.md).
+    struct GroupFix { double s, q; uint32_t n; };
+    static __device__ __noinline__ GroupFix redo_group(MapLines at, double pivot_, uint32_t ownmask) {
+        GroupFix f;
+        f.s = 0.0; f.q = 0.0; f.n = 0;
 #pragma unroll 1
         for (int k = 0; k < kMapUnroll; ++k) {
             const float4 v = __ldcg(at.p);
@@ -171,8 +176,12 @@ struct MapV4F : MomentsF<kMomPlain> {
             const float x[4] = {v.x, v.y, v.z, v.w};
 #pragma unroll
             for (int c = 0; c < 4; ++c)
-                if (own[c] && x[c] == x[c]) { const double dl = (double)x[c] - pivot; s += dl; q = fma(dl, dl, q); n += 1; }
+                if (((ownmask >> c) & 1u) && x[c] == x[c]) {
+                    const double dl = (double)x[c] - pivot_;
+                    f.s += dl; f.q = fma(dl, dl, f.q); f.n += 1;
+                }
         }
+        return f;
     }
     // HOT mode.  -> true when the group held a NaN (or +Inf and -Inf) in an owned column.
     __device__ __forceinline__ bool hot_group(const float4 (&v)[kMapUnroll], const MapLines& at) {
@@ -190,7 +199,11 @@ struct MapV4F : MomentsF<kMomPlain> {
         const double tsum = ts[0] + ts[1];
         const bool bad = !(tsum == tsum);
         if (!bad) { s += tsum; q += tq[0] + tq[1]; n += nown * kMapUnroll; }
-        else redo_group(at);   // min/max are already in (FMNMX ignores NaN)
+        else {   // min/max are already in (FMNMX ignores NaN)
+            const uint32_t ownmask = (own[0] ? 1u : 0u) | (own[1] ? 2u : 0u) | (own[2] ? 4u : 0u) | (own[3] ? 8u : 0u);
+            const GroupFix f = redo_group(at, pivot, ownmask);
+            s += f.s; q += f.q; n += f.n;
+        }
         return bad;
     }
 };
