@@ -66,6 +66,7 @@ def lib():
         L.oracle_sigma_clip.argtypes = [fp, ctypes.c_uint64, ctypes.c_double, ctypes.c_int, ctypes.c_int, mp, fp]
         L.oracle_mad.argtypes = [fp, ctypes.c_uint64, fp, fp]
         L.oracle_minimap.argtypes = [fp] + [ctypes.c_int64] * 6 + [ctypes.c_int, mp]
+        L.oracle_torben_capped.argtypes = [fp, ctypes.c_uint64, ctypes.c_int, fp, ctypes.POINTER(ctypes.c_int)]
         _lib = L
     return _lib
 
@@ -198,3 +199,11 @@ def minimap(a, dims, part, sample_std=False):
     dt = np.dtype([("count", "<u8"), ("nan_count", "<u8"), ("min", "<f4"), ("max", "<f4"), ("mean", "<f8"),
                    ("std", "<f8")])
     return np.frombuffer(bytes(cells), dtype=dt).reshape(mz, my, mx).copy()
+
+
+def torben_capped(a, max_iter):
+    """Alg. 1 stopped after at most ``max_iter`` passes.  -> (value, passes made, converged)."""
+    a, p = _arr(a)
+    out, conv = ctypes.c_float(), ctypes.c_int()
+    it = lib().oracle_torben_capped(p, a.size, int(max_iter), ctypes.byref(out), ctypes.byref(conv))
+    return np.float32(out.value), it, bool(conv.value)

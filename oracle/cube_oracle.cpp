@@ -262,6 +262,52 @@ int oracle_torben_median(const float* d, uint64_t N, float* out, double* trace, 
     return iter;
 }
 
+// Alg. 1 stopped after at most max_iter passes over the data -- the paper's remark that "if a median approximation
+// is accepted, the number of iterations could have been reduced to 20 with an error of order 1e-6" (
+// "Torben-on-GPU as the paper-faithful comparison and early-stop approximate median").
+// Same steps as oracle_torben_median; when the cap is reached before the stop test fires, the final
+// selection is applied to the counts of the last pass made (reading R26).  *converged = 1 when
+// the stop test fired (then the result is the exact lower median).  Returns the passes made; -1 and NaN when there
+// is no non-NaN voxel; max_iter <= 0 makes no pass and returns NaN.
+int oracle_torben_capped(const float* d, uint64_t N, int max_iter, float* out, int* converged) {
+    uint64_t n = 0;
+    float Min = 0.f, Max = 0.f;
+    *converged = 0;
+    *out = std::numeric_limits<float>::quiet_NaN();
+    for (uint64_t i = 0; i < N; ++i) {
+        float x = d[i];
+        if (is_nan(x)) continue;
+        if (n == 0) { Min = Max = x; }
+        else { if (x < Min) Min = x; if (x > Max) Max = x; }
+        ++n;
+    }
+    if (n == 0) return -1;
+    if (max_iter <= 0) return 0;
+    int iter = 0;
+    float Guess, MaxLt, MinGt;
+    uint64_t Less, Greater, Equal;
+    for (;;) {
+        Guess = oracle_torben_guess(Min, Max);
+        Less = Greater = Equal = 0;
+        MaxLt = Min;
+        MinGt = Max;
+        for (uint64_t i = 0; i < N; ++i) {
+            float x = d[i];
+            if (is_nan(x)) continue;
+            if (x < Guess) { ++Less; if (x > MaxLt) MaxLt = x; }
+            else if (x > Guess) { ++Greater; if (x < MinGt) MinGt = x; }
+            else ++Equal;
+        }
+        ++iter;
+        if (oracle_torben_stop(Less, Greater, n)) { *converged = 1; break; }
+        if (iter >= max_iter) break;
+        if (Less > Greater) Max = MaxLt;
+        else Min = MinGt;
+    }
+    *out = oracle_torben_pick(Less, Equal, n, MaxLt, Guess, MinGt);
+    return iter;
+}
+
 // ---------------------------------------------------------------------------------
 // NEXT-1: median absolute deviation and sigma-clipped moments.
 // The paper only names them: Torben's method "can be easily modified to address the median absolute

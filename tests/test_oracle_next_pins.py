@@ -247,3 +247,65 @@ def test_minimap_single_cell_is_global_moments_and_constant():
     # cell (0,0,0): values 0,1,4,5,8,9,12,13
     vals = np.array([0, 1, 4, 5, 8, 9, 12, 13], dtype=np.float64)
     assert s[0, 0, 0]["std"] == pytest.approx(vals.std(ddof=1), rel=1e-15)
+
+
+# --------------------------------------------------------------------------------------- capped Torben (Alg. 1)
+def restated_torben(vals, max_iter):
+    """Alg. 1 restated independently with numpy float32 scalars; stops after max_iter passes."""
+    v = np.asarray([x for x in vals if not math.isnan(x)], dtype=np.float32)
+    n = v.size
+    mn, mx = v.min(), v.max()
+    it = 0
+    while True:
+        guess = np.float32((mn + mx) / np.float32(2))
+        less, greater = int((v < guess).sum()), int((v > guess).sum())
+        equal = n - less - greater
+        maxlt = v[v < guess].max() if less else mn
+        mingt = v[v > guess].min() if greater else mx
+        it += 1
+        half = (n + 1) // 2
+        conv = less <= half and greater <= half
+        if conv or it >= max_iter:
+            break
+        if less > greater:
+            mx = maxlt
+        else:
+            mn = mingt
+    res = maxlt if less >= half else (guess if less + equal >= half else mingt)
+    return np.float32(res), it, conv
+
+
+@pytest.mark.parametrize("seed", range(10))
+def test_torben_capped_against_restatement_and_sort(seed):
+    r = np.random.default_rng(300 + seed)
+    n = int(r.integers(2, 3000))
+    a = (r.standard_normal(n) * 10 ** r.uniform(-3, 3) + r.uniform(-1, 1)).astype(np.float32)
+    if seed % 3 == 0:
+        a = np.round(a * 2) / 2
+    a[r.integers(0, n, n // 20)] = np.nan
+    if np.isnan(a).all():
+        a[0] = 1.0
+    full, it_full, conv_full = oracle.torben_capped(a, 10000)
+    v = np.sort(a[~np.isnan(a)])
+    assert conv_full and full == v[(v.size - 1) // 2]                   # uncapped: the exact lower median
+    assert (full, it_full) == oracle.torben_median(a)[:2]
+    for cap in (1, 2, 3, 5, 8, it_full - 1, it_full, it_full + 3):
+        if cap < 1:
+            continue
+        got = oracle.torben_capped(a, cap)
+        ref = restated_torben(a, cap)
+        assert got[1] == ref[1] == min(cap, it_full) and got[2] == ref[2] and got[0] == ref[0], (cap, got, ref)
+        assert v[0] <= got[0] <= v[-1]
+    # the approximation tightens: after c passes the result is within (max-min) / 2^(c-1) of the median
+    span = float(v[-1]) - float(v[0])
+    for cap in (4, 8, 12):
+        if cap < it_full:
+            assert abs(float(oracle.torben_capped(a, cap)[0]) - float(full)) <= span / 2 ** (cap - 1) + 1e-30
+
+
+def test_torben_capped_degenerate():
+    assert oracle.torben_capped(np.full(5, np.nan, np.float32), 10)[1] == -1
+    val, it, conv = oracle.torben_capped(np.full(9, 2.5, np.float32), 10)
+    assert (val, it, conv) == (2.5, 1, True)
+    val, it, conv = oracle.torben_capped(np.array([1, 2, 3], np.float32), 0)
+    assert math.isnan(val) and it == 0 and not conv
