@@ -390,6 +390,7 @@ def main():
     # NEXT rows: MAD, clipped moments, sigma clipping, 30^3 statistical mini-map
     out_w = torch.zeros(2, dtype=torch.float32, device=dev)
     out_i = torch.zeros(1, dtype=torch.int32, device=dev)
+    out_w2 = torch.zeros(1, dtype=torch.int32, device=dev)
     part = (30, 30, 30)
     mmx, mmy, mmz = ctx.minimap_dims(nx, ny, nz, *part)
     out_cells = torch.zeros(mmx * mmy * mmz * 40, dtype=torch.uint8, device=dev)
@@ -402,6 +403,9 @@ def main():
 
     def op_sigma_clip():
         ctx.sigma_clip(cube_t, nx, ny, nz, 3.0, 5, out=out_m, iters=out_i, window=out_w, stream=stream)
+
+    def op_torben():                         # the paper's own median method (Alg. 1), ~30 passes over the cube
+        ctx.median_torben(cube_t, nx, ny, nz, 64, out=out_f, iters=out_i, converged=out_w2, stream=stream)
 
     def op_minimap():
         ctx.minimap(cube_t, nx, ny, nz, part[0], part[1], part[2], out_cells, stream=stream)
@@ -453,7 +457,13 @@ def main():
         op_sigma_clip()
         torch.cuda.synchronize()
         clip_passes = int(out_i.item()) + 1          # the plain pass + the clipped passes actually made
-        for nm, fn, bpv in [("next_mad", op_mad, 16.0), ("next_clipped_moments", op_clipped, 4.0),
+        op_torben()
+        torch.cuda.synchronize()
+        torben_passes = int(out_i.item()) + 1        # the moments pass (Min, Max, n) + the passes of Alg. 1
+        op_sigma_clip()
+        torch.cuda.synchronize()
+        for nm, fn, bpv in [("paper_alg1_torben_median", op_torben, 4.0 * torben_passes),
+                            ("next_mad", op_mad, 16.0), ("next_clipped_moments", op_clipped, 4.0),
                             ("next_sigma_clip_3sigma_max5", op_sigma_clip, 4.0 * clip_passes),
                             ("next_minimap_30x30x30", op_minimap, 4.0)]:
             for _ in range(2):

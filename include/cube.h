@@ -232,6 +232,19 @@ int cube_clipped_moments(cube_ctx* ctx, const float* d, int64_t nx, int64_t ny, 
 int cube_sigma_clip(cube_ctx* ctx, const float* d, int64_t nx, int64_t ny, int64_t nz, double kappa, int max_iter,
                     unsigned flags, cube_moments_t* out, int* iters, float* window /* [2] */, cudaStream_t stream);
 
+/* cube_median_torben: the paper's own median method, Alg. 1 (Torben's bisection, sec. 4.3), kept
+ *   for comparison with the radix select and for the paper's early-stop approximation.  One pass over
+ *   the cube per guess -- counts of voxels less / greater / equal, largest voxel below, smallest above -- and a
+ *   1-thread kernel between passes in the role of the paper's server; at most max_iter passes
+ *   (0..1000) are enqueued, those after the stop test has fired return at once; no host synchronisation.
+ *   *out = the exact lower median when the stop test fired (*converged = 1; ~30 passes for float32 data), else the
+ *   final selection of Alg. 1 applied to the counts of the last pass made (R26: within (max-min)/2^(p-1)
+ *   of the median after p passes).  *iters = passes made.  Comparisons are numeric, so +0.0 and -0.0 are one
+ *   value: a zero result carries no sign guarantee.  No non-NaN voxel, or max_iter == 0: NaN.  iters / converged
+ *   may be NULL; all outputs device, pinned or pageable host memory. */
+int cube_median_torben(cube_ctx* ctx, const float* d, int64_t nx, int64_t ny, int64_t nz, int max_iter, float* out,
+                       int* iters, int* converged, cudaStream_t stream);
+
 /* ---- NEXT-2: the statistical mini-map (Fig. 7): one cube_moments_t per partition of
  * px x py x pz voxels ("30x30x30 pixel"), cell (cx,cy,cz) covering x in [cx*px, min((cx+1)*px, nx)) and likewise
  * in y and z (ragged last cells are smaller; R25).  cells[(cz*my + cy)*mx + cx] with mx = ceil(nx/px),
@@ -281,7 +294,8 @@ enum {
     CUBE_K_OTHER = 10,
     CUBE_K_MOMENTS_WINDOW = 11, /* moments_kernel<window>: cube_clipped_moments, cube_sigma_clip passes */
     CUBE_K_MINIMAP = 12,        /* minimap_kernel */
-    CUBE_K_KINDS = 13
+    CUBE_K_TORBEN = 13,         /* torben_pass_kernel (cube_median_torben) */
+    CUBE_K_KINDS = 14
 };
 int cube_profile_enable(cube_ctx* ctx, int on);
 /* Read-only STREAM probe: streams nvox float32 voxels through the same loop as the statistics kernels with one

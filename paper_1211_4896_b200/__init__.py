@@ -33,11 +33,11 @@ SYMBOLS = ["cube_create", "cube_destroy", "cube_moments", "cube_histogram", "cub
            "cube_last_cuda_error", "cube_set_launch", "cube_set_knob", "cube_launch_count",
            "cube_profile_enable", "cube_profile_reset", "cube_profile_read",
            "cube_mad", "cube_clipped_moments", "cube_sigma_clip", "cube_minimap_dims", "cube_minimap",
-           "cube_shard_buffers", "cube_shard_merge_records", "cube_shard_advance"]
+           "cube_shard_buffers", "cube_shard_merge_records", "cube_shard_advance", "cube_median_torben"]
 SHARD_RECORD_BYTES, SHARD_DIGITS = 40, 8192
 KNOB_CTAS_PER_SM, KNOB_BIGHIST = 0, 1
 KIND_NAMES = ["moments", "moments_coarse", "histogram", "select_pass0", "select_pass1", "select_pass2",
-              "select_cand", "select_scan", "hist_select", "probe_read", "other", "moments_window", "minimap"]
+              "select_cand", "select_scan", "hist_select", "probe_read", "other", "moments_window", "minimap", "torben_pass"]
 
 
 class CubeError(RuntimeError):
@@ -114,6 +114,7 @@ def load():
     L.cube_sigma_clip.argtypes = [vp, vp, i64, i64, i64, f64, ci, cu, vp, vp, vp, vp]
     L.cube_minimap_dims.argtypes = [i64] * 6 + [ctypes.POINTER(i64)] * 3
     L.cube_minimap.argtypes = [vp, vp, i64, i64, i64, i64, i64, i64, cu, vp, vp]
+    L.cube_median_torben.argtypes = [vp, vp, i64, i64, i64, ci, vp, vp, vp, vp]
     L.cube_shard_buffers.argtypes = [vp, ctypes.POINTER(ShardBuffersT)]
     L.cube_shard_merge_records.argtypes = [vp, vp, ci, cu, vp]
     L.cube_shard_advance.argtypes = [vp, ctypes.POINTER(ci), vp]
@@ -259,6 +260,20 @@ class Context:
                                             ctypes.cast(ctypes.byref(it), ctypes.c_void_p),
                                             ctypes.cast(w, ctypes.c_void_p), stream))
         return m.as_dict(), int(it.value), (np.float32(w[0]), np.float32(w[1]))
+
+    def median_torben(self, d, nx, ny, nz, max_iter=64, out=None, iters=None, converged=None, stream=0):
+        """cube_median_torben (Alg. 1 of the paper) -> (value, passes made, converged) on the host, or None when
+        device/pinned outputs are given."""
+        if out is not None:
+            self._check(self._L.cube_median_torben(self._h, _ptr(d), nx, ny, nz, max_iter, _ptr(out), _ptr(iters),
+                                                   _ptr(converged), stream))
+            return None
+        r, it, cv = ctypes.c_float(), ctypes.c_int(), ctypes.c_int()
+        self._check(self._L.cube_median_torben(self._h, _ptr(d), nx, ny, nz, max_iter,
+                                               ctypes.cast(ctypes.byref(r), ctypes.c_void_p),
+                                               ctypes.cast(ctypes.byref(it), ctypes.c_void_p),
+                                               ctypes.cast(ctypes.byref(cv), ctypes.c_void_p), stream))
+        return np.float32(r.value), int(it.value), bool(cv.value)
 
     def minimap_dims(self, nx, ny, nz, px, py, pz):
         mx, my, mz = ctypes.c_int64(), ctypes.c_int64(), ctypes.c_int64()

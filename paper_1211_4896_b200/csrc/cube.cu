@@ -34,6 +34,7 @@ struct cube_ctx {
     float* probe_out = nullptr;            // cube_probe_read sink
     BigHistPlan* plan = nullptr;           // hist_window_kernel's plan for the > 16384-bin histogram kernels
     ClipState* clip = nullptr;             // sigma-clip loop state (NEXT-1)
+    TorbenState* torben = nullptr;         // Alg. 1 loop state (cube_median_torben)
     float* center = nullptr;               // cube_mad: the median the deviations are taken from
     uint32_t* cand = nullptr;              // candidate keys of the select (step 8)
     unsigned long long cand_cap = 0;       // in keys
@@ -337,6 +338,7 @@ int cube_create(cube_ctx** out, size_t scratch_bytes_hint) {
     ok = ok && cudaMalloc(&c->probe_out, sizeof(float)) == cudaSuccess;
     ok = ok && cudaMalloc(&c->plan, sizeof(BigHistPlan)) == cudaSuccess;
     ok = ok && cudaMalloc(&c->clip, sizeof(ClipState)) == cudaSuccess;
+    ok = ok && cudaMalloc(&c->torben, sizeof(TorbenState)) == cudaSuccess;
     ok = ok && cudaMalloc(&c->center, sizeof(float)) == cudaSuccess;
     ok = ok && cudaMemset(c->plan, 0, sizeof(BigHistPlan)) == cudaSuccess;
     ok = ok && cudaMemset(c->ticket, 0, sizeof(unsigned int)) == cudaSuccess;
@@ -367,7 +369,7 @@ int cube_destroy(cube_ctx* c) {
     if (!c) return CUBE_EINVAL;
     cudaFree(c->partials); cudaFree(c->ticket); cudaFree(c->ticket2); cudaFree(c->acc);
     cudaFree(c->mom_out); cudaFree(c->gbins); cudaFree(c->gdigits); cudaFree(c->coarse); cudaFree(c->sel);
-    cudaFree(c->range3); cudaFree(c->probe_out); cudaFree(c->plan); cudaFree(c->clip); cudaFree(c->center);
+    cudaFree(c->range3); cudaFree(c->probe_out); cudaFree(c->plan); cudaFree(c->clip); cudaFree(c->torben); cudaFree(c->center);
     cudaFree(c->cand);
     cudaFree(c->resident); cudaFree(c->chunk[0]); cudaFree(c->chunk[1]);
     if (c->pinned_results) cudaFreeHost(c->pinned_results);
@@ -547,6 +549,37 @@ int cube_sigma_clip(cube_ctx* c, const float* d, int64_t nx, int64_t ny, int64_t
     CUBE_CUDA(c, cudaMemcpyAsync(out, c->mom_out, sizeof(MomentsOut), cudaMemcpyDefault, s));
     if (iters) CUBE_CUDA(c, cudaMemcpyAsync(iters, &c->clip->iters, sizeof(int), cudaMemcpyDefault, s));
     if (window) CUBE_CUDA(c, cudaMemcpyAsync(window, &c->clip->lo, 2 * sizeof(float), cudaMemcpyDefault, s));
+    return CUBE_OK;
+}
+
+int cube_median_torben(cube_ctx* c, const float* d, int64_t nx, int64_t ny, int64_t nz, int max_iter, float* out,
+                       int* iters, int* converged, cudaStream_t s) {
+    uint64_t n;
+    if (!c || !d || !out || !dims_ok(nx, ny, nz, &n) || max_iter < 0 || max_iter > 1000) return CUBE_EINVAL;
+    CUBE_CUDA(c, cudaMemsetAsync(c->torben, 0, sizeof(TorbenState), s));
+    int rc = launch_moments(c, d, n, 0u, 0, s, kMomPlain);   // Min, Max, n ("calculated while the dataset is loading")
+    if (rc) return rc;
+    const int occ = occupancy_of(c, torben_pass_kernel, kThreads, 0);
+    const int grid = grid_for(c, 4, occ < kMaxCtasPerSm ? occ : kMaxCtasPerSm);
+    for (int i = 0; i < max_iter; ++i) {
+        {
+            ProfScope prof(c, CUBE_K_OTHER, s);
+            torben_step_kernel<<<1, 1, 0, s>>>(c->mom_out, c->torben, 0);
+        }
+        {
+            ProfScope prof(c, CUBE_K_TORBEN, s);
+            torben_pass_kernel<<<grid, kThreads, 0, s>>>(d, n, c->torben);
+        }
+        CUBE_CUDA(c, cudaGetLastError());
+    }
+    {
+        ProfScope prof(c, CUBE_K_OTHER, s);
+        torben_step_kernel<<<1, 1, 0, s>>>(c->mom_out, c->torben, 1);
+    }
+    CUBE_CUDA(c, cudaGetLastError());
+    CUBE_CUDA(c, cudaMemcpyAsync(out, &c->torben->result, sizeof(float), cudaMemcpyDefault, s));
+    if (iters) CUBE_CUDA(c, cudaMemcpyAsync(iters, &c->torben->iters, sizeof(int), cudaMemcpyDefault, s));
+    if (converged) CUBE_CUDA(c, cudaMemcpyAsync(converged, &c->torben->converged, sizeof(int), cudaMemcpyDefault, s));
     return CUBE_OK;
 }
 

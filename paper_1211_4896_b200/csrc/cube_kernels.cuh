@@ -566,3 +566,4 @@ probe_read_kernel(const float* __restrict__ d, uint64_t n, float* __restrict__ o
 #include "cube_fused.cuh"
 #include "cube_fused_big.cuh"
 #include "cube_minimap.cuh"
+#include "cube_torben.cuh"

@@ -262,3 +262,52 @@ def test_minimap_invalid_arguments(ctx):
         ctx.minimap(t, 4, 4, 4, 2, 2, 2, np.zeros(40 * 8, dtype=np.uint8))      # pageable host memory
     with pytest.raises(cube.CubeError):
         ctx.minimap_dims(4, 4, 4, 2, -1, 2)
+
+
+# --------------------------------------------------------------------------------------- Torben (Alg. 1) on the GPU
+def check_torben(ctx, t, a, dims, cap):
+    nx, ny, nz = dims
+    val, it, conv = ctx.median_torben(t, nx, ny, nz, cap)
+    rval, rit, rconv = oracle.torben_capped(a, cap)
+    if rit < 0:                                           # no non-NaN voxel
+        assert math.isnan(float(val)) and it == 0 and not conv
+        return val, it, conv
+    assert it == rit and conv == rconv, (cap, it, rit, conv, rconv)
+    # Alg. 1 compares numerically: +0.0 and -0.0 are one value (cube.h), everything else is bit-exact
+    assert (math.isnan(float(val)) and math.isnan(float(rval))) or float(val) == float(rval), (cap, val, rval)
+    return val, it, conv
+
+
+@pytest.mark.parametrize("name,dims", [("c1", (96, 80, 64)), ("c2", (128, 128, 96)), ("c3", (64, 64, 300)),
+                                       ("c4", (256, 128, 40))])
+def test_torben_scaled_configs(ctx, name, dims):
+    t, a, dims = scaled_cube(name, dims)
+    val, it, conv = check_torben(ctx, t, a, dims, 200)
+    assert conv and same_float(val, oracle.median(a)) or float(val) == float(oracle.median(a))   # the exact lower median
+    assert 1 <= it <= 200
+    for cap in (0, 1, 2, 5, 10, 20, it - 1, it, it + 1):
+        if cap >= 0:
+            check_torben(ctx, t, a, dims, cap)
+    # the radix select reads the cube twice, Alg. 1 `it` times: same value
+    assert float(ctx.median(t, *dims)) == float(val)
+
+
+def test_torben_edge_cases_and_async(ctx):
+    for a in (np.full(1000, np.nan, np.float32), np.array([3.5], np.float32), np.full(4097, -2.0, np.float32),
+              np.array([1, 2, 3, 4], np.float32), np.array([0.0, -0.0, 0.0, -0.0, 1.0], np.float32),
+              np.array([-np.inf, 1.0, 2.0, np.inf, np.nan], np.float32),
+              np.round(np.random.default_rng(4).standard_normal(100001) * 2).astype(np.float32)):
+        for cap in (0, 1, 3, 300):
+            check_torben(ctx, dev(a, 1), a, (a.size, 1, 1), cap)
+    with pytest.raises(cube.CubeError):
+        ctx.median_torben(dev(np.zeros(8, np.float32)), 8, 1, 1, -1)
+    a = (np.random.default_rng(6).standard_normal(300000) * 0.002).astype(np.float32)
+    t = dev(a)
+    s = torch.cuda.Stream()
+    o = torch.zeros(1, dtype=torch.float32, device="cuda")
+    oi = torch.zeros(2, dtype=torch.int32, device="cuda")
+    with torch.cuda.stream(s):
+        ctx.median_torben(t, a.size, 1, 1, 100, out=o, iters=oi[0:1], converged=oi[1:2], stream=s.cuda_stream)
+    s.synchronize()
+    rval, rit, rconv = oracle.torben_capped(a, 100)
+    assert float(o.item()) == float(rval) and oi[0].item() == rit and bool(oi[1].item()) == rconv
