@@ -26,7 +26,8 @@ struct cube_ctx {
     Partial* acc = nullptr;                // running moments (out-of-core)
     unsigned long long* nvox_acc = nullptr;
     MomentsOut* mom_out = nullptr;
-    unsigned long long* gbins = nullptr;   // CUBE_MAX_BINS + 2 (outside) counters
+    unsigned long long* gout = nullptr;    // allocation: [outside (2)][bins (CUBE_MAX_BINS)] -- one memset clears both
+    unsigned long long* gbins = nullptr;   // = gout + 2
     unsigned long long* gdigits = nullptr; // kDigitBins
     unsigned long long* coarse = nullptr;  // kDigitBins: digit histogram kept by CUBE_COARSE_HIST
     SelectState* sel = nullptr;
@@ -131,6 +132,17 @@ inline bool dims_ok(int64_t nx, int64_t ny, int64_t nz, uint64_t* n) {
     return true;
 }
 
+// Device-side address of a caller's output buffer when the kernels can write it themselves (memory of this device,
+// or pinned / managed host memory): small results are then stored by the producing kernel and no copy is enqueued.
+// nullptr for pageable host memory or another device's memory (the cudaMemcpyAsync path).
+inline void* device_reachable(const cube_ctx* c, void* p) {
+    cudaPointerAttributes at;
+    if (!p || cudaPointerGetAttributes(&at, p) != cudaSuccess) { cudaGetLastError(); return nullptr; }
+    if (at.type == cudaMemoryTypeDevice) return at.device == c->device ? at.devicePointer : nullptr;
+    if (at.type == cudaMemoryTypeHost || at.type == cudaMemoryTypeManaged) return at.devicePointer;
+    return nullptr;
+}
+
 template <class K>
 int occupancy_of(cube_ctx* c, K kernel, int threads, size_t smem) {
     const void* fn = reinterpret_cast<const void*>(kernel);
@@ -164,7 +176,7 @@ inline bool hist_scale(int nbins, float lo, float hi, float* scale) {
 // mode: kMomPlain / kMomCoarse / kMomWindow (window = (wlo, whi), or the context's ClipState when use_clip)
 int launch_moments(cube_ctx* c, const float* d, uint64_t n, unsigned flags, int accumulate, cudaStream_t s,
                    int mode = -1, float wlo = 0.f, float whi = 0.f, bool use_clip = false,
-                   const SelectInit* fuse_scan = nullptr) {
+                   const SelectInit* fuse_scan = nullptr, MomentsOut* out_user = nullptr) {
     if (mode < 0) mode = (flags & CUBE_COARSE_HIST) ? kMomCoarse : kMomPlain;
     const bool coarse = mode == kMomCoarse;
     const int occ_m = mode == kMomCoarse ? occupancy_of(c, moments_kernel<kMomCoarse>, kThreads, 0)
@@ -176,20 +188,20 @@ int launch_moments(cube_ctx* c, const float* d, uint64_t n, unsigned flags, int 
     ProfScope prof(c, coarse ? CUBE_K_MOMENTS_COARSE : mode == kMomWindow ? CUBE_K_MOMENTS_WINDOW : CUBE_K_MOMENTS, s);
     const ClipState* clip = use_clip ? c->clip : nullptr;
     SelectInit none;
-    none.k = 0; none.cand_cap = 0; none.use_median = 0; none.enabled = 0;
+    none.k = 0; none.cand_cap = 0; none.result_out = nullptr; none.use_median = 0; none.enabled = 0;
     if (coarse) {   // fuse_scan: the kernel's last CTA also locates the first-digit bucket (cube_stats)
         moments_kernel<kMomCoarse><<<grid, kThreads, 0, s>>>(d, n, c->partials, c->ticket, c->acc, c->nvox_acc,
                                                              accumulate, flags, c->mom_out, c->coarse, 0.f, 0.f, nullptr,
                                                              c->sel, fuse_scan ? c->ticket2 : nullptr,
-                                                             fuse_scan ? *fuse_scan : none);
+                                                             fuse_scan ? *fuse_scan : none, out_user);
     } else if (mode == kMomWindow) {
         moments_kernel<kMomWindow><<<grid, kThreads, 0, s>>>(d, n, c->partials, c->ticket, c->acc, c->nvox_acc,
                                                              accumulate, flags, c->mom_out, c->coarse, wlo, whi, clip,
-                                                             nullptr, nullptr, none);
+                                                             nullptr, nullptr, none, out_user);
     } else {
         moments_kernel<kMomPlain><<<grid, kThreads, 0, s>>>(d, n, c->partials, c->ticket, c->acc, c->nvox_acc,
                                                             accumulate, flags, c->mom_out, c->coarse, 0.f, 0.f, nullptr,
-                                                            nullptr, nullptr, none);
+                                                            nullptr, nullptr, none, out_user);
     }
     }
     CUBE_CUDA(c, cudaGetLastError());
@@ -198,7 +210,7 @@ int launch_moments(cube_ctx* c, const float* d, uint64_t n, unsigned flags, int 
 
 int launch_hist(cube_ctx* c, const float* d, uint64_t n, int nbins, float lo, float hi, float scale,
                 cudaStream_t s, const float* range3 = nullptr, bool fused_select = false) {
-    unsigned long long* outside = c->gbins + CUBE_MAX_BINS;
+    unsigned long long* outside = c->gout;
     {
     ProfScope prof(c, fused_select ? CUBE_K_HIST_SELECT : CUBE_K_HIST, s);
     if (nbins <= kSmemHistMaxBins) {
@@ -234,8 +246,10 @@ int launch_hist(cube_ctx* c, const float* d, uint64_t n, int nbins, float lo, fl
     return CUBE_OK;
 }
 
-inline SelectInit select_init_args(const cube_ctx* c, uint64_t k, int use_median, bool enabled) {
+inline SelectInit select_init_args(const cube_ctx* c, uint64_t k, int use_median, bool enabled,
+                                   float* result_out = nullptr) {
     SelectInit i;
+    i.result_out = result_out;
     i.k = k; i.cand_cap = c->cand ? c->cand_cap : 0; i.use_median = use_median ? 1u : 0u; i.enabled = enabled ? 1u : 0u;
     return i;
 }
@@ -288,7 +302,8 @@ int kth_impl(cube_ctx* c, const float* d, uint64_t n, uint64_t k, int use_median
     int rc;
     // three launches: every pass kernel ends with the bucket location in its last CTA; the select state is
     // initialised by the first of them from kernel arguments (no host-to-device copy)
-    const SelectInit init = select_init_args(c, k, use_median, true), cont = select_init_args(c, 0, 0, false);
+    float* direct = static_cast<float*>(device_reachable(c, out));   // pass C stores the result there itself
+    const SelectInit init = select_init_args(c, k, use_median, true), cont = select_init_args(c, 0, 0, false, direct);
     if (!DEV && (flags & CUBE_REUSE_COARSE)) {
         if ((rc = launch_select_scan<0>(c, c->coarse, s, &init))) return rc;
     } else {
@@ -297,7 +312,7 @@ int kth_impl(cube_ctx* c, const float* d, uint64_t n, uint64_t k, int use_median
     }
     if ((rc = launch_select_pass<1, DEV>(c, d, n, s, &cont))) return rc;
     if ((rc = launch_select_pass<2, DEV>(c, d, n, s, &cont))) return rc;
-    if (out) CUBE_CUDA(c, cudaMemcpyAsync(out, &c->sel->result, sizeof(float), cudaMemcpyDefault, s));
+    if (out && !direct) CUBE_CUDA(c, cudaMemcpyAsync(out, &c->sel->result, sizeof(float), cudaMemcpyDefault, s));
     return CUBE_OK;
 }
 
@@ -330,7 +345,8 @@ int cube_create(cube_ctx** out, size_t scratch_bytes_hint) {
     c->acc = reinterpret_cast<Partial*>(rec);
     c->nvox_acc = rec ? reinterpret_cast<unsigned long long*>(static_cast<char*>(rec) + sizeof(Partial)) : nullptr;
     ok = ok && cudaMalloc(&c->mom_out, sizeof(MomentsOut)) == cudaSuccess;
-    ok = ok && cudaMalloc(&c->gbins, bytes_bins) == cudaSuccess;
+    ok = ok && cudaMalloc(&c->gout, bytes_bins) == cudaSuccess;
+    c->gbins = c->gout ? c->gout + 2 : nullptr;
     ok = ok && cudaMalloc(&c->gdigits, kDigitBins * sizeof(unsigned long long)) == cudaSuccess;
     ok = ok && cudaMalloc(&c->coarse, kDigitBins * sizeof(unsigned long long)) == cudaSuccess;
     ok = ok && cudaMalloc(&c->sel, sizeof(SelectState)) == cudaSuccess;
@@ -368,7 +384,7 @@ int cube_create(cube_ctx** out, size_t scratch_bytes_hint) {
 int cube_destroy(cube_ctx* c) {
     if (!c) return CUBE_EINVAL;
     cudaFree(c->partials); cudaFree(c->ticket); cudaFree(c->ticket2); cudaFree(c->acc);
-    cudaFree(c->mom_out); cudaFree(c->gbins); cudaFree(c->gdigits); cudaFree(c->coarse); cudaFree(c->sel);
+    cudaFree(c->mom_out); cudaFree(c->gout); cudaFree(c->gdigits); cudaFree(c->coarse); cudaFree(c->sel);
     cudaFree(c->range3); cudaFree(c->probe_out); cudaFree(c->plan); cudaFree(c->clip); cudaFree(c->torben); cudaFree(c->center);
     cudaFree(c->cand);
     cudaFree(c->resident); cudaFree(c->chunk[0]); cudaFree(c->chunk[1]);
@@ -395,9 +411,10 @@ int cube_moments(cube_ctx* c, const float* d, int64_t nx, int64_t ny, int64_t nz
     uint64_t n;
     if (!c || !d || !out || !dims_ok(nx, ny, nz, &n)) return CUBE_EINVAL;
     static_assert(sizeof(cube_moments_t) == sizeof(MomentsOut), "layout");
-    int rc = launch_moments(c, d, n, flags, 0, s);
+    MomentsOut* direct = static_cast<MomentsOut*>(device_reachable(c, out));
+    int rc = launch_moments(c, d, n, flags, 0, s, -1, 0.f, 0.f, false, nullptr, direct);
     if (rc) return rc;
-    CUBE_CUDA(c, cudaMemcpyAsync(out, c->mom_out, sizeof(MomentsOut), cudaMemcpyDefault, s));
+    if (!direct) CUBE_CUDA(c, cudaMemcpyAsync(out, c->mom_out, sizeof(MomentsOut), cudaMemcpyDefault, s));
     return CUBE_OK;
 }
 
@@ -407,12 +424,11 @@ int cube_histogram(cube_ctx* c, const float* d, int64_t nx, int64_t ny, int64_t 
     float scale;
     if (!c || !d || !bins || !outside || !dims_ok(nx, ny, nz, &n)) return CUBE_EINVAL;
     if (!hist_scale(nbins, lo, hi, &scale)) return CUBE_EINVAL;
-    CUBE_CUDA(c, cudaMemsetAsync(c->gbins, 0, (size_t)nbins * sizeof(unsigned long long), s));
-    CUBE_CUDA(c, cudaMemsetAsync(c->gbins + CUBE_MAX_BINS, 0, 2 * sizeof(unsigned long long), s));
+    CUBE_CUDA(c, cudaMemsetAsync(c->gout, 0, (size_t)(nbins + 2) * sizeof(unsigned long long), s));
     int rc = launch_hist(c, d, n, nbins, lo, hi, scale, s);
     if (rc) return rc;
     CUBE_CUDA(c, cudaMemcpyAsync(bins, c->gbins, (size_t)nbins * sizeof(uint64_t), cudaMemcpyDefault, s));
-    CUBE_CUDA(c, cudaMemcpyAsync(outside, c->gbins + CUBE_MAX_BINS, 2 * sizeof(uint64_t), cudaMemcpyDefault, s));
+    CUBE_CUDA(c, cudaMemcpyAsync(outside, c->gout, 2 * sizeof(uint64_t), cudaMemcpyDefault, s));
     return CUBE_OK;
 }
 
@@ -455,15 +471,16 @@ int cube_stats(cube_ctx* c, const float* d, int64_t nx, int64_t ny, int64_t nz, 
     }
     int rc;
     // pass A: moments (+ first select digit)
-    const SelectInit init = select_init_args(c, 0, 1, true), cont = select_init_args(c, 0, 0, false);
+    float* med_direct = static_cast<float*>(device_reachable(c, median));
+    MomentsOut* mom_direct = static_cast<MomentsOut*>(device_reachable(c, moments));
+    const SelectInit init = select_init_args(c, 0, 1, true), cont = select_init_args(c, 0, 0, false, med_direct);
     const unsigned mflags = (flags & CUBE_SAMPLE_STD) | (want_median ? (unsigned)CUBE_COARSE_HIST : 0u);
-    if ((rc = launch_moments(c, d, n, mflags, 0, s, -1, 0.f, 0.f, false, want_median ? &init : nullptr))) return rc;
+    if ((rc = launch_moments(c, d, n, mflags, 0, s, -1, 0.f, 0.f, false, want_median ? &init : nullptr, mom_direct))) return rc;
     if (want_hist) {
-        CUBE_CUDA(c, cudaMemsetAsync(c->gbins, 0, (size_t)nbins * sizeof(unsigned long long), s));
-        CUBE_CUDA(c, cudaMemsetAsync(c->gbins + CUBE_MAX_BINS, 0, 2 * sizeof(unsigned long long), s));
+        CUBE_CUDA(c, cudaMemsetAsync(c->gout, 0, (size_t)(nbins + 2) * sizeof(unsigned long long), s));
     }
     // pass B: histogram + second digit + compaction
-    unsigned long long* goutside = c->gbins + CUBE_MAX_BINS;
+    unsigned long long* goutside = c->gout;
     if (want_median) CUBE_CUDA(c, cudaMemsetAsync(c->gdigits, 0, kDigitBins * sizeof(unsigned long long), s));
     if (want_median && want_hist && nbins <= kSmemHistMaxBins) {
         const size_t smem = (size_t)hist_select_smem(nbins);
@@ -496,9 +513,9 @@ int cube_stats(cube_ctx* c, const float* d, int64_t nx, int64_t ny, int64_t nz, 
     }
     if (want_median) {
         if ((rc = launch_select_pass<2>(c, d, n, s, &cont))) return rc;   // on the candidates unless they did not fit
-        CUBE_CUDA(c, cudaMemcpyAsync(median, &c->sel->result, sizeof(float), cudaMemcpyDefault, s));
+        if (!med_direct) CUBE_CUDA(c, cudaMemcpyAsync(median, &c->sel->result, sizeof(float), cudaMemcpyDefault, s));
     }
-    if (moments) CUBE_CUDA(c, cudaMemcpyAsync(moments, c->mom_out, sizeof(MomentsOut), cudaMemcpyDefault, s));
+    if (moments && !mom_direct) CUBE_CUDA(c, cudaMemcpyAsync(moments, c->mom_out, sizeof(MomentsOut), cudaMemcpyDefault, s));
     if (want_hist) {
         CUBE_CUDA(c, cudaMemcpyAsync(bins, c->gbins, (size_t)nbins * sizeof(uint64_t), cudaMemcpyDefault, s));
         CUBE_CUDA(c, cudaMemcpyAsync(outside, goutside, 2 * sizeof(uint64_t), cudaMemcpyDefault, s));

@@ -154,7 +154,7 @@ hist_win_select_kernel(const float* __restrict__ d, uint64_t n, int nbins, float
     if (scan_ticket) {   // the last CTA locates the second-digit bucket
         __shared__ unsigned long long scan_sm[kScanSmem];
         SelectInit none;
-        none.k = 0; none.cand_cap = 0; none.use_median = 0; none.enabled = 0;
+        none.k = 0; none.cand_cap = 0; none.result_out = nullptr; none.use_median = 0; none.enabled = 0;
         select_scan_if_last_n<1, kBigThreads>(st, gdigits, 1, none, scan_ticket, scan_sm);
     }
 }

@@ -187,7 +187,8 @@ moments_kernel(const float* __restrict__ d, uint64_t n, Partial* __restrict__ pa
                unsigned long long* __restrict__ nvox_acc, int accumulate, unsigned flags,
                MomentsOut* __restrict__ out, unsigned long long* __restrict__ gdigits,
                float wlo, float whi, const ClipState* __restrict__ clip,
-               SelectState* __restrict__ sel, unsigned int* __restrict__ scan_ticket, SelectInit init) {
+               SelectState* __restrict__ sel, unsigned int* __restrict__ scan_ticket, SelectInit init,
+               MomentsOut* __restrict__ out_user) {
     constexpr bool COARSE = (MODE == kMomCoarse);
     __shared__ Partial scratch[kThreads / 32];
     __shared__ uint32_t sbins[COARSE ? kDigitBins + 1 : 1];
@@ -243,6 +244,7 @@ moments_kernel(const float* __restrict__ d, uint64_t n, Partial* __restrict__ pa
         *acc = m;
         *nvox_acc = tot;
         moments_finalize(m, tot, flags, out);
+        if (out_user) *out_user = *out;   // the caller's record, when the device can reach it (no copy is enqueued then)
         *ticket = 0u;
     }
 }

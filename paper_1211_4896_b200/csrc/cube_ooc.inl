@@ -14,7 +14,7 @@ int cube_ooc_begin(cube_ctx* c, int nbins, float lo, float hi, int want_median, 
     c->ooc_active = 1; c->ooc_sweep = 0; c->ooc_bricks = 0;
     c->ooc_nbins = nbins; c->ooc_lo = lo; c->ooc_hi = hi; c->ooc_scale = scale;
     c->ooc_want_median = want_median ? 1 : 0;
-    CUBE_CUDA(c, cudaMemsetAsync(c->gbins, 0, (CUBE_MAX_BINS + 2) * sizeof(unsigned long long), s));
+    CUBE_CUDA(c, cudaMemsetAsync(c->gout, 0, (CUBE_MAX_BINS + 2) * sizeof(unsigned long long), s));
     CUBE_CUDA(c, cudaMemsetAsync(c->gdigits, 0, kDigitBins * sizeof(unsigned long long), s));
     return select_init(c, 0, 1, s);
 }
@@ -86,7 +86,7 @@ int cube_ooc_result(cube_ctx* c, unsigned flags, cube_moments_t* moments, uint64
     if (bins && c->ooc_nbins > 0)
         CUBE_CUDA(c, cudaMemcpyAsync(bins, c->gbins, (size_t)c->ooc_nbins * sizeof(uint64_t), cudaMemcpyDefault, s));
     if (outside && c->ooc_nbins > 0)
-        CUBE_CUDA(c, cudaMemcpyAsync(outside, c->gbins + CUBE_MAX_BINS, 2 * sizeof(uint64_t), cudaMemcpyDefault, s));
+        CUBE_CUDA(c, cudaMemcpyAsync(outside, c->gout, 2 * sizeof(uint64_t), cudaMemcpyDefault, s));
     if (median) {
         if (!c->ooc_want_median || c->ooc_sweep < 3) return CUBE_EINVAL;
         CUBE_CUDA(c, cudaMemcpyAsync(median, &c->sel->result, sizeof(float), cudaMemcpyDefault, s));
@@ -103,7 +103,7 @@ int cube_shard_buffers(cube_ctx* c, cube_shard_buffers_t* out) {
     if (!c || !out) return CUBE_EINVAL;
     out->record = c->acc;
     out->bins = reinterpret_cast<uint64_t*>(c->gbins);
-    out->outside = reinterpret_cast<uint64_t*>(c->gbins + CUBE_MAX_BINS);
+    out->outside = reinterpret_cast<uint64_t*>(c->gout);
     out->digits = reinterpret_cast<uint64_t*>(c->gdigits);
     return CUBE_OK;
 }

@@ -216,6 +216,7 @@ __device__ __forceinline__ void select_run(const float* __restrict__ d, uint64_t
 // copy precedes a selection.  `sm` = kScanSmem words of shared memory.
 struct SelectInit {
     unsigned long long k, cand_cap;
+    float* result_out;   // PASS 2: also write the result here (the caller's buffer when the device can reach it), or null
     uint32_t use_median, enabled;
 };
 
@@ -285,6 +286,7 @@ __device__ __forceinline__ void select_scan_body(SelectState* __restrict__ st, u
                 }
             }
             if (PASS == 0 || invalid) { st->k = k; st->prefix = prefix; st->result = __int_as_float(0x7fc00000); }
+            if (PASS == 2 && invalid && init.result_out) *init.result_out = __int_as_float(0x7fc00000);
             s_k = k;
             s_flags = (unsigned long long)invalid | ((unsigned long long)prefix << 32);
         }
@@ -317,7 +319,10 @@ __device__ __forceinline__ void select_scan_body(SelectState* __restrict__ st, u
                 const uint32_t pre = (PASS == 0) ? b : ((prefix << BITS) | b);
                 st->prefix = pre;
                 st->k = kk - ex2;
-                if (PASS == 2) st->result = __uint_as_float(bits_of_key(pre));
+                if (PASS == 2) {
+                    st->result = __uint_as_float(bits_of_key(pre));
+                    if (init.result_out) *init.result_out = st->result;
+                }
             }
         }
     }
