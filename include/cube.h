@@ -264,13 +264,19 @@ int cube_last_cuda_error(const cube_ctx* ctx);
 int cube_set_launch(cube_ctx* ctx, int ctas_per_sm);
 enum {
     CUBE_KNOB_CTAS_PER_SM = 0, /* same as cube_set_launch */
-    CUBE_KNOB_BIGHIST = 1      /* histograms with more than 16384 bins, one CTA of 1024 threads per SM:
+    CUBE_KNOB_BIGHIST = 1,     /* histograms with more than 16384 bins, one CTA of 1024 threads per SM:
                                   0 = automatic (default): 32-bit shared-memory counters for a window of 32768
                                       consecutive bins chosen by sampling + global REDs for the rest when at most
                                       1/32 of the sampled voxels fall outside the window, else 16-bit packed counters
                                       for all bins (the choice is made on the device),
                                   1 = clusters of two CTAs holding 32-bit counters in distributed shared memory,
                                   2 = always the 16-bit packed counters */
+    CUBE_KNOB_MINIMAP = 2      /* cube_minimap kernel: 0 = automatic (default): lines staged through a shared-memory
+                                  ring by TMA bulk copies when the rows are 16-byte aligned, the cells at most 480
+                                  voxels wide and a cell row has at least 512 lines (or the 128-bit kernel is not
+                                  eligible), else as 1; 1 = 128-bit register kernel when eligible (rows 16-byte
+                                  aligned, px >= 4), else the scalar one; 2 = always the scalar kernel; 3 = the TMA
+                                  ring whenever it is eligible, whatever the number of lines */
 };
 int cube_set_knob(cube_ctx* ctx, int knob, int value);
 /* Number of kernels launched through this context since creation (bench.py's gpu_launches). */

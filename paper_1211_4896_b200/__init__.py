@@ -35,7 +35,7 @@ SYMBOLS = ["cube_create", "cube_destroy", "cube_moments", "cube_histogram", "cub
            "cube_mad", "cube_clipped_moments", "cube_sigma_clip", "cube_minimap_dims", "cube_minimap",
            "cube_shard_buffers", "cube_shard_merge_records", "cube_shard_advance", "cube_median_torben"]
 SHARD_RECORD_BYTES, SHARD_DIGITS = 40, 8192
-KNOB_CTAS_PER_SM, KNOB_BIGHIST = 0, 1
+KNOB_CTAS_PER_SM, KNOB_BIGHIST, KNOB_MINIMAP = 0, 1, 2
 KIND_NAMES = ["moments", "moments_coarse", "histogram", "select_pass0", "select_pass1", "select_pass2",
               "select_cand", "select_scan", "hist_select", "probe_read", "other", "moments_window", "minimap", "torben_pass"]
 

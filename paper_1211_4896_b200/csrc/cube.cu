@@ -6,9 +6,11 @@
 #include <math.h>
 #include <new>
 #include <string.h>
+#include <algorithm>
 #include <vector>
 
 #include "cube_kernels.cuh"
+#include "cube_minimap_tma.cuh"
 
 using namespace cube;
 
@@ -17,6 +19,7 @@ struct cube_ctx {
     int num_sms = 0;
     int ctas_per_sm = 0;  // 0 = per-kernel default
     int bighist = 0;      // CUBE_KNOB_BIGHIST: 0 = 16-bit packed counters, 1 = cluster DSM
+    int minimap_variant = 0;  // CUBE_KNOB_MINIMAP: 0 = automatic, 1 = no TMA ring, 2 = scalar kernel only, 3 = TMA ring whenever eligible
     int last_cuda = 0;
     uint64_t launches = 0;
     // device scratch
@@ -370,6 +373,8 @@ int cube_create(cube_ctx** out, size_t scratch_bytes_hint) {
                                     (kBigWords + 4) * (int)sizeof(uint32_t)) == cudaSuccess;
     ok = ok && cudaFuncSetAttribute(hist_win_select_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize,
                                     kBigFusedSmem) == cudaSuccess;
+    ok = ok && cudaFuncSetAttribute(minimap_tma_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                    kMapTmaSmem) == cudaSuccess;
     ok = ok && cudaFuncSetAttribute(hist_dsm_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize,
                                     (32768 + 1) * (int)sizeof(uint32_t)) == cudaSuccess;
     if (!ok) { cube_destroy(c); return CUBE_ENOMEM; }
@@ -619,14 +624,30 @@ int cube_minimap(cube_ctx* c, const float* d, int64_t nx, int64_t ny, int64_t nz
         cudaGetLastError();
         return CUBE_EINVAL;
     }
-    // 128-bit kernel: rows 16-byte aligned, segments of whole cells that start on a multiple of 4 voxels
+    // Segments of whole cells that start on a multiple of 4 voxels (16 bytes): what both the TMA-ring kernel (bulk
+    // copies of whole lines) and the 128-bit register kernel need; rows must be 16-byte aligned as well.
     const long long unit = (px % 4 == 0) ? 1 : (px % 2 == 0) ? 2 : 4;     // cells per segment must be a multiple of it
+    const bool rows16 = (nx % 4 == 0) && (((uintptr_t)d & 15u) == 0);
+    // TMA ring: segments that are also whole 128-byte lines (32 voxels) when the cell width allows it within
+    // kMapTmaCols columns (px = 30: 16 cells = 480 voxels) -- no L2 line is then shared by two CTAs; such segments
+    // are not re-balanced (the last one of a row is simply narrower).
+    long long unit128 = 1;
+    while ((unit128 * px) % 32 != 0) ++unit128;                           // 32 / gcd(px, 32)
+    const bool seg128 = unit128 * px <= kMapTmaCols;
+    const long long unit_t = seg128 ? unit128 : unit;
+    const long long cpst = (kMapTmaCols / px) / unit_t * unit_t;
     const long long cps4 = (kMap4Cols / px) / unit * unit;
-    const bool v4 = (nx % 4 == 0) && (((uintptr_t)d & 15u) == 0) && cps4 >= 1 && px >= 4;
-    g.cells_per_seg = v4 ? cps4 : (px > kMapThreads ? 1 : kMapThreads / px);
+    // A CTA of the ring kernel pays for filling and draining its ring once per cell row: it wins from about 512
+    // lines per cell row upwards (measured on c2: 30^3 cells 6.3 vs 4.4 TB/s, 16^3 cells 5.0 vs 5.8 TB/s).
+    const bool v4_ok = rows16 && cps4 >= 1 && px >= 4;
+    const long double lines = (long double)std::min(py, ny) * (long double)std::min(pz, nz);
+    const bool tma = rows16 && cpst >= 1 && lines < 2147483000.0L &&
+                     (c->minimap_variant == 3 || (c->minimap_variant == 0 && (lines >= 512.0L || !v4_ok)));
+    const bool v4 = !tma && v4_ok && c->minimap_variant <= 1;
+    g.cells_per_seg = tma ? cpst : v4 ? cps4 : (px > kMapThreads ? 1 : kMapThreads / px);
     g.nseg = (g.mx + g.cells_per_seg - 1) / g.cells_per_seg;
     {   // balance the segments of a row (35 cells: 18 + 17 instead of 34 + 1)
-        const long long u = v4 ? unit : 1;
+        const long long u = tma ? unit_t : v4 ? unit : 1;
         const long long even = ((g.mx + g.nseg - 1) / g.nseg + u - 1) / u * u;
         if (even < g.cells_per_seg) { g.cells_per_seg = even; g.nseg = (g.mx + even - 1) / even; }
     }
@@ -637,8 +658,13 @@ int cube_minimap(cube_ctx* c, const float* d, int64_t nx, int64_t ny, int64_t nz
         const unsigned grid = (unsigned)(g.nseg * g.my * g.mz);
         g.main_threads = ((g.cells_per_seg * px / 4) + 31) / 32 * 32;
         const unsigned block4 = (unsigned)g.main_threads + (unsigned)((g.cells_per_seg - 1 + 31) / 32 * 32);  // + boundary threads
-        if (v4) minimap_v4_kernel<<<grid, block4, 0, s>>>(d, g, flags & CUBE_SAMPLE_STD,
-                                                          reinterpret_cast<MomentsOut*>(cells));
+        if (tma) {
+            const long long wmax = std::min<long long>(g.cells_per_seg * px, nx);     // widest segment, a multiple of 4
+            const unsigned block = (unsigned)((wmax + 31) / 32 * 32) + 32u;           // + the producer warp
+            minimap_tma_kernel<<<grid, block, kMapTmaSmem, s>>>(d, g, flags & CUBE_SAMPLE_STD,
+                                                                reinterpret_cast<MomentsOut*>(cells));
+        } else if (v4) minimap_v4_kernel<<<grid, block4, 0, s>>>(d, g, flags & CUBE_SAMPLE_STD,
+                                                                 reinterpret_cast<MomentsOut*>(cells));
         else minimap_kernel<<<grid, kMapThreads, 0, s>>>(d, g, flags & CUBE_SAMPLE_STD,
                                                          reinterpret_cast<MomentsOut*>(cells));
     }
@@ -684,6 +710,10 @@ int cube_set_knob(cube_ctx* c, int knob, int value) {
         case CUBE_KNOB_BIGHIST:
             if (value < 0 || value > 2) return CUBE_EINVAL;
             c->bighist = value;
+            return CUBE_OK;
+        case CUBE_KNOB_MINIMAP:
+            if (value < 0 || value > 3) return CUBE_EINVAL;
+            c->minimap_variant = value;
             return CUBE_OK;
         default: return CUBE_EINVAL;
     }

@@ -1,0 +1,162 @@
+// cube_minimap_tma.cuh -- the statistical mini-map (DESIGN.md sec. 11 NEXT-2) with the lines of
+// a cell row staged through a shared-memory ring by TMA bulk copies (cp.async.bulk + mbarrier).
+//
+// Why a ring here and not in the global passes: a cell row of 30-voxel cells has no 128-bit register tiling that
+// respects the cell boundaries (minimap_v4_kernel masks columns, reads straddling float4s twice and spends 16.7
+// instructions per voxel).  With the lines in shared memory a thread simply owns ONE COLUMN of the segment -- a
+// conflict-free LDS.32 per voxel, one accumulator set, no masks -- and the copy engine keeps ~96 KiB per CTA in
+// flight whatever the consumers are doing.
+//
+// CTA = (segment of whole cells along x, cy, cz), exactly as in minimap_kernel.  Warps 0..W-1 own the columns,
+// the last warp is the producer: for every group of kMapUnroll lines it waits for the stage to be released
+// (`empty` barrier: one arrival per consumer warp), posts the byte count on the stage's `full` barrier and lets 8
+// lanes issue one bulk copy each (a line of the segment is contiguous, 16-byte aligned, a multiple of 16 bytes).
+// Consumers wait on `full`, take their column of the 8 lines into registers, release the stage at once and then
+// run MapColF::group (the hot / safe paths of the moments pass).  The per-cell merge is the scalar kernel's.
+#pragma once
+#include "cube_minimap.cuh"
+
+namespace cube {
+
+constexpr int kMapTmaCols = 480;                       // most columns (consumer threads) per segment: 15 warps + producer
+constexpr int kMapTmaMaxThreads = kMapTmaCols + 32;    // + the producer warp
+constexpr int kMapTmaLine = kMapTmaCols * 4;           // bytes between lines of a stage (compile time: LDS [R + imm])
+constexpr int kMapTmaStageLines = 2 * kMapUnroll;      // lines per stage = two MapColF groups per barrier wait
+constexpr int kMapTmaStage = kMapTmaStageLines * kMapTmaLine;
+constexpr int kMapTmaStages = 3;
+constexpr int kMapTmaBarBytes = 128;                   // full[3], empty[3] in front of the ring
+constexpr int kMapTmaSmem = kMapTmaBarBytes + kMapTmaStages * kMapTmaStage;   // 92288 B: 2 CTAs per SM
+
+__device__ __forceinline__ void mbar_init(uint32_t bar, uint32_t count) {
+    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" :: "r"(bar), "r"(count) : "memory");
+}
+__device__ __forceinline__ void mbar_arrive(uint32_t bar) {
+    asm volatile("{\n\t.reg .b64 st;\n\tmbarrier.arrive.shared::cta.b64 st, [%0];\n\t}" :: "r"(bar) : "memory");
+}
+__device__ __forceinline__ void mbar_arrive_expect_tx(uint32_t bar, uint32_t bytes) {
+    asm volatile("{\n\t.reg .b64 st;\n\tmbarrier.arrive.expect_tx.shared::cta.b64 st, [%0], %1;\n\t}"
+                 :: "r"(bar), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void mbar_wait(uint32_t bar, uint32_t parity) {
+    uint32_t done;
+    do {
+        asm volatile("{\n\t.reg .pred p;\n\tmbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2, %3;\n\t"
+                     "selp.u32 %0, 1, 0, p;\n\t}" : "=r"(done) : "r"(bar), "r"(parity), "r"(20000u) : "memory");
+    } while (!done);
+}
+// 1-D bulk copy global -> shared, completion counted in bytes on `bar` (TMA without a tensor map).
+__device__ __forceinline__ void bulk_load(uint32_t dst, const void* src, uint32_t bytes, uint32_t bar) {
+    asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];"
+                 :: "r"(dst), "l"(src), "r"(bytes), "r"(bar) : "memory");
+}
+
+
+// column value k of the current stage: `base` = shared address of this thread's column in line 0 of the stage
+template <int K>
+__device__ __forceinline__ float lds_line(uint32_t base) {
+    float v;
+    asm volatile("ld.shared.f32 %0, [%1+%2];" : "=f"(v) : "r"(base), "n"(K * kMapTmaLine) : "memory");
+    return v;
+}
+template <int K0>
+__device__ __forceinline__ void lds_group(uint32_t base, float (&v)[kMapUnroll]) {
+    v[0] = lds_line<K0 + 0>(base); v[1] = lds_line<K0 + 1>(base); v[2] = lds_line<K0 + 2>(base); v[3] = lds_line<K0 + 3>(base);
+    v[4] = lds_line<K0 + 4>(base); v[5] = lds_line<K0 + 5>(base); v[6] = lds_line<K0 + 6>(base); v[7] = lds_line<K0 + 7>(base);
+}
+
+// g.cells_per_seg * g.px is a multiple of 4 and <= kMapTmaCols; g.nx % 4 == 0; d is 16-byte aligned; py * pz < 2^31.
+// blockDim.x = 32 * (warps that cover the widest segment + 1); kMapTmaSmem bytes of dynamic shared memory.
+__global__ void __launch_bounds__(kMapTmaMaxThreads, 2)
+minimap_tma_kernel(const float* __restrict__ d, MapGeom g, unsigned flags, MomentsOut* __restrict__ cells) {
+    extern __shared__ __align__(128) unsigned char smem[];
+    const long long b = blockIdx.x;
+    const long long seg = b % g.nseg, cy = (b / g.nseg) % g.my, cz = b / (g.nseg * g.my);
+    const long long c0 = seg * g.cells_per_seg;
+    const long long x0 = c0 * g.px;
+    const long long x1 = min((c0 + g.cells_per_seg) * g.px, g.nx);
+    const long long y0 = cy * g.py, y1 = min(y0 + g.py, g.ny);
+    const long long z0 = cz * g.pz, z1 = min(z0 + g.pz, g.nz);
+    const int width = (int)(x1 - x0), pyn = (int)(y1 - y0);
+    const int total = pyn * (int)(z1 - z0);                        // lines of the cell row, taken as one sequence
+    const int nstages = (total + kMapTmaStageLines - 1) / kMapTmaStageLines;
+    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    const int producer = (int)(blockDim.x >> 5) - 1;               // the last warp
+    const int nactive = (width + 31) >> 5;                         // consumer warps that own a column
+    const uint32_t full0 = smem_addr(smem), empty0 = full0 + 8u * kMapTmaStages, ring0 = full0 + kMapTmaBarBytes;
+
+    if (tid == 0) {
+#pragma unroll
+        for (int s = 0; s < kMapTmaStages; ++s) { mbar_init(full0 + 8u * s, 1u); mbar_init(empty0 + 8u * s, (uint32_t)nactive); }
+        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+    }
+    __syncthreads();
+
+    MapColF f;
+    if (warp == producer) {
+        // ---- producer warp: lane k copies line k of every stage
+        const uint32_t lbytes = (uint32_t)width * 4u;
+        const float* const base = d + ((z0 * g.ny + y0) * g.nx + x0);
+        const long long plane = g.ny * g.nx;
+        int st = 0;
+        uint32_t par = 1;   // parity to wait for on `empty`: the first round passes at once
+        for (int si = 0; si < nstages; ++si) {
+            mbar_wait(empty0 + 8u * st, par);
+            const int l0 = si * kMapTmaStageLines;
+            const int cnt = min(kMapTmaStageLines, total - l0);
+            if (lane == 0) mbar_arrive_expect_tx(full0 + 8u * st, lbytes * (uint32_t)cnt);
+            __syncwarp();
+            if (lane < cnt) {
+                const int l = l0 + lane;
+                const int zz = l / pyn, yy = l - zz * pyn;
+                bulk_load(ring0 + (uint32_t)(st * kMapTmaStage + lane * kMapTmaLine), base + zz * plane + yy * g.nx, lbytes,
+                          full0 + 8u * st);
+            }
+            if (++st == kMapTmaStages) { st = 0; par ^= 1u; }
+        }
+    } else if (warp < nactive) {
+        // ---- consumers: thread t owns column x0 + t (warps beyond the segment's width go straight to the merge)
+        const bool active = tid < width;
+        bool safe_mode = true;
+        int st = 0;
+        uint32_t par = 0;
+        const uint32_t mycol = ring0 + 4u * (uint32_t)tid;
+        for (int si = 0; si < nstages; ++si) {
+            const uint32_t col = mycol + (uint32_t)(st * kMapTmaStage);
+            mbar_wait(full0 + 8u * st, par);
+            const int cnt = total - si * kMapTmaStageLines;
+            if (cnt >= kMapTmaStageLines) {
+                float v0[kMapUnroll], v1[kMapUnroll];
+                lds_group<0>(col, v0);
+                lds_group<kMapUnroll>(col, v1);
+                __syncwarp();
+                if (lane == 0) mbar_arrive(empty0 + 8u * st);      // values are in registers: release the stage
+                if (active) { f.group(v0, safe_mode); f.group(v1, safe_mode); }
+            } else {                                               // the last (py * pz) mod 16 lines of the cell row
+                if (active)
+                    for (int k = 0; k < cnt; ++k) {
+                        float x;
+                        asm volatile("ld.shared.f32 %0, [%1];" : "=f"(x) : "r"(col + (uint32_t)(k * kMapTmaLine)) : "memory");
+                        f(x);
+                    }
+                __syncwarp();
+                if (lane == 0) mbar_arrive(empty0 + 8u * st);
+            }
+            if (++st == kMapTmaStages) { st = 0; par ^= 1u; }
+        }
+    }
+    __syncthreads();   // every copy has landed and has been consumed: the ring is free for the column records
+    Partial* cols = reinterpret_cast<Partial*>(smem + kMapTmaBarBytes);
+    if (tid < width) cols[tid] = f.partial();
+    __syncthreads();
+    const long long ncell = min(g.cells_per_seg, g.mx - c0);
+    if (tid < ncell) {
+        const long long cb = (long long)tid * g.px;
+        const long long w = min(g.px, (long long)width - cb);
+        Partial m = partial_empty();
+        for (long long i = 0; i < w; ++i) m = partial_merge(m, cols[cb + i]);
+        moments_finalize(m, (unsigned long long)total * (unsigned long long)w, flags,
+                         &cells[(cz * g.my + cy) * g.mx + c0 + tid]);
+    }
+}
+
+}  // namespace cube

@@ -132,3 +132,85 @@ def test_config3_full_size():
 def test_config4_full_size():
     ref = _big_config("c4", [256, 65536], [])
     assert bits(ref["min"]) == 0 and (ref["count"] - 1) // 2 == 2 ** 32 - 1
+
+
+def _merge_brick_moments(parts):
+    """Whole-cube (count, mean, population std) from the oracle's per-brick records, in exact rational
+    arithmetic (a double is a dyadic rational): mean = sum n_i mean_i / n, M2 = sum M2_i + sum n_i (mean_i - mean)^2
+    with M2_i = n_i std_i^2 (the definition of the population variance regrouped by brick, nothing else)."""
+    from fractions import Fraction
+    n = sum(p["count"] for p in parts)
+    mean = sum(Fraction(p["mean"]) * p["count"] for p in parts if p["count"]) / n
+    m2 = sum(Fraction(p["std"]) ** 2 * p["count"] + (Fraction(p["mean"]) - mean) ** 2 * p["count"]
+             for p in parts if p["count"])
+    return n, float(mean), math.sqrt(float(m2 / n))
+
+
+@pytest.mark.skipif(not FULL, reason="256 GiB out-of-core job + the oracle on all 512 bricks: set CUBE_FULLSIZE=1")
+def test_config5_full_size():
+    """BASELINE.json configs[4] at full size, through the call bench.py --config c5 times (cube_stats_stream, 512
+    bricks of 512^3 produced by a callback, 128 GiB kept in HBM after sweep 1).  The oracle cannot hold 256 GiB, so
+    it runs brick by brick on the SAME bytes (each brick regenerated by the same device generator and copied to the
+    host; SURVEY.md sec. 8(c) "oracle at scale"): count / nan_count / min / max / bins / outside are exact sums and
+    extrema of the per-brick oracle results, mean / std their exact regrouping (above), and the median is proved by
+    the rank certificate summed over the bricks.  Oracle calls run in a thread pool (one brick per call, the
+    oracle itself stays single-threaded)."""
+    from concurrent.futures import ThreadPoolExecutor
+    cfg = cubegen.CONFIGS["c5"]
+    nx, ny, nz = cfg["dims"]
+    n = nx * ny * nz
+    brick = (512, 512, 512)
+    bvox = 512 ** 3
+    origins = cubegen.brick_grid(cfg, brick)
+    assert len(origins) == 512 and n == 512 * bvox
+    nb, lo, hi = 4096, -0.02, 0.5
+    scr = torch.empty(bvox, dtype=torch.float32, device="cuda")
+    ctx = cube.Context(scratch_bytes_hint=1 << 30)
+    try:
+        ctx.stream_workspace(bvox * 4, host_slots=4, resident_bytes=256 * bvox * 4)
+
+        def fill(b, sweep, h_dst, nvox, fs):
+            cubegen.generate_to_host(cfg, h_dst, scr.data_ptr(), origin=origins[b], brick=brick, stream=fs)
+            return 0
+
+        m, bins, outside, med, info = ctx.stats_stream(len(origins), bvox, n, fill, nb, lo, hi)
+        assert info["sweeps"] == 2
+    finally:
+        ctx.close()
+    medv = np.float32(med)
+
+    def oracle_brick(a):
+        r = oracle.moments(a)
+        hb, ho = oracle.histogram(a, nb, lo, hi)
+        less, equal = oracle.rank_counts(a, medv)
+        return r, hb.astype(np.uint64), ho.astype(np.uint64), less, equal
+
+    workers = max(1, min(14, (os.cpu_count() or 2) - 2))
+    futs = []
+    with ThreadPoolExecutor(workers) as pool:
+        for i, org in enumerate(origins):
+            cubegen.generate_device(cfg, scr.data_ptr(), origin=org, brick=brick)
+            torch.cuda.synchronize()
+            a = scr.cpu().numpy()
+            futs.append(pool.submit(oracle_brick, a))
+            del a
+            while sum(not f.done() for f in futs) > workers + 4:          # bound the host copies in flight
+                futs[max(0, i - workers - 4)].result()
+        parts = [f.result() for f in futs]
+    recs = [p[0] for p in parts]
+    count, mean, std = _merge_brick_moments(recs)
+    assert m["count"] == count and m["nan_count"] == n - count == sum(r["nan_count"] for r in recs)
+    live = [r for r in recs if r["count"]]
+    omin = min((r["min"] for r in live), key=lambda v: (float(v), not math.copysign(1.0, float(v)) < 0))
+    omax = max((r["max"] for r in live), key=lambda v: (float(v), not math.copysign(1.0, float(v)) < 0))
+    assert bits(m["min"]) == bits(omin) and bits(m["max"]) == bits(omax)
+    assert abs(m["mean"] - mean) <= REL * abs(mean), (m, mean)
+    assert abs(m["std"] - std) <= REL * std, (m, std)
+    rb = sum(p[1] for p in parts)
+    ro = sum(p[2] for p in parts)
+    assert (bins == rb).all() and (outside == ro).all()
+    assert int(rb.sum()) + int(ro.sum()) == count and int(ro[1]) > 0
+    less = sum(p[3] for p in parts)
+    equal = sum(p[4] for p in parts)
+    k = (count - 1) // 2
+    assert equal >= 1 and less <= k < less + equal, (float(medv), k, less, equal)

@@ -226,8 +226,10 @@ def check_minimap(got, ref):
                                        ((100, 33, 17), (7, 5, 3)), ((37, 29, 11), (37, 29, 11)),
                                        ((1200, 9, 5), (600, 4, 2)), ((1300, 6, 4), (1300, 3, 2)),
                                        ((130, 70, 50), (1, 1, 1)), ((50, 40, 30), (64, 64, 64)),
-                                       ((513, 20, 19), (30, 30, 30))])
-def test_minimap_shapes(ctx, dims, part):
+                                       ((513, 20, 19), (30, 30, 30)), ((960, 20, 19), (30, 30, 30)),
+                                       ((1024, 35, 9), (30, 7, 9)), ((484, 12, 10), (480, 5, 5))])
+@pytest.mark.parametrize("variant", [0, 1, 2, 3])   # automatic / 128-bit register kernel / scalar kernel / TMA ring
+def test_minimap_shapes(ctx, dims, part, variant):
     nx, ny, nz = dims
     r = np.random.default_rng(nx * 31 + ny)
     a = (r.standard_normal(nx * ny * nz) * 0.002 + 0.001).astype(np.float32)
@@ -235,8 +237,32 @@ def test_minimap_shapes(ctx, dims, part):
     cubev = a.reshape(nz, ny, nx)
     cubev[0:min(part[2], nz), 0:min(part[1], ny), 0:min(part[0], nx)] = np.nan          # one fully blanked cell
     t = dev(a, misalign=nx % 4)
-    check_minimap(run_minimap(ctx, t, dims, part), oracle.minimap(a, dims, part))
-    check_minimap(run_minimap(ctx, t, dims, part, flags=cube.SAMPLE_STD), oracle.minimap(a, dims, part, sample_std=True))
+    ctx.set_knob(cube.KNOB_MINIMAP, variant)
+    try:
+        check_minimap(run_minimap(ctx, t, dims, part), oracle.minimap(a, dims, part))
+        check_minimap(run_minimap(ctx, t, dims, part, flags=cube.SAMPLE_STD),
+                      oracle.minimap(a, dims, part, sample_std=True))
+    finally:
+        ctx.set_knob(cube.KNOB_MINIMAP, 0)
+
+
+def test_minimap_variants_agree_on_nan_free_and_nan_heavy_rows(ctx):
+    # hot path (no NaN), safe path (scattered NaN) and whole blanked planes in one cube; the three kernels must
+    # give the same integers and the oracle's values
+    nx, ny, nz = 480, 64, 45
+    r = np.random.default_rng(77)
+    a = (r.standard_normal(nx * ny * nz) * 0.002).astype(np.float32).reshape(nz, ny, nx)
+    a[10:20][r.random((10, ny, nx)) < 0.01] = np.nan
+    a[30:33] = np.nan
+    a = a.reshape(-1)
+    t = dev(a)
+    ref = oracle.minimap(a, (nx, ny, nz), (30, 30, 30))
+    for variant in (0, 1, 2, 3):
+        ctx.set_knob(cube.KNOB_MINIMAP, variant)
+        try:
+            check_minimap(run_minimap(ctx, t, (nx, ny, nz), (30, 30, 30)), ref)
+        finally:
+            ctx.set_knob(cube.KNOB_MINIMAP, 0)
 
 
 def test_minimap_scaled_config_and_global_consistency(ctx):
