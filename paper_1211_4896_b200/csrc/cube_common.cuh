@@ -34,7 +34,11 @@ __device__ __forceinline__ uint32_t key_of(float x) {
 // Radix digits of the exact select: 13 + 10 + 9 bits of the order-preserving key.  A wide first
 // digit makes the median's bucket small (sign + exponent + 4 mantissa bits: ~0.08 % of config 2), which is what
 // the second pass has to revisit and compact.
-constexpr int kBits0 = 13, kBits1 = 10, kBits2 = 9;
+#ifndef CUBE_BITS0      // build-time override for digit-width experiments
+#define CUBE_BITS0 13
+#define CUBE_BITS1 10
+#endif
+constexpr int kBits0 = CUBE_BITS0, kBits1 = CUBE_BITS1, kBits2 = 32 - CUBE_BITS0 - CUBE_BITS1;
 constexpr int kShift0 = 32 - kBits0;          // 19: key >> kShift0 is the first digit
 constexpr int kBins0 = 1 << kBits0, kBins1 = 1 << kBits1, kBins2 = 1 << kBits2;
 constexpr int kDigitBins = kBins0;            // size of the global digit arrays
