@@ -227,17 +227,64 @@ moments_kernel(const float* __restrict__ d, uint64_t n, Partial* __restrict__ pa
     }
     __syncthreads();
     if (!is_last) return;
-    // last CTA: fixed-order merge of the per-CTA partials (thread i takes i, i+256, ...; then the tree)
+    // last CTA: fixed-order merge of the per-CTA partials.  A tree of Chan merges is a chain of ~13 dependent fp64
+    // divisions (5 us of tail on a cube that streams in 10 us: profiles/r1_v10_c2.md), so the partials are first
+    // re-expressed as sums about ONE pivot P -- the mean of the lowest-indexed non-empty partial: s_i = n_i (mean_i -
+    // P), q_i = M2_i + n_i (mean_i - P)^2 -- which merge by plain additions (thread i takes i, i+256, ...; then
+    // shuffles).  P is the mean of a CTA whose tiles are spread over the whole cube, so |P - mean| << std and
+    // q - s^2/n loses nothing; a constant cube gives mean_i == P, s = q = 0 and std = 0 exactly.
     __threadfence();
-    Partial m = partial_empty();
-    for (unsigned i = threadIdx.x; i < gridDim.x; i += kThreads) {
-        Partial b;  // written by other CTAs: read through L2
-        b.n = __ldcg(&partials[i].n); b.mean = __ldcg(&partials[i].mean); b.m2 = __ldcg(&partials[i].m2);
-        b.kmin = __ldcg(&partials[i].kmin); b.kmax = __ldcg(&partials[i].kmax);
-        m = partial_merge(m, b);
+    __shared__ unsigned int first_live;
+    if (threadIdx.x == 0) first_live = 0xFFFFFFFFu;
+    __syncthreads();
+    {
+        unsigned int mine = 0xFFFFFFFFu;
+        for (unsigned i = threadIdx.x; i < gridDim.x; i += kThreads)
+            if (mine == 0xFFFFFFFFu && __ldcg(&partials[i].n) != 0) mine = i;
+        if (mine != 0xFFFFFFFFu) atomicMin(&first_live, mine);
     }
     __syncthreads();
-    m = partial_block_reduce(m, scratch);
+    Partial m = partial_empty();
+    if (first_live != 0xFFFFFFFFu) {
+        const double P = __ldcg(&partials[first_live].mean);
+        unsigned long long cn = 0;
+        double cs = 0.0, cq = 0.0;
+        uint32_t kmin = 0xFFFFFFFFu, kmax = 0u;
+        for (unsigned i = threadIdx.x; i < gridDim.x; i += kThreads) {   // written by other CTAs: read through L2
+            const unsigned long long bn = __ldcg(&partials[i].n);
+            const double bmean = __ldcg(&partials[i].mean), bm2 = __ldcg(&partials[i].m2);
+            kmin = min(kmin, __ldcg(&partials[i].kmin));
+            kmax = max(kmax, __ldcg(&partials[i].kmax));
+            if (bn) {
+                const double nb = (double)bn, dm = bmean - P, nd = nb * dm;
+                cn += bn; cs += nd; cq += bm2 + nd * dm;
+            }
+        }
+#pragma unroll
+        for (int off = 16; off > 0; off >>= 1) {
+            cn += __shfl_down_sync(0xffffffffu, cn, off);
+            cs += __shfl_down_sync(0xffffffffu, cs, off);
+            cq += __shfl_down_sync(0xffffffffu, cq, off);
+            kmin = min(kmin, __shfl_down_sync(0xffffffffu, kmin, off));
+            kmax = max(kmax, __shfl_down_sync(0xffffffffu, kmax, off));
+        }
+        const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+        __syncthreads();   // scratch is free (the CTA's own block reduce is over)
+        if (lane == 0) { scratch[warp].n = cn; scratch[warp].mean = cs; scratch[warp].m2 = cq; scratch[warp].kmin = kmin; scratch[warp].kmax = kmax; }
+        __syncthreads();
+        if (threadIdx.x == 0) {
+            cn = 0; cs = 0.0; cq = 0.0; kmin = 0xFFFFFFFFu; kmax = 0u;
+#pragma unroll
+            for (int w = 0; w < kThreads / 32; ++w) {
+                cn += scratch[w].n; cs += scratch[w].mean; cq += scratch[w].m2;
+                kmin = min(kmin, scratch[w].kmin); kmax = max(kmax, scratch[w].kmax);
+            }
+            const double nn = (double)cn;
+            const double m2 = cq - cs * (cs / nn);
+            m.n = cn; m.mean = P + cs / nn; m.m2 = (m2 < 0.0) ? 0.0 : m2;   // rounding only; a NaN (Inf voxels) stays
+            m.kmin = kmin; m.kmax = kmax;
+        }
+    }
     if (threadIdx.x == 0) {
         unsigned long long tot = n;
         if (accumulate) { m = partial_merge(*acc, m); tot += *nvox_acc; }

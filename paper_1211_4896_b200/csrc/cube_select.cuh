@@ -229,29 +229,50 @@ __device__ __forceinline__ unsigned long long warp_sum_u64(unsigned long long v)
 }
 
 // Two levels, every global load coalesced and independent of the others: (1) each warp sums chunks of 32 consecutive
-// bins (one load per lane per chunk, several chunks in flight) into shared memory; (2) warp 0 scans the <= 256 chunk
-// totals, finds the chunk holding rank k, loads that chunk once more and finds the bin.  ~2-3 us for 8192 bins
-// (the one-thread-per-32-bins form spent 5-10 us in dependent L2 round trips).
+// bins (one load per lane per chunk, up to 8 chunks in flight) into shared memory; (2) warp 0 scans the <= 256 chunk
+// totals and finds the chunk holding rank k; (3) the warp that loaded that chunk finds the bin in its registers (when
+// a warp's chunks did not all fit one round -- 8192 bins on 256 threads -- it loads the chunk once more).  The scan
+// is a chain of dependent L2 round trips run by ONE CTA at the tail of a pass (~0.5 us each), so everything that
+// does not depend on the counts (the rank asked for, the prefix so far) is loaded before the bins.
 template <int PASS, int THREADS>
 __device__ __forceinline__ void select_scan_body(SelectState* __restrict__ st, unsigned long long* __restrict__ gdigits,
                                                  int clear, const SelectInit& init, unsigned long long* sm) {
     constexpr int NB = (PASS == 0) ? kBins0 : (PASS == 1) ? kBins1 : kBins2;
     constexpr int BITS = (PASS == 0) ? kBits0 : (PASS == 1) ? kBits1 : kBits2;
     constexpr int CHUNKS = NB / 32, NW = THREADS / 32;
-    constexpr int CPL = (CHUNKS + 31) / 32;     // chunk totals per lane of warp 0
+    constexpr int CPL = (CHUNKS + 31) / 32;               // chunk totals per lane of warp 0
+    constexpr int CPW = (CHUNKS + NW - 1) / NW;           // chunks per warp
+    constexpr int INFL = CPW < 8 ? CPW : 8;               // loads in flight per lane
+    constexpr bool KEEP = (CPW <= INFL);                  // a warp's chunks stay in registers
     static_assert(CHUNKS <= 256, "chunk totals must fit the shared array");
     unsigned long long* ctot = sm;              // [256]
     unsigned long long& s_excl = sm[256];       // rank of the first element of the chosen chunk
     unsigned long long& s_k = sm[257];
     unsigned long long& s_flags = sm[258];      // invalid | chunk << 1 | prefix << 32
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    // the request: the same values in every thread, in flight together with the bins
+    const bool fresh = (PASS == 0) && init.enabled;
+    unsigned long long k = fresh ? init.k : st->k;
+    uint32_t invalid = (PASS == 0) ? 0u : st->invalid;
+    const uint32_t prefix = (PASS == 0) ? 0u : st->prefix;
+    const bool med = (PASS == 0) && (fresh ? init.use_median != 0 : st->use_median != 0);
     auto bin = [&](uint32_t b) -> unsigned long long {   // PASS 0 bins are indexed by the raw top bits of the float
         return __ldcg(&gdigits[PASS == 0 ? raw_of_digit(b) : b]);
     };
-#pragma unroll 4
-    for (int ch = warp; ch < CHUNKS; ch += NW) {
-        const unsigned long long v = warp_sum_u64(bin((uint32_t)(ch * 32 + lane)));
-        if (lane == 0) ctot[ch] = v;
+    unsigned long long v[INFL];
+#pragma unroll 1
+    for (int c0 = 0; c0 < CPW; c0 += INFL) {
+#pragma unroll
+        for (int j = 0; j < INFL; ++j) {
+            const int ch = warp + (c0 + j) * NW;
+            v[j] = (c0 + j < CPW && ch < CHUNKS) ? bin((uint32_t)(ch * 32 + lane)) : 0ull;
+        }
+#pragma unroll
+        for (int j = 0; j < INFL; ++j) {
+            const int ch = warp + (c0 + j) * NW;
+            const unsigned long long t = warp_sum_u64(v[j]);
+            if (lane == 0 && c0 + j < CPW && ch < CHUNKS) ctot[ch] = t;
+        }
     }
     __syncthreads();
     if (warp == 0) {
@@ -261,23 +282,14 @@ __device__ __forceinline__ void select_scan_body(SelectState* __restrict__ st, u
         unsigned long long incl = mine;
 #pragma unroll
         for (int off = 1; off < 32; off <<= 1) {
-            unsigned long long v = __shfl_up_sync(0xffffffffu, incl, off);
-            if (lane >= off) incl += v;
+            unsigned long long u = __shfl_up_sync(0xffffffffu, incl, off);
+            if (lane >= off) incl += u;
         }
         const unsigned long long total = __shfl_sync(0xffffffffu, incl, 31);
-        // rank, validity and prefix: the same values in every lane
-        unsigned long long k;
-        uint32_t invalid, prefix;
         if (PASS == 0) {
-            const bool med = init.enabled ? init.use_median != 0 : st->use_median != 0;
-            k = init.enabled ? init.k : st->k;
             if (med) k = total ? (total - 1) / 2 : 0;
             invalid = (k >= total) ? 1u : 0u;
-            prefix = 0;
-        } else {
-            k = st->k; invalid = st->invalid; prefix = st->prefix;
         }
-        __syncwarp();
         if (lane == 0) {
             if (PASS == 0) {
                 st->count = total; st->invalid = invalid;
@@ -302,32 +314,46 @@ __device__ __forceinline__ void select_scan_body(SelectState* __restrict__ st, u
                 excl += c[j];
             }
         }
-        __syncwarp();
-        if (!invalid) {
-            const uint32_t ch = (uint32_t)((s_flags >> 1) & 0x7FFFFFFFu);
+    }
+    __syncthreads();   // the chosen chunk, its first rank and k are in shared memory; lane 0's record is written
+    {
+        const unsigned long long fl = s_flags;
+        const uint32_t ch = (uint32_t)((fl >> 1) & 0x7FFFFFFFu);
+        const bool bad = (fl & 1ull) != 0;
+        const int owner = KEEP ? (int)(ch % NW) : 0;
+        if (!bad && warp == owner) {
             const unsigned long long kk = s_k - s_excl;           // rank inside the chunk
-            const unsigned long long v = bin(ch * 32 + lane);
-            unsigned long long inc2 = v;
+            unsigned long long x = 0;
+            if (KEEP) {
+#pragma unroll
+                for (int j = 0; j < INFL; ++j)
+                    if ((int)(ch / NW) == j) x = v[j];
+            } else {
+                x = bin(ch * 32 + lane);
+            }
+            unsigned long long inc2 = x;
 #pragma unroll
             for (int off = 1; off < 32; off <<= 1) {
                 unsigned long long u = __shfl_up_sync(0xffffffffu, inc2, off);
                 if (lane >= off) inc2 += u;
             }
-            const unsigned long long ex2 = inc2 - v;
-            if (v && ex2 <= kk && kk < inc2) {                    // exactly one lane
+            const unsigned long long ex2 = inc2 - x;
+            if (x && ex2 <= kk && kk < inc2) {                    // exactly one lane
                 const uint32_t b = ch * 32 + lane;
-                const uint32_t pre = (PASS == 0) ? b : ((prefix << BITS) | b);
+                const uint32_t pfx = (uint32_t)(fl >> 32);
+                const uint32_t pre = (PASS == 0) ? b : ((pfx << BITS) | b);
                 st->prefix = pre;
                 st->k = kk - ex2;
                 if (PASS == 2) {
-                    st->result = __uint_as_float(bits_of_key(pre));
-                    if (init.result_out) *init.result_out = st->result;
+                    const float r = __uint_as_float(bits_of_key(pre));
+                    st->result = r;
+                    if (init.result_out) *init.result_out = r;
                 }
             }
         }
     }
     if (clear) {  // leave the digit bins zeroed for the next pass
-        __syncthreads();   // warp 0 has re-read its chunk
+        __syncthreads();   // the owner has read its chunk
         for (int i = tid; i < kDigitBins; i += THREADS) gdigits[i] = 0ull;
     }
 }
