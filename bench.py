@@ -512,8 +512,11 @@ def main():
     clocks = sampler.stop() if sampler else None
     streams_cube = {"moments", "moments_coarse", "histogram", "select_pass0", "select_pass1", "hist_select"}
     tot_k = sum(ms for ms, _ in prof.values()) or 1.0
+    # a launch that returns at once (an enqueued fallback whose turn did not come: DESIGN.md sec. 4) has read nothing:
+    # it gets no bandwidth figure (anything "faster" than twice the read probe cannot have streamed the cube)
     kernels = {k: {"launches": c, "avg_ms": ms / c, "share": ms / tot_k,
-                   "achieved_gbs": (ALGO_BYTES_PER_VOXEL * n / (ms / c * 1e-3) / 1e9) if k in streams_cube else None}
+                   "achieved_gbs": (ALGO_BYTES_PER_VOXEL * n / (ms / c * 1e-3) / 1e9)
+                   if k in streams_cube and ms / c > 0.5 * probe_ms else None}
                for k, (ms, c) in prof.items() if c}
     dom = max(kernels, key=lambda k: kernels[k]["share"])
     achieved = kernels[dom]["achieved_gbs"]

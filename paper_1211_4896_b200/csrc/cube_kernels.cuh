@@ -228,7 +228,7 @@ moments_kernel(const float* __restrict__ d, uint64_t n, Partial* __restrict__ pa
     __syncthreads();
     if (!is_last) return;
     // last CTA: fixed-order merge of the per-CTA partials.  A tree of Chan merges is a chain of ~13 dependent fp64
-    // divisions (5 us of tail on a cube that streams in 10 us: profiles/r1_v10_c2.md), so the partials are first
+    // divisions (5 us of tail on a cube that streams in 10 us: profiles/r1_v11_c2.md), so the partials are first
     // re-expressed as sums about ONE pivot P -- the mean of the lowest-indexed non-empty partial: s_i = n_i (mean_i -
     // P), q_i = M2_i + n_i (mean_i - P)^2 -- which merge by plain additions (thread i takes i, i+256, ...; then
     // shuffles).  P is the mean of a CTA whose tiles are spread over the whole cube, so |P - mean| << std and
