@@ -273,7 +273,7 @@ enum {
                                   2 = always the 16-bit packed counters */
     CUBE_KNOB_MINIMAP = 2      /* cube_minimap kernel: 0 = automatic (default): lines staged through a shared-memory
                                   ring by TMA bulk copies when the rows are 16-byte aligned, the cells at most 480
-                                  voxels wide and a cell row has at least 512 lines (or the 128-bit kernel is not
+                                  voxels wide and a cell row has at least 256 lines (or the 128-bit kernel is not
                                   eligible), else as 1; 1 = 128-bit register kernel when eligible (rows 16-byte
                                   aligned, px >= 4), else the scalar one; 2 = always the scalar kernel; 3 = the TMA
                                   ring whenever it is eligible, whatever the number of lines */

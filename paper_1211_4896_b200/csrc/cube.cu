@@ -637,12 +637,13 @@ int cube_minimap(cube_ctx* c, const float* d, int64_t nx, int64_t ny, int64_t nz
     const long long unit_t = seg128 ? unit128 : unit;
     const long long cpst = (kMapTmaCols / px) / unit_t * unit_t;
     const long long cps4 = (kMap4Cols / px) / unit * unit;
-    // A CTA of the ring kernel pays for filling and draining its ring once per cell row: it wins from about 512
-    // lines per cell row upwards (measured on c2: 30^3 cells 6.3 vs 4.4 TB/s, 16^3 cells 5.0 vs 5.8 TB/s).
+    // The ring kernel takes several cell rows per CTA, but every cell row still ends with two barriers and the per-cell
+    // merge: it wins from about 256 lines per cell row upwards (measured on c2, TB/s ring vs 128-bit kernel: 30^3 cells
+    // 6.36 vs 4.44, 64^3 6.10 vs 4.12, 16^3 5.76 vs 5.70, 24x8x8 4.09 vs 4.74, 100x10x10 3.29 vs 4.64).
     const bool v4_ok = rows16 && cps4 >= 1 && px >= 4;
     const long double lines = (long double)std::min(py, ny) * (long double)std::min(pz, nz);
     const bool tma = rows16 && cpst >= 1 && lines < 2147483000.0L &&
-                     (c->minimap_variant == 3 || (c->minimap_variant == 0 && (lines >= 512.0L || !v4_ok)));
+                     (c->minimap_variant == 3 || (c->minimap_variant == 0 && (lines >= 256.0L || !v4_ok)));
     const bool v4 = !tma && v4_ok && c->minimap_variant <= 1;
     g.cells_per_seg = tma ? cpst : v4 ? cps4 : (px > kMapThreads ? 1 : kMapThreads / px);
     g.nseg = (g.mx + g.cells_per_seg - 1) / g.cells_per_seg;
@@ -661,8 +662,11 @@ int cube_minimap(cube_ctx* c, const float* d, int64_t nx, int64_t ny, int64_t nz
         if (tma) {
             const long long wmax = std::min<long long>(g.cells_per_seg * px, nx);     // widest segment, a multiple of 4
             const unsigned block = (unsigned)((wmax + 31) / 32 * 32) + 32u;           // + the producer warp
-            minimap_tma_kernel<<<grid, block, kMapTmaSmem, s>>>(d, g, flags & CUBE_SAMPLE_STD,
-                                                                reinterpret_cast<MomentsOut*>(cells));
+            // cell rows per CTA: about 1024 lines, so that filling and draining the ring is a small part of a CTA
+            const long long rows = std::max<long long>(1, std::min<long long>(g.my, (long long)(1024.0L / lines)));
+            const long double ctas_t = (long double)g.nseg * (long double)((g.my + rows - 1) / rows) * (long double)g.mz;
+            minimap_tma_kernel<<<(unsigned)ctas_t, block, kMapTmaSmem, s>>>(d, g, flags & CUBE_SAMPLE_STD, (int)rows,
+                                                                            reinterpret_cast<MomentsOut*>(cells));
         } else if (v4) minimap_v4_kernel<<<grid, block4, 0, s>>>(d, g, flags & CUBE_SAMPLE_STD,
                                                                  reinterpret_cast<MomentsOut*>(cells));
         else minimap_kernel<<<grid, kMapThreads, 0, s>>>(d, g, flags & CUBE_SAMPLE_STD,

@@ -222,10 +222,14 @@ struct SelectInit {
 
 constexpr int kScanSmem = 256 + 4;   // words (u64) of shared memory select_scan_body needs
 
+// Sum of a 64-bit value over the warp, every lane gets it: three REDUX.SUM on 24-bit limbs (32 x 2^24 < 2^32, so no
+// limb sum wraps) instead of five 64-bit shuffle-and-add steps -- 3 instructions per chunk, not ~25; the bucket
+// location is ONE CTA's instruction and latency chain at the tail of every pass.
 __device__ __forceinline__ unsigned long long warp_sum_u64(unsigned long long v) {
-#pragma unroll
-    for (int off = 16; off > 0; off >>= 1) v += __shfl_xor_sync(0xffffffffu, v, off);
-    return v;
+    const uint32_t a = (uint32_t)v & 0xFFFFFFu, b = (uint32_t)(v >> 24) & 0xFFFFFFu, c = (uint32_t)(v >> 48);
+    return (unsigned long long)__reduce_add_sync(0xffffffffu, a) +
+           ((unsigned long long)__reduce_add_sync(0xffffffffu, b) << 24) +
+           ((unsigned long long)__reduce_add_sync(0xffffffffu, c) << 48);
 }
 
 // Two levels, every global load coalesced and independent of the others: (1) each warp sums chunks of 32 consecutive

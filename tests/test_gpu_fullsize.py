@@ -164,6 +164,9 @@ def test_config5_full_size():
     origins = cubegen.brick_grid(cfg, brick)
     assert len(origins) == 512 and n == 512 * bvox
     nb, lo, hi = 4096, -0.02, 0.5
+    import gc
+    gc.collect()
+    torch.cuda.empty_cache()          # the 64 / 32 GiB cubes of the tests before this one: libcube allocates with cudaMalloc
     scr = torch.empty(bvox, dtype=torch.float32, device="cuda")
     ctx = cube.Context(scratch_bytes_hint=1 << 30)
     try:
