@@ -246,43 +246,58 @@ moments_kernel(const float* __restrict__ d, uint64_t n, Partial* __restrict__ pa
     __syncthreads();
     Partial m = partial_empty();
     if (first_live != 0xFFFFFFFFu) {
-        const double P = __ldcg(&partials[first_live].mean);
-        unsigned long long cn = 0;
-        double cs = 0.0, cq = 0.0;
-        uint32_t kmin = 0xFFFFFFFFu, kmax = 0u;
-        for (unsigned i = threadIdx.x; i < gridDim.x; i += kThreads) {   // written by other CTAs: read through L2
-            const unsigned long long bn = __ldcg(&partials[i].n);
-            const double bmean = __ldcg(&partials[i].mean), bm2 = __ldcg(&partials[i].m2);
-            kmin = min(kmin, __ldcg(&partials[i].kmin));
-            kmax = max(kmax, __ldcg(&partials[i].kmax));
-            if (bn) {
-                const double nb = (double)bn, dm = bmean - P, nd = nb * dm;
-                cn += bn; cs += nd; cq += bm2 + nd * dm;
-            }
-        }
-#pragma unroll
-        for (int off = 16; off > 0; off >>= 1) {
-            cn += __shfl_down_sync(0xffffffffu, cn, off);
-            cs += __shfl_down_sync(0xffffffffu, cs, off);
-            cq += __shfl_down_sync(0xffffffffu, cq, off);
-            kmin = min(kmin, __shfl_down_sync(0xffffffffu, kmin, off));
-            kmax = max(kmax, __shfl_down_sync(0xffffffffu, kmax, off));
-        }
-        const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
-        __syncthreads();   // scratch is free (the CTA's own block reduce is over)
-        if (lane == 0) { scratch[warp].n = cn; scratch[warp].mean = cs; scratch[warp].m2 = cq; scratch[warp].kmin = kmin; scratch[warp].kmax = kmax; }
+        __shared__ double pivot_sm;
+        __shared__ int again_sm;
+        if (threadIdx.x == 0) { pivot_sm = __ldcg(&partials[first_live].mean); again_sm = 0; }
         __syncthreads();
-        if (threadIdx.x == 0) {
-            cn = 0; cs = 0.0; cq = 0.0; kmin = 0xFFFFFFFFu; kmax = 0u;
-#pragma unroll
-            for (int w = 0; w < kThreads / 32; ++w) {
-                cn += scratch[w].n; cs += scratch[w].mean; cq += scratch[w].m2;
-                kmin = min(kmin, scratch[w].kmin); kmax = max(kmax, scratch[w].kmax);
+        // Second round only if the pivot turned out to be far from the mean (more than 16 standard deviations: data
+        // arranged so that CTA first_live saw something else than the rest): q - s^2/n would then cancel ~2^8 or more
+        // of the 2^53; the refined pivot P + s/n is as good as the mean itself.
+#pragma unroll 1
+        for (int round = 0; round < 2; ++round) {
+            const double P = pivot_sm;
+            unsigned long long cn = 0;
+            double cs = 0.0, cq = 0.0;
+            uint32_t kmin = 0xFFFFFFFFu, kmax = 0u;
+            for (unsigned i = threadIdx.x; i < gridDim.x; i += kThreads) {   // written by other CTAs: read through L2
+                const unsigned long long bn = __ldcg(&partials[i].n);
+                const double bmean = __ldcg(&partials[i].mean), bm2 = __ldcg(&partials[i].m2);
+                kmin = min(kmin, __ldcg(&partials[i].kmin));
+                kmax = max(kmax, __ldcg(&partials[i].kmax));
+                if (bn) {
+                    const double nb = (double)bn, dm = bmean - P, nd = nb * dm;
+                    cn += bn; cs += nd; cq += bm2 + nd * dm;
+                }
             }
-            const double nn = (double)cn;
-            const double m2 = cq - cs * (cs / nn);
-            m.n = cn; m.mean = P + cs / nn; m.m2 = (m2 < 0.0) ? 0.0 : m2;   // rounding only; a NaN (Inf voxels) stays
-            m.kmin = kmin; m.kmax = kmax;
+#pragma unroll
+            for (int off = 16; off > 0; off >>= 1) {
+                cn += __shfl_down_sync(0xffffffffu, cn, off);
+                cs += __shfl_down_sync(0xffffffffu, cs, off);
+                cq += __shfl_down_sync(0xffffffffu, cq, off);
+                kmin = min(kmin, __shfl_down_sync(0xffffffffu, kmin, off));
+                kmax = max(kmax, __shfl_down_sync(0xffffffffu, kmax, off));
+            }
+            const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+            __syncthreads();   // scratch is free (the CTA's own block reduce / the round before is over)
+            if (lane == 0) { scratch[warp].n = cn; scratch[warp].mean = cs; scratch[warp].m2 = cq; scratch[warp].kmin = kmin; scratch[warp].kmax = kmax; }
+            __syncthreads();
+            if (threadIdx.x == 0) {
+                cn = 0; cs = 0.0; cq = 0.0; kmin = 0xFFFFFFFFu; kmax = 0u;
+#pragma unroll
+                for (int w = 0; w < kThreads / 32; ++w) {
+                    cn += scratch[w].n; cs += scratch[w].mean; cq += scratch[w].m2;
+                    kmin = min(kmin, scratch[w].kmin); kmax = max(kmax, scratch[w].kmax);
+                }
+                const double nn = (double)cn, shift = cs / nn;
+                const double m2 = cq - cs * shift;
+                m.n = cn; m.mean = P + shift; m.m2 = (m2 < 0.0) ? 0.0 : m2;   // rounding only; a NaN (Inf voxels) stays
+                m.kmin = kmin; m.kmax = kmax;
+                const bool far = round == 0 && shift * shift * nn > 256.0 * m.m2 && isfinite(m.mean);
+                again_sm = far ? 1 : 0;
+                if (far) pivot_sm = m.mean;
+            }
+            __syncthreads();
+            if (!again_sm) break;
         }
     }
     if (threadIdx.x == 0) {

@@ -70,21 +70,28 @@ __device__ __forceinline__ void lds_group(uint32_t base, float (&v)[kMapUnroll])
 __device__ __forceinline__ Partial map_merge_columns(const Partial* __restrict__ cols, int w) {
     Partial m = partial_empty();
     bool have = false;
-    double P = 0.0, cs = 0.0, cq = 0.0;
-    unsigned long long cn = 0;
-    for (int i = 0; i < w; ++i) {
-        const Partial c = cols[i];
-        m.kmin = min(m.kmin, c.kmin);
-        m.kmax = max(m.kmax, c.kmax);
-        if (c.n) {
-            if (!have) { have = true; P = c.mean; }
-            const double nb = (double)c.n, dm = c.mean - P, nd = nb * dm;
-            cn += c.n; cs += nd; cq += c.m2 + nd * dm;
+    double P = 0.0;
+    for (int i = 0; i < w && !have; ++i)
+        if (cols[i].n) { have = true; P = cols[i].mean; }
+    if (!have) return m;
+#pragma unroll 1
+    for (int round = 0; round < 2; ++round) {   // a second round only if the first column was far from the cell's mean
+        double cs = 0.0, cq = 0.0;
+        unsigned long long cn = 0;
+        m.kmin = 0xFFFFFFFFu; m.kmax = 0u;
+        for (int i = 0; i < w; ++i) {
+            const Partial c = cols[i];
+            m.kmin = min(m.kmin, c.kmin);
+            m.kmax = max(m.kmax, c.kmax);
+            if (c.n) {
+                const double nb = (double)c.n, dm = c.mean - P, nd = nb * dm;
+                cn += c.n; cs += nd; cq += c.m2 + nd * dm;
+            }
         }
-    }
-    if (have) {
-        const double nn = (double)cn, m2 = cq - cs * (cs / nn);
-        m.n = cn; m.mean = P + cs / nn; m.m2 = (m2 < 0.0) ? 0.0 : m2;   // rounding only; a NaN (Inf voxels) stays
+        const double nn = (double)cn, shift = cs / nn, m2 = cq - cs * shift;
+        m.n = cn; m.mean = P + shift; m.m2 = (m2 < 0.0) ? 0.0 : m2;   // rounding only; a NaN (Inf voxels) stays
+        if (!(shift * shift * nn > 256.0 * m.m2 && isfinite(m.mean))) break;   // else q - s^2/n cancelled: refine P
+        P = m.mean;
     }
     return m;
 }

@@ -265,6 +265,27 @@ def test_minimap_variants_agree_on_nan_free_and_nan_heavy_rows(ctx):
             ctx.set_knob(cube.KNOB_MINIMAP, 0)
 
 
+def test_minimap_merge_pivot_far_from_the_cell_mean(ctx):
+    # first column of a cell: blanked except one voxel of 1e6; the other columns 1e-3 noise -- the per-cell merge
+    # starts from a pivot hundreds of standard deviations away and has to refine it (every kernel variant)
+    nx, ny, nz = 64, 32, 32
+    r = np.random.default_rng(5)
+    a = (r.standard_normal(nx * ny * nz) * 1e-3).astype(np.float32).reshape(nz, ny, nx)
+    a[:, :, 0] = np.nan
+    a[3, 4, 0] = 1e6
+    a[:, :, 32] = np.nan
+    a[7, 1, 32] = -1e6
+    a = a.reshape(-1)
+    t = dev(a)
+    ref = oracle.minimap(a, (nx, ny, nz), (32, 32, 32))
+    for variant in (0, 1, 2, 3):
+        ctx.set_knob(cube.KNOB_MINIMAP, variant)
+        try:
+            check_minimap(run_minimap(ctx, t, (nx, ny, nz), (32, 32, 32)), ref)
+        finally:
+            ctx.set_knob(cube.KNOB_MINIMAP, 0)
+
+
 def test_minimap_scaled_config_and_global_consistency(ctx):
     t, a, dims = scaled_cube("c2", (160, 128, 96))
     nx, ny, nz = dims

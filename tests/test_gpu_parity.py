@@ -190,6 +190,27 @@ def test_degenerate_cubes(ctx):
             assert m["std"] == 0.0 and m["mean"] == float(fin[0])           # exactly
 
 
+def test_moments_merge_pivot_far_from_the_mean(ctx):
+    # The last CTA merges the per-CTA partials as sums about the mean of the first non-empty partial.  Here that
+    # partial is one voxel of 1e6 (the rest of CTA 0's first tile is blanked) in front of 2^24 voxels of 1e-3 noise:
+    # the pivot is ~4000 standard deviations from the mean, q - s^2/n would lose 7 digits, and the merge has to
+    # refine its pivot to stay within 1e-9 (moments numerics).
+    n = 1 << 24
+    r = np.random.default_rng(2024)
+    a = (r.standard_normal(n) * 1e-3).astype(np.float32)
+    a[:8192] = np.nan
+    a[5] = 1e6
+    t = dev(a)
+    ref = oracle.moments(a)
+    assert abs(1e6 - ref["mean"]) > 1000 * ref["std"]
+    for per in (0, 1, 4):
+        ctx.set_launch(per)
+        check_moments(ctx.moments(t, n, 1, 1), ref, a)
+        m = ctx.stats(t, n, 1, 1, 64, None, None)[0]
+        check_moments(m, ref, a)
+    ctx.set_launch(0)
+
+
 def test_ramp_closed_forms_direct(ctx):
     # independent of the oracle: north_star's closed forms
     N = 1 << 24
