@@ -42,8 +42,12 @@ struct MapColF : MomentsF<kMomPlain> {
     __device__ __forceinline__ void group(const float (&v)[kMapUnroll], bool& safe_mode) {
         if (safe_mode) {
             const uint32_t n0 = n;
+            if (!have) {   // only until this column has met its first voxel that takes part
 #pragma unroll
-            for (int k = 0; k < kMapUnroll; ++k) { take_pivot(v[k]); core(v[k]); }
+                for (int k = 0; k < kMapUnroll; ++k) take_pivot(v[k]);
+            }
+#pragma unroll
+            for (int k = 0; k < kMapUnroll; ++k) core(v[k]);
             safe_mode = __any_sync(__activemask(), n - n0 != (uint32_t)kMapUnroll);
             return;
         }
