@@ -235,27 +235,28 @@ moments_kernel(const float* __restrict__ d, uint64_t n, Partial* __restrict__ pa
     // q - s^2/n loses nothing; a constant cube gives mean_i == P, s = q = 0 and std = 0 exactly.
     __threadfence();
     __shared__ unsigned int first_live;
-    if (threadIdx.x == 0) first_live = 0xFFFFFFFFu;
-    __syncthreads();
-    {
+    __shared__ double pivot_sm;
+    __shared__ int again_sm;
+    unsigned int first = 0;   // block-uniform: partial 0 unless CTA 0 saw only NULL voxels (then the search below)
+    if (__ldcg(&partials[0].n) == 0) {
+        if (threadIdx.x == 0) first_live = 0xFFFFFFFFu;
+        __syncthreads();
         unsigned int mine = 0xFFFFFFFFu;
         for (unsigned i = threadIdx.x; i < gridDim.x; i += kThreads)
             if (mine == 0xFFFFFFFFu && __ldcg(&partials[i].n) != 0) mine = i;
         if (mine != 0xFFFFFFFFu) atomicMin(&first_live, mine);
-    }
-    __syncthreads();
-    Partial m = partial_empty();
-    if (first_live != 0xFFFFFFFFu) {
-        __shared__ double pivot_sm;
-        __shared__ int again_sm;
-        if (threadIdx.x == 0) { pivot_sm = __ldcg(&partials[first_live].mean); again_sm = 0; }
         __syncthreads();
+        first = first_live;
+    }
+    Partial m = partial_empty();
+    if (first != 0xFFFFFFFFu) {
+        if (threadIdx.x == 0) again_sm = 0;
+        double P = __ldcg(&partials[first].mean);
         // Second round only if the pivot turned out to be far from the mean (more than 16 standard deviations: data
         // arranged so that CTA first_live saw something else than the rest): q - s^2/n would then cancel ~2^8 or more
         // of the 2^53; the refined pivot P + s/n is as good as the mean itself.
 #pragma unroll 1
         for (int round = 0; round < 2; ++round) {
-            const double P = pivot_sm;
             unsigned long long cn = 0;
             double cs = 0.0, cq = 0.0;
             uint32_t kmin = 0xFFFFFFFFu, kmax = 0u;
@@ -298,6 +299,7 @@ moments_kernel(const float* __restrict__ d, uint64_t n, Partial* __restrict__ pa
             }
             __syncthreads();
             if (!again_sm) break;
+            P = pivot_sm;
         }
     }
     if (threadIdx.x == 0) {
