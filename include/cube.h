@@ -103,6 +103,15 @@ int cube_kth(cube_ctx* ctx, const float* d, int64_t nx, int64_t ny, int64_t nz, 
 int cube_kth_ex(cube_ctx* ctx, const float* d, int64_t nx, int64_t ny, int64_t nz, uint64_t k, unsigned flags,
                 float* out, cudaStream_t stream);
 
+/* Several ranks of the same cube (config 3 of BASELINE.json asks for the median and the values at n/100 and
+ * 99n/100): out[i] = the element of rank k[i], i < nk, each exactly what cube_kth gives.  The first select digit is
+ * counted ONCE and every rank then costs one read of the cube: 1 + nk reads instead of 2 nk.  `k` is a HOST array
+ * read before the call returns; `out` (nk floats) may be device, pinned or pageable host memory.  The first-digit
+ * histogram stays in the context as after CUBE_COARSE_HIST; with CUBE_REUSE_COARSE in `flags` the one already there
+ * is used (nk reads; the caller vouches that it belongs to this cube).  nk >= 1. */
+int cube_kth_multi(cube_ctx* ctx, const float* d, int64_t nx, int64_t ny, int64_t nz, int nk, const uint64_t* k,
+                   unsigned flags, float* out, cudaStream_t stream);
+
 /* Lower median: k = (count-1)/2 with count = number of non-NaN voxels (what Alg. 1, PAPER.md:603-609,
  * returns). count == 0 -> NaN. */
 int cube_median(cube_ctx* ctx, const float* d, int64_t nx, int64_t ny, int64_t nz, float* out,

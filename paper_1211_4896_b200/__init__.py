@@ -26,7 +26,7 @@ SAMPLE_STD, COARSE_HIST, REUSE_COARSE, RANGE_MINMAX = 1, 2, 4, 8
 MAX_BINS = 65536
 
 # every symbol include/cube.h declares (checked by tests/test_abi.py)
-SYMBOLS = ["cube_create", "cube_destroy", "cube_moments", "cube_histogram", "cube_kth", "cube_kth_ex",
+SYMBOLS = ["cube_create", "cube_destroy", "cube_moments", "cube_histogram", "cube_kth", "cube_kth_ex", "cube_kth_multi",
            "cube_median", "cube_median_ex", "cube_stats", "cube_probe_read", "cube_ooc_begin", "cube_ooc_brick", "cube_ooc_next_sweep",
            "cube_ooc_result", "cube_host_workspace", "cube_stats_host", "cube_stream_workspace", "cube_stats_stream",
            "cube_stream_info", "cube_strerror",
@@ -85,6 +85,7 @@ def load():
     L.cube_histogram.argtypes = [vp, vp, i64, i64, i64, ci, f32, f32, vp, vp, vp]
     L.cube_kth.argtypes = [vp, vp, i64, i64, i64, u64, vp, vp]
     L.cube_kth_ex.argtypes = [vp, vp, i64, i64, i64, u64, cu, vp, vp]
+    L.cube_kth_multi.argtypes = [vp, vp, i64, i64, i64, ci, vp, cu, vp, vp]
     L.cube_median.argtypes = [vp, vp, i64, i64, i64, vp, vp]
     L.cube_median_ex.argtypes = [vp, vp, i64, i64, i64, cu, vp, vp]
     L.cube_stats.argtypes = [vp, vp, i64, i64, i64, ci, f32, f32, cu, vp, vp, vp, vp, vp]
@@ -194,6 +195,19 @@ class Context:
         self._check(self._L.cube_kth_ex(self._h, _ptr(d), nx, ny, nz, k, flags,
                                         ctypes.cast(ctypes.byref(r), ctypes.c_void_p), stream))
         return np.float32(r.value)
+
+    def kth_multi(self, d, nx, ny, nz, ks, flags=0, out=None, stream=0):
+        """cube_kth_multi: the elements of ranks ``ks`` in 1 + len(ks) reads of the cube (len(ks) with REUSE_COARSE).
+        ``out``: device / pinned buffer of len(ks) floats, else the values come back as a float32 array."""
+        karr = np.ascontiguousarray(ks, dtype=np.uint64)
+        if out is not None:
+            self._check(self._L.cube_kth_multi(self._h, _ptr(d), nx, ny, nz, karr.size, karr.ctypes.data, flags,
+                                               _ptr(out), stream))
+            return None
+        r = np.full(karr.size, np.nan, dtype=np.float32)
+        self._check(self._L.cube_kth_multi(self._h, _ptr(d), nx, ny, nz, karr.size, karr.ctypes.data, flags,
+                                           r.ctypes.data, stream))
+        return r
 
     def median(self, d, nx, ny, nz, flags=0, out=None, stream=0):
         if out is not None:

@@ -449,6 +449,25 @@ int cube_kth(cube_ctx* c, const float* d, int64_t nx, int64_t ny, int64_t nz, ui
     return cube_kth_ex(c, d, nx, ny, nz, k, 0u, out, s);
 }
 
+int cube_kth_multi(cube_ctx* c, const float* d, int64_t nx, int64_t ny, int64_t nz, int nk, const uint64_t* k,
+                   unsigned flags, float* out, cudaStream_t s) {
+    uint64_t n;
+    int rc;
+    if (!c || !d || !out || !k || nk < 1 || !dims_ok(nx, ny, nz, &n)) return CUBE_EINVAL;
+    if (!(flags & CUBE_REUSE_COARSE)) {
+        // first digit of every voxel, once: the pass kernel without its bucket location leaves the counts in gdigits;
+        // they move to the slot CUBE_COARSE_HIST uses, where every rank's bucket location reads them
+        CUBE_CUDA(c, cudaMemsetAsync(c->gdigits, 0, kDigitBins * sizeof(unsigned long long), s));
+        if ((rc = launch_select_pass<0, false>(c, d, n, s, nullptr))) return rc;
+        CUBE_CUDA(c, cudaMemcpyAsync(c->coarse, c->gdigits, kDigitBins * sizeof(unsigned long long),
+                                     cudaMemcpyDeviceToDevice, s));
+        CUBE_CUDA(c, cudaMemsetAsync(c->gdigits, 0, kDigitBins * sizeof(unsigned long long), s));
+    }
+    for (int i = 0; i < nk; ++i)   // bucket location on the kept counts + passes 1 and 2: one read of the cube each
+        if ((rc = kth_impl<false>(c, d, n, k[i], 0, CUBE_REUSE_COARSE, out + i, s))) return rc;
+    return CUBE_OK;
+}
+
 int cube_median_ex(cube_ctx* c, const float* d, int64_t nx, int64_t ny, int64_t nz, unsigned flags, float* out,
                    cudaStream_t s) {
     uint64_t n;

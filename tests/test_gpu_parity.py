@@ -211,6 +211,41 @@ def test_moments_merge_pivot_far_from_the_mean(ctx):
     ctx.set_launch(0)
 
 
+def test_kth_multi_matches_single_selections(ctx):
+    # cube_kth_multi: several ranks after ONE first-digit pass -- config 3's request (median, n/100, 99n/100) and
+    # edge ranks, ties, a rank beyond the count (NaN), device output, reuse of the kept histogram
+    cfg = cubegen.scaled("c3", (64, 64, 300))
+    a = cubegen.generate_numpy(cfg).reshape(-1)
+    t = dev(a)
+    n = a.size
+    cnt = int(np.count_nonzero(a == a))
+    ks = [(cnt - 1) // 2, cnt // 100, 99 * cnt // 100, 0, cnt - 1, cnt, cnt + 5]
+    got = ctx.kth_multi(t, n, 1, 1, ks)
+    for k, g in zip(ks, got):
+        if k >= cnt:
+            assert math.isnan(float(g))
+        else:
+            assert same_float(g, oracle.kth(a, k)), (k, g)
+    assert same_float(got[0], oracle.median(a))
+    # the first-digit histogram stays in the context: more ranks of the same cube without the first pass
+    more = ctx.kth_multi(t, n, 1, 1, [cnt // 2, cnt // 3], flags=cube.REUSE_COARSE)
+    assert same_float(more[0], oracle.kth(a, cnt // 2)) and same_float(more[1], oracle.kth(a, cnt // 3))
+    out = torch.zeros(3, dtype=torch.float32, device="cuda")
+    ctx.kth_multi(t, n, 1, 1, ks[:3], out=out, stream=torch.cuda.current_stream().cuda_stream)
+    torch.cuda.synchronize()
+    assert (out.cpu().numpy().view(np.uint32) == got[:3].view(np.uint32)).all()
+    # heavy ties and signed zeros
+    b = np.array([0.0, -0.0, 1.0, 1.0, 1.0, -2.5, np.nan, 7.0] * 500, dtype=np.float32)
+    tb = dev(b)
+    nb = int(np.count_nonzero(b == b))
+    kb = list(range(0, nb, 377)) + [nb - 1]
+    gb = ctx.kth_multi(tb, b.size, 1, 1, kb)
+    for k, g in zip(kb, gb):
+        assert same_float(g, oracle.kth(b, k)), (k, g)
+    with pytest.raises(cube.CubeError):
+        ctx.kth_multi(t, n, 1, 1, [])
+
+
 def test_ramp_closed_forms_direct(ctx):
     # independent of the oracle: north_star's closed forms
     N = 1 << 24
