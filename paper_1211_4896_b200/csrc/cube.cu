@@ -5,12 +5,14 @@
 
 #include <math.h>
 #include <new>
+#include <stddef.h>
 #include <string.h>
 #include <algorithm>
 #include <vector>
 
 #include "cube_kernels.cuh"
 #include "cube_minimap_tma.cuh"
+#include "cube_select_multi.cuh"
 
 using namespace cube;
 
@@ -34,6 +36,7 @@ struct cube_ctx {
     unsigned long long* gdigits = nullptr; // kDigitBins
     unsigned long long* coarse = nullptr;  // kDigitBins: digit histogram kept by CUBE_COARSE_HIST
     SelectState* sel = nullptr;
+    MultiState* multi = nullptr;           // cube_kth_multi: the ranks of one group (cube_select_multi.cuh)
     float* range3 = nullptr;               // (lo, hi, scale) resolved on the device by cube_stats
     float* probe_out = nullptr;            // cube_probe_read sink
     BigHistPlan* plan = nullptr;           // hist_window_kernel's plan for the > 16384-bin histogram kernels
@@ -301,7 +304,7 @@ int select_init(cube_ctx* c, uint64_t k, int use_median, cudaStream_t s) {
 // DEV: rank |fl32(x - *c->center)| instead of x (cube_mad)
 template <bool DEV = false>
 int kth_impl(cube_ctx* c, const float* d, uint64_t n, uint64_t k, int use_median, unsigned flags, float* out,
-             cudaStream_t s) {
+             cudaStream_t s, const uint32_t* skip_if_set = nullptr) {
     int rc;
     // three launches: every pass kernel ends with the bucket location in its last CTA; the select state is
     // initialised by the first of them from kernel arguments (no host-to-device copy)
@@ -313,8 +316,9 @@ int kth_impl(cube_ctx* c, const float* d, uint64_t n, uint64_t k, int use_median
         CUBE_CUDA(c, cudaMemsetAsync(c->gdigits, 0, kDigitBins * sizeof(unsigned long long), s));
         if ((rc = launch_select_pass<0, DEV>(c, d, n, s, &init))) return rc;
     }
-    if ((rc = launch_select_pass<1, DEV>(c, d, n, s, &cont))) return rc;
-    if ((rc = launch_select_pass<2, DEV>(c, d, n, s, &cont))) return rc;
+    // skip_if_set (cube_kth_multi's fallback): both reads return at once when the word is set on the device
+    if ((rc = launch_select_pass<1, DEV>(c, d, n, s, &cont, skip_if_set))) return rc;
+    if ((rc = launch_select_pass<2, DEV>(c, d, n, s, &cont, skip_if_set))) return rc;
     if (out && !direct) CUBE_CUDA(c, cudaMemcpyAsync(out, &c->sel->result, sizeof(float), cudaMemcpyDefault, s));
     return CUBE_OK;
 }
@@ -353,6 +357,7 @@ int cube_create(cube_ctx** out, size_t scratch_bytes_hint) {
     ok = ok && cudaMalloc(&c->gdigits, kDigitBins * sizeof(unsigned long long)) == cudaSuccess;
     ok = ok && cudaMalloc(&c->coarse, kDigitBins * sizeof(unsigned long long)) == cudaSuccess;
     ok = ok && cudaMalloc(&c->sel, sizeof(SelectState)) == cudaSuccess;
+    ok = ok && cudaMalloc(&c->multi, sizeof(MultiState)) == cudaSuccess;
     ok = ok && cudaMalloc(&c->range3, 4 * sizeof(float)) == cudaSuccess;
     ok = ok && cudaMalloc(&c->probe_out, sizeof(float)) == cudaSuccess;
     ok = ok && cudaMalloc(&c->plan, sizeof(BigHistPlan)) == cudaSuccess;
@@ -389,7 +394,7 @@ int cube_create(cube_ctx** out, size_t scratch_bytes_hint) {
 int cube_destroy(cube_ctx* c) {
     if (!c) return CUBE_EINVAL;
     cudaFree(c->partials); cudaFree(c->ticket); cudaFree(c->ticket2); cudaFree(c->acc);
-    cudaFree(c->mom_out); cudaFree(c->gout); cudaFree(c->gdigits); cudaFree(c->coarse); cudaFree(c->sel);
+    cudaFree(c->mom_out); cudaFree(c->gout); cudaFree(c->gdigits); cudaFree(c->coarse); cudaFree(c->sel); cudaFree(c->multi);
     cudaFree(c->range3); cudaFree(c->probe_out); cudaFree(c->plan); cudaFree(c->clip); cudaFree(c->torben); cudaFree(c->center);
     cudaFree(c->cand);
     cudaFree(c->resident); cudaFree(c->chunk[0]); cudaFree(c->chunk[1]);
@@ -463,8 +468,39 @@ int cube_kth_multi(cube_ctx* c, const float* d, int64_t nx, int64_t ny, int64_t 
                                      cudaMemcpyDeviceToDevice, s));
         CUBE_CUDA(c, cudaMemsetAsync(c->gdigits, 0, kDigitBins * sizeof(unsigned long long), s));
     }
-    for (int i = 0; i < nk; ++i)   // bucket location on the kept counts + passes 1 and 2: one read of the cube each
-        if ((rc = kth_impl<false>(c, d, n, k[i], 0, CUBE_REUSE_COARSE, out + i, s))) return rc;
+    // groups of kMultiGroup ranks: ONE more read of the cube gathers the voxels of all their first-digit buckets, the
+    // other two digits are counted on the candidates (cube_select_multi.cuh).  The per-rank selections enqueued
+    // behind (one read each) skip themselves on the device unless the buckets did not fit the candidate buffer.
+    const uint32_t* ok_word = reinterpret_cast<const uint32_t*>(reinterpret_cast<const char*>(c->multi) +
+                                                                 offsetof(MultiState, ok));
+    const int occ = occupancy_of(c, multi_gather_kernel, kThreads, 0);
+    const int grid = grid_for(c, 4, occ < kMaxCtasPerSm ? occ : kMaxCtasPerSm);
+    for (int g0 = 0; g0 < nk; g0 += kMultiGroup) {
+        const int m = nk - g0 < kMultiGroup ? nk - g0 : kMultiGroup;
+        MultiRanks req;
+        memset(&req, 0, sizeof(req));
+        req.nk = (uint32_t)m;
+        for (int i = 0; i < m; ++i) req.k[i] = k[g0 + i];
+        multi_locate_kernel<<<1, 1024, 0, s>>>(c->multi, c->coarse, req, c->cand ? c->cand_cap : 0);
+        {
+            ProfScope prof(c, CUBE_K_SELECT_PASS1, s);
+            multi_gather_kernel<<<grid, kThreads, 0, s>>>(d, n, c->multi, c->cand);
+        }
+        const dim3 cgrid((unsigned)(2 * c->num_sms), (unsigned)m);
+        multi_cand_kernel<1><<<cgrid, kThreads, 0, s>>>(c->multi, c->gdigits, c->cand);
+        multi_scan_kernel<1><<<m, kBins1, 0, s>>>(c->multi, c->gdigits);
+        multi_cand_kernel<2><<<cgrid, kThreads, 0, s>>>(c->multi, c->gdigits, c->cand);
+        multi_scan_kernel<2><<<m, kBins1, 0, s>>>(c->multi, c->gdigits);
+        multi_done_kernel<<<1, 1, 0, s>>>(c->multi);
+        CUBE_CUDA(c, cudaGetLastError());
+        for (int i = 0; i < m; ++i) {
+            if ((rc = kth_impl<false>(c, d, n, k[g0 + i], 0, CUBE_REUSE_COARSE, nullptr, s, ok_word))) return rc;
+            multi_pick_kernel<<<1, 1, 0, s>>>(c->multi, i, c->sel);
+        }
+        CUBE_CUDA(c, cudaGetLastError());
+        CUBE_CUDA(c, cudaMemcpyAsync(out + g0, reinterpret_cast<const char*>(c->multi) + offsetof(MultiState, result),
+                                     (size_t)m * sizeof(float), cudaMemcpyDefault, s));
+    }
     return CUBE_OK;
 }
 

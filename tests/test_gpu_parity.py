@@ -246,6 +246,50 @@ def test_kth_multi_matches_single_selections(ctx):
         ctx.kth_multi(t, n, 1, 1, [])
 
 
+def test_kth_multi_two_reads_edges_and_fallback(ctx):
+    # cube_kth_multi gathers the first-digit buckets of up to four ranks in ONE read (cube_select_multi.cuh):
+    # +-Inf share their first-digit bucket with NaNs, duplicated ranks, ranks of one bucket, a misaligned
+    # ragged cube, only invalid ranks -- and the per-rank selections that take over on the device when the
+    # buckets do not fit the candidate buffer (a context with a 4 KiB buffer, and a constant cube)
+    rng = np.random.default_rng(77)
+    a = rng.standard_normal(200003).astype(np.float32)
+    a[::97] = np.nan
+    a[5::1013] = np.inf
+    a[7::2027] = -np.inf
+    a[11::31] = 0.25          # a heavy tie
+    cnt = int(np.count_nonzero(a == a))
+    ks = [0, 3, cnt // 2, cnt // 2, cnt // 2 + 1, cnt - 1, cnt - 2, cnt // 7, 5 * cnt // 7, cnt + 1]
+    ref = [oracle.kth(a, k) if k < cnt else np.float32(np.nan) for k in ks]
+    small = cube.Context(scratch_bytes_hint=4096)
+    try:
+        for mis in (0, 1, 3):
+            t = dev(a, misalign=mis)
+            for c in (ctx, small):
+                got = c.kth_multi(t, a.size, 1, 1, ks)
+                for k, g, r in zip(ks, got, ref):
+                    assert same_float(g, r), (mis, c is small, k, g, r)
+        t = dev(a)
+        for c in (ctx, small):
+            bad = c.kth_multi(t, a.size, 1, 1, [cnt, cnt + 9, 1 << 60])
+            assert all(math.isnan(float(g)) for g in bad)
+            one = c.kth_multi(t, a.size, 1, 1, [cnt // 3])
+            assert same_float(one[0], oracle.kth(a, cnt // 3))
+        # every voxel is a candidate: overflow of the small buffer on a constant cube, exact fit questions aside
+        cst = np.full(70001, -3.5, dtype=np.float32)
+        tc = dev(cst)
+        for c in (ctx, small):
+            g = c.kth_multi(tc, cst.size, 1, 1, [0, 35000, 70000, 70001, 12])
+            assert [bits(x) for x in g[:3]] == [bits(-3.5)] * 3 and math.isnan(float(g[3])) and bits(g[4]) == bits(-3.5)
+        # all NaN
+        tn = dev(np.full(5000, np.nan, dtype=np.float32))
+        assert all(math.isnan(float(x)) for x in ctx.kth_multi(tn, 5000, 1, 1, [0, 1, 2]))
+        # the digit bins are left clean: a plain selection afterwards is still right
+        assert same_float(ctx.kth(t, a.size, 1, 1, cnt // 5), oracle.kth(a, cnt // 5))
+        assert same_float(small.median(t, a.size, 1, 1), oracle.median(a))
+    finally:
+        small.close()
+
+
 def test_ramp_closed_forms_direct(ctx):
     # independent of the oracle: north_star's closed forms
     N = 1 << 24
