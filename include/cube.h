@@ -104,11 +104,16 @@ int cube_kth_ex(cube_ctx* ctx, const float* d, int64_t nx, int64_t ny, int64_t n
                 float* out, cudaStream_t stream);
 
 /* Several ranks of the same cube (config 3 of BASELINE.json asks for the median and the values at n/100 and
- * 99n/100): out[i] = the element of rank k[i], i < nk, each exactly what cube_kth gives.  The first select digit is
- * counted ONCE and every rank then costs one read of the cube: 1 + nk reads instead of 2 nk.  `k` is a HOST array
- * read before the call returns; `out` (nk floats) may be device, pinned or pageable host memory.  The first-digit
- * histogram stays in the context as after CUBE_COARSE_HIST; with CUBE_REUSE_COARSE in `flags` the one already there
- * is used (nk reads; the caller vouches that it belongs to this cube).  nk >= 1. */
+ * 99n/100): out[i] = the element of rank k[i], i < nk, each exactly what cube_kth gives (NaN for k[i] >= count).
+ * The first select digit is counted ONCE (read 1); then, per group of up to four ranks, ONE more read gathers the
+ * keys of the voxels of all their first-digit buckets into the context's candidate buffer and the other two digits
+ * are counted there: 1 + ceil(nk/4) reads instead of 2 nk.  If a group's buckets do not fit the candidate buffer
+ * (cube_create's scratch_bytes_hint; decided on the device, no host synchronisation) each of its ranks costs one
+ * more read.  `k` is a HOST array read before the call returns; `out` (nk floats) may be device, pinned or pageable
+ * host memory.  The first-digit histogram stays in the context as after CUBE_COARSE_HIST; with CUBE_REUSE_COARSE in
+ * `flags` the one already there is used (read 1 is skipped; the caller vouches that it belongs to this cube).
+ * nk >= 1.  Like every selection here it replaces the ~31 passes of Alg. 1; the cube is
+ * never written. */
 int cube_kth_multi(cube_ctx* ctx, const float* d, int64_t nx, int64_t ny, int64_t nz, int nk, const uint64_t* k,
                    unsigned flags, float* out, cudaStream_t stream);
 

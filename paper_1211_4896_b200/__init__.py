@@ -197,7 +197,8 @@ class Context:
         return np.float32(r.value)
 
     def kth_multi(self, d, nx, ny, nz, ks, flags=0, out=None, stream=0):
-        """cube_kth_multi: the elements of ranks ``ks`` in 1 + len(ks) reads of the cube (len(ks) with REUSE_COARSE).
+        """cube_kth_multi: the elements of ranks ``ks`` in 1 + ceil(len(ks)/4) reads of the cube (one less with
+        REUSE_COARSE; one more per rank of a group whose buckets do not fit the candidate buffer).
         ``out``: device / pinned buffer of len(ks) floats, else the values come back as a float32 array."""
         karr = np.ascontiguousarray(ks, dtype=np.uint64)
         if out is not None:

@@ -24,7 +24,8 @@ struct MultiState {
     unsigned long long count;                // non-NaN voxels
     unsigned long long cand_n, cand_cap;     // keys gathered / capacity of the candidate buffer
     uint32_t prefix[kMultiGroup];            // key bits fixed so far (right aligned)
-    uint32_t rawbase[kMultiGroup];           // raw_of_digit(first digit) << kShift0 (duplicates pad the group)
+    uint32_t rawbase[kMultiGroup];           // raw_of_digit(first digit) << kShift0 of the nb DISTINCT buckets
+    uint32_t nb;                             // distinct first-digit buckets of the valid ranks (0: idle)
     uint32_t invalid[kMultiGroup];           // 1: k >= count, result NaN
     uint32_t nk;
     uint32_t ok;                             // 1: every result of this group was found on the candidates
@@ -41,6 +42,7 @@ multi_locate_kernel(MultiState* __restrict__ ms, const unsigned long long* __res
                     unsigned long long cand_cap) {
     constexpr int PER = kBins0 / 1024;
     static_assert(kBins0 % 1024 == 0, "first digit bins per thread");
+    static_assert(kMultiGroup == 4, "multi_gather_kernel dispatches on 1...4 distinct buckets");
     __shared__ unsigned long long wtot[32];
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     unsigned long long v[PER], mine = 0;
@@ -57,54 +59,60 @@ multi_locate_kernel(MultiState* __restrict__ ms, const unsigned long long* __res
     unsigned long long before = 0, total = 0;
     for (int w = 0; w < 32; ++w) { const unsigned long long t = wtot[w]; if (w < warp) before += t; total += t; }
     unsigned long long excl = before + incl - mine;
-    if (tid == 0) {
-        ms->count = total; ms->cand_n = 0; ms->cand_cap = cand_cap; ms->nk = req.nk; ms->ok = 0; ms->idle = 0;
-        for (int i = 0; i < kMultiGroup; ++i) {
-            ms->invalid[i] = (i < (int)req.nk && req.k[i] < total) ? 0u : 1u;
-            ms->result[i] = __int_as_float(0x7fc00000);
-            ms->k[i] = 0; ms->prefix[i] = 0;
-        }
-    }
-    __syncthreads();
+    // owners leave (bucket, residual rank) in shared memory; thread 0 then writes the whole record once (no global
+    // read-backs in this one-CTA latency chain)
+    __shared__ uint32_t s_b[kMultiGroup];
+    __shared__ unsigned long long s_k[kMultiGroup];
 #pragma unroll
     for (int j = 0; j < PER; ++j) {
         for (int i = 0; i < (int)req.nk; ++i) {
             const unsigned long long k = req.k[i];
             if (v[j] && excl <= k && k < excl + v[j]) {          // exactly one (thread, j) per valid rank
-                const uint32_t b = (uint32_t)(tid * PER + j);
-                ms->prefix[i] = b; ms->k[i] = k - excl;
-                ms->rawbase[i] = raw_of_digit(b) << kShift0;
+                s_b[i] = (uint32_t)(tid * PER + j);
+                s_k[i] = k - excl;
             }
         }
         excl += v[j];
     }
     __syncthreads();
-    if (tid == 0) {   // pad: invalid and unused slots repeat a valid bucket (the gather tests all kMultiGroup)
-        __threadfence_block();
-        uint32_t any = 0xFFFFFFFFu;
-        bool have = false;
-        for (int i = 0; i < (int)req.nk; ++i)
-            if (!ms->invalid[i]) { any = ms->rawbase[i]; have = true; break; }
-        if (!have) { ms->idle = 1; any = 0; }   // the gather returns at once; every result is NaN already
-        for (int i = 0; i < kMultiGroup; ++i)
-            if (i >= (int)req.nk || ms->invalid[i]) ms->rawbase[i] = any;
+    if (tid == 0) {
+        uint32_t ub[kMultiGroup], nb = 0;   // the distinct buckets of the valid ranks (the gather tests exactly nb)
+        for (int i = 0; i < kMultiGroup; ++i) {
+            const bool valid = i < (int)req.nk && req.k[i] < total;
+            ms->invalid[i] = valid ? 0u : 1u;
+            ms->result[i] = __int_as_float(0x7fc00000);
+            ms->k[i] = valid ? s_k[i] : 0ull;
+            ms->prefix[i] = valid ? s_b[i] : 0u;
+            if (!valid) continue;
+            const uint32_t b = raw_of_digit(s_b[i]) << kShift0;
+            bool seen = false;
+            for (uint32_t j = 0; j < nb; ++j) seen = seen || ub[j] == b;
+            if (!seen) ub[nb++] = b;
+        }
+        for (uint32_t j = 0; j < (uint32_t)kMultiGroup; ++j) ms->rawbase[j] = j < nb ? ub[j] : 0u;
+        ms->count = total; ms->cand_n = 0; ms->cand_cap = cand_cap; ms->nk = req.nk; ms->ok = 0;
+        ms->nb = nb;
+        ms->idle = nb == 0 ? 1u : 0u;   // no rank below count: the gather returns at once, every result is NaN
     }
 }
 
 // Read 2: append the key of every non-NaN voxel whose first digit is one of the group's buckets.
-// Hot path per voxel: kMultiGroup LOP3 (bits ^ rawbase < 2^19 <=> the raw top bits match) + minima; one test per
-// thread per tile; the flagged rows are revisited from the registers.  Staging per warp as in SelectF (PASS 1).
+// Hot path per voxel: NB IMAD (bits - rawbase < 2^19 <=> the raw top bits match) + minima (NB = the number of
+// DISTINCT buckets, 1...kMultiGroup: compiled for each); one test per thread per tile; the flagged rows are
+// revisited from the registers.  Staging per warp as in SelectF (PASS 1).
+template <int NB>
 struct GatherF {
     static constexpr uint32_t kSpan = 1u << kShift0;
-    uint32_t rb[kMultiGroup];
+    uint32_t rb[NB];
     uint32_t* s_cnt; uint32_t* s_buf;
     uint32_t* cand; unsigned long long* cand_n; unsigned long long cand_cap;
     bool compacting;
+    // bits - rawbase < 2^19 (mod 2^32) <=> the raw top bits match; the subtraction is issued as IMAD on the FMA pipe
+    // (multiplier 1 from constant memory, as in SelectF), so only the minima use the ALU pipe; rb[] holds -rawbase
     __device__ __forceinline__ uint32_t dist(float x) const {
-        const uint32_t u = __float_as_uint(x);
-        uint32_t m = u ^ rb[0];
+        uint32_t m = SelectF<1, false>::sub_fma(x, rb[0]);
 #pragma unroll
-        for (int i = 1; i < kMultiGroup; ++i) m = min(m, u ^ rb[i]);
+        for (int i = 1; i < NB; ++i) m = min(m, SelectF<1, false>::sub_fma(x, rb[i]));
         return m;
     }
     __device__ __forceinline__ void take(float x) {
@@ -151,6 +159,21 @@ struct GatherF {
     }
 };
 
+template <int NB>
+__device__ __forceinline__ void gather_run(const float* __restrict__ d, uint64_t n, MultiState* __restrict__ ms,
+                                           uint32_t* __restrict__ cand, unsigned long long cap, uint32_t* s_buf,
+                                           uint32_t* s_cnt) {
+    GatherF<NB> f;
+#pragma unroll
+    for (int i = 0; i < NB; ++i) f.rb[i] = 0u - ms->rawbase[i];
+    f.s_buf = s_buf; f.s_cnt = s_cnt;
+    f.cand = cand; f.cand_n = &ms->cand_n; f.cand_cap = cap; f.compacting = true;
+    stream_cube<kThreads>(d, n, f);
+    __syncwarp();
+    const uint32_t c = *reinterpret_cast<volatile uint32_t*>(s_cnt);
+    if (c) f.flush(c);
+}
+
 __global__ void __launch_bounds__(kThreads, 3)
 multi_gather_kernel(const float* __restrict__ d, uint64_t n, MultiState* __restrict__ ms, uint32_t* __restrict__ cand) {
     __shared__ uint32_t stage[(kThreads / 32) * (kStageCap + 1)];
@@ -160,19 +183,17 @@ multi_gather_kernel(const float* __restrict__ d, uint64_t n, MultiState* __restr
         if (blockIdx.x == 0 && threadIdx.x == 0) ms->cand_n = ~0ull;
         return;
     }
-    GatherF f;
-#pragma unroll
-    for (int i = 0; i < kMultiGroup; ++i) f.rb[i] = ms->rawbase[i];
     const uint32_t warp = threadIdx.x >> 5;
-    f.s_buf = stage + warp * kStageCap;
-    f.s_cnt = stage + (kThreads / 32) * kStageCap + warp;
-    if ((threadIdx.x & 31) == 0) *f.s_cnt = 0;
+    uint32_t* s_buf = stage + warp * kStageCap;
+    uint32_t* s_cnt = stage + (kThreads / 32) * kStageCap + warp;
+    if ((threadIdx.x & 31) == 0) *s_cnt = 0;
     __syncwarp();
-    f.cand = cand; f.cand_n = &ms->cand_n; f.cand_cap = cap; f.compacting = true;
-    stream_cube<kThreads>(d, n, f);
-    __syncwarp();
-    const uint32_t c = *reinterpret_cast<volatile uint32_t*>(f.s_cnt);
-    if (c) f.flush(c);
+    switch (ms->nb) {   // uniform over the grid
+        case 1: gather_run<1>(d, n, ms, cand, cap, s_buf, s_cnt); break;
+        case 2: gather_run<2>(d, n, ms, cand, cap, s_buf, s_cnt); break;
+        case 3: gather_run<3>(d, n, ms, cand, cap, s_buf, s_cnt); break;
+        default: gather_run<kMultiGroup>(d, n, ms, cand, cap, s_buf, s_cnt); break;
+    }
 }
 
 // Digit counts of one rank (blockIdx.y) over the candidates: PASS 1 = second digit of the keys of its first-digit
@@ -183,17 +204,17 @@ multi_cand_kernel(const MultiState* __restrict__ ms, unsigned long long* __restr
                   const uint32_t* __restrict__ cand) {
     constexpr int NB = (PASS == 1) ? kBins1 : kBins2;
     static_assert(kMultiGroup * kBins1 <= kDigitBins && kBins2 <= kBins1, "per-rank digit slots");
-    __shared__ uint32_t sbins[NB + 1];
+    __shared__ uint32_t sbins[NB];
     const int r = blockIdx.y;
     const unsigned long long m = ms->cand_n;
     if (ms->invalid[r] || m > ms->cand_cap) return;
-    for (int i = threadIdx.x; i <= NB; i += kThreads) sbins[i] = 0;
+    for (int i = threadIdx.x; i < NB; i += kThreads) sbins[i] = 0;
     __syncthreads();
     const uint32_t base = (PASS == 1) ? (ms->prefix[r] << kShift0) : (ms->prefix[r] << kBits2);
     for (uint64_t i = (uint64_t)blockIdx.x * kThreads + threadIdx.x; i < m; i += (uint64_t)gridDim.x * kThreads) {
         const uint32_t t = __ldg(cand + i) - base;
         const uint32_t idx = (PASS == 1) ? (t >> kBits2) : t;    // outside the bucket: >= NB
-        atomicAdd(&sbins[min(idx, (uint32_t)NB)], 1u);
+        if (idx < (uint32_t)NB) atomicAdd(&sbins[idx], 1u);      // (no trash counter: it would be ONE hot address)
     }
     __syncthreads();
     unsigned long long* g = gdigits + (size_t)r * kBins1;
