@@ -486,7 +486,7 @@ int cube_kth_multi(cube_ctx* c, const float* d, int64_t nx, int64_t ny, int64_t 
             ProfScope prof(c, CUBE_K_SELECT_PASS1, s);
             multi_gather_kernel<<<grid, kThreads, 0, s>>>(d, n, c->multi, c->cand);
         }
-        const dim3 cgrid((unsigned)(2 * c->num_sms), (unsigned)m);
+        const int cgrid = 4 * c->num_sms;
         multi_cand_kernel<1><<<cgrid, kThreads, 0, s>>>(c->multi, c->gdigits, c->cand);
         multi_scan_kernel<1><<<m, kBins1, 0, s>>>(c->multi, c->gdigits);
         multi_cand_kernel<2><<<cgrid, kThreads, 0, s>>>(c->multi, c->gdigits, c->cand);

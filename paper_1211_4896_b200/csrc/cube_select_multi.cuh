@@ -7,8 +7,7 @@
 //           multi_locate_kernel: the first-digit bucket and the residual rank of EVERY requested rank;
 //   read 2  multi_gather_kernel: the keys of the voxels of ANY of those buckets go to the candidate buffer;
 //   then, on the candidates only (a few per cent of the cube): per rank the second digit (multi_cand_kernel<1>,
-//   multi_scan_kernel<1>) and the third (multi_cand_kernel<2>, multi_scan_kernel<2>), all ranks in one launch
-//   (blockIdx.y = rank).
+//   multi_scan_kernel<1>) and the third (multi_cand_kernel<2>, multi_scan_kernel<2>), all ranks in one launch.
 // If the buckets together do not fit the candidate buffer, MultiState::ok stays 0 and the caller's per-rank
 // selections (enqueued behind, skipped when ok == 1) give the results: the decision never leaves the device.
 // The cube is never written.
@@ -196,31 +195,55 @@ multi_gather_kernel(const float* __restrict__ d, uint64_t n, MultiState* __restr
     }
 }
 
-// Digit counts of one rank (blockIdx.y) over the candidates: PASS 1 = second digit of the keys of its first-digit
-// bucket, PASS 2 = third digit of the keys of its (first, second) prefix.  Counts go to gdigits[rank * kBins1 ...].
+// Digit counts of every rank of the group over the candidates, ONE read of the buffer (two 128-bit loads in flight
+// per thread): PASS 1 = second digit of the keys of a rank's first-digit bucket, PASS 2 = third digit of the keys of
+// its (first, second) prefix.  Counts go to gdigits[rank * kBins1 ...].  A key outside a rank's bucket touches no
+// counter (a trash counter would be one hot address).
 template <int PASS>
 __global__ void __launch_bounds__(kThreads)
 multi_cand_kernel(const MultiState* __restrict__ ms, unsigned long long* __restrict__ gdigits,
                   const uint32_t* __restrict__ cand) {
     constexpr int NB = (PASS == 1) ? kBins1 : kBins2;
     static_assert(kMultiGroup * kBins1 <= kDigitBins && kBins2 <= kBins1, "per-rank digit slots");
-    __shared__ uint32_t sbins[NB];
-    const int r = blockIdx.y;
+    __shared__ uint32_t sbins[kMultiGroup][NB];
     const unsigned long long m = ms->cand_n;
-    if (ms->invalid[r] || m > ms->cand_cap) return;
-    for (int i = threadIdx.x; i < NB; i += kThreads) sbins[i] = 0;
-    __syncthreads();
-    const uint32_t base = (PASS == 1) ? (ms->prefix[r] << kShift0) : (ms->prefix[r] << kBits2);
-    for (uint64_t i = (uint64_t)blockIdx.x * kThreads + threadIdx.x; i < m; i += (uint64_t)gridDim.x * kThreads) {
-        const uint32_t t = __ldg(cand + i) - base;
-        const uint32_t idx = (PASS == 1) ? (t >> kBits2) : t;    // outside the bucket: >= NB
-        if (idx < (uint32_t)NB) atomicAdd(&sbins[idx], 1u);      // (no trash counter: it would be ONE hot address)
+    if (m > ms->cand_cap) return;
+    uint32_t base[kMultiGroup];
+    bool live[kMultiGroup];
+#pragma unroll
+    for (int r = 0; r < kMultiGroup; ++r) {
+        live[r] = r < (int)ms->nk && !ms->invalid[r];
+        base[r] = (PASS == 1) ? (ms->prefix[r] << kShift0) : (ms->prefix[r] << kBits2);
     }
+    for (int i = threadIdx.x; i < kMultiGroup * NB; i += kThreads) (&sbins[0][0])[i] = 0;
     __syncthreads();
-    unsigned long long* g = gdigits + (size_t)r * kBins1;
-    for (int i = threadIdx.x; i < NB; i += kThreads) {
-        const uint32_t c = sbins[i];
-        if (c) atomicAdd(&g[i], (unsigned long long)c);
+    auto one = [&](uint32_t key) {
+#pragma unroll
+        for (int r = 0; r < kMultiGroup; ++r) {
+            const uint32_t t = key - base[r];
+            const uint32_t idx = (PASS == 1) ? (t >> kBits2) : t;    // outside the bucket: >= NB
+            if (live[r] && idx < (uint32_t)NB) atomicAdd(&sbins[r][idx], 1u);
+        }
+    };
+    const uint4* __restrict__ c4 = reinterpret_cast<const uint4*>(cand);   // cudaMalloc'ed: 16-byte aligned
+    const uint64_t m4 = m >> 2, stride = (uint64_t)gridDim.x * kThreads, g = (uint64_t)blockIdx.x * kThreads + threadIdx.x;
+    for (uint64_t i = g; i < m4; i += 2 * stride) {
+        const uint4 a = __ldg(c4 + i);
+        const bool two = i + stride < m4;
+        const uint4 b = two ? __ldg(c4 + i + stride) : make_uint4(0, 0, 0, 0);
+        one(a.x); one(a.y); one(a.z); one(a.w);
+        if (two) { one(b.x); one(b.y); one(b.z); one(b.w); }
+    }
+    if (g < (m & 3ull)) one(__ldg(cand + (m4 << 2) + g));
+    __syncthreads();
+#pragma unroll
+    for (int r = 0; r < kMultiGroup; ++r) {
+        if (!live[r]) continue;
+        unsigned long long* gd = gdigits + (size_t)r * kBins1;
+        for (int i = threadIdx.x; i < NB; i += kThreads) {
+            const uint32_t c = sbins[r][i];
+            if (c) atomicAdd(&gd[i], (unsigned long long)c);
+        }
     }
 }
 

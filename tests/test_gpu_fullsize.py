@@ -92,6 +92,13 @@ def test_config2_full_size():
         k = ref["count"] // 100
         assert bits(ctx.kth(t, *dims, k)) == bits(oracle.kth(a, k))
         certify(a, med, (ref["count"] - 1) // 2)
+        # the three ranks bench.py asks cube_kth_multi for (two reads of the cube), and a second group of ranks
+        ks = [(ref["count"] - 1) // 2, k, 99 * ref["count"] // 100, 0, ref["count"] - 1, ref["count"]]
+        got = ctx.kth_multi(t, *dims, ks)
+        assert bits(got[0]) == bits(omed) and bits(got[1]) == bits(oracle.kth(a, k))
+        for kk, g in zip(ks[2:5], got[2:5]):
+            certify(a, g, kk)
+        assert np.isnan(got[5])
     finally:
         ctx.close()
 
@@ -113,10 +120,17 @@ def _big_config(name, hists, ks):
             if first:
                 certify(a, med, (ref["count"] - 1) // 2)
                 assert bits(ctx.median(t, *dims)) == bits(med)
+                med0 = med
                 first = False
+        singles = []
         for kf in ks:
             k = int(kf(ref["count"]))
-            certify(a, ctx.kth(t, *dims, k), k)
+            singles.append(ctx.kth(t, *dims, k))
+            certify(a, singles[-1], k)
+        # the same ranks and the median through cube_kth_multi (two reads): bit-identical to the certified values
+        kk = [(ref["count"] - 1) // 2] + [int(kf(ref["count"])) for kf in ks]
+        got = ctx.kth_multi(t, *dims, kk)
+        assert [bits(g) for g in got] == [bits(med0)] + [bits(v) for v in singles]
         return ref
     finally:
         ctx.close()
