@@ -493,13 +493,11 @@ int cube_kth_multi(cube_ctx* c, const float* d, int64_t nx, int64_t ny, int64_t 
         multi_scan_kernel<2><<<m, kBins1, 0, s>>>(c->multi, c->gdigits);
         multi_done_kernel<<<1, 1, 0, s>>>(c->multi);
         CUBE_CUDA(c, cudaGetLastError());
-        for (int i = 0; i < m; ++i) {
-            if ((rc = kth_impl<false>(c, d, n, k[g0 + i], 0, CUBE_REUSE_COARSE, nullptr, s, ok_word))) return rc;
-            multi_pick_kernel<<<1, 1, 0, s>>>(c->multi, i, c->sel);
-        }
-        CUBE_CUDA(c, cudaGetLastError());
-        CUBE_CUDA(c, cudaMemcpyAsync(out + g0, reinterpret_cast<const char*>(c->multi) + offsetof(MultiState, result),
-                                     (size_t)m * sizeof(float), cudaMemcpyDefault, s));
+        // a fallback selection stores its result straight into the group's record (its last pass, when it runs)
+        float* results = reinterpret_cast<float*>(reinterpret_cast<char*>(c->multi) + offsetof(MultiState, result));
+        for (int i = 0; i < m; ++i)
+            if ((rc = kth_impl<false>(c, d, n, k[g0 + i], 0, CUBE_REUSE_COARSE, results + i, s, ok_word))) return rc;
+        CUBE_CUDA(c, cudaMemcpyAsync(out + g0, results, (size_t)m * sizeof(float), cudaMemcpyDefault, s));
     }
     return CUBE_OK;
 }

@@ -9,7 +9,7 @@
 //   then, on the candidates only (a few per cent of the cube): per rank the second digit (multi_cand_kernel<1>,
 //   multi_scan_kernel<1>) and the third (multi_cand_kernel<2>, multi_scan_kernel<2>), all ranks in one launch.
 // If the buckets together do not fit the candidate buffer, MultiState::ok stays 0 and the caller's per-rank
-// selections (enqueued behind, skipped when ok == 1) give the results: the decision never leaves the device.
+// selections (enqueued behind, skipped when ok == 1) store the results into the same record: the decision never leaves the device.
 // The cube is never written.
 #pragma once
 #include "cube_select.cuh"
@@ -284,11 +284,6 @@ multi_scan_kernel(MultiState* __restrict__ ms, unsigned long long* __restrict__ 
 // per-rank selections enqueued behind skip themselves when it is set).
 __global__ void multi_done_kernel(MultiState* __restrict__ ms) {
     if (ms->cand_n <= ms->cand_cap) ms->ok = 1;
-}
-
-// Fallback bookkeeping: when the candidates did not fit, rank r's result is the one the per-rank selection left.
-__global__ void multi_pick_kernel(MultiState* __restrict__ ms, int r, const SelectState* __restrict__ st) {
-    if (!ms->ok) ms->result[r] = st->result;
 }
 
 }  // namespace cube

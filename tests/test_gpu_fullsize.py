@@ -144,7 +144,9 @@ def test_config3_full_size():
 
 @pytest.mark.skipif(not FULL, reason="32 GiB cube + single-thread oracle passes: set CUBE_FULLSIZE=1")
 def test_config4_full_size():
-    ref = _big_config("c4", [256, 65536], [])
+    # rank 0 is one of the 30 % of voxels that are exactly +0.0: its first-digit bucket cannot fit the candidate
+    # buffer, so cube_kth_multi's group falls back, on the device, to the per-rank selections -- at full size
+    ref = _big_config("c4", [256, 65536], [lambda c: 0])
     assert bits(ref["min"]) == 0 and (ref["count"] - 1) // 2 == 2 ** 32 - 1
 
 
