@@ -102,6 +102,14 @@ int oracle_moments(const float* d, uint64_t N, int sample_std, oracle_moments_t*
         out->mean = out->std = std::numeric_limits<double>::quiet_NaN();
         return 0;
     }
+    // Reading R8: a set with an infinite member has no finite mean or deviation; both are reported as
+    // NaN (count, min, max stay exact).  Stated here rather than left to what Inf does to a compensated sum.
+    if (std::isinf(mn) || std::isinf(mx)) {
+        out->min = mn;
+        out->max = mx;
+        out->mean = out->std = std::numeric_limits<double>::quiet_NaN();
+        return 0;
+    }
     long double mean = sum.value() / (long double)n;
     // second pass: corrected two-pass M2 = sum(delta^2) - (sum delta)^2 / n
     Comp sd, sd2;

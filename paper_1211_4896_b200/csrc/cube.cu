@@ -20,7 +20,7 @@ struct cube_ctx {
     int device = 0;
     int num_sms = 0;
     int ctas_per_sm = 0;  // 0 = per-kernel default
-    int bighist = 0;      // CUBE_KNOB_BIGHIST: 0 = 16-bit packed counters, 1 = cluster DSM
+    int bighist = 0;      // CUBE_KNOB_BIGHIST: 0 = automatic (window or packed, chosen on the device), 1 = cluster DSM, 2 = packed
     int minimap_variant = 0;  // CUBE_KNOB_MINIMAP: 0 = automatic, 1 = no TMA ring, 2 = scalar kernel only, 3 = TMA ring whenever eligible
     int last_cuda = 0;
     uint64_t launches = 0;
@@ -180,16 +180,20 @@ inline bool hist_scale(int nbins, float lo, float hi, float* scale) {
 }
 
 // mode: kMomPlain / kMomCoarse / kMomWindow (window = (wlo, whi), or the context's ClipState when use_clip)
+// digits: where kMomCoarse adds the first-digit counts (nullptr: the context's `coarse` array, zeroed first unless
+// accumulating; the brick-streamed path passes gdigits, which cube_ooc_begin has zeroed)
 int launch_moments(cube_ctx* c, const float* d, uint64_t n, unsigned flags, int accumulate, cudaStream_t s,
                    int mode = -1, float wlo = 0.f, float whi = 0.f, bool use_clip = false,
-                   const SelectInit* fuse_scan = nullptr, MomentsOut* out_user = nullptr) {
+                   const SelectInit* fuse_scan = nullptr, MomentsOut* out_user = nullptr,
+                   unsigned long long* digits = nullptr) {
     if (mode < 0) mode = (flags & CUBE_COARSE_HIST) ? kMomCoarse : kMomPlain;
     const bool coarse = mode == kMomCoarse;
     const int occ_m = mode == kMomCoarse ? occupancy_of(c, moments_kernel<kMomCoarse>, kThreads, 0)
                     : mode == kMomWindow ? occupancy_of(c, moments_kernel<kMomWindow>, kThreads, 0)
                                          : occupancy_of(c, moments_kernel<kMomPlain>, kThreads, 0);
     const int grid = grid_for(c, 4, occ_m < kMaxCtasPerSm ? occ_m : kMaxCtasPerSm);
-    if (coarse && !accumulate) CUBE_CUDA(c, cudaMemsetAsync(c->coarse, 0, kDigitBins * sizeof(unsigned long long), s));
+    if (coarse && !accumulate && !digits) CUBE_CUDA(c, cudaMemsetAsync(c->coarse, 0, kDigitBins * sizeof(unsigned long long), s));
+    if (!digits) digits = c->coarse;
     {
     ProfScope prof(c, coarse ? CUBE_K_MOMENTS_COARSE : mode == kMomWindow ? CUBE_K_MOMENTS_WINDOW : CUBE_K_MOMENTS, s);
     const ClipState* clip = use_clip ? c->clip : nullptr;
@@ -197,7 +201,7 @@ int launch_moments(cube_ctx* c, const float* d, uint64_t n, unsigned flags, int 
     none.k = 0; none.cand_cap = 0; none.result_out = nullptr; none.use_median = 0; none.enabled = 0;
     if (coarse) {   // fuse_scan: the kernel's last CTA also locates the first-digit bucket (cube_stats)
         moments_kernel<kMomCoarse><<<grid, kThreads, 0, s>>>(d, n, c->partials, c->ticket, c->acc, c->nvox_acc,
-                                                             accumulate, flags, c->mom_out, c->coarse, 0.f, 0.f, nullptr,
+                                                             accumulate, flags, c->mom_out, digits, 0.f, 0.f, nullptr,
                                                              c->sel, fuse_scan ? c->ticket2 : nullptr,
                                                              fuse_scan ? *fuse_scan : none, out_user);
     } else if (mode == kMomWindow) {
@@ -214,8 +218,11 @@ int launch_moments(cube_ctx* c, const float* d, uint64_t n, unsigned flags, int 
     return CUBE_OK;
 }
 
+// fused_select: more than 16384 bins, the window histogram shares its read with the second select digit
+// (hist_win_select_kernel); fused_scan: its last CTA also locates the bucket (in-core calls; the brick-streamed
+// path locates it after the last brick)
 int launch_hist(cube_ctx* c, const float* d, uint64_t n, int nbins, float lo, float hi, float scale,
-                cudaStream_t s, const float* range3 = nullptr, bool fused_select = false) {
+                cudaStream_t s, const float* range3 = nullptr, bool fused_select = false, bool fused_scan = true) {
     unsigned long long* outside = c->gout;
     {
     ProfScope prof(c, fused_select ? CUBE_K_HIST_SELECT : CUBE_K_HIST, s);
@@ -236,7 +243,8 @@ int launch_hist(cube_ctx* c, const float* d, uint64_t n, int nbins, float lo, fl
             if (fused_select) {   // cube_stats: window histogram + second select digit in one kernel
                 c->launches++;
                 hist_win_select_kernel<<<c->num_sms, kBigThreads, kBigFusedSmem, s>>>(
-                    d, n, nbins, lo, hi, scale, range3, c->plan, c->gbins, outside, c->sel, c->gdigits, c->cand, c->ticket2);
+                    d, n, nbins, lo, hi, scale, range3, c->plan, c->gbins, outside, c->sel, c->gdigits, c->cand,
+                    fused_scan ? c->ticket2 : nullptr);
             } else if (window_allowed) {
                 c->launches++;
                 hist_win_kernel<<<c->num_sms, kBigThreads, smem, s>>>(d, n, nbins, lo, hi, scale, range3, c->plan,
@@ -261,14 +269,15 @@ inline SelectInit select_init_args(const cube_ctx* c, uint64_t k, int use_median
 }
 
 // fuse != nullptr: the last CTA of the pass also locates the bucket (select_scan_if_last) -- in-core selections
+// brick_only (PASS 2 of a brick-streamed run): never read the candidate buffer -- select_cand_kernel counts it once
 template <int PASS, bool DEV = false>
 int launch_select_pass(cube_ctx* c, const float* d, uint64_t n, cudaStream_t s, const SelectInit* fuse = nullptr,
-                       const uint32_t* skip_if_set = nullptr) {
+                       const uint32_t* skip_if_set = nullptr, bool brick_only = false) {
     const int occ = occupancy_of(c, select_pass_kernel<PASS, DEV>, kThreads, 0);  // every CTA must be resident (static tile dealing)
     const int grid = grid_for(c, 4, occ < kMaxCtasPerSm ? occ : kMaxCtasPerSm);
     {
         ProfScope prof(c, PASS == 0 ? CUBE_K_SELECT_PASS0 : PASS == 1 ? CUBE_K_SELECT_PASS1 : CUBE_K_SELECT_PASS2, s);
-        select_pass_kernel<PASS, DEV><<<grid, kThreads, 0, s>>>(d, n, c->sel, c->gdigits, c->cand, c->center,
+        select_pass_kernel<PASS, DEV><<<grid, kThreads, 0, s>>>(d, n, c->sel, c->gdigits, brick_only ? nullptr : c->cand, c->center,
                                                                 fuse ? c->ticket2 : nullptr,
                                                                 fuse ? *fuse : select_init_args(c, 0, 0, false), skip_if_set);
     }
@@ -277,12 +286,13 @@ int launch_select_pass(cube_ctx* c, const float* d, uint64_t n, cudaStream_t s, 
 }
 
 template <int PASS>
-int launch_select_scan(cube_ctx* c, unsigned long long* digits, cudaStream_t s, const SelectInit* init = nullptr) {
+int launch_select_scan(cube_ctx* c, unsigned long long* digits, cudaStream_t s, const SelectInit* init = nullptr,
+                       const uint32_t* skip_if_set = nullptr) {
     // the coarse histogram kept by CUBE_COARSE_HIST is left intact so that several k can reuse it
     {
         ProfScope prof(c, CUBE_K_SELECT_SCAN, s);
         select_scan_kernel<PASS><<<1, 1024, 0, s>>>(c->sel, digits, digits == c->gdigits ? 1 : 0,
-                                                    init ? *init : select_init_args(c, 0, 0, false));
+                                                    init ? *init : select_init_args(c, 0, 0, false), skip_if_set);
     }
     CUBE_CUDA(c, cudaGetLastError());
     return CUBE_OK;
@@ -311,7 +321,7 @@ int kth_impl(cube_ctx* c, const float* d, uint64_t n, uint64_t k, int use_median
     float* direct = static_cast<float*>(device_reachable(c, out));   // pass C stores the result there itself
     const SelectInit init = select_init_args(c, k, use_median, true), cont = select_init_args(c, 0, 0, false, direct);
     if (!DEV && (flags & CUBE_REUSE_COARSE)) {
-        if ((rc = launch_select_scan<0>(c, c->coarse, s, &init))) return rc;
+        if ((rc = launch_select_scan<0>(c, c->coarse, s, &init, skip_if_set))) return rc;
     } else {
         CUBE_CUDA(c, cudaMemsetAsync(c->gdigits, 0, kDigitBins * sizeof(unsigned long long), s));
         if ((rc = launch_select_pass<0, DEV>(c, d, n, s, &init))) return rc;
@@ -481,17 +491,35 @@ int cube_kth_multi(cube_ctx* c, const float* d, int64_t nx, int64_t ny, int64_t 
         memset(&req, 0, sizeof(req));
         req.nk = (uint32_t)m;
         for (int i = 0; i < m; ++i) req.k[i] = k[g0 + i];
-        multi_locate_kernel<<<1, 1024, 0, s>>>(c->multi, c->coarse, req, c->cand ? c->cand_cap : 0);
+        {
+            ProfScope prof(c, CUBE_K_SELECT_SCAN, s);
+            multi_locate_kernel<<<1, 1024, 0, s>>>(c->multi, c->coarse, req, c->cand ? c->cand_cap : 0);
+        }
         {
             ProfScope prof(c, CUBE_K_SELECT_PASS1, s);
             multi_gather_kernel<<<grid, kThreads, 0, s>>>(d, n, c->multi, c->cand);
         }
         const int cgrid = 4 * c->num_sms;
-        multi_cand_kernel<1><<<cgrid, kThreads, 0, s>>>(c->multi, c->gdigits, c->cand);
-        multi_scan_kernel<1><<<m, kBins1, 0, s>>>(c->multi, c->gdigits);
-        multi_cand_kernel<2><<<cgrid, kThreads, 0, s>>>(c->multi, c->gdigits, c->cand);
-        multi_scan_kernel<2><<<m, kBins1, 0, s>>>(c->multi, c->gdigits);
-        multi_done_kernel<<<1, 1, 0, s>>>(c->multi);
+        {
+            ProfScope prof(c, CUBE_K_SELECT_CAND, s);
+            multi_cand_kernel<1><<<cgrid, kThreads, 0, s>>>(c->multi, c->gdigits, c->cand);
+        }
+        {
+            ProfScope prof(c, CUBE_K_SELECT_SCAN, s);
+            multi_scan_kernel<1><<<m, kBins1, 0, s>>>(c->multi, c->gdigits);
+        }
+        {
+            ProfScope prof(c, CUBE_K_SELECT_CAND, s);
+            multi_cand_kernel<2><<<cgrid, kThreads, 0, s>>>(c->multi, c->gdigits, c->cand);
+        }
+        {
+            ProfScope prof(c, CUBE_K_SELECT_SCAN, s);
+            multi_scan_kernel<2><<<m, kBins1, 0, s>>>(c->multi, c->gdigits);
+        }
+        {
+            ProfScope prof(c, CUBE_K_OTHER, s);
+            multi_done_kernel<<<1, 1, 0, s>>>(c->multi);
+        }
         CUBE_CUDA(c, cudaGetLastError());
         // a fallback selection stores its result straight into the group's record (its last pass, when it runs)
         float* results = reinterpret_cast<float*>(reinterpret_cast<char*>(c->multi) + offsetof(MultiState, result));

@@ -36,13 +36,20 @@ struct HistWinSelectF {
     bool select;                   // false: nothing to select (k >= count)
     BigSelShared* sh;
 
+    // Single voxels (head / tail / ragged last tile: up to 8 rows x 4 voxels per lane with no fill check in between)
+    // never go through the warp's stage slice, which only holds what HALF a tile share can add: their keys are
+    // appended straight to the candidate buffer, one global atomic each (at most one ragged tile per launch).
     __device__ __forceinline__ void operator()(float x) {
         h(x);
         if (select) {
-            const int warp = threadIdx.x >> 5;
-            uint32_t* s_buf = sh->stage + warp * kBigStageCap;
-            uint32_t* s_cnt = sh->stage + kBigWarps * kBigStageCap + warp;
-            SelectF<1, false>::take1(x, sh->base, sh->sbins, sh->compacting[warp] ? s_cnt : nullptr, s_buf);
+            const uint32_t kk = key_of(x) - sh->base;
+            if (kk < SelectF<1, false>::kSpan && x == x) {
+                atomicAdd(&sh->sbins[kk >> kBits2], 1u);
+                if (sh->cand && sh->cand_cap) {
+                    const unsigned long long pos = atomicAdd(sh->cand_n, 1ull);   // beyond the capacity: cand_n says so
+                    if (pos < sh->cand_cap) sh->cand[pos] = kk + sh->base;
+                }
+            }
         }
     }
     // rows `rows` (bit j = row j0 + j) of this lane hold a voxel of the bucket: count its digit, stage its key

@@ -61,8 +61,11 @@ struct MomentsF {
         n += ok ? 1u : 0u;
         if (COARSE) smem_inc(sbins, ok ? raw_digit(x) : (uint32_t)kDigitBins);  // raw top bits; NaN -> trash
     }
+    // The pivot is the first FINITE voxel that takes part: about an infinite pivot every deviation would be
+    // infinite or NaN.  (A cube with +-Inf voxels has mean = std = NaN whatever the summation order: reading R8,
+    // applied in moments_finalize.)
     __device__ __forceinline__ void take_pivot(float x) {
-        if (!have && taken(x)) { have = true; pivf = x; pivot = (double)x; }
+        if (!have && taken(x) && fabsf(x) < INFINITY) { have = true; pivf = x; pivot = (double)x; }
     }
     __device__ __forceinline__ void operator()(float x) { take_pivot(x); core(x); }
 
@@ -142,7 +145,8 @@ struct MomentsF {
         Partial p = partial_empty();
         if (n) {
             const double nn = (double)n, ms = s / nn;
-            p.n = n; p.mean = pivot + ms; p.m2 = fmax(q - s * ms, 0.0);
+            const double m2 = q - s * ms;
+            p.n = n; p.mean = pivot + ms; p.m2 = (m2 < 0.0) ? 0.0 : m2;   // rounding only; a NaN (Inf voxels) stays
             p.kmin = key_of(mn); p.kmax = key_of(mx);
         }
         return p;
@@ -164,6 +168,9 @@ __device__ __forceinline__ void moments_finalize(const Partial& t, uint64_t nvox
         o.mean = t.mean;
         const double den = (flags & 1u) ? (double)t.n - 1.0 : (double)t.n;
         o.std = (den > 0.0) ? sqrt(fmax(t.m2, 0.0) / den) : (double)qnan;
+        // reading R8: a set with an infinite member has no finite mean or deviation -- both are NaN, decided on the
+        // extrema so that the answer depends neither on the summation order nor on the grid
+        if (isinf(o.min) || isinf(o.max)) o.mean = o.std = (double)qnan;
     }
     *out = o;
 }
@@ -348,6 +355,15 @@ __global__ void shard_merge_kernel(const unsigned char* __restrict__ gathered, i
     *acc = m;
     *nvox = tot;
     moments_finalize(m, tot, flags, out);
+}
+
+// Start of a brick-streamed / sharded accumulation: the running record is the empty one (a rank whose slab holds no
+// voxel contributes exactly that to the all-gather), the voxel total 0, the finalised record that of an empty cube.
+__global__ void moments_reset_kernel(Partial* __restrict__ acc, unsigned long long* __restrict__ nvox,
+                                     MomentsOut* __restrict__ out) {
+    *acc = partial_empty();
+    *nvox = 0ull;
+    moments_finalize(*acc, 0ull, 0u, out);
 }
 
 // Re-evaluate mean/std of the running partial with other flags (sample std) -- O(1).

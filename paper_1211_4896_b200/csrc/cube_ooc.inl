@@ -16,26 +16,69 @@ int cube_ooc_begin(cube_ctx* c, int nbins, float lo, float hi, int want_median, 
     c->ooc_want_median = want_median ? 1 : 0;
     CUBE_CUDA(c, cudaMemsetAsync(c->gout, 0, (CUBE_MAX_BINS + 2) * sizeof(unsigned long long), s));
     CUBE_CUDA(c, cudaMemsetAsync(c->gdigits, 0, kDigitBins * sizeof(unsigned long long), s));
+    {   // the running record starts empty: a rank that presents no brick (empty slab) all-gathers exactly that
+        ProfScope prof(c, CUBE_K_OTHER, s);
+        moments_reset_kernel<<<1, 1, 0, s>>>(c->acc, c->nvox_acc, c->mom_out);
+    }
+    CUBE_CUDA(c, cudaGetLastError());
     return select_init(c, 0, 1, s);
 }
 
+// The bricks are read TWICE when the median is asked for, like the cube in cube_stats (8 B per voxel, DESIGN.md
+// sec. 8): sweep 0 = fused pass A (moments + first select digit), sweep 1 = fused pass B (histogram + second digit +
+// compaction), last digit on the candidates (a third sweep only if the bucket did not fit the buffer).  Without
+// the median: one sweep, moments and histogram.
 int cube_ooc_brick(cube_ctx* c, const float* d, uint64_t nvox, cudaStream_t s) {
     if (!c || !c->ooc_active || !d || nvox == 0 || nvox > (1ull << 37)) return CUBE_EINVAL;
     int rc = CUBE_OK;
+    const int acc = 1;   // cube_ooc_begin has made the running record the empty one: merging into it is the identity
     if (c->ooc_sweep == 0) {
-        if ((rc = launch_moments(c, d, nvox, 0u, c->ooc_bricks > 0, s))) return rc;
-        if (c->ooc_nbins > 0 &&
-            (rc = launch_hist(c, d, nvox, c->ooc_nbins, c->ooc_lo, c->ooc_hi, c->ooc_scale, s))) return rc;
-        if (c->ooc_want_median && (rc = launch_select_pass<0>(c, d, nvox, s))) return rc;
+        if (c->ooc_want_median) {
+            rc = launch_moments(c, d, nvox, CUBE_COARSE_HIST, acc, s, kMomCoarse, 0.f, 0.f, false, nullptr, nullptr, c->gdigits);
+        } else {
+            if ((rc = launch_moments(c, d, nvox, 0u, acc, s))) return rc;
+            if (c->ooc_nbins > 0) rc = launch_hist(c, d, nvox, c->ooc_nbins, c->ooc_lo, c->ooc_hi, c->ooc_scale, s);
+        }
     } else if (c->ooc_sweep == 1) {
-        rc = launch_select_pass<1>(c, d, nvox, s);
+        const int nbins = c->ooc_nbins;
+        if (nbins > 0 && nbins <= kSmemHistMaxBins) {
+            const size_t smem = (size_t)hist_select_smem(nbins);
+            const int occ = occupancy_of(c, hist_select_kernel, kThreads, smem);
+            const int grid = grid_for(c, 4, occ < kMaxCtasPerSm ? occ : kMaxCtasPerSm);
+            {
+                ProfScope prof(c, CUBE_K_HIST_SELECT, s);
+                hist_select_kernel<<<grid, kThreads, smem, s>>>(d, nvox, nbins, c->ooc_lo, c->ooc_hi, c->ooc_scale, nullptr,
+                                                                c->gbins, c->gout, c->sel, c->gdigits, c->cand, nullptr);
+            }
+            CUBE_CUDA(c, cudaGetLastError());
+        } else if (nbins > 0) {
+            // window histogram + second digit in one read when the sampled plan allows it (and the automatic variant
+            // is selected); else the histogram kernel and select_pass_kernel<1> read the brick one after the other
+            const bool fused_big = c->bighist == 0;
+            if ((rc = launch_hist(c, d, nvox, nbins, c->ooc_lo, c->ooc_hi, c->ooc_scale, s, nullptr, fused_big, false))) return rc;
+            rc = launch_select_pass<1>(c, d, nvox, s, nullptr, fused_big ? &c->plan->use_window : nullptr);
+        } else {
+            rc = launch_select_pass<1>(c, d, nvox, s);
+        }
     } else if (c->ooc_sweep == 2) {
-        rc = launch_select_pass<2>(c, d, nvox, s);
+        // only the brick itself, and only if the candidates did not fit (else select_cand_kernel has counted them)
+        rc = launch_select_pass<2>(c, d, nvox, s, nullptr, &c->sel->cand_done, true);
     } else {
         return CUBE_EINVAL;
     }
     c->ooc_bricks++;
     return rc;
+}
+
+// Last digit on the candidates, once per context and selection: runs iff they fitted (decided on the device).
+static int ooc_count_candidates(cube_ctx* c, cudaStream_t s) {
+    if (!c->cand) return CUBE_OK;
+    {
+        ProfScope prof(c, CUBE_K_SELECT_CAND, s);
+        select_cand_kernel<<<c->num_sms, kThreads, 0, s>>>(c->sel, c->gdigits, c->cand);
+    }
+    CUBE_CUDA(c, cudaGetLastError());
+    return CUBE_OK;
 }
 
 int cube_ooc_next_sweep(cube_ctx* c, int* more, cudaStream_t s) {
@@ -46,18 +89,14 @@ int cube_ooc_next_sweep(cube_ctx* c, int* more, cudaStream_t s) {
         if (c->ooc_sweep == 0) { rc = launch_select_scan<0>(c, c->gdigits, s); *more = 1; }
         else if (c->ooc_sweep == 1) {
             if ((rc = launch_select_scan<1>(c, c->gdigits, s))) return rc;
+            if ((rc = ooc_count_candidates(c, s))) return rc;
             *more = 1;
-            // Did the median's bucket fit the candidate buffer?  One 16-byte read per cube: if so the last
-            // digit is counted on the candidates right now and no third sweep over the bricks is needed.
-            unsigned long long cn[2] = {0, 0};
-            CUBE_CUDA(c, cudaMemcpyAsync(cn, &c->sel->cand_n, sizeof(cn), cudaMemcpyDeviceToHost, s));
+            // Did the median's bucket fit the candidate buffer?  One 4-byte read per cube: if so the last digit
+            // has just been counted on the candidates and no third sweep over the bricks is needed.
+            uint32_t done = 0;
+            CUBE_CUDA(c, cudaMemcpyAsync(&done, &c->sel->cand_done, sizeof(done), cudaMemcpyDeviceToHost, s));
             CUBE_CUDA(c, cudaStreamSynchronize(s));
-            if (c->cand && cn[0] <= cn[1]) {
-                {
-                    ProfScope prof(c, CUBE_K_SELECT_CAND, s);
-                    select_cand_kernel<<<c->num_sms, kThreads, 0, s>>>(c->sel, c->gdigits, c->cand);
-                }
-                CUBE_CUDA(c, cudaGetLastError());
+            if (done) {
                 if ((rc = launch_select_scan<2>(c, c->gdigits, s))) return rc;
                 c->ooc_sweep = 2;  // becomes 3 below: result ready
                 *more = 0;
@@ -125,7 +164,13 @@ int cube_shard_advance(cube_ctx* c, int* more, cudaStream_t s) {
     *more = 0;
     if (c->ooc_want_median) {
         if (c->ooc_sweep == 0) { rc = launch_select_scan<0>(c, c->gdigits, s); *more = 1; }
-        else if (c->ooc_sweep == 1) { rc = launch_select_scan<1>(c, c->gdigits, s); *more = 1; }
+        else if (c->ooc_sweep == 1) {
+            // stage 2 of this rank: its own candidates are counted here, ONCE (the scan has just cleared the digit
+            // counts); the bricks presented in stage 2 are then read only if the candidates did not fit
+            if ((rc = launch_select_scan<1>(c, c->gdigits, s))) return rc;
+            rc = ooc_count_candidates(c, s);
+            *more = 1;
+        }
         else if (c->ooc_sweep == 2) { rc = launch_select_scan<2>(c, c->gdigits, s); }
         else return CUBE_EINVAL;
     }

@@ -26,6 +26,8 @@ struct SelectState {
     float result;
     unsigned long long cand_n;  // keys of the pass-0 bucket seen by the compacting pass 1
     unsigned long long cand_cap;  // capacity of the candidate buffer, in keys
+    uint32_t cand_done;         // 1: the last digit has been counted on the candidates (select_cand_kernel), so the
+    uint32_t pad_;              //    per-brick PASS 2 launches of a brick-streamed / sharded run return at once
 };
 
 // PASS 1 compaction ("step 8"): every warp stages the keys of the prefix bucket in its own slice of shared
@@ -298,7 +300,7 @@ __device__ __forceinline__ void select_scan_body(SelectState* __restrict__ st, u
             if (PASS == 0) {
                 st->count = total; st->invalid = invalid;
                 if (init.enabled) {
-                    st->use_median = init.use_median; st->cand_n = 0; st->cand_cap = init.cand_cap;
+                    st->use_median = init.use_median; st->cand_n = 0; st->cand_cap = init.cand_cap; st->cand_done = 0;
                 }
             }
             if (PASS == 0 || invalid) { st->k = k; st->prefix = prefix; st->result = __int_as_float(0x7fc00000); }
@@ -364,8 +366,10 @@ __device__ __forceinline__ void select_scan_body(SelectState* __restrict__ st, u
 
 template <int PASS>
 __global__ void __launch_bounds__(1024)
-select_scan_kernel(SelectState* __restrict__ st, unsigned long long* __restrict__ gdigits, int clear, SelectInit init) {
+select_scan_kernel(SelectState* __restrict__ st, unsigned long long* __restrict__ gdigits, int clear, SelectInit init,
+                   const uint32_t* __restrict__ skip_if_set) {
     __shared__ unsigned long long sm[kScanSmem];
+    if (skip_if_set && *skip_if_set) return;   // cube_kth_multi's fallback selection is not needed
     select_scan_body<PASS, 1024>(st, gdigits, clear, init, sm);
 }
 
@@ -428,12 +432,16 @@ select_pass_kernel(const float* __restrict__ d, uint64_t n, SelectState* __restr
     }
 }
 
-// PASS 2 over the candidate buffer only (out-of-core: no third sweep over the host link).  The caller has
-// checked cand_n <= cand_cap on the host.
+// PASS 2 over the candidate buffer only (out-of-core: no third sweep over the host link; sharded: every rank counts
+// its own candidates ONCE, however many bricks its slab is presented in).  Runs iff the bucket fitted the buffer
+// (cand_n <= cand_cap, decided here on the device) and then sets cand_done, which makes the per-brick PASS 2
+// launches that may follow return at once.
 __global__ void __launch_bounds__(kThreads)
 select_cand_kernel(SelectState* __restrict__ st, unsigned long long* __restrict__ gdigits,
                    const uint32_t* __restrict__ cand) {
     __shared__ uint32_t sbins[kBins2 + 1];
+    if (st->cand_n > st->cand_cap) return;   // uniform over the grid: the bricks are streamed again instead
+    if (blockIdx.x == 0 && threadIdx.x == 0) st->cand_done = 1u;   // read by LATER launches only
     for (int i = threadIdx.x; i <= kBins2; i += kThreads) sbins[i] = 0;
     __syncthreads();
     SelectF<2, false> f;

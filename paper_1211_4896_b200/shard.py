@@ -5,7 +5,7 @@ This is the paper's client/server decomposition: every merge 
 and commutative, so each rank reduces its own slab with the single-GPU kernels and only O(bins)
 counters cross the links -- an all-gather of one 40-byte moments record per rank, one all-reduce of the histogram and
 three all-reduces of 64 KiB of digit counts, against the paper's ~31 rounds of five scalars for Torben's median
-(PAPER.md:294-296).  All payloads are latency-bound; every step is enqueued on one stream and nothing synchronises
+(PAPER.md:294-296); every rank reads its slab twice (8 B per voxel), as cube_stats reads the cube.  All payloads are latency-bound; every step is enqueued on one stream and nothing synchronises
 the host.
 
 Plumbing only: every arithmetic step (accumulation, record merge, bucket location) runs in libcube's kernels; this
@@ -40,8 +40,11 @@ def alias(ptr, nbytes, dtype, device):
 class ShardedStats:
     """One rank's side of a sharded moments + histogram + exact-median run.
 
-    ``stage`` 0: moments + histogram + first select digit; 1: second digit + candidate compaction; 2: last digit.
-    Per stage: ``local_pass()`` -> combine ``payload()`` across ranks -> ``advance()``.
+    With the median the slab is read twice, like the cube in ``cube_stats`` (8 B per voxel): ``stage`` 0 = moments +
+    first select digit (libcube's fused pass A), 1 = histogram + second digit + candidate compaction (fused pass B),
+    2 = last digit on this rank's own candidates (counted once inside ``advance()``; the slab is read a third time
+    only if they did not fit the candidate buffer -- decided on the device).  Without the median: one stage, moments
+    and histogram.  Per stage: ``local_pass()`` -> combine ``payload()`` across ranks -> ``advance()``.
     """
 
     def __init__(self, ctx, slab, nvox, nbins, lo, hi, want_median=True, flags=0, stream=None, device=None):
@@ -63,10 +66,10 @@ class ShardedStats:
 
     def payload(self):
         """-> (record to all-gather or None, [tensors to all-reduce SUM])."""
+        hist = [self.bins, self.outside] if self.nbins else []
         if self.stage == 0:
-            sums = ([self.bins, self.outside] if self.nbins else []) + ([self.digits] if self.want_median else [])
-            return self.record, sums
-        return None, [self.digits]
+            return self.record, ([self.digits] if self.want_median else hist)
+        return None, (hist if self.stage == 1 else []) + [self.digits]
 
     def merge_records(self, gathered, world):
         self.ctx.shard_merge_records(gathered, world, self.flags, self.stream)

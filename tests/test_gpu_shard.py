@@ -29,11 +29,22 @@ def same_float(a, b):
     return a.view(np.uint32) == b.view(np.uint32)
 
 
-def lockstep(slabs, nbins, lo, hi, want_median=True, flags=0, scratch=0):
+class SeveralBricks(shard.ShardedStats):
+    """A rank that presents its slab as three bricks per stage (cube.h allows any split into contiguous runs)."""
+
+    def local_pass(self):
+        step = (self.nvox + 2) // 3
+        for o in range(0, self.nvox, step):
+            self.ctx.ooc_brick(self.slab[o:o + step], min(step, self.nvox - o), self.stream)
+
+
+def lockstep(slabs, nbins, lo, hi, want_median=True, flags=0, scratch=0, cls=shard.ShardedStats, ctxs=None):
     """Drive len(slabs) ranks through shard.ShardedStats in one process; the combine step is what the collectives do."""
     world = len(slabs)
-    ctxs = [cube.Context(scratch_bytes_hint=scratch) for _ in slabs]
-    sts = [shard.ShardedStats(c, s, s.numel(), nbins, lo, hi, want_median, flags) for c, s in zip(ctxs, slabs)]
+    own = ctxs is None
+    if own:
+        ctxs = [cube.Context(scratch_bytes_hint=scratch) for _ in slabs]
+    sts = [cls(c, s, s.numel(), nbins, lo, hi, want_median, flags) for c, s in zip(ctxs, slabs)]
     rounds = 0
     while sts[0].more:
         for st in sts:
@@ -51,8 +62,9 @@ def lockstep(slabs, nbins, lo, hi, want_median=True, flags=0, scratch=0):
             st.advance()
         rounds += 1
     res = [st.result() for st in sts]
-    for c in ctxs:
-        c.close()
+    if own:
+        for c in ctxs:
+            c.close()
     return res, rounds
 
 
@@ -129,3 +141,57 @@ def test_run_with_nccl_world1():
         ctx.close()
     finally:
         dist.destroy_process_group()
+
+
+def test_sharded_empty_slab_and_reused_contexts():
+    # world > nz: the last rank has NO voxel and presents no brick -- it all-gathers the empty record that
+    # cube_ooc_begin leaves, also when its context still holds the record of an earlier run
+    cfg = cubegen.scaled("c2", (64, 48, 3))
+    t = torch.empty(64 * 48 * 3, dtype=torch.float32, device="cuda")
+    cubegen.generate_device(cfg, t.data_ptr())
+    torch.cuda.synchronize()
+    a = t.cpu().numpy()
+    slabs = []
+    for r in range(4):
+        z0, z1 = shard.slab_bounds(3, 4, r)
+        slabs.append(t[z0 * 64 * 48:z1 * 64 * 48])
+    assert slabs[3].numel() == 0
+    ctxs = [cube.Context() for _ in slabs]
+    try:
+        junk = torch.full((5000,), 1e6, dtype=torch.float32, device="cuda")
+        for c in ctxs:                                   # leave a stale running record in every context
+            c.ooc_begin(16, 0.0, 1.0, True)
+            c.ooc_brick(junk, junk.numel())
+        for _ in range(2):
+            res, rounds = lockstep(slabs, 4096, -0.02, 0.5, ctxs=ctxs)
+            assert rounds == 3
+            check_against_oracle(res, a, 4096, -0.02, 0.5)
+        res, _ = lockstep(slabs, 4096, -0.02, 0.5, want_median=False, ctxs=ctxs)
+        ref = oracle.moments(a)
+        rb, ro = oracle.histogram(a, 4096, -0.02, 0.5)
+        for m, b, o, _ in res:
+            assert m["count"] == ref["count"] and (b == rb).all() and (o == ro).all()
+    finally:
+        for c in ctxs:
+            c.close()
+
+
+@pytest.mark.parametrize("scratch", [0, 4096])
+@pytest.mark.parametrize("nbins,lo,hi", [(64, -8.0, 8.0), (40000, -8.0, 8.0)])
+def test_sharded_slab_presented_as_several_bricks(scratch, nbins, lo, hi):
+    # three bricks per rank and stage: the candidates of a rank are counted ONCE (in cube_shard_advance), whether they
+    # fitted the buffer (scratch 0 = default size) or not (4096 bytes: stage 2 re-reads the bricks, each once);
+    # both pass-B kernels (<= 16384 bins, and the window / packed ones above)
+    r = np.random.default_rng(21)
+    b = np.round(r.standard_normal(400003) * 2).astype(np.float32)       # heavy ties: big buckets
+    b[r.integers(0, b.size, 4000)] = np.nan
+    tb = torch.from_numpy(b).cuda()
+    cuts = [0, 150001, 150002, 400003]
+    slabs = [tb[cuts[i]:cuts[i + 1]] for i in range(3)]
+    res, rounds = lockstep(slabs, nbins, lo, hi, scratch=scratch, cls=SeveralBricks)
+    assert rounds == 3
+    check_against_oracle(res, b, nbins, lo, hi)
+    c2 = (r.standard_normal(300000) * 0.002 + 0.0004).astype(np.float32)  # continuous data: small bucket
+    tc = torch.from_numpy(c2).cuda()
+    res, _ = lockstep([tc[:100000], tc[100000:]], 4096, -0.02, 0.5, scratch=scratch, cls=SeveralBricks)
+    check_against_oracle(res, c2, 4096, -0.02, 0.5)

@@ -366,3 +366,24 @@ def test_torben_iteration_count_scales_like_log_n():
     a = (rng.standard_normal(200000) * 0.05).astype(np.float32)
     med, iters, _ = oracle.torben_median(a)
     assert med == oracle.median(a) and 10 <= iters <= 40
+
+
+def test_moments_with_infinite_voxels_reading_r8():
+    # DESIGN.md R8: count / min / max are exact, mean and std are NaN as soon as one voxel is infinite -- for either
+    # sign, both signs, any position and any number of them; a cube without one is untouched by the rule
+    base = np.array([1.0, -2.0, 0.5, 3.0, np.nan], dtype=np.float32)
+    for extra in ([np.inf], [-np.inf], [np.inf, -np.inf], [np.inf] * 5, [-np.inf, -np.inf, 7.0]):
+        for pos in (0, 3, 5):
+            a = np.insert(base, pos, np.array(extra, dtype=np.float32))
+            m = oracle.moments(a)
+            assert m["count"] == a.size - 1 and m["nan_count"] == 1
+            assert m["min"] == np.nanmin(a) and m["max"] == np.nanmax(a)
+            assert np.isnan(m["mean"]) and np.isnan(m["std"])
+            s = oracle.moments(a, sample_std=True)
+            assert np.isnan(s["mean"]) and np.isnan(s["std"])
+    m = oracle.moments(base)
+    assert m["mean"] == 0.625 and abs(m["std"] - np.sqrt(np.mean((np.array([1.0, -2.0, 0.5, 3.0]) - 0.625) ** 2))) < 1e-15
+    # the clipped moments see the rule only when the window holds an infinity
+    a = np.array([1.0, 2.0, 3.0, np.inf], dtype=np.float32)
+    assert oracle.clipped_moments(a, 0.0, 10.0)["mean"] == 2.0
+    assert np.isnan(oracle.clipped_moments(a, 0.0, np.inf)["mean"])

@@ -62,6 +62,8 @@ class StubContext:
     def ooc_begin(self, nbins, lo, hi, want_median, stream):
         self.nbins, self.lo, self.hi, self.stage = nbins, np.float32(lo), np.float32(hi), 0
         self.prefix, self.k, self.total = 0, None, None
+        self.record[:] = [0, 0, 0, np.inf, -np.inf]          # the empty record: a rank without voxels gathers this
+        self.cand = np.zeros(0, dtype=np.uint32)
         self.calls.append("begin")
 
     def ooc_brick(self, slab, nvox, stream):
@@ -70,20 +72,17 @@ class StubContext:
         if self.stage == 0:
             self.record[:] = [a.size, a.astype(np.float64).sum(), (a.astype(np.float64) ** 2).sum(),
                               a.min() if a.size else np.inf, a.max() if a.size else -np.inf]
+            self.digits += np.bincount(key >> 19, minlength=8192)
+        elif self.stage == 1:                                # the histogram shares the second read of the slab
             inr = a[(a >= self.lo) & (a <= self.hi)]
             scale = np.float32(self.nbins) / np.float32(self.hi - self.lo)
             b = np.minimum(np.floor((inr - self.lo) * scale).astype(np.int64), self.nbins - 1)
             self.bins[:self.nbins] += np.bincount(b, minlength=self.nbins)
             self.outside += [int((a < self.lo).sum()), int((a > self.hi).sum())]
-            self.digits += np.bincount(key >> 19, minlength=8192)
-        elif self.stage == 1:
             sel = key[(key >> 19) == self.prefix]
             self.cand = sel
             self.digits[:1024] += np.bincount((sel >> 9) & 1023, minlength=1024)
-        else:
-            sel = self.cand[(self.cand >> 9) == self.prefix]
-            self.digits[:512] += np.bincount(sel & 511, minlength=512)
-        self.calls.append("pass%%d" %% self.stage)
+        self.calls.append("pass%%d" %% self.stage)           # stage 2: the candidates were counted by advance()
 
     def shard_merge_records(self, gathered, world, flags, stream):
         g = gathered.numpy().view(np.float64).reshape(world, 5)
@@ -102,6 +101,9 @@ class StubContext:
         self.prefix = (self.prefix << BITS[self.stage]) | b
         self.digits[:] = 0
         self.stage += 1
+        if self.stage == 2:                                  # this rank's own candidates, once (as cube_shard_advance)
+            sel = self.cand[(self.cand >> 9) == self.prefix]
+            self.digits[:512] += np.bincount(sel & 511, minlength=512)
         self.calls.append("advance")
         return self.stage < 3
 
@@ -118,7 +120,7 @@ def alias(buf, nbytes, dtype, device):                       # numpy memory inst
 shard.alias = alias
 dist.init_process_group("gloo")
 rank, world = dist.get_rank(), dist.get_world_size()
-nx, ny, nz = 16, 12, 37
+nx, ny, nz = 16, 12, int(os.environ.get("SHARD_TEST_NZ", "37"))
 rng = np.random.default_rng(5)
 cube = (rng.standard_normal(nx * ny * nz) * 0.002 + 0.0005).astype(np.float32)
 cube[rng.integers(0, cube.size, 200)] = np.nan
@@ -152,13 +154,15 @@ def _free_port():
     return p
 
 
-@pytest.mark.parametrize("nproc", [2, 3])
-def test_sharded_driver_sequence_gloo(tmp_path, nproc):
+# (4, 3): world size 4 over 3 z-planes -- the last rank's slab is EMPTY (it presents no brick and all-gathers the
+# empty record left by cube_ooc_begin)
+@pytest.mark.parametrize("nproc,nz", [(2, 37), (3, 37), (4, 3)])
+def test_sharded_driver_sequence_gloo(tmp_path, nproc, nz):
     w = tmp_path / "worker.py"
     w.write_text(WORKER % {"root": ROOT} + WORKER_MAIN)
     cmd = [sys.executable, "-m", "torch.distributed.run", "--nnodes=1", "--nproc-per-node", str(nproc),
            "--master-addr", "127.0.0.1", "--master-port", str(_free_port()), str(w)]
-    env = dict(os.environ, MASTER_ADDR="127.0.0.1", OMP_NUM_THREADS="1")
+    env = dict(os.environ, MASTER_ADDR="127.0.0.1", OMP_NUM_THREADS="1", SHARD_TEST_NZ=str(nz))
     r = subprocess.run(cmd, cwd=ROOT, env=env, capture_output=True, text=True, timeout=300)
     assert r.returncode == 0, r.stderr[-3000:]
     line = [l for l in r.stdout.splitlines() if l.startswith("RESULT ")]
@@ -170,6 +174,9 @@ def test_sharded_driver_sequence_gloo(tmp_path, nproc):
         assert o["med_bits"] == o["ref_bits"]                                # exact lower median of the WHOLE cube
         assert o["bins_sum"] + sum(o["outside"]) == o["ref_count"]
         assert o["min"] == o["ref_min"] and o["max"] == o["ref_max"]
-        assert o["calls"] == ["begin", "pass0", "merge%d" % nproc, "advance", "pass1", "advance", "pass2", "advance"]
+        empty = o["slab"][0] == o["slab"][1]
+        assert o["calls"] == (["begin", "merge%d" % nproc, "advance", "advance", "advance"] if empty else
+                              ["begin", "pass0", "merge%d" % nproc, "advance", "pass1", "advance", "pass2", "advance"])
     assert [o["slab"][0] for o in res] == sorted(o["slab"][0] for o in res)
-    assert res[0]["slab"][0] == 0 and res[-1]["slab"][1] == 37
+    assert res[0]["slab"][0] == 0 and res[-1]["slab"][1] == nz
+    assert (nz >= nproc) or any(o["slab"][0] == o["slab"][1] for o in res)
