@@ -37,6 +37,24 @@ class Moments(ctypes.Structure):
                 ("mean", ctypes.c_double), ("std", ctypes.c_double)]
 
 
+class View(ctypes.Structure):
+    """oracle_view_t: origin, du, dv, step (data coordinates = voxel indices), width, height, nsteps."""
+    _fields_ = [("origin", ctypes.c_float * 3), ("du", ctypes.c_float * 3), ("dv", ctypes.c_float * 3),
+                ("step", ctypes.c_float * 3), ("width", ctypes.c_int32), ("height", ctypes.c_int32),
+                ("nsteps", ctypes.c_int32)]
+
+
+def _view(v):
+    """dict(origin, du, dv, step, width, height, nsteps) (cubegen.view_*) -> View."""
+    w = View()
+    for name in ("origin", "du", "dv", "step"):
+        a = np.asarray(v[name], dtype=np.float32)
+        for c in range(3):
+            getattr(w, name)[c] = float(a[c])
+    w.width, w.height, w.nsteps = int(v["width"]), int(v["height"]), int(v["nsteps"])
+    return w
+
+
 _lib = None
 
 
@@ -67,6 +85,14 @@ def lib():
         L.oracle_mad.argtypes = [fp, ctypes.c_uint64, fp, fp]
         L.oracle_minimap.argtypes = [fp] + [ctypes.c_int64] * 6 + [ctypes.c_int, mp]
         L.oracle_torben_capped.argtypes = [fp, ctypes.c_uint64, ctypes.c_int, fp, ctypes.POINTER(ctypes.c_int)]
+        L.oracle_minimap_median.argtypes = [fp] + [ctypes.c_int64] * 6 + [fp]
+        vwp = ctypes.POINTER(View)
+        i64 = ctypes.c_int64
+        L.oracle_trilinear.argtypes = [fp, i64, i64, i64, fp, fp]
+        L.oracle_spectrum.argtypes = [fp, i64, i64, i64, vwp, ctypes.c_int, ctypes.c_int, fp]
+        L.oracle_render_mip.argtypes = [fp, i64, i64, i64, vwp, ctypes.c_float, fp]
+        L.oracle_render_tf.argtypes = [fp, i64, i64, i64, vwp, ctypes.c_int, ctypes.c_float, ctypes.c_float, fp,
+                                       ctypes.c_float, fp]
         _lib = L
     return _lib
 
@@ -207,3 +233,65 @@ def torben_capped(a, max_iter):
     out, conv = ctypes.c_float(), ctypes.c_int()
     it = lib().oracle_torben_capped(p, a.size, int(max_iter), ctypes.byref(out), ctypes.byref(conv))
     return np.float32(out.value), it, bool(conv.value)
+
+
+def minimap_median(a, dims, part):
+    """Lower median of every mini-map cell (NaN for a cell without a non-NaN voxel) -> float32 [mz, my, mx]."""
+    a, p = _arr(a)
+    nx, ny, nz = dims
+    px, py, pz = part
+    assert a.size == nx * ny * nz
+    mx, my, mz = -(-nx // px), -(-ny // py), -(-nz // pz)
+    out = np.zeros(mx * my * mz, dtype=np.float32)
+    rc = lib().oracle_minimap_median(p, nx, ny, nz, px, py, pz, out.ctypes.data_as(ctypes.POINTER(ctypes.c_float)))
+    if rc != 0:
+        raise ValueError("oracle_minimap_median: invalid arguments")
+    return out.reshape(mz, my, mx)
+
+
+# ---- NEXT-4: ray casting (PAPER.md:162-180, 298-306).  dims = (nx, ny, nz), x fastest; view = cubegen.view_* dict.
+def trilinear(a, dims, point):
+    """Trilinear sample at the data coordinates ``point`` (float32 x, y, z) -> float32, or None when outside."""
+    a, p = _arr(a)
+    nx, ny, nz = dims
+    pt = (ctypes.c_float * 3)(*[float(np.float32(c)) for c in point])
+    out = ctypes.c_float()
+    ok = lib().oracle_trilinear(p, nx, ny, nz, pt, ctypes.byref(out))
+    return np.float32(out.value) if ok else None
+
+
+def spectrum(a, dims, view, u, v):
+    """3-D spectrum tool: the nsteps trilinear samples of pixel (u, v)'s ray (NaN outside the cube)."""
+    a, p = _arr(a)
+    nx, ny, nz = dims
+    w = _view(view)
+    out = np.zeros(w.nsteps, dtype=np.float32)
+    lib().oracle_spectrum(p, nx, ny, nz, ctypes.byref(w), int(u), int(v), out.ctypes.data_as(ctypes.POINTER(ctypes.c_float)))
+    return out
+
+
+def render_mip(a, dims, view, vmin=-np.inf):
+    """Maximum intensity projection -> float32 [height, width] (NaN: no sample >= vmin on the ray)."""
+    a, p = _arr(a)
+    nx, ny, nz = dims
+    w = _view(view)
+    out = np.zeros(w.width * w.height, dtype=np.float32)
+    lib().oracle_render_mip(p, nx, ny, nz, ctypes.byref(w), float(np.float32(vmin)),
+                            out.ctypes.data_as(ctypes.POINTER(ctypes.c_float)))
+    return out.reshape(w.height, w.width)
+
+
+def render_tf(a, dims, view, table, lo, hi, opacity_cut=2.0):
+    """Generic transfer function, front-to-back compositing.  table: [nlevels, 4] float32 (r, g, b, opacity).
+    -> float32 [height, width, 4] (opacity-weighted r, g, b and the accumulated opacity)."""
+    a, p = _arr(a)
+    nx, ny, nz = dims
+    w = _view(view)
+    t = np.ascontiguousarray(table, dtype=np.float32).reshape(-1, 4)
+    out = np.zeros(w.width * w.height * 4, dtype=np.float32)
+    fp = ctypes.POINTER(ctypes.c_float)
+    rc = lib().oracle_render_tf(p, nx, ny, nz, ctypes.byref(w), t.shape[0], float(np.float32(lo)), float(np.float32(hi)),
+                                t.ctypes.data_as(fp), float(np.float32(opacity_cut)), out.ctypes.data_as(fp))
+    if rc != 0:
+        raise ValueError("oracle_render_tf: invalid arguments")
+    return out.reshape(w.height, w.width, 4)

@@ -31,8 +31,13 @@
 //
 // Parity pins (tests/test_oracle_*.py): closed forms (constant cube, ramp 0..N-1, two-value
 // cube), exact rational sums computed with Python big integers, brute-force full sort on
-// tiny cubes, power-of-two ramp histograms, Table 1 of the paper.  The only unpinned
-// behaviour is +-Inf voxels in mean/std (R8): "parity unpinned" for that case.
+// tiny cubes, power-of-two ramp histograms, Table 1 of the paper.  +-Inf voxels: mean = std = NaN by
+// reading R8 (stated in oracle_moments, pinned in tests/test_oracle_pins.py).
+//
+//   ray casting: trilinear sample, maximum intensity
+//                       projection, generic transfer function with front-to-back compositing, 3-D spectrum
+//                       profile -- the march restated sample by sample at the end of this file
+//                       (readings R27-R32 of DESIGN.md; pins in tests/test_oracle_render_pins.py).
 //
 // Build: g++ -O2 -std=c++17 -ffp-contract=off -fno-fast-math -fPIC -shared (oracle/build.py).
 
@@ -415,6 +420,172 @@ int oracle_minimap(const float* d, int64_t nx, int64_t ny, int64_t nz, int64_t p
                             v.push_back(d[(z * ny + y) * nx + x]);
                 oracle_moments(v.data(), v.size(), sample_std, &cells[(cz * my + cy) * mx + cx]);
             }
+    return 0;
+}
+
+
+// Per-cell lower median of the mini-map (SURVEY.md sec. 8(f) NEXT-2 "mean/std (then median) per user partition";
+// PAPER.md:352 "each data point represents the data statistics of a bigger region"): the lower median
+// (k = (n-1)/2 over the cell's non-NaN voxels, reading R5) of every cell of oracle_minimap's partition; NaN for a cell
+// without a non-NaN voxel.
+int oracle_minimap_median(const float* d, int64_t nx, int64_t ny, int64_t nz, int64_t px, int64_t py, int64_t pz,
+                          float* med) {
+    if (nx <= 0 || ny <= 0 || nz <= 0 || px <= 0 || py <= 0 || pz <= 0) return 1;
+    const int64_t mx = (nx + px - 1) / px, my = (ny + py - 1) / py, mz = (nz + pz - 1) / pz;
+    std::vector<float> v;
+    for (int64_t cz = 0; cz < mz; ++cz)
+        for (int64_t cy = 0; cy < my; ++cy)
+            for (int64_t cx = 0; cx < mx; ++cx) {
+                v.clear();
+                for (int64_t z = cz * pz; z < std::min((cz + 1) * pz, nz); ++z)
+                    for (int64_t y = cy * py; y < std::min((cy + 1) * py, ny); ++y)
+                        for (int64_t x = cx * px; x < std::min((cx + 1) * px, nx); ++x)
+                            v.push_back(d[(z * ny + y) * nx + x]);
+                oracle_median(v.data(), v.size(), &med[(cz * my + cy) * mx + cx]);
+            }
+    return 0;
+}
+
+// ---------------------------------------------------------------------------------
+// NEXT-4: ray casting into a headless buffer -- the paper's volume rendering transfer
+// functions and its 3-D spectrum tool (Fig. 6: "evaluating the sampled data
+// points on an arbitrary ray with a constant sampling step ... in 3D with trilinear interpolation").  The paper
+// gives no formulas beyond that; the readings (R27-R32) are restated at each function.  Everything is
+// float32, one rounding per operation, no contraction (this file is built with -ffp-contract=off), in the order
+// written, so that a kernel doing the same operations in the same order gives the same bits.
+//
+// Geometry (R27): data coordinates are voxel indices, voxel (i,j,k) sits at (i,j,k); orthographic rays.  A view is
+//   origin[3], du[3], dv[3], step[3], width, height, nsteps:
+//   first sample of pixel (u,v):  o_c = (origin_c + (float)u * du_c) + (float)v * dv_c        c = x, y, z
+//   sample i of that ray:         p_c = o_c + (float)i * step_c,                              0 <= i < nsteps
+// A sample is INSIDE iff 0 <= p_x <= nx-1, 0 <= p_y <= ny-1 and 0 <= p_z <= nz-1 (tested on the float32 p).
+// ---------------------------------------------------------------------------------
+struct oracle_view_t {
+    float origin[3], du[3], dv[3], step[3];
+    int32_t width, height, nsteps;
+};
+
+static inline void oracle_ray_origin(const oracle_view_t* vw, int u, int v, float o[3]) {
+    for (int c = 0; c < 3; ++c) {
+        volatile float a = (float)u * vw->du[c];
+        volatile float b = vw->origin[c] + a;
+        volatile float e = (float)v * vw->dv[c];
+        o[c] = b + e;
+    }
+}
+static inline void oracle_ray_point(const oracle_view_t* vw, const float o[3], int i, float p[3]) {
+    for (int c = 0; c < 3; ++c) {
+        volatile float a = (float)i * vw->step[c];
+        p[c] = o[c] + a;
+    }
+}
+
+// Trilinear sample (R28; "trilinear interpolation to interpolate the data values ... from the original
+// data points"): x0 = floor(p_x), f_x = p_x - x0, x1 = x0 + 1 when f_x > 0 and x1 = x0 when f_x = 0 (a neighbour
+// of weight zero does not take part: a sample at a voxel centre IS that voxel, whatever lies next to it, and
+// p_x = nx - 1 needs no voxel beyond the cube); likewise y, z; interpolation along x, then y, then z, each step
+// a + f * (b - a).  Returns 0 and leaves *out alone when the point is outside.
+// A NULL (NaN) voxel among those that take part makes the sample NaN (IEEE propagation: the sample is NULL itself).
+int oracle_trilinear(const float* d, int64_t nx, int64_t ny, int64_t nz, const float p[3], float* out) {
+    if (!(p[0] >= 0.0f && p[0] <= (float)(nx - 1) && p[1] >= 0.0f && p[1] <= (float)(ny - 1) &&
+          p[2] >= 0.0f && p[2] <= (float)(nz - 1))) return 0;
+    const float flx = floorf(p[0]), fly = floorf(p[1]), flz = floorf(p[2]);
+    const int64_t x0 = (int64_t)flx, y0 = (int64_t)fly, z0 = (int64_t)flz;
+    const float fx = p[0] - flx, fy = p[1] - fly, fz = p[2] - flz;
+    const int64_t x1 = x0 + (fx > 0.0f ? 1 : 0), y1 = y0 + (fy > 0.0f ? 1 : 0), z1 = z0 + (fz > 0.0f ? 1 : 0);
+    auto at = [&](int64_t x, int64_t y, int64_t z) { return d[(z * ny + y) * nx + x]; };
+    auto lerp = [](float a, float b, float f) {
+        volatile float diff = b - a;
+        volatile float prod = f * diff;
+        return a + prod;
+    };
+    const float c00 = lerp(at(x0, y0, z0), at(x1, y0, z0), fx);
+    const float c10 = lerp(at(x0, y1, z0), at(x1, y1, z0), fx);
+    const float c01 = lerp(at(x0, y0, z1), at(x1, y0, z1), fx);
+    const float c11 = lerp(at(x0, y1, z1), at(x1, y1, z1), fx);
+    const float c0 = lerp(c00, c10, fy);
+    const float c1 = lerp(c01, c11, fy);
+    *out = lerp(c0, c1, fz);
+    return 1;
+}
+
+// 3-D spectrum tool: the data profile along the line of sight of pixel (u,v): out[i] = the
+// trilinear sample at sample i, NaN where the sample is outside the cube (or NULL).
+int oracle_spectrum(const float* d, int64_t nx, int64_t ny, int64_t nz, const oracle_view_t* vw, int u, int v,
+                    float* out) {
+    float o[3], p[3];
+    oracle_ray_origin(vw, u, v, o);
+    for (int i = 0; i < vw->nsteps; ++i) {
+        oracle_ray_point(vw, o, i, p);
+        float s;
+        out[i] = oracle_trilinear(d, nx, ny, nz, p, &s) ? s : std::numeric_limits<float>::quiet_NaN();
+    }
+    return 0;
+}
+
+// Maximum intensity projection ("only the value of the maximum voxel through each cast ray is
+// shown for each pixel"; "the minimum data value" as a global threshold): image[v*width + u] = the largest sample of
+// the ray among those that are inside, not NULL and >= vmin, taken in march order with  if (s > m) m = s  (R29);
+// NaN when the ray has no such sample.
+int oracle_render_mip(const float* d, int64_t nx, int64_t ny, int64_t nz, const oracle_view_t* vw, float vmin,
+                      float* image) {
+    for (int v = 0; v < vw->height; ++v)
+        for (int u = 0; u < vw->width; ++u) {
+            float o[3], p[3], m = 0.0f;
+            bool have = false;
+            oracle_ray_origin(vw, u, v, o);
+            for (int i = 0; i < vw->nsteps; ++i) {
+                oracle_ray_point(vw, o, i, p);
+                float s;
+                if (!oracle_trilinear(d, nx, ny, nz, p, &s)) continue;
+                if (!(s >= vmin)) continue;                     // NULL samples fail the comparison
+                if (!have || s > m) { m = s; have = true; }
+            }
+            image[(size_t)v * vw->width + u] = have ? m : std::numeric_limits<float>::quiet_NaN();
+        }
+    return 0;
+}
+
+// Generic transfer function ("The data values' range is partitioned into discrete levels.  Each
+// data level is assigned a colour and opacity value ... from 0 to 1"), ordered front-to-back compositing (Levoy 1988,
+// as the paper cites).  R30: level of a sample s with lo <= s (NULL and s < lo: skipped -- the global threshold of
+// PAPER.md:170, 344):  L = min(floor((s - lo) * scale), nlevels - 1), scale = (float)nlevels / (hi - lo), every
+// operation float32 -- the histogram's bin formula (R10, R11) with everything above hi in the top level (hi == lo:
+// level 0).  R31: with table[L] = (r, g, b, a), accumulated colour C and opacity A start at 0 and per sample
+//     w = (1 - A) * a;   C_c = C_c + w * c_c  (c = r, g, b);   A = A + w;   stop the ray when A >= opacity_cut.
+// rgba[(v*width + u)*4 ..] = (C_r, C_g, C_b, A): opacity-weighted (premultiplied) colour.
+int oracle_render_tf(const float* d, int64_t nx, int64_t ny, int64_t nz, const oracle_view_t* vw, int nlevels,
+                     float lo, float hi, const float* table, float opacity_cut, float* rgba) {
+    if (nlevels < 1 || !(lo <= hi)) return 1;
+    volatile float width = hi - lo;
+    volatile float scale_v = (hi == lo) ? 0.0f : (float)nlevels / width;
+    const float scale = scale_v;
+    for (int v = 0; v < vw->height; ++v)
+        for (int u = 0; u < vw->width; ++u) {
+            float o[3], p[3], C[3] = {0.0f, 0.0f, 0.0f}, A = 0.0f;
+            oracle_ray_origin(vw, u, v, o);
+            for (int i = 0; i < vw->nsteps; ++i) {
+                oracle_ray_point(vw, o, i, p);
+                float s;
+                if (!oracle_trilinear(d, nx, ny, nz, p, &s)) continue;
+                if (!(s >= lo)) continue;
+                volatile float t = s - lo;
+                volatile float q = t * scale;
+                float fl = floorf(q);
+                int L = (fl >= (float)(nlevels - 1)) ? nlevels - 1 : (int)fl;
+                const float* e = table + 4 * (size_t)L;
+                volatile float rem = 1.0f - A;
+                volatile float w = rem * e[3];
+                for (int c = 0; c < 3; ++c) {
+                    volatile float wc = w * e[c];
+                    C[c] = C[c] + wc;
+                }
+                A = A + w;
+                if (A >= opacity_cut) break;
+            }
+            float* px = rgba + 4 * ((size_t)v * vw->width + u);
+            px[0] = C[0]; px[1] = C[1]; px[2] = C[2]; px[3] = A;
+        }
     return 0;
 }
 
