@@ -270,6 +270,50 @@ int cube_minimap_dims(int64_t nx, int64_t ny, int64_t nz, int64_t px, int64_t py
 int cube_minimap(cube_ctx* ctx, const float* d, int64_t nx, int64_t ny, int64_t nz, int64_t px, int64_t py,
                  int64_t pz, unsigned flags, cube_moments_t* cells, cudaStream_t stream);
 
+/* ---- NEXT-4: volume ray casting and the 3-D spectrum tool as compute kernels writing into
+ * headless buffers (the paper's renderer is CUDA as well; its viewer / window is left out).
+ * Geometry (R27): data coordinates are voxel indices -- voxel (i,j,k) sits at (i,j,k) -- and the rays are
+ * orthographic.  With every operation a float32 operation in the order written,
+ *     first sample of pixel (u,v):  o = (origin + (float)u * du) + (float)v * dv
+ *     sample i of that ray:         p = o + (float)i * step,   0 <= i < nsteps
+ * a sample is inside iff 0 <= p_x <= nx-1, 0 <= p_y <= ny-1, 0 <= p_z <= nz-1, and its value is the trilinear
+ * interpolation of the (up to) eight surrounding voxels, x then y then z, each step a + f * (b - a) (R28);
+ * a neighbour of weight zero does not take part; a NULL (NaN) voxel among those that do makes the sample NULL.
+ * Every dimension must be <= 2^24 (coordinates are float32).  The cube is never written. */
+typedef struct {
+    float origin[3], du[3], dv[3], step[3];
+    int32_t width, height, nsteps;
+} cube_view_t;
+
+/* A camera orbiting the cube's centre (host-side convenience, no device work): viewing direction -z turned by
+ * pitch about x, then by yaw about y (degrees); the image spans the bounding sphere of the cube, rays start on its
+ * near side and take ceil(diameter / step) + 1 samples `step` voxels apart.  PAPER.md:400 ("2 degrees steps"). */
+int cube_view_orbit(int64_t nx, int64_t ny, int64_t nz, double yaw_deg, double pitch_deg, int width, int height,
+                    double step, cube_view_t* out);
+
+/* Maximum intensity projection: image[v * width + u] = the largest sample of the ray of pixel
+ * (u,v) among those inside the cube, not NULL and >= vmin (-INFINITY: no threshold; "the minimum data
+ * value ... as a global thresholding technique"); NaN when there is none.  `image`: width * height floats the DEVICE
+ * can write (device or pinned host memory).  `view` is a HOST pointer read before the call returns. */
+int cube_render_mip(cube_ctx* ctx, const float* d, int64_t nx, int64_t ny, int64_t nz, const cube_view_t* view,
+                    float vmin, float* image, cudaStream_t stream);
+
+/* Generic transfer function with ordered front-to-back compositing (R30, R31).
+ * table[L] = (r, g, b, opacity in [0,1]) for data level L < nlevels (1 <= nlevels <= 4096; host or device memory);
+ * level of a sample s >= lo:  L = min(floor((s - lo) * ((float)nlevels / (hi - lo))), nlevels - 1) -- the histogram's
+ * bin formula with everything above hi in the top level; samples below lo and NULL samples are skipped.  Per sample
+ *     w = (1 - A) * a_L;   C = C + w * c_L;   A = A + w;   the ray stops once A >= opacity_cut (> 1: never).
+ * rgba[(v * width + u) * 4 ...] = (C_r, C_g, C_b, A): opacity-weighted colour; device-writable memory, 16-byte aligned. */
+int cube_render_tf(cube_ctx* ctx, const float* d, int64_t nx, int64_t ny, int64_t nz, const cube_view_t* view,
+                   int nlevels, float lo, float hi, const float* table, float opacity_cut, float* rgba,
+                   cudaStream_t stream);
+
+/* 3-D spectrum tool (Fig. 6): out[i] = sample i of the ray of pixel (u,v) (any integers: the
+ * pixel need not lie inside the image), NaN where the sample is outside the cube or NULL; nsteps floats,
+ * device-writable memory. */
+int cube_spectrum(cube_ctx* ctx, const float* d, int64_t nx, int64_t ny, int64_t nz, const cube_view_t* view,
+                  int u, int v, float* out, cudaStream_t stream);
+
 const char* cube_strerror(int code);
 int cube_last_cuda_error(const cube_ctx* ctx);
 
@@ -315,7 +359,8 @@ enum {
     CUBE_K_MOMENTS_WINDOW = 11, /* moments_kernel<window>: cube_clipped_moments, cube_sigma_clip passes */
     CUBE_K_MINIMAP = 12,        /* minimap_kernel */
     CUBE_K_TORBEN = 13,         /* torben_pass_kernel (cube_median_torben) */
-    CUBE_K_KINDS = 14
+    CUBE_K_RENDER = 14,         /* render_mip_kernel / render_tf_kernel / spectrum_kernel */
+    CUBE_K_KINDS = 15
 };
 int cube_profile_enable(cube_ctx* ctx, int on);
 /* Read-only STREAM probe: streams nvox float32 voxels through the same loop as the statistics kernels with one

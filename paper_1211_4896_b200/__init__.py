@@ -33,11 +33,13 @@ SYMBOLS = ["cube_create", "cube_destroy", "cube_moments", "cube_histogram", "cub
            "cube_last_cuda_error", "cube_set_launch", "cube_set_knob", "cube_launch_count",
            "cube_profile_enable", "cube_profile_reset", "cube_profile_read",
            "cube_mad", "cube_clipped_moments", "cube_sigma_clip", "cube_minimap_dims", "cube_minimap",
-           "cube_shard_buffers", "cube_shard_merge_records", "cube_shard_advance", "cube_median_torben"]
+           "cube_shard_buffers", "cube_shard_merge_records", "cube_shard_advance", "cube_median_torben",
+           "cube_view_orbit", "cube_render_mip", "cube_render_tf", "cube_spectrum"]
 SHARD_RECORD_BYTES, SHARD_DIGITS = 40, 8192
 KNOB_CTAS_PER_SM, KNOB_BIGHIST, KNOB_MINIMAP = 0, 1, 2
 KIND_NAMES = ["moments", "moments_coarse", "histogram", "select_pass0", "select_pass1", "select_pass2",
-              "select_cand", "select_scan", "hist_select", "probe_read", "other", "moments_window", "minimap", "torben_pass"]
+              "select_cand", "select_scan", "hist_select", "probe_read", "other", "moments_window", "minimap", "torben_pass",
+              "render"]
 
 
 class CubeError(RuntimeError):
@@ -59,6 +61,30 @@ class MomentsT(ctypes.Structure):
 class ShardBuffersT(ctypes.Structure):
     _fields_ = [("record", ctypes.c_void_p), ("bins", ctypes.c_void_p), ("outside", ctypes.c_void_p),
                 ("digits", ctypes.c_void_p)]
+
+
+class ViewT(ctypes.Structure):
+    """cube_view_t (include/cube.h): orthographic rays in data coordinates."""
+    _fields_ = [("origin", ctypes.c_float * 3), ("du", ctypes.c_float * 3), ("dv", ctypes.c_float * 3),
+                ("step", ctypes.c_float * 3), ("width", ctypes.c_int32), ("height", ctypes.c_int32),
+                ("nsteps", ctypes.c_int32)]
+
+    @classmethod
+    def from_dict(cls, v):
+        """dict(origin, du, dv, step (3 floats each), width, height, nsteps) -> ViewT (marshalling only)."""
+        if isinstance(v, cls):
+            return v
+        w = cls()
+        for name in ("origin", "du", "dv", "step"):
+            for c in range(3):
+                getattr(w, name)[c] = float(v[name][c])
+        w.width, w.height, w.nsteps = int(v["width"]), int(v["height"]), int(v["nsteps"])
+        return w
+
+    def as_dict(self):
+        d = {k: np.array(list(getattr(self, k)), dtype=np.float32) for k in ("origin", "du", "dv", "step")}
+        d.update(width=int(self.width), height=int(self.height), nsteps=int(self.nsteps))
+        return d
 
 
 # record layout of cube_moments_t as a numpy dtype (mini-map cells)
@@ -116,6 +142,11 @@ def load():
     L.cube_minimap_dims.argtypes = [i64] * 6 + [ctypes.POINTER(i64)] * 3
     L.cube_minimap.argtypes = [vp, vp, i64, i64, i64, i64, i64, i64, cu, vp, vp]
     L.cube_median_torben.argtypes = [vp, vp, i64, i64, i64, ci, vp, vp, vp, vp]
+    vwp = ctypes.POINTER(ViewT)
+    L.cube_view_orbit.argtypes = [i64, i64, i64, f64, f64, ci, ci, f64, vwp]
+    L.cube_render_mip.argtypes = [vp, vp, i64, i64, i64, vwp, f32, vp, vp]
+    L.cube_render_tf.argtypes = [vp, vp, i64, i64, i64, vwp, ci, f32, f32, vp, f32, vp, vp]
+    L.cube_spectrum.argtypes = [vp, vp, i64, i64, i64, vwp, ci, ci, vp, vp]
     L.cube_shard_buffers.argtypes = [vp, ctypes.POINTER(ShardBuffersT)]
     L.cube_shard_merge_records.argtypes = [vp, vp, ci, cu, vp]
     L.cube_shard_advance.argtypes = [vp, ctypes.POINTER(ci), vp]
@@ -299,6 +330,35 @@ class Context:
     def minimap(self, d, nx, ny, nz, px, py, pz, cells, flags=0, stream=0):
         """cube_minimap: ``cells`` = device (or pinned) buffer of mx*my*mz records of 40 bytes (MINIMAP_DTYPE)."""
         self._check(self._L.cube_minimap(self._h, _ptr(d), nx, ny, nz, px, py, pz, flags, _ptr(cells), stream))
+
+    # --- NEXT-4: ray casting into headless buffers (SURVEY.md sec. 8(f); PAPER.md:162-180, 298-306) --------
+    def view_orbit(self, nx, ny, nz, yaw_deg, pitch_deg, width, height, step=1.0):
+        """cube_view_orbit -> ViewT (host-side geometry, no device work)."""
+        w = ViewT()
+        self._check(self._L.cube_view_orbit(nx, ny, nz, yaw_deg, pitch_deg, width, height, step, ctypes.byref(w)))
+        return w
+
+    def render_mip(self, d, nx, ny, nz, view, image, vmin=float("-inf"), stream=0):
+        """cube_render_mip: ``image`` = device (or pinned) buffer of width * height floats."""
+        w = ViewT.from_dict(view)
+        self._check(self._L.cube_render_mip(self._h, _ptr(d), nx, ny, nz, ctypes.byref(w), vmin, _ptr(image), stream))
+
+    def render_tf(self, d, nx, ny, nz, view, table, lo, hi, rgba, opacity_cut=2.0, stream=0):
+        """cube_render_tf: ``table`` = [nlevels, 4] float32 (numpy array or device tensor); ``rgba`` = device (or
+        pinned) buffer of width * height * 4 floats."""
+        w = ViewT.from_dict(view)
+        if isinstance(table, np.ndarray):
+            table = np.ascontiguousarray(table, dtype=np.float32)
+            nlevels = table.size // 4
+        else:
+            nlevels = table.numel() // 4
+        self._check(self._L.cube_render_tf(self._h, _ptr(d), nx, ny, nz, ctypes.byref(w), nlevels, lo, hi, _ptr(table),
+                                           opacity_cut, _ptr(rgba), stream))
+
+    def spectrum(self, d, nx, ny, nz, view, u, v, out, stream=0):
+        """cube_spectrum: ``out`` = device (or pinned) buffer of nsteps floats."""
+        w = ViewT.from_dict(view)
+        self._check(self._L.cube_spectrum(self._h, _ptr(d), nx, ny, nz, ctypes.byref(w), u, v, _ptr(out), stream))
 
     def probe_read(self, d, nvox, stream=0):
         self._check(self._L.cube_probe_read(self._h, _ptr(d), nvox, stream))

@@ -12,6 +12,7 @@
 
 #include "cube_kernels.cuh"
 #include "cube_minimap_tma.cuh"
+#include "cube_render.cuh"
 #include "cube_select_multi.cuh"
 
 using namespace cube;
@@ -43,6 +44,7 @@ struct cube_ctx {
     ClipState* clip = nullptr;             // sigma-clip loop state (NEXT-1)
     TorbenState* torben = nullptr;         // Alg. 1 loop state (cube_median_torben)
     float* center = nullptr;               // cube_mad: the median the deviations are taken from
+    float4* tf_table = nullptr;            // cube_render_tf: device copy of a host transfer-function table (4096 levels)
     uint32_t* cand = nullptr;              // candidate keys of the select (step 8)
     unsigned long long cand_cap = 0;       // in keys
     // out-of-core state (host side)
@@ -374,6 +376,7 @@ int cube_create(cube_ctx** out, size_t scratch_bytes_hint) {
     ok = ok && cudaMalloc(&c->clip, sizeof(ClipState)) == cudaSuccess;
     ok = ok && cudaMalloc(&c->torben, sizeof(TorbenState)) == cudaSuccess;
     ok = ok && cudaMalloc(&c->center, sizeof(float)) == cudaSuccess;
+    ok = ok && cudaMalloc(&c->tf_table, 4096 * sizeof(float4)) == cudaSuccess;
     ok = ok && cudaMemset(c->plan, 0, sizeof(BigHistPlan)) == cudaSuccess;
     ok = ok && cudaMemset(c->ticket, 0, sizeof(unsigned int)) == cudaSuccess;
     ok = ok && cudaMemset(c->gdigits, 0, kDigitBins * sizeof(unsigned long long)) == cudaSuccess;
@@ -406,7 +409,7 @@ int cube_destroy(cube_ctx* c) {
     cudaFree(c->partials); cudaFree(c->ticket); cudaFree(c->ticket2); cudaFree(c->acc);
     cudaFree(c->mom_out); cudaFree(c->gout); cudaFree(c->gdigits); cudaFree(c->coarse); cudaFree(c->sel); cudaFree(c->multi);
     cudaFree(c->range3); cudaFree(c->probe_out); cudaFree(c->plan); cudaFree(c->clip); cudaFree(c->torben); cudaFree(c->center);
-    cudaFree(c->cand);
+    cudaFree(c->cand); cudaFree(c->tf_table);
     cudaFree(c->resident); cudaFree(c->chunk[0]); cudaFree(c->chunk[1]);
     if (c->pinned_results) cudaFreeHost(c->pinned_results);
     for (int i = 0; i < cube_ctx::kMaxStage; ++i) {
@@ -752,6 +755,105 @@ int cube_minimap(cube_ctx* c, const float* d, int64_t nx, int64_t ny, int64_t nz
                                                                  reinterpret_cast<MomentsOut*>(cells));
         else minimap_kernel<<<grid, kMapThreads, 0, s>>>(d, g, flags & CUBE_SAMPLE_STD,
                                                          reinterpret_cast<MomentsOut*>(cells));
+    }
+    CUBE_CUDA(c, cudaGetLastError());
+    return CUBE_OK;
+}
+
+// ---- NEXT-4: ray casting (cube_render.cuh)
+static bool render_args(cube_ctx* c, const float* d, int64_t nx, int64_t ny, int64_t nz, const cube_view_t* view,
+                        void* out, RenderGeom* g, RenderView* vw) {
+    uint64_t n;
+    if (!c || !d || !view || !out || !dims_ok(nx, ny, nz, &n)) return false;
+    if (nx > (1 << 24) || ny > (1 << 24) || nz > (1 << 24)) return false;      // float32 coordinates
+    if (view->width < 1 || view->height < 1 || view->nsteps < 1) return false;
+    if ((long double)view->width * (long double)view->height > 1073741824.0L) return false;
+    for (int k = 0; k < 3; ++k)
+        if (!isfinite(view->origin[k]) || !isfinite(view->du[k]) || !isfinite(view->dv[k]) || !isfinite(view->step[k])) return false;
+    cudaPointerAttributes at;   // images are written in place by the kernels
+    if (cudaPointerGetAttributes(&at, out) != cudaSuccess || at.type == cudaMemoryTypeUnregistered) {
+        cudaGetLastError();
+        return false;
+    }
+    static_assert(sizeof(cube_view_t) == sizeof(RenderView), "view layout");
+    memcpy(vw, view, sizeof(RenderView));
+    g->nx = nx; g->ny = ny; g->nz = nz;
+    g->xmax = (float)(nx - 1); g->ymax = (float)(ny - 1); g->zmax = (float)(nz - 1);
+    return true;
+}
+
+int cube_view_orbit(int64_t nx, int64_t ny, int64_t nz, double yaw_deg, double pitch_deg, int width, int height,
+                    double step, cube_view_t* out) {
+    uint64_t n;
+    if (!out || !dims_ok(nx, ny, nz, &n) || width < 1 || height < 1 || !(step > 0.0) || !isfinite(step) ||
+        !isfinite(yaw_deg) || !isfinite(pitch_deg)) return CUBE_EINVAL;
+    const double pi = 3.14159265358979323846;
+    const double ya = yaw_deg * pi / 180.0, pa = pitch_deg * pi / 180.0;
+    const double cy = cos(ya), sy = sin(ya), cp = cos(pa), sp = sin(pa);
+    // R = Ry(yaw) Rx(pitch); right = R e_x, up = R e_y, forward = R (-e_z)
+    const double right[3] = {cy, 0.0, -sy};
+    const double up[3] = {sy * sp, cp, cy * sp};
+    const double fwd[3] = {-sy * cp, sp, -cy * cp};
+    const double ctr[3] = {(nx - 1) / 2.0, (ny - 1) / 2.0, (nz - 1) / 2.0};
+    const double diam = sqrt((nx - 1.0) * (nx - 1.0) + (ny - 1.0) * (ny - 1.0) + (nz - 1.0) * (nz - 1.0)) + 1.0;
+    const double nsteps = ceil(diam / step) + 1.0;
+    if (nsteps > 2147483000.0) return CUBE_EINVAL;
+    for (int k = 0; k < 3; ++k) {
+        const double du = right[k] * (diam / width), dv = up[k] * (diam / height);
+        out->du[k] = (float)du;
+        out->dv[k] = (float)dv;
+        out->step[k] = (float)(fwd[k] * step);
+        out->origin[k] = (float)(ctr[k] - fwd[k] * (diam / 2) - right[k] * (diam / 2) - up[k] * (diam / 2) + 0.5 * du + 0.5 * dv);
+    }
+    out->width = width; out->height = height; out->nsteps = (int32_t)nsteps;
+    return CUBE_OK;
+}
+
+int cube_render_mip(cube_ctx* c, const float* d, int64_t nx, int64_t ny, int64_t nz, const cube_view_t* view,
+                    float vmin, float* image, cudaStream_t s) {
+    RenderGeom g; RenderView vw;
+    if (!render_args(c, d, nx, ny, nz, view, image, &g, &vw) || vmin != vmin) return CUBE_EINVAL;
+    {
+        ProfScope prof(c, CUBE_K_RENDER, s);
+        const dim3 block(kRenderTileU, kRenderTileV);
+        const dim3 grid((vw.width + kRenderTileU - 1) / kRenderTileU, (vw.height + kRenderTileV - 1) / kRenderTileV);
+        render_mip_kernel<<<grid, block, 0, s>>>(d, g, vw, vmin, image);
+    }
+    CUBE_CUDA(c, cudaGetLastError());
+    return CUBE_OK;
+}
+
+int cube_render_tf(cube_ctx* c, const float* d, int64_t nx, int64_t ny, int64_t nz, const cube_view_t* view,
+                   int nlevels, float lo, float hi, const float* table, float opacity_cut, float* rgba, cudaStream_t s) {
+    RenderGeom g; RenderView vw;
+    if (!render_args(c, d, nx, ny, nz, view, rgba, &g, &vw) || !table || nlevels < 1 || nlevels > 4096) return CUBE_EINVAL;
+    if (opacity_cut != opacity_cut || ((uintptr_t)rgba & 15u)) return CUBE_EINVAL;
+    float scale;
+    if (!hist_scale(nlevels, lo, hi, &scale)) return CUBE_EINVAL;     // the histogram's scale (R10, R13, R19)
+    const float4* dev_table = static_cast<const float4*>(device_reachable(c, const_cast<float*>(table)));
+    if (!dev_table || ((uintptr_t)dev_table & 15u)) {
+        CUBE_CUDA(c, cudaMemcpyAsync(c->tf_table, table, (size_t)nlevels * sizeof(float4), cudaMemcpyDefault, s));
+        dev_table = c->tf_table;
+    }
+    {
+        ProfScope prof(c, CUBE_K_RENDER, s);
+        const dim3 block(kRenderTileU, kRenderTileV);
+        const dim3 grid((vw.width + kRenderTileU - 1) / kRenderTileU, (vw.height + kRenderTileV - 1) / kRenderTileV);
+        render_tf_kernel<<<grid, block, 0, s>>>(d, g, vw, nlevels, lo, scale, dev_table, opacity_cut,
+                                                reinterpret_cast<float4*>(rgba));
+    }
+    CUBE_CUDA(c, cudaGetLastError());
+    return CUBE_OK;
+}
+
+int cube_spectrum(cube_ctx* c, const float* d, int64_t nx, int64_t ny, int64_t nz, const cube_view_t* view, int u,
+                  int v, float* out, cudaStream_t s) {
+    RenderGeom g; RenderView vw;
+    if (!render_args(c, d, nx, ny, nz, view, out, &g, &vw)) return CUBE_EINVAL;
+    if (u < -(1 << 24) || u > (1 << 24) || v < -(1 << 24) || v > (1 << 24)) return CUBE_EINVAL;
+    {
+        ProfScope prof(c, CUBE_K_RENDER, s);
+        spectrum_kernel<<<(vw.nsteps + 255) / 256, 256, 0, s>>>(d, g, vw, u, v, out);
     }
     CUBE_CUDA(c, cudaGetLastError());
     return CUBE_OK;
