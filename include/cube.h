@@ -143,12 +143,17 @@ int cube_stats(cube_ctx* ctx, const float* d, int64_t nx, int64_t ny, int64_t nz
 /* ---- Out-of-core / streamed cubes (north_star (4); the paper is in-core by design).
  * The cube is presented brick by brick (any split into contiguous runs of voxels); each brick is a device
  * buffer the caller has filled (e.g. by cudaMemcpyAsync from pinned host memory on a side stream).
- * Sweep 1 accumulates moments + histogram + the first select digit; each further sweep (the caller
- * re-presents all bricks) refines the median by one digit.  cube_ooc_next_sweep() tells whether another
- * sweep is needed: *more = 1 until the median is exact: 2 sweeps when the median's first-digit bucket fits the
- * candidate buffer (the second sweep compacts it), else 3; 1 if want_median == 0.  The call after sweep 2
- * synchronises `stream` once to read that decision. */
+ * With the median the bricks are read TWICE, like the cube in cube_stats (8 B per voxel): sweep 1 = moments + first
+ * select digit (fused pass A), sweep 2 = histogram + second digit + candidate compaction (fused pass B), then the
+ * last digit on the candidates; a third sweep only if the median's first-digit bucket did not fit the candidate
+ * buffer.  Without the median: one sweep, moments + histogram.  cube_ooc_next_sweep() tells whether another sweep
+ * is needed (*more); the call after sweep 2 synchronises `stream` once to read the "did it fit" decision. */
 int cube_ooc_begin(cube_ctx* ctx, int nbins, float lo, float hi, int want_median, cudaStream_t stream);
+/* flags: CUBE_RANGE_MINMAX = histogram over [data min, data max] (lo/hi ignored): the range is that of the running
+ * record after sweep 1 (in a sharded run: after cube_shard_merge_records), never leaves the device, and the
+ * histogram is accumulated in sweep 2 -- which then exists even without the median.  Unusable range: as cube_stats. */
+int cube_ooc_begin_ex(cube_ctx* ctx, int nbins, float lo, float hi, int want_median, unsigned flags,
+                      cudaStream_t stream);
 int cube_ooc_brick(cube_ctx* ctx, const float* d_brick, uint64_t nvox, cudaStream_t stream);
 int cube_ooc_next_sweep(cube_ctx* ctx, int* more, cudaStream_t stream);
 int cube_ooc_result(cube_ctx* ctx, unsigned flags, cube_moments_t* moments, uint64_t* bins, uint64_t* outside,
@@ -162,14 +167,17 @@ int cube_ooc_result(cube_ctx* ctx, unsigned flags, cube_moments_t* moments, uint
  * cube_shard_advance() then locates the bucket on the combined counts.  Per stage (three for an exact median, one
  * without):
  *     cube_ooc_brick(slab)                                   every rank, its own voxels (several bricks allowed)
- *     stage 0 only:  all-gather `record` (CUBE_SHARD_RECORD_BYTES per rank) -> cube_shard_merge_records();
+ *     stage 0 only:  all-gather `record` (CUBE_SHARD_RECORD_BYTES per rank) -> cube_shard_merge_records()
+ *     the stage that accumulates the histogram (stage 1 with the median or CUBE_RANGE_MINMAX, else stage 0):
  *                    all-reduce SUM `bins` (nbins x u64) and `outside` (2 x u64)
- *     every stage:   all-reduce SUM `digits` (CUBE_SHARD_DIGITS x u64)
+ *     every stage with the median:   all-reduce SUM `digits` (CUBE_SHARD_DIGITS x u64)
  *     cube_shard_advance(&more)
  * then cube_ooc_result() on any rank: every rank holds the same integers and, because the records are merged in
  * rank order on every rank, the same mean / std bits.  Three rounds of 64 KiB instead of the paper's ~31 rounds of
- * five scalars.  In stage 2 each rank counts the last digit on its own compacted candidates
- * (or re-reads its slab when they did not fit): decided on the device, no host synchronisation anywhere. */
+ * five scalars.  Every rank reads its slab twice (8 B per voxel).  Each rank counts the last digit
+ * on its own compacted candidates ONCE, inside the cube_shard_advance() that ends stage 1; the bricks it presents in
+ * stage 2 are read only when the candidates did not fit: decided on the device, no host synchronisation anywhere.
+ * A rank without voxels (more ranks than z-planes) presents no brick and still takes part in every collective. */
 #define CUBE_SHARD_RECORD_BYTES 40
 #define CUBE_SHARD_DIGITS 8192
 typedef struct {

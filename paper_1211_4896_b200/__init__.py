@@ -27,7 +27,7 @@ MAX_BINS = 65536
 
 # every symbol include/cube.h declares (checked by tests/test_abi.py)
 SYMBOLS = ["cube_create", "cube_destroy", "cube_moments", "cube_histogram", "cube_kth", "cube_kth_ex", "cube_kth_multi",
-           "cube_median", "cube_median_ex", "cube_stats", "cube_probe_read", "cube_ooc_begin", "cube_ooc_brick", "cube_ooc_next_sweep",
+           "cube_median", "cube_median_ex", "cube_stats", "cube_probe_read", "cube_ooc_begin", "cube_ooc_begin_ex", "cube_ooc_brick", "cube_ooc_next_sweep",
            "cube_ooc_result", "cube_host_workspace", "cube_stats_host", "cube_stream_workspace", "cube_stats_stream",
            "cube_stream_info", "cube_strerror",
            "cube_last_cuda_error", "cube_set_launch", "cube_set_knob", "cube_launch_count",
@@ -117,6 +117,7 @@ def load():
     L.cube_stats.argtypes = [vp, vp, i64, i64, i64, ci, f32, f32, cu, vp, vp, vp, vp, vp]
     L.cube_probe_read.argtypes = [vp, vp, u64, vp]
     L.cube_ooc_begin.argtypes = [vp, ci, f32, f32, ci, vp]
+    L.cube_ooc_begin_ex.argtypes = [vp, ci, f32, f32, ci, cu, vp]
     L.cube_ooc_brick.argtypes = [vp, vp, u64, vp]
     L.cube_ooc_next_sweep.argtypes = [vp, ctypes.POINTER(ci), vp]
     L.cube_ooc_result.argtypes = [vp, cu, vp, vp, vp, vp, vp]
@@ -364,8 +365,8 @@ class Context:
         self._check(self._L.cube_probe_read(self._h, _ptr(d), nvox, stream))
 
     # --- brick-streamed (out-of-core) ------------------------------------------------------------------
-    def ooc_begin(self, nbins, lo, hi, want_median=True, stream=0):
-        self._check(self._L.cube_ooc_begin(self._h, nbins, lo, hi, int(bool(want_median)), stream))
+    def ooc_begin(self, nbins, lo, hi, want_median=True, stream=0, flags=0):
+        self._check(self._L.cube_ooc_begin_ex(self._h, nbins, lo, hi, int(bool(want_median)), flags, stream))
 
     def ooc_brick(self, d_brick, nvox, stream=0):
         self._check(self._L.cube_ooc_brick(self._h, _ptr(d_brick), nvox, stream))

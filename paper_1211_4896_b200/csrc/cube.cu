@@ -50,6 +50,7 @@ struct cube_ctx {
     // out-of-core state (host side)
     int ooc_active = 0, ooc_sweep = 0, ooc_nbins = 0, ooc_want_median = 0, ooc_bricks = 0;
     float ooc_lo = 0.f, ooc_hi = 0.f, ooc_scale = 0.f;
+    int ooc_minmax = 0;                    // CUBE_RANGE_MINMAX: histogram over [min, max], in sweep 1
     // host-cube driver workspace
     float* resident = nullptr;
     size_t resident_bytes = 0;

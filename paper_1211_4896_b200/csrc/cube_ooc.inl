@@ -8,9 +8,16 @@
 extern "C" {
 
 int cube_ooc_begin(cube_ctx* c, int nbins, float lo, float hi, int want_median, cudaStream_t s) {
+    return cube_ooc_begin_ex(c, nbins, lo, hi, want_median, 0u, s);
+}
+
+int cube_ooc_begin_ex(cube_ctx* c, int nbins, float lo, float hi, int want_median, unsigned flags, cudaStream_t s) {
     if (!c) return CUBE_EINVAL;
     float scale = 0.f;
-    if (nbins != 0 && !hist_scale(nbins, lo, hi, &scale)) return CUBE_EINVAL;
+    const bool minmax = nbins != 0 && (flags & CUBE_RANGE_MINMAX);
+    if (minmax) { if (nbins < 1 || nbins > CUBE_MAX_BINS) return CUBE_EINVAL; lo = hi = 0.f; }
+    else if (nbins != 0 && !hist_scale(nbins, lo, hi, &scale)) return CUBE_EINVAL;
+    c->ooc_minmax = minmax ? 1 : 0;
     c->ooc_active = 1; c->ooc_sweep = 0; c->ooc_bricks = 0;
     c->ooc_nbins = nbins; c->ooc_lo = lo; c->ooc_hi = hi; c->ooc_scale = scale;
     c->ooc_want_median = want_median ? 1 : 0;
@@ -37,17 +44,32 @@ int cube_ooc_brick(cube_ctx* c, const float* d, uint64_t nvox, cudaStream_t s) {
             rc = launch_moments(c, d, nvox, CUBE_COARSE_HIST, acc, s, kMomCoarse, 0.f, 0.f, false, nullptr, nullptr, c->gdigits);
         } else {
             if ((rc = launch_moments(c, d, nvox, 0u, acc, s))) return rc;
-            if (c->ooc_nbins > 0) rc = launch_hist(c, d, nvox, c->ooc_nbins, c->ooc_lo, c->ooc_hi, c->ooc_scale, s);
+            if (c->ooc_nbins > 0 && !c->ooc_minmax)
+                rc = launch_hist(c, d, nvox, c->ooc_nbins, c->ooc_lo, c->ooc_hi, c->ooc_scale, s);
         }
     } else if (c->ooc_sweep == 1) {
         const int nbins = c->ooc_nbins;
-        if (nbins > 0 && nbins <= kSmemHistMaxBins) {
+        // CUBE_RANGE_MINMAX: [min, max] of the running record -- complete after sweep 0 (a sharded run has merged the
+        // ranks' records by then) -- resolved on the device, as in cube_stats
+        const MomentsOut* range_from = c->ooc_minmax ? c->mom_out : nullptr;
+        const float* range3 = nullptr;
+        if (c->ooc_minmax && !(c->ooc_want_median && nbins <= kSmemHistMaxBins)) {
+            {
+                ProfScope prof(c, CUBE_K_OTHER, s);
+                hist_range_kernel<<<1, 1, 0, s>>>(c->mom_out, nbins, c->range3, c->gout);
+            }
+            CUBE_CUDA(c, cudaGetLastError());
+            range3 = c->range3;
+        }
+        if (!c->ooc_want_median) {    // histogram over [min, max] without the median: the second sweep is its own
+            rc = launch_hist(c, d, nvox, nbins, c->ooc_lo, c->ooc_hi, c->ooc_scale, s, range3);
+        } else if (nbins > 0 && nbins <= kSmemHistMaxBins) {
             const size_t smem = (size_t)hist_select_smem(nbins);
             const int occ = occupancy_of(c, hist_select_kernel, kThreads, smem);
             const int grid = grid_for(c, 4, occ < kMaxCtasPerSm ? occ : kMaxCtasPerSm);
             {
                 ProfScope prof(c, CUBE_K_HIST_SELECT, s);
-                hist_select_kernel<<<grid, kThreads, smem, s>>>(d, nvox, nbins, c->ooc_lo, c->ooc_hi, c->ooc_scale, nullptr,
+                hist_select_kernel<<<grid, kThreads, smem, s>>>(d, nvox, nbins, c->ooc_lo, c->ooc_hi, c->ooc_scale, range_from,
                                                                 c->gbins, c->gout, c->sel, c->gdigits, c->cand, nullptr);
             }
             CUBE_CUDA(c, cudaGetLastError());
@@ -55,7 +77,7 @@ int cube_ooc_brick(cube_ctx* c, const float* d, uint64_t nvox, cudaStream_t s) {
             // window histogram + second digit in one read when the sampled plan allows it (and the automatic variant
             // is selected); else the histogram kernel and select_pass_kernel<1> read the brick one after the other
             const bool fused_big = c->bighist == 0;
-            if ((rc = launch_hist(c, d, nvox, nbins, c->ooc_lo, c->ooc_hi, c->ooc_scale, s, nullptr, fused_big, false))) return rc;
+            if ((rc = launch_hist(c, d, nvox, nbins, c->ooc_lo, c->ooc_hi, c->ooc_scale, s, range3, fused_big, false))) return rc;
             rc = launch_select_pass<1>(c, d, nvox, s, nullptr, fused_big ? &c->plan->use_window : nullptr);
         } else {
             rc = launch_select_pass<1>(c, d, nvox, s);
@@ -85,6 +107,10 @@ int cube_ooc_next_sweep(cube_ctx* c, int* more, cudaStream_t s) {
     if (!c || !c->ooc_active || !more) return CUBE_EINVAL;
     int rc = CUBE_OK;
     *more = 0;
+    if (!c->ooc_want_median && c->ooc_minmax) {
+        *more = c->ooc_sweep == 0 ? 1 : 0;      // sweep 1: the histogram over the [min, max] found by sweep 0
+        if (c->ooc_sweep > 1) return CUBE_EINVAL;
+    }
     if (c->ooc_want_median) {
         if (c->ooc_sweep == 0) { rc = launch_select_scan<0>(c, c->gdigits, s); *more = 1; }
         else if (c->ooc_sweep == 1) {
@@ -173,8 +199,13 @@ int cube_shard_advance(cube_ctx* c, int* more, cudaStream_t s) {
         }
         else if (c->ooc_sweep == 2) { rc = launch_select_scan<2>(c, c->gdigits, s); }
         else return CUBE_EINVAL;
+        c->ooc_sweep++;
+    } else if (c->ooc_minmax && c->ooc_sweep == 0) {
+        *more = 1;                              // stage 1: the histogram over the merged [min, max]
+        c->ooc_sweep = 1;
+    } else {
+        c->ooc_sweep = 3;
     }
-    c->ooc_sweep = c->ooc_want_median ? c->ooc_sweep + 1 : 3;
     return rc;
 }
 
@@ -212,7 +243,7 @@ int cube_stats_host(cube_ctx* c, const float* h, int64_t nx, int64_t ny, int64_t
     }
     const int want_median = median != nullptr;
     cudaStream_t ws = c->work_stream, cs = c->copy_stream;
-    int rc = cube_ooc_begin(c, (bins && outside) ? nbins : 0, lo, hi, want_median, ws);
+    int rc = cube_ooc_begin_ex(c, (bins && outside) ? nbins : 0, lo, hi, want_median, flags & CUBE_RANGE_MINMAX, ws);
     if (rc) return rc;
     const uint64_t chunk_vox = c->chunk_bytes / sizeof(float);
     const uint64_t nchunks = (n + chunk_vox - 1) / chunk_vox;
@@ -287,7 +318,7 @@ int cube_stats_stream(cube_ctx* c, uint64_t nbricks, uint64_t brick_vox, uint64_
     }
     const int want_median = median != nullptr;
     cudaStream_t ws = c->work_stream, cs = c->copy_stream, fs = c->fill_stream;
-    if ((rc = cube_ooc_begin(c, want_hist ? nbins : 0, lo, hi, want_median, ws))) return rc;
+    if ((rc = cube_ooc_begin_ex(c, want_hist ? nbins : 0, lo, hi, want_median, flags & CUBE_RANGE_MINMAX, ws))) return rc;
     const uint64_t nres = c->resident ? (c->resident_bytes / (brick_vox * sizeof(float))) : 0;  // bricks kept in HBM
     c->stream_h2d_bytes = 0; c->stream_sweeps = 0;
     int more = 1;

@@ -14,7 +14,7 @@ same code drives real ranks (``run``) and the single-process lock-step emulation
 """
 import torch
 
-from . import SHARD_DIGITS, SHARD_RECORD_BYTES, MAX_BINS
+from . import SHARD_DIGITS, SHARD_RECORD_BYTES, MAX_BINS, RANGE_MINMAX
 
 
 def slab_bounds(nz, world, rank):
@@ -58,7 +58,12 @@ class ShardedStats:
         self.outside = alias(b["outside"], 16, torch.int64, self.device)
         self.digits = alias(b["digits"], SHARD_DIGITS * 8, torch.int64, self.device)
         self.stage, self.more = 0, True
-        ctx.ooc_begin(self.nbins, lo if self.nbins else 0.0, hi if self.nbins else 0.0, self.want_median, self.stream)
+        # lo=None: histogram over [min, max] of the WHOLE cube (the merged records), resolved on the device
+        self.minmax = bool(self.nbins) and lo is None
+        if self.minmax:
+            ctx.ooc_begin(self.nbins, 0.0, 0.0, self.want_median, self.stream, flags=RANGE_MINMAX)
+        else:
+            ctx.ooc_begin(self.nbins, lo if self.nbins else 0.0, hi if self.nbins else 0.0, self.want_median, self.stream)
 
     def local_pass(self):
         if self.nvox:
@@ -67,9 +72,11 @@ class ShardedStats:
     def payload(self):
         """-> (record to all-gather or None, [tensors to all-reduce SUM])."""
         hist = [self.bins, self.outside] if self.nbins else []
+        two_stage_hist = self.want_median or self.minmax          # the histogram is accumulated in stage 1 then
+        digits = [self.digits] if self.want_median else []
         if self.stage == 0:
-            return self.record, ([self.digits] if self.want_median else hist)
-        return None, (hist if self.stage == 1 else []) + [self.digits]
+            return self.record, (digits if two_stage_hist else hist)
+        return None, (hist if self.stage == 1 and two_stage_hist else []) + digits
 
     def merge_records(self, gathered, world):
         self.ctx.shard_merge_records(gathered, world, self.flags, self.stream)

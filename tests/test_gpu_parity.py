@@ -742,6 +742,16 @@ def test_stats_host_matches_oracle(ctx, resident):
     rb, ro = oracle.histogram(a, 4096, -0.02, 0.5)
     assert (b == rb).all() and (o == ro).all()
     assert same_float(med, oracle.median(a))
+    # histogram over [min, max] found by the first sweep (CUBE_RANGE_MINMAX), small and big bin counts, with and
+    # without the median (without it the second sweep exists for the histogram alone)
+    ref = oracle.moments(a)
+    for nb in (1024, 65536):
+        rb, ro = oracle.histogram(a, nb, float(ref["min"]), float(ref["max"]))
+        for want_median in (True, False):
+            m, b, o, med = ctx.stats_host(h, 96, 96, 200, nb, 0.0, 0.0, flags=cube.RANGE_MINMAX, want_median=want_median)
+            check_moments(m, ref, a)
+            assert (b == rb).all() and (o == ro).all() and int(b.sum()) == ref["count"]
+            assert (not want_median) or same_float(med, oracle.median(a))
     ctx.host_workspace(0, 1 << 20)
 
 

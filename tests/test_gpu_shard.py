@@ -195,3 +195,30 @@ def test_sharded_slab_presented_as_several_bricks(scratch, nbins, lo, hi):
     tc = torch.from_numpy(c2).cuda()
     res, _ = lockstep([tc[:100000], tc[100000:]], 4096, -0.02, 0.5, scratch=scratch, cls=SeveralBricks)
     check_against_oracle(res, c2, 4096, -0.02, 0.5)
+
+
+@pytest.mark.parametrize("name,dims,world,nbins", [("c3", (64, 64, 96), 3, 65536), ("c4", (128, 64, 24), 2, 256),
+                                                   ("c1", (48, 48, 30), 4, 1024)])
+def test_sharded_histogram_over_the_merged_min_max(name, dims, world, nbins):
+    # lo=None: the range is [min, max] of the WHOLE cube, known on every rank after the records are merged and
+    # resolved on the device; the histogram is accumulated in stage 1 (configs 1, 3, 4 bin over [min, max])
+    cfg = cubegen.scaled(name, dims)
+    nx, ny, nz = dims
+    t = torch.empty(nx * ny * nz, dtype=torch.float32, device="cuda")
+    cubegen.generate_device(cfg, t.data_ptr())
+    torch.cuda.synchronize()
+    a = t.cpu().numpy()
+    slabs = []
+    for r in range(world):
+        z0, z1 = shard.slab_bounds(nz, world, r)
+        slabs.append(t[z0 * nx * ny:z1 * nx * ny])
+    ref = oracle.moments(a)
+    lo, hi = float(ref["min"]), float(ref["max"])
+    res, rounds = lockstep(slabs, nbins, None, None)
+    assert rounds == 3
+    check_against_oracle(res, a, nbins, lo, hi)
+    res, rounds = lockstep(slabs, nbins, None, None, want_median=False)
+    assert rounds == 2
+    rb, ro = oracle.histogram(a, nbins, lo, hi)
+    for m, b, o, _ in res:
+        assert m["count"] == ref["count"] and (b == rb).all() and (o == ro).all() and int(b.sum()) == ref["count"]
