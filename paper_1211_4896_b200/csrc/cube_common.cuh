@@ -80,23 +80,29 @@ __device__ __forceinline__ void stream_cube(const float* __restrict__ d, uint64_
             if (t < n) f(d[t]);
         }
     }
-    const uint64_t ntiles = (nvec + TILE - 1) / TILE;
-    for (uint64_t t = blockIdx.x; t < ntiles; t += gridDim.x) {
-        const uint64_t base = t * TILE + threadIdx.x;
-        if ((t + 1) * TILE <= nvec) {  // whole tile in range: CTA-uniform, so batch() may use warp collectives
-            float4 r[kUnroll];
+    // Full tiles: a 32-bit tile counter (n <= 2^37 voxels: fewer than 2^23 tiles) and one running pointer, so that
+    // the loop carries three registers of state and nothing is recomputed per tile (with the 64-bit tile index and
+    // the in-loop "whole tile?" test ptxas rematerialised head / nvec / ntiles every iteration under the 64-register
+    // cap of the 1024-thread kernels: ~85 of ~510 instructions per warp tile, profiles/r2_*).
+    const uint32_t nfull = (uint32_t)(nvec / TILE);
+    const float4* __restrict__ q = v + (uint64_t)blockIdx.x * TILE + threadIdx.x;
+    const uint64_t stride = (uint64_t)gridDim.x * TILE;
+    for (uint32_t t = blockIdx.x; t < nfull; t += gridDim.x, q += stride) {   // CTA-uniform: batch() may use warp collectives
+        float4 r[kUnroll];
 #pragma unroll
-            for (int j = 0; j < kUnroll; ++j) r[j] = ld_stream(v + base + (uint64_t)j * THREADS);
-            asm volatile("" ::: "memory");  // all kUnroll loads are issued before the first counter update
-            f.batch(r, v + base);
-        } else {
+        for (int j = 0; j < kUnroll; ++j) r[j] = ld_stream(q + j * THREADS);
+        asm volatile("" ::: "memory");  // all kUnroll loads are issued before the first counter update
+        f.batch(r, q);
+    }
+    // the ragged last tile goes to the CTA whose turn it would be, voxel by voxel
+    if (nvec % TILE != 0 && nfull % gridDim.x == blockIdx.x) {
+        const uint64_t base = (uint64_t)nfull * TILE + threadIdx.x;
 #pragma unroll 1
-            for (int j = 0; j < kUnroll; ++j) {
-                uint64_t i = base + (uint64_t)j * THREADS;
-                if (i < nvec) {
-                    float4 r = ld_stream(v + i);
-                    f(r.x); f(r.y); f(r.z); f(r.w);
-                }
+        for (int j = 0; j < kUnroll; ++j) {
+            const uint64_t i = base + (uint64_t)j * THREADS;
+            if (i < nvec) {
+                const float4 r = ld_stream(v + i);
+                f(r.x); f(r.y); f(r.z); f(r.w);
             }
         }
     }
