@@ -245,7 +245,7 @@ int launch_hist(cube_ctx* c, const float* d, uint64_t n, int nbins, float lo, fl
             const bool window_allowed = c->bighist != 2;
             if (fused_select) {   // cube_stats: window histogram + second select digit in one kernel
                 c->launches++;
-                hist_win_select_kernel<<<c->num_sms, kBigThreads, kBigFusedSmem, s>>>(
+                hist_win_select_kernel<<<c->num_sms, kFusedThreads, kBigFusedSmem, s>>>(
                     d, n, nbins, lo, hi, scale, range3, c->plan, c->gbins, outside, c->sel, c->gdigits, c->cand,
                     fused_scan ? c->ticket2 : nullptr);
             } else if (window_allowed) {

@@ -14,13 +14,17 @@
 
 namespace cube {
 
-constexpr int kBigWarps = kBigThreads / 32;
+#ifndef CUBE_FUSED_THREADS
+#define CUBE_FUSED_THREADS 896
+#endif
+constexpr int kFusedThreads = CUBE_FUSED_THREADS;   // threads of the one CTA per SM (65536 / threads registers each)
+constexpr int kBigWarps = kFusedThreads / 32;
 // [window counters + trash][digit counters + trash], padded to 16 bytes, then one WarpGather per warp
 constexpr int kBigFusedHead = ((kBigWords + 1 + kBins1 + 1) * (int)sizeof(uint32_t) + 15) / 16 * 16;
 constexpr int kBigFusedSmem = kBigFusedHead + kBigWarps * (int)sizeof(WarpGather);
 
 struct HistWinSelectF {
-    HistWinF h;
+    HistWinFT<kFusedThreads> h;
     uint32_t negbase;              // 0 - (raw_of_digit(prefix) << 19)
     bool select;                   // false: nothing to select (k >= count)
     WarpGather* wq;                // this warp's queue
@@ -33,11 +37,11 @@ struct HistWinSelectF {
     }
     __device__ __forceinline__ void batch(const float4 (&r)[kUnroll], const float4* __restrict__ p) {
         h.batch(r, p);
-        if (select) gather_batch<kBigThreads>(r, p, negbase, wq, sh);
+        if (select) gather_batch<kFusedThreads>(r, p, negbase, wq, sh);
     }
 };
 
-__global__ void __launch_bounds__(kBigThreads, 1)
+__global__ void __launch_bounds__(kFusedThreads, 1)
 hist_win_select_kernel(const float* __restrict__ d, uint64_t n, int nbins, float lo, float hi, float scale,
                        const float* __restrict__ range3, const BigHistPlan* __restrict__ plan,
                        unsigned long long* __restrict__ gbins, unsigned long long* __restrict__ goutside,
@@ -50,7 +54,7 @@ hist_win_select_kernel(const float* __restrict__ d, uint64_t n, int nbins, float
     uint32_t* wbins = dyn_bins;                               // kBigWords + 1
     uint32_t* sbins = dyn_bins + (kBigWords + 1);             // kBins1 + 1
     WarpGather* wgs = reinterpret_cast<WarpGather*>(reinterpret_cast<unsigned char*>(dyn_bins) + kBigFusedHead);
-    for (int i = threadIdx.x; i < kBigWords + 1 + kBins1 + 1; i += kBigThreads) dyn_bins[i] = 0;
+    for (int i = threadIdx.x; i < kBigWords + 1 + kBins1 + 1; i += kFusedThreads) dyn_bins[i] = 0;
     if (threadIdx.x < kBigWarps) {
         wgs[threadIdx.x].nrows = 0; wgs[threadIdx.x].nkeys = 0;
         wgs[threadIdx.x].compacting = (cand && st->cand_cap) ? 1u : 0u;
@@ -68,15 +72,15 @@ hist_win_select_kernel(const float* __restrict__ d, uint64_t n, int nbins, float
     f.select = st->invalid == 0;
     f.wq = wgs + (threadIdx.x >> 5);
     f.sh = &sh;
-    stream_cube<kBigThreads>(d, n, f);
+    stream_cube<kFusedThreads>(d, n, f);
     if (f.select) gather_finish(f.wq, &sh);                   // rows still queued, keys still staged
     __syncthreads();
     const uint32_t w0 = plan->w0;
-    for (int i = threadIdx.x; i < kBigWords; i += kBigThreads) {
+    for (int i = threadIdx.x; i < kBigWords; i += kFusedThreads) {
         const uint32_t c = wbins[i];
         if (c && w0 + i < (uint32_t)nbins) atomicAdd(&gbins[w0 + i], (unsigned long long)c);
     }
-    for (int i = threadIdx.x; i < kBins1; i += kBigThreads) {
+    for (int i = threadIdx.x; i < kBins1; i += kFusedThreads) {
         const uint32_t c = sbins[i];
         if (c) atomicAdd(&gdigits[i], (unsigned long long)c);
     }
@@ -86,7 +90,7 @@ hist_win_select_kernel(const float* __restrict__ d, uint64_t n, int nbins, float
         __shared__ unsigned long long scan_sm[kScanSmem];
         SelectInit none;
         none.k = 0; none.cand_cap = 0; none.result_out = nullptr; none.use_median = 0; none.enabled = 0;
-        select_scan_if_last_n<1, kBigThreads>(st, gdigits, 1, none, scan_ticket, scan_sm);
+        select_scan_if_last_n<1, kFusedThreads>(st, gdigits, 1, none, scan_ticket, scan_sm);
     }
 }
 

@@ -237,7 +237,8 @@ struct BigHistPlan {
     uint32_t pad;
 };
 
-struct HistWinF {
+template <int THREADS>   // threads per CTA: the stride between a thread's rows of a tile
+struct HistWinFT {
     float lo, hi, scale, off;
     int top;
     uint32_t w0, limitbits, sbase;
@@ -278,7 +279,7 @@ struct HistWinF {
         do {
             const int j = __ffs(rows) - 1;
             rows &= rows - 1;
-            const float4 q = __ldcg(p + j * kBigThreads);   // L2 hit: the line has just been streamed
+            const float4 q = __ldcg(p + j * THREADS);   // L2 hit: the line has just been streamed
             if (!counted(q.x)) exact(q.x);
             if (!counted(q.y)) exact(q.y);
             if (!counted(q.z)) exact(q.z);
@@ -297,6 +298,8 @@ struct HistWinF {
         if (rows) cold(rows, p);
     }
 };
+
+using HistWinF = HistWinFT<kBigThreads>;
 
 // 1 CTA: sample 16384 voxels spread over the cube; block histogram (16 blocks of 4096 bins); best window of 8
 // consecutive blocks; also the packed kernel's flip hint.  A performance plan only: every choice is exact.

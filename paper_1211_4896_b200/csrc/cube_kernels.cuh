@@ -187,8 +187,11 @@ struct ClipState {
 // acc : running Partial across calls (out-of-core bricks); merged in call order => deterministic.
 // nvox_acc : running voxel total.  When `accumulate` is 0 both are overwritten.
 // kMomWindow: the window is (wlo, whi), or *clip when clip != nullptr (then a finished clip makes the kernel a no-op).
+#ifndef CUBE_MOM_CTAS
+#define CUBE_MOM_CTAS 4
+#endif
 template <int MODE>
-__global__ void __launch_bounds__(kThreads, 4)
+__global__ void __launch_bounds__(kThreads, CUBE_MOM_CTAS)
 moments_kernel(const float* __restrict__ d, uint64_t n, Partial* __restrict__ partials,
                unsigned int* __restrict__ ticket, Partial* __restrict__ acc,
                unsigned long long* __restrict__ nvox_acc, int accumulate, unsigned flags,
