@@ -44,13 +44,14 @@ struct MomentsF {
     __device__ __forceinline__ bool taken(float x) const {
         return (MODE == kMomWindow) ? (x >= wlo && x <= whi) : (x == x);  // NaN == blanked voxel
     }
+    template <bool MINMAX = true>
     __device__ __forceinline__ void core(float x) {
         const bool ok = taken(x);
         if (MODE == kMomWindow) {  // FMNMX ignores NaN operands: a voxel outside the window is fed as NaN
             const float xw = ok ? x : __int_as_float(0x7fc00000);
             mn = fminf(mn, xw);
             mx = fmaxf(mx, xw);
-        } else {
+        } else if (MINMAX) {
             mn = fminf(mn, x);
             mx = fmaxf(mx, x);
         }
@@ -59,7 +60,18 @@ struct MomentsF {
         s += dlt;
         q = fma(dlt, dlt, q);
         n += ok ? 1u : 0u;
-        if (COARSE) smem_inc(sbins, ok ? raw_digit(x) : (uint32_t)kDigitBins);  // raw top bits; NaN -> trash
+        // COARSE: the digit of xs -- a NULL voxel is counted in the PIVOT's bin (no select per voxel) and taken back
+        // out once per thread after the streaming loop (nsub0 / nsub1: NULL voxels met before / after the pivot was
+        // found; the pivot changes only once, from the initial +0.0f)
+        if (COARSE) smem_inc(sbins, raw_digit(xs));
+    }
+    uint32_t nsub0 = 0, nsub1 = 0;
+    __device__ __forceinline__ void note_subst(uint32_t k) { if (have) nsub1 += k; else nsub0 += k; }
+    // after the streaming loop: take the substituted NULL voxels back out of the pivot's digit bins
+    __device__ __forceinline__ void unsubstitute() const {
+        if (!COARSE) return;
+        if (nsub0) asm volatile("red.shared.add.u32 [%0], %1;" :: "r"(sbins + 4u * raw_digit(0.0f)), "r"(0u - nsub0) : "memory");
+        if (nsub1) asm volatile("red.shared.add.u32 [%0], %1;" :: "r"(sbins + 4u * raw_digit(pivf)), "r"(0u - nsub1) : "memory");
     }
     // The pivot is the first FINITE voxel that takes part: about an infinite pivot every deviation would be
     // infinite or NaN.  (A cube with +-Inf voxels has mean = std = NaN whatever the summation order: reading R8,
@@ -67,7 +79,11 @@ struct MomentsF {
     __device__ __forceinline__ void take_pivot(float x) {
         if (!have && taken(x) && fabsf(x) < INFINITY) { have = true; pivf = x; pivot = (double)x; }
     }
-    __device__ __forceinline__ void operator()(float x) { take_pivot(x); core(x); }
+    __device__ __forceinline__ void operator()(float x) {
+        take_pivot(x);
+        core(x);
+        if (COARSE && !taken(x)) note_subst(1u);
+    }
 
     // A tile share (kUnroll rows of 4 voxels) whose sum of deviations came out NaN holds a NaN voxel (or +Inf and
     // -Inf): the hot path has left it out of s, q and n, and has counted every one of its voxels in the digit bins.
@@ -98,8 +114,8 @@ struct MomentsF {
     //   tq += d0^2+d1^2+d2^2+d3^2 (DFMA chain); the tile share joins s, q, n when ts is not NaN -- no per-voxel NaN
     //   test, select or count (FMNMX ignores NaN operands; the digit increment is unconditional): ~8.5 issue slots
     //   per voxel.  A lane whose ts is NaN (a NaN voxel, or +Inf and -Inf) repairs its share in cold_tile().
-    //  SAFE: the branch-free per-voxel form (core(): FSETP, FSEL, count; ~14 slots per voxel), which costs the same
-    //   whatever the NaN density.
+    //  SAFE: the branch-free per-voxel form (core(): FSETP, FSEL, count; extrema per row; the digit of a NULL voxel is
+    //   the pivot's, put right once per thread: ~11 slots per voxel), which costs the same whatever the NaN density.
     // The warp runs HOT until a tile with a NaN shows up and SAFE until a tile without one has gone by (one vote
     // per tile), so cubes with scattered NULL voxels (config 3: 0.5 %, i.e. some lane of every warp tile) never
     // pay the divergent repair, and NaN-free stretches never pay the per-voxel tests (profiles/: the fused passes
@@ -113,7 +129,14 @@ struct MomentsF {
             }
             const uint32_t n0 = n;
 #pragma unroll
-            for (int j = 0; j < kUnroll; ++j) { core(r[j].x); core(r[j].y); core(r[j].z); core(r[j].w); }
+            for (int j = 0; j < kUnroll; ++j) {
+                if (MODE != kMomWindow) {   // extrema per row of 4 (FMNMX3, NaN-blind) instead of 2 FMNMX per voxel
+                    mn = fminf(fminf(mn, r[j].x), fminf(r[j].y, fminf(r[j].z, r[j].w)));
+                    mx = fmaxf(fmaxf(mx, r[j].x), fmaxf(r[j].y, fmaxf(r[j].z, r[j].w)));
+                }
+                core<false>(r[j].x); core<false>(r[j].y); core<false>(r[j].z); core<false>(r[j].w);
+            }
+            if (COARSE) note_subst(4u * kUnroll - (n - n0));
             if (MODE != kMomWindow) safe = __any_sync(0xffffffffu, n - n0 != 4u * kUnroll);  // every lane has a pivot then
             return;
         }
@@ -217,6 +240,7 @@ moments_kernel(const float* __restrict__ d, uint64_t n, Partial* __restrict__ pa
         __syncthreads();
     }
     stream_cube<kThreads>(d, n, f);
+    f.unsubstitute();
     Partial p = partial_block_reduce(f.partial(), scratch);
     if (COARSE) {
         __syncthreads();
