@@ -322,6 +322,15 @@ int cube_render_tf(cube_ctx* ctx, const float* d, int64_t nx, int64_t ny, int64_
 int cube_spectrum(cube_ctx* ctx, const float* d, int64_t nx, int64_t ny, int64_t nz, const cube_view_t* view,
                   int u, int v, float* out, cudaStream_t stream);
 
+/* Per-cell lower median of the mini-map (NEXT-2, second half: SURVEY.md sec. 8(f) "mean/std (then median) per user
+ * partition"): med[(cz*my + cy)*mx + cx] = the lower median (k = (count-1)/2 over the cell's non-NULL
+ * voxels, as cube_median) of the cell cube_minimap defines; NaN for a cell without a non-NULL voxel.  Exact.  The
+ * cube is read once (cells of up to 56000 voxels: their keys are kept in shared memory while four 8-bit digits are
+ * fixed; larger cells are read once per digit).  A cell may hold at most 2^31 voxels.  `med`: mx*my*mz floats the
+ * DEVICE can write (device or pinned host memory). */
+int cube_minimap_median(cube_ctx* ctx, const float* d, int64_t nx, int64_t ny, int64_t nz, int64_t px, int64_t py,
+                        int64_t pz, float* med, cudaStream_t stream);
+
 const char* cube_strerror(int code);
 int cube_last_cuda_error(const cube_ctx* ctx);
 

@@ -34,7 +34,7 @@ SYMBOLS = ["cube_create", "cube_destroy", "cube_moments", "cube_histogram", "cub
            "cube_profile_enable", "cube_profile_reset", "cube_profile_read",
            "cube_mad", "cube_clipped_moments", "cube_sigma_clip", "cube_minimap_dims", "cube_minimap",
            "cube_shard_buffers", "cube_shard_merge_records", "cube_shard_advance", "cube_median_torben",
-           "cube_view_orbit", "cube_render_mip", "cube_render_tf", "cube_spectrum"]
+           "cube_view_orbit", "cube_render_mip", "cube_render_tf", "cube_spectrum", "cube_minimap_median"]
 SHARD_RECORD_BYTES, SHARD_DIGITS = 40, 8192
 KNOB_CTAS_PER_SM, KNOB_BIGHIST, KNOB_MINIMAP = 0, 1, 2
 KIND_NAMES = ["moments", "moments_coarse", "histogram", "select_pass0", "select_pass1", "select_pass2",
@@ -142,6 +142,7 @@ def load():
     L.cube_sigma_clip.argtypes = [vp, vp, i64, i64, i64, f64, ci, cu, vp, vp, vp, vp]
     L.cube_minimap_dims.argtypes = [i64] * 6 + [ctypes.POINTER(i64)] * 3
     L.cube_minimap.argtypes = [vp, vp, i64, i64, i64, i64, i64, i64, cu, vp, vp]
+    L.cube_minimap_median.argtypes = [vp, vp, i64, i64, i64, i64, i64, i64, vp, vp]
     L.cube_median_torben.argtypes = [vp, vp, i64, i64, i64, ci, vp, vp, vp, vp]
     vwp = ctypes.POINTER(ViewT)
     L.cube_view_orbit.argtypes = [i64, i64, i64, f64, f64, ci, ci, f64, vwp]
@@ -360,6 +361,10 @@ class Context:
         """cube_spectrum: ``out`` = device (or pinned) buffer of nsteps floats."""
         w = ViewT.from_dict(view)
         self._check(self._L.cube_spectrum(self._h, _ptr(d), nx, ny, nz, ctypes.byref(w), u, v, _ptr(out), stream))
+
+    def minimap_median(self, d, nx, ny, nz, px, py, pz, med, stream=0):
+        """cube_minimap_median: ``med`` = device (or pinned) buffer of mx*my*mz floats."""
+        self._check(self._L.cube_minimap_median(self._h, _ptr(d), nx, ny, nz, px, py, pz, _ptr(med), stream))
 
     def probe_read(self, d, nvox, stream=0):
         self._check(self._L.cube_probe_read(self._h, _ptr(d), nvox, stream))

@@ -10,7 +10,7 @@ _HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(_HERE, "csrc")
 LIB = os.path.join(_HERE, "libcube.so")
 SOURCES = ["cube.cu"]
-DEPS = ["cube.cu", "cube_ooc.inl", "cube_kernels.cuh", "cube_common.cuh", "cube_select.cuh", "cube_fused.cuh", "cube_hist_big.cuh", "cube_minimap.cuh", "cube_minimap_tma.cuh", "cube_fused_big.cuh", "cube_torben.cuh", "cube_select_multi.cuh", "cube_render.cuh", os.path.join("..", "..", "include", "cube.h")]
+DEPS = ["cube.cu", "cube_ooc.inl", "cube_kernels.cuh", "cube_common.cuh", "cube_select.cuh", "cube_fused.cuh", "cube_hist_big.cuh", "cube_minimap.cuh", "cube_minimap_tma.cuh", "cube_fused_big.cuh", "cube_torben.cuh", "cube_select_multi.cuh", "cube_render.cuh", "cube_minimap_median.cuh", "cube_gather.cuh", os.path.join("..", "..", "include", "cube.h")]
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17",
               "--fmad=true",            # contraction is confined to fp64 fma() calls we write ourselves;
                                         # the float32 bin formula uses __fsub_rn/__fmul_rn (never contracted)

@@ -13,6 +13,7 @@
 #include "cube_kernels.cuh"
 #include "cube_minimap_tma.cuh"
 #include "cube_render.cuh"
+#include "cube_minimap_median.cuh"
 #include "cube_select_multi.cuh"
 
 using namespace cube;
@@ -394,6 +395,10 @@ int cube_create(cube_ctx** out, size_t scratch_bytes_hint) {
                                     kBigFusedSmem) == cudaSuccess;
     ok = ok && cudaFuncSetAttribute(minimap_tma_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize,
                                     kMapTmaSmem) == cudaSuccess;
+    ok = ok && cudaFuncSetAttribute(minimap_median_cta_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                    kMedStageKeys * 4 + kMedCtaExtra) == cudaSuccess;
+    ok = ok && cudaFuncSetAttribute(minimap_median_warp_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                    (kMedCtaThreads / 32) * kMedWarpSmemPerWarp) == cudaSuccess;
     ok = ok && cudaFuncSetAttribute(hist_dsm_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize,
                                     (32768 + 1) * (int)sizeof(uint32_t)) == cudaSuccess;
     if (!ok) { cube_destroy(c); return CUBE_ENOMEM; }
@@ -855,6 +860,39 @@ int cube_spectrum(cube_ctx* c, const float* d, int64_t nx, int64_t ny, int64_t n
     {
         ProfScope prof(c, CUBE_K_RENDER, s);
         spectrum_kernel<<<(vw.nsteps + 255) / 256, 256, 0, s>>>(d, g, vw, u, v, out);
+    }
+    CUBE_CUDA(c, cudaGetLastError());
+    return CUBE_OK;
+}
+
+int cube_minimap_median(cube_ctx* c, const float* d, int64_t nx, int64_t ny, int64_t nz, int64_t px, int64_t py,
+                        int64_t pz, float* med, cudaStream_t s) {
+    MedGeom g;
+    if (!c || !d || !med) return CUBE_EINVAL;
+    if (cube_minimap_dims(nx, ny, nz, px, py, pz, (int64_t*)&g.mx, (int64_t*)&g.my, (int64_t*)&g.mz)) return CUBE_EINVAL;
+    g.nx = nx; g.ny = ny; g.nz = nz; g.px = px; g.py = py; g.pz = pz;
+    cudaPointerAttributes at;   // the medians are written in place by the kernel
+    if (cudaPointerGetAttributes(&at, med) != cudaSuccess || at.type == cudaMemoryTypeUnregistered) {
+        cudaGetLastError();
+        return CUBE_EINVAL;
+    }
+    const long double cellvox = (long double)std::min(px, nx) * (long double)std::min(py, ny) * (long double)std::min(pz, nz);
+    if (cellvox > 2147483648.0L) return CUBE_EINVAL;
+    const long double ncell = (long double)g.mx * (long double)g.my * (long double)g.mz;
+    {
+        ProfScope prof(c, CUBE_K_MINIMAP, s);
+        if (cellvox < (long double)kMedWarpKeys) {
+            const int per = kMedCtaThreads / 32;
+            const long double want = (ncell + per - 1) / per;
+            const unsigned grid = (unsigned)std::min<long double>(want < 1 ? 1 : want, (long double)c->num_sms * 16);
+            minimap_median_warp_kernel<<<grid, kMedCtaThreads, per * kMedWarpSmemPerWarp, s>>>(d, g, med);
+        } else {
+            const int stage = cellvox <= (long double)kMedStageKeys ? (((int)cellvox + 3) & ~3) : 0;
+            const size_t smem = (size_t)stage * 4 + kMedCtaExtra;
+            const int occ = occupancy_of(c, minimap_median_cta_kernel, kMedCtaThreads, smem);
+            const unsigned grid = (unsigned)std::min<long double>(ncell, (long double)c->num_sms * (occ < 1 ? 1 : occ));
+            minimap_median_cta_kernel<<<grid, kMedCtaThreads, smem, s>>>(d, g, stage, med);
+        }
     }
     CUBE_CUDA(c, cudaGetLastError());
     return CUBE_OK;

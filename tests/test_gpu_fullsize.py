@@ -181,11 +181,12 @@ def test_config2_full_size():
     ctx = bench_like_context(n)
     try:
         # the oracle's NEXT rows at this size take a minute each: run them beside the main checks
-        pool = ThreadPoolExecutor(4)
+        pool = ThreadPoolExecutor(5)
         f_mad = pool.submit(oracle.mad, a)
         f_clip = pool.submit(oracle.sigma_clip, a, 3.0, 5)
         f_map = pool.submit(oracle.minimap, a, dims, (30, 30, 30))
         f_torben = pool.submit(oracle.torben_capped, a, 20)
+        f_mapmed = pool.submit(oracle.minimap_median, a, dims, (30, 30, 30))
         ref = oracle.moments(a)
         assert ref["nan_count"] > 0 and ref["nan_count"] % (dims[0] * dims[1]) == 0      # whole blanked planes
         rb, ro = oracle.histogram(a, 4096, -0.02, 0.5)
@@ -226,6 +227,11 @@ def test_config2_full_size():
         torch.cuda.synchronize()
         gmap = np.frombuffer(cells.cpu().numpy().tobytes(), dtype=cube.MINIMAP_DTYPE).reshape(mz, my, mx)
         check_minimap(gmap, f_map.result())
+        gmed = torch.zeros(mx * my * mz, dtype=torch.float32, device="cuda")
+        ctx.minimap_median(t, *dims, 30, 30, 30, gmed)
+        torch.cuda.synchronize()
+        gm, rmm = gmed.cpu().numpy().reshape(mz, my, mx), f_mapmed.result()
+        assert ((gm.view(np.uint32) == rmm.view(np.uint32)) | (np.isnan(gm) & np.isnan(rmm))).all()
         pool.shutdown()
     finally:
         ctx.close()

@@ -358,3 +358,54 @@ def test_torben_edge_cases_and_async(ctx):
     s.synchronize()
     rval, rit, rconv = oracle.torben_capped(a, 100)
     assert float(o.item()) == float(rval) and oi[0].item() == rit and bool(oi[1].item()) == rconv
+
+
+# --------------------------------------------------------------------------------------- mini-map: per-cell median
+def run_minimap_median(ctx, t, dims, part):
+    nx, ny, nz = dims
+    mx, my, mz = ctx.minimap_dims(nx, ny, nz, *part)
+    med = torch.full((mx * my * mz,), 123.0, dtype=torch.float32, device="cuda")
+    ctx.minimap_median(t, nx, ny, nz, part[0], part[1], part[2], med)
+    torch.cuda.synchronize()
+    return med.cpu().numpy().reshape(mz, my, mx)
+
+
+def same_bits_map(got, ref):
+    g, r = np.ascontiguousarray(got).view(np.uint32), np.ascontiguousarray(ref).view(np.uint32)
+    return bool(((g == r) | (np.isnan(got) & np.isnan(ref))).all())
+
+
+@pytest.mark.parametrize("dims,part", [((64, 48, 40), (30, 30, 30)), ((96, 80, 64), (16, 16, 16)),
+                                       ((100, 33, 17), (7, 5, 3)), ((37, 29, 11), (37, 29, 11)),
+                                       ((1200, 9, 5), (600, 4, 2)), ((130, 70, 50), (1, 1, 1)),
+                                       ((50, 40, 30), (64, 64, 64)), ((513, 20, 19), (30, 30, 30)),
+                                       ((70, 66, 65), (64, 64, 32)),     # 131072 voxels per cell: re-read per digit
+                                       ((40, 40, 40), (38, 38, 38)),     # 54872 voxels: the largest staged cells
+                                       ((33, 32, 31), (11, 10, 9)), ((9, 9, 9), (10, 10, 1024))])
+def test_minimap_median_shapes(ctx, dims, part):
+    nx, ny, nz = dims
+    r = np.random.default_rng(nx * 131 + part[0])
+    a = (r.standard_normal(nx * ny * nz) * 0.002 + 0.001).astype(np.float32)
+    a[r.integers(0, a.size, a.size // 40)] = np.nan
+    a[r.integers(0, a.size, a.size // 50)] = np.round(a[r.integers(0, a.size, a.size // 50)], 3)    # ties
+    a[r.integers(0, a.size, 20)] = np.float32([np.inf, -np.inf, 0.0, -0.0] * 5)
+    a[:min(a.size, part[0])] = np.nan                                       # a NULL run at the start of cell 0
+    got = run_minimap_median(ctx, dev(a, 1), dims, part)
+    assert same_bits_map(got, oracle.minimap_median(a, dims, part))
+
+
+def test_minimap_median_degenerate_cells(ctx):
+    dims, part = (64, 40, 36), (32, 20, 12)
+    a = np.full(64 * 40 * 36, np.nan, dtype=np.float32)                      # every cell empty
+    assert np.isnan(run_minimap_median(ctx, dev(a), dims, part)).all()
+    vol = a.reshape(36, 40, 64)
+    vol[:12, :20, :32] = 2.5                                                 # a constant cell
+    vol[12:24, 20:, 32:] = -0.0
+    vol[12, 20, 32] = 0.0                                                    # -0.0 < +0.0: the lower median stays -0.0
+    vol[30, 5, 40] = 7.0                                                     # a cell with a single voxel
+    got = run_minimap_median(ctx, dev(vol.reshape(-1)), dims, part)
+    assert same_bits_map(got, oracle.minimap_median(vol.reshape(-1), dims, part))
+    for name, d3 in (("c3", (64, 64, 90)), ("c4", (96, 64, 30))):
+        t, b, _ = scaled_cube(name, d3)
+        for p3 in ((30, 30, 30), (8, 8, 8)):
+            assert same_bits_map(run_minimap_median(ctx, t, d3, p3), oracle.minimap_median(b, d3, p3))
