@@ -135,7 +135,8 @@ int cube_median_ex(cube_ctx* ctx, const float* d, int64_t nx, int64_t ny, int64_
  * outside[0] = outside[1] = UINT64_MAX.  More than 16384 bins: still two reads when the voxels concentrate in a
  * window of 32768 consecutive bins (decided on the device from a sample; the usual case for a noise-dominated cube),
  * else a third read (packed histogram and select as separate kernels).  The first-digit histogram stays in the
- * context for cube_kth_ex(..., CUBE_REUSE_COARSE). */
+ * context for cube_kth_ex(..., CUBE_REUSE_COARSE).  A cube of at most 96 MiB (it stays in the L2 cache between the
+ * two reads) with at most 4096 bins and the median takes ONE cooperative launch (CUBE_KNOB_SMALL). */
 int cube_stats(cube_ctx* ctx, const float* d, int64_t nx, int64_t ny, int64_t nz, int nbins, float lo, float hi,
                unsigned flags, cube_moments_t* moments, uint64_t* bins /* [nbins] */, uint64_t* outside /* [2] */,
                float* median, cudaStream_t stream);
@@ -346,6 +347,9 @@ enum {
                                       for all bins (the choice is made on the device),
                                   1 = clusters of two CTAs holding 32-bit counters in distributed shared memory,
                                   2 = always the 16-bit packed counters */
+    CUBE_KNOB_SMALL = 3,       /* cube_stats on a cube of at most 96 MiB with a histogram of at most 4096 bins and the
+                                  median: 0 = automatic (default): ONE cooperative launch (csrc/cube_small.cuh) when the
+                                  device supports it, 1 = always the general three-launch path */
     CUBE_KNOB_MINIMAP = 2      /* cube_minimap kernel: 0 = automatic (default): lines staged through a shared-memory
                                   ring by TMA bulk copies when the rows are 16-byte aligned, the cells at most 480
                                   voxels wide and a cell row has at least 256 lines (or the 128-bit kernel is not
@@ -377,7 +381,8 @@ enum {
     CUBE_K_MINIMAP = 12,        /* minimap_kernel */
     CUBE_K_TORBEN = 13,         /* torben_pass_kernel (cube_median_torben) */
     CUBE_K_RENDER = 14,         /* render_mip_kernel / render_tf_kernel / spectrum_kernel */
-    CUBE_K_KINDS = 15
+    CUBE_K_STATS_SMALL = 15,    /* stats_small_kernel: cube_stats of an L2-resident cube in one cooperative launch (two reads) */
+    CUBE_K_KINDS = 16
 };
 int cube_profile_enable(cube_ctx* ctx, int on);
 /* Read-only STREAM probe: streams nvox float32 voxels through the same loop as the statistics kernels with one

@@ -20,6 +20,16 @@ _LIB = os.path.join(_HERE, "libcube_oracle.so")
 _FLAGS = ["-O2", "-std=c++17", "-ffp-contract=off", "-fno-fast-math", "-fPIC", "-shared"]
 
 
+# CUBE_ORACLE_SANITIZE=1: the same source built with AddressSanitizer + UndefinedBehaviorSanitizer into its own
+# library; run the CPU pins under it with
+#   CUBE_ORACLE_SANITIZE=1 LD_PRELOAD=$(gcc -print-file-name=libasan.so) ASAN_OPTIONS=detect_leaks=0 \
+#       python -m pytest tests/test_oracle_pins.py tests/test_oracle_next_pins.py tests/test_oracle_render_pins.py -q
+_SANITIZE = os.environ.get("CUBE_ORACLE_SANITIZE", "0") == "1"
+if _SANITIZE:
+    _LIB = os.path.join(_HERE, "libcube_oracle_san.so")
+    _FLAGS = _FLAGS + ["-g", "-fsanitize=address,undefined", "-fno-sanitize-recover=undefined", "-fno-omit-frame-pointer"]
+
+
 def build(force=False):
     """Compile cube_oracle.cpp -> libcube_oracle.so (no-op when up to date)."""
     if (not force and os.path.exists(_LIB)

@@ -16,7 +16,8 @@ import os
 import numpy as np
 
 _HERE = os.path.dirname(os.path.abspath(__file__))
-_LIBPATH = os.path.join(_HERE, "libcube.so")
+# CUBE_LIBPATH: load another build of the same library instead (e.g. the bounds-checked one: build.py --checked)
+_LIBPATH = os.environ.get("CUBE_LIBPATH") or os.path.join(_HERE, "libcube.so")
 
 OK, EINVAL, EEMPTY, ECUDA, ERANGE, ENOMEM, ECALLBACK = 0, 1, 2, 3, 4, 5, 6
 # int fill(void* user, uint64_t brick, int sweep, float* h_dst, uint64_t nvox, cudaStream_t fill_stream)
@@ -36,10 +37,10 @@ SYMBOLS = ["cube_create", "cube_destroy", "cube_moments", "cube_histogram", "cub
            "cube_shard_buffers", "cube_shard_merge_records", "cube_shard_advance", "cube_median_torben",
            "cube_view_orbit", "cube_render_mip", "cube_render_tf", "cube_spectrum", "cube_minimap_median"]
 SHARD_RECORD_BYTES, SHARD_DIGITS = 40, 8192
-KNOB_CTAS_PER_SM, KNOB_BIGHIST, KNOB_MINIMAP = 0, 1, 2
+KNOB_CTAS_PER_SM, KNOB_BIGHIST, KNOB_MINIMAP, KNOB_SMALL = 0, 1, 2, 3
 KIND_NAMES = ["moments", "moments_coarse", "histogram", "select_pass0", "select_pass1", "select_pass2",
               "select_cand", "select_scan", "hist_select", "probe_read", "other", "moments_window", "minimap", "torben_pass",
-              "render"]
+              "render", "stats_small"]
 
 
 class CubeError(RuntimeError):

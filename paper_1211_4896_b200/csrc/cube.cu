@@ -7,6 +7,8 @@
 #include <new>
 #include <stddef.h>
 #include <string.h>
+#include <stdio.h>
+#include <stdlib.h>
 #include <algorithm>
 #include <vector>
 
@@ -14,6 +16,7 @@
 #include "cube_minimap_tma.cuh"
 #include "cube_render.cuh"
 #include "cube_minimap_median.cuh"
+#include "cube_small.cuh"
 #include "cube_select_multi.cuh"
 
 using namespace cube;
@@ -23,6 +26,13 @@ struct cube_ctx {
     int num_sms = 0;
     int ctas_per_sm = 0;  // 0 = per-kernel default
     int bighist = 0;      // CUBE_KNOB_BIGHIST: 0 = automatic (window or packed, chosen on the device), 1 = cluster DSM, 2 = packed
+    int no_small = 0;     // CUBE_KNOB_SMALL: 1 = never the single cooperative launch
+    int coop = 0;         // the device supports cooperative launches
+    unsigned int* bar = nullptr;   // grid-barrier counter of stats_small_kernel (only grows)
+    unsigned int bar_base = 0;
+    unsigned long long* coarse_next = nullptr;   // all zero: the first-digit array the next single-launch cube_stats takes
+    unsigned long long* chunk_tot = nullptr;     // kDigitBins / 32 chunk totals, all zero between calls
+    unsigned long long* small_tstamp = nullptr;   // debug builds only (-DCUBE_SMALL_TIMING)
     int minimap_variant = 0;  // CUBE_KNOB_MINIMAP: 0 = automatic, 1 = no TMA ring, 2 = scalar kernel only, 3 = TMA ring whenever eligible
     int last_cuda = 0;
     uint64_t launches = 0;
@@ -379,6 +389,19 @@ int cube_create(cube_ctx** out, size_t scratch_bytes_hint) {
     ok = ok && cudaMalloc(&c->torben, sizeof(TorbenState)) == cudaSuccess;
     ok = ok && cudaMalloc(&c->center, sizeof(float)) == cudaSuccess;
     ok = ok && cudaMalloc(&c->tf_table, 4096 * sizeof(float4)) == cudaSuccess;
+    ok = ok && cudaMalloc(&c->coarse_next, kDigitBins * sizeof(unsigned long long)) == cudaSuccess;
+    ok = ok && cudaMemset(c->coarse_next, 0, kDigitBins * sizeof(unsigned long long)) == cudaSuccess;
+    ok = ok && cudaMalloc(&c->chunk_tot, (kDigitBins / 32) * sizeof(unsigned long long)) == cudaSuccess;
+    ok = ok && cudaMemset(c->chunk_tot, 0, (kDigitBins / 32) * sizeof(unsigned long long)) == cudaSuccess;
+    ok = ok && cudaMalloc(&c->bar, sizeof(unsigned int)) == cudaSuccess;
+    ok = ok && cudaMemset(c->bar, 0, sizeof(unsigned int)) == cudaSuccess;
+    c->coop = prop.cooperativeLaunch ? 1 : 0;
+#ifdef CUBE_SMALL_TIMING
+    ok = ok && cudaMallocManaged(&c->small_tstamp, 16 * sizeof(unsigned long long)) == cudaSuccess;
+    if (getenv("CUBE_SMALL_TSTAMP_PTR")) { FILE* fp = fopen(getenv("CUBE_SMALL_TSTAMP_PTR"), "w"); if (fp) { fprintf(fp, "%llu\n", (unsigned long long)(uintptr_t)c->small_tstamp); fclose(fp); } }
+#endif
+    ok = ok && cudaFuncSetAttribute(stats_small_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                    small_smem(kSmallMaxBins)) == cudaSuccess;
     ok = ok && cudaMemset(c->plan, 0, sizeof(BigHistPlan)) == cudaSuccess;
     ok = ok && cudaMemset(c->ticket, 0, sizeof(unsigned int)) == cudaSuccess;
     ok = ok && cudaMemset(c->gdigits, 0, kDigitBins * sizeof(unsigned long long)) == cudaSuccess;
@@ -415,7 +438,7 @@ int cube_destroy(cube_ctx* c) {
     cudaFree(c->partials); cudaFree(c->ticket); cudaFree(c->ticket2); cudaFree(c->acc);
     cudaFree(c->mom_out); cudaFree(c->gout); cudaFree(c->gdigits); cudaFree(c->coarse); cudaFree(c->sel); cudaFree(c->multi);
     cudaFree(c->range3); cudaFree(c->probe_out); cudaFree(c->plan); cudaFree(c->clip); cudaFree(c->torben); cudaFree(c->center);
-    cudaFree(c->cand); cudaFree(c->tf_table);
+    cudaFree(c->cand); cudaFree(c->tf_table); cudaFree(c->bar); cudaFree(c->coarse_next); cudaFree(c->chunk_tot);
     cudaFree(c->resident); cudaFree(c->chunk[0]); cudaFree(c->chunk[1]);
     if (c->pinned_results) cudaFreeHost(c->pinned_results);
     for (int i = 0; i < cube_ctx::kMaxStage; ++i) {
@@ -565,9 +588,46 @@ int cube_stats(cube_ctx* c, const float* d, int64_t nx, int64_t ny, int64_t nz, 
         else if (!hist_scale(nbins, lo, hi, &scale)) return CUBE_EINVAL;
     }
     int rc;
-    // pass A: moments (+ first select digit)
     float* med_direct = static_cast<float*>(device_reachable(c, median));
     MomentsOut* mom_direct = static_cast<MomentsOut*>(device_reachable(c, moments));
+    // A cube that stays in L2 between its two reads: everything in ONE cooperative launch (cube_small.cuh)
+    if (want_median && want_hist && nbins <= kSmallMaxBins && n * sizeof(float) <= ((size_t)96 << 20) && c->coop &&
+        !c->no_small) {
+        const size_t smem = (size_t)small_smem(nbins);
+        const int occ = occupancy_of(c, stats_small_kernel, kThreads, smem);
+        int per = c->ctas_per_sm > 0 ? c->ctas_per_sm : 2;
+        if (per > occ) per = occ;
+        if (per >= 1) {
+            const unsigned grid = (unsigned)(c->num_sms * per);
+            SmallArgs a;
+            a.d = d; a.n = n; a.nbins = nbins; a.lo = lo; a.hi = hi; a.scale = scale; a.minmax = minmax ? 1 : 0;
+            a.flags = flags & CUBE_SAMPLE_STD;
+            a.partials = c->partials; a.acc = c->acc; a.nvox_acc = c->nvox_acc; a.mom_out = c->mom_out; a.out_user = mom_direct;
+            std::swap(c->coarse, c->coarse_next);     // the zeroed array becomes the current one
+            a.coarse = c->coarse; a.coarse_next = c->coarse_next; a.chunk_tot = c->chunk_tot;
+            a.gdigits = c->gdigits; a.gout = c->gout;
+            a.sel = c->sel; a.cand = c->cand; a.cand_cap = c->cand ? c->cand_cap : 0; a.result_out = med_direct;
+            a.bar = c->bar; a.bar_base = c->bar_base; a.tstamp = c->small_tstamp;
+            a.bins_user = static_cast<unsigned long long*>(device_reachable(c, bins));
+            a.outside_user = static_cast<unsigned long long*>(device_reachable(c, outside));
+            if (!a.bins_user || !a.outside_user) a.bins_user = a.outside_user = nullptr;
+            void* args[] = {&a};
+            {
+                ProfScope prof(c, CUBE_K_STATS_SMALL, s);
+                CUBE_CUDA(c, cudaLaunchCooperativeKernel(reinterpret_cast<void*>(stats_small_kernel), dim3(grid), dim3(kThreads),
+                                                         args, smem, s));
+            }
+            c->bar_base += kSmallBarriers * grid;
+            if (!med_direct) CUBE_CUDA(c, cudaMemcpyAsync(median, &c->sel->result, sizeof(float), cudaMemcpyDefault, s));
+            if (moments && !mom_direct) CUBE_CUDA(c, cudaMemcpyAsync(moments, c->mom_out, sizeof(MomentsOut), cudaMemcpyDefault, s));
+            if (!a.bins_user) {
+                CUBE_CUDA(c, cudaMemcpyAsync(bins, c->gbins, (size_t)nbins * sizeof(uint64_t), cudaMemcpyDefault, s));
+                CUBE_CUDA(c, cudaMemcpyAsync(outside, c->gout, 2 * sizeof(uint64_t), cudaMemcpyDefault, s));
+            }
+            return CUBE_OK;
+        }
+    }
+    // pass A: moments (+ first select digit)
     const SelectInit init = select_init_args(c, 0, 1, true), cont = select_init_args(c, 0, 0, false, med_direct);
     const unsigned mflags = (flags & CUBE_SAMPLE_STD) | (want_median ? (unsigned)CUBE_COARSE_HIST : 0u);
     if ((rc = launch_moments(c, d, n, mflags, 0, s, -1, 0.f, 0.f, false, want_median ? &init : nullptr, mom_direct))) return rc;
@@ -936,6 +996,10 @@ int cube_set_knob(cube_ctx* c, int knob, int value) {
         case CUBE_KNOB_BIGHIST:
             if (value < 0 || value > 2) return CUBE_EINVAL;
             c->bighist = value;
+            return CUBE_OK;
+        case CUBE_KNOB_SMALL:
+            if (value < 0 || value > 1) return CUBE_EINVAL;
+            c->no_small = value;
             return CUBE_OK;
         case CUBE_KNOB_MINIMAP:
             if (value < 0 || value > 3) return CUBE_EINVAL;

@@ -9,6 +9,16 @@
 #include <cuda_runtime.h>
 #include <stdint.h>
 
+// -DCUBE_CHECKED: every index into a per-warp queue, key stage or the candidate buffer is checked against its
+// capacity and a violation traps (the launch fails with cudaErrorLaunchFailure and every test that runs it fails).
+// compute-sanitizer is not available on the GPU pool this library is developed on; the checked build run over the
+// GPU test suite stands in for its memcheck on the hand-rolled staging structures (profiles/r2_checks.md).
+#ifdef CUBE_CHECKED
+#define CUBE_CHECK(cond) do { if (!(cond)) __trap(); } while (0)
+#else
+#define CUBE_CHECK(cond) do { } while (0)
+#endif
+
 namespace cube {
 
 constexpr int kThreads = 256;  // threads per CTA (8 warps)

@@ -26,11 +26,24 @@ struct HistSelectF {
     }
 };
 
+// What pass B needs to know of the selection: the first-digit bucket (or "nothing to select") and where the
+// candidates go.  Read from the SelectState in device memory, or -- cube_small.cuh -- from a CTA's own copy.
+struct SelView {
+    uint32_t invalid, prefix;
+    unsigned long long* cand_n;
+    unsigned long long cand_cap;
+};
+__device__ __forceinline__ SelView sel_view(SelectState* __restrict__ st) {
+    SelView v;
+    v.invalid = st->invalid; v.prefix = st->prefix; v.cand_n = &st->cand_n; v.cand_cap = st->cand_cap;
+    return v;
+}
+
 template <class H>
 __device__ __forceinline__ void hist_select_run(const float* __restrict__ d, uint64_t n, const H& h,
-                                                SelectState* __restrict__ st, uint32_t* sbins, uint32_t* stage,
+                                                const SelView& sv, uint32_t* sbins, uint32_t* stage,
                                                 uint32_t* __restrict__ cand, uint32_t& below, uint32_t& above) {
-    if (st->invalid) {  // nothing to select (k >= count): histogram only
+    if (sv.invalid) {  // nothing to select (k >= count): histogram only
         H f = h;
         stream_cube<kThreads>(d, n, f);
         below = f.below; above = f.above;
@@ -38,9 +51,9 @@ __device__ __forceinline__ void hist_select_run(const float* __restrict__ d, uin
     }
     HistSelectF<H> f;
     f.h = h;
-    const uint32_t top = st->prefix;
+    const uint32_t top = sv.prefix;
     f.s.base = top << kShift0; f.s.rawbase = raw_of_digit(top) << kShift0; f.s.sbins = sbins;
-    f.s.init_stage(stage, cand, &st->cand_n, st->cand_cap);
+    f.s.init_stage(stage, cand, sv.cand_n, sv.cand_cap);
     stream_cube<kThreads>(d, n, f);
     f.s.finish();
     below = f.h.below; above = f.h.above;
@@ -83,11 +96,11 @@ hist_select_kernel(const float* __restrict__ d, uint64_t n, int nbins, float lo,
     if (hist_use_fast(nbins, lo, hi, scale)) {
         HistFastF h;
         h.setup(lo, hi, scale, nbins, hbins, s_out);
-        hist_select_run(d, n, h, st, sbins, stage, cand, below, above);
+        hist_select_run(d, n, h, sel_view(st), sbins, stage, cand, below, above);
     } else {
         HistF h;
         h.lo = lo; h.hi = hi; h.scale = scale; h.top = nbins - 1; h.sbins = hbins;
-        hist_select_run(d, n, h, st, sbins, stage, cand, below, above);
+        hist_select_run(d, n, h, sel_view(st), sbins, stage, cand, below, above);
     }
     __syncthreads();
     hist_flush_bins(hbins, nbins, gbins);

@@ -44,6 +44,7 @@ static __device__ __forceinline__ void gather_flush(WarpGather* w, const GatherS
     if (lane == 0) pos = atomicAdd(sh->cand_n, (unsigned long long)c);
     pos = __shfl_sync(0xffffffffu, pos, 0);
     if (pos + c <= sh->cand_cap) {
+        CUBE_CHECK(c <= (uint32_t)kKeyCap);
         for (uint32_t i = lane; i < c; i += 32) sh->cand[pos + i] = w->keys[i];
     } else if (lane == 0) {
         w->compacting = 0;           // the bucket does not fit: the last digit will be counted over the cube
@@ -58,6 +59,7 @@ static __device__ __noinline__ void gather_rows(WarpGather* w, const GatherShare
     constexpr uint32_t kSpan = 1u << kShift0;
     const uint32_t lane = threadIdx.x & 31;
     const bool act = lane < n;
+    CUBE_CHECK(first + n <= (uint32_t)kRowQCap && n <= 32u);
     const float4 v = w->rows[first + (act ? lane : 0)];
     const uint32_t base = sh->base;
     const float x[4] = {v.x, v.y, v.z, v.w};
@@ -73,6 +75,7 @@ static __device__ __noinline__ void gather_rows(WarpGather* w, const GatherShare
     if (w->compacting) {             // warp-uniform
         uint32_t pos = nh ? atomicAdd(&w->nkeys, nh) : 0u;
 #pragma unroll
+        CUBE_CHECK(pos + nh <= (uint32_t)kKeyCap);
         for (int i = 0; i < 4; ++i)
             if (hit[i]) w->keys[pos++] = kk[i] + base;
         __syncwarp();
@@ -111,6 +114,7 @@ static __device__ __noinline__ void gather_cold(uint32_t rows, const float4* __r
         const uint32_t cnt = (j0 >= 0 ? 1u : 0u) + (j1 >= 0 ? 1u : 0u);
         if (cnt) {
             uint32_t slot = atomicAdd(&w->nrows, cnt);
+            CUBE_CHECK(slot + cnt <= (uint32_t)kRowQCap);
             w->rows[slot] = a;
             if (j1 >= 0) w->rows[slot + 1] = b;
         }

@@ -207,6 +207,86 @@ struct ClipState {
     unsigned long long prev_count;  // count of the statistics the window was formed from
 };
 
+// Fixed-order merge of `nparts` per-CTA partials by ONE CTA of kThreads threads (all of them call; the result is valid
+// in thread 0).  `scratch`: kThreads / 32 Partials of shared memory, free on entry.
+__device__ __forceinline__ Partial partials_merge_block(const Partial* __restrict__ partials, unsigned nparts, Partial* scratch) {
+    // last CTA: fixed-order merge of the per-CTA partials.  A tree of Chan merges is a chain of ~13 dependent fp64
+    // divisions (5 us of tail on a cube that streams in 10 us: profiles/r1_v11_c2.md), so the partials are first
+    // re-expressed as sums about ONE pivot P -- the mean of the lowest-indexed non-empty partial: s_i = n_i (mean_i -
+    // P), q_i = M2_i + n_i (mean_i - P)^2 -- which merge by plain additions (thread i takes i, i+256, ...; then
+    // shuffles).  P is the mean of a CTA whose tiles are spread over the whole cube, so |P - mean| << std and
+    // q - s^2/n loses nothing; a constant cube gives mean_i == P, s = q = 0 and std = 0 exactly.
+    __shared__ unsigned int first_live;
+    __shared__ double pivot_sm;
+    __shared__ int again_sm;
+    unsigned int first = 0;   // block-uniform: partial 0 unless CTA 0 saw only NULL voxels (then the search below)
+    if (__ldcg(&partials[0].n) == 0) {
+        if (threadIdx.x == 0) first_live = 0xFFFFFFFFu;
+        __syncthreads();
+        unsigned int mine = 0xFFFFFFFFu;
+        for (unsigned i = threadIdx.x; i < nparts; i += kThreads)
+            if (mine == 0xFFFFFFFFu && __ldcg(&partials[i].n) != 0) mine = i;
+        if (mine != 0xFFFFFFFFu) atomicMin(&first_live, mine);
+        __syncthreads();
+        first = first_live;
+    }
+    Partial m = partial_empty();
+    if (first != 0xFFFFFFFFu) {
+        if (threadIdx.x == 0) again_sm = 0;
+        double P = __ldcg(&partials[first].mean);
+        // Second round only if the pivot turned out to be far from the mean (more than 16 standard deviations: data
+        // arranged so that CTA first_live saw something else than the rest): q - s^2/n would then cancel ~2^8 or more
+        // of the 2^53; the refined pivot P + s/n is as good as the mean itself.
+#pragma unroll 1
+        for (int round = 0; round < 2; ++round) {
+            unsigned long long cn = 0;
+            double cs = 0.0, cq = 0.0;
+            uint32_t kmin = 0xFFFFFFFFu, kmax = 0u;
+            for (unsigned i = threadIdx.x; i < nparts; i += kThreads) {   // written by other CTAs: read through L2
+                const unsigned long long bn = __ldcg(&partials[i].n);
+                const double bmean = __ldcg(&partials[i].mean), bm2 = __ldcg(&partials[i].m2);
+                kmin = min(kmin, __ldcg(&partials[i].kmin));
+                kmax = max(kmax, __ldcg(&partials[i].kmax));
+                if (bn) {
+                    const double nb = (double)bn, dm = bmean - P, nd = nb * dm;
+                    cn += bn; cs += nd; cq += bm2 + nd * dm;
+                }
+            }
+#pragma unroll
+            for (int off = 16; off > 0; off >>= 1) {
+                cn += __shfl_down_sync(0xffffffffu, cn, off);
+                cs += __shfl_down_sync(0xffffffffu, cs, off);
+                cq += __shfl_down_sync(0xffffffffu, cq, off);
+                kmin = min(kmin, __shfl_down_sync(0xffffffffu, kmin, off));
+                kmax = max(kmax, __shfl_down_sync(0xffffffffu, kmax, off));
+            }
+            const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+            __syncthreads();   // scratch is free (the CTA's own block reduce / the round before is over)
+            if (lane == 0) { scratch[warp].n = cn; scratch[warp].mean = cs; scratch[warp].m2 = cq; scratch[warp].kmin = kmin; scratch[warp].kmax = kmax; }
+            __syncthreads();
+            if (threadIdx.x == 0) {
+                cn = 0; cs = 0.0; cq = 0.0; kmin = 0xFFFFFFFFu; kmax = 0u;
+#pragma unroll
+                for (int w = 0; w < kThreads / 32; ++w) {
+                    cn += scratch[w].n; cs += scratch[w].mean; cq += scratch[w].m2;
+                    kmin = min(kmin, scratch[w].kmin); kmax = max(kmax, scratch[w].kmax);
+                }
+                const double nn = (double)cn, shift = cs / nn;
+                const double m2 = cq - cs * shift;
+                m.n = cn; m.mean = P + shift; m.m2 = (m2 < 0.0) ? 0.0 : m2;   // rounding only; a NaN (Inf voxels) stays
+                m.kmin = kmin; m.kmax = kmax;
+                const bool far = round == 0 && shift * shift * nn > 256.0 * m.m2 && isfinite(m.mean);
+                again_sm = far ? 1 : 0;
+                if (far) pivot_sm = m.mean;
+            }
+            __syncthreads();
+            if (!again_sm) break;
+            P = pivot_sm;
+        }
+    }
+    return m;
+}
+
 // acc : running Partial across calls (out-of-core bricks); merged in call order => deterministic.
 // nvox_acc : running voxel total.  When `accumulate` is 0 both are overwritten.
 // kMomWindow: the window is (wlo, whi), or *clip when clip != nullptr (then a finished clip makes the kernel a no-op).
@@ -261,81 +341,9 @@ moments_kernel(const float* __restrict__ d, uint64_t n, Partial* __restrict__ pa
     }
     __syncthreads();
     if (!is_last) return;
-    // last CTA: fixed-order merge of the per-CTA partials.  A tree of Chan merges is a chain of ~13 dependent fp64
-    // divisions (5 us of tail on a cube that streams in 10 us: profiles/r1_v11_c2.md), so the partials are first
-    // re-expressed as sums about ONE pivot P -- the mean of the lowest-indexed non-empty partial: s_i = n_i (mean_i -
-    // P), q_i = M2_i + n_i (mean_i - P)^2 -- which merge by plain additions (thread i takes i, i+256, ...; then
-    // shuffles).  P is the mean of a CTA whose tiles are spread over the whole cube, so |P - mean| << std and
-    // q - s^2/n loses nothing; a constant cube gives mean_i == P, s = q = 0 and std = 0 exactly.
+    // last CTA: fixed-order merge of the per-CTA partials (partials_merge_block)
     __threadfence();
-    __shared__ unsigned int first_live;
-    __shared__ double pivot_sm;
-    __shared__ int again_sm;
-    unsigned int first = 0;   // block-uniform: partial 0 unless CTA 0 saw only NULL voxels (then the search below)
-    if (__ldcg(&partials[0].n) == 0) {
-        if (threadIdx.x == 0) first_live = 0xFFFFFFFFu;
-        __syncthreads();
-        unsigned int mine = 0xFFFFFFFFu;
-        for (unsigned i = threadIdx.x; i < gridDim.x; i += kThreads)
-            if (mine == 0xFFFFFFFFu && __ldcg(&partials[i].n) != 0) mine = i;
-        if (mine != 0xFFFFFFFFu) atomicMin(&first_live, mine);
-        __syncthreads();
-        first = first_live;
-    }
-    Partial m = partial_empty();
-    if (first != 0xFFFFFFFFu) {
-        if (threadIdx.x == 0) again_sm = 0;
-        double P = __ldcg(&partials[first].mean);
-        // Second round only if the pivot turned out to be far from the mean (more than 16 standard deviations: data
-        // arranged so that CTA first_live saw something else than the rest): q - s^2/n would then cancel ~2^8 or more
-        // of the 2^53; the refined pivot P + s/n is as good as the mean itself.
-#pragma unroll 1
-        for (int round = 0; round < 2; ++round) {
-            unsigned long long cn = 0;
-            double cs = 0.0, cq = 0.0;
-            uint32_t kmin = 0xFFFFFFFFu, kmax = 0u;
-            for (unsigned i = threadIdx.x; i < gridDim.x; i += kThreads) {   // written by other CTAs: read through L2
-                const unsigned long long bn = __ldcg(&partials[i].n);
-                const double bmean = __ldcg(&partials[i].mean), bm2 = __ldcg(&partials[i].m2);
-                kmin = min(kmin, __ldcg(&partials[i].kmin));
-                kmax = max(kmax, __ldcg(&partials[i].kmax));
-                if (bn) {
-                    const double nb = (double)bn, dm = bmean - P, nd = nb * dm;
-                    cn += bn; cs += nd; cq += bm2 + nd * dm;
-                }
-            }
-#pragma unroll
-            for (int off = 16; off > 0; off >>= 1) {
-                cn += __shfl_down_sync(0xffffffffu, cn, off);
-                cs += __shfl_down_sync(0xffffffffu, cs, off);
-                cq += __shfl_down_sync(0xffffffffu, cq, off);
-                kmin = min(kmin, __shfl_down_sync(0xffffffffu, kmin, off));
-                kmax = max(kmax, __shfl_down_sync(0xffffffffu, kmax, off));
-            }
-            const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
-            __syncthreads();   // scratch is free (the CTA's own block reduce / the round before is over)
-            if (lane == 0) { scratch[warp].n = cn; scratch[warp].mean = cs; scratch[warp].m2 = cq; scratch[warp].kmin = kmin; scratch[warp].kmax = kmax; }
-            __syncthreads();
-            if (threadIdx.x == 0) {
-                cn = 0; cs = 0.0; cq = 0.0; kmin = 0xFFFFFFFFu; kmax = 0u;
-#pragma unroll
-                for (int w = 0; w < kThreads / 32; ++w) {
-                    cn += scratch[w].n; cs += scratch[w].mean; cq += scratch[w].m2;
-                    kmin = min(kmin, scratch[w].kmin); kmax = max(kmax, scratch[w].kmax);
-                }
-                const double nn = (double)cn, shift = cs / nn;
-                const double m2 = cq - cs * shift;
-                m.n = cn; m.mean = P + shift; m.m2 = (m2 < 0.0) ? 0.0 : m2;   // rounding only; a NaN (Inf voxels) stays
-                m.kmin = kmin; m.kmax = kmax;
-                const bool far = round == 0 && shift * shift * nn > 256.0 * m.m2 && isfinite(m.mean);
-                again_sm = far ? 1 : 0;
-                if (far) pivot_sm = m.mean;
-            }
-            __syncthreads();
-            if (!again_sm) break;
-            P = pivot_sm;
-        }
-    }
+    Partial m = partials_merge_block(partials, gridDim.x, scratch);
     if (threadIdx.x == 0) {
         unsigned long long tot = n;
         if (accumulate) { m = partial_merge(*acc, m); tot += *nvox_acc; }

@@ -123,7 +123,7 @@ __device__ __forceinline__ float med_cell(const float* __restrict__ d, const Med
         const uint32_t hi_mask = pass == 0 ? 0u : (0xFFFFFFFFu << (shift + 8));   // bits fixed so far
         if (pass == 0 || !STAGED) {
             for_each_key([&](uint32_t key, uint32_t idx) {
-                if (pass == 0) { nan += key == 0xFFFFFFFFu ? 1u : 0u; if (STAGED) keys[idx] = key; }
+                if (pass == 0) { nan += key == 0xFFFFFFFFu ? 1u : 0u; if (STAGED) { CUBE_CHECK(idx < nvox); keys[idx] = key; } }
                 if ((key & hi_mask) == prefix) atomicAdd(&hist[(key >> shift) & 255u], 1u);
             });
         } else {

@@ -108,7 +108,11 @@ struct SelectF {
         const uint32_t kk = key_of(x) - base_;
         if (kk < kSpan && x == x) {
             atomicAdd(&sbins_[kk >> kBits2], 1u);
-            if (s_cnt_) s_buf_[atomicAdd(s_cnt_, 1u)] = kk + base_;
+            if (s_cnt_) {
+                const uint32_t slot = atomicAdd(s_cnt_, 1u);
+                CUBE_CHECK(slot < kStageCap);
+                s_buf_[slot] = kk + base_;
+            }
         }
     }
     static __device__ __noinline__ void cold(uint32_t rows, const float4* __restrict__ p, uint32_t base_,
@@ -129,6 +133,7 @@ struct SelectF {
         unsigned long long pos = 0;
         if (lane == 0) pos = atomicAdd(cand_n, (unsigned long long)c);
         pos = __shfl_sync(0xffffffffu, pos, 0);
+        CUBE_CHECK(c <= kStageCap);
         if (pos + c <= cand_cap) {
             for (uint32_t i = lane; i < c; i += 32) cand[pos + i] = s_buf[i];
         } else {

@@ -115,7 +115,11 @@ struct GatherF {
         return m;
     }
     __device__ __forceinline__ void take(float x) {
-        if (dist(x) < kSpan && x == x && compacting) s_buf[atomicAdd(s_cnt, 1u)] = key_of(x);
+        if (dist(x) < kSpan && x == x && compacting) {
+            const uint32_t slot = atomicAdd(s_cnt, 1u);
+            CUBE_CHECK(slot < kStageCap);
+            s_buf[slot] = key_of(x);
+        }
     }
     __device__ __forceinline__ void operator()(float x) {   // head / tail / ragged last tile: straight to the buffer
         if (dist(x) < kSpan && x == x) {

@@ -1,0 +1,300 @@
+// cube_small.cuh -- cube_stats for cubes that fit the L2 cache (config 1 of BASELINE.json: 256^3, 64 MiB) in ONE
+// cooperative launch instead of three dependent ones.
+//
+// A 64 MiB cube streams in ~10 us; the three launches of the general path (pass A, pass B, pass C) then cost more in
+// launch gaps and serial tails -- the last CTA of pass A alone merging 592 partials and scanning 8192 digit bins while
+// 147 SMs idle -- than in reading (73 us against a 2 x 13 us floor, profiles/r1_v11_c2.md sec. 3).  Here all CTAs are
+// resident (cooperative launch), the passes are separated by grid barriers, and what used to be a last-CTA tail is
+// done by EVERY CTA for itself: each CTA merges the per-CTA partials and locates the first-digit bucket redundantly
+// (the inputs are a few KiB in L2), so nobody waits for one CTA's chain of dependent L2 round trips and no
+// selection state crosses a launch boundary.  The kernels' arithmetic is that of the general path -- the same functors
+// (MomentsF, HistFastF / HistF, SelectF), the same merge, the same bucket location -- so the results are bit for bit
+// the same integers; mean / std differ in the last bits only through the grid size (tolerance R20).
+//
+//   phase A  moments + first digit (pass A); the histogram bins are zeroed on the way  | grid barrier
+//            every CTA: merge the partials, locate the median's first-digit bucket (from 256 chunk totals)
+//   phase B  histogram + second digit + candidate compaction (pass B), from L2        | grid barrier
+//            candidates fit (the usual case): CTA 0 counts the last digit on them and finishes; the other CTAs exit
+//            else: every CTA locates the second-digit bucket, counts the last digit over the cube | grid barrier, CTA 0 finishes
+#pragma once
+#include "cube_fused.cuh"
+
+namespace cube {
+
+struct SmallArgs {
+    const float* d; uint64_t n;
+    int nbins; float lo, hi, scale; int minmax; unsigned flags;
+    Partial* partials; Partial* acc; unsigned long long* nvox_acc; MomentsOut* mom_out; MomentsOut* out_user;
+    unsigned long long* coarse;      // kDigitBins first-digit counts (kept for CUBE_REUSE_COARSE); all zero on entry
+    unsigned long long* coarse_next; // the array the NEXT call will use: zeroed here by the CTAs that finish early
+    unsigned long long* chunk_tot;   // kDigitBins / 32 totals of 32 consecutive first digits, in KEY order; zero on
+                                     // entry, left zeroed
+    unsigned long long* gdigits;     // kDigitBins: [0, 1024) second digit, [4096, 4608) last digit; left zeroed
+    unsigned long long* gout;        // [outside (2)][bins (nbins)]
+    SelectState* sel; uint32_t* cand; unsigned long long cand_cap; float* result_out;
+    unsigned long long* bins_user;   // the caller's bins / outside when the device can reach them (no copy is enqueued then)
+    unsigned long long* outside_user;
+    unsigned int* bar; unsigned int bar_base;
+    unsigned long long* tstamp;      // debug (-DCUBE_SMALL_TIMING): %globaltimer of CTA 0 at the phase boundaries
+};
+
+constexpr int kSmallMaxBins = 4096;
+constexpr int kSmallDigit2Off = 4096;
+constexpr int small_smem(int nbins) {
+    const int b = (nbins + 2 + kBins1 + 1 + (kThreads / 32) * ((int)kStageCap + 1)) * 4;
+    const int a = (kDigitBins + 1) * 4;
+    return a > b ? a : b;
+}
+
+// Grid barrier for a cooperative launch (all CTAs resident).  The counter only grows: arrival number base + k * grid
+// ends barrier k, so nothing has to be reset while CTAs may still be spinning.
+__device__ __forceinline__ void small_grid_sync(unsigned int* bar, unsigned int target) {
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        __threadfence();
+        atomicAdd(bar, 1u);
+        unsigned int v;
+        do {
+            asm volatile("ld.acquire.gpu.global.u32 %0, [%1];" : "=r"(v) : "l"(bar) : "memory");
+        } while ((int)(v - target) < 0);
+        __threadfence();
+    }
+    __syncthreads();
+}
+// Arrive without waiting (a CTA that is done): every launch makes the same number of arrivals, which is what the
+// host advances the barrier base by.
+__device__ __forceinline__ void small_grid_arrive(unsigned int* bar) {
+    __syncthreads();
+    if (threadIdx.x == 0) { __threadfence(); atomicAdd(bar, 1u); }
+}
+constexpr unsigned kSmallBarriers = 3;
+
+// First-digit bucket of the median from the chunk totals (256 sums of 32 consecutive digits, key order) and the one
+// chunk that holds the rank: two dependent L2 round trips of ONE warp instead of a scan of all 8192 bins.  Called by
+// warp 0 of every CTA; fills the CTA's own SelectState.
+__device__ __forceinline__ void small_locate0(SelectState* st, const unsigned long long* __restrict__ coarse,
+                                              const unsigned long long* __restrict__ chunk_tot, unsigned long long cand_cap) {
+    constexpr int NCH = kDigitBins / 32, PER = NCH / 32;
+    const int lane = threadIdx.x & 31;
+    unsigned long long c[PER], mine = 0;
+#pragma unroll
+    for (int j = 0; j < PER; ++j) { c[j] = __ldcg(&chunk_tot[lane * PER + j]); mine += c[j]; }
+    unsigned long long incl = mine;
+#pragma unroll
+    for (int off = 1; off < 32; off <<= 1) {
+        const unsigned long long u = __shfl_up_sync(0xffffffffu, incl, off);
+        if (lane >= off) incl += u;
+    }
+    const unsigned long long total = __shfl_sync(0xffffffffu, incl, 31);
+    const unsigned long long k = total ? (total - 1) / 2 : 0;
+    unsigned long long excl = incl - mine;
+    int ch = -1;
+    unsigned long long kin = 0;
+#pragma unroll
+    for (int j = 0; j < PER; ++j) {
+        if (c[j] && excl <= k && k < excl + c[j]) { ch = lane * PER + j; kin = k - excl; }   // exactly one lane (total > 0)
+        excl += c[j];
+    }
+    const unsigned ball = __ballot_sync(0xffffffffu, ch >= 0);
+    if (lane == 0) {
+        st->count = total; st->invalid = total ? 0u : 1u; st->use_median = 1u; st->cand_n = 0; st->cand_cap = cand_cap;
+        st->cand_done = 0u; st->k = k; st->prefix = 0u; st->result = __int_as_float(0x7fc00000);
+    }
+    if (!ball) return;
+    const int src = __ffs(ball) - 1;
+    ch = __shfl_sync(0xffffffffu, ch, src);
+    kin = __shfl_sync(0xffffffffu, kin, src);
+    const uint32_t digit = (uint32_t)ch * 32u + (uint32_t)lane;
+    const unsigned long long x = __ldcg(&coarse[raw_of_digit(digit)]);
+    unsigned long long inc2 = x;
+#pragma unroll
+    for (int off = 1; off < 32; off <<= 1) {
+        const unsigned long long u = __shfl_up_sync(0xffffffffu, inc2, off);
+        if (lane >= off) inc2 += u;
+    }
+    const unsigned long long ex2 = inc2 - x;
+    __syncwarp();
+    if (x && ex2 <= kin && kin < inc2) { st->prefix = digit; st->k = kin - ex2; }   // exactly one lane
+}
+
+#ifdef CUBE_SMALL_TIMING
+#define SMALL_T(i) do { if (a.tstamp && blockIdx.x == 0 && threadIdx.x == 0) { unsigned long long t_; asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t_)); a.tstamp[i] = t_; } } while (0)
+#else
+#define SMALL_T(i) do { } while (0)
+#endif
+
+__global__ void __launch_bounds__(kThreads, 3)
+stats_small_kernel(SmallArgs a) {
+    extern __shared__ __align__(16) uint32_t dyn_bins[];
+    __shared__ Partial scratch[kThreads / 32];
+    __shared__ SelectState s_sel;
+    __shared__ unsigned long long scan_sm[kScanSmem];
+    __shared__ MomentsOut s_mom;
+    __shared__ uint32_t s_out[2];
+    const unsigned grid = gridDim.x;
+    const unsigned gtid = blockIdx.x * kThreads + threadIdx.x, gthreads = grid * kThreads;
+
+    SMALL_T(0);
+    // ---- phase 0 (no barrier): what phase B accumulates into is zeroed now -- two grid barriers lie in between; the
+    // first-digit bins and the chunk totals arrive zeroed (every call leaves the next call's arrays that way)
+    for (unsigned i = gtid; i < (unsigned)a.nbins + 2u; i += gthreads) a.gout[i] = 0ull;
+    if (gtid == 0) { a.sel->cand_n = 0ull; a.sel->cand_done = 0u; }
+    SMALL_T(1);
+    // ---- phase A: moments + first digit
+    {
+        MomentsF<kMomCoarse> f;
+        f.sbins = smem_addr(dyn_bins);
+        for (int i = threadIdx.x; i <= kDigitBins; i += kThreads) dyn_bins[i] = 0;
+        __syncthreads();
+        stream_cube<kThreads>(a.d, a.n, f);
+        SMALL_T(2);
+        f.unsubstitute();
+        const Partial p = partial_block_reduce(f.partial(), scratch);
+        __syncthreads();
+        // flush: a warp takes chunks of 32 consecutive raw digits; their sum also goes to the chunk's total (a chunk of
+        // raw digits IS a chunk of key-order digits: raw chunk r <-> key chunk r + 128 (positive) or 255 - r (negative))
+        for (int ch = threadIdx.x >> 5; ch < kDigitBins / 32; ch += kThreads / 32) {
+            const uint32_t c = dyn_bins[ch * 32 + (threadIdx.x & 31)];
+            if (c) atomicAdd(&a.coarse[ch * 32 + (threadIdx.x & 31)], (unsigned long long)c);
+            const uint32_t tot = __reduce_add_sync(0xffffffffu, c);
+            if ((threadIdx.x & 31) == 0 && tot)
+                atomicAdd(&a.chunk_tot[ch < 128 ? ch + 128 : 255 - ch], (unsigned long long)tot);
+        }
+        if (threadIdx.x == 0) a.partials[blockIdx.x] = p;
+    }
+    small_grid_sync(a.bar, a.bar_base + grid);
+
+    SMALL_T(3);
+    // ---- every CTA for itself: the merged moments record and the first-digit bucket
+    {
+        const Partial m = partials_merge_block(a.partials, grid, scratch);
+        if (threadIdx.x == 0) {
+            moments_finalize(m, a.n, a.flags, &s_mom);
+            if (blockIdx.x == 0) {
+                *a.acc = m; *a.nvox_acc = a.n; *a.mom_out = s_mom;
+                if (a.out_user) *a.out_user = s_mom;
+            }
+        }
+        if (threadIdx.x < 32) small_locate0(&s_sel, a.coarse, a.chunk_tot, a.cand ? a.cand_cap : 0);
+        __syncthreads();
+    }
+
+    SMALL_T(4);
+    // ---- phase B: histogram + second digit + compaction (the cube comes from L2 now)
+    {
+        uint32_t* hbins = dyn_bins;
+        uint32_t* sbins = dyn_bins + (a.nbins + 2);
+        uint32_t* stage = sbins + (kBins1 + 1);
+        for (int i = threadIdx.x; i < a.nbins + 2 + kBins1 + 1; i += kThreads) dyn_bins[i] = 0;
+        if (threadIdx.x < 2) s_out[threadIdx.x] = 0;
+        __syncthreads();
+        float lo = a.lo, hi = a.hi, scale = a.scale;
+        const bool range_ok = hist_range(a.minmax ? &s_mom : nullptr, a.nbins, lo, hi, scale);
+        if (!range_ok) { lo = INFINITY; hi = -INFINITY; }   // nothing is in range: every counter stays 0
+        SelView sv;
+        sv.invalid = s_sel.invalid; sv.prefix = s_sel.prefix; sv.cand_n = &a.sel->cand_n; sv.cand_cap = a.cand ? a.cand_cap : 0;
+        uint32_t below = 0, above = 0;
+        if (hist_use_fast(a.nbins, lo, hi, scale)) {
+            HistFastF h;
+            h.setup(lo, hi, scale, a.nbins, hbins, s_out);
+            hist_select_run(a.d, a.n, h, sv, sbins, stage, a.cand, below, above);
+        } else {
+            HistF h;
+            h.lo = lo; h.hi = hi; h.scale = scale; h.top = a.nbins - 1; h.sbins = hbins;
+            hist_select_run(a.d, a.n, h, sv, sbins, stage, a.cand, below, above);
+        }
+        __syncthreads();
+        SMALL_T(5);
+        hist_flush_bins(hbins, a.nbins, a.gout + 2);
+        for (int i = threadIdx.x; i < kBins1; i += kThreads) {
+            const uint32_t c = sbins[i];
+            if (c) atomicAdd(&a.gdigits[i], (unsigned long long)c);
+        }
+        if (range_ok) {
+            if (below) atomicAdd(&s_out[0], below);
+            if (above) atomicAdd(&s_out[1], above);
+            __syncthreads();
+            if (threadIdx.x < 2 && s_out[threadIdx.x]) atomicAdd(&a.gout[threadIdx.x], (unsigned long long)s_out[threadIdx.x]);
+        } else if (blockIdx.x == 0 && threadIdx.x < 2) {
+            a.gout[threadIdx.x] = ~0ull;  // marker: the [min,max] range was unusable
+        }
+    }
+    small_grid_sync(a.bar, a.bar_base + 2 * grid);
+
+    SMALL_T(6);
+    // ---- last digit
+    unsigned long long cn;
+    asm volatile("ld.relaxed.gpu.global.u64 %0, [%1];" : "=l"(cn) : "l"(&a.sel->cand_n) : "memory");
+    const bool fits = a.cand != nullptr && cn <= a.cand_cap;   // the same on every CTA: cand_n is final
+    // the array the next call counts first digits into (nobody reads it in this call)
+    for (unsigned i = gtid; i < (unsigned)kDigitBins; i += gthreads) a.coarse_next[i] = 0ull;
+    if (a.bins_user) {   // the histogram is complete: straight into the caller's buffers
+        for (unsigned i = gtid; i < (unsigned)a.nbins; i += gthreads) a.bins_user[i] = __ldcg(&a.gout[2 + i]);
+        if (gtid < 2) a.outside_user[gtid] = __ldcg(&a.gout[gtid]);
+    }
+    if (fits && blockIdx.x != 0) { small_grid_arrive(a.bar); return; }
+    SelectInit none;
+    none.k = 0; none.cand_cap = 0; none.result_out = nullptr; none.use_median = 0; none.enabled = 0;
+    select_scan_body<1, kThreads>(&s_sel, a.gdigits, 0, none, scan_sm);     // every remaining CTA: second-digit bucket
+    __syncthreads();
+    unsigned long long* g2 = a.gdigits + kSmallDigit2Off;
+    {
+        uint32_t* sbins = dyn_bins;
+        for (int i = threadIdx.x; i <= kBins2; i += kThreads) sbins[i] = 0;
+        __syncthreads();
+        if (!s_sel.invalid) {
+            if (fits) {
+                SelectF<2, false> f;
+                f.base = s_sel.prefix << kBits2; f.sbins = sbins;
+                for (uint64_t i0 = 0; i0 < cn; i0 += 8 * kThreads) {      // eight loads in flight per thread
+                    uint32_t key[8];
+#pragma unroll
+                    for (int u = 0; u < 8; ++u) {
+                        const uint64_t i = i0 + (uint64_t)u * kThreads + threadIdx.x;
+                        key[u] = i < cn ? __ldcg(a.cand + i) : 0u;
+                    }
+#pragma unroll
+                    for (int u = 0; u < 8; ++u)
+                        if (i0 + (uint64_t)u * kThreads + threadIdx.x < cn) f.key(key[u]);
+                }
+            } else {   // the bucket did not fit the candidate buffer: the cube once more, all CTAs
+                const uint32_t top = s_sel.prefix >> kBits1;
+                if (digit_may_hold_nan(top)) {
+                    SelectF<2, true> f; f.base = s_sel.prefix << kBits2; f.sbins = sbins;
+                    stream_cube<kThreads>(a.d, a.n, f);
+                } else {
+                    SelectF<2, false> f; f.base = s_sel.prefix << kBits2; f.sbins = sbins;
+                    stream_cube<kThreads>(a.d, a.n, f);
+                }
+            }
+        }
+        __syncthreads();
+        for (int i = threadIdx.x; i < kBins2; i += kThreads) {
+            const uint32_t c = sbins[i];
+            if (c) atomicAdd(&g2[i], (unsigned long long)c);
+        }
+    }
+    if (!fits) {
+        small_grid_sync(a.bar, a.bar_base + 3 * grid);
+        if (blockIdx.x != 0) return;
+    } else {
+        small_grid_arrive(a.bar);
+        __syncthreads();
+    }
+    SMALL_T(7);
+    // ---- CTA 0: the key is complete
+    SelectInit fin = none;
+    fin.result_out = a.result_out;
+    select_scan_body<2, kThreads>(&s_sel, g2, 0, fin, scan_sm);
+    __syncthreads();
+    for (int i = threadIdx.x; i < kDigitBins; i += kThreads) a.gdigits[i] = 0ull;   // as the general path leaves them
+    for (int i = threadIdx.x; i < kDigitBins / 32; i += kThreads) a.chunk_tot[i] = 0ull;
+    if (threadIdx.x == 0) {
+        SelectState* g = a.sel;          // the state a later CUBE_REUSE_COARSE selection or a reader of the context finds
+        g->k = s_sel.k; g->count = s_sel.count; g->prefix = s_sel.prefix; g->invalid = s_sel.invalid;
+        SMALL_T(8);
+        g->use_median = 1u; g->result = s_sel.result; g->cand_cap = a.cand ? a.cand_cap : 0; g->cand_done = fits ? 1u : 0u;
+    }
+}
+
+}  // namespace cube
