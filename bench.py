@@ -428,6 +428,8 @@ def measure_in_hbm(name, args, dev, rank, world, dist, steps, warmup, sustain_s,
     for _ in range(warmup):
         step()
     torch.cuda.synchronize()
+    # clocks / throttle reasons are sampled from here on: the same steps, run back to back, through the timed region
+    sampler = ClockSampler(dev.index or 0) if (rank == 0 and headline) else None
     pre_steps, t_pre = 0, time.perf_counter()
     while time.perf_counter() - t_pre < sustain_s:
         for _ in range(max(1, steps // 4)):
@@ -436,7 +438,6 @@ def measure_in_hbm(name, args, dev, rank, world, dist, steps, warmup, sustain_s,
         pre_steps += max(1, steps // 4)
     pre_s = time.perf_counter() - t_pre
     barrier()
-    sampler = ClockSampler(dev.index or 0) if (rank == 0 and headline) else None
     e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
     l0 = ctx.launch_count
     e0.record()
@@ -504,8 +505,11 @@ def measure_in_hbm(name, args, dev, rank, world, dist, steps, warmup, sustain_s,
     tot_k = sum(ms for ms, _ in prof.values()) or 1.0
     # a launch that returns at once (an enqueued fallback whose turn did not come: DESIGN.md sec. 4) has read nothing:
     # it gets no bandwidth figure (anything "faster" than twice the read probe cannot have streamed the cube)
+    # algorithmic bytes per launch: 4 B per voxel for a kernel that reads the cube once, 8 for the one cooperative
+    # launch that reads it twice (stats_small)
+    reads = lambda k: 2.0 if k == "stats_small" else 1.0   # noqa: E731
     kernels = {k: {"launches": c, "avg_ms": ms / c, "share": ms / tot_k,
-                   "achieved_gbs": (ALGO_BYTES_PER_VOXEL * n / (ms / c * 1e-3) / 1e9)
+                   "achieved_gbs": (reads(k) * ALGO_BYTES_PER_VOXEL * n / (ms / c * 1e-3) / 1e9)
                    if k in STREAMS_CUBE and ms / c > 0.5 * probe_ms else None}
                for k, (ms, c) in prof.items() if c}
     dom = max(kernels, key=lambda k: kernels[k]["share"])
@@ -514,7 +518,7 @@ def measure_in_hbm(name, args, dev, rank, world, dist, steps, warmup, sustain_s,
     roofline = {"bound": "hbm", "kernel": dom, "achieved": achieved, "peak": peak, "unit": "GB/s",
                 "frac": achieved / peak if achieved else None, "traffic": traffic,
                 "traffic_source": traffic_src, "peak_source": peak_src,
-                "algorithmic_bytes_per_launch": ALGO_BYTES_PER_VOXEL * n,
+                "algorithmic_bytes_per_launch": reads(dom) * ALGO_BYTES_PER_VOXEL * n,
                 "read_probe_gbs": read_peak, "frac_of_read_probe": achieved / read_peak if achieved else None,
                 "per_kernel": kernels}
 
@@ -679,12 +683,12 @@ def run_sharded(args, name):
 
     for _ in range(max(args.warmup, 3)):
         step()
+    sampler = ClockSampler(local_rank) if rank == 0 else None
     t_pre = time.perf_counter()
     while time.perf_counter() - t_pre < 1.0:
         step()
     dist.barrier()
     torch.cuda.synchronize()
-    sampler = ClockSampler(local_rank) if rank == 0 else None
     e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
     l0 = ctx.launch_count
     e0.record()
