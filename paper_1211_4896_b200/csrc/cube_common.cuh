@@ -93,7 +93,7 @@ __device__ __forceinline__ void stream_cube(const float* __restrict__ d, uint64_
     // Full tiles: a 32-bit tile counter (n <= 2^37 voxels: fewer than 2^23 tiles) and one running pointer, so that
     // the loop carries three registers of state and nothing is recomputed per tile (with the 64-bit tile index and
     // the in-loop "whole tile?" test ptxas rematerialised head / nvec / ntiles every iteration under the 64-register
-    // cap of the 1024-thread kernels: ~85 of ~510 instructions per warp tile, profiles/r2_*).
+    // cap of the 1024-thread kernels: ~85 of ~510 instructions per warp tile, profiles/r2_c3.md).
     const uint32_t nfull = (uint32_t)(nvec / TILE);
     const float4* __restrict__ q = v + (uint64_t)blockIdx.x * TILE + threadIdx.x;
     const uint64_t stride = (uint64_t)gridDim.x * TILE;

@@ -6,7 +6,7 @@
 // bits - rawbase, cube_select.cuh).  Before, every lane then revisited its own flagged rows one after the other
 // (re-loaded through L2), so a warp ran that code as often as its busiest lane had flagged rows, with most lanes idle:
 // on config 4 (the bucket holds 2.2 % of the voxels, 8.5 % of the rows) a third of pass B's instructions were issued
-// with 11 of 32 lanes active and the pass ran at 0.58 of the HBM rate (profiles/r2_*).  Now a lane PUSHES its flagged
+// with 11 of 32 lanes active and the pass ran at 0.58 of the HBM rate (profiles/r2_c3.md).  Now a lane PUSHES its flagged
 // rows onto a per-warp queue in shared memory, two at a time (re-loaded through L2, both loads in flight together:
 // keeping the 32 data registers alive across the cold code made ptxas spill in the hot loop), and the warp takes them
 // off 32 at a time -- one row per lane, every lane busy: the work per flagged row no longer depends on how the rows

@@ -19,7 +19,7 @@
 // The scan costs 8 LDS.128 + ~25 ALU instructions per thread per 48 voxels (~0.7 per voxel); the loads of the next
 // tile are issued before the current one is binned, so the barrier does not drain the memory pipeline.
 // (v1 detected wraps from the value returned by atomicAdd: ~20 instructions per voxel and same-address
-// serialisation; 2.7 TB/s on config 4, 3.9 TB/s on config 3 -- profiles/r1_v4_c2.md.)
+// serialisation; 2.7 TB/s on config 4, 3.9 TB/s on config 3 -- round-1 ncu capture.)
 #pragma once
 #include "cube_kernels.cuh"
 

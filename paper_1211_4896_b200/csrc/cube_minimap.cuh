@@ -168,7 +168,7 @@ struct MapV4F : MomentsF<kMomPlain> {
     }
     // repair of a HOT group whose sum came out NaN: reload the lines (L2 hits), add the owned non-NaN voxels.
     // Static, arguments and result by value: the functor itself stays in registers (a member function taking
-    // `this` put it on the stack -- 116 M local-memory sectors per pass, profiles/r1_v8_c2.md).
+    // `this` put it on the stack -- 116 M local-memory sectors per pass in a round-1 ncu capture).
     struct GroupFix { double s, q; uint32_t n; };
     static __device__ __noinline__ GroupFix redo_group(MapLines at, double pivot_, uint32_t ownmask) {
         GroupFix f;

@@ -36,7 +36,7 @@ struct SelectState {
 // threshold plus one whole tile and can never overflow -- also on a constant cube, where every voxel is a
 // candidate.  (v2 reserved space by ballot + warp scan per tile: at the 0.3 % bucket density of config 2
 // ~95 % of the warp tiles took that path to place ~3 keys, 564 M instructions, 5.1 TB/s;
-// profiles/r1_v2_baseline.md.)
+// round-1 ncu capture.)
 constexpr uint32_t kStageThresh = 128;                                 // flush when more keys than this wait
 constexpr uint32_t kStageCap = kStageThresh + 32u * 4u * kUnroll;      // + one tile of a warp: 1152 keys
 constexpr int kStageBytes = (kThreads / 32) * (int)kStageCap * 4;      // 36 KiB per CTA
