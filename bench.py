@@ -474,6 +474,12 @@ def measure_in_hbm(name, args, dev, rank, world, dist, steps, warmup, sustain_s,
     op_s = 0.4 if headline else 0.25
     for nm, fn, bpv in op_list:
         ops[nm] = op_record(timed(fn, reps_for(fn, op_s)), n, bpv, peak)
+    if name == "c4" and not args.no_next:
+        # MAD on the adversarial config: 30 % of the voxels share one deviation, so the second selection's first-digit
+        # bucket is dense (PASS 1 counts in its hot loop, PASS 2 reads the cube a third time: 20 B per voxel moved)
+        out_w4 = torch.zeros(2, dtype=torch.float32, device=dev)
+        fn_mad = lambda: ctx.mad(cube_t, nx, ny, nz, median_out=out_w4[0:1], mad_out=out_w4[1:2], stream=stream)   # noqa: E731
+        ops["next_mad"] = op_record(timed(fn_mad, reps_for(fn_mad, 0.25)), n, 16.0, peak)
     if name == "c2" and not args.no_next:
         ops.update(next_rows(ctx, cube_t, (nx, ny, nz), lo, hi, out_m, out_f, dev, stream, timed, reps_for, peak))
     ops["stats_fused"] = {"ms": total_ms / steps, "voxels_per_s": total_units / (total_ms * 1e-3) / world,

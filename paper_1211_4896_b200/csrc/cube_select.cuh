@@ -28,7 +28,13 @@ struct SelectState {
     unsigned long long cand_cap;  // capacity of the candidate buffer, in keys
     uint32_t cand_done;         // 1: the last digit has been counted on the candidates (select_cand_kernel), so the
     uint32_t pad_;              //    per-brick PASS 2 launches of a brick-streamed / sharded run return at once
+    unsigned long long bucket_n;  // voxels in the bucket chosen by the last bucket location
 };
+// A first-digit bucket holding more than 1/8 of the voxels (tie-heavy data: 30 % of config 4's voxels are one value)
+// cannot be compacted into a candidate buffer of 1/16 of the cube and would keep PASS 1's cold path busy on nearly
+// every row: PASS 1 then counts the second digit of every voxel in its hot loop instead (as PASS 0 and PASS 2 do) and
+// PASS 2 reads the cube a third time.  Decided on the device from the counts.
+__device__ __forceinline__ bool select_dense(const SelectState* st) { return st->bucket_n * 8ull > st->count; }
 
 // PASS 1 compaction ("step 8"): every warp stages the keys of the prefix bucket in its own slice of shared
 // memory and moves them to the candidate buffer in coalesced runs, reserving the space with ONE global atomic
@@ -198,10 +204,32 @@ struct SelectF {
     }
 };
 
+// PASS 1 on a dense bucket: digit (key - base) >> 9 of every voxel, everything outside the bucket to the trash counter.
+template <bool NANCHK, bool DEV>
+struct SelectDense1F {
+    uint32_t base;
+    uint32_t* sbins;   // kBins1 + 1
+    float center;
+    __device__ __forceinline__ void operator()(float x) {
+        const float y = SelectF<1, NANCHK, DEV>::xf(x, center);
+        uint32_t idx = min((key_of(y) - base) >> kBits2, (uint32_t)kBins1);
+        if (NANCHK) idx = (y == y) ? idx : (uint32_t)kBins1;
+        atomicAdd(&sbins[idx], 1u);
+    }
+    CUBE_DEFAULT_BATCH()
+};
+
 template <int PASS, bool NANCHK, bool DEV>
 __device__ __forceinline__ void select_run(const float* __restrict__ d, uint64_t n, SelectState* __restrict__ st,
                                            uint32_t* sbins, uint32_t* stage, uint32_t* __restrict__ cand,
                                            float center) {
+    if (PASS == 1 && select_dense(st)) {   // uniform over the grid
+        SelectDense1F<NANCHK, DEV> g;
+        g.base = st->prefix << kShift0; g.sbins = sbins; g.center = center;
+        stream_cube<kThreads>(d, n, g);
+        if (blockIdx.x == 0 && threadIdx.x == 0) st->cand_n = st->cand_cap + 1ull;   // "did not fit": PASS 2 streams the cube
+        return;
+    }
     SelectF<PASS, NANCHK, DEV> f;
     f.base = (PASS == 0) ? 0u : (PASS == 1) ? (st->prefix << kShift0) : (st->prefix << kBits2);
     f.rawbase = (PASS == 1) ? (raw_of_digit(st->prefix) << kShift0) : 0u;
@@ -355,6 +383,7 @@ __device__ __forceinline__ void select_scan_body(SelectState* __restrict__ st, u
                 const uint32_t pre = (PASS == 0) ? b : ((pfx << BITS) | b);
                 st->prefix = pre;
                 st->k = kk - ex2;
+                st->bucket_n = x;
                 if (PASS == 2) {
                     const float r = __uint_as_float(bits_of_key(pre));
                     st->result = r;

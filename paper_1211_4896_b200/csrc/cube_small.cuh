@@ -98,7 +98,7 @@ __device__ __forceinline__ void small_locate0(SelectState* st, const unsigned lo
     const unsigned ball = __ballot_sync(0xffffffffu, ch >= 0);
     if (lane == 0) {
         st->count = total; st->invalid = total ? 0u : 1u; st->use_median = 1u; st->cand_n = 0; st->cand_cap = cand_cap;
-        st->cand_done = 0u; st->k = k; st->prefix = 0u; st->result = __int_as_float(0x7fc00000);
+        st->cand_done = 0u; st->k = k; st->prefix = 0u; st->result = __int_as_float(0x7fc00000); st->bucket_n = 0ull;
     }
     if (!ball) return;
     const int src = __ffs(ball) - 1;
@@ -114,7 +114,7 @@ __device__ __forceinline__ void small_locate0(SelectState* st, const unsigned lo
     }
     const unsigned long long ex2 = inc2 - x;
     __syncwarp();
-    if (x && ex2 <= kin && kin < inc2) { st->prefix = digit; st->k = kin - ex2; }   // exactly one lane
+    if (x && ex2 <= kin && kin < inc2) { st->prefix = digit; st->k = kin - ex2; st->bucket_n = x; }   // exactly one lane
 }
 
 #ifdef CUBE_SMALL_TIMING
@@ -293,7 +293,7 @@ stats_small_kernel(SmallArgs a) {
         SelectState* g = a.sel;          // the state a later CUBE_REUSE_COARSE selection or a reader of the context finds
         g->k = s_sel.k; g->count = s_sel.count; g->prefix = s_sel.prefix; g->invalid = s_sel.invalid;
         SMALL_T(8);
-        g->use_median = 1u; g->result = s_sel.result; g->cand_cap = a.cand ? a.cand_cap : 0; g->cand_done = fits ? 1u : 0u;
+        g->use_median = 1u; g->result = s_sel.result; g->bucket_n = s_sel.bucket_n; g->cand_cap = a.cand ? a.cand_cap : 0; g->cand_done = fits ? 1u : 0u;
     }
 }
 
