@@ -603,8 +603,7 @@ int cube_stats(cube_ctx* c, const float* d, int64_t nx, int64_t ny, int64_t nz, 
             a.d = d; a.n = n; a.nbins = nbins; a.lo = lo; a.hi = hi; a.scale = scale; a.minmax = minmax ? 1 : 0;
             a.flags = flags & CUBE_SAMPLE_STD;
             a.partials = c->partials; a.acc = c->acc; a.nvox_acc = c->nvox_acc; a.mom_out = c->mom_out; a.out_user = mom_direct;
-            std::swap(c->coarse, c->coarse_next);     // the zeroed array becomes the current one
-            a.coarse = c->coarse; a.coarse_next = c->coarse_next; a.chunk_tot = c->chunk_tot;
+            a.coarse = c->coarse_next; a.coarse_next = c->coarse; a.chunk_tot = c->chunk_tot;   // the zeroed array becomes the current one
             a.gdigits = c->gdigits; a.gout = c->gout;
             a.sel = c->sel; a.cand = c->cand; a.cand_cap = c->cand ? c->cand_cap : 0; a.result_out = med_direct;
             a.bar = c->bar; a.bar_base = c->bar_base; a.tstamp = c->small_tstamp;
@@ -617,6 +616,7 @@ int cube_stats(cube_ctx* c, const float* d, int64_t nx, int64_t ny, int64_t nz, 
                 CUBE_CUDA(c, cudaLaunchCooperativeKernel(reinterpret_cast<void*>(stats_small_kernel), dim3(grid), dim3(kThreads),
                                                          args, smem, s));
             }
+            std::swap(c->coarse, c->coarse_next);     // only once the launch is enqueued: coarse_next stays "all zero"
             c->bar_base += kSmallBarriers * grid;
             if (!med_direct) CUBE_CUDA(c, cudaMemcpyAsync(median, &c->sel->result, sizeof(float), cudaMemcpyDefault, s));
             if (moments && !mom_direct) CUBE_CUDA(c, cudaMemcpyAsync(moments, c->mom_out, sizeof(MomentsOut), cudaMemcpyDefault, s));

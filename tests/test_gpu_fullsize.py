@@ -232,6 +232,20 @@ def test_config2_full_size():
         torch.cuda.synchronize()
         gm, rmm = gmed.cpu().numpy().reshape(mz, my, mx), f_mapmed.result()
         assert ((gm.view(np.uint32) == rmm.view(np.uint32)) | (np.isnan(gm) & np.isnan(rmm))).all()
+        # NEXT-4 through the full cube: a small image (64 x 48 rays of ~1775 samples) and two profiles, bit for bit
+        view = cubegen.view_orbit(dims, 30.0, 20.0, 64, 48, step=1.0)
+        img = torch.zeros(64 * 48, dtype=torch.float32, device="cuda")
+        ctx.render_mip(t, *dims, view, img)
+        tab = np.linspace(0.0, 1.0, 64, dtype=np.float32)[:, None] * np.array([1.0, 0.5, 0.25, 0.05], dtype=np.float32)
+        rgba = torch.zeros(64 * 48 * 4, dtype=torch.float32, device="cuda")
+        ctx.render_tf(t, *dims, view, tab, 0.004, 0.1, rgba, opacity_cut=0.98)
+        prof = torch.zeros(view["nsteps"], dtype=torch.float32, device="cuda")
+        ctx.spectrum(t, *dims, view, 31, 25, prof)
+        torch.cuda.synchronize()
+        for got_a, ref_a in ((img.cpu().numpy().reshape(48, 64), oracle.render_mip(a, dims, view)),
+                             (rgba.cpu().numpy().reshape(48, 64, 4), oracle.render_tf(a, dims, view, tab, 0.004, 0.1, 0.98)),
+                             (prof.cpu().numpy(), oracle.spectrum(a, dims, view, 31, 25))):
+            assert ((got_a.view(np.uint32) == ref_a.view(np.uint32)) | (np.isnan(got_a) & np.isnan(ref_a))).all()
         pool.shutdown()
     finally:
         ctx.close()
