@@ -19,8 +19,8 @@ constexpr int kMedCtaThreads = 512;
 constexpr int kMedStageKeys = 56000;                 // most keys a CTA can stage (219 KiB: one CTA per SM; a 30^3 cell
                                                      // takes 105 KiB: two CTAs per SM)
 constexpr int kMedWarpKeys = 1024;                   // cells below this many voxels: one warp per cell
-constexpr int kMedCtaExtra = (256 + 40) * 4;         // histogram + reduction words behind the staged keys
-constexpr int kMedWarpSmemPerWarp = (kMedWarpKeys + 256 + 8) * 4;
+constexpr int kMedCtaExtra = (264 + 40) * 4;         // histogram + reduction words behind the staged keys
+constexpr int kMedWarpSmemPerWarp = (kMedWarpKeys + 264 + 8) * 4;
 
 template <int GROUP> __device__ __forceinline__ void med_sync() {
     if (GROUP == 32) __syncwarp(); else __syncthreads();
@@ -89,26 +89,39 @@ __device__ __forceinline__ float med_cell(const float* __restrict__ d, const Med
     constexpr int NW = GROUP / 32;
     // visit every voxel of the cell: a warp takes rows (a row is px contiguous voxels), eight rows at a time so that
     // eight loads per lane are in flight (one load at a time left the read of a 30^3 cell at the latency of 113
-    // dependent L2 / HBM round trips per warp); the (y, z) of a warp's row advances by additions, no division per row
+    // dependent L2 / HBM round trips per warp); the (y, z) of a warp's row advances by additions, no division per row,
+    // and a full batch of eight rows carries no per-row bounds test
+    const long long row_step = g.nx, plane_step = g.ny * g.nx;
     auto for_each_key = [&](auto&& fn) {
         int yy = wid % h, zz = wid / h;
         for (int r0 = wid; r0 < rows; r0 += NW * 8) {
             const float* p[8];
 #pragma unroll
             for (int u = 0; u < 8; ++u) {
-                p[u] = base + ((long long)zz * g.ny + yy) * g.nx;
+                p[u] = base + (long long)zz * plane_step + (long long)yy * row_step;
                 yy += NW;
                 while (yy >= h) { yy -= h; ++zz; }
             }
-            for (int xc = 0; xc < w; xc += 32) {
-                const int xx = xc + lane;
-                float v[8];
+            const bool full = r0 + 7 * NW < rows;            // warp-uniform
+            uint32_t idx0 = (uint32_t)r0 * (uint32_t)w + (uint32_t)lane;
+            for (int xc = 0; xc < w; xc += 32, idx0 += 32) {
+                if (xc + lane < w) {
+                    float v[8];
+                    if (full) {
 #pragma unroll
-                for (int u = 0; u < 8; ++u) v[u] = (r0 + u * NW < rows && xx < w) ? __ldg(p[u] + xx) : 0.0f;
+                        for (int u = 0; u < 8; ++u) v[u] = __ldg(p[u] + xc + lane);
 #pragma unroll
-                for (int u = 0; u < 8; ++u)
-                    if (r0 + u * NW < rows && xx < w)
-                        fn(v[u] == v[u] ? key_of(v[u]) : 0xFFFFFFFFu, (uint32_t)(r0 + u * NW) * (uint32_t)w + (uint32_t)xx);
+                        for (int u = 0; u < 8; ++u)
+                            fn(v[u] == v[u] ? key_of(v[u]) : 0xFFFFFFFFu, idx0 + (uint32_t)(u * NW) * (uint32_t)w);
+                    } else {
+#pragma unroll
+                        for (int u = 0; u < 8; ++u) v[u] = (r0 + u * NW < rows) ? __ldg(p[u] + xc + lane) : 0.0f;
+#pragma unroll
+                        for (int u = 0; u < 8; ++u)
+                            if (r0 + u * NW < rows)
+                                fn(v[u] == v[u] ? key_of(v[u]) : 0xFFFFFFFFu, idx0 + (uint32_t)(u * NW) * (uint32_t)w);
+                    }
+                }
             }
         }
     };
@@ -127,7 +140,17 @@ __device__ __forceinline__ float med_cell(const float* __restrict__ d, const Med
                 if ((key & hi_mask) == prefix) atomicAdd(&hist[(key >> shift) & 255u], 1u);
             });
         } else {
-            for (uint32_t i = tid; i < nvox; i += GROUP) {
+            // the staged keys, four per load (the stage is 16-byte aligned; nvox4 * 4 <= nvox)
+            const uint32_t nvox4 = nvox >> 2;
+            const uint4* __restrict__ k4 = reinterpret_cast<const uint4*>(keys);
+            for (uint32_t i = tid; i < nvox4; i += GROUP) {
+                const uint4 q = k4[i];
+                if ((q.x & hi_mask) == prefix) atomicAdd(&hist[(q.x >> shift) & 255u], 1u);
+                if ((q.y & hi_mask) == prefix) atomicAdd(&hist[(q.y >> shift) & 255u], 1u);
+                if ((q.z & hi_mask) == prefix) atomicAdd(&hist[(q.z >> shift) & 255u], 1u);
+                if ((q.w & hi_mask) == prefix) atomicAdd(&hist[(q.w >> shift) & 255u], 1u);
+            }
+            for (uint32_t i = (nvox4 << 2) + tid; i < nvox; i += GROUP) {
                 const uint32_t key = keys[i];
                 if ((key & hi_mask) == prefix) atomicAdd(&hist[(key >> shift) & 255u], 1u);
             }
@@ -153,7 +176,7 @@ minimap_median_cta_kernel(const float* __restrict__ d, MedGeom g, int stage_keys
     uint32_t* keys = med_smem;
     uint32_t* hist = med_smem + stage_keys;          // stage_keys = 0: the cell is re-read for every digit
     const bool staged = stage_keys > 0;
-    uint32_t* red = hist + 256;
+    uint32_t* red = hist + 264;
     const long long ncell = g.mx * g.my * g.mz;
     for (long long cell = blockIdx.x; cell < ncell; cell += gridDim.x) {
         const float r = staged ? med_cell<kMedCtaThreads, true>(d, g, cell, keys, hist, red, threadIdx.x)
@@ -170,7 +193,7 @@ minimap_median_warp_kernel(const float* __restrict__ d, MedGeom g, float* __rest
     const int wid = threadIdx.x >> 5, lane = threadIdx.x & 31;
     uint32_t* keys = med_smem + wid * (kMedWarpSmemPerWarp / 4);
     uint32_t* hist = keys + kMedWarpKeys;
-    uint32_t* red = hist + 256;
+    uint32_t* red = hist + 264;
     const long long ncell = g.mx * g.my * g.mz;
     const long long nwarps = (long long)gridDim.x * (kMedCtaThreads / 32);
     for (long long cell = (long long)blockIdx.x * (kMedCtaThreads / 32) + wid; cell < ncell; cell += nwarps) {

@@ -933,6 +933,17 @@ def test_single_launch_path_for_l2_resident_cubes(scratch):
                     else:
                         assert not b.any() and (o == np.uint64(2 ** 64 - 1)).all()
                 c.set_launch(0)
+                # device-resident outputs are written by the kernel itself (no copy is enqueued)
+                d_m = torch.zeros(40, dtype=torch.uint8, device="cuda")
+                d_b = torch.full((nb,), -1, dtype=torch.int64, device="cuda")
+                d_o = torch.full((2,), -1, dtype=torch.int64, device="cuda")
+                d_f = torch.zeros(1, dtype=torch.float32, device="cuda")
+                c.stats(t, a.size, 1, 1, nb, lo, hi, out=d_m, bins=d_b, outside=d_o, median=d_f)
+                torch.cuda.synchronize()
+                assert (d_b.cpu().numpy().astype(np.uint64) == gb).all() and (d_o.cpu().numpy().astype(np.uint64) == go).all()
+                assert same_float(d_f.cpu()[0].item(), gmed)
+                dm = cube.MomentsT.from_buffer_copy(d_m.cpu().numpy().tobytes()).as_dict()
+                assert dm["count"] == ref["count"] and same_float(dm["min"], ref["min"]) and same_float(dm["max"], ref["max"])
                 # the first-digit histogram is left in the context as by the general path
                 k = ref["count"] // 3
                 if ref["count"]:
