@@ -2,8 +2,9 @@
 // (cube_hist_big.cuh) + second select digit + candidate compaction in ONE read of the cube, so that cube_stats()
 // takes two reads for 65536 bins as well (configs 3 and 4 of BASELINE.json; steps 4-6 and 8 of SURVEY.md sec. 8(a)).
 //
-// One CTA of 1024 threads per SM.  Dynamic shared memory (201 KiB of the 227 KiB):
-//     [32768 + 1 window counters][1024 + 1 digit counters][32 warps x WarpGather (96-row queue + 160 staged keys)]
+// One CTA of 896 threads per SM (73 registers per thread: under the 64-register cap of 1024 threads ptxas rematerialised
+// the loop state every tile).  Dynamic shared memory (192 KiB of the 227 KiB):
+//     [32768 + 1 window counters][1024 + 1 digit counters][28 warps x WarpGather (96-row queue + 160 staged keys)]
 // The select side is cube_gather.cuh: flagged rows are pushed onto the warp's queue two rows per lane at a time and
 // taken off 32 at a time, so neither the queue nor the key stage has to hold a whole tile share.
 // It only runs when the sampled plan chose the window (BigHistPlan::use_window); otherwise it returns at once
