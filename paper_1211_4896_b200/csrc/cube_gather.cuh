@@ -74,8 +74,8 @@ static __device__ __noinline__ void gather_rows(WarpGather* w, const GatherShare
     }
     if (w->compacting) {             // warp-uniform
         uint32_t pos = nh ? atomicAdd(&w->nkeys, nh) : 0u;
-#pragma unroll
         CUBE_CHECK(pos + nh <= (uint32_t)kKeyCap);
+#pragma unroll
         for (int i = 0; i < 4; ++i)
             if (hit[i]) w->keys[pos++] = kk[i] + base;
         __syncwarp();
