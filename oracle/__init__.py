@@ -101,6 +101,9 @@ def lib():
         L.oracle_trilinear.argtypes = [fp, i64, i64, i64, fp, fp]
         L.oracle_spectrum.argtypes = [fp, i64, i64, i64, vwp, ctypes.c_int, ctypes.c_int, fp]
         L.oracle_render_mip.argtypes = [fp, i64, i64, i64, vwp, ctypes.c_float, fp]
+        L.oracle_minimap_lookup.argtypes = [mp] + [i64] * 6 + [fp, fp, fp]
+        L.oracle_render_sigma.argtypes = [fp, i64, i64, i64, vwp, mp, i64, i64, i64, ctypes.c_int, ctypes.c_float,
+                                          ctypes.c_float, fp, ctypes.c_float, fp]
         L.oracle_render_tf.argtypes = [fp, i64, i64, i64, vwp, ctypes.c_int, ctypes.c_float, ctypes.c_float, fp,
                                        ctypes.c_float, fp]
         _lib = L
@@ -304,4 +307,41 @@ def render_tf(a, dims, view, table, lo, hi, opacity_cut=2.0):
                                 t.ctypes.data_as(fp), float(np.float32(opacity_cut)), out.ctypes.data_as(fp))
     if rc != 0:
         raise ValueError("oracle_render_tf: invalid arguments")
+    return out.reshape(w.height, w.width, 4)
+
+
+_MAP_DT = np.dtype([("count", "<u8"), ("nan_count", "<u8"), ("min", "<f4"), ("max", "<f4"), ("mean", "<f8"), ("std", "<f8")])
+
+
+def _cells(cells):
+    """mini-map records (structured array as returned by ``minimap``) -> ctypes array of Moments."""
+    c = np.ascontiguousarray(cells, dtype=_MAP_DT).reshape(-1)
+    return (Moments * c.size).from_buffer_copy(c.tobytes())
+
+
+def minimap_lookup(cells, dims, part, point):
+    """(mean, std) of the mini-map ``cells`` (structured array [mz, my, mx]) interpolated at the data point (R34)."""
+    nx, ny, nz = dims
+    px, py, pz = part
+    pt = (ctypes.c_float * 3)(*[float(np.float32(c)) for c in point])
+    m, s = ctypes.c_float(), ctypes.c_float()
+    lib().oracle_minimap_lookup(_cells(cells), nx, ny, nz, px, py, pz, pt, ctypes.byref(m), ctypes.byref(s))
+    return np.float32(m.value), np.float32(s.value)
+
+
+def render_sigma(a, dims, view, cells, part, table, zlo, zhi, opacity_cut=2.0):
+    """Sigma-clipping transfer function: levels of z = (sample - local mean) / local std over
+    [zlo, zhi], local statistics interpolated in the mini-map.  -> float32 [height, width, 4]."""
+    a, p = _arr(a)
+    nx, ny, nz = dims
+    px, py, pz = part
+    w = _view(view)
+    t = np.ascontiguousarray(table, dtype=np.float32).reshape(-1, 4)
+    out = np.zeros(w.width * w.height * 4, dtype=np.float32)
+    fp = ctypes.POINTER(ctypes.c_float)
+    rc = lib().oracle_render_sigma(p, nx, ny, nz, ctypes.byref(w), _cells(cells), px, py, pz, t.shape[0],
+                                   float(np.float32(zlo)), float(np.float32(zhi)), t.ctypes.data_as(fp),
+                                   float(np.float32(opacity_cut)), out.ctypes.data_as(fp))
+    if rc != 0:
+        raise ValueError("oracle_render_sigma: invalid arguments")
     return out.reshape(w.height, w.width, 4)

@@ -37,7 +37,8 @@
 //   ray casting: trilinear sample, maximum intensity
 //                       projection, generic transfer function with front-to-back compositing, 3-D spectrum
 //                       profile -- the march restated sample by sample at the end of this file
-//                       (readings R27-R32 of DESIGN.md; pins in tests/test_oracle_render_pins.py).
+//                       (readings R27-R32, R34 of DESIGN.md; pins in tests/test_oracle_render_pins.py); the
+//                       sigma-clipping transfer function with its second lookup in the mini-map.
 //
 // Build: g++ -O2 -std=c++17 -ffp-contract=off -fno-fast-math -fPIC -shared (oracle/build.py).
 
@@ -585,6 +586,102 @@ int oracle_render_tf(const float* d, int64_t nx, int64_t ny, int64_t nz, const o
             }
             float* px = rgba + 4 * ((size_t)v * vw->width + u);
             px[0] = C[0]; px[1] = C[1]; px[2] = C[2]; px[3] = A;
+        }
+    return 0;
+}
+
+
+// Sigma-clipping transfer function (Fig. 7, Fig. 9): "For each sampled data point over the traced rays,
+// two trilinear interpolation operations are required.  The first one is performed to get the actual data value at
+// this point using the original data grid.  The second is performed to get the data properties at this point using
+// the mini-map.  The point's data value is then scaled using its region's data properties to generate the look-up
+// value used to calculate the colour and the opacity".  Reading R34 (the paper gives no formula):
+//   * the mini-map is the array of cell records oracle_minimap produces; cell (cx, cy, cz) sits at the centre of its
+//     nominal px x py x pz block: data coordinate  cx * px + (px - 1) / 2  along x, likewise y, z;
+//   * map coordinate of a data point:  q_c = (p_c - (px_c - 1) / 2) / px_c  (float32: one subtraction, one IEEE
+//     division), clamped to [0, m_c - 1]; local mean and std = trilinear interpolation (the rule of
+//     oracle_trilinear: floor, a neighbour of weight zero does not take part, a + f * (b - a), x then y then z) of the
+//     cells' mean and std, each rounded to float32 first; a cell without voxels (NaN record) makes them NaN;
+//   * look-up value  z = (s - mean) / std  (float32, IEEE division); the sample is skipped unless std > 0 and z is
+//     not NaN; levels over [zlo, zhi] and compositing exactly as in oracle_render_tf (R30, R31) with z in place of s:
+//     zlo is the clipping threshold in units of the local sigma ("2 sigma, 3 sigma, 4 sigma and 7 sigma").
+static inline float oracle_lerp(float a, float b, float f) {
+    volatile float diff = b - a;
+    volatile float prod = f * diff;
+    return a + prod;
+}
+
+// mean and std of the mini-map at the data point p (see above).  Exposed for the pins.
+int oracle_minimap_lookup(const oracle_moments_t* cells, int64_t nx, int64_t ny, int64_t nz, int64_t px, int64_t py,
+                          int64_t pz, const float p[3], float* mean_out, float* std_out) {
+    const int64_t n[3] = {nx, ny, nz}, part[3] = {px, py, pz};
+    int64_t m[3], i0[3], i1[3];
+    float f[3];
+    for (int c = 0; c < 3; ++c) {
+        m[c] = (n[c] + part[c] - 1) / part[c];
+        volatile float off = (float)(part[c] - 1) / 2.0f;
+        volatile float rel = p[c] - off;
+        float q = rel / (float)part[c];
+        if (!(q >= 0.0f)) q = 0.0f;                         // clamp (also a NaN coordinate)
+        if (q > (float)(m[c] - 1)) q = (float)(m[c] - 1);
+        const float fl = floorf(q);
+        i0[c] = (int64_t)fl;
+        f[c] = q - fl;
+        i1[c] = i0[c] + (f[c] > 0.0f ? 1 : 0);
+    }
+    float out[2];
+    for (int which = 0; which < 2; ++which) {
+        auto at = [&](int64_t x, int64_t y, int64_t z) {
+            const oracle_moments_t& r = cells[(z * m[1] + y) * m[0] + x];
+            return (float)(which == 0 ? r.mean : r.std);
+        };
+        const float c00 = oracle_lerp(at(i0[0], i0[1], i0[2]), at(i1[0], i0[1], i0[2]), f[0]);
+        const float c10 = oracle_lerp(at(i0[0], i1[1], i0[2]), at(i1[0], i1[1], i0[2]), f[0]);
+        const float c01 = oracle_lerp(at(i0[0], i0[1], i1[2]), at(i1[0], i0[1], i1[2]), f[0]);
+        const float c11 = oracle_lerp(at(i0[0], i1[1], i1[2]), at(i1[0], i1[1], i1[2]), f[0]);
+        out[which] = oracle_lerp(oracle_lerp(c00, c10, f[1]), oracle_lerp(c01, c11, f[1]), f[2]);
+    }
+    *mean_out = out[0];
+    *std_out = out[1];
+    return 0;
+}
+
+int oracle_render_sigma(const float* d, int64_t nx, int64_t ny, int64_t nz, const oracle_view_t* vw,
+                        const oracle_moments_t* cells, int64_t px, int64_t py, int64_t pz, int nlevels, float zlo,
+                        float zhi, const float* table, float opacity_cut, float* rgba) {
+    if (nlevels < 1 || !(zlo <= zhi) || px < 1 || py < 1 || pz < 1) return 1;
+    volatile float width = zhi - zlo;
+    volatile float scale_v = (zhi == zlo) ? 0.0f : (float)nlevels / width;
+    const float scale = scale_v;
+    for (int v = 0; v < vw->height; ++v)
+        for (int u = 0; u < vw->width; ++u) {
+            float o[3], p[3], C[3] = {0.0f, 0.0f, 0.0f}, A = 0.0f;
+            oracle_ray_origin(vw, u, v, o);
+            for (int i = 0; i < vw->nsteps; ++i) {
+                oracle_ray_point(vw, o, i, p);
+                float s, mean, sd;
+                if (!oracle_trilinear(d, nx, ny, nz, p, &s)) continue;
+                oracle_minimap_lookup(cells, nx, ny, nz, px, py, pz, p, &mean, &sd);
+                if (!(sd > 0.0f)) continue;
+                volatile float num = s - mean;
+                const float z = num / sd;
+                if (!(z >= zlo)) continue;                       // below the clipping threshold, or NULL
+                volatile float t = z - zlo;
+                volatile float q = t * scale;
+                float fl = floorf(q);
+                int L = (fl >= (float)(nlevels - 1)) ? nlevels - 1 : (int)fl;
+                const float* e = table + 4 * (size_t)L;
+                volatile float rem = 1.0f - A;
+                volatile float w = rem * e[3];
+                for (int c = 0; c < 3; ++c) {
+                    volatile float wc = w * e[c];
+                    C[c] = C[c] + wc;
+                }
+                A = A + w;
+                if (A >= opacity_cut) break;
+            }
+            float* pxl = rgba + 4 * ((size_t)v * vw->width + u);
+            pxl[0] = C[0]; pxl[1] = C[1]; pxl[2] = C[2]; pxl[3] = A;
         }
     return 0;
 }

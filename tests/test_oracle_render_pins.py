@@ -192,3 +192,101 @@ def test_minimap_median_is_the_block_sort():
                         assert math.isnan(got[cz, cy, cx])
                     else:
                         assert float(got[cz, cy, cx]) == float(ok[(ok.size - 1) // 2])
+
+
+def map_cells(shape, mean, std):
+    """a mini-map (structured array [mz, my, mx]) with the given mean / std arrays"""
+    dt = np.dtype([("count", "<u8"), ("nan_count", "<u8"), ("min", "<f4"), ("max", "<f4"), ("mean", "<f8"),
+                   ("std", "<f8")])
+    c = np.zeros(shape, dtype=dt)
+    c["count"] = 1
+    c["mean"] = mean
+    c["std"] = std
+    return c
+
+
+def test_minimap_lookup_centres_linear_maps_and_clamping():
+    # cells of 4 x 2 x 8 voxels on a 20 x 6 x 16 cube -> a 5 x 3 x 2 map; cell (cx, cy, cz) sits at data coordinate
+    # (4 cx + 1.5, 2 cy + 0.5, 8 cz + 3.5)
+    dims, part = (20, 6, 16), (4, 2, 8)
+    mz, my, mx = 2, 3, 5
+    cz, cy, cx = np.meshgrid(np.arange(mz), np.arange(my), np.arange(mx), indexing="ij")
+    mean = 2.0 * cx + 8.0 * cy + 32.0 * cz + 1.0          # linear in the map index: trilinear reproduces it exactly
+    std = 0.5 * cx + 0.25 * cy + 4.0 * cz + 1.0
+    cells = map_cells((mz, my, mx), mean, std)
+    # at the cell centres: the cell's own values
+    for (z, y, x) in [(0, 0, 0), (1, 2, 4), (0, 1, 3), (1, 0, 2)]:
+        p = (4 * x + 1.5, 2 * y + 0.5, 8 * z + 3.5)
+        m, s = oracle.minimap_lookup(cells, dims, part, p)
+        assert float(m) == mean[z, y, x] and float(s) == std[z, y, x]
+    # between centres, on a dyadic grid: the linear function of q = (p - (part - 1) / 2) / part
+    r = np.random.default_rng(3)
+    for _ in range(200):
+        q = np.array([r.integers(0, 8 * (mx - 1) + 1) / 8.0, r.integers(0, 8 * (my - 1) + 1) / 8.0,
+                      r.integers(0, 8 * (mz - 1) + 1) / 8.0])
+        p = q * np.array(part) + (np.array(part) - 1) / 2.0
+        m, s = oracle.minimap_lookup(cells, dims, part, p)
+        assert float(m) == 2.0 * q[0] + 8.0 * q[1] + 32.0 * q[2] + 1.0
+        assert float(s) == 0.5 * q[0] + 0.25 * q[1] + 4.0 * q[2] + 1.0
+    # outside the centres' hull the map is clamped: the cube's corner voxels see the corner cells
+    m, s = oracle.minimap_lookup(cells, dims, part, (0.0, 0.0, 0.0))
+    assert float(m) == mean[0, 0, 0] and float(s) == std[0, 0, 0]
+    m, s = oracle.minimap_lookup(cells, dims, part, (19.0, 5.0, 15.0))
+    assert float(m) == mean[1, 2, 4] and float(s) == std[1, 2, 4]
+    m, s = oracle.minimap_lookup(cells, dims, part, (19.0, 0.0, 3.5))
+    assert float(m) == mean[0, 0, 4]
+    # an empty cell (NaN record) poisons what touches it, and only that: weight-zero neighbours do not take part
+    mean2 = mean.copy()
+    mean2[0, 1, 2] = np.nan
+    cells2 = map_cells((mz, my, mx), mean2, std)
+    m, _ = oracle.minimap_lookup(cells2, dims, part, (4 * 2 + 1.5 - 1.0, 2 * 1 + 0.5, 3.5))    # between cx = 1 and 2
+    assert math.isnan(float(m))
+    m, _ = oracle.minimap_lookup(cells2, dims, part, (4 * 1 + 1.5, 2 * 1 + 0.5, 3.5))          # exactly on cell cx = 1
+    assert float(m) == mean[0, 1, 1]
+    # a ragged map (21 voxels in cells of 4 -> 6 cells): the last centre is nominal, x = 21.5, beyond the cube
+    cells3 = map_cells((1, 1, 6), np.arange(6.0).reshape(1, 1, 6), np.ones((1, 1, 6)))
+    m, _ = oracle.minimap_lookup(cells3, (21, 1, 1), (4, 1, 1), (20.0, 0.0, 0.0))
+    assert float(m) == (20.0 - 1.5) / 4.0
+
+
+def test_sigma_clipping_transfer_function_closed_forms():
+    dims, part = (4, 4, 12), (2, 2, 4)
+    view = cubegen.view_axis(dims, 2)
+    a = np.full(4 * 4 * 12, 3.0, dtype=np.float32)
+    one = np.array([[0.25, 0.5, 1.0, 0.5]], dtype=np.float32)
+    # uniform map, mean 1, std 0.5: every sample has z = (3 - 1) / 0.5 = 4 -> inside [3, 5]: A = 1 - 2^-12
+    cells = map_cells((3, 2, 2), 1.0, 0.5)
+    img = oracle.render_sigma(a, dims, view, cells, part, one, 3.0, 5.0)
+    acc = 1.0 - 2.0 ** -12
+    assert np.all(img[..., 3] == np.float32(acc)) and np.all(img[..., 0] == np.float32(0.25 * acc))
+    # threshold above z: everything is clipped
+    img = oracle.render_sigma(a, dims, view, cells, part, one, 4.5, 5.0)
+    assert np.all(img == 0)
+    # std = 0 or NaN cells: the samples are skipped
+    for bad in (0.0, np.nan):
+        img = oracle.render_sigma(a, dims, view, map_cells((3, 2, 2), 1.0, bad), part, one, 3.0, 5.0)
+        assert np.all(img == 0)
+    # the LOCAL statistics decide: mean grows along z (cells at z = 1.5, 5.5, 9.5 with mean 0, 2, 4 -> mean(z) =
+    # (z - 1.5) / 2 clamped to [0, 4]), std 1, data 3: z-score = 3 - mean(z); threshold 1.5 -> the samples with
+    # mean(z) <= 1.5, i.e. z <= 4.5: slices 0 .. 4 pass, five samples: A = 1 - 2^-5
+    mean = np.zeros((3, 2, 2))
+    mean[1] = 2.0
+    mean[2] = 4.0
+    img = oracle.render_sigma(a, dims, view, map_cells((3, 2, 2), mean, 1.0), part, one, 1.5, 10.0)
+    assert np.all(img[..., 3] == np.float32(1.0 - 2.0 ** -5))
+    # level lookup on z: 4 levels over [0, 4]; data 3, std 1, uniform mean m -> level floor(3 - m)
+    table = np.array([[1, 0, 0, 1.0], [0, 1, 0, 1.0], [0, 0, 1, 1.0], [1, 1, 1, 1.0]], dtype=np.float32)
+    for m, colour in [(2.5, (1, 0, 0, 1)), (1.5, (0, 1, 0, 1)), (0.5, (0, 0, 1, 1)), (-0.5, (1, 1, 1, 1)),
+                      (-7.0, (1, 1, 1, 1))]:
+        img = oracle.render_sigma(a, dims, view, map_cells((3, 2, 2), m, 1.0), part, table, 0.0, 4.0)
+        assert np.all(img == np.array(colour, dtype=np.float32)), m
+    # with mean 0 and std 1 everywhere it is oracle.render_tf on the data values (same bins, same compositing)
+    r = np.random.default_rng(9)
+    b = r.standard_normal(4 * 4 * 12).astype(np.float32)
+    half = np.array([[1, 0, 0, 0.5], [0, 1, 0, 0.25], [0, 0, 1, 0.5], [0.5, 0.5, 0.5, 0.125]], dtype=np.float32)
+    rot = cubegen.view_orbit(dims, 30.0, 20.0, 24, 24, 0.5)
+    for v in (view, rot):
+        assert np.array_equal(oracle.render_sigma(b, dims, v, map_cells((3, 2, 2), 0.0, 1.0), part, half, -1.0, 2.0),
+                              oracle.render_tf(b, dims, v, half, -1.0, 2.0))
+    with pytest.raises(ValueError):
+        oracle.render_sigma(a, dims, view, cells, part, one, 1.0, 0.0)
