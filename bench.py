@@ -642,7 +642,9 @@ def next_rows(ctx, cube_t, dims, lo, hi, out_m, out_f, dev, stream, timed, reps_
     axis_view = cubegen.view_axis(dims, 2)
     for nm, fn, vw in [("next4_mip_1024x1024_yaw30_pitch20", lambda: ctx.render_mip(cube_t, nx, ny, nz, view, img, stream=stream), view),
                        ("next4_mip_along_z", lambda: ctx.render_mip(cube_t, nx, ny, nz, axis_view, img[:nx * ny], stream=stream), axis_view),
-                       ("next4_transfer_function_256_levels", lambda: ctx.render_tf(cube_t, nx, ny, nz, view, tab_d, 0.004, 0.1, rgba, opacity_cut=0.98, stream=stream), view)]:
+                       ("next4_transfer_function_256_levels", lambda: ctx.render_tf(cube_t, nx, ny, nz, view, tab_d, 0.004, 0.1, rgba, opacity_cut=0.98, stream=stream), view),
+                       # the sigma-clipping transfer function on the 30^3 mini-map computed above (3 sigma)
+                       ("paper_sigma_clipping_tf_3sigma_256_levels", lambda: ctx.render_sigma(cube_t, nx, ny, nz, view, out_cells, part[0], part[1], part[2], tab_d, 3.0, 12.0, rgba, opacity_cut=0.98, stream=stream), view)]:
         ms = timed(fn, reps_for(fn, 0.25, lo_reps=3))
         rays = vw["width"] * vw["height"]
         ops[nm] = {"ms": ms, "frames_per_s": 1e3 / ms, "rays": rays, "samples_per_ray": vw["nsteps"],

@@ -317,6 +317,20 @@ int cube_render_tf(cube_ctx* ctx, const float* d, int64_t nx, int64_t ny, int64_
                    int nlevels, float lo, float hi, const float* table, float opacity_cut, float* rgba,
                    cudaStream_t stream);
 
+/* Sigma-clipping transfer function (Fig. 7, Fig. 9; R34): cube_render_tf applied, sample
+ * by sample, to   z = (s - mean(p)) / std(p)   where mean(p), std(p) are the LOCAL statistics at the sample point p,
+ * trilinearly interpolated (the rule of the data lookup, float32) in the statistical mini-map `cells` that
+ * cube_minimap(ctx, d, nx, ny, nz, px, py, pz, ...) wrote: cell (cx,cy,cz) sits at the centre of its nominal block,
+ * data coordinate (cx*px + (px-1)/2, ...); map coordinate q = (p - (px-1)/2) / px clamped to [0, mx-1], likewise y, z.
+ * "Two trilinear interpolation operations" per sample.  Levels partition [zlo, zhi] (zlo = the
+ * clipping threshold in local sigmas, "2, 3, 4 and 7 sigma"); z < zlo, NULL samples and samples where
+ * the interpolated std is not > 0 (or the map is NULL: an empty cell takes part) are skipped; compositing, table,
+ * opacity_cut and rgba as cube_render_tf.  `cells`: memory the DEVICE can read (device or pinned host), mx*my*mz
+ * records; read only. */
+int cube_render_sigma(cube_ctx* ctx, const float* d, int64_t nx, int64_t ny, int64_t nz, const cube_view_t* view,
+                      const cube_moments_t* cells, int64_t px, int64_t py, int64_t pz, int nlevels, float zlo,
+                      float zhi, const float* table, float opacity_cut, float* rgba, cudaStream_t stream);
+
 /* 3-D spectrum tool (Fig. 6): out[i] = sample i of the ray of pixel (u,v) (any integers: the
  * pixel need not lie inside the image), NaN where the sample is outside the cube or NULL; nsteps floats,
  * device-writable memory. */

@@ -35,7 +35,8 @@ SYMBOLS = ["cube_create", "cube_destroy", "cube_moments", "cube_histogram", "cub
            "cube_profile_enable", "cube_profile_reset", "cube_profile_read",
            "cube_mad", "cube_clipped_moments", "cube_sigma_clip", "cube_minimap_dims", "cube_minimap",
            "cube_shard_buffers", "cube_shard_merge_records", "cube_shard_advance", "cube_median_torben",
-           "cube_view_orbit", "cube_render_mip", "cube_render_tf", "cube_spectrum", "cube_minimap_median"]
+           "cube_view_orbit", "cube_render_mip", "cube_render_tf", "cube_render_sigma", "cube_spectrum",
+           "cube_minimap_median"]
 SHARD_RECORD_BYTES, SHARD_DIGITS = 40, 8192
 KNOB_CTAS_PER_SM, KNOB_BIGHIST, KNOB_MINIMAP, KNOB_SMALL = 0, 1, 2, 3
 KIND_NAMES = ["moments", "moments_coarse", "histogram", "select_pass0", "select_pass1", "select_pass2",
@@ -149,6 +150,7 @@ def load():
     L.cube_view_orbit.argtypes = [i64, i64, i64, f64, f64, ci, ci, f64, vwp]
     L.cube_render_mip.argtypes = [vp, vp, i64, i64, i64, vwp, f32, vp, vp]
     L.cube_render_tf.argtypes = [vp, vp, i64, i64, i64, vwp, ci, f32, f32, vp, f32, vp, vp]
+    L.cube_render_sigma.argtypes = [vp, vp, i64, i64, i64, vwp, vp, i64, i64, i64, ci, f32, f32, vp, f32, vp, vp]
     L.cube_spectrum.argtypes = [vp, vp, i64, i64, i64, vwp, ci, ci, vp, vp]
     L.cube_shard_buffers.argtypes = [vp, ctypes.POINTER(ShardBuffersT)]
     L.cube_shard_merge_records.argtypes = [vp, vp, ci, cu, vp]
@@ -357,6 +359,18 @@ class Context:
             nlevels = table.numel() // 4
         self._check(self._L.cube_render_tf(self._h, _ptr(d), nx, ny, nz, ctypes.byref(w), nlevels, lo, hi, _ptr(table),
                                            opacity_cut, _ptr(rgba), stream))
+
+    def render_sigma(self, d, nx, ny, nz, view, cells, px, py, pz, table, zlo, zhi, rgba, opacity_cut=2.0, stream=0):
+        """cube_render_sigma: ``cells`` = the device (or pinned) buffer cube_minimap filled for partitions px, py, pz;
+        levels of (sample - local mean) / local std over [zlo, zhi]; the rest as render_tf."""
+        w = ViewT.from_dict(view)
+        if isinstance(table, np.ndarray):
+            table = np.ascontiguousarray(table, dtype=np.float32)
+            nlevels = table.size // 4
+        else:
+            nlevels = table.numel() // 4
+        self._check(self._L.cube_render_sigma(self._h, _ptr(d), nx, ny, nz, ctypes.byref(w), _ptr(cells), px, py, pz,
+                                              nlevels, zlo, zhi, _ptr(table), opacity_cut, _ptr(rgba), stream))
 
     def spectrum(self, d, nx, ny, nz, view, u, v, out, stream=0):
         """cube_spectrum: ``out`` = device (or pinned) buffer of nsteps floats."""

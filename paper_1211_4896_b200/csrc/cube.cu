@@ -889,13 +889,31 @@ int cube_render_mip(cube_ctx* c, const float* d, int64_t nx, int64_t ny, int64_t
     return CUBE_OK;
 }
 
-int cube_render_tf(cube_ctx* c, const float* d, int64_t nx, int64_t ny, int64_t nz, const cube_view_t* view,
-                   int nlevels, float lo, float hi, const float* table, float opacity_cut, float* rgba, cudaStream_t s) {
+static int render_tf_common(cube_ctx* c, const float* d, int64_t nx, int64_t ny, int64_t nz, const cube_view_t* view,
+                            int nlevels, float lo, float hi, const float* table, float opacity_cut,
+                            const cube_moments_t* cells, int64_t px, int64_t py, int64_t pz, float* rgba, cudaStream_t s) {
     RenderGeom g; RenderView vw;
     if (!render_args(c, d, nx, ny, nz, view, rgba, &g, &vw) || !table || nlevels < 1 || nlevels > 4096) return CUBE_EINVAL;
     if (opacity_cut != opacity_cut || ((uintptr_t)rgba & 15u)) return CUBE_EINVAL;
     float scale;
     if (!hist_scale(nlevels, lo, hi, &scale)) return CUBE_EINVAL;     // the histogram's scale (R10, R13, R19)
+    MapLookupGeom mg = {};
+    const double* dev_cells = nullptr;
+    if (cells) {
+        if (px < 1 || py < 1 || pz < 1) return CUBE_EINVAL;
+        static_assert(sizeof(cube_moments_t) == 5 * sizeof(double), "record layout");
+        dev_cells = static_cast<const double*>(device_reachable(c, const_cast<cube_moments_t*>(cells)));
+        if (!dev_cells || ((uintptr_t)dev_cells & 7u)) return CUBE_EINVAL;
+        const int64_t part[3] = {px, py, pz}, n[3] = {nx, ny, nz};
+        long long m[3];
+        for (int k = 0; k < 3; ++k) {
+            m[k] = (n[k] + part[k] - 1) / part[k];
+            mg.part[k] = (float)part[k];
+            mg.off[k] = (float)(part[k] - 1) / 2.0f;
+            mg.top[k] = (float)(m[k] - 1);
+        }
+        mg.mx = m[0]; mg.my = m[1]; mg.mz = m[2];
+    }
     const float4* dev_table = static_cast<const float4*>(device_reachable(c, const_cast<float*>(table)));
     if (!dev_table || ((uintptr_t)dev_table & 15u)) {
         CUBE_CUDA(c, cudaMemcpyAsync(c->tf_table, table, (size_t)nlevels * sizeof(float4), cudaMemcpyDefault, s));
@@ -905,11 +923,27 @@ int cube_render_tf(cube_ctx* c, const float* d, int64_t nx, int64_t ny, int64_t 
         ProfScope prof(c, CUBE_K_RENDER, s);
         const dim3 block(kRenderTileU, kRenderTileV);
         const dim3 grid((vw.width + kRenderTileU - 1) / kRenderTileU, (vw.height + kRenderTileV - 1) / kRenderTileV);
-        render_tf_kernel<<<grid, block, 0, s>>>(d, g, vw, nlevels, lo, scale, dev_table, opacity_cut,
-                                                reinterpret_cast<float4*>(rgba));
+        if (dev_cells)
+            render_tf_kernel<true><<<grid, block, 0, s>>>(d, g, vw, nlevels, lo, scale, dev_table, opacity_cut, dev_cells,
+                                                          mg, reinterpret_cast<float4*>(rgba));
+        else
+            render_tf_kernel<false><<<grid, block, 0, s>>>(d, g, vw, nlevels, lo, scale, dev_table, opacity_cut, nullptr,
+                                                           mg, reinterpret_cast<float4*>(rgba));
     }
     CUBE_CUDA(c, cudaGetLastError());
     return CUBE_OK;
+}
+
+int cube_render_tf(cube_ctx* c, const float* d, int64_t nx, int64_t ny, int64_t nz, const cube_view_t* view,
+                   int nlevels, float lo, float hi, const float* table, float opacity_cut, float* rgba, cudaStream_t s) {
+    return render_tf_common(c, d, nx, ny, nz, view, nlevels, lo, hi, table, opacity_cut, nullptr, 0, 0, 0, rgba, s);
+}
+
+int cube_render_sigma(cube_ctx* c, const float* d, int64_t nx, int64_t ny, int64_t nz, const cube_view_t* view,
+                      const cube_moments_t* cells, int64_t px, int64_t py, int64_t pz, int nlevels, float zlo, float zhi,
+                      const float* table, float opacity_cut, float* rgba, cudaStream_t s) {
+    if (!cells) return CUBE_EINVAL;
+    return render_tf_common(c, d, nx, ny, nz, view, nlevels, zlo, zhi, table, opacity_cut, cells, px, py, pz, rgba, s);
 }
 
 int cube_spectrum(cube_ctx* c, const float* d, int64_t nx, int64_t ny, int64_t nz, const cube_view_t* view, int u,

@@ -4,6 +4,8 @@
 //   maximum intensity projection       PAPER.md:166-172  "only the value of the maximum voxel through each cast ray"
 //   generic transfer function          PAPER.md:174-180  "The data values' range is partitioned into discrete levels.
 //                                      Each data level is assigned a colour and opacity value", ordered compositing
+//   sigma-clipping transfer function   PAPER.md:352-358, Fig. 7, Fig. 9: the generic one applied to (sample - local
+//                                      mean) / local std, "two trilinear interpolation operations" per sample
 //   3-D spectrum tool                  PAPER.md:298-306, Fig. 6: the profile along an arbitrary line of sight, "a
 //                                      constant sampling step ... trilinear interpolation"
 //
@@ -65,13 +67,18 @@ __device__ __forceinline__ RayF ray_setup(const RenderView& vw, const RenderGeom
     return r;
 }
 
-// Trilinear sample at sample i of the ray (R28).  false: outside the cube.
-__device__ __forceinline__ bool ray_sample(const float* __restrict__ d, const RenderGeom& g, const RenderView& vw,
-                                           const float (&o)[3], int i, float& out) {
+// Sample i of the ray (R27): p = o + (float)i * step.
+__device__ __forceinline__ void ray_point(const RenderView& vw, const float (&o)[3], int i, float (&p)[3]) {
     const float fi = (float)i;
-    const float px = __fadd_rn(o[0], __fmul_rn(fi, vw.step[0]));
-    const float py = __fadd_rn(o[1], __fmul_rn(fi, vw.step[1]));
-    const float pz = __fadd_rn(o[2], __fmul_rn(fi, vw.step[2]));
+#pragma unroll
+    for (int c = 0; c < 3; ++c) p[c] = __fadd_rn(o[c], __fmul_rn(fi, vw.step[c]));
+}
+
+__device__ __forceinline__ float lerp_rn(float a, float b, float f) { return __fadd_rn(a, __fmul_rn(f, __fsub_rn(b, a))); }
+
+// Trilinear sample at the data point p (R28).  false: outside the cube.
+__device__ __forceinline__ bool sample_at(const float* __restrict__ d, const RenderGeom& g, const float (&pt)[3], float& out) {
+    const float px = pt[0], py = pt[1], pz = pt[2];
     if (!(px >= 0.0f && px <= g.xmax && py >= 0.0f && py <= g.ymax && pz >= 0.0f && pz <= g.zmax)) return false;
     const float flx = floorf(px), fly = floorf(py), flz = floorf(pz);
     const float fx = __fsub_rn(px, flx), fy = __fsub_rn(py, fly), fz = __fsub_rn(pz, flz);
@@ -81,11 +88,56 @@ __device__ __forceinline__ bool ray_sample(const float* __restrict__ d, const Re
     const float* __restrict__ p = d + ((z0 * g.ny + y0) * g.nx + x0);
     const float v000 = __ldg(p), v100 = __ldg(p + dx), v010 = __ldg(p + dy), v110 = __ldg(p + dy + dx);
     const float v001 = __ldg(p + dz), v101 = __ldg(p + dz + dx), v011 = __ldg(p + dz + dy), v111 = __ldg(p + dz + dy + dx);
-    auto lerp = [](float a, float b, float f) { return __fadd_rn(a, __fmul_rn(f, __fsub_rn(b, a))); };
-    const float c00 = lerp(v000, v100, fx), c10 = lerp(v010, v110, fx);
-    const float c01 = lerp(v001, v101, fx), c11 = lerp(v011, v111, fx);
-    out = lerp(lerp(c00, c10, fy), lerp(c01, c11, fy), fz);
+    const float c00 = lerp_rn(v000, v100, fx), c10 = lerp_rn(v010, v110, fx);
+    const float c01 = lerp_rn(v001, v101, fx), c11 = lerp_rn(v011, v111, fx);
+    out = lerp_rn(lerp_rn(c00, c10, fy), lerp_rn(c01, c11, fy), fz);
     return true;
+}
+
+__device__ __forceinline__ bool ray_sample(const float* __restrict__ d, const RenderGeom& g, const RenderView& vw,
+                                           const float (&o)[3], int i, float& out) {
+    float p[3];
+    ray_point(vw, o, i, p);
+    return sample_at(d, g, p, out);
+}
+
+// The statistical mini-map as the second lookup of the sigma-clipping transfer function (R34): cell
+// (cx, cy, cz) sits at the centre of its nominal block, data coordinate cx * px + (px - 1) / 2.
+struct MapLookupGeom {
+    long long mx, my, mz;
+    float part[3], off[3], top[3];       // (float)px ..., (px - 1) / 2 ..., (float)(mx - 1) ...
+};
+
+// cells: the records cube_minimap wrote, viewed as doubles (5 per record: count, nan_count, min|max, mean, std).
+__device__ __forceinline__ void map_lookup(const double* __restrict__ cells, const MapLookupGeom& m, const float (&pt)[3],
+                                           float& mean, float& sd) {
+    long long i0[3], st[3];
+    float f[3];
+    const long long stride[3] = {1, m.mx, m.mx * m.my};
+#pragma unroll
+    for (int c = 0; c < 3; ++c) {
+        float q = __fdiv_rn(__fsub_rn(pt[c], m.off[c]), m.part[c]);
+        if (!(q >= 0.0f)) q = 0.0f;
+        if (q > m.top[c]) q = m.top[c];
+        const float fl = floorf(q);
+        i0[c] = (long long)fl;
+        f[c] = __fsub_rn(q, fl);
+        st[c] = f[c] > 0.0f ? stride[c] : 0;
+    }
+    const double* __restrict__ p = cells + ((i0[2] * m.my + i0[1]) * m.mx + i0[0]) * 5;
+    float out[2];
+#pragma unroll
+    for (int which = 0; which < 2; ++which) {
+        const double* __restrict__ q = p + 3 + which;
+        auto at = [&](long long o) { return (float)__ldg(q + o * 5); };
+        const float c00 = lerp_rn(at(0), at(st[0]), f[0]);
+        const float c10 = lerp_rn(at(st[1]), at(st[1] + st[0]), f[0]);
+        const float c01 = lerp_rn(at(st[2]), at(st[2] + st[0]), f[0]);
+        const float c11 = lerp_rn(at(st[2] + st[1]), at(st[2] + st[1] + st[0]), f[0]);
+        out[which] = lerp_rn(lerp_rn(c00, c10, f[1]), lerp_rn(c01, c11, f[1]), f[2]);
+    }
+    mean = out[0];
+    sd = out[1];
 }
 
 constexpr int kRenderTileU = 32, kRenderTileV = 8;   // a warp = 32 neighbouring pixels of one image row
@@ -111,17 +163,30 @@ render_mip_kernel(const float* __restrict__ d, RenderGeom g, RenderView vw, floa
 // Generic transfer function (R30, R31): level of the sample by the histogram's bin formula, front-to-back compositing
 //   w = (1 - A) * a;  C = C + w * c;  A = A + w;  stop when A >= opacity_cut.
 // table: nlevels x (r, g, b, opacity), device memory.
+// SIGMA: the sigma-clipping transfer function (R34) -- the looked-up value is the sample's distance
+// from the LOCAL mean in units of the LOCAL standard deviation, both interpolated in the mini-map; `lo` is then the
+// clipping threshold ("3 sigma").  Samples where the map has no statistics (std not > 0, NaN) are skipped.
+template <bool SIGMA>
 __global__ void __launch_bounds__(kRenderTileU * kRenderTileV)
 render_tf_kernel(const float* __restrict__ d, RenderGeom g, RenderView vw, int nlevels, float lo, float scale,
-                 const float4* __restrict__ table, float opacity_cut, float4* __restrict__ rgba) {
+                 const float4* __restrict__ table, float opacity_cut, const double* __restrict__ cells, MapLookupGeom mg,
+                 float4* __restrict__ rgba) {
     const int u = blockIdx.x * kRenderTileU + threadIdx.x, v = blockIdx.y * kRenderTileV + threadIdx.y;
     if (u >= vw.width || v >= vw.height) return;
     const RayF r = ray_setup(vw, g, u, v);
     float cr = 0.0f, cg = 0.0f, cb = 0.0f, A = 0.0f;
     const float top = (float)(nlevels - 1);
     for (int i = r.i0; i <= r.i1; ++i) {
-        float s;
-        if (!ray_sample(d, g, vw, r.o, i, s)) continue;
+        float s, p[3];
+        ray_point(vw, r.o, i, p);
+        if (!sample_at(d, g, p, s)) continue;
+        if (SIGMA) {
+            if (s != s) continue;            // NULL sample: no need to look at the map
+            float mean, sd;
+            map_lookup(cells, mg, p, mean, sd);
+            if (!(sd > 0.0f)) continue;
+            s = __fdiv_rn(__fsub_rn(s, mean), sd);
+        }
         if (!(s >= lo)) continue;            // below the range (the global threshold) or NULL
         const float fl = floorf(__fmul_rn(__fsub_rn(s, lo), scale));
         const int L = (fl >= top) ? nlevels - 1 : (int)fl;

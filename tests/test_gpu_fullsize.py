@@ -246,6 +246,18 @@ def test_config2_full_size():
                              (rgba.cpu().numpy().reshape(48, 64, 4), oracle.render_tf(a, dims, view, tab, 0.004, 0.1, 0.98)),
                              (prof.cpu().numpy(), oracle.spectrum(a, dims, view, 31, 25))):
             assert ((got_a.view(np.uint32) == ref_a.view(np.uint32)) | (np.isnan(got_a) & np.isnan(ref_a))).all()
+        # the sigma-clipping transfer function on the oracle's 30^3 mini-map (uploaded, so both sides read the same
+        # records): 3-sigma threshold, bit for bit
+        ref_cells = f_map.result()
+        cells_o = torch.frombuffer(bytearray(np.ascontiguousarray(ref_cells, dtype=cube.MINIMAP_DTYPE).tobytes()),
+                                   dtype=torch.uint8).cuda()
+        sig = torch.zeros(64 * 48 * 4, dtype=torch.float32, device="cuda")
+        ctx.render_sigma(t, *dims, view, cells_o, 30, 30, 30, tab, 3.0, 12.0, sig, opacity_cut=0.98)
+        torch.cuda.synchronize()
+        got_s = sig.cpu().numpy().reshape(48, 64, 4)
+        assert (got_s.view(np.uint32) == oracle.render_sigma(a, dims, view, ref_cells, (30, 30, 30), tab, 3.0, 12.0, 0.98)
+                .view(np.uint32)).all()
+        assert (got_s[..., 3] > 0).any()
         pool.shutdown()
     finally:
         ctx.close()

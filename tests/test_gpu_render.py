@@ -160,3 +160,92 @@ def test_view_orbit_matches_the_recipe_and_arguments_are_checked(ctx):
     v2 = cubegen.view_orbit((16, 16, 16), 20, 30, 24, 24)
     assert same_bits(gpu_tf(ctx, ta, (16, 16, 16), v2, torch.from_numpy(tab).cuda(), 0.0, 0.01),
                      gpu_tf(ctx, ta, (16, 16, 16), v2, tab, 0.0, 0.01))
+
+
+# ---- the sigma-clipping transfer function (R34) -----------------------------------------------
+
+def gpu_sigma(ctx, t, dims, view, cells_dev, part, table, zlo, zhi, cut=2.0):
+    out = torch.full((view["height"] * view["width"] * 4,), 123.0, dtype=torch.float32, device="cuda")
+    ctx.render_sigma(t, *dims, view, cells_dev, *part, table, zlo, zhi, out, opacity_cut=cut)
+    torch.cuda.synchronize()
+    return out.cpu().numpy().reshape(view["height"], view["width"], 4)
+
+
+def upload_cells(cells):
+    """the oracle's mini-map records -> device bytes in cube_moments_t layout"""
+    raw = np.ascontiguousarray(cells, dtype=cube.MINIMAP_DTYPE).tobytes()
+    return torch.frombuffer(bytearray(raw), dtype=torch.uint8).cuda()
+
+
+@pytest.mark.parametrize("name,dims,part", [("c2", (96, 80, 64), (30, 30, 30)), ("c3", (48, 40, 120), (8, 8, 8)),
+                                            ("c1", (33, 17, 9), (4, 5, 2)), ("c4", (64, 64, 16), (64, 64, 16)),
+                                            ("c2", (50, 40, 30), (1, 1, 1))])
+def test_sigma_clipping_rotated_views(ctx, name, dims, part):
+    # both sides read the SAME mini-map (the oracle's, uploaded): the images must then agree bit for bit
+    t, a = scaled_cube(name, dims, misalign=1 if name == "c1" else 0)
+    cells = oracle.minimap(a, dims, part)
+    cd = upload_cells(cells)
+    for yaw, pitch, step in VIEWS[:5]:
+        view = cubegen.view_orbit(dims, yaw, pitch, 64, 48, step=step)
+        for nlev, zlo, zhi, cut in ((16, 2.0, 7.0, 2.0), (256, 3.0, 12.0, 0.95), (1, 1.0, 1.0, 2.0), (64, -2.0, 2.0, 0.5)):
+            tab = colour_table(nlev, nlev + 1)
+            tab[:, 3] = np.maximum(tab[:, 3], np.float32(0.05))
+            got = gpu_sigma(ctx, t, dims, view, cd, part, tab, zlo, zhi, cut)
+            ref = oracle.render_sigma(a, dims, view, cells, part, tab, zlo, zhi, cut)
+            assert same_bits(got, ref), (yaw, pitch, nlev)
+    # something was drawn at the 2-sigma threshold (1 x 1 x 1 cells have std 0 everywhere: nothing is drawn there)
+    view = cubegen.view_orbit(dims, 30, 20, 64, 48)
+    img = gpu_sigma(ctx, t, dims, view, cd, part, colour_table(16, 2) + np.float32(0.01), 2.0, 7.0)
+    assert (img[..., 3] > 0).any() == (part != (1, 1, 1))
+
+
+def test_sigma_clipping_map_edge_cases(ctx):
+    dims, part = (40, 30, 20), (8, 7, 6)
+    r = np.random.default_rng(11)
+    a = r.standard_normal(40 * 30 * 20).astype(np.float32)
+    vol = a.reshape(20, 30, 40)
+    vol[0:6, 0:7, 0:8] = np.nan                      # an empty cell: NaN record, poisons its neighbourhood only
+    vol[6:12, 7:14, 8:16] = 1.5                      # a constant cell: std 0
+    a[r.integers(0, a.size, a.size // 40)] = np.nan
+    t = torch.from_numpy(a).cuda()
+    cells = oracle.minimap(a, dims, part)
+    assert np.isnan(cells["mean"][0, 0, 0]) and cells["std"][1, 1, 1] == 0.0
+    cd = upload_cells(cells)
+    tab = colour_table(32, 5)
+    for view in (cubegen.view_axis(dims, 0), cubegen.view_axis(dims, 1, step=0.5), cubegen.view_axis(dims, 2),
+                 cubegen.view_orbit(dims, 33, 44, 50, 50, 0.7)):
+        assert same_bits(gpu_sigma(ctx, t, dims, view, cd, part, tab, 0.5, 4.0),
+                         oracle.render_sigma(a, dims, view, cells, part, tab, 0.5, 4.0))
+    # pinned host records are read in place
+    pinned = torch.frombuffer(bytearray(np.ascontiguousarray(cells).tobytes()), dtype=torch.uint8).pin_memory()
+    view = cubegen.view_orbit(dims, 10, 20, 32, 32)
+    assert same_bits(gpu_sigma(ctx, t, dims, view, pinned, part, tab, 0.5, 4.0),
+                     oracle.render_sigma(a, dims, view, cells, part, tab, 0.5, 4.0))
+    # argument checks: pageable records, zero partition, inverted range
+    out = torch.zeros(32 * 32 * 4, device="cuda")
+    host_cells = np.frombuffer(np.ascontiguousarray(cells).tobytes(), dtype=np.uint8).copy()
+    for bad in (lambda: ctx.render_sigma(t, *dims, view, host_cells, *part, tab, 0.5, 4.0, out),
+                lambda: ctx.render_sigma(t, *dims, view, cd, 0, 7, 6, tab, 0.5, 4.0, out),
+                lambda: ctx.render_sigma(t, *dims, view, cd, *part, tab, 4.0, 0.5, out)):
+        with pytest.raises(cube.CubeError):
+            bad()
+
+
+def test_sigma_clipping_on_the_librarys_own_minimap(ctx):
+    # end to end through the C ABI: cube_minimap -> cube_render_sigma.  The device's cell means and deviations agree
+    # with the oracle's to ~1e-12 (fp64), so after rounding to float32 a record differs with probability ~1e-5 and
+    # an image pixel essentially never: at least 99.9 % of the pixels are bit-equal, the rest close
+    dims, part = (96, 80, 64), (30, 30, 30)
+    t, a = scaled_cube("c2", dims)
+    mx, my, mz = ctx.minimap_dims(*dims, *part)
+    cells_dev = torch.zeros(mx * my * mz * 40, dtype=torch.uint8, device="cuda")
+    ctx.minimap(t, *dims, *part, cells_dev)
+    cells = oracle.minimap(a, dims, part)
+    tab = colour_table(64, 9)
+    for yaw, pitch in ((30, 20), (200, -40)):
+        view = cubegen.view_orbit(dims, yaw, pitch, 96, 96, 0.5)
+        got = gpu_sigma(ctx, t, dims, view, cells_dev, part, tab, 2.0, 7.0)
+        ref = oracle.render_sigma(a, dims, view, cells, part, tab, 2.0, 7.0)
+        equal = (got.view(np.uint32) == ref.view(np.uint32)).all(axis=-1)
+        assert equal.mean() >= 0.999
+        assert np.abs(got - ref).max() <= 0.05
