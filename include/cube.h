@@ -364,6 +364,10 @@ enum {
     CUBE_KNOB_SMALL = 3,       /* cube_stats on a cube of at most 96 MiB with a histogram of at most 4096 bins and the
                                   median: 0 = automatic (default): ONE cooperative launch (csrc/cube_small.cuh) when the
                                   device supports it, 1 = always the general three-launch path */
+    CUBE_KNOB_MAPMEDIAN = 4,   /* cube_minimap_median on cells of at least 1024 voxels: 0 = automatic (default) = 2;
+                                  1 = the cell's keys staged in shared memory, four 8-bit digits (cells of more than
+                                      56000 voxels: re-read per digit); 2 = two reads of the cell, 11-bit first digit,
+                                      the bucket's keys kept in shared memory (csrc/cube_minimap_median.cuh) */
     CUBE_KNOB_MINIMAP = 2      /* cube_minimap kernel: 0 = automatic (default): lines staged through a shared-memory
                                   ring by TMA bulk copies when the rows are 16-byte aligned, the cells at most 480
                                   voxels wide and a cell row has at least 256 lines (or the 128-bit kernel is not

@@ -38,7 +38,7 @@ SYMBOLS = ["cube_create", "cube_destroy", "cube_moments", "cube_histogram", "cub
            "cube_view_orbit", "cube_render_mip", "cube_render_tf", "cube_render_sigma", "cube_spectrum",
            "cube_minimap_median"]
 SHARD_RECORD_BYTES, SHARD_DIGITS = 40, 8192
-KNOB_CTAS_PER_SM, KNOB_BIGHIST, KNOB_MINIMAP, KNOB_SMALL = 0, 1, 2, 3
+KNOB_CTAS_PER_SM, KNOB_BIGHIST, KNOB_MINIMAP, KNOB_SMALL, KNOB_MAPMEDIAN = 0, 1, 2, 3, 4
 KIND_NAMES = ["moments", "moments_coarse", "histogram", "select_pass0", "select_pass1", "select_pass2",
               "select_cand", "select_scan", "hist_select", "probe_read", "other", "moments_window", "minimap", "torben_pass",
               "render", "stats_small"]

@@ -27,6 +27,7 @@ struct cube_ctx {
     int ctas_per_sm = 0;  // 0 = per-kernel default
     int bighist = 0;      // CUBE_KNOB_BIGHIST: 0 = automatic (window or packed, chosen on the device), 1 = cluster DSM, 2 = packed
     int no_small = 0;     // CUBE_KNOB_SMALL: 1 = never the single cooperative launch
+    int mapmedian = 0;    // CUBE_KNOB_MAPMEDIAN
     int coop = 0;         // the device supports cooperative launches
     unsigned int* bar = nullptr;   // grid-barrier counter of stats_small_kernel (only grows)
     unsigned int bar_base = 0;
@@ -959,6 +960,14 @@ int cube_spectrum(cube_ctx* c, const float* d, int64_t nx, int64_t ny, int64_t n
     return CUBE_OK;
 }
 
+// The two-read kernel addresses a cell's voxels by 32-bit byte offsets and divides row numbers by a multiplication
+// (cube_minimap_median.cuh): both hold for every cell anyone would use; the rest takes the staged kernel.
+static bool med_two_reads_ok(int64_t nx, int64_t ny, int64_t nz, int64_t py, int64_t pz) {
+    const long double h = (long double)std::min(py, ny), dep = (long double)std::min(pz, nz);
+    return dep * (long double)ny * (long double)nx < 1073741824.0L && h * h * dep < 4294967296.0L &&
+           dep * dep < 4294967296.0L;
+}
+
 int cube_minimap_median(cube_ctx* c, const float* d, int64_t nx, int64_t ny, int64_t nz, int64_t px, int64_t py,
                         int64_t pz, float* med, cudaStream_t s) {
     MedGeom g;
@@ -980,6 +989,10 @@ int cube_minimap_median(cube_ctx* c, const float* d, int64_t nx, int64_t ny, int
             const long double want = (ncell + per - 1) / per;
             const unsigned grid = (unsigned)std::min<long double>(want < 1 ? 1 : want, (long double)c->num_sms * 16);
             minimap_median_warp_kernel<<<grid, kMedCtaThreads, per * kMedWarpSmemPerWarp, s>>>(d, g, med);
+        } else if (c->mapmedian != 1 && med_two_reads_ok(nx, ny, nz, py, pz)) {
+            const int occ = occupancy_of(c, minimap_median_two_reads_kernel, kMed2Threads, kMed2Smem);
+            const unsigned grid = (unsigned)std::min<long double>(ncell, (long double)c->num_sms * (occ < 1 ? 1 : occ));
+            minimap_median_two_reads_kernel<<<grid, kMed2Threads, kMed2Smem, s>>>(d, g, med);
         } else {
             const int stage = cellvox <= (long double)kMedStageKeys ? (((int)cellvox + 3) & ~3) : 0;
             const size_t smem = (size_t)stage * 4 + kMedCtaExtra;
@@ -1034,6 +1047,10 @@ int cube_set_knob(cube_ctx* c, int knob, int value) {
         case CUBE_KNOB_SMALL:
             if (value < 0 || value > 1) return CUBE_EINVAL;
             c->no_small = value;
+            return CUBE_OK;
+        case CUBE_KNOB_MAPMEDIAN:
+            if (value < 0 || value > 2) return CUBE_EINVAL;
+            c->mapmedian = value;
             return CUBE_OK;
         case CUBE_KNOB_MINIMAP:
             if (value < 0 || value > 3) return CUBE_EINVAL;

@@ -9,6 +9,8 @@
 // kMedStageKeys voxels) are re-read from global memory for each digit instead (L2 / HBM: 16 B per voxel).
 // The paper's Alg. 1 would take ~31 passes per cell.
 #pragma once
+#include <type_traits>
+
 #include "cube_common.cuh"
 
 namespace cube {
@@ -40,16 +42,26 @@ __device__ __forceinline__ uint32_t med_sum(uint32_t v, uint32_t* red, int tid) 
     return t;
 }
 
-// The bin holding rank k in hist[256] (counts of the keys still in play) and the rank left inside it; every thread
-// gets both.  GROUP >= 256: thread t < 256 owns bin t; GROUP = 32: lane l owns bins 8l .. 8l+7.
-template <int GROUP>
+// The bin holding rank k in hist[BINS] (counts of the keys still in play) and the rank left inside it; every thread
+// gets both.  Thread t < OWNERS = min(GROUP, BINS) owns the BINS / OWNERS bins from t * PER on.
+template <int GROUP, int BINS = 256>
 __device__ __forceinline__ void med_locate(const uint32_t* hist, uint32_t k, uint32_t* red, int tid, uint32_t& bin, uint32_t& krem) {
-    constexpr int OWNERS = GROUP < 256 ? GROUP : 256;   // threads that own bins
-    constexpr int PER = 256 / OWNERS;
+    constexpr int OWNERS = GROUP < BINS ? GROUP : BINS;   // threads that own bins
+    constexpr int PER = BINS / OWNERS;
     const bool owner = tid < OWNERS;
     uint32_t c[PER], mine = 0;
+    if (PER % 4 == 0) {
 #pragma unroll
-    for (int j = 0; j < PER; ++j) { c[j] = owner ? hist[tid * PER + j] : 0u; mine += c[j]; }
+        for (int j = 0; j < PER; j += 4) {
+            const uint4 q = owner ? *reinterpret_cast<const uint4*>(hist + tid * PER + j) : make_uint4(0u, 0u, 0u, 0u);
+            c[j] = q.x; c[j + 1] = q.y; c[j + 2] = q.z; c[j + 3] = q.w;
+        }
+    } else {
+#pragma unroll
+        for (int j = 0; j < PER; ++j) c[j] = owner ? hist[tid * PER + j] : 0u;
+    }
+#pragma unroll
+    for (int j = 0; j < PER; ++j) mine += c[j];
     uint32_t incl = mine;
     const int lane = tid & 31;
 #pragma unroll
@@ -66,13 +78,299 @@ __device__ __forceinline__ void med_locate(const uint32_t* hist, uint32_t k, uin
     }
     uint32_t excl = before + incl - mine;
     med_sync<GROUP>();                               // red[0..1] become the answer
+    if (excl <= k && k < excl + mine) {              // exactly one owner
 #pragma unroll
-    for (int j = 0; j < PER; ++j) {
-        if (c[j] && excl <= k && k < excl + c[j]) { red[0] = (uint32_t)(tid * PER + j); red[1] = k - excl; }   // exactly one
-        excl += c[j];
+        for (int j = 0; j < PER; ++j) {
+            if (c[j] && excl <= k && k < excl + c[j]) { red[0] = (uint32_t)(tid * PER + j); red[1] = k - excl; }
+            excl += c[j];
+        }
     }
     med_sync<GROUP>();
     bin = red[0]; krem = red[1];
+}
+
+// The voxels of one cell: `rows` rows of w contiguous voxels.
+struct MedCell {
+    const float* base;
+    int w, h, rows;
+    uint32_t nvox, magic;            // magic = floor(2^32 / h) + 1: r / h == umulhi(r, magic) while r * h < 2^32
+    int lpr_log1, lpr_log2;          // log2 of the lanes a row takes, read as floats / as float2 (-1: not eligible)
+    long long row_step, plane_step;
+};
+
+__device__ __forceinline__ MedCell med_cell_of(const float* __restrict__ d, const MedGeom& g, long long cell) {
+    const long long cx = cell % g.mx, cy = (cell / g.mx) % g.my, cz = cell / (g.mx * g.my);
+    const long long x0 = cx * g.px, y0 = cy * g.py, z0 = cz * g.pz;
+    MedCell c;
+    c.w = (int)min(g.px, g.nx - x0);
+    c.h = (int)min(g.py, g.ny - y0);
+    c.rows = c.h * (int)min(g.pz, g.nz - z0);
+    c.nvox = (uint32_t)c.w * (uint32_t)c.rows;
+    c.base = d + ((z0 * g.ny + y0) * g.nx + x0);
+    c.row_step = g.nx;
+    c.plane_step = g.ny * g.nx;
+    if (c.h == 1) { c.h = c.rows; c.row_step = c.plane_step; }      // one line per plane: the planes are the rows
+    c.magic = c.h == 1 ? 0u : (uint32_t)(0x100000000ull / (uint32_t)c.h) + 1u;   // h == 1: a single row, r = 0
+    auto lanes_log = [](int n) { int l = 0; while ((1 << l) < n && l < 5) ++l; return l; };
+    c.lpr_log1 = lanes_log(c.w);
+    const bool pairs = (c.w & 1) == 0 && (reinterpret_cast<uintptr_t>(c.base) & 7u) == 0 && (c.row_step & 1) == 0 &&
+                       (c.plane_step & 1) == 0;
+    c.lpr_log2 = pairs ? lanes_log(c.w / 2) : -1;
+    return c;
+}
+
+// fn(v) for every voxel of the cell: a warp takes rows, kMedInFlight at a time (that many loads per lane in flight:
+// the read of a cell is a chain of dependent round trips otherwise); the (y, z) of a warp's row advances by
+// additions; offsets from the cell's first voxel fit 32 bits (checked by the caller).
+#ifndef CUBE_MED_INFLIGHT
+#define CUBE_MED_INFLIGHT 8
+#endif
+constexpr int kMedInFlight = CUBE_MED_INFLIGHT;
+
+// A row of the cell takes LPR = 2^lpr_log lanes (the smallest power of two holding w / VEC elements, at most 32), so a
+// warp load covers 32 / LPR rows: a 30-voxel row read as 15 float2 (VEC = 2: rows 8-byte aligned, w even) shares its
+// load with a second row, a 16-voxel row with three more.  What a load costs in address arithmetic (the division of
+// the row number by the cell's height is a multiplication by c.magic, exact while r * h < 2^32; the byte offset three
+// IMADs; base + 32-bit offset) is spent once per load, hence the packing.
+template <int GROUP, int VEC, class F>
+__device__ __forceinline__ void med_for_each_voxel_v(const MedCell& c, int tid, F&& fn) {
+    constexpr int NW = GROUP / 32, U = kMedInFlight;
+    const int lane = tid & 31, wid = tid >> 5;
+    const int lpr_log = VEC == 2 ? c.lpr_log2 : c.lpr_log1, rpw_log = 5 - lpr_log;
+    const uint32_t sub = (uint32_t)lane >> lpr_log, col = ((uint32_t)lane & ((1u << lpr_log) - 1u)) * VEC;
+    const uint32_t rstep = (uint32_t)NW << rpw_log;                          // rows per step of the whole CTA
+    const uint32_t xstep = (uint32_t)VEC << lpr_log;
+    const uint32_t hh = (uint32_t)c.h, magic = c.magic, rows = (uint32_t)c.rows, w = (uint32_t)c.w;
+    const uint32_t row_bytes = (uint32_t)c.row_step * 4u, plane_bytes = (uint32_t)c.plane_step * 4u;
+    const char* __restrict__ base = reinterpret_cast<const char*>(c.base);
+    for (uint32_t rw = (uint32_t)wid << rpw_log; rw < rows; rw += rstep * U) {   // rw: the warp's first row of the batch
+        uint32_t o[U];
+#pragma unroll
+        for (int u = 0; u < U; ++u) {
+            const uint32_t r = rw + sub + (uint32_t)u * rstep;
+            const uint32_t z = __umulhi(r, magic), y = r - z * hh;
+            o[u] = z * plane_bytes + y * row_bytes + col * 4u;
+        }
+        const bool full = rw + ((1u << rpw_log) - 1u) + (U - 1) * rstep < rows;   // warp-uniform
+        for (uint32_t x0 = 0; x0 < w; x0 += xstep) {
+            const char* __restrict__ q = base + x0 * 4u;                     // warp-uniform
+            if (col + x0 < w) {
+                float a[U], b[U];
+                if (full) {
+#pragma unroll
+                    for (int u = 0; u < U; ++u) {
+                        if (VEC == 2) {
+                            const float2 t = __ldg(reinterpret_cast<const float2*>(q + o[u]));
+                            a[u] = t.x; b[u] = t.y;
+                        } else {
+                            a[u] = __ldg(reinterpret_cast<const float*>(q + o[u]));
+                        }
+                    }
+#pragma unroll
+                    for (int u = 0; u < U; ++u) { fn(a[u]); if (VEC == 2) fn(b[u]); }
+                } else {
+#pragma unroll
+                    for (int u = 0; u < U; ++u) {
+                        if (rw + sub + (uint32_t)u * rstep < rows) {
+                            if (VEC == 2) {
+                                const float2 t = __ldg(reinterpret_cast<const float2*>(q + o[u]));
+                                fn(t.x); fn(t.y);
+                            } else {
+                                fn(__ldg(reinterpret_cast<const float*>(q + o[u])));
+                            }
+                        }
+                    }
+                }
+            }
+        }
+    }
+}
+
+template <int GROUP, class F>
+__device__ __forceinline__ void med_for_each_voxel(const MedCell& c, int tid, F&& fn) {
+    if (c.lpr_log2 >= 0) med_for_each_voxel_v<GROUP, 2>(c, tid, fn);        // uniform over the CTA
+    else med_for_each_voxel_v<GROUP, 1>(c, tid, fn);
+}
+
+// Two-read selection of one cell by one CTA (cells of any size).
+//   read 1 (HBM): the 11-bit first digit counted in shared memory.  The digit is taken from the RAW bits (sign, exponent,
+//       two mantissa bits) -- no key conversion per voxel; NULL voxels are left out by a predicate (5 instructions per
+//       voxel: LDG, FSETP, SHF, LOP3, predicated RED) and the buckets are only put in key order when they are
+//       scanned: key-order bucket j is raw bucket 2047 - j (negative values, descending) or j - 1024.
+//   read 2 (the cell's lines are in L2: a 30^3 cell is 105 KiB): the voxels of the median's bucket -- a few per cent
+//       of the cell -- are appended to a buffer in shared memory (bits - rawbase < 2^21, predicated ATOMS + STS); the
+//       remaining 11 + 10 key bits are fixed on those.
+// A bucket that does not fit kMed2Cand keys (constant cells, heavy ties) has its digits counted by further reads of
+// the cell instead.  24.1 KiB of shared memory per CTA whatever the cell size.
+constexpr int kMed2Threads = 256;
+constexpr int kMed2Bins = 2048;
+constexpr int kMed2Cand = 4096;
+constexpr int kMed2Smem = (kMed2Bins + kMed2Cand + 16) * 4;
+
+// counts of key-order buckets 8 * tid .. 8 * tid + 7 from the raw-order histogram (256 threads)
+__device__ __forceinline__ void med_load_raw_order(const uint32_t* hist, int tid, uint32_t (&c)[8]) {
+    const bool neg = tid < 128;
+    const int base = neg ? 2040 - 8 * tid : 8 * tid - 1024;
+    const uint4 a = *reinterpret_cast<const uint4*>(hist + base), b = *reinterpret_cast<const uint4*>(hist + base + 4);
+    const uint32_t r[8] = {a.x, a.y, a.z, a.w, b.x, b.y, b.z, b.w};
+#pragma unroll
+    for (int j = 0; j < 8; ++j) c[j] = neg ? r[7 - j] : r[j];
+}
+
+// as med_locate, on bucket counts already in registers (256 threads, 8 buckets each, bucket index = 8 * tid + j)
+__device__ __forceinline__ void med_locate_regs(const uint32_t (&c)[8], uint32_t k, uint32_t* red, int tid, uint32_t& bin,
+                                                uint32_t& krem, uint32_t& total) {
+    uint32_t mine = 0;
+#pragma unroll
+    for (int j = 0; j < 8; ++j) mine += c[j];
+    uint32_t incl = mine;
+    const int lane = tid & 31;
+#pragma unroll
+    for (int off = 1; off < 32; off <<= 1) {
+        const uint32_t u = __shfl_up_sync(0xffffffffu, incl, off);
+        if (lane >= off) incl += u;
+    }
+    __syncthreads();
+    if (lane == 31) red[tid >> 5] = incl;
+    __syncthreads();
+    uint32_t before = 0, all = 0;
+#pragma unroll
+    for (int w = 0; w < 8; ++w) { const uint32_t t = red[w]; all += t; before += w < (tid >> 5) ? t : 0u; }
+    total = all;
+    if (k == 0xFFFFFFFFu) k = all ? (all - 1) / 2 : 0;      // the lower median of what was counted
+    uint32_t excl = before + incl - mine;
+    __syncthreads();
+    if (excl <= k && k < excl + mine) {                      // exactly one thread (none when all == 0)
+#pragma unroll
+        for (int j = 0; j < 8; ++j) {
+            if (c[j] && excl <= k && k < excl + c[j]) { red[0] = (uint32_t)(tid * 8 + j); red[1] = k - excl; red[2] = c[j]; }
+            excl += c[j];
+        }
+    }
+    __syncthreads();
+    bin = red[0]; krem = red[1];
+}
+
+__device__ __forceinline__ float med_cell_two_reads(const MedCell& c, uint32_t* hist, uint32_t* cand, uint32_t* red, int tid) {
+    constexpr int GROUP = kMed2Threads;
+    const uint32_t hist_s = (uint32_t)__cvta_generic_to_shared(hist);
+    const uint32_t cand_s = (uint32_t)__cvta_generic_to_shared(cand);
+    const uint32_t ncand_s = (uint32_t)__cvta_generic_to_shared(red + 8);
+    auto zero_hist = [&]() {
+        uint4* h4 = reinterpret_cast<uint4*>(hist);
+        for (int i = tid; i < kMed2Bins / 4; i += GROUP) h4[i] = make_uint4(0u, 0u, 0u, 0u);
+        if (tid == 0) red[8] = 0;                    // the candidate counter
+    };
+    zero_hist();
+    __syncthreads();
+    // read 1: every voxel counted by its raw top 11 bits, NULL voxels included (SHF, LEA, ATOMS per voxel).  The raw
+    // buckets 0x3FD-0x3FF / 0x7FD-0x7FF hold nothing but NaN patterns and are dropped when the buckets are scanned;
+    // 0x3FC / 0x7FC hold +-Inf AND the NaN patterns with a payload below 2^21: a cell with anything in those two is
+    // counted again with the NULL test per voxel (rare: cells holding infinities).
+    med_for_each_voxel<GROUP>(c, tid, [&](float v) {
+        const uint32_t a = hist_s + (__float_as_uint(v) >> 21) * 4u;
+        asm volatile("red.shared.add.u32 [%0], 1;" ::"r"(a) : "memory");
+    });
+    __syncthreads();
+    uint32_t cnt[8], k, b0, b1, b2, count;
+    auto load_counts = [&]() {
+        med_load_raw_order(hist, tid, cnt);
+        if (tid == 0) cnt[0] = cnt[1] = cnt[2] = 0;            // key-order buckets 0-2 and 2045-2047: NaN patterns only
+        if (tid == GROUP - 1) cnt[5] = cnt[6] = cnt[7] = 0;
+    };
+    load_counts();
+    if (tid == 0) red[9] = cnt[3];                             // -Inf and negative NaNs of small payload
+    if (tid == GROUP - 1) red[10] = cnt[4];                    // +Inf and positive NaNs of small payload
+    __syncthreads();
+    const bool careful = (red[9] | red[10]) != 0;              // uniform over the CTA
+    if (careful) {
+        __syncthreads();
+        zero_hist();
+        __syncthreads();
+        med_for_each_voxel<GROUP>(c, tid, [&](float v) {
+            if (v == v) atomicAdd(&hist[__float_as_uint(v) >> 21], 1u);
+        });
+        __syncthreads();
+        load_counts();
+    }
+    med_locate_regs(cnt, 0xFFFFFFFFu, red, tid, b0, k, count);
+    if (count == 0) return __int_as_float(0x7fc00000);       // uniform over the CTA: no non-NULL voxel
+    const uint32_t c0 = red[2];
+    const uint32_t rawbase = (b0 >= 1024u ? b0 - 1024u : 2047u - b0) << 21;
+    __syncthreads();
+    zero_hist();
+    __syncthreads();
+    if (c0 <= (uint32_t)kMed2Cand) {
+        // read 2: the voxels of the bucket (bits - rawbase < 2^21; a NULL voxel can only pass in a `careful` cell)
+        if (!careful) {
+            med_for_each_voxel<GROUP>(c, tid, [&](float v) {
+                const uint32_t bits = __float_as_uint(v);
+                if (bits - rawbase < 0x200000u) {
+                    uint32_t pos;
+                    asm volatile("atom.shared.add.u32 %0, [%1], 1;" : "=r"(pos) : "r"(ncand_s) : "memory");
+                    CUBE_CHECK(pos < (uint32_t)kMed2Cand);
+                    asm volatile("st.shared.u32 [%0], %1;" ::"r"(cand_s + pos * 4u), "r"(bits) : "memory");
+                }
+            });
+        } else {
+            med_for_each_voxel<GROUP>(c, tid, [&](float v) {
+                const uint32_t bits = __float_as_uint(v);
+                if (bits - rawbase < 0x200000u && v == v) {
+                    const uint32_t pos = atomicAdd(&red[8], 1u);
+                    CUBE_CHECK(pos < (uint32_t)kMed2Cand);
+                    cand[pos] = bits;
+                }
+            });
+        }
+        __syncthreads();
+        CUBE_CHECK(red[8] == c0);
+        for (uint32_t i = tid; i < c0; i += GROUP) atomicAdd(&hist[(key_of(__uint_as_float(cand[i])) >> 10) & 2047u], 1u);
+        __syncthreads();
+        med_locate<GROUP, kMed2Bins>(hist, k, red, tid, b1, k);
+        __syncthreads();
+        zero_hist();
+        __syncthreads();
+        for (uint32_t i = tid; i < c0; i += GROUP) {
+            const uint32_t key = key_of(__uint_as_float(cand[i]));
+            if (((key >> 10) & 2047u) == b1) atomicAdd(&hist[key & 1023u], 1u);
+        }
+    } else {
+        med_for_each_voxel<GROUP>(c, tid, [&](float v) {
+            const uint32_t key = key_of(v);
+            if ((key >> 21) == b0 && v == v) atomicAdd(&hist[(key >> 10) & 2047u], 1u);
+        });
+        __syncthreads();
+        med_locate<GROUP, kMed2Bins>(hist, k, red, tid, b1, k);
+        __syncthreads();
+        zero_hist();
+        __syncthreads();
+        const uint32_t top = (b0 << 11) | b1;
+        med_for_each_voxel<GROUP>(c, tid, [&](float v) {
+            const uint32_t key = key_of(v);
+            if ((key >> 10) == top && v == v) atomicAdd(&hist[key & 1023u], 1u);
+        });
+    }
+    __syncthreads();
+    med_locate<GROUP, kMed2Bins>(hist, k, red, tid, b2, k);
+    return __uint_as_float(bits_of_key((b0 << 21) | (b1 << 10) | b2));
+}
+
+#ifndef CUBE_MED2_CTAS
+#define CUBE_MED2_CTAS 5
+#endif
+__global__ void __launch_bounds__(kMed2Threads, CUBE_MED2_CTAS)
+minimap_median_two_reads_kernel(const float* __restrict__ d, MedGeom g, float* __restrict__ med) {
+    extern __shared__ __align__(16) uint32_t med_smem[];
+    uint32_t* hist = med_smem;
+    uint32_t* cand = med_smem + kMed2Bins;
+    uint32_t* red = cand + kMed2Cand;
+    const long long ncell = g.mx * g.my * g.mz;
+    for (long long cell = blockIdx.x; cell < ncell; cell += gridDim.x) {
+        const MedCell c = med_cell_of(d, g, cell);
+        const float r = med_cell_two_reads(c, hist, cand, red, threadIdx.x);
+        if (threadIdx.x == 0) med[cell] = r;
+        __syncthreads();
+    }
 }
 
 // One group, one cell.  keys: the group's stage (STAGED) ; hist: 256 counters; red: 8 words.

@@ -362,12 +362,21 @@ def test_torben_edge_cases_and_async(ctx):
 
 # --------------------------------------------------------------------------------------- mini-map: per-cell median
 def run_minimap_median(ctx, t, dims, part):
+    """every kernel variant (CUBE_KNOB_MAPMEDIAN: two reads / keys staged in shared memory) must give the same bits"""
     nx, ny, nz = dims
     mx, my, mz = ctx.minimap_dims(nx, ny, nz, *part)
-    med = torch.full((mx * my * mz,), 123.0, dtype=torch.float32, device="cuda")
-    ctx.minimap_median(t, nx, ny, nz, part[0], part[1], part[2], med)
-    torch.cuda.synchronize()
-    return med.cpu().numpy().reshape(mz, my, mx)
+    outs = []
+    try:
+        for variant in (0, 1, 2):
+            ctx.set_knob(cube.KNOB_MAPMEDIAN, variant)
+            med = torch.full((mx * my * mz,), 123.0, dtype=torch.float32, device="cuda")
+            ctx.minimap_median(t, nx, ny, nz, part[0], part[1], part[2], med)
+            torch.cuda.synchronize()
+            outs.append(med.cpu().numpy().reshape(mz, my, mx))
+    finally:
+        ctx.set_knob(cube.KNOB_MAPMEDIAN, 0)
+    assert same_bits_map(outs[0], outs[1]) and same_bits_map(outs[0], outs[2])
+    return outs[0]
 
 
 def same_bits_map(got, ref):
@@ -381,7 +390,8 @@ def same_bits_map(got, ref):
                                        ((50, 40, 30), (64, 64, 64)), ((513, 20, 19), (30, 30, 30)),
                                        ((70, 66, 65), (64, 64, 32)),     # 131072 voxels per cell: re-read per digit
                                        ((40, 40, 40), (38, 38, 38)),     # 54872 voxels: the largest staged cells
-                                       ((33, 32, 31), (11, 10, 9)), ((9, 9, 9), (10, 10, 1024))])
+                                       ((33, 32, 31), (11, 10, 9)), ((9, 9, 9), (10, 10, 1024)),
+                                       ((300, 40, 30), (150, 40, 30))])  # 180000 voxels per cell
 def test_minimap_median_shapes(ctx, dims, part):
     nx, ny, nz = dims
     r = np.random.default_rng(nx * 131 + part[0])
@@ -405,6 +415,34 @@ def test_minimap_median_degenerate_cells(ctx):
     vol[30, 5, 40] = 7.0                                                     # a cell with a single voxel
     got = run_minimap_median(ctx, dev(vol.reshape(-1)), dims, part)
     assert same_bits_map(got, oracle.minimap_median(vol.reshape(-1), dims, part))
+    # buckets larger than the candidate buffer of the two-read kernel (4096 keys): a cell of two values, the median
+    # among 20000 copies of the upper one; a cell whose first digit ties but whose second differs; 0 / 1 data
+    r = np.random.default_rng(8)
+    two = np.where(r.random(64 * 40 * 36) < 0.45, np.float32(1.0), np.float32(1.0000001)).astype(np.float32)
+    got = run_minimap_median(ctx, dev(two), dims, (64, 40, 36))
+    assert same_bits_map(got, oracle.minimap_median(two, dims, (64, 40, 36)))
+    near = (1.0 + r.random(64 * 40 * 36) * 1e-3).astype(np.float32)           # 8000 distinct keys in one first-digit bin
+    near[r.integers(0, near.size, 500)] = np.nan
+    for p3 in ((64, 40, 36), (32, 20, 12)):
+        assert same_bits_map(run_minimap_median(ctx, dev(near), dims, p3), oracle.minimap_median(near, dims, p3))
+    flags = (r.random(64 * 40 * 36) < 0.5).astype(np.float32)
+    assert same_bits_map(run_minimap_median(ctx, dev(flags), dims, (32, 20, 12)), oracle.minimap_median(flags, dims, (32, 20, 12)))
+    # infinities and NaN patterns that share their top 11 bits with them (payload below 2^21), the median an infinity
+    odd = r.standard_normal(64 * 40 * 36).astype(np.float32)
+    bits = odd.view(np.uint32)
+    where = r.random(odd.size)
+    bits[where < 0.55] = 0x7F800000                                          # +Inf: the median of most cells
+    bits[(where >= 0.55) & (where < 0.70)] = 0x7F800001 + r.integers(0, 1 << 20)   # signalling NaNs, same raw bucket
+    bits[(where >= 0.70) & (where < 0.75)] = 0xFF800123                      # their negative twins, beside -Inf
+    bits[(where >= 0.75) & (where < 0.77)] = 0xFF800000
+    vol3 = odd.reshape(36, 40, 64)
+    vol3[:12, :20, :32] = np.where(r.random((12, 20, 32)) < 0.6, np.float32(-np.inf), np.float32(np.nan))   # median -Inf
+    assert np.isnan(odd).sum() > 1000
+    for p3 in ((32, 20, 12), (64, 40, 36), (8, 8, 8)):
+        got = run_minimap_median(ctx, dev(odd), dims, p3)
+        assert same_bits_map(got, oracle.minimap_median(odd, dims, p3))
+        if p3 == (32, 20, 12):
+            assert np.isposinf(got).sum() >= 4 and np.isneginf(got[0, 0, 0])
     for name, d3 in (("c3", (64, 64, 90)), ("c4", (96, 64, 30))):
         t, b, _ = scaled_cube(name, d3)
         for p3 in ((30, 30, 30), (8, 8, 8)):
