@@ -1,12 +1,16 @@
 // cube_minimap_median.cuh -- per-cell lower median of the statistical mini-map (SURVEY.md sec. 8(f) NEXT-2 "mean/std
 // (then median) per user partition"; "each data point represents the data statistics of a bigger region").
 //
-// The exact selection of cube_select.cuh, segmented: one GROUP of threads (a CTA of 512 for cells of >= 1024 voxels,
-// a warp otherwise) owns one cell at a time, reads its px x py x pz voxels ONCE (4 B per voxel, rows of px voxels),
-// keeps their order-preserving keys in shared memory (a 30^3 cell is 27000 keys = 105 KiB; NULL voxels become the key
-// 0xFFFFFFFF, above every value, and are counted) and fixes the key of rank k = (count - 1) / 2 with four 8-bit digit
-// histograms over the staged keys -- no second read of the cube.  Cells too large for shared memory (more than
-// kMedStageKeys voxels) are re-read from global memory for each digit instead (L2 / HBM: 16 B per voxel).
+// The exact selection of cube_select.cuh, segmented: one group of threads owns one cell at a time.
+//   * cells of >= 1024 voxels, default: minimap_median_two_reads_kernel -- a CTA of 256 threads reads the cell from
+//     HBM counting an 11-bit first digit, reads it again from L2 keeping the median bucket's voxels in shared memory,
+//     and fixes the other 21 bits on those (8 B per voxel through the SM, 4 B from HBM when the cell's lines stay in
+//     L2; 24 KiB of shared memory whatever the cell size);
+//   * CUBE_KNOB_MAPMEDIAN = 1 (and cells whose offsets do not fit 32 bits): minimap_median_cta_kernel -- 512 threads
+//     read the cell ONCE and keep all its keys in shared memory (a 30^3 cell is 105 KiB; NULL voxels become the key
+//     0xFFFFFFFF, above every value), four 8-bit digit histograms over the staged keys; cells of more than
+//     kMedStageKeys voxels are re-read from global memory for each digit instead;
+//   * cells below 1024 voxels: minimap_median_warp_kernel, one warp per cell, keys staged in shared memory.
 // The paper's Alg. 1 would take ~31 passes per cell.
 #pragma once
 #include <type_traits>
@@ -132,8 +136,35 @@ constexpr int kMedInFlight = CUBE_MED_INFLIGHT;
 // load with a second row, a 16-voxel row with three more.  What a load costs in address arithmetic (the division of
 // the row number by the cell's height is a multiplication by c.magic, exact while r * h < 2^32; the byte offset three
 // IMADs; base + 32-bit offset) is spent once per load, hence the packing.
-template <int GROUP, int VEC, class F>
+// L2 eviction hints of the two reads: the lines of a cell are wanted again (read 2) by the same CTA a few
+// microseconds later and never after that.  Load POLICY 0: plain read-only loads; 1: evict_last; 2: evict_first.
+// CUBE_MED_POLICY 1 (default): read 2 marks its lines evict_first (their last use); 2: read 1 evict_last as well
+// (measured: 1.58 vs 1.62 ms without hints on c2 30^3; the two settings tie).
+#ifndef CUBE_MED_POLICY
+#define CUBE_MED_POLICY 1
+#endif
+template <int POLICY> __device__ __forceinline__ uint64_t med_policy() {
+    uint64_t p = 0;
+    if (POLICY == 1) asm("createpolicy.fractional.L2::evict_last.b64 %0, 1.0;" : "=l"(p));
+    if (POLICY == 2) asm("createpolicy.fractional.L2::evict_first.b64 %0, 1.0;" : "=l"(p));
+    return p;
+}
+template <int POLICY> __device__ __forceinline__ float med_ld(const float* p, uint64_t pol) {
+    if (POLICY == 0) return __ldg(p);
+    float v;
+    asm volatile("ld.global.nc.L2::cache_hint.f32 %0, [%1], %2;" : "=f"(v) : "l"(p), "l"(pol));
+    return v;
+}
+template <int POLICY> __device__ __forceinline__ float2 med_ld(const float2* p, uint64_t pol) {
+    if (POLICY == 0) return __ldg(p);
+    float2 v;
+    asm volatile("ld.global.nc.L2::cache_hint.v2.f32 {%0, %1}, [%2], %3;" : "=f"(v.x), "=f"(v.y) : "l"(p), "l"(pol));
+    return v;
+}
+
+template <int GROUP, int VEC, int POLICY, class F>
 __device__ __forceinline__ void med_for_each_voxel_v(const MedCell& c, int tid, F&& fn) {
+    const uint64_t pol = med_policy<POLICY>();
     constexpr int NW = GROUP / 32, U = kMedInFlight;
     const int lane = tid & 31, wid = tid >> 5;
     const int lpr_log = VEC == 2 ? c.lpr_log2 : c.lpr_log1, rpw_log = 5 - lpr_log;
@@ -160,10 +191,10 @@ __device__ __forceinline__ void med_for_each_voxel_v(const MedCell& c, int tid, 
 #pragma unroll
                     for (int u = 0; u < U; ++u) {
                         if (VEC == 2) {
-                            const float2 t = __ldg(reinterpret_cast<const float2*>(q + o[u]));
+                            const float2 t = med_ld<POLICY>(reinterpret_cast<const float2*>(q + o[u]), pol);
                             a[u] = t.x; b[u] = t.y;
                         } else {
-                            a[u] = __ldg(reinterpret_cast<const float*>(q + o[u]));
+                            a[u] = med_ld<POLICY>(reinterpret_cast<const float*>(q + o[u]), pol);
                         }
                     }
 #pragma unroll
@@ -173,10 +204,10 @@ __device__ __forceinline__ void med_for_each_voxel_v(const MedCell& c, int tid, 
                     for (int u = 0; u < U; ++u) {
                         if (rw + sub + (uint32_t)u * rstep < rows) {
                             if (VEC == 2) {
-                                const float2 t = __ldg(reinterpret_cast<const float2*>(q + o[u]));
+                                const float2 t = med_ld<POLICY>(reinterpret_cast<const float2*>(q + o[u]), pol);
                                 fn(t.x); fn(t.y);
                             } else {
-                                fn(__ldg(reinterpret_cast<const float*>(q + o[u])));
+                                fn(med_ld<POLICY>(reinterpret_cast<const float*>(q + o[u]), pol));
                             }
                         }
                     }
@@ -186,10 +217,10 @@ __device__ __forceinline__ void med_for_each_voxel_v(const MedCell& c, int tid, 
     }
 }
 
-template <int GROUP, class F>
+template <int GROUP, int POLICY = 0, class F>
 __device__ __forceinline__ void med_for_each_voxel(const MedCell& c, int tid, F&& fn) {
-    if (c.lpr_log2 >= 0) med_for_each_voxel_v<GROUP, 2>(c, tid, fn);        // uniform over the CTA
-    else med_for_each_voxel_v<GROUP, 1>(c, tid, fn);
+    if (c.lpr_log2 >= 0) med_for_each_voxel_v<GROUP, 2, POLICY>(c, tid, fn);        // uniform over the CTA
+    else med_for_each_voxel_v<GROUP, 1, POLICY>(c, tid, fn);
 }
 
 // Two-read selection of one cell by one CTA (cells of any size).
@@ -267,7 +298,7 @@ __device__ __forceinline__ float med_cell_two_reads(const MedCell& c, uint32_t* 
     // buckets 0x3FD-0x3FF / 0x7FD-0x7FF hold nothing but NaN patterns and are dropped when the buckets are scanned;
     // 0x3FC / 0x7FC hold +-Inf AND the NaN patterns with a payload below 2^21: a cell with anything in those two is
     // counted again with the NULL test per voxel (rare: cells holding infinities).
-    med_for_each_voxel<GROUP>(c, tid, [&](float v) {
+    med_for_each_voxel<GROUP, (CUBE_MED_POLICY >= 2 ? 1 : 0)>(c, tid, [&](float v) {
         const uint32_t a = hist_s + (__float_as_uint(v) >> 21) * 4u;
         asm volatile("red.shared.add.u32 [%0], 1;" ::"r"(a) : "memory");
     });
@@ -303,7 +334,7 @@ __device__ __forceinline__ float med_cell_two_reads(const MedCell& c, uint32_t* 
     if (c0 <= (uint32_t)kMed2Cand) {
         // read 2: the voxels of the bucket (bits - rawbase < 2^21; a NULL voxel can only pass in a `careful` cell)
         if (!careful) {
-            med_for_each_voxel<GROUP>(c, tid, [&](float v) {
+            med_for_each_voxel<GROUP, (CUBE_MED_POLICY >= 1 ? 2 : 0)>(c, tid, [&](float v) {
                 const uint32_t bits = __float_as_uint(v);
                 if (bits - rawbase < 0x200000u) {
                     uint32_t pos;
