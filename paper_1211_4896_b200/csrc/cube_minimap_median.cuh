@@ -233,27 +233,39 @@ __device__ __forceinline__ void med_for_each_voxel(const MedCell& c, int tid, F&
 //       remaining 11 + 10 key bits are fixed on those.
 // A bucket that does not fit kMed2Cand keys (constant cells, heavy ties) has its digits counted by further reads of
 // the cell instead.  24.1 KiB of shared memory per CTA whatever the cell size.
-constexpr int kMed2Threads = 256;
+#ifndef CUBE_MED2_THREADS
+#define CUBE_MED2_THREADS 256
+#endif
+constexpr int kMed2Threads = CUBE_MED2_THREADS;
 constexpr int kMed2Bins = 2048;
+constexpr int kMed2Per = kMed2Bins / kMed2Threads;            // buckets a thread scans
 constexpr int kMed2Cand = 4096;
-constexpr int kMed2Smem = (kMed2Bins + kMed2Cand + 16) * 4;
+constexpr int kMed2Smem = (kMed2Bins + kMed2Cand + 32) * 4;
+static_assert(kMed2Per >= 4 && kMed2Per % 4 == 0 && kMed2Threads % 64 == 0, "four +-Inf / NaN buckets per end thread");
 
-// counts of key-order buckets 8 * tid .. 8 * tid + 7 from the raw-order histogram (256 threads)
-__device__ __forceinline__ void med_load_raw_order(const uint32_t* hist, int tid, uint32_t (&c)[8]) {
-    const bool neg = tid < 128;
-    const int base = neg ? 2040 - 8 * tid : 8 * tid - 1024;
-    const uint4 a = *reinterpret_cast<const uint4*>(hist + base), b = *reinterpret_cast<const uint4*>(hist + base + 4);
-    const uint32_t r[8] = {a.x, a.y, a.z, a.w, b.x, b.y, b.z, b.w};
+// counts of key-order buckets PER * tid .. PER * tid + PER - 1 from the raw-order histogram
+__device__ __forceinline__ void med_load_raw_order(const uint32_t* hist, int tid, uint32_t (&c)[kMed2Per]) {
+    constexpr int PER = kMed2Per;
+    const bool neg = tid < kMed2Threads / 2;
+    const int base = neg ? kMed2Bins - PER * (tid + 1) : PER * tid - kMed2Bins / 2;
+    uint32_t r[PER];
 #pragma unroll
-    for (int j = 0; j < 8; ++j) c[j] = neg ? r[7 - j] : r[j];
+    for (int j = 0; j < PER; j += 4) {
+        const uint4 a = *reinterpret_cast<const uint4*>(hist + base + j);
+        r[j] = a.x; r[j + 1] = a.y; r[j + 2] = a.z; r[j + 3] = a.w;
+    }
+#pragma unroll
+    for (int j = 0; j < PER; ++j) c[j] = neg ? r[PER - 1 - j] : r[j];
 }
 
-// as med_locate, on bucket counts already in registers (256 threads, 8 buckets each, bucket index = 8 * tid + j)
-__device__ __forceinline__ void med_locate_regs(const uint32_t (&c)[8], uint32_t k, uint32_t* red, int tid, uint32_t& bin,
+// as med_locate, on bucket counts already in registers (bucket index = PER * tid + j); k = 0xFFFFFFFF: the lower
+// median of what was counted.  red[0..2] = bucket, rank inside it, its count.
+__device__ __forceinline__ void med_locate_regs(const uint32_t (&c)[kMed2Per], uint32_t k, uint32_t* red, int tid, uint32_t& bin,
                                                 uint32_t& krem, uint32_t& total) {
+    constexpr int PER = kMed2Per, NWARP = kMed2Threads / 32;
     uint32_t mine = 0;
 #pragma unroll
-    for (int j = 0; j < 8; ++j) mine += c[j];
+    for (int j = 0; j < PER; ++j) mine += c[j];
     uint32_t incl = mine;
     const int lane = tid & 31;
 #pragma unroll
@@ -262,19 +274,18 @@ __device__ __forceinline__ void med_locate_regs(const uint32_t (&c)[8], uint32_t
         if (lane >= off) incl += u;
     }
     __syncthreads();
-    if (lane == 31) red[tid >> 5] = incl;
+    if (lane == 31) red[12 + (tid >> 5)] = incl;
     __syncthreads();
     uint32_t before = 0, all = 0;
 #pragma unroll
-    for (int w = 0; w < 8; ++w) { const uint32_t t = red[w]; all += t; before += w < (tid >> 5) ? t : 0u; }
+    for (int w = 0; w < NWARP; ++w) { const uint32_t t = red[12 + w]; all += t; before += w < (tid >> 5) ? t : 0u; }
     total = all;
-    if (k == 0xFFFFFFFFu) k = all ? (all - 1) / 2 : 0;      // the lower median of what was counted
+    if (k == 0xFFFFFFFFu) k = all ? (all - 1) / 2 : 0;
     uint32_t excl = before + incl - mine;
-    __syncthreads();
     if (excl <= k && k < excl + mine) {                      // exactly one thread (none when all == 0)
 #pragma unroll
-        for (int j = 0; j < 8; ++j) {
-            if (c[j] && excl <= k && k < excl + c[j]) { red[0] = (uint32_t)(tid * 8 + j); red[1] = k - excl; red[2] = c[j]; }
+        for (int j = 0; j < PER; ++j) {
+            if (c[j] && excl <= k && k < excl + c[j]) { red[0] = (uint32_t)(tid * PER + j); red[1] = k - excl; red[2] = c[j]; }
             excl += c[j];
         }
     }
@@ -303,15 +314,16 @@ __device__ __forceinline__ float med_cell_two_reads(const MedCell& c, uint32_t* 
         asm volatile("red.shared.add.u32 [%0], 1;" ::"r"(a) : "memory");
     });
     __syncthreads();
-    uint32_t cnt[8], k, b0, b1, b2, count;
+    constexpr int PER = kMed2Per;
+    uint32_t cnt[PER], k, b0, b1, b2, count;
     auto load_counts = [&]() {
         med_load_raw_order(hist, tid, cnt);
         if (tid == 0) cnt[0] = cnt[1] = cnt[2] = 0;            // key-order buckets 0-2 and 2045-2047: NaN patterns only
-        if (tid == GROUP - 1) cnt[5] = cnt[6] = cnt[7] = 0;
+        if (tid == GROUP - 1) cnt[PER - 3] = cnt[PER - 2] = cnt[PER - 1] = 0;
     };
     load_counts();
     if (tid == 0) red[9] = cnt[3];                             // -Inf and negative NaNs of small payload
-    if (tid == GROUP - 1) red[10] = cnt[4];                    // +Inf and positive NaNs of small payload
+    if (tid == GROUP - 1) red[10] = cnt[PER - 4];              // +Inf and positive NaNs of small payload
     __syncthreads();
     const bool careful = (red[9] | red[10]) != 0;              // uniform over the CTA
     if (careful) {
@@ -357,7 +369,7 @@ __device__ __forceinline__ float med_cell_two_reads(const MedCell& c, uint32_t* 
         CUBE_CHECK(red[8] == c0);
         for (uint32_t i = tid; i < c0; i += GROUP) atomicAdd(&hist[(key_of(__uint_as_float(cand[i])) >> 10) & 2047u], 1u);
         __syncthreads();
-        med_locate<GROUP, kMed2Bins>(hist, k, red, tid, b1, k);
+        med_locate<GROUP, kMed2Bins>(hist, k, red + 12, tid, b1, k);
         __syncthreads();
         zero_hist();
         __syncthreads();
@@ -371,7 +383,7 @@ __device__ __forceinline__ float med_cell_two_reads(const MedCell& c, uint32_t* 
             if ((key >> 21) == b0 && v == v) atomicAdd(&hist[(key >> 10) & 2047u], 1u);
         });
         __syncthreads();
-        med_locate<GROUP, kMed2Bins>(hist, k, red, tid, b1, k);
+        med_locate<GROUP, kMed2Bins>(hist, k, red + 12, tid, b1, k);
         __syncthreads();
         zero_hist();
         __syncthreads();
@@ -382,7 +394,7 @@ __device__ __forceinline__ float med_cell_two_reads(const MedCell& c, uint32_t* 
         });
     }
     __syncthreads();
-    med_locate<GROUP, kMed2Bins>(hist, k, red, tid, b2, k);
+    med_locate<GROUP, kMed2Bins>(hist, k, red + 12, tid, b2, k);
     return __uint_as_float(bits_of_key((b0 << 21) | (b1 << 10) | b2));
 }
 
