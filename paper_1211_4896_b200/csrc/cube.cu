@@ -398,7 +398,7 @@ int cube_create(cube_ctx** out, size_t scratch_bytes_hint) {
     ok = ok && cudaMemset(c->bar, 0, sizeof(unsigned int)) == cudaSuccess;
     c->coop = prop.cooperativeLaunch ? 1 : 0;
 #ifdef CUBE_SMALL_TIMING
-    ok = ok && cudaMallocManaged(&c->small_tstamp, 16 * sizeof(unsigned long long)) == cudaSuccess;
+    ok = ok && cudaMallocManaged(&c->small_tstamp, (16 + 8 * 4096) * sizeof(unsigned long long)) == cudaSuccess;
     if (getenv("CUBE_SMALL_TSTAMP_PTR")) { FILE* fp = fopen(getenv("CUBE_SMALL_TSTAMP_PTR"), "w"); if (fp) { fprintf(fp, "%llu\n", (unsigned long long)(uintptr_t)c->small_tstamp); fclose(fp); } }
 #endif
     ok = ok && cudaFuncSetAttribute(stats_small_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize,

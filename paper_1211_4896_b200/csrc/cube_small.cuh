@@ -119,8 +119,11 @@ __device__ __forceinline__ void small_locate0(SelectState* st, const unsigned lo
 
 #ifdef CUBE_SMALL_TIMING
 #define SMALL_T(i) do { if (a.tstamp && blockIdx.x == 0 && threadIdx.x == 0) { unsigned long long t_; asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t_)); a.tstamp[i] = t_; } } while (0)
+// per-CTA stamps (slot i < 8 of CTA b at tstamp[16 + 8 b + i])
+#define SMALL_TC(i) do { if (a.tstamp && threadIdx.x == 0) { unsigned long long t_; asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t_)); a.tstamp[16 + 8 * blockIdx.x + (i)] = t_; } } while (0)
 #else
 #define SMALL_T(i) do { } while (0)
+#define SMALL_TC(i) do { } while (0)
 #endif
 
 __global__ void __launch_bounds__(kThreads, 3)
@@ -135,6 +138,7 @@ stats_small_kernel(SmallArgs a) {
     const unsigned gtid = blockIdx.x * kThreads + threadIdx.x, gthreads = grid * kThreads;
 
     SMALL_T(0);
+    SMALL_TC(0);
     // ---- phase 0 (no barrier): what phase B accumulates into is zeroed now -- two grid barriers lie in between; the
     // first-digit bins and the chunk totals arrive zeroed (every call leaves the next call's arrays that way)
     for (unsigned i = gtid; i < (unsigned)a.nbins + 2u; i += gthreads) a.gout[i] = 0ull;
@@ -146,8 +150,10 @@ stats_small_kernel(SmallArgs a) {
         f.sbins = smem_addr(dyn_bins);
         for (int i = threadIdx.x; i <= kDigitBins; i += kThreads) dyn_bins[i] = 0;
         __syncthreads();
+        SMALL_TC(1);
         stream_cube<kThreads>(a.d, a.n, f);
         SMALL_T(2);
+        SMALL_TC(2);
         f.unsubstitute();
         const Partial p = partial_block_reduce(f.partial(), scratch);
         __syncthreads();
@@ -162,7 +168,9 @@ stats_small_kernel(SmallArgs a) {
         }
         if (threadIdx.x == 0) a.partials[blockIdx.x] = p;
     }
+    SMALL_TC(3);
     small_grid_sync(a.bar, a.bar_base + grid);
+    SMALL_TC(4);
 
     SMALL_T(3);
     // ---- every CTA for itself: the merged moments record and the first-digit bucket
@@ -205,6 +213,7 @@ stats_small_kernel(SmallArgs a) {
         }
         __syncthreads();
         SMALL_T(5);
+        SMALL_TC(5);
         hist_flush_bins(hbins, a.nbins, a.gout + 2);
         for (int i = threadIdx.x; i < kBins1; i += kThreads) {
             const uint32_t c = sbins[i];
@@ -219,7 +228,9 @@ stats_small_kernel(SmallArgs a) {
             a.gout[threadIdx.x] = ~0ull;  // marker: the [min,max] range was unusable
         }
     }
+    SMALL_TC(6);
     small_grid_sync(a.bar, a.bar_base + 2 * grid);
+    SMALL_TC(7);
 
     SMALL_T(6);
     // ---- last digit
