@@ -33,6 +33,7 @@ struct cube_ctx {
     unsigned int bar_base = 0;
     unsigned long long* coarse_next = nullptr;   // all zero: the first-digit array the next single-launch cube_stats takes
     unsigned long long* chunk_tot = nullptr;     // kDigitBins / 32 chunk totals, all zero between calls
+    unsigned int* small_ext = nullptr;           // stats_small_kernel: {min key, max key, ticket} = {~0, 0, 0} between calls
     unsigned long long* small_tstamp = nullptr;   // debug builds only (-DCUBE_SMALL_TIMING)
     int minimap_variant = 0;  // CUBE_KNOB_MINIMAP: 0 = automatic, 1 = no TMA ring, 2 = scalar kernel only, 3 = TMA ring whenever eligible
     int last_cuda = 0;
@@ -394,6 +395,11 @@ int cube_create(cube_ctx** out, size_t scratch_bytes_hint) {
     ok = ok && cudaMemset(c->coarse_next, 0, kDigitBins * sizeof(unsigned long long)) == cudaSuccess;
     ok = ok && cudaMalloc(&c->chunk_tot, (kDigitBins / 32) * sizeof(unsigned long long)) == cudaSuccess;
     ok = ok && cudaMemset(c->chunk_tot, 0, (kDigitBins / 32) * sizeof(unsigned long long)) == cudaSuccess;
+    {
+        const unsigned int ext0[4] = {0xFFFFFFFFu, 0u, 0u, 0u};
+        ok = ok && cudaMalloc(&c->small_ext, sizeof(ext0)) == cudaSuccess;
+        ok = ok && cudaMemcpy(c->small_ext, ext0, sizeof(ext0), cudaMemcpyHostToDevice) == cudaSuccess;
+    }
     ok = ok && cudaMalloc(&c->bar, sizeof(unsigned int)) == cudaSuccess;
     ok = ok && cudaMemset(c->bar, 0, sizeof(unsigned int)) == cudaSuccess;
     c->coop = prop.cooperativeLaunch ? 1 : 0;
@@ -439,7 +445,7 @@ int cube_destroy(cube_ctx* c) {
     cudaFree(c->partials); cudaFree(c->ticket); cudaFree(c->ticket2); cudaFree(c->acc);
     cudaFree(c->mom_out); cudaFree(c->gout); cudaFree(c->gdigits); cudaFree(c->coarse); cudaFree(c->sel); cudaFree(c->multi);
     cudaFree(c->range3); cudaFree(c->probe_out); cudaFree(c->plan); cudaFree(c->clip); cudaFree(c->torben); cudaFree(c->center);
-    cudaFree(c->cand); cudaFree(c->tf_table); cudaFree(c->bar); cudaFree(c->coarse_next); cudaFree(c->chunk_tot);
+    cudaFree(c->cand); cudaFree(c->tf_table); cudaFree(c->bar); cudaFree(c->coarse_next); cudaFree(c->chunk_tot); cudaFree(c->small_ext);
     cudaFree(c->resident); cudaFree(c->chunk[0]); cudaFree(c->chunk[1]);
     if (c->pinned_results) cudaFreeHost(c->pinned_results);
     for (int i = 0; i < cube_ctx::kMaxStage; ++i) {
@@ -607,7 +613,7 @@ int cube_stats(cube_ctx* c, const float* d, int64_t nx, int64_t ny, int64_t nz, 
             a.coarse = c->coarse_next; a.coarse_next = c->coarse; a.chunk_tot = c->chunk_tot;   // the zeroed array becomes the current one
             a.gdigits = c->gdigits; a.gout = c->gout;
             a.sel = c->sel; a.cand = c->cand; a.cand_cap = c->cand ? c->cand_cap : 0; a.result_out = med_direct;
-            a.bar = c->bar; a.bar_base = c->bar_base; a.tstamp = c->small_tstamp;
+            a.bar = c->bar; a.bar_base = c->bar_base; a.ext = c->small_ext; a.tstamp = c->small_tstamp;
             a.bins_user = static_cast<unsigned long long*>(device_reachable(c, bins));
             a.outside_user = static_cast<unsigned long long*>(device_reachable(c, outside));
             if (!a.bins_user || !a.outside_user) a.bins_user = a.outside_user = nullptr;

@@ -35,6 +35,7 @@ struct SmallArgs {
     unsigned long long* bins_user;   // the caller's bins / outside when the device can reach them (no copy is enqueued then)
     unsigned long long* outside_user;
     unsigned int* bar; unsigned int bar_base;
+    unsigned int* ext;               // [0] = smallest key seen (0xFFFFFFFF between calls), [1] = largest (0), [2] = ticket (0)
     unsigned long long* tstamp;      // debug (-DCUBE_SMALL_TIMING): %globaltimer of CTA 0 at the phase boundaries
 };
 
@@ -53,6 +54,17 @@ __device__ __forceinline__ void small_grid_sync(unsigned int* bar, unsigned int 
     if (threadIdx.x == 0) {
         __threadfence();
         atomicAdd(bar, 1u);
+        unsigned int v;
+        do {
+            asm volatile("ld.acquire.gpu.global.u32 %0, [%1];" : "=r"(v) : "l"(bar) : "memory");
+        } while ((int)(v - target) < 0);
+        __threadfence();
+    }
+    __syncthreads();
+}
+// The two halves of small_grid_sync, for work that can be done between arriving and being released.
+__device__ __forceinline__ void small_grid_wait(unsigned int* bar, unsigned int target) {
+    if (threadIdx.x == 0) {
         unsigned int v;
         do {
             asm volatile("ld.acquire.gpu.global.u32 %0, [%1];" : "=r"(v) : "l"(bar) : "memory");
@@ -134,6 +146,9 @@ stats_small_kernel(SmallArgs a) {
     __shared__ unsigned long long scan_sm[kScanSmem];
     __shared__ MomentsOut s_mom;
     __shared__ uint32_t s_out[2];
+    __shared__ uint32_t s_ext[2];
+    __shared__ int s_last;
+    __shared__ Partial parked[kThreads];          // the threads' moments of phase A, reduced while waiting at barrier B
     const unsigned grid = gridDim.x;
     const unsigned gtid = blockIdx.x * kThreads + threadIdx.x, gthreads = grid * kThreads;
 
@@ -149,14 +164,25 @@ stats_small_kernel(SmallArgs a) {
         MomentsF<kMomCoarse> f;
         f.sbins = smem_addr(dyn_bins);
         for (int i = threadIdx.x; i <= kDigitBins; i += kThreads) dyn_bins[i] = 0;
+        if (threadIdx.x == 0) { s_ext[0] = 0xFFFFFFFFu; s_ext[1] = 0u; }
         __syncthreads();
         SMALL_TC(1);
         stream_cube<kThreads>(a.d, a.n, f);
         SMALL_T(2);
         SMALL_TC(2);
         f.unsubstitute();
-        const Partial p = partial_block_reduce(f.partial(), scratch);
+        // Only the extrema are wanted before phase B (the [min, max] histogram range): they go to two global words by
+        // atomics.  The threads' (n, mean, M2) are parked; their reduction over the CTA and the merge over the grid --
+        // chains of dependent fp64 operations and L2 round trips -- leave the critical path: each CTA reduces its own
+        // while it waits at barrier B, and the CTA that finishes last merges them all, beside CTA 0's last digit.
+        {
+            const Partial mine = f.partial();
+            parked[threadIdx.x] = mine;
+            const uint32_t wmin = __reduce_min_sync(0xffffffffu, mine.kmin), wmax = __reduce_max_sync(0xffffffffu, mine.kmax);
+            if ((threadIdx.x & 31) == 0) { atomicMin(&s_ext[0], wmin); atomicMax(&s_ext[1], wmax); }
+        }
         __syncthreads();
+        if (threadIdx.x == 0) { atomicMin(&a.ext[0], s_ext[0]); atomicMax(&a.ext[1], s_ext[1]); }
         // flush: a warp takes chunks of 32 consecutive raw digits; their sum also goes to the chunk's total (a chunk of
         // raw digits IS a chunk of key-order digits: raw chunk r <-> key chunk r + 128 (positive) or 255 - r (negative))
         for (int ch = threadIdx.x >> 5; ch < kDigitBins / 32; ch += kThreads / 32) {
@@ -166,24 +192,21 @@ stats_small_kernel(SmallArgs a) {
             if ((threadIdx.x & 31) == 0 && tot)
                 atomicAdd(&a.chunk_tot[ch < 128 ? ch + 128 : 255 - ch], (unsigned long long)tot);
         }
-        if (threadIdx.x == 0) a.partials[blockIdx.x] = p;
     }
     SMALL_TC(3);
     small_grid_sync(a.bar, a.bar_base + grid);
     SMALL_TC(4);
 
     SMALL_T(3);
-    // ---- every CTA for itself: the merged moments record and the first-digit bucket
+    // ---- every CTA for itself: the first-digit bucket (warp 0) and the extrema (warp 1)
     {
-        const Partial m = partials_merge_block(a.partials, grid, scratch);
-        if (threadIdx.x == 0) {
-            moments_finalize(m, a.n, a.flags, &s_mom);
-            if (blockIdx.x == 0) {
-                *a.acc = m; *a.nvox_acc = a.n; *a.mom_out = s_mom;
-                if (a.out_user) *a.out_user = s_mom;
-            }
-        }
         if (threadIdx.x < 32) small_locate0(&s_sel, a.coarse, a.chunk_tot, a.cand ? a.cand_cap : 0);
+        if (threadIdx.x == 32) {
+            s_mom.min = __uint_as_float(bits_of_key(__ldcg(&a.ext[0])));
+            s_mom.max = __uint_as_float(bits_of_key(__ldcg(&a.ext[1])));
+        }
+        __syncthreads();
+        if (threadIdx.x == 0) s_mom.count = s_sel.count;     // all that hist_range() looks at: count, min, max
         __syncthreads();
     }
 
@@ -229,7 +252,28 @@ stats_small_kernel(SmallArgs a) {
         }
     }
     SMALL_TC(6);
-    small_grid_sync(a.bar, a.bar_base + 2 * grid);
+    small_grid_arrive(a.bar);
+    {   // between arriving and being released: this CTA's moments, and -- for the CTA that is last -- the whole cube's
+        const Partial p = partial_block_reduce(parked[threadIdx.x], scratch);
+        if (threadIdx.x == 0) {
+            a.partials[blockIdx.x] = p;
+            __threadfence();
+            s_last = atomicAdd(&a.ext[2], 1u) == grid - 1u;
+        }
+        __syncthreads();
+        if (s_last) {
+            __threadfence();
+            const Partial m = partials_merge_block(a.partials, grid, scratch);
+            if (threadIdx.x == 0) {
+                MomentsOut o;
+                moments_finalize(m, a.n, a.flags, &o);
+                *a.acc = m; *a.nvox_acc = a.n; *a.mom_out = o;
+                if (a.out_user) *a.out_user = o;
+                a.ext[0] = 0xFFFFFFFFu; a.ext[1] = 0u; a.ext[2] = 0u;     // every CTA has read them: as the next call wants them
+            }
+        }
+    }
+    small_grid_wait(a.bar, a.bar_base + 2 * grid);
     SMALL_TC(7);
 
     SMALL_T(6);
