@@ -275,7 +275,8 @@ __device__ __forceinline__ unsigned long long warp_sum_u64(unsigned long long v)
 // does not depend on the counts (the rank asked for, the prefix so far) is loaded before the bins.
 template <int PASS, int THREADS>
 __device__ __forceinline__ void select_scan_body(SelectState* __restrict__ st, unsigned long long* __restrict__ gdigits,
-                                                 int clear, const SelectInit& init, unsigned long long* sm) {
+                                                 int clear, const SelectInit& init, unsigned long long* sm,
+                                                 const uint32_t* local_bins = nullptr) {
     constexpr int NB = (PASS == 0) ? kBins0 : (PASS == 1) ? kBins1 : kBins2;
     constexpr int BITS = (PASS == 0) ? kBits0 : (PASS == 1) ? kBits1 : kBits2;
     constexpr int CHUNKS = NB / 32, NW = THREADS / 32;
@@ -296,6 +297,7 @@ __device__ __forceinline__ void select_scan_body(SelectState* __restrict__ st, u
     const uint32_t prefix = (PASS == 0) ? 0u : st->prefix;
     const bool med = (PASS == 0) && (fresh ? init.use_median != 0 : st->use_median != 0);
     auto bin = [&](uint32_t b) -> unsigned long long {   // PASS 0 bins are indexed by the raw top bits of the float
+        if (local_bins) return (unsigned long long)local_bins[b];   // one CTA counted everything: its shared-memory counters
         return __ldcg(&gdigits[PASS == 0 ? raw_of_digit(b) : b]);
     };
     unsigned long long v[INFL];

@@ -185,12 +185,22 @@ stats_small_kernel(SmallArgs a) {
         if (threadIdx.x == 0) { atomicMin(&a.ext[0], s_ext[0]); atomicMax(&a.ext[1], s_ext[1]); }
         // flush: a warp takes chunks of 32 consecutive raw digits; their sum also goes to the chunk's total (a chunk of
         // raw digits IS a chunk of key-order digits: raw chunk r <-> key chunk r + 128 (positive) or 255 - r (negative))
-        for (int ch = threadIdx.x >> 5; ch < kDigitBins / 32; ch += kThreads / 32) {
-            const uint32_t c = dyn_bins[ch * 32 + (threadIdx.x & 31)];
-            if (c) atomicAdd(&a.coarse[ch * 32 + (threadIdx.x & 31)], (unsigned long long)c);
-            const uint32_t tot = __reduce_add_sync(0xffffffffu, c);
-            if ((threadIdx.x & 31) == 0 && tot)
-                atomicAdd(&a.chunk_tot[ch < 128 ? ch + 128 : 255 - ch], (unsigned long long)tot);
+        // (eight chunks per step: the loads and the warp sums of a step are independent, the loop is latency otherwise)
+        constexpr int NCH = kDigitBins / 32, WARPS = kThreads / 32, STEP = 8;
+        static_assert(NCH % (WARPS * STEP) == 0, "flush shape");
+        const int lane = threadIdx.x & 31;
+        for (int ch0 = threadIdx.x >> 5; ch0 < NCH; ch0 += WARPS * STEP) {
+            uint32_t c[STEP], tot[STEP];
+#pragma unroll
+            for (int u = 0; u < STEP; ++u) c[u] = dyn_bins[(ch0 + u * WARPS) * 32 + lane];
+#pragma unroll
+            for (int u = 0; u < STEP; ++u) tot[u] = __reduce_add_sync(0xffffffffu, c[u]);
+#pragma unroll
+            for (int u = 0; u < STEP; ++u) {
+                const int ch = ch0 + u * WARPS;
+                if (c[u]) atomicAdd(&a.coarse[ch * 32 + lane], (unsigned long long)c[u]);
+                if (lane == 0 && tot[u]) atomicAdd(&a.chunk_tot[ch < 128 ? ch + 128 : 255 - ch], (unsigned long long)tot[u]);
+            }
         }
     }
     SMALL_TC(3);
@@ -278,14 +288,19 @@ stats_small_kernel(SmallArgs a) {
 
     SMALL_T(6);
     // ---- last digit
-    unsigned long long cn;
-    asm volatile("ld.relaxed.gpu.global.u64 %0, [%1];" : "=l"(cn) : "l"(&a.sel->cand_n) : "memory");
-    const bool fits = a.cand != nullptr && cn <= a.cand_cap;   // the same on every CTA: cand_n is final
-    // the array the next call counts first digits into (nobody reads it in this call)
-    for (unsigned i = gtid; i < (unsigned)kDigitBins; i += gthreads) a.coarse_next[i] = 0ull;
-    if (a.bins_user) {   // the histogram is complete: straight into the caller's buffers
-        for (unsigned i = gtid; i < (unsigned)a.nbins; i += gthreads) a.bins_user[i] = __ldcg(&a.gout[2 + i]);
-        if (gtid < 2) a.outside_user[gtid] = __ldcg(&a.gout[gtid]);
+    const unsigned long long cn = __ldcg(&a.sel->cand_n);      // final: every CTA's appends precede its arrival
+    const bool fits = a.cand != nullptr && cn <= a.cand_cap;   // the same on every CTA
+    // housekeeping nobody waits for -- the array the next call counts first digits into (nobody reads it in this call)
+    // and the histogram, complete now, straight into the caller's buffers -- is left to the CTAs other than 0, whose
+    // chain of dependent round trips ends the call
+    if (grid == 1 || blockIdx.x != 0) {
+        const unsigned hthreads = (grid == 1 ? 1u : grid - 1u) * kThreads;
+        const unsigned htid = (grid == 1 ? 0u : blockIdx.x - 1u) * kThreads + threadIdx.x;
+        for (unsigned i = htid; i < (unsigned)kDigitBins; i += hthreads) a.coarse_next[i] = 0ull;
+        if (a.bins_user) {
+            for (unsigned i = htid; i < (unsigned)a.nbins; i += hthreads) a.bins_user[i] = __ldcg(&a.gout[2 + i]);
+            if (htid < 2) a.outside_user[htid] = __ldcg(&a.gout[htid]);
+        }
     }
     if (fits && blockIdx.x != 0) { small_grid_arrive(a.bar); return; }
     SelectInit none;
@@ -324,9 +339,11 @@ stats_small_kernel(SmallArgs a) {
             }
         }
         __syncthreads();
-        for (int i = threadIdx.x; i < kBins2; i += kThreads) {
-            const uint32_t c = sbins[i];
-            if (c) atomicAdd(&g2[i], (unsigned long long)c);
+        if (!fits) {
+            for (int i = threadIdx.x; i < kBins2; i += kThreads) {
+                const uint32_t c = sbins[i];
+                if (c) atomicAdd(&g2[i], (unsigned long long)c);
+            }
         }
     }
     if (!fits) {
@@ -337,10 +354,10 @@ stats_small_kernel(SmallArgs a) {
         __syncthreads();
     }
     SMALL_T(7);
-    // ---- CTA 0: the key is complete
+    // ---- CTA 0: the key is complete (candidates: CTA 0 alone counted them, its shared-memory counters are the counts)
     SelectInit fin = none;
     fin.result_out = a.result_out;
-    select_scan_body<2, kThreads>(&s_sel, g2, 0, fin, scan_sm);
+    select_scan_body<2, kThreads>(&s_sel, g2, 0, fin, scan_sm, fits ? dyn_bins : nullptr);
     __syncthreads();
     for (int i = threadIdx.x; i < kDigitBins; i += kThreads) a.gdigits[i] = 0ull;   // as the general path leaves them
     for (int i = threadIdx.x; i < kDigitBins / 32; i += kThreads) a.chunk_tot[i] = 0ull;
