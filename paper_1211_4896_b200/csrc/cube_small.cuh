@@ -58,7 +58,6 @@ __device__ __forceinline__ void small_grid_sync(unsigned int* bar, unsigned int 
         do {
             asm volatile("ld.acquire.gpu.global.u32 %0, [%1];" : "=r"(v) : "l"(bar) : "memory");
         } while ((int)(v - target) < 0);
-        __threadfence();
     }
     __syncthreads();
 }
@@ -68,8 +67,7 @@ __device__ __forceinline__ void small_grid_wait(unsigned int* bar, unsigned int 
         unsigned int v;
         do {
             asm volatile("ld.acquire.gpu.global.u32 %0, [%1];" : "=r"(v) : "l"(bar) : "memory");
-        } while ((int)(v - target) < 0);
-        __threadfence();
+        } while ((int)(v - target) < 0);      // the acquire load orders what follows (bar.sync carries it to the CTA)
     }
     __syncthreads();
 }
