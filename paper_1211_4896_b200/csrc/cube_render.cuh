@@ -101,6 +101,45 @@ __device__ __forceinline__ bool ray_sample(const float* __restrict__ d, const Re
     return sample_at(d, g, p, out);
 }
 
+// The same sample in two halves, so that the loads of several samples of a ray are in flight together (the march is
+// a chain of dependent L1 / L2 / HBM round trips otherwise: ncu showed 14 % of the issue slots used and 35 stalled
+// warps per issued instruction): tap_load issues the eight loads -- for a sample outside the cube from voxel 0, so
+// that they need no branch --, tap_value interpolates.  Same operations, same order, same bits as sample_at.
+// Samples of a ray fetched before the first is consumed.  MIP: 1 (the branch-free loads alone took c2 at yaw 30 deg
+// from 9.6 to 7.7 ms; larger groups cost occupancy and gain nothing: a sample is consumed by one compare).  Transfer
+// functions: 6 (each sample ends in a dependent table load and five dependent float operations: 8.0 -> 5.2 ms at
+// 128 registers per thread).
+#ifndef CUBE_RENDER_GROUP_MIP
+#define CUBE_RENDER_GROUP_MIP 1
+#endif
+#ifndef CUBE_RENDER_GROUP_TF
+#define CUBE_RENDER_GROUP_TF 6
+#endif
+
+struct Tap {
+    float v[8];
+    float fx, fy, fz;
+    bool in;
+};
+
+__device__ __forceinline__ void tap_load(const float* __restrict__ d, const RenderGeom& g, const float (&pt)[3], bool wanted, Tap& t) {
+    t.in = wanted && pt[0] >= 0.0f && pt[0] <= g.xmax && pt[1] >= 0.0f && pt[1] <= g.ymax && pt[2] >= 0.0f && pt[2] <= g.zmax;
+    const float px = t.in ? pt[0] : 0.0f, py = t.in ? pt[1] : 0.0f, pz = t.in ? pt[2] : 0.0f;
+    const float flx = floorf(px), fly = floorf(py), flz = floorf(pz);
+    t.fx = __fsub_rn(px, flx); t.fy = __fsub_rn(py, fly); t.fz = __fsub_rn(pz, flz);
+    const long long x0 = (long long)flx, y0 = (long long)fly, z0 = (long long)flz;
+    const long long dx = t.fx > 0.0f ? 1 : 0, dy = t.fy > 0.0f ? g.nx : 0, dz = t.fz > 0.0f ? g.nx * g.ny : 0;
+    const float* __restrict__ p = d + ((z0 * g.ny + y0) * g.nx + x0);
+    t.v[0] = __ldg(p); t.v[1] = __ldg(p + dx); t.v[2] = __ldg(p + dy); t.v[3] = __ldg(p + dy + dx);
+    t.v[4] = __ldg(p + dz); t.v[5] = __ldg(p + dz + dx); t.v[6] = __ldg(p + dz + dy); t.v[7] = __ldg(p + dz + dy + dx);
+}
+
+__device__ __forceinline__ float tap_value(const Tap& t) {
+    const float c00 = lerp_rn(t.v[0], t.v[1], t.fx), c10 = lerp_rn(t.v[2], t.v[3], t.fx);
+    const float c01 = lerp_rn(t.v[4], t.v[5], t.fx), c11 = lerp_rn(t.v[6], t.v[7], t.fx);
+    return lerp_rn(lerp_rn(c00, c10, t.fy), lerp_rn(c01, c11, t.fy), t.fz);
+}
+
 // The statistical mini-map as the second lookup of the sigma-clipping transfer function (R34): cell
 // (cx, cy, cz) sits at the centre of its nominal block, data coordinate cx * px + (px - 1) / 2.
 struct MapLookupGeom {
@@ -150,12 +189,20 @@ render_mip_kernel(const float* __restrict__ d, RenderGeom g, RenderView vw, floa
     const RayF r = ray_setup(vw, g, u, v);
     float m = 0.0f;
     bool have = false;
-#pragma unroll 4
-    for (int i = r.i0; i <= r.i1; ++i) {
-        float s;
-        if (!ray_sample(d, g, vw, r.o, i, s)) continue;
-        if (!(s >= vmin)) continue;          // NULL samples fail the comparison
-        if (!have || s > m) { m = s; have = true; }
+#pragma unroll 1
+    for (int i = r.i0; i <= r.i1; i += CUBE_RENDER_GROUP_MIP) {
+        Tap t[CUBE_RENDER_GROUP_MIP];
+#pragma unroll
+        for (int j = 0; j < CUBE_RENDER_GROUP_MIP; ++j) {
+            float p[3];
+            ray_point(vw, r.o, i + j, p);
+            tap_load(d, g, p, i + j <= r.i1, t[j]);
+        }
+#pragma unroll
+        for (int j = 0; j < CUBE_RENDER_GROUP_MIP; ++j) {
+            const float s = tap_value(t[j]);
+            if (t[j].in && s >= vmin && (!have || s > m)) { m = s; have = true; }   // NULL samples fail the comparison
+        }
     }
     image[(size_t)v * vw.width + u] = have ? m : __int_as_float(0x7fc00000);
 }
@@ -176,10 +223,21 @@ render_tf_kernel(const float* __restrict__ d, RenderGeom g, RenderView vw, int n
     const RayF r = ray_setup(vw, g, u, v);
     float cr = 0.0f, cg = 0.0f, cb = 0.0f, A = 0.0f;
     const float top = (float)(nlevels - 1);
-    for (int i = r.i0; i <= r.i1; ++i) {
-        float s, p[3];
-        ray_point(vw, r.o, i, p);
-        if (!sample_at(d, g, p, s)) continue;
+    bool done = false;
+#pragma unroll 1
+    for (int i0 = r.i0; i0 <= r.i1 && !done; i0 += CUBE_RENDER_GROUP_TF) {
+      Tap t[CUBE_RENDER_GROUP_TF];
+      float pts[CUBE_RENDER_GROUP_TF][3];
+#pragma unroll
+      for (int j = 0; j < CUBE_RENDER_GROUP_TF; ++j) {
+          ray_point(vw, r.o, i0 + j, pts[j]);
+          tap_load(d, g, pts[j], i0 + j <= r.i1, t[j]);
+      }
+#pragma unroll
+      for (int j = 0; j < CUBE_RENDER_GROUP_TF; ++j) {
+        if (done || !t[j].in) continue;
+        float s = tap_value(t[j]);
+        const float (&p)[3] = pts[j];
         if (SIGMA) {
             if (s != s) continue;            // NULL sample: no need to look at the map
             float mean, sd;
@@ -196,7 +254,8 @@ render_tf_kernel(const float* __restrict__ d, RenderGeom g, RenderView vw, int n
         cg = __fadd_rn(cg, __fmul_rn(w, e.y));
         cb = __fadd_rn(cb, __fmul_rn(w, e.z));
         A = __fadd_rn(A, w);
-        if (A >= opacity_cut) break;
+        if (A >= opacity_cut) done = true;
+      }
     }
     rgba[(size_t)v * vw.width + u] = make_float4(cr, cg, cb, A);
 }
