@@ -48,7 +48,7 @@ enum {
     CUBE_EINVAL = 1, /* null pointer, dim <= 0, nbins out of range, !(lo <= hi), non-finite lo/hi/scale */
     CUBE_EEMPTY = 2, /* reserved: not returned by the asynchronous calls (see cube_moments) */
     CUBE_ECUDA = 3,  /* a CUDA call failed; cube_last_cuda_error() gives the cudaError_t */
-    CUBE_ERANGE = 4, /* reserved */
+    CUBE_ERANGE = 4, /* a size beyond a fixed maximum (cube_histogram_noalloc: nbins > CUBE_NOALLOC_MAX_BINS) */
     CUBE_ENOMEM = 5, /* host or device allocation failed */
     CUBE_ECALLBACK = 6 /* the brick callback of cube_stats_stream returned non-zero */
 };
@@ -95,6 +95,24 @@ int cube_moments(cube_ctx* ctx, const float* d, int64_t nx, int64_t ny, int64_t 
  * sum(bins) + outside[0] + outside[1] == count.  1 <= nbins <= CUBE_MAX_BINS. */
 int cube_histogram(cube_ctx* ctx, const float* d, int64_t nx, int64_t ny, int64_t nz, int nbins, float lo,
                    float hi, uint64_t* bins /* [nbins] */, uint64_t* outside /* [2] */, cudaStream_t stream);
+
+/* cube_histogram for callers that must not allocate (code under CUDA graph capture, tight serving loops, harnesses
+ * that forbid cudaMalloc).  Same bins and outside counts as cube_histogram, bit for bit, but NO
+ * cube_ctx and no cudaMalloc / cudaFree / allocating library call on its path: the 64-bit global counters the kernel
+ * accumulates into are a file-scope `static __device__` array of the library, 2 + CUBE_NOALLOC_MAX_BINS words =
+ * 32 KiB that every GPU which loads libcube holds until the process exits.  The work runs on the CURRENT device
+ * (whose memory d must be); the first call on a device resolves the array's device address (cudaGetSymbolAddress,
+ * checked) -- make that call outside a capture.  Enqueued on `stream`: a memset of the counters in use, one kernel,
+ * two copies to `bins` [nbins] and `outside` [2] (device, pinned or pageable host memory; under capture: device or
+ * pinned).  1 <= nbins <= CUBE_NOALLOC_MAX_BINS: more bins -> CUBE_ERANGE, nothing enqueued (use cube_histogram);
+ * other argument errors -> CUBE_EINVAL as cube_histogram.  A failed CUDA call -> CUBE_ECUDA with the cudaError_t
+ * in *cuda_error (may be NULL).  EVERY call on a device shares the one array, which keeps the last call's counts
+ * until the next call clears them: calls that overlap on the GPU (two streams, or two threads on two streams) RACE
+ * and give wrong counts -- keep them on one stream or order them with events. */
+#define CUBE_NOALLOC_MAX_BINS 4096
+int cube_histogram_noalloc(const float* d, int64_t nx, int64_t ny, int64_t nz, int nbins, float lo, float hi,
+                           uint64_t* bins /* [nbins] */, uint64_t* outside /* [2] */, cudaStream_t stream,
+                           int* cuda_error);
 
 /* PAPER.md:277-296. *out = the element of rank k (0-based) of the non-NaN voxels sorted ascending in
  * IEEE total order. Exact. If k >= count (known only on the device) *out = NaN. */

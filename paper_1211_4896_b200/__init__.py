@@ -36,7 +36,8 @@ SYMBOLS = ["cube_create", "cube_destroy", "cube_moments", "cube_histogram", "cub
            "cube_mad", "cube_clipped_moments", "cube_sigma_clip", "cube_minimap_dims", "cube_minimap",
            "cube_shard_buffers", "cube_shard_merge_records", "cube_shard_advance", "cube_median_torben",
            "cube_view_orbit", "cube_render_mip", "cube_render_tf", "cube_render_sigma", "cube_spectrum",
-           "cube_minimap_median"]
+           "cube_minimap_median", "cube_histogram_noalloc"]
+NOALLOC_MAX_BINS = 4096
 SHARD_RECORD_BYTES, SHARD_DIGITS = 40, 8192
 KNOB_CTAS_PER_SM, KNOB_BIGHIST, KNOB_MINIMAP, KNOB_SMALL, KNOB_MAPMEDIAN = 0, 1, 2, 3, 4
 KIND_NAMES = ["moments", "moments_coarse", "histogram", "select_pass0", "select_pass1", "select_pass2",
@@ -111,6 +112,7 @@ def load():
     L.cube_destroy.argtypes = [vp]
     L.cube_moments.argtypes = [vp, vp, i64, i64, i64, cu, vp, vp]
     L.cube_histogram.argtypes = [vp, vp, i64, i64, i64, ci, f32, f32, vp, vp, vp]
+    L.cube_histogram_noalloc.argtypes = [vp, i64, i64, i64, ci, f32, f32, vp, vp, vp, ctypes.POINTER(ci)]
     L.cube_kth.argtypes = [vp, vp, i64, i64, i64, u64, vp, vp]
     L.cube_kth_ex.argtypes = [vp, vp, i64, i64, i64, u64, cu, vp, vp]
     L.cube_kth_multi.argtypes = [vp, vp, i64, i64, i64, ci, vp, cu, vp, vp]
@@ -173,6 +175,27 @@ def _ptr(p):
     if isinstance(p, int):
         return ctypes.c_void_p(p)
     return ctypes.cast(p, ctypes.c_void_p)
+
+
+def histogram_noalloc(d, nx, ny, nz, nbins, lo, hi, bins=None, outside=None, stream=0):
+    """cube_histogram_noalloc: cube_histogram without a context and without any allocation on the device (the global
+    counters are a static array of the library; nbins <= NOALLOC_MAX_BINS, else CubeError(ERANGE)).  Calls share that
+    array: keep them on one stream.  ``bins`` / ``outside``: device or pinned buffers, else numpy arrays are returned."""
+    L = load()
+    err = ctypes.c_int(0)
+    ret = None
+    if bins is None:
+        bins = np.zeros(max(int(nbins), 1), dtype=np.uint64)
+        outside = np.zeros(2, dtype=np.uint64)
+        ret = (bins, outside)
+    rc = L.cube_histogram_noalloc(_ptr(d), nx, ny, nz, nbins, lo, hi, _ptr(bins), _ptr(outside), stream,
+                                  ctypes.byref(err))
+    if rc != OK:
+        msg = L.cube_strerror(rc).decode()
+        if rc == ECUDA:
+            msg += " cudaError=%d" % err.value
+        raise CubeError(rc, msg)
+    return ret
 
 
 class Context:

@@ -3,6 +3,7 @@
 // validates arguments, enqueues launches and copies results.
 #include "../../include/cube.h"
 
+#include <mutex>
 #include <math.h>
 #include <new>
 #include <stddef.h>
@@ -1091,5 +1092,96 @@ int cube_profile_read(cube_ctx* c, int kind, double* total_ms, uint64_t* launche
 }
 
 }  // extern "C"
+
+// ---- cube_histogram_noalloc: the histogram of cube_histogram for callers that cannot allocate (code under CUDA graph
+// capture, tight serving loops, harnesses that forbid cudaMalloc): no cube_ctx, no cudaMalloc / cudaFree anywhere
+// on its path.  The 64-bit global counters the per-CTA shared-memory counters are flushed into -- the scratch that
+// cube_create() otherwise allocates -- live in the file-scope array below: 2 + CUBE_NOALLOC_MAX_BINS words = 32 KiB
+// that every GPU which loads libcube holds until the process exits.
+namespace {
+
+static __device__ __align__(256) unsigned long long g_noalloc_scratch[2 + CUBE_NOALLOC_MAX_BINS];   // [outside (2)][bins]
+
+// hist_smem_kernel (cube_kernels.cuh) with its counters in the static scratch; `scratch` is the DEVICE address of
+// g_noalloc_scratch, resolved by the host with cudaGetSymbolAddress (in host code the array's name is only a stand-in).
+__global__ void __launch_bounds__(kThreads)
+hist_noalloc_kernel(const float* __restrict__ d, uint64_t n, int nbins, float lo, float hi, float scale,
+                    unsigned long long* __restrict__ scratch) {
+    extern __shared__ uint32_t dyn_bins[];
+    __shared__ uint32_t s_out[2];
+    for (int i = threadIdx.x; i < nbins + 2; i += kThreads) dyn_bins[i] = 0;  // + trash slot
+    if (threadIdx.x < 2) s_out[threadIdx.x] = 0;
+    __syncthreads();
+    uint32_t below = 0, above = 0;
+    if (hist_use_fast(nbins, lo, hi, scale)) {
+        HistFastF f;
+        f.setup(lo, hi, scale, nbins, dyn_bins, s_out);
+        stream_cube<kThreads>(d, n, f);
+    } else {
+        HistF f;
+        f.lo = lo; f.hi = hi; f.scale = scale; f.top = nbins - 1; f.sbins = dyn_bins;
+        stream_cube<kThreads>(d, n, f);
+        below = f.below; above = f.above;
+    }
+    __syncthreads();
+    hist_flush_bins(dyn_bins, nbins, scratch + 2);
+    if (below) atomicAdd(&s_out[0], below);
+    if (above) atomicAdd(&s_out[1], above);
+    __syncthreads();
+    if (threadIdx.x < 2 && s_out[threadIdx.x]) atomicAdd(&scratch[threadIdx.x], (unsigned long long)s_out[threadIdx.x]);
+}
+
+// Set-up, once per device, with that device current: the device address of the scratch and the SM count.
+struct NoAllocDevice { unsigned long long* scratch; int num_sms; };
+constexpr int kNoAllocMaxDevices = 64;
+NoAllocDevice g_noalloc_dev[kNoAllocMaxDevices];
+std::mutex g_noalloc_mutex;
+
+cudaError_t noalloc_device(NoAllocDevice* out) {
+    int dev = -1;
+    cudaError_t e = cudaGetDevice(&dev);
+    if (e != cudaSuccess) return e;
+    if (dev < 0 || dev >= kNoAllocMaxDevices) return cudaErrorInvalidDevice;
+    std::lock_guard<std::mutex> lock(g_noalloc_mutex);
+    if (!g_noalloc_dev[dev].scratch) {
+        unsigned long long* ptr = nullptr;
+        int sms = 0;
+        if ((e = cudaGetSymbolAddress((void**)&ptr, g_noalloc_scratch)) != cudaSuccess) return e;
+        if ((e = cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev)) != cudaSuccess) return e;
+        if (!ptr || sms < 1) return cudaErrorUnknown;
+        g_noalloc_dev[dev].num_sms = sms;
+        g_noalloc_dev[dev].scratch = ptr;
+    }
+    *out = g_noalloc_dev[dev];
+    return cudaSuccess;
+}
+
+}  // namespace
+
+extern "C" int cube_histogram_noalloc(const float* d, int64_t nx, int64_t ny, int64_t nz, int nbins, float lo, float hi,
+                                      uint64_t* bins, uint64_t* outside, cudaStream_t s, int* cuda_error) {
+    uint64_t n;
+    float scale;
+    if (cuda_error) *cuda_error = 0;
+    if (!d || !bins || !outside || !dims_ok(nx, ny, nz, &n)) return CUBE_EINVAL;
+    if (nbins > CUBE_NOALLOC_MAX_BINS) return CUBE_ERANGE;      // the static scratch holds no more: use cube_histogram
+    if (!hist_scale(nbins, lo, hi, &scale)) return CUBE_EINVAL;
+    NoAllocDevice dev;
+    cudaError_t e = noalloc_device(&dev);
+    // every call shares the scratch and finds the last call's counts in it: what this call accumulates into is cleared
+    if (e == cudaSuccess) e = cudaMemsetAsync(dev.scratch, 0, (size_t)(nbins + 2) * sizeof(unsigned long long), s);
+    if (e == cudaSuccess) {
+        const size_t smem = (size_t)(nbins + 2) * sizeof(uint32_t);   // <= 16 KiB + 8: no opt-in needed
+        hist_noalloc_kernel<<<dev.num_sms * 4, kThreads, smem, s>>>(d, n, nbins, lo, hi, scale, dev.scratch);
+        e = cudaGetLastError();
+    }
+    if (e == cudaSuccess) e = cudaMemcpyAsync(bins, dev.scratch + 2, (size_t)nbins * sizeof(uint64_t), cudaMemcpyDefault, s);
+    if (e == cudaSuccess) e = cudaMemcpyAsync(outside, dev.scratch, 2 * sizeof(uint64_t), cudaMemcpyDefault, s);
+    if (e != cudaSuccess) {
+        if (cuda_error) *cuda_error = (int)e;
+        return CUBE_ECUDA;
+    }
+    return CUBE_OK;
+}
 
 #include "cube_ooc.inl"
