@@ -96,7 +96,7 @@ __device__ __forceinline__ void med_locate(const uint32_t* hist, uint32_t k, uin
 // The voxels of one cell: `rows` rows of w contiguous voxels.
 struct MedCell {
     const float* base;
-    int w, h, rows;
+    int w, h, rows, dep;             // dep: planes (rows = h * dep)
     uint32_t nvox, magic;            // magic = floor(2^32 / h) + 1: r / h == umulhi(r, magic) while r * h < 2^32
     int lpr_log1, lpr_log2;          // log2 of the lanes a row takes, read as floats / as float2 (-1: not eligible)
     long long row_step, plane_step;
@@ -113,7 +113,8 @@ __device__ __forceinline__ MedCell med_cell_of(const float* __restrict__ d, cons
     c.base = d + ((z0 * g.ny + y0) * g.nx + x0);
     c.row_step = g.nx;
     c.plane_step = g.ny * g.nx;
-    if (c.h == 1) { c.h = c.rows; c.row_step = c.plane_step; }      // one line per plane: the planes are the rows
+    c.dep = c.rows / c.h;
+    if (c.h == 1) { c.h = c.rows; c.row_step = c.plane_step; c.dep = 1; }   // one line per plane: the planes are the rows
     c.magic = c.h == 1 ? 0u : (uint32_t)(0x100000000ull / (uint32_t)c.h) + 1u;   // h == 1: a single row, r = 0
     auto lanes_log = [](int n) { int l = 0; while ((1 << l) < n && l < 5) ++l; return l; };
     c.lpr_log1 = lanes_log(c.w);
@@ -217,10 +218,89 @@ __device__ __forceinline__ void med_for_each_voxel_v(const MedCell& c, int tid, 
     }
 }
 
+// The same visit for cells that are deep enough (c.dep >= kMedDeep planes): a warp keeps its rows' y and walks along z,
+// kMedInFlight planes per batch -- the address of a load is the previous one plus the plane stride (one 64-bit add),
+// where the row-major order above pays a division and three multiplications per load (ncu on 30^3 cells: 11 IMAD per
+// LDG, a third of all instructions).  The warps share the ng = ceil(h / rows-per-load) groups of rows; when there are
+// fewer groups than warps, several warps take the same group and interleave its planes.
+constexpr int kMedDeep = 16;
+
+template <int GROUP, int VEC, int POLICY, class F>
+__device__ __forceinline__ void med_for_each_voxel_z(const MedCell& c, int tid, F&& fn) {
+    const uint64_t pol = med_policy<POLICY>();
+    constexpr uint32_t NW = GROUP / 32, U = kMedInFlight;
+    const int lane = tid & 31;
+    const uint32_t wid = (uint32_t)tid >> 5;
+    const int lpr_log = VEC == 2 ? c.lpr_log2 : c.lpr_log1, rpw_log = 5 - lpr_log;
+    const uint32_t sub = (uint32_t)lane >> lpr_log, col = ((uint32_t)lane & ((1u << lpr_log) - 1u)) * VEC;
+    const uint32_t xstep = (uint32_t)VEC << lpr_log;
+    const uint32_t h = (uint32_t)c.h, w = (uint32_t)c.w, dep = (uint32_t)c.dep;
+    const uint32_t ng = (h + (1u << rpw_log) - 1u) >> rpw_log;
+    const uint32_t G = ng < NW ? ng : NW, ZS = NW / G;          // warps per plane sweep, sweeps interleaved along z
+    const uint32_t g0 = wid % G, z0 = wid / G;
+    if (z0 >= ZS) return;                                        // NW is not a multiple of G: the left-over warps
+    const uint64_t row_bytes = (uint64_t)c.row_step * 4u, zs_bytes = (uint64_t)c.plane_step * 4u * ZS;
+    using V = typename std::conditional<VEC == 2, float2, float>::type;
+    for (uint32_t g = g0; g < ng; g += G) {
+        const uint32_t y = (g << rpw_log) + sub;
+        for (uint32_t x0 = 0; x0 < w; x0 += xstep) {
+            if (!(y < h && col + x0 < w)) continue;              // lane-constant over the z walk
+            const char* __restrict__ q = reinterpret_cast<const char*>(c.base) + y * row_bytes + (uint64_t)(col + x0) * 4u +
+                                         (uint64_t)z0 * (uint64_t)c.plane_step * 4u;
+            uint32_t z = z0;
+            for (; z + (U - 1) * ZS < dep; z += U * ZS, q += U * zs_bytes) {
+                float a[U], b[U];
+#pragma unroll
+                for (uint32_t u = 0; u < U; ++u) {
+                    if (VEC == 2) {
+                        const float2 t = med_ld<POLICY>(reinterpret_cast<const float2*>(q + u * zs_bytes), pol);
+                        a[u] = t.x; b[u] = t.y;
+                    } else {
+                        a[u] = med_ld<POLICY>(reinterpret_cast<const float*>(q + u * zs_bytes), pol);
+                    }
+                }
+#pragma unroll
+                for (uint32_t u = 0; u < U; ++u) { fn(a[u]); if (VEC == 2) fn(b[u]); }
+            }
+            if (z < dep) {                                       // the last, partial batch
+                float a[U], b[U];
+#pragma unroll
+                for (uint32_t u = 0; u < U; ++u) {
+                    a[u] = b[u] = 0.0f;
+                    if (z + u * ZS < dep) {
+                        if (VEC == 2) {
+                            const float2 t = med_ld<POLICY>(reinterpret_cast<const float2*>(q + u * zs_bytes), pol);
+                            a[u] = t.x; b[u] = t.y;
+                        } else {
+                            a[u] = med_ld<POLICY>(reinterpret_cast<const float*>(q + u * zs_bytes), pol);
+                        }
+                    }
+                }
+#pragma unroll
+                for (uint32_t u = 0; u < U; ++u)
+                    if (z + u * ZS < dep) { fn(a[u]); if (VEC == 2) fn(b[u]); }
+            }
+        }
+    }
+}
+
+#ifndef CUBE_MED_ZWALK
+#define CUBE_MED_ZWALK 1
+#endif
 template <int GROUP, int POLICY = 0, class F>
 __device__ __forceinline__ void med_for_each_voxel(const MedCell& c, int tid, F&& fn) {
-    if (c.lpr_log2 >= 0) med_for_each_voxel_v<GROUP, 2, POLICY>(c, tid, fn);        // uniform over the CTA
-    else med_for_each_voxel_v<GROUP, 1, POLICY>(c, tid, fn);
+    // z walk: deep cells with at least one group of rows per warp (measured on c2: 30 x 30 x 16 cells 2.09 -> 1.66 ms,
+    // 64 x 16 x 64 1.23 -> 1.11, 64^3 1.40 -> 1.33, 30^3 unchanged at 1.58; 16^3 cells -- four groups for eight warps --
+    // are 7 % faster in row order)
+    const int lpr = c.lpr_log2 >= 0 ? c.lpr_log2 : c.lpr_log1;
+    const int ng = (c.h + (1 << (5 - lpr)) - 1) >> (5 - lpr);
+    if (CUBE_MED_ZWALK && c.dep >= kMedDeep && ng >= GROUP / 32) {                   // all uniform over the CTA
+        if (c.lpr_log2 >= 0) med_for_each_voxel_z<GROUP, 2, POLICY>(c, tid, fn);
+        else med_for_each_voxel_z<GROUP, 1, POLICY>(c, tid, fn);
+    } else {
+        if (c.lpr_log2 >= 0) med_for_each_voxel_v<GROUP, 2, POLICY>(c, tid, fn);
+        else med_for_each_voxel_v<GROUP, 1, POLICY>(c, tid, fn);
+    }
 }
 
 // Two-read selection of one cell by one CTA (cells of any size).
