@@ -653,16 +653,22 @@ def next_rows(ctx, cube_t, dims, lo, hi, out_m, out_f, dev, stream, timed, reps_
     # the paper's measurement: the cube turned through 360 degrees ("2 degrees steps"; here every 10th
     # of those views), pitch 0 and pitch 20, MIP: mean, best and worst frame
     for pitch in (0.0, 20.0):
-        per_view = []
-        for yaw in range(0, 360, 20):
-            vw = cubegen.view_orbit(dims, float(yaw), pitch, w, h, step=1.0)
-            fn = lambda: ctx.render_mip(cube_t, nx, ny, nz, vw, img, stream=stream)   # noqa: E731
-            per_view.append(timed(fn, 2))
-        ms = sum(per_view) / len(per_view)
-        ops["next4_mip_orbit_18_views_pitch%d" % int(pitch)] = {
-            "ms": ms, "frames_per_s": 1e3 / ms, "ms_best_view": min(per_view), "ms_worst_view": max(per_view),
-            "rays": w * h, "voxels_per_s": n / (ms * 1e-3), "algorithmic_bytes_per_voxel": 4.0,
-            "algorithmic_gbs": 4.0 * n / (ms * 1e-3) / 1e9, "frac_of_peak": 4.0 * n / (ms * 1e-3) / 1e9 / peak}
+        for kind in ("mip", "transfer_function", "sigma_clipping_tf"):
+            per_view = []
+            for yaw in range(0, 360, 20):
+                vw = cubegen.view_orbit(dims, float(yaw), pitch, w, h, step=1.0)
+                if kind == "mip":
+                    fn = lambda: ctx.render_mip(cube_t, nx, ny, nz, vw, img, stream=stream)   # noqa: E731
+                elif kind == "transfer_function":
+                    fn = lambda: ctx.render_tf(cube_t, nx, ny, nz, vw, tab_d, 0.004, 0.1, rgba, opacity_cut=0.98, stream=stream)   # noqa: E731
+                else:
+                    fn = lambda: ctx.render_sigma(cube_t, nx, ny, nz, vw, out_cells, part[0], part[1], part[2], tab_d, 3.0, 12.0, rgba, opacity_cut=0.98, stream=stream)   # noqa: E731
+                per_view.append(timed(fn, 2))
+            ms = sum(per_view) / len(per_view)
+            ops["next4_%s_orbit_18_views_pitch%d" % (kind, int(pitch))] = {
+                "ms": ms, "frames_per_s": 1e3 / ms, "ms_best_view": min(per_view), "ms_worst_view": max(per_view),
+                "rays": w * h, "voxels_per_s": n / (ms * 1e-3), "algorithmic_bytes_per_voxel": 4.0,
+                "algorithmic_gbs": 4.0 * n / (ms * 1e-3) / 1e9, "frac_of_peak": 4.0 * n / (ms * 1e-3) / 1e9 / peak}
     return ops
 
 

@@ -386,10 +386,10 @@ enum {
                                   1 = the cell's keys staged in shared memory, four 8-bit digits (cells of more than
                                       56000 voxels: re-read per digit); 2 = two reads of the cell, 11-bit first digit,
                                       the bucket's keys kept in shared memory (csrc/cube_minimap_median.cuh) */
-    CUBE_KNOB_RENDER = 5,      /* cube_render_mip: 0 = automatic (default): one ray per THREAD (a warp = 32 neighbouring pixels
-                                  of an image row) unless the rays run mostly along the cube's x axis, or rays and image
-                                  rows lie in planes y = const (an orbit at pitch 0), then one ray per WARP (lanes =
-                                  consecutive samples); 1 / 2 = always the former / the latter.  Same images bit for bit. */
+    CUBE_KNOB_RENDER = 5,      /* cube_render_mip / _tf / _sigma: 0 = automatic (default): one ray per THREAD (a warp = 32
+                                  neighbouring pixels of an image row) or one ray per WARP (lanes = consecutive samples),
+                                  by the z component of the ray direction (csrc/cube.cu, render_along); 1 / 2 = always
+                                  the former / the latter.  Same images bit for bit. */
     CUBE_KNOB_MINIMAP = 2      /* cube_minimap kernel: 0 = automatic (default): lines staged through a shared-memory
                                   ring by TMA bulk copies when the rows are 16-byte aligned, the cells at most 480
                                   voxels wide and a cell row has at least 256 lines (or the 128-bit kernel is not

@@ -884,6 +884,26 @@ int cube_view_orbit(int64_t nx, int64_t ny, int64_t nz, double yaw_deg, double p
     return CUBE_OK;
 }
 
+// Which ray-casting kernel (CUBE_KNOB_RENDER)?  One ray per warp (cube_render.cuh) pays for every PLANE of the cube that
+// the 32 consecutive samples of a ray cross (planes are megabytes apart), one ray per thread for every plane the 32
+// neighbouring pixels of an image row span.  Measured on c2, 1024^2 rays, over 40 views: the
+// ray-per-warp kernels win when the z component of the ray direction is at most 0.5 (yaw 90: MIP 13.6 -> 1.7 ms,
+// transfer function 10.7 -> 2.2), up to 0.9 when rays and image rows lie in planes y = const (an orbit at pitch 0:
+// neighbouring rays then share their lines), and -- with the mini-map lookups of the sigma-clipping transfer function,
+// which do not care about the direction, on top -- up to 0.9 (0.95 in such planes).
+static bool render_along(const cube_ctx* c, const RenderView& vw, bool sigma) {
+    const double sn = sqrt((double)vw.step[0] * vw.step[0] + (double)vw.step[1] * vw.step[1] + (double)vw.step[2] * vw.step[2]);
+    const double un = sqrt((double)vw.du[0] * vw.du[0] + (double)vw.du[1] * vw.du[1] + (double)vw.du[2] * vw.du[2]);
+    bool along_auto = false;
+    if (sn > 0.0) {
+        const double ay = fabs((double)vw.step[1]) / sn, az = fabs((double)vw.step[2]) / sn;
+        const double uy = un > 0.0 ? fabs((double)vw.du[1]) / un : 0.0;
+        const bool flat = ay <= 1e-3 && uy <= 1e-3;
+        along_auto = az <= (sigma ? (flat ? 0.95 : 0.9) : flat ? 0.9 : 0.5);
+    }
+    return c->render_variant == 0 ? along_auto : c->render_variant == 2;
+}
+
 int cube_render_mip(cube_ctx* c, const float* d, int64_t nx, int64_t ny, int64_t nz, const cube_view_t* view,
                     float vmin, float* image, cudaStream_t s) {
     RenderGeom g; RenderView vw;
@@ -892,20 +912,7 @@ int cube_render_mip(cube_ctx* c, const float* d, int64_t nx, int64_t ny, int64_t
         ProfScope prof(c, CUBE_K_RENDER, s);
         const dim3 block(kRenderTileU, kRenderTileV);
         const dim3 grid((vw.width + kRenderTileU - 1) / kRenderTileU, (vw.height + kRenderTileV - 1) / kRenderTileV);
-        // One ray per warp (cube_render.cuh) when the 32 consecutive samples of a ray touch few lines of the cube --
-        // the ray runs mostly along x: |y| + |z| components of its direction at most 0.6 -- or when ray and image rows
-        // both lie in planes y = const (an orbit at pitch 0) and the ray is not along z: neighbouring rays then share
-        // their lines.  Measured on c2, 1024^2 rays: yaw 90: 13.6 -> 1.7 ms, yaw 60: 14.6 -> 2.3,
-        // yaw 20 pitch 0: 6.1 -> 5.9; elsewhere the ray-per-thread kernel is the faster one.
-        const double sn = sqrt((double)vw.step[0] * vw.step[0] + (double)vw.step[1] * vw.step[1] + (double)vw.step[2] * vw.step[2]);
-        const double un = sqrt((double)vw.du[0] * vw.du[0] + (double)vw.du[1] * vw.du[1] + (double)vw.du[2] * vw.du[2]);
-        bool along_auto = false;
-        if (sn > 0.0) {
-            const double ax = fabs((double)vw.step[0]) / sn, ay = fabs((double)vw.step[1]) / sn, az = fabs((double)vw.step[2]) / sn;
-            const double uy = un > 0.0 ? fabs((double)vw.du[1]) / un : 0.0;
-            along_auto = (ay + az <= 0.6) || (ay <= 1e-3 && uy <= 1e-3 && ax >= 0.3);
-        }
-        const bool along = c->render_variant == 0 ? along_auto : c->render_variant == 2;
+        const bool along = render_along(c, vw, false);
         if (along) {
             const long long npix = (long long)vw.width * vw.height;
             render_mip_along_kernel<<<(unsigned)((npix + kRenderRaysPerCta - 1) / kRenderRaysPerCta), 32 * kRenderRaysPerCta, 0, s>>>(
@@ -952,7 +959,16 @@ static int render_tf_common(cube_ctx* c, const float* d, int64_t nx, int64_t ny,
         ProfScope prof(c, CUBE_K_RENDER, s);
         const dim3 block(kRenderTileU, kRenderTileV);
         const dim3 grid((vw.width + kRenderTileU - 1) / kRenderTileU, (vw.height + kRenderTileV - 1) / kRenderTileV);
-        if (dev_cells)
+        if (render_along(c, vw, dev_cells != nullptr)) {
+            const long long npix = (long long)vw.width * vw.height;
+            const unsigned agrid = (unsigned)((npix + kRenderRaysPerCta - 1) / kRenderRaysPerCta);
+            if (dev_cells)
+                render_tf_along_kernel<true><<<agrid, 32 * kRenderRaysPerCta, 0, s>>>(
+                    d, g, vw, nlevels, lo, scale, dev_table, opacity_cut, dev_cells, mg, reinterpret_cast<float4*>(rgba));
+            else
+                render_tf_along_kernel<false><<<agrid, 32 * kRenderRaysPerCta, 0, s>>>(
+                    d, g, vw, nlevels, lo, scale, dev_table, opacity_cut, nullptr, mg, reinterpret_cast<float4*>(rgba));
+        } else if (dev_cells)
             render_tf_kernel<true><<<grid, block, 0, s>>>(d, g, vw, nlevels, lo, scale, dev_table, opacity_cut, dev_cells,
                                                           mg, reinterpret_cast<float4*>(rgba));
         else

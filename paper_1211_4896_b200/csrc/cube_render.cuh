@@ -303,6 +303,71 @@ render_tf_kernel(const float* __restrict__ d, RenderGeom g, RenderView vw, int n
     rgba[(size_t)v * vw.width + u] = make_float4(cr, cg, cb, A);
 }
 
+// The transfer functions with one ray per warp (see render_mip_along_kernel for when).  Compositing is ordered, so
+// only the part of a sample that does not depend on the samples before it is done by its lane -- the trilinear value,
+// the mini-map lookup, the level, the table entry --; the recurrence itself is then run by the whole warp, uniformly,
+// over the lanes whose sample contributes, in march order (ballot + shuffles): the same float32 operations in the same
+// order as the sequential march, hence the same bits.  A transfer function skips what lies below its threshold --
+// nearly every sample of a noise-dominated cube -- so that loop is short.
+template <bool SIGMA>
+__global__ void __launch_bounds__(32 * kRenderRaysPerCta)
+render_tf_along_kernel(const float* __restrict__ d, RenderGeom g, RenderView vw, int nlevels, float lo, float scale,
+                       const float4* __restrict__ table, float opacity_cut, const double* __restrict__ cells,
+                       MapLookupGeom mg, float4* __restrict__ rgba) {
+    const int lane = threadIdx.x & 31;
+    const long long pix = (long long)blockIdx.x * kRenderRaysPerCta + (threadIdx.x >> 5);
+    if (pix >= (long long)vw.width * vw.height) return;                  // warp-uniform
+    const int u = (int)(pix % vw.width), v = (int)(pix / vw.width);
+    const RayF r = ray_setup(vw, g, u, v);
+    float cr = 0.0f, cg = 0.0f, cb = 0.0f, A = 0.0f;
+    const float top = (float)(nlevels - 1);
+    bool done = false;
+#pragma unroll 1
+    for (int i0 = r.i0; i0 <= r.i1 && !done; i0 += 64) {                 // two samples per lane in flight
+        Tap t[2];
+        float pts[2][3];
+#pragma unroll
+        for (int j = 0; j < 2; ++j) {
+            ray_point(vw, r.o, i0 + 32 * j + lane, pts[j]);
+            tap_load(d, g, pts[j], i0 + 32 * j + lane <= r.i1, t[j]);
+        }
+#pragma unroll
+        for (int j = 0; j < 2; ++j) {
+            float s = tap_value(t[j]);
+            bool c = t[j].in;
+            if (SIGMA && c) {
+                c = s == s;                                              // NULL sample: no need to look at the map
+                if (c) {
+                    float mean, sd;
+                    map_lookup(cells, mg, pts[j], mean, sd);
+                    c = sd > 0.0f;
+                    if (c) s = __fdiv_rn(__fsub_rn(s, mean), sd);
+                }
+            }
+            c = c && s >= lo;                                            // below the range (the threshold) or NULL
+            float4 e = make_float4(0.0f, 0.0f, 0.0f, 0.0f);
+            if (c) {
+                const float fl = floorf(__fmul_rn(__fsub_rn(s, lo), scale));
+                e = __ldg(table + ((fl >= top) ? nlevels - 1 : (int)fl));
+            }
+            unsigned mask = done ? 0u : __ballot_sync(0xffffffffu, c);   // done is warp-uniform
+            while (mask) {
+                const int src = __ffs(mask) - 1;
+                mask &= mask - 1;
+                const float ex = __shfl_sync(0xffffffffu, e.x, src), ey = __shfl_sync(0xffffffffu, e.y, src);
+                const float ez = __shfl_sync(0xffffffffu, e.z, src), ew = __shfl_sync(0xffffffffu, e.w, src);
+                const float w = __fmul_rn(__fsub_rn(1.0f, A), ew);
+                cr = __fadd_rn(cr, __fmul_rn(w, ex));
+                cg = __fadd_rn(cg, __fmul_rn(w, ey));
+                cb = __fadd_rn(cb, __fmul_rn(w, ez));
+                A = __fadd_rn(A, w);
+                if (A >= opacity_cut) { done = true; break; }
+            }
+        }
+    }
+    if (lane == 0) rgba[pix] = make_float4(cr, cg, cb, A);
+}
+
 // 3-D spectrum tool: sample i of pixel (u, v)'s ray, NaN outside the cube; one thread per sample.
 __global__ void __launch_bounds__(256)
 spectrum_kernel(const float* __restrict__ d, RenderGeom g, RenderView vw, int u, int v, float* __restrict__ out) {

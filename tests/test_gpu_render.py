@@ -58,11 +58,25 @@ def gpu_mip(ctx, t, dims, view, vmin=float("-inf")):
     return outs[0]
 
 
+def every_render_kernel(ctx, shape, call):
+    """call(out) under CUBE_KNOB_RENDER = automatic / ray per thread / ray per warp: identical bits"""
+    outs = []
+    try:
+        for variant in (0, 1, 2):
+            ctx.set_knob(cube.KNOB_RENDER, variant)
+            out = torch.full((int(np.prod(shape)),), 123.0, dtype=torch.float32, device="cuda")
+            call(out)
+            torch.cuda.synchronize()
+            outs.append(out.cpu().numpy().reshape(shape))
+    finally:
+        ctx.set_knob(cube.KNOB_RENDER, 0)
+    assert same_bits(outs[0], outs[1]) and same_bits(outs[0], outs[2])
+    return outs[0]
+
+
 def gpu_tf(ctx, t, dims, view, table, lo, hi, cut=2.0):
-    out = torch.full((view["height"] * view["width"] * 4,), 123.0, dtype=torch.float32, device="cuda")
-    ctx.render_tf(t, *dims, view, table, lo, hi, out, opacity_cut=cut)
-    torch.cuda.synchronize()
-    return out.cpu().numpy().reshape(view["height"], view["width"], 4)
+    return every_render_kernel(ctx, (view["height"], view["width"], 4),
+                               lambda out: ctx.render_tf(t, *dims, view, table, lo, hi, out, opacity_cut=cut))
 
 
 def colour_table(nlevels, seed):
@@ -175,10 +189,9 @@ def test_view_orbit_matches_the_recipe_and_arguments_are_checked(ctx):
 # ---- the sigma-clipping transfer function (R34) -----------------------------------------------
 
 def gpu_sigma(ctx, t, dims, view, cells_dev, part, table, zlo, zhi, cut=2.0):
-    out = torch.full((view["height"] * view["width"] * 4,), 123.0, dtype=torch.float32, device="cuda")
-    ctx.render_sigma(t, *dims, view, cells_dev, *part, table, zlo, zhi, out, opacity_cut=cut)
-    torch.cuda.synchronize()
-    return out.cpu().numpy().reshape(view["height"], view["width"], 4)
+    return every_render_kernel(ctx, (view["height"], view["width"], 4),
+                               lambda out: ctx.render_sigma(t, *dims, view, cells_dev, *part, table, zlo, zhi, out,
+                                                            opacity_cut=cut))
 
 
 def upload_cells(cells):
@@ -195,7 +208,7 @@ def test_sigma_clipping_rotated_views(ctx, name, dims, part):
     t, a = scaled_cube(name, dims, misalign=1 if name == "c1" else 0)
     cells = oracle.minimap(a, dims, part)
     cd = upload_cells(cells)
-    for yaw, pitch, step in VIEWS[:5]:
+    for yaw, pitch, step in VIEWS[:5] + VIEWS[7:]:
         view = cubegen.view_orbit(dims, yaw, pitch, 64, 48, step=step)
         for nlev, zlo, zhi, cut in ((16, 2.0, 7.0, 2.0), (256, 3.0, 12.0, 0.95), (1, 1.0, 1.0, 2.0), (64, -2.0, 2.0, 0.5)):
             tab = colour_table(nlev, nlev + 1)
@@ -276,3 +289,17 @@ def test_mip_ties_between_signed_zeros_keep_the_first_in_march_order(ctx):
         ref = oracle.render_mip(a, dims, view)
         assert same_bits(got, ref)
     assert np.signbit(got[~np.isnan(got)]).any() or True
+
+
+def test_dense_transfer_function_every_sample_contributes(ctx):
+    # every sample above the threshold, low opacities, no early termination: the ordered recurrence of the
+    # ray-per-warp kernel runs over all 32 lanes of every batch; and a cut that stops rays in the middle of a batch
+    dims = (90, 20, 12)
+    t, a = scaled_cube("c2", dims)
+    tab = colour_table(64, 21)
+    tab[:, 3] = np.float32(0.01) + tab[:, 3] * np.float32(0.05)
+    lo = float(np.nanmin(a)) - 1.0
+    for view in (cubegen.view_orbit(dims, 90, 0, 40, 24, 0.5), cubegen.view_orbit(dims, 80, 12, 40, 24, 1.0),
+                 cubegen.view_axis(dims, 0)):
+        for cut in (2.0, 0.5, 0.05):
+            assert same_bits(gpu_tf(ctx, t, dims, view, tab, lo, lo + 2.0, cut), oracle.render_tf(a, dims, view, tab, lo, lo + 2.0, cut))
