@@ -575,6 +575,10 @@ int cube_median_ex(cube_ctx* c, const float* d, int64_t nx, int64_t ny, int64_t 
                    cudaStream_t s) {
     uint64_t n;
     if (!c || !d || !out || !dims_ok(nx, ny, nz, &n)) return CUBE_EINVAL;
+    // A cube that stays in L2 between its reads: the single cooperative launch of cube_stats (cube_small.cuh) with a
+    // without the histogram -- one launch and two reads instead of three of each
+    if (flags == 0u && n * sizeof(float) <= ((size_t)96 << 20) && c->coop && !c->no_small)
+        return cube_stats(c, d, nx, ny, nz, 0, 0.f, 0.f, 0u, nullptr, nullptr, nullptr, out, s);
     return kth_impl<false>(c, d, n, 0, 1, flags, out, s);
 }
 
@@ -600,8 +604,8 @@ int cube_stats(cube_ctx* c, const float* d, int64_t nx, int64_t ny, int64_t nz, 
     float* med_direct = static_cast<float*>(device_reachable(c, median));
     MomentsOut* mom_direct = static_cast<MomentsOut*>(device_reachable(c, moments));
     // A cube that stays in L2 between its two reads: everything in ONE cooperative launch (cube_small.cuh)
-    if (want_median && want_hist && nbins <= kSmallMaxBins && n * sizeof(float) <= ((size_t)96 << 20) && c->coop &&
-        !c->no_small) {
+    if (!want_hist) nbins = 0;
+    if (want_median && nbins <= kSmallMaxBins && n * sizeof(float) <= ((size_t)96 << 20) && c->coop && !c->no_small) {
         const size_t smem = (size_t)small_smem(nbins);
         const int occ = occupancy_of(c, stats_small_kernel, kThreads, smem);
         int per = c->ctas_per_sm > 0 ? c->ctas_per_sm : 2;
@@ -629,7 +633,7 @@ int cube_stats(cube_ctx* c, const float* d, int64_t nx, int64_t ny, int64_t nz, 
             c->bar_base += kSmallBarriers * grid;
             if (!med_direct) CUBE_CUDA(c, cudaMemcpyAsync(median, &c->sel->result, sizeof(float), cudaMemcpyDefault, s));
             if (moments && !mom_direct) CUBE_CUDA(c, cudaMemcpyAsync(moments, c->mom_out, sizeof(MomentsOut), cudaMemcpyDefault, s));
-            if (!a.bins_user) {
+            if (want_hist && !a.bins_user) {
                 CUBE_CUDA(c, cudaMemcpyAsync(bins, c->gbins, (size_t)nbins * sizeof(uint64_t), cudaMemcpyDefault, s));
                 CUBE_CUDA(c, cudaMemcpyAsync(outside, c->gout, 2 * sizeof(uint64_t), cudaMemcpyDefault, s));
             }

@@ -228,12 +228,20 @@ stats_small_kernel(SmallArgs a) {
         if (threadIdx.x < 2) s_out[threadIdx.x] = 0;
         __syncthreads();
         float lo = a.lo, hi = a.hi, scale = a.scale;
-        const bool range_ok = hist_range(a.minmax ? &s_mom : nullptr, a.nbins, lo, hi, scale);
+        const bool range_ok = a.nbins == 0 || hist_range(a.minmax ? &s_mom : nullptr, a.nbins, lo, hi, scale);
         if (!range_ok) { lo = INFINITY; hi = -INFINITY; }   // nothing is in range: every counter stays 0
         SelView sv;
         sv.invalid = s_sel.invalid; sv.prefix = s_sel.prefix; sv.cand_n = &a.sel->cand_n; sv.cand_cap = a.cand ? a.cand_cap : 0;
         uint32_t below = 0, above = 0;
-        if (hist_use_fast(a.nbins, lo, hi, scale)) {
+        if (a.nbins == 0) {                    // cube_median / cube_stats without a histogram: the select pass alone
+            if (!sv.invalid) {
+                SelectF<1, false> f;
+                f.base = sv.prefix << kShift0; f.rawbase = raw_of_digit(sv.prefix) << kShift0; f.sbins = sbins;
+                f.init_stage(stage, a.cand, sv.cand_n, sv.cand_cap);
+                stream_cube<kThreads>(a.d, a.n, f);
+                f.finish();
+            }
+        } else if (hist_use_fast(a.nbins, lo, hi, scale)) {
             HistFastF h;
             h.setup(lo, hi, scale, a.nbins, hbins, s_out);
             hist_select_run(a.d, a.n, h, sv, sbins, stage, a.cand, below, above);

@@ -17,11 +17,15 @@ pytestmark = pytest.mark.gpu
 REL = 1e-9
 
 
-@pytest.fixture(scope="module")
-def ctx():
+@pytest.fixture(scope="module", params=["l2_resident_single_launch", "general_path"])
+def ctx(request):
+    """Every test of this file runs twice: as a user gets it (cubes of at most 96 MiB: cube_stats with the median and
+    cube_median are ONE cooperative launch), and with CUBE_KNOB_SMALL = 1 (the general multi-launch path that larger
+    cubes take), so that both see every edge case here."""
     assert torch.cuda.is_available(), "gpu tests need a CUDA device (there is no CPU fallback)"
     torch.cuda.init()
     c = cube.Context()
+    c.set_knob(cube.KNOB_SMALL, 1 if request.param == "general_path" else 0)
     yield c
     c.close()
 
@@ -950,5 +954,24 @@ def test_single_launch_path_for_l2_resident_cubes(scratch):
                     assert same_float(c.kth(t, a.size, 1, 1, k, flags=cube.REUSE_COARSE), oracle.kth(a, k))
                 ms = c.stats(t, a.size, 1, 1, nb, lo, hi, flags=cube.SAMPLE_STD)[0]
                 check_moments(ms, oracle.moments(a, sample_std=True), a)
+            # cube_median alone takes the same single launch, without the histogram; the three-launch path under the knob
+            c.set_knob(cube.KNOB_SMALL, 1)
+            l0 = c.launch_count
+            gmed = c.median(t, a.size, 1, 1)
+            assert c.launch_count - l0 >= 3 and same_float(gmed, omed)
+            c.set_knob(cube.KNOB_SMALL, 0)
+            for per_sm in (0, 1, 3):
+                c.set_launch(per_sm)
+                l0 = c.launch_count
+                assert same_float(c.median(t, a.size, 1, 1), omed)
+                assert c.launch_count - l0 == 1
+                d_f = torch.full((1,), 7.0, dtype=torch.float32, device="cuda")
+                c.median(t, a.size, 1, 1, out=d_f)
+                torch.cuda.synchronize()
+                assert same_float(d_f.cpu()[0].item(), omed)
+            c.set_launch(0)
+            # and the state it leaves serves a later selection on the same cube
+            if ref["count"]:
+                assert same_float(c.kth(t, a.size, 1, 1, ref["count"] // 5, flags=cube.REUSE_COARSE), oracle.kth(a, ref["count"] // 5))
     finally:
         c.close()
