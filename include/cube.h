@@ -344,7 +344,9 @@ int cube_render_tf(cube_ctx* ctx, const float* d, int64_t nx, int64_t ny, int64_
  * clipping threshold in local sigmas, "2, 3, 4 and 7 sigma"); z < zlo, NULL samples and samples where
  * the interpolated std is not > 0 (or the map is NULL: an empty cell takes part) are skipped; compositing, table,
  * opacity_cut and rgba as cube_render_tf.  `cells`: memory the DEVICE can read (device or pinned host), mx*my*mz
- * records; read only. */
+ * records; read only.  Each call first rounds the cells' (mean, std) to float32 pairs in a buffer of the context
+ * (8 bytes per cell; it is allocated -- the only allocation a render call can make -- when a map larger than any
+ * before comes: CUBE_ENOMEM if that fails). */
 int cube_render_sigma(cube_ctx* ctx, const float* d, int64_t nx, int64_t ny, int64_t nz, const cube_view_t* view,
                       const cube_moments_t* cells, int64_t px, int64_t py, int64_t pz, int nlevels, float zlo,
                       float zhi, const float* table, float opacity_cut, float* rgba, cudaStream_t stream);

@@ -30,6 +30,8 @@ struct cube_ctx {
     int no_small = 0;     // CUBE_KNOB_SMALL: 1 = never the single cooperative launch
     int mapmedian = 0;    // CUBE_KNOB_MAPMEDIAN
     int render_variant = 0;   // CUBE_KNOB_RENDER
+    float2* map32 = nullptr;  // cube_render_sigma: (mean, std) of the mini-map's cells as float32 pairs
+    size_t map32_cap = 0;     // cells it holds
     int coop = 0;         // the device supports cooperative launches
     unsigned int* bar = nullptr;   // grid-barrier counter of stats_small_kernel (only grows)
     unsigned int bar_base = 0;
@@ -447,7 +449,7 @@ int cube_destroy(cube_ctx* c) {
     cudaFree(c->partials); cudaFree(c->ticket); cudaFree(c->ticket2); cudaFree(c->acc);
     cudaFree(c->mom_out); cudaFree(c->gout); cudaFree(c->gdigits); cudaFree(c->coarse); cudaFree(c->sel); cudaFree(c->multi);
     cudaFree(c->range3); cudaFree(c->probe_out); cudaFree(c->plan); cudaFree(c->clip); cudaFree(c->torben); cudaFree(c->center);
-    cudaFree(c->cand); cudaFree(c->tf_table); cudaFree(c->bar); cudaFree(c->coarse_next); cudaFree(c->chunk_tot); cudaFree(c->small_ext);
+    cudaFree(c->cand); cudaFree(c->tf_table); cudaFree(c->bar); cudaFree(c->coarse_next); cudaFree(c->chunk_tot); cudaFree(c->small_ext); cudaFree(c->map32);
     cudaFree(c->resident); cudaFree(c->chunk[0]); cudaFree(c->chunk[1]);
     if (c->pinned_results) cudaFreeHost(c->pinned_results);
     for (int i = 0; i < cube_ctx::kMaxStage; ++i) {
@@ -953,6 +955,23 @@ static int render_tf_common(cube_ctx* c, const float* d, int64_t nx, int64_t ny,
             mg.top[k] = (float)(m[k] - 1);
         }
         mg.mx = m[0]; mg.my = m[1]; mg.mz = m[2];
+        // (mean, std) of the cells as float32 pairs, what the rays interpolate (cube_render.cuh): 8 bytes per cell in a
+        // buffer of the context that grows when a larger map comes (the only allocation a render call can make)
+        const long double ncell_ld = (long double)m[0] * (long double)m[1] * (long double)m[2];
+        if (ncell_ld > 4294967296.0L) return CUBE_EINVAL;
+        const size_t ncell = (size_t)ncell_ld;
+        if (ncell > c->map32_cap) {
+            float2* bigger = nullptr;
+            if (cudaMalloc(&bigger, ncell * sizeof(float2)) != cudaSuccess) { cudaGetLastError(); return CUBE_ENOMEM; }
+            cudaFree(c->map32);          // synchronises: no earlier render is still reading it
+            c->map32 = bigger;
+            c->map32_cap = ncell;
+        }
+        {
+            ProfScope prof(c, CUBE_K_OTHER, s);
+            map_compact_kernel<<<(unsigned)((ncell + 255) / 256), 256, 0, s>>>(dev_cells, (long long)ncell, c->map32);
+        }
+        CUBE_CUDA(c, cudaGetLastError());
     }
     const float4* dev_table = static_cast<const float4*>(device_reachable(c, const_cast<float*>(table)));
     if (!dev_table || ((uintptr_t)dev_table & 15u)) {
@@ -968,12 +987,12 @@ static int render_tf_common(cube_ctx* c, const float* d, int64_t nx, int64_t ny,
             const unsigned agrid = (unsigned)((npix + kRenderRaysPerCta - 1) / kRenderRaysPerCta);
             if (dev_cells)
                 render_tf_along_kernel<true><<<agrid, 32 * kRenderRaysPerCta, 0, s>>>(
-                    d, g, vw, nlevels, lo, scale, dev_table, opacity_cut, dev_cells, mg, reinterpret_cast<float4*>(rgba));
+                    d, g, vw, nlevels, lo, scale, dev_table, opacity_cut, c->map32, mg, reinterpret_cast<float4*>(rgba));
             else
                 render_tf_along_kernel<false><<<agrid, 32 * kRenderRaysPerCta, 0, s>>>(
                     d, g, vw, nlevels, lo, scale, dev_table, opacity_cut, nullptr, mg, reinterpret_cast<float4*>(rgba));
         } else if (dev_cells)
-            render_tf_kernel<true><<<grid, block, 0, s>>>(d, g, vw, nlevels, lo, scale, dev_table, opacity_cut, dev_cells,
+            render_tf_kernel<true><<<grid, block, 0, s>>>(d, g, vw, nlevels, lo, scale, dev_table, opacity_cut, c->map32,
                                                           mg, reinterpret_cast<float4*>(rgba));
         else
             render_tf_kernel<false><<<grid, block, 0, s>>>(d, g, vw, nlevels, lo, scale, dev_table, opacity_cut, nullptr,
