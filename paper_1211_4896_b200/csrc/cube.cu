@@ -34,8 +34,7 @@ struct cube_ctx {
     size_t map32_cap = 0;     // cells it holds
     int coop = 0;         // the device supports cooperative launches
     unsigned int* bar = nullptr;   // grid-barrier counter of stats_small_kernel (only grows)
-    unsigned int bar_base = 0;
-    unsigned long long* coarse_next = nullptr;   // all zero: the first-digit array the next single-launch cube_stats takes
+    unsigned long long* coarse_next = nullptr;   // all zero between calls: the first-digit array of the single-launch cube_stats
     unsigned long long* chunk_tot = nullptr;     // kDigitBins / 32 chunk totals, all zero between calls
     unsigned int* small_ext = nullptr;           // stats_small_kernel: {min key, max key, ticket} = {~0, 0, 0} between calls
     unsigned long long* small_tstamp = nullptr;   // debug builds only (-DCUBE_SMALL_TIMING)
@@ -404,8 +403,8 @@ int cube_create(cube_ctx** out, size_t scratch_bytes_hint) {
         ok = ok && cudaMalloc(&c->small_ext, sizeof(ext0)) == cudaSuccess;
         ok = ok && cudaMemcpy(c->small_ext, ext0, sizeof(ext0), cudaMemcpyHostToDevice) == cudaSuccess;
     }
-    ok = ok && cudaMalloc(&c->bar, sizeof(unsigned int)) == cudaSuccess;
-    ok = ok && cudaMemset(c->bar, 0, sizeof(unsigned int)) == cudaSuccess;
+    ok = ok && cudaMalloc(&c->bar, 2 * sizeof(unsigned int)) == cudaSuccess;      // counter, base of the next launch
+    ok = ok && cudaMemset(c->bar, 0, 2 * sizeof(unsigned int)) == cudaSuccess;
     c->coop = prop.cooperativeLaunch ? 1 : 0;
 #ifdef CUBE_SMALL_TIMING
     ok = ok && cudaMallocManaged(&c->small_tstamp, (16 + 8 * 4096) * sizeof(unsigned long long)) == cudaSuccess;
@@ -618,10 +617,10 @@ int cube_stats(cube_ctx* c, const float* d, int64_t nx, int64_t ny, int64_t nz, 
             a.d = d; a.n = n; a.nbins = nbins; a.lo = lo; a.hi = hi; a.scale = scale; a.minmax = minmax ? 1 : 0;
             a.flags = flags & CUBE_SAMPLE_STD;
             a.partials = c->partials; a.acc = c->acc; a.nvox_acc = c->nvox_acc; a.mom_out = c->mom_out; a.out_user = mom_direct;
-            a.coarse = c->coarse_next; a.coarse_next = c->coarse; a.chunk_tot = c->chunk_tot;   // the zeroed array becomes the current one
+            a.coarse = c->coarse_next; a.coarse_keep = c->coarse; a.chunk_tot = c->chunk_tot;
             a.gdigits = c->gdigits; a.gout = c->gout;
             a.sel = c->sel; a.cand = c->cand; a.cand_cap = c->cand ? c->cand_cap : 0; a.result_out = med_direct;
-            a.bar = c->bar; a.bar_base = c->bar_base; a.ext = c->small_ext; a.tstamp = c->small_tstamp;
+            a.bar = c->bar; a.ext = c->small_ext; a.tstamp = c->small_tstamp;
             a.bins_user = static_cast<unsigned long long*>(device_reachable(c, bins));
             a.outside_user = static_cast<unsigned long long*>(device_reachable(c, outside));
             if (!a.bins_user || !a.outside_user) a.bins_user = a.outside_user = nullptr;
@@ -631,8 +630,6 @@ int cube_stats(cube_ctx* c, const float* d, int64_t nx, int64_t ny, int64_t nz, 
                 CUBE_CUDA(c, cudaLaunchCooperativeKernel(reinterpret_cast<void*>(stats_small_kernel), dim3(grid), dim3(kThreads),
                                                          args, smem, s));
             }
-            std::swap(c->coarse, c->coarse_next);     // only once the launch is enqueued: coarse_next stays "all zero"
-            c->bar_base += kSmallBarriers * grid;
             if (!med_direct) CUBE_CUDA(c, cudaMemcpyAsync(median, &c->sel->result, sizeof(float), cudaMemcpyDefault, s));
             if (moments && !mom_direct) CUBE_CUDA(c, cudaMemcpyAsync(moments, c->mom_out, sizeof(MomentsOut), cudaMemcpyDefault, s));
             if (want_hist && !a.bins_user) {

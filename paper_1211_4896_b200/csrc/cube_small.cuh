@@ -12,7 +12,7 @@
 // the same integers; mean / std differ in the last bits only through the grid size (tolerance R20).
 //
 //   phase A  moments + first digit (pass A); the histogram bins are zeroed on the way  | grid barrier
-//            every CTA: merge the partials, locate the median's first-digit bucket (from 256 chunk totals)
+//            every CTA: locate the median's first-digit bucket (from 256 chunk totals)
 //   phase B  histogram + second digit + candidate compaction (pass B), from L2        | grid barrier
 //            candidates fit (the usual case): CTA 0 counts the last digit on them and finishes; the other CTAs exit
 //            else: every CTA locates the second-digit bucket, counts the last digit over the cube | grid barrier, CTA 0 finishes
@@ -25,8 +25,9 @@ struct SmallArgs {
     const float* d; uint64_t n;
     int nbins; float lo, hi, scale; int minmax; unsigned flags;
     Partial* partials; Partial* acc; unsigned long long* nvox_acc; MomentsOut* mom_out; MomentsOut* out_user;
-    unsigned long long* coarse;      // kDigitBins first-digit counts (kept for CUBE_REUSE_COARSE); all zero on entry
-    unsigned long long* coarse_next; // the array the NEXT call will use: zeroed here by the CTAs that finish early
+    unsigned long long* coarse;      // kDigitBins first-digit counts of THIS call: all zero on entry, left all zero
+    unsigned long long* coarse_keep; // where they are kept for CUBE_REUSE_COARSE: copied there (and `coarse` zeroed for
+                                     // the next call) by the CTAs that have nothing else left to do
     unsigned long long* chunk_tot;   // kDigitBins / 32 totals of 32 consecutive first digits, in KEY order; zero on
                                      // entry, left zeroed
     unsigned long long* gdigits;     // kDigitBins: [0, 1024) second digit, [4096, 4608) last digit; left zeroed
@@ -34,7 +35,9 @@ struct SmallArgs {
     SelectState* sel; uint32_t* cand; unsigned long long cand_cap; float* result_out;
     unsigned long long* bins_user;   // the caller's bins / outside when the device can reach them (no copy is enqueued then)
     unsigned long long* outside_user;
-    unsigned int* bar; unsigned int bar_base;
+    unsigned int* bar;               // [0] the barrier counter (only grows), [1] its value when this launch starts: read
+                                     // by every CTA at its start, advanced by CTA 0 at the very end -- no state of the
+                                     // call lives on the host, so a CUDA graph holding the launch can be replayed
     unsigned int* ext;               // [0] = smallest key seen (0xFFFFFFFF between calls), [1] = largest (0), [2] = ticket (0)
     unsigned long long* tstamp;      // debug (-DCUBE_SMALL_TIMING): %globaltimer of CTA 0 at the phase boundaries
 };
@@ -149,6 +152,7 @@ stats_small_kernel(SmallArgs a) {
     __shared__ Partial parked[kThreads];          // the threads' moments of phase A, reduced while waiting at barrier B
     const unsigned grid = gridDim.x;
     const unsigned gtid = blockIdx.x * kThreads + threadIdx.x, gthreads = grid * kThreads;
+    const unsigned bar_base = __ldcg(&a.bar[1]);      // CTA 0 rewrites it behind barrier B, which needs every CTA's arrival
 
     SMALL_T(0);
     SMALL_TC(0);
@@ -202,7 +206,7 @@ stats_small_kernel(SmallArgs a) {
         }
     }
     SMALL_TC(3);
-    small_grid_sync(a.bar, a.bar_base + grid);
+    small_grid_sync(a.bar, bar_base + grid);
     SMALL_TC(4);
 
     SMALL_T(3);
@@ -289,20 +293,24 @@ stats_small_kernel(SmallArgs a) {
             }
         }
     }
-    small_grid_wait(a.bar, a.bar_base + 2 * grid);
+    small_grid_wait(a.bar, bar_base + 2 * grid);
     SMALL_TC(7);
 
     SMALL_T(6);
     // ---- last digit
     const unsigned long long cn = __ldcg(&a.sel->cand_n);      // final: every CTA's appends precede its arrival
     const bool fits = a.cand != nullptr && cn <= a.cand_cap;   // the same on every CTA
-    // housekeeping nobody waits for -- the array the next call counts first digits into (nobody reads it in this call)
-    // and the histogram, complete now, straight into the caller's buffers -- is left to the CTAs other than 0, whose
-    // chain of dependent round trips ends the call
+    // housekeeping nobody waits for -- the first-digit counts (every CTA has read what it needed of them before barrier
+    // B) move to where CUBE_REUSE_COARSE finds them and their array is zeroed for the next call; the histogram, complete
+    // now, goes straight into the caller's buffers -- is left to the CTAs other than 0, whose chain of dependent round
+    // trips ends the call
     if (grid == 1 || blockIdx.x != 0) {
         const unsigned hthreads = (grid == 1 ? 1u : grid - 1u) * kThreads;
         const unsigned htid = (grid == 1 ? 0u : blockIdx.x - 1u) * kThreads + threadIdx.x;
-        for (unsigned i = htid; i < (unsigned)kDigitBins; i += hthreads) a.coarse_next[i] = 0ull;
+        for (unsigned i = htid; i < (unsigned)kDigitBins; i += hthreads) {
+            a.coarse_keep[i] = __ldcg(&a.coarse[i]);
+            a.coarse[i] = 0ull;
+        }
         if (a.bins_user) {
             for (unsigned i = htid; i < (unsigned)a.nbins; i += hthreads) a.bins_user[i] = __ldcg(&a.gout[2 + i]);
             if (htid < 2) a.outside_user[htid] = __ldcg(&a.gout[htid]);
@@ -353,7 +361,7 @@ stats_small_kernel(SmallArgs a) {
         }
     }
     if (!fits) {
-        small_grid_sync(a.bar, a.bar_base + 3 * grid);
+        small_grid_sync(a.bar, bar_base + 3 * grid);
         if (blockIdx.x != 0) return;
     } else {
         small_grid_arrive(a.bar);
@@ -372,6 +380,7 @@ stats_small_kernel(SmallArgs a) {
         g->k = s_sel.k; g->count = s_sel.count; g->prefix = s_sel.prefix; g->invalid = s_sel.invalid;
         SMALL_T(8);
         g->use_median = 1u; g->result = s_sel.result; g->bucket_n = s_sel.bucket_n; g->cand_cap = a.cand ? a.cand_cap : 0; g->cand_done = fits ? 1u : 0u;
+        a.bar[1] = bar_base + kSmallBarriers * grid;   // every CTA arrives kSmallBarriers times per launch
     }
 }
 
