@@ -67,3 +67,54 @@ def test_cube_stats_replays_from_a_cuda_graph(general_path):
             assert np.float32(d_f2.item()).tobytes() == np.float32(rmed).tobytes()
     finally:
         ctx.close()
+
+
+def test_single_operations_replay_from_a_cuda_graph():
+    # cube_moments, cube_histogram with 65536 bins (the window / packed kernels and their device-side plan), cube_kth and
+    # cube_kth_multi: captured once, replayed on other data
+    n, nb = 262144 + 77, 65536
+    r = np.random.default_rng(6)
+    cubes = [(r.standard_normal(n) * s + m).astype(np.float32) for s, m in ((0.002, 0.0003), (0.3, 2.0), (0.0005, -0.015))]
+    cubes[2][r.integers(0, n, 2000)] = np.nan
+    lo, hi = -0.02, 3.0
+    ks = [n // 100, n // 2, n - n // 50]
+    ctx = cube.Context()
+    try:
+        t = torch.from_numpy(cubes[0]).cuda()
+        d_m = torch.zeros(40, dtype=torch.uint8, device="cuda")
+        d_b = torch.zeros(nb, dtype=torch.int64, device="cuda")
+        d_o = torch.zeros(2, dtype=torch.int64, device="cuda")
+        d_k = torch.zeros(1, dtype=torch.float32, device="cuda")
+        d_ks = torch.zeros(len(ks), dtype=torch.float32, device="cuda")
+        side = torch.cuda.Stream()
+
+        def calls(s):
+            ctx.moments(t, n, 1, 1, out=d_m, stream=s)
+            ctx.histogram(t, n, 1, 1, nb, lo, hi, bins=d_b, outside=d_o, stream=s)
+            ctx.kth(t, n, 1, 1, ks[0], out=d_k, stream=s)
+            ctx.kth_multi(t, n, 1, 1, ks, out=d_ks, stream=s)
+
+        calls(side.cuda_stream)
+        side.synchronize()
+        g = torch.cuda.CUDAGraph()
+        with torch.cuda.graph(g, stream=side):
+            calls(torch.cuda.current_stream().cuda_stream)
+        for a in (cubes[1], cubes[2], cubes[0]):
+            t.copy_(torch.from_numpy(a))
+            for buf in (d_m, d_b, d_o, d_k, d_ks):
+                buf.zero_()
+            torch.cuda.synchronize()
+            g.replay()
+            torch.cuda.synchronize()
+            ref, (rb, ro) = oracle.moments(a), oracle.histogram(a, nb, lo, hi)
+            m = moments_of(d_m)
+            assert m["count"] == ref["count"] and np.float32(m["max"]).tobytes() == np.float32(ref["max"]).tobytes()
+            assert abs(m["std"] - ref["std"]) <= 1e-9 * ref["std"]
+            assert (d_b.cpu().numpy().astype(np.uint64) == rb).all() and (d_o.cpu().numpy().astype(np.uint64) == ro).all()
+            cnt = ref["count"]
+            want = [oracle.kth(a, k) if k < cnt else np.float32(np.nan) for k in ks]
+            got = d_ks.cpu().numpy()
+            assert all(np.float32(x).tobytes() == np.float32(y).tobytes() or (np.isnan(x) and np.isnan(y)) for x, y in zip(got, want))
+            assert np.float32(d_k.item()).tobytes() == np.float32(want[0]).tobytes()
+    finally:
+        ctx.close()
