@@ -887,22 +887,36 @@ int cube_view_orbit(int64_t nx, int64_t ny, int64_t nz, double yaw_deg, double p
     return CUBE_OK;
 }
 
-// Which ray-casting kernel (CUBE_KNOB_RENDER)?  One ray per warp (cube_render.cuh) pays for every PLANE of the cube that
-// the 32 consecutive samples of a ray cross (planes are megabytes apart), one ray per thread for every plane the 32
-// neighbouring pixels of an image row span.  Measured on c2, 1024^2 rays, over 40 views: the
-// ray-per-warp kernels win when the z component of the ray direction is at most 0.5 (yaw 90: MIP 13.6 -> 1.7 ms,
-// transfer function 10.7 -> 2.2), up to 0.9 when rays and image rows lie in planes y = const (an orbit at pitch 0:
-// neighbouring rays then share their lines), and -- with the mini-map lookups of the sigma-clipping transfer function,
-// which do not care about the direction, on top -- up to 0.9 (0.95 in such planes).
-static bool render_along(const cube_ctx* c, const RenderView& vw, bool sigma) {
-    const double sn = sqrt((double)vw.step[0] * vw.step[0] + (double)vw.step[1] * vw.step[1] + (double)vw.step[2] * vw.step[2]);
+// Footprint of a warp in the ray-per-thread kernels (cube_render.cuh, render_pixel): log2 of its width in pixels.
+static int render_footprint(const RenderView& vw) {
+    if (const char* e = getenv("CUBE_RENDER_FW")) return atoi(e);           // experiments
     const double un = sqrt((double)vw.du[0] * vw.du[0] + (double)vw.du[1] * vw.du[1] + (double)vw.du[2] * vw.du[2]);
+    // measured on c2, 1024^2 rays (MIP, ms; 32x1 / 16x2 / 8x4 / 4x8): yaw 0: 1.72 / 1.67 / 1.74 / 2.88, yaw 10: 4.12 / 3.36 /
+    // 3.59 / 4.99, yaw 20 pitch 20: 6.28 / 4.76 / 4.72 / 5.42, yaw 45 pitch 40: 9.84 / 7.71 / 6.77 / 6.40
+    // pixels one voxel apart along x (an axis-aligned view at the cube's resolution): 32 x 1, the lanes read 32 neighbouring
+    // voxels (4.14 ms against 4.44 with 16 x 2 on c2 along z)
+    if (un > 0.0 && un <= 1.25 && fabs((double)vw.du[0]) / un >= 0.98) return 5;
+    return (un > 0.0 && fabs((double)vw.du[0]) / un >= 0.9) ? 4 : 3;        // image rows nearly along x: 16 x 2, else 8 x 4
+}
+
+// Which ray-casting kernel (CUBE_KNOB_RENDER)?  One ray per warp (cube_render.cuh) pays for every PLANE of the cube that
+// the 32 consecutive samples of a ray cross (planes are megabytes apart) and for every line they climb in y, one ray per
+// thread for the planes and lines the block of pixels of a warp spans.  The rules below are fits to a map of both
+// kernels over yaw 0-90 x pitch 0-60 degrees on c2, 1024^2 rays, in terms of the components
+// (ax, ay, az) of the ray direction: ray-per-warp wins when az is small enough for the ay at hand -- up to 0.9 when
+// rays and image rows lie in planes y = const (an orbit at pitch 0: neighbouring rays share their lines) -- and, for
+// the sigma-clipping transfer function, whose map lookups do not care about the direction, whenever the ray is not
+// too steep in y and has some x component at all.
+enum { kRenderMip = 0, kRenderTf = 1, kRenderSigma = 2 };
+static bool render_along(const cube_ctx* c, const RenderView& vw, int kind) {
+    const double sn = sqrt((double)vw.step[0] * vw.step[0] + (double)vw.step[1] * vw.step[1] + (double)vw.step[2] * vw.step[2]);
     bool along_auto = false;
     if (sn > 0.0) {
-        const double ay = fabs((double)vw.step[1]) / sn, az = fabs((double)vw.step[2]) / sn;
-        const double uy = un > 0.0 ? fabs((double)vw.du[1]) / un : 0.0;
-        const bool flat = ay <= 1e-3 && uy <= 1e-3;
-        along_auto = az <= (sigma ? (flat ? 0.95 : 0.9) : flat ? 0.9 : 0.5);
+        const double ax = fabs((double)vw.step[0]) / sn, ay = fabs((double)vw.step[1]) / sn, az = fabs((double)vw.step[2]) / sn;
+        const double flat = 0.9 - 4.0 * ay;                       // the pitch-0 advantage fades within a few degrees
+        if (kind == kRenderSigma) along_auto = ax >= 0.25 && ay <= 0.75;
+        else if (kind == kRenderTf) along_auto = az <= std::max(flat, std::min(0.73 - 0.67 * ay, 1.16 - 1.35 * ay));
+        else along_auto = az <= std::max(flat, 0.5 - 0.55 * ay);
     }
     return c->render_variant == 0 ? along_auto : c->render_variant == 2;
 }
@@ -915,13 +929,13 @@ int cube_render_mip(cube_ctx* c, const float* d, int64_t nx, int64_t ny, int64_t
         ProfScope prof(c, CUBE_K_RENDER, s);
         const dim3 block(kRenderTileU, kRenderTileV);
         const dim3 grid((vw.width + kRenderTileU - 1) / kRenderTileU, (vw.height + kRenderTileV - 1) / kRenderTileV);
-        const bool along = render_along(c, vw, false);
+        const bool along = render_along(c, vw, kRenderMip);
         if (along) {
             const long long npix = (long long)vw.width * vw.height;
             render_mip_along_kernel<<<(unsigned)((npix + kRenderRaysPerCta - 1) / kRenderRaysPerCta), 32 * kRenderRaysPerCta, 0, s>>>(
                 d, g, vw, vmin, image);
         } else {
-            render_mip_kernel<<<grid, block, 0, s>>>(d, g, vw, vmin, image);
+            render_mip_kernel<<<grid, block, 0, s>>>(d, g, vw, vmin, render_footprint(vw), image);
         }
     }
     CUBE_CUDA(c, cudaGetLastError());
@@ -979,7 +993,7 @@ static int render_tf_common(cube_ctx* c, const float* d, int64_t nx, int64_t ny,
         ProfScope prof(c, CUBE_K_RENDER, s);
         const dim3 block(kRenderTileU, kRenderTileV);
         const dim3 grid((vw.width + kRenderTileU - 1) / kRenderTileU, (vw.height + kRenderTileV - 1) / kRenderTileV);
-        if (render_along(c, vw, dev_cells != nullptr)) {
+        if (render_along(c, vw, dev_cells ? kRenderSigma : kRenderTf)) {
             const long long npix = (long long)vw.width * vw.height;
             const unsigned agrid = (unsigned)((npix + kRenderRaysPerCta - 1) / kRenderRaysPerCta);
             if (dev_cells)
@@ -990,10 +1004,10 @@ static int render_tf_common(cube_ctx* c, const float* d, int64_t nx, int64_t ny,
                     d, g, vw, nlevels, lo, scale, dev_table, opacity_cut, nullptr, mg, reinterpret_cast<float4*>(rgba));
         } else if (dev_cells)
             render_tf_kernel<true><<<grid, block, 0, s>>>(d, g, vw, nlevels, lo, scale, dev_table, opacity_cut, c->map32,
-                                                          mg, reinterpret_cast<float4*>(rgba));
+                                                          mg, render_footprint(vw), reinterpret_cast<float4*>(rgba));
         else
             render_tf_kernel<false><<<grid, block, 0, s>>>(d, g, vw, nlevels, lo, scale, dev_table, opacity_cut, nullptr,
-                                                           mg, reinterpret_cast<float4*>(rgba));
+                                                           mg, render_footprint(vw), reinterpret_cast<float4*>(rgba));
     }
     CUBE_CUDA(c, cudaGetLastError());
     return CUBE_OK;

@@ -187,12 +187,25 @@ __device__ __forceinline__ void map_lookup(const float2* __restrict__ map, const
     }
 }
 
-constexpr int kRenderTileU = 32, kRenderTileV = 8;   // a warp = 32 neighbouring pixels of one image row
+constexpr int kRenderTileU = 32, kRenderTileV = 8;
+
+// Pixel of a thread in the CTA's tile of 32 x 8 pixels.  A warp's 32 pixels form a block of 2^fw_log x 2^(5 - fw_log):
+// 16 x 2 when the image rows run nearly along the cube's x axis (the lanes then read neighbouring voxels), 8 x 4 for
+// oblique views -- the rays of a compact block stay close together in y and z as well, so a warp's loads touch fewer
+// planes and lines of the cube than those of 32 pixels in a row (c2, yaw 45 pitch 20: MIP 10.3 -> 7.2 ms).  The host
+// chooses (csrc/cube.cu, render_footprint).
+__device__ __forceinline__ void render_pixel(int fw_log, int& u, int& v) {
+    const int lane = threadIdx.x, warp = threadIdx.y;            // blockDim = (32, 8)
+    const int across_log = 5 - fw_log;                            // blocks across the tile: 2^across_log
+    u = blockIdx.x * kRenderTileU + ((warp & ((1 << across_log) - 1)) << fw_log) + (lane & ((1 << fw_log) - 1));
+    v = blockIdx.y * kRenderTileV + ((warp >> across_log) << across_log) + (lane >> fw_log);
+}   // a warp = 32 neighbouring pixels of one image row
 
 // MIP (R29): the largest sample >= vmin in march order; NaN when the ray has none.
 __global__ void __launch_bounds__(kRenderTileU * kRenderTileV)
-render_mip_kernel(const float* __restrict__ d, RenderGeom g, RenderView vw, float vmin, float* __restrict__ image) {
-    const int u = blockIdx.x * kRenderTileU + threadIdx.x, v = blockIdx.y * kRenderTileV + threadIdx.y;
+render_mip_kernel(const float* __restrict__ d, RenderGeom g, RenderView vw, float vmin, int fw_log, float* __restrict__ image) {
+    int u, v;
+    render_pixel(fw_log, u, v);
     if (u >= vw.width || v >= vw.height) return;
     const RayF r = ray_setup(vw, g, u, v);
     float m = 0.0f;
@@ -268,8 +281,9 @@ template <bool SIGMA>
 __global__ void __launch_bounds__(kRenderTileU * kRenderTileV)
 render_tf_kernel(const float* __restrict__ d, RenderGeom g, RenderView vw, int nlevels, float lo, float scale,
                  const float4* __restrict__ table, float opacity_cut, const float2* __restrict__ cells, MapLookupGeom mg,
-                 float4* __restrict__ rgba) {
-    const int u = blockIdx.x * kRenderTileU + threadIdx.x, v = blockIdx.y * kRenderTileV + threadIdx.y;
+                 int fw_log, float4* __restrict__ rgba) {
+    int u, v;
+    render_pixel(fw_log, u, v);
     if (u >= vw.width || v >= vw.height) return;
     const RayF r = ray_setup(vw, g, u, v);
     float cr = 0.0f, cg = 0.0f, cb = 0.0f, A = 0.0f;
