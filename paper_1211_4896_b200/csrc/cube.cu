@@ -899,24 +899,36 @@ static int render_footprint(const RenderView& vw) {
     return (un > 0.0 && fabs((double)vw.du[0]) / un >= 0.9) ? 4 : 3;        // image rows nearly along x: 16 x 2, else 8 x 4
 }
 
+// The block of rays of a CTA in the ray-per-warp kernels (cube_render.cuh, render_ray_of_warp): log2 of its width.
+static int render_ray_block(const RenderView& vw) {
+    if (const char* e = getenv("CUBE_RENDER_RW")) return atoi(e);           // experiments
+    // 8 x 1 when the rays lie in planes y = const (neighbours along the image row share their lines), else 4 x 2
+    // (c2, MIP: yaw 70 pitch 20: 4.7 -> 3.0 ms, yaw 90 pitch 40: 3.7 -> 3.0; at pitch 0 4 x 2 doubles the time)
+    const double sn = sqrt((double)vw.step[0] * vw.step[0] + (double)vw.step[1] * vw.step[1] + (double)vw.step[2] * vw.step[2]);
+    return (sn > 0.0 && fabs((double)vw.step[1]) / sn > 0.05) ? 2 : 3;
+}
+static unsigned render_ray_blocks(const RenderView& vw, int rw_log) {
+    const unsigned across = ((unsigned)vw.width + (1u << rw_log) - 1u) >> rw_log;
+    const unsigned down = ((unsigned)vw.height + (1u << (3 - rw_log)) - 1u) >> (3 - rw_log);
+    return across * down;
+}
+
 // Which ray-casting kernel (CUBE_KNOB_RENDER)?  One ray per warp (cube_render.cuh) pays for every PLANE of the cube that
 // the 32 consecutive samples of a ray cross (planes are megabytes apart) and for every line they climb in y, one ray per
 // thread for the planes and lines the block of pixels of a warp spans.  The rules below are fits to a map of both
 // kernels over yaw 0-90 x pitch 0-60 degrees on c2, 1024^2 rays, in terms of the components
 // (ax, ay, az) of the ray direction: ray-per-warp wins when az is small enough for the ay at hand -- up to 0.9 when
 // rays and image rows lie in planes y = const (an orbit at pitch 0: neighbouring rays share their lines) -- and, for
-// the sigma-clipping transfer function, whose map lookups do not care about the direction, whenever the ray is not
-// too steep in y and has some x component at all.
+// the sigma-clipping transfer function, whose map lookups do not care about the direction, whenever the ray has some
+// x component at all.
 enum { kRenderMip = 0, kRenderTf = 1, kRenderSigma = 2 };
 static bool render_along(const cube_ctx* c, const RenderView& vw, int kind) {
     const double sn = sqrt((double)vw.step[0] * vw.step[0] + (double)vw.step[1] * vw.step[1] + (double)vw.step[2] * vw.step[2]);
     bool along_auto = false;
     if (sn > 0.0) {
         const double ax = fabs((double)vw.step[0]) / sn, ay = fabs((double)vw.step[1]) / sn, az = fabs((double)vw.step[2]) / sn;
-        const double flat = 0.9 - 4.0 * ay;                       // the pitch-0 advantage fades within a few degrees
-        if (kind == kRenderSigma) along_auto = ax >= 0.25 && ay <= 0.75;
-        else if (kind == kRenderTf) along_auto = az <= std::max(flat, std::min(0.73 - 0.67 * ay, 1.16 - 1.35 * ay));
-        else along_auto = az <= std::max(flat, 0.5 - 0.55 * ay);
+        if (kind == kRenderSigma) along_auto = ax >= 0.25;
+        else along_auto = az <= std::max(0.9 - 4.0 * ay, 0.82 - 0.6 * ay);   // 0.9 at pitch 0, fading within a few degrees
     }
     return c->render_variant == 0 ? along_auto : c->render_variant == 2;
 }
@@ -931,9 +943,8 @@ int cube_render_mip(cube_ctx* c, const float* d, int64_t nx, int64_t ny, int64_t
         const dim3 grid((vw.width + kRenderTileU - 1) / kRenderTileU, (vw.height + kRenderTileV - 1) / kRenderTileV);
         const bool along = render_along(c, vw, kRenderMip);
         if (along) {
-            const long long npix = (long long)vw.width * vw.height;
-            render_mip_along_kernel<<<(unsigned)((npix + kRenderRaysPerCta - 1) / kRenderRaysPerCta), 32 * kRenderRaysPerCta, 0, s>>>(
-                d, g, vw, vmin, image);
+            const int rw = render_ray_block(vw);
+            render_mip_along_kernel<<<render_ray_blocks(vw, rw), 32 * kRenderRaysPerCta, 0, s>>>(d, g, vw, vmin, rw, image);
         } else {
             render_mip_kernel<<<grid, block, 0, s>>>(d, g, vw, vmin, render_footprint(vw), image);
         }
@@ -994,14 +1005,14 @@ static int render_tf_common(cube_ctx* c, const float* d, int64_t nx, int64_t ny,
         const dim3 block(kRenderTileU, kRenderTileV);
         const dim3 grid((vw.width + kRenderTileU - 1) / kRenderTileU, (vw.height + kRenderTileV - 1) / kRenderTileV);
         if (render_along(c, vw, dev_cells ? kRenderSigma : kRenderTf)) {
-            const long long npix = (long long)vw.width * vw.height;
-            const unsigned agrid = (unsigned)((npix + kRenderRaysPerCta - 1) / kRenderRaysPerCta);
+            const int rw = render_ray_block(vw);
+            const unsigned agrid = render_ray_blocks(vw, rw);
             if (dev_cells)
                 render_tf_along_kernel<true><<<agrid, 32 * kRenderRaysPerCta, 0, s>>>(
-                    d, g, vw, nlevels, lo, scale, dev_table, opacity_cut, c->map32, mg, reinterpret_cast<float4*>(rgba));
+                    d, g, vw, nlevels, lo, scale, dev_table, opacity_cut, c->map32, mg, rw, reinterpret_cast<float4*>(rgba));
             else
                 render_tf_along_kernel<false><<<agrid, 32 * kRenderRaysPerCta, 0, s>>>(
-                    d, g, vw, nlevels, lo, scale, dev_table, opacity_cut, nullptr, mg, reinterpret_cast<float4*>(rgba));
+                    d, g, vw, nlevels, lo, scale, dev_table, opacity_cut, nullptr, mg, rw, reinterpret_cast<float4*>(rgba));
         } else if (dev_cells)
             render_tf_kernel<true><<<grid, block, 0, s>>>(d, g, vw, nlevels, lo, scale, dev_table, opacity_cut, c->map32,
                                                           mg, render_footprint(vw), reinterpret_cast<float4*>(rgba));

@@ -236,12 +236,22 @@ render_mip_kernel(const float* __restrict__ d, RenderGeom g, RenderView vw, floa
 // the sample index and a tie goes to the smaller one -- the images stay bit-identical to render_mip_kernel's.
 constexpr int kRenderRaysPerCta = 8;
 
+// The ray of a warp: the CTA's kRenderRaysPerCta = 8 rays are a block of 2^rw_log x 2^(3 - rw_log) pixels (blockIdx.x
+// runs over the blocks row by row).
+__device__ __forceinline__ bool render_ray_of_warp(const RenderView& vw, int rw_log, int& u, int& v) {
+    const int warp = threadIdx.x >> 5;
+    const unsigned across = ((unsigned)vw.width + (1u << rw_log) - 1u) >> rw_log;     // blocks per row of blocks
+    u = (int)((blockIdx.x % across) << rw_log) + (warp & ((1 << rw_log) - 1));
+    v = (int)((blockIdx.x / across) << (3 - rw_log)) + (warp >> rw_log);
+    return u < vw.width && v < vw.height;
+}
+
 __global__ void __launch_bounds__(32 * kRenderRaysPerCta)
-render_mip_along_kernel(const float* __restrict__ d, RenderGeom g, RenderView vw, float vmin, float* __restrict__ image) {
+render_mip_along_kernel(const float* __restrict__ d, RenderGeom g, RenderView vw, float vmin, int rw_log, float* __restrict__ image) {
     const int lane = threadIdx.x & 31;
-    const long long pix = (long long)blockIdx.x * kRenderRaysPerCta + (threadIdx.x >> 5);
-    if (pix >= (long long)vw.width * vw.height) return;                  // warp-uniform
-    const int u = (int)(pix % vw.width), v = (int)(pix / vw.width);
+    int u, v;
+    if (!render_ray_of_warp(vw, rw_log, u, v)) return;                   // warp-uniform
+    const long long pix = (long long)v * vw.width + u;
     const RayF r = ray_setup(vw, g, u, v);
     float m = 0.0f;
     int mi = 0x7fffffff;
@@ -335,11 +345,11 @@ template <bool SIGMA>
 __global__ void __launch_bounds__(32 * kRenderRaysPerCta)
 render_tf_along_kernel(const float* __restrict__ d, RenderGeom g, RenderView vw, int nlevels, float lo, float scale,
                        const float4* __restrict__ table, float opacity_cut, const float2* __restrict__ cells,
-                       MapLookupGeom mg, float4* __restrict__ rgba) {
+                       MapLookupGeom mg, int rw_log, float4* __restrict__ rgba) {
     const int lane = threadIdx.x & 31;
-    const long long pix = (long long)blockIdx.x * kRenderRaysPerCta + (threadIdx.x >> 5);
-    if (pix >= (long long)vw.width * vw.height) return;                  // warp-uniform
-    const int u = (int)(pix % vw.width), v = (int)(pix / vw.width);
+    int u, v;
+    if (!render_ray_of_warp(vw, rw_log, u, v)) return;                   // warp-uniform
+    const long long pix = (long long)v * vw.width + u;
     const RayF r = ray_setup(vw, g, u, v);
     float cr = 0.0f, cg = 0.0f, cb = 0.0f, A = 0.0f;
     const float top = (float)(nlevels - 1);
