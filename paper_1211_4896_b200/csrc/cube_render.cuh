@@ -11,8 +11,11 @@
 //
 // The paper keeps the cube in 3-D texture memory; texture filtering interpolates with 9-bit fixed-point
 // weights, which no CPU restatement can match bit for bit, and a 64 GiB cube would have to be copied into a CUDA
-// array first.  Here the cube stays the caller's plain float32 array, read through the read-only L1 path (LDG.NC): the
-// 32 rays of a warp are neighbours in the image, so their eight-voxel neighbourhoods overlap and most loads hit L1/L2.
+// array first.  Here the cube stays the caller's plain float32 array, read through the read-only L1 path (LDG.NC).
+// Two families of kernels, chosen per view by the host (csrc/cube.cu, render_along): one ray per THREAD -- the 32 rays
+// of a warp are a compact block of the image, so their eight-voxel neighbourhoods overlap and most loads hit L1/L2 --
+// and one ray per WARP with the lanes on consecutive samples, for rays that run along the cube's x axis, where
+// neighbouring samples are neighbouring voxels of a line.  Both give the same images bit for bit.
 // Every floating-point operation is an explicitly rounded float32 operation (__fadd_rn / __fmul_rn / __fsub_rn, never
 // contracted), in the order DESIGN.md R27-R31 state, so the images equal the oracle's bit for bit.
 #pragma once
@@ -228,9 +231,9 @@ render_mip_kernel(const float* __restrict__ d, RenderGeom g, RenderView vw, floa
     image[(size_t)v * vw.width + u] = have ? m : __int_as_float(0x7fc00000);
 }
 
-// MIP for views whose rays run along the cube's x axis more than the image rows do (an orbit camera near yaw 90 /
-// 270 degrees): there the 32 rays of a warp read 32 different planes per load (32 sectors per request, none shared),
-// so a warp takes ONE ray instead and its lanes consecutive samples -- the eight loads of a warp then cover
+// MIP for views whose rays run along the cube's x axis (an orbit camera towards yaw 90 / 270 degrees): there the 32 rays
+// of a ray-per-thread warp read up to 32 different planes per load (32 sectors per request, none shared), so a warp
+// takes ONE ray instead and its lanes consecutive samples -- the eight loads of a warp then cover
 // neighbouring voxels of the same lines.  The maximum does not depend on the order of the samples, except between
 // equal maxima (-0.0 and +0.0 compare equal): the sequential march keeps the first, so lanes and the reduction carry
 // the sample index and a tie goes to the smaller one -- the images stay bit-identical to render_mip_kernel's.
