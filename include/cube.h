@@ -381,8 +381,8 @@ enum {
                                       for all bins (the choice is made on the device),
                                   1 = clusters of two CTAs holding 32-bit counters in distributed shared memory,
                                   2 = always the 16-bit packed counters */
-    CUBE_KNOB_SMALL = 3,       /* cube_stats with the median (histogram, if any, of at most 4096 bins) and cube_median on a
-                                  cube of at most 96 MiB: 0 = automatic (default): ONE cooperative launch
+    CUBE_KNOB_SMALL = 3,       /* cube_stats with the median (histogram, if any, of at most 4096 bins), cube_median and
+                                  cube_kth on a cube of at most 96 MiB: 0 = automatic (default): ONE cooperative launch
                                   (csrc/cube_small.cuh) when the device supports it, 1 = always the general three-launch
                                   path */
     CUBE_KNOB_MAPMEDIAN = 4,   /* cube_minimap_median on cells of at least 1024 voxels: 0 = automatic (default) = 2;

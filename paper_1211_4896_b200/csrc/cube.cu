@@ -494,10 +494,66 @@ int cube_histogram(cube_ctx* c, const float* d, int64_t nx, int64_t ny, int64_t 
     return CUBE_OK;
 }
 
+// cube_stats / cube_median / cube_kth on a cube that stays in L2 between its reads: ONE cooperative launch
+// (cube_small.cuh).  *launched = false: no CTA fits, the caller takes the general path.
+static bool small_path_ok(const cube_ctx* c, uint64_t n, int nbins) {
+    return nbins <= kSmallMaxBins && n * sizeof(float) <= ((size_t)96 << 20) && c->coop && !c->no_small;
+}
+
+static int small_launch(cube_ctx* c, const float* d, uint64_t n, int nbins, float lo, float hi, float scale, bool minmax,
+                        unsigned flags, cube_moments_t* moments, uint64_t* bins, uint64_t* outside, float* median,
+                        uint64_t k, int use_median, cudaStream_t s, bool* launched) {
+    const bool want_hist = nbins > 0;
+    float* med_direct = static_cast<float*>(device_reachable(c, median));
+    MomentsOut* mom_direct = static_cast<MomentsOut*>(device_reachable(c, moments));
+    *launched = false;
+    {
+        const size_t smem = (size_t)small_smem(nbins);
+        const int occ = occupancy_of(c, stats_small_kernel, kThreads, smem);
+        int per = c->ctas_per_sm > 0 ? c->ctas_per_sm : 2;
+        if (per > occ) per = occ;
+        if (per >= 1) {
+            const unsigned grid = (unsigned)(c->num_sms * per);
+            SmallArgs a;
+            a.d = d; a.n = n; a.nbins = nbins; a.lo = lo; a.hi = hi; a.scale = scale; a.minmax = minmax ? 1 : 0;
+            a.flags = flags & CUBE_SAMPLE_STD;
+            a.partials = c->partials; a.acc = c->acc; a.nvox_acc = c->nvox_acc; a.mom_out = c->mom_out; a.out_user = mom_direct;
+            a.coarse = c->coarse_next; a.coarse_keep = c->coarse; a.chunk_tot = c->chunk_tot;
+            a.gdigits = c->gdigits; a.gout = c->gout;
+            a.sel = c->sel; a.cand = c->cand; a.cand_cap = c->cand ? c->cand_cap : 0; a.result_out = med_direct;
+            a.k = k; a.use_median = use_median;
+            a.bar = c->bar; a.ext = c->small_ext; a.tstamp = c->small_tstamp;
+            a.bins_user = static_cast<unsigned long long*>(device_reachable(c, bins));
+            a.outside_user = static_cast<unsigned long long*>(device_reachable(c, outside));
+            if (!a.bins_user || !a.outside_user) a.bins_user = a.outside_user = nullptr;
+            void* args[] = {&a};
+            {
+                ProfScope prof(c, CUBE_K_STATS_SMALL, s);
+                CUBE_CUDA(c, cudaLaunchCooperativeKernel(reinterpret_cast<void*>(stats_small_kernel), dim3(grid), dim3(kThreads),
+                                                         args, smem, s));
+            }
+            if (!med_direct) CUBE_CUDA(c, cudaMemcpyAsync(median, &c->sel->result, sizeof(float), cudaMemcpyDefault, s));
+            if (moments && !mom_direct) CUBE_CUDA(c, cudaMemcpyAsync(moments, c->mom_out, sizeof(MomentsOut), cudaMemcpyDefault, s));
+            if (want_hist && !a.bins_user) {
+                CUBE_CUDA(c, cudaMemcpyAsync(bins, c->gbins, (size_t)nbins * sizeof(uint64_t), cudaMemcpyDefault, s));
+                CUBE_CUDA(c, cudaMemcpyAsync(outside, c->gout, 2 * sizeof(uint64_t), cudaMemcpyDefault, s));
+            }
+            *launched = true;
+            return CUBE_OK;
+        }
+    }
+    return CUBE_OK;
+}
+
 int cube_kth_ex(cube_ctx* c, const float* d, int64_t nx, int64_t ny, int64_t nz, uint64_t k, unsigned flags,
                 float* out, cudaStream_t s) {
     uint64_t n;
     if (!c || !d || !out || !dims_ok(nx, ny, nz, &n)) return CUBE_EINVAL;
+    if (flags == 0u && small_path_ok(c, n, 0)) {       // an L2-resident cube: one cooperative launch, as cube_median
+        bool launched = false;
+        const int rc = small_launch(c, d, n, 0, 0.f, 0.f, 0.f, false, 0u, nullptr, nullptr, nullptr, out, k, 0, s, &launched);
+        if (rc || launched) return rc;
+    }
     return kth_impl<false>(c, d, n, k, 0, flags, out, s);
 }
 
@@ -576,10 +632,13 @@ int cube_median_ex(cube_ctx* c, const float* d, int64_t nx, int64_t ny, int64_t 
                    cudaStream_t s) {
     uint64_t n;
     if (!c || !d || !out || !dims_ok(nx, ny, nz, &n)) return CUBE_EINVAL;
-    // A cube that stays in L2 between its reads: the single cooperative launch of cube_stats (cube_small.cuh) with a
-    // without the histogram -- one launch and two reads instead of three of each
-    if (flags == 0u && n * sizeof(float) <= ((size_t)96 << 20) && c->coop && !c->no_small)
-        return cube_stats(c, d, nx, ny, nz, 0, 0.f, 0.f, 0u, nullptr, nullptr, nullptr, out, s);
+    // A cube that stays in L2 between its reads: the single cooperative launch of cube_stats (cube_small.cuh) without
+    // the histogram -- one launch and two reads instead of three of each
+    if (flags == 0u && small_path_ok(c, n, 0)) {
+        bool launched = false;
+        const int rc = small_launch(c, d, n, 0, 0.f, 0.f, 0.f, false, 0u, nullptr, nullptr, nullptr, out, 0, 1, s, &launched);
+        if (rc || launched) return rc;
+    }
     return kth_impl<false>(c, d, n, 0, 1, flags, out, s);
 }
 
@@ -606,38 +665,10 @@ int cube_stats(cube_ctx* c, const float* d, int64_t nx, int64_t ny, int64_t nz, 
     MomentsOut* mom_direct = static_cast<MomentsOut*>(device_reachable(c, moments));
     // A cube that stays in L2 between its two reads: everything in ONE cooperative launch (cube_small.cuh)
     if (!want_hist) nbins = 0;
-    if (want_median && nbins <= kSmallMaxBins && n * sizeof(float) <= ((size_t)96 << 20) && c->coop && !c->no_small) {
-        const size_t smem = (size_t)small_smem(nbins);
-        const int occ = occupancy_of(c, stats_small_kernel, kThreads, smem);
-        int per = c->ctas_per_sm > 0 ? c->ctas_per_sm : 2;
-        if (per > occ) per = occ;
-        if (per >= 1) {
-            const unsigned grid = (unsigned)(c->num_sms * per);
-            SmallArgs a;
-            a.d = d; a.n = n; a.nbins = nbins; a.lo = lo; a.hi = hi; a.scale = scale; a.minmax = minmax ? 1 : 0;
-            a.flags = flags & CUBE_SAMPLE_STD;
-            a.partials = c->partials; a.acc = c->acc; a.nvox_acc = c->nvox_acc; a.mom_out = c->mom_out; a.out_user = mom_direct;
-            a.coarse = c->coarse_next; a.coarse_keep = c->coarse; a.chunk_tot = c->chunk_tot;
-            a.gdigits = c->gdigits; a.gout = c->gout;
-            a.sel = c->sel; a.cand = c->cand; a.cand_cap = c->cand ? c->cand_cap : 0; a.result_out = med_direct;
-            a.bar = c->bar; a.ext = c->small_ext; a.tstamp = c->small_tstamp;
-            a.bins_user = static_cast<unsigned long long*>(device_reachable(c, bins));
-            a.outside_user = static_cast<unsigned long long*>(device_reachable(c, outside));
-            if (!a.bins_user || !a.outside_user) a.bins_user = a.outside_user = nullptr;
-            void* args[] = {&a};
-            {
-                ProfScope prof(c, CUBE_K_STATS_SMALL, s);
-                CUBE_CUDA(c, cudaLaunchCooperativeKernel(reinterpret_cast<void*>(stats_small_kernel), dim3(grid), dim3(kThreads),
-                                                         args, smem, s));
-            }
-            if (!med_direct) CUBE_CUDA(c, cudaMemcpyAsync(median, &c->sel->result, sizeof(float), cudaMemcpyDefault, s));
-            if (moments && !mom_direct) CUBE_CUDA(c, cudaMemcpyAsync(moments, c->mom_out, sizeof(MomentsOut), cudaMemcpyDefault, s));
-            if (want_hist && !a.bins_user) {
-                CUBE_CUDA(c, cudaMemcpyAsync(bins, c->gbins, (size_t)nbins * sizeof(uint64_t), cudaMemcpyDefault, s));
-                CUBE_CUDA(c, cudaMemcpyAsync(outside, c->gout, 2 * sizeof(uint64_t), cudaMemcpyDefault, s));
-            }
-            return CUBE_OK;
-        }
+    if (want_median && small_path_ok(c, n, nbins)) {
+        bool launched = false;
+        rc = small_launch(c, d, n, nbins, lo, hi, scale, minmax, flags, moments, bins, outside, median, 0, 1, s, &launched);
+        if (rc || launched) return rc;
     }
     // pass A: moments (+ first select digit)
     const SelectInit init = select_init_args(c, 0, 1, true), cont = select_init_args(c, 0, 0, false, med_direct);

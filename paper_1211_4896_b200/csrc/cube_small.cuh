@@ -33,6 +33,7 @@ struct SmallArgs {
     unsigned long long* gdigits;     // kDigitBins: [0, 1024) second digit, [4096, 4608) last digit; left zeroed
     unsigned long long* gout;        // [outside (2)][bins (nbins)]
     SelectState* sel; uint32_t* cand; unsigned long long cand_cap; float* result_out;
+    unsigned long long k; int use_median;   // the rank asked for: the lower median of the non-NaN voxels, or k
     unsigned long long* bins_user;   // the caller's bins / outside when the device can reach them (no copy is enqueued then)
     unsigned long long* outside_user;
     unsigned int* bar;               // [0] the barrier counter (only grows), [1] its value when this launch starts: read
@@ -86,7 +87,8 @@ constexpr unsigned kSmallBarriers = 3;
 // chunk that holds the rank: two dependent L2 round trips of ONE warp instead of a scan of all 8192 bins.  Called by
 // warp 0 of every CTA; fills the CTA's own SelectState.
 __device__ __forceinline__ void small_locate0(SelectState* st, const unsigned long long* __restrict__ coarse,
-                                              const unsigned long long* __restrict__ chunk_tot, unsigned long long cand_cap) {
+                                              const unsigned long long* __restrict__ chunk_tot, unsigned long long cand_cap,
+                                              unsigned long long k_asked, int use_median) {
     constexpr int NCH = kDigitBins / 32, PER = NCH / 32;
     const int lane = threadIdx.x & 31;
     unsigned long long c[PER], mine = 0;
@@ -99,7 +101,8 @@ __device__ __forceinline__ void small_locate0(SelectState* st, const unsigned lo
         if (lane >= off) incl += u;
     }
     const unsigned long long total = __shfl_sync(0xffffffffu, incl, 31);
-    const unsigned long long k = total ? (total - 1) / 2 : 0;
+    const unsigned long long k = use_median ? (total ? (total - 1) / 2 : 0) : k_asked;
+    const bool invalid = k >= total;                  // also: no non-NaN voxel
     unsigned long long excl = incl - mine;
     int ch = -1;
     unsigned long long kin = 0;
@@ -110,7 +113,7 @@ __device__ __forceinline__ void small_locate0(SelectState* st, const unsigned lo
     }
     const unsigned ball = __ballot_sync(0xffffffffu, ch >= 0);
     if (lane == 0) {
-        st->count = total; st->invalid = total ? 0u : 1u; st->use_median = 1u; st->cand_n = 0; st->cand_cap = cand_cap;
+        st->count = total; st->invalid = invalid ? 1u : 0u; st->use_median = use_median ? 1u : 0u; st->cand_n = 0; st->cand_cap = cand_cap;
         st->cand_done = 0u; st->k = k; st->prefix = 0u; st->result = __int_as_float(0x7fc00000); st->bucket_n = 0ull;
     }
     if (!ball) return;
@@ -212,7 +215,7 @@ stats_small_kernel(SmallArgs a) {
     SMALL_T(3);
     // ---- every CTA for itself: the first-digit bucket (warp 0) and the extrema (warp 1)
     {
-        if (threadIdx.x < 32) small_locate0(&s_sel, a.coarse, a.chunk_tot, a.cand ? a.cand_cap : 0);
+        if (threadIdx.x < 32) small_locate0(&s_sel, a.coarse, a.chunk_tot, a.cand ? a.cand_cap : 0, a.k, a.use_median);
         if (threadIdx.x == 32) {
             s_mom.min = __uint_as_float(bits_of_key(__ldcg(&a.ext[0])));
             s_mom.max = __uint_as_float(bits_of_key(__ldcg(&a.ext[1])));
@@ -379,7 +382,7 @@ stats_small_kernel(SmallArgs a) {
         SelectState* g = a.sel;          // the state a later CUBE_REUSE_COARSE selection or a reader of the context finds
         g->k = s_sel.k; g->count = s_sel.count; g->prefix = s_sel.prefix; g->invalid = s_sel.invalid;
         SMALL_T(8);
-        g->use_median = 1u; g->result = s_sel.result; g->bucket_n = s_sel.bucket_n; g->cand_cap = a.cand ? a.cand_cap : 0; g->cand_done = fits ? 1u : 0u;
+        g->use_median = a.use_median ? 1u : 0u; g->result = s_sel.result; g->bucket_n = s_sel.bucket_n; g->cand_cap = a.cand ? a.cand_cap : 0; g->cand_done = fits ? 1u : 0u;
         a.bar[1] = bar_base + kSmallBarriers * grid;   // every CTA arrives kSmallBarriers times per launch
     }
 }

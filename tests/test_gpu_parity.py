@@ -970,6 +970,12 @@ def test_single_launch_path_for_l2_resident_cubes(scratch):
                 torch.cuda.synchronize()
                 assert same_float(d_f.cpu()[0].item(), omed)
             c.set_launch(0)
+            # cube_kth takes the same launch with the rank it is given: first, last, a middle one, one beyond the count
+            for kk in sorted({0, ref["count"] // 7, max(ref["count"] - 1, 0), ref["count"], ref["count"] + 5}):
+                want = oracle.kth(a, kk) if kk < ref["count"] else np.float32(np.nan)
+                l0 = c.launch_count
+                assert same_float(c.kth(t, a.size, 1, 1, kk), want)
+                assert c.launch_count - l0 == 1
             # and the state it leaves serves a later selection on the same cube
             if ref["count"]:
                 assert same_float(c.kth(t, a.size, 1, 1, ref["count"] // 5, flags=cube.REUSE_COARSE), oracle.kth(a, ref["count"] // 5))
