@@ -220,6 +220,11 @@ stats_small_kernel(SmallArgs a) {
             s_mom.min = __uint_as_float(bits_of_key(__ldcg(&a.ext[0])));
             s_mom.max = __uint_as_float(bits_of_key(__ldcg(&a.ext[1])));
         }
+        // meanwhile the other warps zero phase B's counters (phase A's are flushed: barrier A lies behind)
+        if (threadIdx.x >= 64) {
+            for (int i = threadIdx.x - 64; i < a.nbins + 2 + kBins1 + 1; i += kThreads - 64) dyn_bins[i] = 0;
+            if (threadIdx.x < 66) s_out[threadIdx.x - 64] = 0;
+        }
         __syncthreads();
         if (threadIdx.x == 0) s_mom.count = s_sel.count;     // all that hist_range() looks at: count, min, max
         __syncthreads();
@@ -231,9 +236,6 @@ stats_small_kernel(SmallArgs a) {
         uint32_t* hbins = dyn_bins;
         uint32_t* sbins = dyn_bins + (a.nbins + 2);
         uint32_t* stage = sbins + (kBins1 + 1);
-        for (int i = threadIdx.x; i < a.nbins + 2 + kBins1 + 1; i += kThreads) dyn_bins[i] = 0;
-        if (threadIdx.x < 2) s_out[threadIdx.x] = 0;
-        __syncthreads();
         float lo = a.lo, hi = a.hi, scale = a.scale;
         const bool range_ok = a.nbins == 0 || hist_range(a.minmax ? &s_mom : nullptr, a.nbins, lo, hi, scale);
         if (!range_ok) { lo = INFINITY; hi = -INFINITY; }   // nothing is in range: every counter stays 0
